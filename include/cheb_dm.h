@@ -1,0 +1,180 @@
+/*
+ * cheb_dm.h -- C ABI of the B200-native dense Chebyshev Fermi-operator solver.
+ *
+ * Hot path of arXiv 2306.12616 ("A fast, dense Chebyshev solver for electronic structure on
+ * GPUs"), cited below as PAPER.md:<line>:
+ *
+ *     D = f(H) = [I + exp(beta (H - mu I))]^{-1}                         (Eq. 3)
+ *       ~ sum_{n=0}^{M-1} c_n T_n(X),   X = (2H - (a+b) I)/(b - a)
+ *
+ * evaluated with the baby-step/giant-step factorisation of Eq. (4):
+ * T_2..T_k by T_{a+b} = 2 T_a T_b - T_|a-b| (Eq. 7, 22-23, Algorithm 1),
+ * then p-1 further products in T_k whose epilogues add the independent low-order sums of
+ * Eq. (21).  k*p >= M; M is the number of terms (the paper's L+1), p is the
+ * paper's `m`.
+ *
+ * Conventions
+ *  - Every call returns a cheb_dm_status_t (0 = OK); nothing throws or aborts; on error no
+ *    output argument is written.
+ *  - "device pointer" = CUDA global memory of the device that was current in cheb_dm_plan();
+ *    "host pointer" = ordinary host memory.  Matrices are dense row-major FP64 with leading
+ *    dimension N (row i starts at element i*N).  H must be symmetric (row-major == col-major).
+ *  - The plan owns its workspace (cudaMalloc'ed in cheb_dm_plan(), freed in cheb_dm_destroy());
+ *    the caller owns H, D and every output buffer.  D must not alias H.
+ *  - cheb_dm_compute / cheb_dm_trace / cheb_dm_moments / cheb_dm_product are asynchronous on the
+ *    given stream (a cudaStream_t passed as void*; NULL = legacy default stream), allocate nothing
+ *    and never synchronise with the host.  Calls that return scalars to HOST memory
+ *    (cheb_dm_get_bounds, cheb_dm_get_coeffs, cheb_dm_solve_mu, cheb_dm_get_T) synchronise the
+ *    stream they are given.
+ *  - A plan is not thread-safe; distinct plans are independent.  There is no CPU fallback: without
+ *    a CUDA device cheb_dm_plan() returns CHEB_DM_ECUDA.
+ */
+#ifndef CHEB_DM_H
+#define CHEB_DM_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct cheb_dm_plan_s* cheb_dm_plan_t; /* opaque, owned by the library */
+
+typedef enum { CHEB_DM_F64 = 0 } cheb_dm_dtype_t; /* the paper and all configs are FP64 */
+
+typedef enum {
+    CHEB_DM_OK = 0,
+    CHEB_DM_EINVAL = 1,       /* bad argument (N < 1, M < 1, NULL pointer, bad option)          */
+    CHEB_DM_EALLOC = 2,       /* workspace allocation failed                                     */
+    CHEB_DM_ECUDA = 3,        /* CUDA runtime/driver error, or no device                         */
+    CHEB_DM_ESTATE = 4,       /* call order: compute before coeffs, solve_mu before moments ...  */
+    CHEB_DM_EBOUNDS = 5,      /* b <= a or non-finite bounds                                     */
+    CHEB_DM_EUNSUPPORTED = 6, /* dtype other than CHEB_DM_F64                                    */
+    CHEB_DM_ENOCONV = 7       /* plan-time stability guard of the power-basis outer recursion    */
+} cheb_dm_status_t;
+
+/* Outer (giant-step) recursion.
+ *  CHEB_DM_OUTER_CHEBYSHEV (default): Clenshaw recursion in T_k,
+ *      B_l = G_l + 2 T_k B_{l+1} - B_{l+2},  D = G_0 + T_k B_1 - B_2,  G_l = sum_i g_{i,l} T_i,
+ *      with g_{i,l} = d_i^T a_l the intermediate of Eq. (16)-(17).  Same p-1
+ *      products and the same independent low-order sums as Eq. (4); stable in FP64.
+ *  CHEB_DM_OUTER_POWER: Eq. (4) literally, acc <- S_j + T_k acc with S_j = sum_i d_{i,j} T_i
+ *      (Eq. 21).  d grows like 2^p; reading A6.                  */
+typedef enum { CHEB_DM_OUTER_CHEBYSHEV = 0, CHEB_DM_OUTER_POWER = 1 } cheb_dm_outer_t;
+
+/* Scheduling of the products.
+ *  CHEB_DM_SCHED_GROUPED (default): one persistent kernel runs every product of the solve; the
+ *      independent baby-step products of a stage (Algorithm 1) run concurrently
+ *      and successive giant steps are pipelined at column-panel granularity.
+ *  CHEB_DM_SCHED_SERIAL: one launch per product on the stream (the paper's single-stream mode,
+ *      PAPER.md:190); used as the ablation baseline.                                            */
+typedef enum { CHEB_DM_SCHED_GROUPED = 0, CHEB_DM_SCHED_SERIAL = 1 } cheb_dm_sched_t;
+
+/* Operand pairing of the baby steps (any a+b=n is valid by Eq. 7).
+ *  CHEB_DM_PAIR_ALG1 (default): Algorithm 1's pairing, ceil(log2 k) stages.
+ *  CHEB_DM_PAIR_SERIAL: T_{n+1} = 2 T_1 T_n - T_{n-1} (k-1 serial products; best rounding).    */
+typedef enum { CHEB_DM_PAIR_ALG1 = 0, CHEB_DM_PAIR_SERIAL = 1 } cheb_dm_pairing_t;
+
+typedef struct {
+    int k;       /* baby-step block size; 0 = auto: ceil(sqrt(M))                 */
+    int p;       /* number of Horner blocks (paper's m); 0 = auto: ceil(M/k); need k*p >= M     */
+    int outer;   /* cheb_dm_outer_t                                                              */
+    int sched;   /* cheb_dm_sched_t                                                              */
+    int pairing; /* cheb_dm_pairing_t                                                            */
+    int tile;    /* CTA tile: 0 = auto, 1 = 128x128, 2 = 128x64, 3 = 64x64                         */
+    int fuse_sums; /* 1 (default when 0 passed via cheb_dm_plan): low-order sums G_l / S_j are
+                      formed inside the giant-step epilogues; 2: formed by separate (bandwidth-
+                      bound) passes before the giant steps -- ablation of PAPER.md:234           */
+    int reserved[9];
+} cheb_dm_options_t;
+
+/* Create a plan for N x N matrices and an M_terms-term expansion.  Chooses (k,p), allocates the
+ * workspace ((k+2) padded matrices + scalar tables) and builds the product/tile/dependency tables.
+ * plan: host pointer, receives the handle.  EINVAL: N<1, M_terms<1, k*p<M; EUNSUPPORTED: dtype. */
+cheb_dm_status_t cheb_dm_plan(cheb_dm_plan_t* plan, int N, int M_terms, cheb_dm_dtype_t dtype);
+/* Same with explicit options (host pointer; NULL = defaults). */
+cheb_dm_status_t cheb_dm_plan_ex(cheb_dm_plan_t* plan, int N, int M_terms, cheb_dm_dtype_t dtype,
+                                 const cheb_dm_options_t* opts);
+cheb_dm_status_t cheb_dm_destroy(cheb_dm_plan_t plan);
+
+/* Set the Fermi function and the spectral bounds used by the next cheb_dm_compute().
+ * beta: inverse temperature (>0, finite); mu: chemical potential (Eq. 2-3).
+ * bounds: host pointer to {a, b} = (eps_a, eps_b) of PAPER.md:96, or NULL => Gershgorin bounds
+ *   a = min_i(h_ii - R_i), b = max_i(h_ii + R_i), R_i = sum_{j!=i}|h_ij|, computed from H on the
+ *   device at compute time (a == b is widened to [a-1, b+1]).
+ * The Chebyshev coefficients c_n (n < M) of f~(x) = 1/(1+exp(beta~ (x - mu~))),
+ *   beta~ = beta (b-a)/2, mu~ = (2 mu - (a+b))/(b-a), are computed ON THE DEVICE inside
+ *   cheb_dm_compute() by the DCT at the N_q = 2^ceil(log2(4M)) Chebyshev nodes
+ *   x_j = cos(pi (j+1/2)/N_q):  c_n = ((2 - delta_n0)/N_q) sum_j f~(x_j) cos(n pi (j+1/2)/N_q)
+ *   (c_0 not halved: the expansion is sum c_n T_n), followed by the tables g (and d)
+ *   of Eq. (16)-(20).
+ * EINVAL: non-finite beta/mu or beta <= 0; EBOUNDS: explicit bounds with b <= a or non-finite. */
+cheb_dm_status_t cheb_dm_coeffs(cheb_dm_plan_t plan, double beta, double mu, const double* bounds);
+
+/* D <- sum_{n<M} c_n T_n(X) for the symmetric H (Eq. 3-4).  dH, dD: device pointers, N*N doubles,
+ * leading dimension N.  Runs, on `cuda_stream` and without host synchronisation: bounds (Gershgorin
+ * unless explicit) + rescale of H into X; coefficient tables; baby steps T_2..T_k; giant steps.
+ * ESTATE if cheb_dm_coeffs() was never called; EINVAL on NULL/aliased pointers. */
+cheb_dm_status_t cheb_dm_compute(cheb_dm_plan_t plan, const double* dH, double* dD, void* cuda_stream);
+
+/* trace_out[0] <- tr D = sum_i D_ii (electron count, north_star item 4).  dD: device pointer (N*N,
+ * ld N).  trace_out: DEVICE pointer (or pinned mapped host memory), 1 double, written
+ * asynchronously on the stream in a fixed summation order (bitwise reproducible). */
+cheb_dm_status_t cheb_dm_trace(cheb_dm_plan_t plan, const double* dD, double* trace_out, void* cuda_stream);
+
+/* Bounds {a,b} used by the last cheb_dm_compute()/cheb_dm_moments() (host pointer, 2 doubles).
+ * Synchronises `cuda_stream`.  EBOUNDS if the device flagged non-finite bounds. */
+cheb_dm_status_t cheb_dm_get_bounds(cheb_dm_plan_t plan, double* bounds_out, void* cuda_stream);
+
+/* Scalar tables of the last compute, copied to host memory (any pointer may be NULL):
+ *   c_out[k*p]  c_n (zero for n >= M);   g_out[k*p]  g_{i,l} at [i*p + l];
+ *   d_out[k*p]  d_{i,j} at [i*p + j] (only filled when outer == POWER, else zeros).
+ * Synchronises `cuda_stream`. */
+cheb_dm_status_t cheb_dm_get_coeffs(cheb_dm_plan_t plan, double* c_out, double* g_out, double* d_out,
+                                    void* cuda_stream);
+
+/* The block sizes chosen by the plan. */
+cheb_dm_status_t cheb_dm_get_kp(cheb_dm_plan_t plan, int* k_out, int* p_out);
+
+/* Copy the baby-step matrix T_n(X), 1 <= n <= k, of the last compute into dOut (device pointer,
+ * N*N, ld N).  Test/diagnostic access to the block of Eq. (22)-(23).  Synchronises the stream. */
+cheb_dm_status_t cheb_dm_get_T(cheb_dm_plan_t plan, int n, double* dOut, void* cuda_stream);
+
+/* Chebyshev moments tau_n = tr T_n(X), n < k*p, of H (north_star item 4; reading A10):
+ * bounds + rescale, baby steps, the giant block T_{jk} = T_j(T_k) (p-2 further products) and
+ * tau_{jk+i} = 2 <T_{jk}, T_i>_F - tau_{jk-i} (from Eq. 7 and symmetry), the Frobenius inner
+ * products being fused into the epilogues of the products that form T_{jk}.  Results stay on the
+ * device inside the plan for cheb_dm_solve_mu(); if tau_host != NULL (host pointer, k*p doubles)
+ * they are also copied out (this synchronises the stream).  Uses the bounds mode of the last
+ * cheb_dm_coeffs() call (explicit or Gershgorin); ESTATE if there was none. */
+cheb_dm_status_t cheb_dm_moments(cheb_dm_plan_t plan, const double* dH, double* tau_host, void* cuda_stream);
+
+/* Chemical potential for a target electron count: solves N_e(mu) = sum_n c_n(mu) tau_n = n_occ by
+ * bisection on [a,b] with exactly `iters` halvings (if N_e(mid) < n_occ then lo = mid else
+ * hi = mid; result (lo+hi)/2), all on the device; mu_out: host pointer.  Synchronises the stream.
+ * ESTATE unless cheb_dm_moments() ran on this plan. */
+cheb_dm_status_t cheb_dm_solve_mu(cheb_dm_plan_t plan, double beta, double n_occ, int iters,
+                                  double* mu_out, void* cuda_stream);
+
+/* One product of the recurrence as a stand-alone call (kernel-level tests and GEMM benchmark):
+ *   Out = alpha * A B + beta * C,   A, B, C, Out symmetric-operand N x N device matrices (ld N),
+ * computed by the same DMMA kernel as the solve (A is read through its transpose, which equals A
+ * for the symmetric operands of this method).  C may be NULL (beta ignored).  Out may alias C. */
+cheb_dm_status_t cheb_dm_product(cheb_dm_plan_t plan, double alpha, const double* dA, const double* dB,
+                                 double beta, const double* dC, double* dOut, void* cuda_stream);
+
+/* Bytes of device workspace owned by the plan. */
+cheb_dm_status_t cheb_dm_workspace_bytes(cheb_dm_plan_t plan, size_t* bytes_out);
+
+/* Number of kernel launches issued by the last cheb_dm_compute() (for bench.py's gpu_launches). */
+cheb_dm_status_t cheb_dm_last_launch_count(cheb_dm_plan_t plan, int* launches_out);
+
+/* Executed FP64 tensor flops of one cheb_dm_compute() on this plan: 2*N^3 per product. */
+cheb_dm_status_t cheb_dm_flops_per_compute(cheb_dm_plan_t plan, double* flops_out);
+
+const char* cheb_dm_strerror(cheb_dm_status_t status);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* CHEB_DM_H */

@@ -1,0 +1,179 @@
+"""ctypes binding of include/cheb_dm.h (same names, marshalling only)."""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+from . import build as _build
+
+OUTER_CHEBYSHEV, OUTER_POWER = 0, 1
+SCHED_GROUPED, SCHED_SERIAL = 0, 1
+PAIR_ALG1, PAIR_SERIAL = 0, 1
+TILE_AUTO, TILE_128x128, TILE_128x64, TILE_64x64 = 0, 1, 2, 3
+STATUS_NAMES = ["OK", "EINVAL", "EALLOC", "ECUDA", "ESTATE", "EBOUNDS", "EUNSUPPORTED", "ENOCONV"]
+
+EXPORTS = [
+    "cheb_dm_plan", "cheb_dm_plan_ex", "cheb_dm_destroy", "cheb_dm_coeffs", "cheb_dm_compute",
+    "cheb_dm_trace", "cheb_dm_get_bounds", "cheb_dm_get_coeffs", "cheb_dm_get_kp", "cheb_dm_get_T",
+    "cheb_dm_moments", "cheb_dm_solve_mu", "cheb_dm_product", "cheb_dm_workspace_bytes",
+    "cheb_dm_last_launch_count", "cheb_dm_flops_per_compute", "cheb_dm_strerror",
+]
+
+
+class Options(C.Structure):
+    _fields_ = [("k", C.c_int), ("p", C.c_int), ("outer", C.c_int), ("sched", C.c_int),
+                ("pairing", C.c_int), ("tile", C.c_int), ("fuse_sums", C.c_int),
+                ("reserved", C.c_int * 9)]
+
+
+class ChebDMError(RuntimeError):
+    def __init__(self, status: int, where: str):
+        self.status = status
+        name = STATUS_NAMES[status] if 0 <= status < len(STATUS_NAMES) else str(status)
+        msg = lib().cheb_dm_strerror(status).decode() if _LIB is not None else ""
+        super().__init__(f"{where}: CHEB_DM_{name} ({msg})")
+
+
+_LIB = None
+
+
+def lib_path() -> str:
+    return _build.LIB_PATH
+
+
+def lib():
+    """Load libcheb_dm.so (building it in-tree with nvcc if it is missing or stale)."""
+    global _LIB
+    if _LIB is not None:
+        return _LIB
+    path = _build.LIB_PATH
+    if _build.is_stale():
+        try:
+            _build.build()
+        except Exception as e:  # no nvcc: use what is there, or fail loudly
+            if not os.path.exists(path):
+                raise RuntimeError(f"libcheb_dm.so is missing and could not be built: {e}") from e
+    L = C.CDLL(path)
+    vp, dp, ip = C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_int)
+    L.cheb_dm_plan.argtypes = [C.POINTER(vp), C.c_int, C.c_int, C.c_int]
+    L.cheb_dm_plan_ex.argtypes = [C.POINTER(vp), C.c_int, C.c_int, C.c_int, C.POINTER(Options)]
+    L.cheb_dm_destroy.argtypes = [vp]
+    L.cheb_dm_coeffs.argtypes = [vp, C.c_double, C.c_double, dp]
+    L.cheb_dm_compute.argtypes = [vp, vp, vp, vp]
+    L.cheb_dm_trace.argtypes = [vp, vp, vp, vp]
+    L.cheb_dm_get_bounds.argtypes = [vp, dp, vp]
+    L.cheb_dm_get_coeffs.argtypes = [vp, dp, dp, dp, vp]
+    L.cheb_dm_get_kp.argtypes = [vp, ip, ip]
+    L.cheb_dm_get_T.argtypes = [vp, C.c_int, vp, vp]
+    L.cheb_dm_moments.argtypes = [vp, vp, dp, vp]
+    L.cheb_dm_solve_mu.argtypes = [vp, C.c_double, C.c_double, C.c_int, dp, vp]
+    L.cheb_dm_product.argtypes = [vp, C.c_double, vp, vp, C.c_double, vp, vp, vp]
+    L.cheb_dm_workspace_bytes.argtypes = [vp, C.POINTER(C.c_size_t)]
+    L.cheb_dm_last_launch_count.argtypes = [vp, ip]
+    L.cheb_dm_flops_per_compute.argtypes = [vp, dp]
+    for n in EXPORTS:
+        getattr(L, n).restype = C.c_int
+    L.cheb_dm_strerror.argtypes = [C.c_int]
+    L.cheb_dm_strerror.restype = C.c_char_p
+    _LIB = L
+    return L
+
+
+def _chk(status: int, where: str):
+    if status != 0:
+        raise ChebDMError(status, where)
+
+
+def _darr(a):
+    import numpy as np
+    a = np.ascontiguousarray(a, dtype=np.float64)
+    return a, a.ctypes.data_as(C.POINTER(C.c_double))
+
+
+class Plan:
+    """cheb_dm_plan_t with the same calls as the C ABI.  Pointers are raw device addresses (int)."""
+
+    def __init__(self, N: int, M: int, *, k: int = 0, p: int = 0, outer: int = OUTER_CHEBYSHEV,
+                 sched: int = SCHED_GROUPED, pairing: int = PAIR_ALG1, tile: int = TILE_AUTO,
+                 fuse_sums: int = 0, dtype: int = 0):
+        self._h = C.c_void_p()
+        self.N, self.M = N, M
+        o = Options(k=k, p=p, outer=outer, sched=sched, pairing=pairing, tile=tile, fuse_sums=fuse_sums)
+        _chk(lib().cheb_dm_plan_ex(C.byref(self._h), N, M, dtype, C.byref(o)), "cheb_dm_plan_ex")
+        kk, pp = C.c_int(), C.c_int()
+        _chk(lib().cheb_dm_get_kp(self._h, C.byref(kk), C.byref(pp)), "cheb_dm_get_kp")
+        self.k, self.p = kk.value, pp.value
+
+    def destroy(self):
+        if self._h:
+            lib().cheb_dm_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+    def coeffs(self, beta: float, mu: float, bounds=None):
+        if bounds is None:
+            _chk(lib().cheb_dm_coeffs(self._h, beta, mu, None), "cheb_dm_coeffs")
+        else:
+            arr = (C.c_double * 2)(float(bounds[0]), float(bounds[1]))
+            _chk(lib().cheb_dm_coeffs(self._h, beta, mu, arr), "cheb_dm_coeffs")
+
+    def compute(self, dH: int, dD: int, stream: int = 0):
+        _chk(lib().cheb_dm_compute(self._h, dH, dD, stream), "cheb_dm_compute")
+
+    def trace(self, dD: int, d_out: int, stream: int = 0):
+        _chk(lib().cheb_dm_trace(self._h, dD, d_out, stream), "cheb_dm_trace")
+
+    def get_bounds(self, stream: int = 0):
+        out = (C.c_double * 2)()
+        _chk(lib().cheb_dm_get_bounds(self._h, out, stream), "cheb_dm_get_bounds")
+        return float(out[0]), float(out[1])
+
+    def get_coeffs(self, stream: int = 0):
+        import numpy as np
+        n = self.k * self.p
+        c, g, d = np.zeros(n), np.zeros(n), np.zeros(n)
+        _chk(lib().cheb_dm_get_coeffs(self._h, c.ctypes.data_as(C.POINTER(C.c_double)),
+                                      g.ctypes.data_as(C.POINTER(C.c_double)),
+                                      d.ctypes.data_as(C.POINTER(C.c_double)), stream), "cheb_dm_get_coeffs")
+        return c, g.reshape(self.k, self.p), d.reshape(self.k, self.p)
+
+    def get_T(self, n: int, d_out: int, stream: int = 0):
+        _chk(lib().cheb_dm_get_T(self._h, n, d_out, stream), "cheb_dm_get_T")
+
+    def moments(self, dH: int, want_host: bool = True, stream: int = 0):
+        import numpy as np
+        if want_host:
+            tau = np.zeros(self.k * self.p)
+            _chk(lib().cheb_dm_moments(self._h, dH, tau.ctypes.data_as(C.POINTER(C.c_double)), stream),
+                 "cheb_dm_moments")
+            return tau
+        _chk(lib().cheb_dm_moments(self._h, dH, None, stream), "cheb_dm_moments")
+        return None
+
+    def solve_mu(self, beta: float, n_occ: float, iters: int = 100, stream: int = 0) -> float:
+        mu = C.c_double()
+        _chk(lib().cheb_dm_solve_mu(self._h, beta, n_occ, iters, C.byref(mu), stream), "cheb_dm_solve_mu")
+        return mu.value
+
+    def product(self, alpha: float, dA: int, dB: int, beta: float, dC, d_out: int, stream: int = 0):
+        _chk(lib().cheb_dm_product(self._h, alpha, dA, dB, beta, dC, d_out, stream), "cheb_dm_product")
+
+    def workspace_bytes(self) -> int:
+        v = C.c_size_t()
+        _chk(lib().cheb_dm_workspace_bytes(self._h, C.byref(v)), "cheb_dm_workspace_bytes")
+        return v.value
+
+    def last_launch_count(self) -> int:
+        v = C.c_int()
+        _chk(lib().cheb_dm_last_launch_count(self._h, C.byref(v)), "cheb_dm_last_launch_count")
+        return v.value
+
+    def flops_per_compute(self) -> float:
+        v = C.c_double()
+        _chk(lib().cheb_dm_flops_per_compute(self._h, C.byref(v)), "cheb_dm_flops_per_compute")
+        return v.value

@@ -1,0 +1,425 @@
+// aux_kernels.cuh -- the non-GEMM kernels of the hot path (sm_100a): Gershgorin bounds fused with the
+// affine rescale (north_star item 1), the device-side coefficient pipeline (c_n by DCT, then the g/d
+// tables of Eq. 16-20), trace / mu search (north_star item 4).  Product code; shares nothing with oracle/.
+#pragma once
+#include <cooperative_groups.h>
+#include "common.cuh"
+
+namespace chebdm {
+namespace cg = cooperative_groups;
+
+// ---------------------------------------------------------------------------------------------------
+// Device-resident scalar state of a plan.
+// ---------------------------------------------------------------------------------------------------
+struct DevScalars {
+    double a, b;                      // bounds in use (eps_a, eps_b)
+    unsigned long long enc_lo, enc_hi;  // order-preserving encodings for the atomic min / max
+    int bad_bounds;                   // set when the bounds are non-finite
+    int pad;
+    double mu;                        // result of the device-side bisection
+    double ne;                        // N_e at that mu
+};
+
+__device__ __forceinline__ unsigned long long enc_f64(double x) {
+    unsigned long long u = (unsigned long long)__double_as_longlong(x);
+    return (u & 0x8000000000000000ull) ? ~u : (u | 0x8000000000000000ull);
+}
+__device__ __forceinline__ double dec_f64(unsigned long long e) {
+    unsigned long long u = (e & 0x8000000000000000ull) ? (e & 0x7fffffffffffffffull) : ~e;
+    return __longlong_as_double((long long)u);
+}
+
+__global__ void init_scalars_kernel(DevScalars* sc, double a, double b, int explicit_bounds) {
+    sc->enc_lo = ~0ull;
+    sc->enc_hi = 0ull;
+    sc->bad_bounds = 0;
+    if (explicit_bounds) {
+        sc->a = a;
+        sc->b = b;
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------
+// a-1: Gershgorin bounds + rescale, one cooperative launch (scaling of PAPER.md:96 read
+// as X = (2H - (a+b) I)/(b-a), reading A1).
+//   phase 1: one warp per row: R_i = sum_{j != i} |h_ij|; block min of h_ii - R_i / max of h_ii + R_i;
+//            one atomicMin/atomicMax per block on order-preserving integer encodings (order-independent,
+//            hence bitwise reproducible).
+//   grid sync
+//   phase 2: X[i][j] = (2 h_ij - (a+b) delta_ij) * (1/(b-a)), written with the workspace's padded leading
+//            dimension (pad columns stay zero).  For N <= ~2500 the second read of H is an L2 hit.
+// HBM bytes: 8N^2 (read) + 8N^2 (re-read, L2 for small N) + 8N^2 (write).
+// ---------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(512) bounds_rescale_kernel(const double* __restrict__ H, int N, double* __restrict__ X,
+                                                             long long ldx, DevScalars* sc, int explicit_bounds) {
+    cg::grid_group grid = cg::this_grid();
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int warps_per_block = blockDim.x >> 5;
+    __shared__ double s_lo[32], s_hi[32];
+    // 16-byte vector path: even N and aligned base make every row start 16-byte aligned
+    const bool vec = ((N & 1) == 0) && ((reinterpret_cast<uintptr_t>(H) & 15) == 0);
+    if (!explicit_bounds) {
+        double lo = INFINITY, hi = -INFINITY;
+        for (int row = blockIdx.x * warps_per_block + warp; row < N; row += gridDim.x * warps_per_block) {
+            const double* hr = H + (long long)row * N;
+            double r = 0.0, hii = 0.0;
+            if (vec) {
+                for (int j = 2 * lane; j < N; j += 64) {
+                    const double2 v = *reinterpret_cast<const double2*>(hr + j);
+                    if (j == row) hii = v.x; else r += fabs(v.x);
+                    if (j + 1 == row) hii = v.y; else r += fabs(v.y);
+                }
+            } else {
+                for (int j = lane; j < N; j += 32) {
+                    const double v = hr[j];
+                    if (j == row) hii = v; else r += fabs(v);
+                }
+            }
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) {
+                r += __shfl_xor_sync(0xffffffffu, r, o);
+                hii += __shfl_xor_sync(0xffffffffu, hii, o);  // exactly one lane holds h_ii, the rest 0
+            }
+            lo = fmin(lo, hii - r);
+            hi = fmax(hi, hii + r);
+            if (!(isfinite(r) && isfinite(hii))) { lo = -INFINITY; hi = INFINITY; }
+        }
+        if (lane == 0) { s_lo[warp] = lo; s_hi[warp] = hi; }
+        __syncthreads();
+        if (warp == 0) {
+            lo = lane < warps_per_block ? s_lo[lane] : INFINITY;
+            hi = lane < warps_per_block ? s_hi[lane] : -INFINITY;
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) {
+                lo = fmin(lo, __shfl_xor_sync(0xffffffffu, lo, o));
+                hi = fmax(hi, __shfl_xor_sync(0xffffffffu, hi, o));
+            }
+            if (lane == 0) {
+                atomicMin(&sc->enc_lo, enc_f64(lo));
+                atomicMax(&sc->enc_hi, enc_f64(hi));
+            }
+        }
+        __threadfence();
+        grid.sync();
+        if (blockIdx.x == 0 && threadIdx.x == 0) {
+            double a = dec_f64(sc->enc_lo), b = dec_f64(sc->enc_hi);
+            if (!(isfinite(a) && isfinite(b))) sc->bad_bounds = 1;
+            if (a == b) { a -= 1.0; b += 1.0; }  // degenerate H = cI (reading A2-iv)
+            sc->a = a;
+            sc->b = b;
+        }
+    }
+    double a, b;
+    if (explicit_bounds) {
+        a = sc->a;
+        b = sc->b;
+    } else {
+        a = dec_f64(*reinterpret_cast<volatile unsigned long long*>(&sc->enc_lo));
+        b = dec_f64(*reinterpret_cast<volatile unsigned long long*>(&sc->enc_hi));
+        if (a == b) { a -= 1.0; b += 1.0; }
+    }
+    const double inv = 1.0 / (b - a), shift = a + b;
+    for (int row = blockIdx.x * warps_per_block + warp; row < N; row += gridDim.x * warps_per_block) {
+        const double* hr = H + (long long)row * N;
+        double* xr = X + (long long)row * ldx;
+        if (vec) {
+            for (int j = 2 * lane; j < N; j += 64) {
+                const double2 v = *reinterpret_cast<const double2*>(hr + j);
+                double h0 = 2.0 * v.x, h1 = 2.0 * v.y;
+                if (j == row) h0 -= shift;
+                if (j + 1 == row) h1 -= shift;
+                *reinterpret_cast<double2*>(xr + j) = make_double2(h0 * inv, h1 * inv);
+            }
+        } else {
+            for (int j = lane; j < N; j += 32) {
+                double h = 2.0 * hr[j];
+                if (j == row) h -= shift;
+                xr[j] = h * inv;
+            }
+        }
+    }
+}
+
+// Copy a user matrix (ld N) into a padded workspace matrix (ld ldx).
+__global__ void pad_copy_kernel(const double* __restrict__ src, int N, double* __restrict__ dst, long long ldx) {
+    const long long total = (long long)N * N;
+    for (long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x; e < total; e += (long long)gridDim.x * blockDim.x) {
+        const int i = (int)(e / N), j = (int)(e - (long long)i * N);
+        dst[(long long)i * ldx + j] = src[e];
+    }
+}
+__global__ void unpad_copy_kernel(const double* __restrict__ src, long long ldx, int N, double* __restrict__ dst) {
+    const long long total = (long long)N * N;
+    for (long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x; e < total; e += (long long)gridDim.x * blockDim.x) {
+        const int i = (int)(e / N), j = (int)(e - (long long)i * N);
+        dst[e] = src[(long long)i * ldx + j];
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------
+// Double-double helpers (error-free transformations) for the scalar reductions: the parity gate on D
+// needs sum_n |delta c_n| << 1e-10 with N_q up to 8192 quadrature terms per coefficient.
+// ---------------------------------------------------------------------------------------------------
+struct dd { double hi, lo; };
+__device__ __forceinline__ dd dd_add_prod(dd s, double x, double y) {  // s + x*y
+    const double p = x * y;
+    const double e = fma(x, y, -p);
+    const double t = s.hi + p;
+    const double bb = t - s.hi;
+    const double err = (s.hi - (t - bb)) + (p - bb);
+    dd r;
+    r.hi = t;
+    r.lo = s.lo + err + e;
+    return r;
+}
+__device__ __forceinline__ dd dd_add(dd x, dd y) {
+    const double t = x.hi + y.hi;
+    const double bb = t - x.hi;
+    const double err = (x.hi - (t - bb)) + (y.hi - bb);
+    dd r;
+    r.hi = t;
+    r.lo = x.lo + y.lo + err;
+    return r;
+}
+// Fixed-order block reduction of a dd (blockDim.x <= 1024, multiple of 32). Result valid in thread 0.
+__device__ __forceinline__ dd dd_block_reduce(dd v, dd* s_buf) {
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        dd other;
+        other.hi = __shfl_down_sync(0xffffffffu, v.hi, o);
+        other.lo = __shfl_down_sync(0xffffffffu, v.lo, o);
+        v = dd_add(v, other);
+    }
+    if (lane == 0) s_buf[warp] = v;
+    __syncthreads();
+    if (warp == 0) {
+        const int nw = blockDim.x >> 5;
+        v.hi = lane < nw ? s_buf[lane].hi : 0.0;
+        v.lo = lane < nw ? s_buf[lane].lo : 0.0;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            dd other;
+            other.hi = __shfl_down_sync(0xffffffffu, v.hi, o);
+            other.lo = __shfl_down_sync(0xffffffffu, v.lo, o);
+            v = dd_add(v, other);
+        }
+    }
+    __syncthreads();
+    return v;
+}
+
+// Fermi function of the scaled variable, overflow-safe (Eq. 2).
+__device__ __forceinline__ double fermi_scaled(double beta_t, double mu_t, double x) {
+    const double y = beta_t * (x - mu_t);
+    if (y > 0.0) {
+        const double e = exp(-y);
+        return e / (1.0 + e);
+    }
+    return 1.0 / (1.0 + exp(y));
+}
+
+// ---------------------------------------------------------------------------------------------------
+// a-2: c_n by the DCT at the N_q Chebyshev nodes (cheb_dm.h, cheb_dm_coeffs).  costab[r] = cos(pi r/(2 N_q)),
+// r < 4 N_q, is built once on the host at plan time (correctly rounded), so the angle n*theta_j is reduced
+// exactly: n theta_j = pi ((n (2j+1)) mod 4N_q) / (2 N_q).
+//   fermi_nodes_kernel: fn[j] = f~(x_j), x_j = costab[2j+1]
+//   dct_kernel: block n -> c[n] (zero for n >= M), double-double accumulation, fixed order.
+// ---------------------------------------------------------------------------------------------------
+__global__ void fermi_nodes_kernel(const DevScalars* sc, double beta, double mu, const double* __restrict__ costab, int Nq,
+                                   double* __restrict__ fn) {
+    const int j = blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= Nq) return;
+    const double a = sc->a, b = sc->b;
+    const double beta_t = beta * (b - a) * 0.5;
+    const double mu_t = (2.0 * mu - (a + b)) / (b - a);
+    fn[j] = fermi_scaled(beta_t, mu_t, costab[2 * j + 1]);
+}
+
+__global__ void __launch_bounds__(256) dct_kernel(const double* __restrict__ fn, const double* __restrict__ costab, int Nq, int M,
+                                                  double* __restrict__ c) {
+    __shared__ dd s_buf[32];
+    const int n = blockIdx.x;
+    if (n >= M) {
+        if (threadIdx.x == 0) c[n] = 0.0;
+        return;
+    }
+    const unsigned mask = 4u * (unsigned)Nq - 1u;
+    dd s;
+    s.hi = 0.0;
+    s.lo = 0.0;
+    for (int j = threadIdx.x; j < Nq; j += blockDim.x) {
+        const unsigned r = ((unsigned)n * (2u * (unsigned)j + 1u)) & mask;
+        s = dd_add_prod(s, fn[j], costab[r]);
+    }
+    s = dd_block_reduce(s, s_buf);
+    if (threadIdx.x == 0) c[n] = ((n == 0) ? 1.0 : 2.0) * (s.hi + s.lo) / (double)Nq;
+}
+
+// ---------------------------------------------------------------------------------------------------
+// a-3: tables of Eq. (16)-(20), without forming the kp x kp matrix:
+//   g_{0,l} = c_{lk};  g_{i,p-1} = 2 c_{(p-1)k+i};  g_{i,l} = 2 c_{lk+i} - g_{k-i,l+1} (1 <= l <= p-2);
+//   g_{i,0} = c_i - g_{k-i,1}/2  (p >= 2), g_{i,0} = c_i (p == 1)                       (Eq. 16-17)
+//   d_i: back substitution of sum_{j>=l} a_{j,l} d_{i,j} = g_{i,l} (Eq. 24) with the
+//   matrix A of Eq. (10)-(11) (built on the host at plan time).
+// Output layout: gT[l*k + i] (row l is the coefficient vector of giant step l), dT likewise.
+// One block; thread i owns row i.
+// ---------------------------------------------------------------------------------------------------
+__global__ void tables_kernel(const double* __restrict__ c, int k, int p, const double* __restrict__ Amat, int want_d,
+                              double* __restrict__ gT, double* __restrict__ dT) {
+    for (int l = threadIdx.x; l < p; l += blockDim.x) gT[(size_t)l * k] = c[(size_t)l * k];
+    __syncthreads();
+    for (int l = p - 1; l >= 0; --l) {
+        for (int i = 1 + threadIdx.x; i < k; i += blockDim.x) {
+            double v;
+            if (p == 1) v = c[i];
+            else if (l == p - 1) v = 2.0 * c[(size_t)l * k + i];
+            else if (l >= 1) v = 2.0 * c[(size_t)l * k + i] - gT[(size_t)(l + 1) * k + (k - i)];
+            else v = c[i] - 0.5 * gT[(size_t)1 * k + (k - i)];
+            gT[(size_t)l * k + i] = v;
+        }
+        __syncthreads();
+    }
+    if (want_d) {
+        for (int i = threadIdx.x; i < k; i += blockDim.x) {
+            for (int l = p - 1; l >= 0; --l) {
+                double s = gT[(size_t)l * k + i];
+                for (int j = l + 1; j < p; ++j) s -= Amat[(size_t)j * p + l] * dT[(size_t)j * k + i];
+                dT[(size_t)l * k + i] = s / Amat[(size_t)l * p + l];
+            }
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------
+// a-7: trace.  One block, fixed summation order (bitwise reproducible).  8N useful bytes.
+// ---------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(1024) trace_kernel(const double* __restrict__ D, int N, long long ld, double* __restrict__ out) {
+    __shared__ dd s_buf[32];
+    dd s;
+    s.hi = 0.0;
+    s.lo = 0.0;
+    for (int i = threadIdx.x; i < N; i += blockDim.x) s = dd_add_prod(s, D[(long long)i * ld + i], 1.0);
+    s = dd_block_reduce(s, s_buf);
+    if (threadIdx.x == 0) out[0] = s.hi + s.lo;
+}
+
+// ---------------------------------------------------------------------------------------------------
+// a-7: moments tau_n = tr T_n(X) (reading A10).
+//   frob_partial_kernel: block (i, chunk): partial <U, T_{i+1}> over a slice of rows, i < count;
+//                        i == count: partial tr U; i == count + 1 + n: partial tr T_{n+1}, n < ntrace.
+//   moments_kernel (one block): tau_0 = N; tau_i = tr T_i (i <= k); for j >= 1:
+//       tau_{jk} = tr U_j,  tau_{jk+i} = 2 <U_j, T_i> - tau_{jk-i}  (Eq. 7 + symmetry), U_j = T_j(T_k).
+//   Partials are summed in a fixed order (bitwise reproducible).
+// ---------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) frob_partial_kernel(const double* __restrict__ U, const double* __restrict__ Tbase,
+                                                           long long stride, long long ld, int N, int count, int ntrace,
+                                                           double* __restrict__ part) {
+    __shared__ dd s_buf[32];
+    const int i = blockIdx.x, chunk = blockIdx.y, nchunks = gridDim.y;
+    const int r0 = (int)((long long)N * chunk / nchunks), r1 = (int)((long long)N * (chunk + 1) / nchunks);
+    dd s;
+    s.hi = 0.0;
+    s.lo = 0.0;
+    if (i < count) {
+        const double* Ti = Tbase + (long long)i * stride;
+        for (int r = r0; r < r1; ++r)
+            for (int c = threadIdx.x; c < N; c += blockDim.x) s = dd_add_prod(s, U[(long long)r * ld + c], Ti[(long long)r * ld + c]);
+    } else {
+        const double* Mx = (i == count) ? U : Tbase + (long long)(i - count - 1) * stride;
+        for (int r = r0 + threadIdx.x; r < r1; r += blockDim.x) s = dd_add_prod(s, Mx[(long long)r * ld + r], 1.0);
+    }
+    s = dd_block_reduce(s, s_buf);
+    if (threadIdx.x == 0) part[(size_t)i * nchunks + chunk] = s.hi + s.lo;
+}
+
+// part1: [k-1 dots | tr U_1 | tr T_1..T_k] x nchunks from frob_partial_kernel (U = T_k);
+// dots: [j][tile][k] from the fused epilogues of the chain U_j, j = 2..p-1 (slot k-1 = trace).
+__global__ void moments_kernel(const double* __restrict__ part1, int nchunks, const double* __restrict__ dots, int tiles, int k, int p,
+                               int N, double* __restrict__ tau) {
+    const int kp = k * p;
+    if (threadIdx.x == 0) tau[0] = (double)N;
+    for (int n = 1 + threadIdx.x; n <= k && n < kp; n += blockDim.x) {
+        double s = 0.0;
+        for (int ch = 0; ch < nchunks; ++ch) s += part1[(size_t)(k + n - 1) * nchunks + ch];
+        tau[n] = s;
+    }
+    __syncthreads();
+    for (int j = 1; j < p; ++j) {
+        for (int i = 1 + threadIdx.x; i < k; i += blockDim.x) {
+            double s = 0.0;
+            if (j == 1) {
+                for (int ch = 0; ch < nchunks; ++ch) s += part1[(size_t)(i - 1) * nchunks + ch];
+            } else {
+                for (int t = 0; t < tiles; ++t) s += dots[((size_t)j * tiles + t) * k + (i - 1)];
+            }
+            tau[j * k + i] = 2.0 * s - tau[j * k - i];
+        }
+        if (threadIdx.x == 0 && j >= 2) {
+            double s = 0.0;
+            for (int t = 0; t < tiles; ++t) s += dots[((size_t)j * tiles + t) * k + (k - 1)];
+            tau[j * k] = s;
+        }
+        __syncthreads();
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------
+// a-7: mu search.  N_e(mu) = sum_n c_n(mu) tau_n = sum_j f~(x_j; mu) w_j with the mu-independent weights
+//   w_j = (1/N_q) sum_{n<M} (2 - delta_n0) tau_n cos(n theta_j)
+// (the DCT of cheb_dm_coeffs with the two sums exchanged), so one bisection step costs N_q Fermi values.
+//   mu_weights_kernel: block j -> w[j]
+//   mu_bisect_kernel : one block, `iters` halvings of [a,b]: N_e(mid) < n_occ ? lo = mid : hi = mid.
+// ---------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(128) mu_weights_kernel(const double* __restrict__ tau, const double* __restrict__ costab, int Nq, int M,
+                                                         double* __restrict__ w) {
+    __shared__ dd s_buf[32];
+    const int j = blockIdx.x;
+    const unsigned mask = 4u * (unsigned)Nq - 1u;
+    dd s;
+    s.hi = 0.0;
+    s.lo = 0.0;
+    for (int n = threadIdx.x; n < M; n += blockDim.x) {
+        const unsigned r = ((unsigned)n * (2u * (unsigned)j + 1u)) & mask;
+        s = dd_add_prod(s, (n == 0 ? 1.0 : 2.0) * tau[n], costab[r]);
+    }
+    s = dd_block_reduce(s, s_buf);
+    if (threadIdx.x == 0) w[j] = (s.hi + s.lo) / (double)Nq;
+}
+
+__global__ void __launch_bounds__(1024) mu_bisect_kernel(DevScalars* sc, double beta, double n_occ, int iters,
+                                                         const double* __restrict__ costab, int Nq, const double* __restrict__ w) {
+    __shared__ dd s_buf[32];
+    __shared__ double s_lo, s_hi, s_ne;
+    const double a = sc->a, b = sc->b;
+    const double beta_t = beta * (b - a) * 0.5;
+    if (threadIdx.x == 0) { s_lo = a; s_hi = b; s_ne = 0.0; }
+    __syncthreads();
+    for (int it = 0; it <= iters; ++it) {
+        const double lo = s_lo, hi = s_hi;
+        const double mid = 0.5 * (lo + hi);
+        const double mu_t = (2.0 * mid - (a + b)) / (b - a);
+        dd s;
+        s.hi = 0.0;
+        s.lo = 0.0;
+        for (int j = threadIdx.x; j < Nq; j += blockDim.x) s = dd_add_prod(s, fermi_scaled(beta_t, mu_t, costab[2 * j + 1]), w[j]);
+        s = dd_block_reduce(s, s_buf);
+        if (threadIdx.x == 0) {
+            const double ne = s.hi + s.lo;
+            if (it == iters) {
+                s_ne = ne;  // N_e at the returned mu = (lo+hi)/2
+            } else if (ne < n_occ) {
+                s_lo = mid;
+            } else {
+                s_hi = mid;
+            }
+        }
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) {
+        sc->mu = 0.5 * (s_lo + s_hi);
+        sc->ne = s_ne;
+    }
+}
+
+}  // namespace chebdm

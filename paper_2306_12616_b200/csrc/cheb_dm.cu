@@ -1,0 +1,853 @@
+// cheb_dm.cu -- host side of the C ABI declared in include/cheb_dm.h: plan (block sizes, workspace,
+// TMA descriptors, task/dependency tables) and the launches of the sm_100a kernels.  Product code;
+// shares nothing with oracle/.  There is no CPU path: every step of the solve runs in the kernels of
+// gemm_dmma.cuh / aux_kernels.cuh.
+#include <cuda.h>
+#include <cuda_runtime.h>
+#include <math.h>
+#include <stdio.h>
+#include <stdlib.h>
+#include <string.h>
+
+#include <new>
+#include <vector>
+
+#include "../../include/cheb_dm.h"
+#include "aux_kernels.cuh"
+#include "common.cuh"
+#include "gemm_dmma.cuh"
+
+using namespace chebdm;
+
+namespace {
+
+typedef GemmCfg<128, 128, 4, 1> Cfg128x128;  // 16 consumer warps, 128 KB ring, 1 CTA/SM
+typedef GemmCfg<128, 64, 4, 2> Cfg128x64;    //  8 consumer warps,  96 KB ring, 2 CTA/SM
+typedef GemmCfg<64, 64, 6, 3> Cfg64x64;      //  4 consumer warps,  96 KB ring (6 stages), up to 3 CTA/SM
+
+enum TileSel { TILE_AUTO = 0, TILE_128x128 = 1, TILE_128x64 = 2, TILE_64x64 = 3 };
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+EncodeTiledFn get_encode_fn() {
+    static EncodeTiledFn fn = nullptr;
+    if (fn) return fn;
+    void* p = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &qres) != cudaSuccess) return nullptr;
+    if (qres != cudaDriverEntryPointSuccess) return nullptr;
+    fn = reinterpret_cast<EncodeTiledFn>(p);
+    return fn;
+}
+
+struct HostTaskMeta {
+    int has_gemm;
+};
+
+}  // namespace
+
+struct cheb_dm_plan_s {
+    int N, M, k, p, Nq;
+    cheb_dm_options_t opt;
+    int device, num_sms;
+    int tile;  // TileSel actually used
+    int BM, BN;
+    long long ld;        // padded leading dimension of workspace matrices (multiple of 16)
+    size_t mat_elems;    // elements per workspace matrix
+    int nmat;            // k + 2 (+ p when the sums are pre-formed)
+    double* ws;          // nmat matrices
+    // scalar tables (device)
+    double *costab, *fn, *c, *gT, *dT, *Amat, *tau, *w, *dots;
+    DevScalars* sc;
+    CUtensorMap* maps;   // nmat descriptors
+    int tma2d;
+    // task tables
+    int ntasks_solve;        // tasks [0, ntasks_solve) = the solve; [ntasks_solve, ntasks_all) = moments chain
+    int ntasks_all;
+    int nbaby;               // baby tasks are [0, nbaby)
+    int product_task;        // index of the scratch task used by cheb_dm_product
+    Task* tasks;             // device
+    int* task_first;         // device, ntasks_all + 2
+    std::vector<Task> h_tasks;
+    std::vector<int> h_first;
+    int* counters;           // device: [work counters | task_done | group_done | panel_done | error]
+    size_t counters_ints;
+    int off_work, off_task, off_group, off_panel, off_error;
+    int panel_stride;
+    int nwork;               // number of work counters (one per possible launch)
+    // state
+    int have_coeffs, explicit_bounds, have_moments, computed;
+    double beta, mu, a, b;
+    int last_launches;
+    double flops_per_compute;
+    size_t ws_bytes;
+};
+
+namespace {
+
+#define CUDA_TRY(expr)                                \
+    do {                                              \
+        cudaError_t e__ = (expr);                     \
+        if (e__ != cudaSuccess) return CHEB_DM_ECUDA; \
+    } while (0)
+
+double* T_ptr(const cheb_dm_plan_s* P, int n) {  // T_n, 1 <= n <= k
+    return P->ws + (size_t)(n - 1) * P->mat_elems;
+}
+int T_map(int n) { return n - 1; }
+double* buf_ptr(const cheb_dm_plan_s* P, int i) { return P->ws + (size_t)(P->k + i) * P->mat_elems; }
+int buf_map(const cheb_dm_plan_s* P, int i) { return P->k + i; }
+
+// Algorithm 1, reading A7 for s = 1.  Each entry: T_n = 2 T_l T_r - T_m.
+struct BabyProd {
+    int n, l, r, m, stage;
+};
+std::vector<BabyProd> baby_schedule(int k, int pairing) {
+    std::vector<BabyProd> v;
+    if (k < 2) return v;
+    if (pairing == CHEB_DM_PAIR_SERIAL) {
+        for (int n = 2; n <= k; ++n) v.push_back({n, 1, n - 1, n - 2, n - 1});
+        return v;
+    }
+    int nstages = 0;
+    while ((1 << nstages) < k) ++nstages;
+    for (int s = 1; s <= nstages; ++s) {
+        if (s == 1) {
+            v.push_back({2, 1, 1, 0, 1});
+            continue;
+        }
+        const int u = 1 << (s - 2), w = 1 << (s - 1);
+        for (int i = u + 1; i <= w; ++i)
+            if (i + u <= k) v.push_back({i + u, i, u, i - u, s});
+        for (int i = u + 1; i <= w; ++i)
+            if (i + w <= k) v.push_back({i + w, w, i, w - i, s});
+    }
+    return v;
+}
+
+// cos(pi r / (2 Nq)), r < 4 Nq, from first-octant long-double evaluations (angle reduced exactly).
+void build_costab(int Nq, std::vector<double>& tab) {
+    tab.resize((size_t)4 * Nq);
+    const long double h = 3.14159265358979323846264338327950288L / (2.0L * Nq);
+    for (int r = 0; r < 4 * Nq; ++r) {
+        int q = r;
+        long double sign = 1.0L;
+        if (q > 2 * Nq) q = 4 * Nq - q;           // cos(2pi - t) = cos t
+        if (q > Nq) { q = 2 * Nq - q; sign = -1.0L; }  // cos(pi - t) = -cos t
+        // q in [0, Nq]: angle in [0, pi/2]
+        long double v = (2 * q <= Nq) ? cosl(h * q) : sinl(h * (Nq - q));
+        if (q == Nq) v = 0.0L;
+        tab[r] = (double)(sign * v);
+    }
+}
+
+// Matrix A of Eq. (10)-(11): T_k^j = sum_l a_{j,l} T_{lk}.  Row-major p x p.
+void build_Amat(int p, std::vector<double>& A) {
+    A.assign((size_t)p * p, 0.0);
+    auto at = [&](int j, int l) -> double& { return A[(size_t)j * p + l]; };
+    at(0, 0) = 1.0;
+    if (p > 1) at(1, 1) = 1.0;
+    for (int j = 2; j < p; ++j) {
+        auto prev = [&](int l) { return (l >= 0 && l <= j - 1) ? at(j - 1, l) : 0.0; };
+        at(j, 0) = 0.5 * prev(1);
+        at(j, 1) = prev(0) + 0.5 * prev(2);
+        for (int l = 2; l <= j; ++l) at(j, l) = 0.5 * (prev(l - 1) + prev(l + 1));
+    }
+}
+
+}  // namespace
+
+namespace {
+
+int ceil_div(int a, int b) { return (a + b - 1) / b; }
+
+void choose_tile(cheb_dm_plan_s* P) {
+    int sel = P->opt.tile;
+    if (sel < TILE_AUTO || sel > TILE_64x64) sel = TILE_AUTO;
+    if (sel == TILE_AUTO) {
+        // Enough 128x128 tiles to give every SM one: large tile (least L2 traffic per flop).  Otherwise the
+        // small tile, so that the serial giant steps of small N still spread over the SMs.
+        const int t128 = ceil_div(P->N, 128) * ceil_div(P->N, 128);
+        const int t12864 = ceil_div(P->N, 128) * ceil_div(P->N, 64);
+        if (t128 >= P->num_sms) sel = TILE_128x128;
+        else if (t12864 >= 2 * P->num_sms) sel = TILE_128x64;
+        else sel = TILE_64x64;
+    }
+    P->tile = sel;
+    P->BM = (sel == TILE_64x64) ? 64 : 128;
+    P->BN = (sel == TILE_128x128) ? 128 : 64;
+}
+
+Task blank_task(const cheb_dm_plan_s* P) {
+    Task t;
+    memset(&t, 0, sizeof(t));
+    t.mapA = t.mapB = 0;
+    t.ktiles = ceil_div(P->N, BK);
+    t.tiles_m = ceil_div(P->N, P->BM);
+    t.tiles_n = ceil_div(P->N, P->BN);
+    t.alpha = 1.0;
+    t.lds = P->ld;
+    t.sum_stride = (long long)P->mat_elems;
+    return t;
+}
+
+void add_dep(Task& t, int kind, int idx, int target) {
+    if (t.ndeps >= MAX_DEPS) return;  // callers never exceed MAX_DEPS
+    t.dep_kind[t.ndeps] = kind;
+    t.dep_idx[t.ndeps] = idx;
+    t.dep_target[t.ndeps] = target;
+    ++t.ndeps;
+}
+
+// Groups: 0 = baby steps of the solve, 1 = giant steps, 2 = moments chain, 3 = cheb_dm_product scratch.
+enum { GROUP_BABY = 0, GROUP_GIANT = 1, GROUP_MOM = 2, GROUP_MISC = 3, NGROUPS = 4 };
+
+void build_tasks(cheb_dm_plan_s* P) {
+    const int k = P->k, p = P->p;
+    std::vector<Task>& T = P->h_tasks;
+    T.clear();
+    const int tiles = ceil_div(P->N, P->BM) * ceil_div(P->N, P->BN);
+    const int tiles_m = ceil_div(P->N, P->BM);
+
+    // ---- baby steps: T_n = 2 T_l T_r - T_m (Eq. 7 / 22-23 / Algorithm 1) ----
+    std::vector<BabyProd> sched = baby_schedule(k, P->opt.pairing);
+    std::vector<int> task_of(k + 1, -1);  // task index that produces T_n (n >= 2)
+    for (const BabyProd& bp : sched) {
+        Task t = blank_task(P);
+        t.mapA = T_map(bp.l);
+        t.mapB = T_map(bp.r);
+        t.group = GROUP_BABY;
+        t.alpha = 2.0;
+        if (bp.m == 0) {
+            t.C = nullptr;
+            t.diag_const = -1.0;  // - T_0 = -I
+        } else {
+            t.C = T_ptr(P, bp.m);
+            t.ldc = P->ld;
+            t.beta = -1.0;
+        }
+        t.Out = T_ptr(P, bp.n);
+        t.ldo = P->ld;
+        int deps[3] = {bp.l, bp.r, bp.m};
+        for (int d = 0; d < 3; ++d) {
+            const int n = deps[d];
+            if (n < 2) continue;
+            bool dup = false;
+            for (int e = 0; e < d; ++e) dup = dup || (deps[e] == n);
+            if (!dup) add_dep(t, DEP_TASK, task_of[n], tiles);
+        }
+        task_of[bp.n] = (int)T.size();
+        T.push_back(t);
+    }
+    P->nbaby = (int)T.size();
+    const int baby_tiles = P->nbaby * tiles;
+
+    // ---- giant steps ----
+    // CHEBYSHEV: B_l = G_l + 2 Y B_{l+1} - B_{l+2} (l = p-1..1), D = G_0 + Y B_1 - B_2, G_l = sum_i g_{i,l} T_i.
+    // POWER    : acc_j = S_j + Y acc_{j+1} (Eq. 4), S_j = sum_i d_{i,j} T_i (Eq. 21).
+    // B_l / acc_l lives in buf[l & 1]; Y = T_k.  Column panels of successive steps are independent chains, so
+    // step l only waits for the SAME column panel of step l+1 (DEP_PANEL_N).
+    const bool power = (P->opt.outer == CHEB_DM_OUTER_POWER);
+    const double* coefT = power ? P->dT : P->gT;
+    const int first_giant = (int)T.size();
+    for (int l = p - 1; l >= 0; --l) {
+        Task t = blank_task(P);
+        t.group = GROUP_GIANT;
+        const bool has_prod = (l + 1 <= p - 1);
+        if (has_prod) {
+            t.mapA = T_map(k);
+            t.mapB = buf_map(P, (l + 1) & 1);
+            t.alpha = (power || l == 0) ? 1.0 : 2.0;
+            if (!power && l + 2 <= p - 1) {
+                t.C = buf_ptr(P, (l + 2) & 1);
+                t.ldc = P->ld;
+                t.beta = -1.0;
+            }
+        } else {
+            t.ktiles = 0;
+        }
+        if (l == 0) {
+            t.out_is_user = 1;
+        } else {
+            t.Out = buf_ptr(P, l & 1);
+            t.ldo = P->ld;
+        }
+        // low-order sum: T_1..T_{k-1} with coefficients row l of the table, T_0 = I through diag_ptr
+        t.sum_base = T_ptr(P, 1);
+        t.sum_count = k - 1;
+        t.coef = coefT + (size_t)l * k + 1;
+        t.diag_ptr = coefT + (size_t)l * k;
+        if (P->nbaby > 0) add_dep(t, DEP_GROUP, GROUP_BABY, baby_tiles);
+        if (has_prod) add_dep(t, DEP_PANEL_N, (int)T.size() - 1, tiles_m);
+        T.push_back(t);
+    }
+    (void)first_giant;
+    P->ntasks_solve = (int)T.size();
+
+    // ---- moments chain (cheb_dm_moments): U_j = T_j(Y), U_{j+1} = 2 Y U_j - U_{j-1}, j = 1..p-2, with the
+    // Frobenius products <U_{j+1}, T_i>, i < k, fused into the epilogue (dot_count).  U_j lives in buf[j & 1]
+    // for j >= 2 (U_1 = Y = T_k, U_0 = I).
+    for (int j = 1; j + 1 <= p - 1; ++j) {
+        Task t = blank_task(P);
+        t.group = GROUP_MOM;
+        t.mapA = T_map(k);
+        t.mapB = (j == 1) ? T_map(k) : buf_map(P, j & 1);
+        t.alpha = 2.0;
+        if (j == 1) {
+            t.diag_const = -1.0;
+        } else if (j == 2) {
+            t.C = T_ptr(P, k);
+            t.ldc = P->ld;
+            t.beta = -1.0;
+        } else {
+            t.C = buf_ptr(P, (j - 1) & 1);
+            t.ldc = P->ld;
+            t.beta = -1.0;
+        }
+        t.Out = buf_ptr(P, (j + 1) & 1);
+        t.ldo = P->ld;
+        t.sum_base = T_ptr(P, 1);
+        t.dot_count = k - 1;  // <U_{j+1}, T_i> for i = 1..k-1; slot k-1 = tr U_{j+1} (= <U, T_0>)
+        t.dot_out = P->dots + (size_t)(j + 1) * tiles * k;
+        if (P->nbaby > 0) add_dep(t, DEP_GROUP, GROUP_BABY, baby_tiles);
+        if (j >= 2) add_dep(t, DEP_TASK, (int)T.size() - 1, tiles);
+        T.push_back(t);
+    }
+    P->ntasks_all = (int)T.size();
+
+    // ---- scratch task of cheb_dm_product ----
+    {
+        Task t = blank_task(P);
+        t.group = GROUP_MISC;
+        t.mapA = buf_map(P, 0);
+        t.mapB = buf_map(P, 1);
+        t.out_is_user = 1;
+        P->product_task = (int)T.size();
+        T.push_back(t);
+    }
+
+    P->h_first.assign(T.size() + 1, 0);
+    for (size_t i = 0; i < T.size(); ++i) P->h_first[i + 1] = P->h_first[i] + T[i].tiles_m * T[i].tiles_n;
+
+    double nprod = 0;
+    for (int i = 0; i < P->ntasks_solve; ++i) nprod += (T[i].ktiles > 0) ? 1.0 : 0.0;
+    P->flops_per_compute = nprod * 2.0 * (double)P->N * (double)P->N * (double)P->N;
+}
+
+cheb_dm_status_t encode_maps(cheb_dm_plan_s* P) {
+    EncodeTiledFn enc = get_encode_fn();
+    if (!enc) return CHEB_DM_ECUDA;
+    std::vector<CUtensorMap> h(P->nmat);
+    const char* env2d = getenv("CHEB_DM_TMA2D");
+    int want2d = (env2d && env2d[0] == '1') ? 1 : 0;
+    for (int pass = 0; pass < 2; ++pass) {
+        bool ok = true;
+        for (int i = 0; i < P->nmat && ok; ++i) {
+            void* base = P->ws + (size_t)i * P->mat_elems;
+            CUresult r;
+            if (!want2d) {
+                // {16 columns (128 B), N rows, ld/16 slabs}: a box of 4 slabs x BK rows lands in shared memory as
+                // [slab][row][128 B] with the 128-byte swizzle keyed on the row.
+                cuuint64_t dims[3] = {16, (cuuint64_t)P->N, (cuuint64_t)(P->ld / 16)};
+                cuuint64_t strides[2] = {(cuuint64_t)P->ld * 8, 128};
+                cuuint32_t box[3] = {16, (cuuint32_t)BK, 4};
+                cuuint32_t estr[3] = {1, 1, 1};
+                r = enc(&h[i], CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, base, dims, strides, box, estr,
+                        CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                        CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+            } else {
+                cuuint64_t dims[2] = {(cuuint64_t)P->ld, (cuuint64_t)P->N};
+                cuuint64_t strides[1] = {(cuuint64_t)P->ld * 8};
+                cuuint32_t box[2] = {16, (cuuint32_t)BK};
+                cuuint32_t estr[2] = {1, 1};
+                r = enc(&h[i], CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, base, dims, strides, box, estr,
+                        CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                        CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+            }
+            ok = (r == CUDA_SUCCESS);
+        }
+        if (ok) {
+            P->tma2d = want2d;
+            CUDA_TRY(cudaMemcpy(P->maps, h.data(), sizeof(CUtensorMap) * P->nmat, cudaMemcpyHostToDevice));
+            return CHEB_DM_OK;
+        }
+        if (want2d) break;
+        want2d = 1;  // the driver refused the slab view: fall back to one 2-D box per slab
+    }
+    return CHEB_DM_ECUDA;
+}
+
+template <class Cfg>
+cheb_dm_status_t launch_cfg(const LaunchArgs& la, int items, int num_sms, cudaStream_t st) {
+    static bool attr_set = false;
+    if (!attr_set) {
+        CUDA_TRY(cudaFuncSetAttribute(gemm_dmma_kernel<Cfg>, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg::SMEM_BYTES));
+        attr_set = true;
+    }
+    int per_sm = 1;
+    CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, gemm_dmma_kernel<Cfg>, Cfg::THREADS, Cfg::SMEM_BYTES));
+    if (per_sm < 1) return CHEB_DM_ECUDA;
+    int grid = per_sm * num_sms;
+    if (grid > items) grid = items;
+    if (grid < 1) grid = 1;
+    gemm_dmma_kernel<Cfg><<<grid, Cfg::THREADS, Cfg::SMEM_BYTES, st>>>(la);
+    CUDA_TRY(cudaGetLastError());
+    return CHEB_DM_OK;
+}
+
+// Launch tasks [t0, t1) as one persistent grid; `work_slot` selects the work counter.
+cheb_dm_status_t launch_tasks(cheb_dm_plan_s* P, int t0, int t1, int use_deps, int work_slot, double* userD,
+                              long long ldD, cudaStream_t st) {
+    LaunchArgs la;
+    la.tasks = P->tasks;
+    la.task_first = P->task_first;
+    la.maps = P->maps;
+    la.work_counter = P->counters + P->off_work + work_slot;
+    la.task_done = P->counters + P->off_task;
+    la.panel_done = P->counters + P->off_panel;
+    la.group_done = P->counters + P->off_group;
+    la.panel_stride = P->panel_stride;
+    la.task_begin = t0;
+    la.task_end = t1;
+    la.use_deps = use_deps;
+    la.N = P->N;
+    la.userD = userD;
+    la.ldD = ldD;
+    la.tma2d = P->tma2d;
+    la.error_flag = P->counters + P->off_error;
+    const int items = P->h_first[t1] - P->h_first[t0];
+    ++P->last_launches;
+    switch (P->tile) {
+        case TILE_128x128: return launch_cfg<Cfg128x128>(la, items, P->num_sms, st);
+        case TILE_128x64: return launch_cfg<Cfg128x64>(la, items, P->num_sms, st);
+        default: return launch_cfg<Cfg64x64>(la, items, P->num_sms, st);
+    }
+}
+
+}  // namespace
+
+// =====================================================================================================
+// C ABI
+// =====================================================================================================
+extern "C" {
+
+const char* cheb_dm_strerror(cheb_dm_status_t s) {
+    switch (s) {
+        case CHEB_DM_OK: return "ok";
+        case CHEB_DM_EINVAL: return "invalid argument";
+        case CHEB_DM_EALLOC: return "workspace allocation failed";
+        case CHEB_DM_ECUDA: return "CUDA error or no device";
+        case CHEB_DM_ESTATE: return "call order violated";
+        case CHEB_DM_EBOUNDS: return "bad spectral bounds";
+        case CHEB_DM_EUNSUPPORTED: return "unsupported dtype";
+        case CHEB_DM_ENOCONV: return "power-basis outer recursion would lose accuracy (use the Chebyshev outer recursion)";
+    }
+    return "unknown status";
+}
+
+cheb_dm_status_t cheb_dm_destroy(cheb_dm_plan_t P) {
+    if (!P) return CHEB_DM_EINVAL;
+    cudaFree(P->ws);
+    cudaFree(P->costab);
+    cudaFree(P->fn);
+    cudaFree(P->c);
+    cudaFree(P->gT);
+    cudaFree(P->dT);
+    cudaFree(P->Amat);
+    cudaFree(P->tau);
+    cudaFree(P->w);
+    cudaFree(P->dots);
+    cudaFree(P->sc);
+    cudaFree(P->maps);
+    cudaFree(P->tasks);
+    cudaFree(P->task_first);
+    cudaFree(P->counters);
+    delete P;
+    return CHEB_DM_OK;
+}
+
+cheb_dm_status_t cheb_dm_plan_ex(cheb_dm_plan_t* plan, int N, int M_terms, cheb_dm_dtype_t dtype,
+                                 const cheb_dm_options_t* opts) {
+    if (!plan || N < 1 || M_terms < 1) return CHEB_DM_EINVAL;
+    if (dtype != CHEB_DM_F64) return CHEB_DM_EUNSUPPORTED;
+    cheb_dm_options_t o;
+    memset(&o, 0, sizeof(o));
+    if (opts) o = *opts;
+    if (o.k < 0 || o.p < 0) return CHEB_DM_EINVAL;
+    if (o.outer != CHEB_DM_OUTER_CHEBYSHEV && o.outer != CHEB_DM_OUTER_POWER) return CHEB_DM_EINVAL;
+    if (o.sched != CHEB_DM_SCHED_GROUPED && o.sched != CHEB_DM_SCHED_SERIAL) return CHEB_DM_EINVAL;
+    if (o.pairing != CHEB_DM_PAIR_ALG1 && o.pairing != CHEB_DM_PAIR_SERIAL) return CHEB_DM_EINVAL;
+    if (o.fuse_sums == 0) o.fuse_sums = 1;
+    int k = o.k, p = o.p;
+    if (k == 0 && p == 0) {
+        k = 1;
+        while ((long long)k * k < M_terms) ++k;  // k = ceil(sqrt(M))
+        p = (M_terms + k - 1) / k;
+    } else if (k == 0) {
+        k = (M_terms + p - 1) / p;
+    } else if (p == 0) {
+        p = (M_terms + k - 1) / k;
+    }
+    if ((long long)k * p < M_terms) return CHEB_DM_EINVAL;
+
+    int dev = 0, ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) return CHEB_DM_ECUDA;
+    CUDA_TRY(cudaGetDevice(&dev));
+    cudaDeviceProp prop;
+    CUDA_TRY(cudaGetDeviceProperties(&prop, dev));
+    if (prop.major < 10) return CHEB_DM_ECUDA;  // the kernels are sm_100a only
+
+    cheb_dm_plan_s* P = new (std::nothrow) cheb_dm_plan_s();
+    if (!P) return CHEB_DM_EALLOC;
+    P->N = N; P->M = M_terms; P->k = k; P->p = p;
+    P->opt = o; P->opt.k = k; P->opt.p = p;
+    P->device = dev; P->num_sms = prop.multiProcessorCount;
+    int nq = 1;
+    while (nq < 4 * M_terms) nq <<= 1;  // N_q = 2^ceil(log2(4M)) (cheb_dm.h)
+    P->Nq = nq;
+    choose_tile(P);
+    P->ld = ((long long)N + 15) / 16 * 16;
+    P->mat_elems = (((size_t)N * (size_t)P->ld) + 127) / 128 * 128;
+    P->nmat = k + 2;
+    P->ws = nullptr; P->costab = P->fn = P->c = P->gT = P->dT = P->Amat = P->tau = P->w = P->dots = nullptr;
+    P->sc = nullptr; P->maps = nullptr; P->tasks = nullptr; P->task_first = nullptr; P->counters = nullptr;
+    P->have_coeffs = P->explicit_bounds = P->have_moments = P->computed = 0;
+    P->last_launches = 0;
+
+    const int tiles = ceil_div(N, P->BM) * ceil_div(N, P->BN);
+    const size_t kp = (size_t)k * p;
+    P->ws_bytes = sizeof(double) * P->mat_elems * P->nmat;
+    bool ok = true;
+    ok = ok && cudaMalloc(&P->ws, P->ws_bytes) == cudaSuccess;
+    ok = ok && cudaMalloc(&P->costab, sizeof(double) * 4 * nq) == cudaSuccess;
+    ok = ok && cudaMalloc(&P->fn, sizeof(double) * nq) == cudaSuccess;
+    ok = ok && cudaMalloc(&P->c, sizeof(double) * kp) == cudaSuccess;
+    ok = ok && cudaMalloc(&P->gT, sizeof(double) * kp) == cudaSuccess;
+    ok = ok && cudaMalloc(&P->dT, sizeof(double) * kp) == cudaSuccess;
+    ok = ok && cudaMalloc(&P->Amat, sizeof(double) * p * p) == cudaSuccess;
+    ok = ok && cudaMalloc(&P->tau, sizeof(double) * kp) == cudaSuccess;
+    ok = ok && cudaMalloc(&P->w, sizeof(double) * nq) == cudaSuccess;
+    ok = ok && cudaMalloc(&P->dots, sizeof(double) * ((size_t)(p + 1) * tiles * k + (size_t)2 * k * 16)) == cudaSuccess;
+    ok = ok && cudaMalloc(&P->sc, sizeof(DevScalars)) == cudaSuccess;
+    ok = ok && cudaMalloc(&P->maps, sizeof(CUtensorMap) * P->nmat) == cudaSuccess;
+    if (!ok) {
+        cudaGetLastError();
+        cheb_dm_destroy(P);
+        return CHEB_DM_EALLOC;
+    }
+    P->ws_bytes += sizeof(double) * (4 * (size_t)nq + 2 * nq + 4 * kp + (size_t)p * p + (size_t)(p + 1) * tiles * k);
+
+    cheb_dm_status_t st = CHEB_DM_OK;
+    do {
+        if (cudaMemset(P->ws, 0, sizeof(double) * P->mat_elems * P->nmat) != cudaSuccess) { st = CHEB_DM_ECUDA; break; }
+        cudaMemset(P->dT, 0, sizeof(double) * kp);
+        cudaMemset(P->gT, 0, sizeof(double) * kp);
+        cudaMemset(P->c, 0, sizeof(double) * kp);
+        cudaMemset(P->sc, 0, sizeof(DevScalars));
+        std::vector<double> tab, A;
+        build_costab(nq, tab);
+        build_Amat(p, A);
+        if (cudaMemcpy(P->costab, tab.data(), sizeof(double) * tab.size(), cudaMemcpyHostToDevice) != cudaSuccess ||
+            cudaMemcpy(P->Amat, A.data(), sizeof(double) * A.size(), cudaMemcpyHostToDevice) != cudaSuccess) {
+            st = CHEB_DM_ECUDA;
+            break;
+        }
+        st = encode_maps(P);
+        if (st != CHEB_DM_OK) break;
+        build_tasks(P);
+        const int nt = (int)P->h_tasks.size();
+        P->panel_stride = ceil_div(N, P->BN);
+        P->nwork = nt + 4;
+        P->off_work = 0;
+        P->off_task = P->off_work + P->nwork;
+        P->off_group = P->off_task + nt;
+        P->off_error = P->off_group + NGROUPS;
+        P->off_panel = P->off_error + 1;
+        P->counters_ints = (size_t)P->off_panel + (size_t)nt * P->panel_stride;
+        if (cudaMalloc(&P->tasks, sizeof(Task) * nt) != cudaSuccess ||
+            cudaMalloc(&P->task_first, sizeof(int) * (nt + 1)) != cudaSuccess ||
+            cudaMalloc(&P->counters, sizeof(int) * P->counters_ints) != cudaSuccess) {
+            cudaGetLastError();
+            st = CHEB_DM_EALLOC;
+            break;
+        }
+        if (cudaMemcpy(P->tasks, P->h_tasks.data(), sizeof(Task) * nt, cudaMemcpyHostToDevice) != cudaSuccess ||
+            cudaMemcpy(P->task_first, P->h_first.data(), sizeof(int) * (nt + 1), cudaMemcpyHostToDevice) != cudaSuccess ||
+            cudaMemset(P->counters, 0, sizeof(int) * P->counters_ints) != cudaSuccess) {
+            st = CHEB_DM_ECUDA;
+            break;
+        }
+        if (cudaDeviceSynchronize() != cudaSuccess) { st = CHEB_DM_ECUDA; break; }
+    } while (0);
+    if (st != CHEB_DM_OK) {
+        cheb_dm_destroy(P);
+        return st;
+    }
+    *plan = P;
+    return CHEB_DM_OK;
+}
+
+cheb_dm_status_t cheb_dm_plan(cheb_dm_plan_t* plan, int N, int M_terms, cheb_dm_dtype_t dtype) {
+    return cheb_dm_plan_ex(plan, N, M_terms, dtype, nullptr);
+}
+
+cheb_dm_status_t cheb_dm_coeffs(cheb_dm_plan_t P, double beta, double mu, const double* bounds) {
+    if (!P) return CHEB_DM_EINVAL;
+    if (!isfinite(beta) || !isfinite(mu) || !(beta > 0.0)) return CHEB_DM_EINVAL;
+    if (bounds) {
+        if (!isfinite(bounds[0]) || !isfinite(bounds[1]) || !(bounds[1] > bounds[0])) return CHEB_DM_EBOUNDS;
+        P->a = bounds[0];
+        P->b = bounds[1];
+        P->explicit_bounds = 1;
+    } else {
+        P->explicit_bounds = 0;
+    }
+    P->beta = beta;
+    P->mu = mu;
+    P->have_coeffs = 1;
+    return CHEB_DM_OK;
+}
+
+cheb_dm_status_t cheb_dm_get_kp(cheb_dm_plan_t P, int* k_out, int* p_out) {
+    if (!P || !k_out || !p_out) return CHEB_DM_EINVAL;
+    *k_out = P->k;
+    *p_out = P->p;
+    return CHEB_DM_OK;
+}
+
+cheb_dm_status_t cheb_dm_workspace_bytes(cheb_dm_plan_t P, size_t* bytes_out) {
+    if (!P || !bytes_out) return CHEB_DM_EINVAL;
+    *bytes_out = P->ws_bytes;
+    return CHEB_DM_OK;
+}
+
+cheb_dm_status_t cheb_dm_last_launch_count(cheb_dm_plan_t P, int* launches_out) {
+    if (!P || !launches_out) return CHEB_DM_EINVAL;
+    *launches_out = P->last_launches;
+    return CHEB_DM_OK;
+}
+
+cheb_dm_status_t cheb_dm_flops_per_compute(cheb_dm_plan_t P, double* flops_out) {
+    if (!P || !flops_out) return CHEB_DM_EINVAL;
+    *flops_out = P->flops_per_compute;
+    return CHEB_DM_OK;
+}
+
+}  // extern "C"
+
+namespace {
+
+// Steps a-1 .. a-3 on the stream: bounds (+ rescale of H into T_1), c_n, g (and d).
+cheb_dm_status_t front_end(cheb_dm_plan_s* P, const double* dH, cudaStream_t st) {
+    init_scalars_kernel<<<1, 1, 0, st>>>(P->sc, P->a, P->b, P->explicit_bounds);
+    ++P->last_launches;
+    {
+        static int coop_blocks_per_sm = 0;
+        if (coop_blocks_per_sm == 0) {
+            CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&coop_blocks_per_sm, bounds_rescale_kernel, 512, 0));
+            if (coop_blocks_per_sm < 1) return CHEB_DM_ECUDA;
+        }
+        const int warps_per_block = 512 / 32;
+        int grid = ceil_div(P->N, warps_per_block);
+        const int cap = coop_blocks_per_sm * P->num_sms;
+        if (grid > cap) grid = cap;
+        const double* H = dH;
+        int N = P->N;
+        double* X = T_ptr(P, 1);
+        long long ldx = P->ld;
+        DevScalars* sc = P->sc;
+        int eb = P->explicit_bounds;
+        void* args[] = {(void*)&H, (void*)&N, (void*)&X, (void*)&ldx, (void*)&sc, (void*)&eb};
+        CUDA_TRY(cudaLaunchCooperativeKernel((const void*)bounds_rescale_kernel, dim3(grid), dim3(512), args, 0, st));
+        ++P->last_launches;
+    }
+    fermi_nodes_kernel<<<ceil_div(P->Nq, 256), 256, 0, st>>>(P->sc, P->beta, P->mu, P->costab, P->Nq, P->fn);
+    dct_kernel<<<P->k * P->p, 256, 0, st>>>(P->fn, P->costab, P->Nq, P->M, P->c);
+    int tb = P->k < 32 ? 32 : (P->k > 1024 ? 1024 : (P->k + 31) / 32 * 32);
+    tables_kernel<<<1, tb, 0, st>>>(P->c, P->k, P->p, P->Amat, P->opt.outer == CHEB_DM_OUTER_POWER ? 1 : 0, P->gT, P->dT);
+    P->last_launches += 3;
+    CUDA_TRY(cudaGetLastError());
+    return CHEB_DM_OK;
+}
+
+cheb_dm_status_t reset_counters(cheb_dm_plan_s* P, cudaStream_t st) {
+    CUDA_TRY(cudaMemsetAsync(P->counters, 0, sizeof(int) * P->counters_ints, st));
+    return CHEB_DM_OK;
+}
+
+cheb_dm_status_t run_tasks(cheb_dm_plan_s* P, int t0, int t1, double* userD, long long ldD, cudaStream_t st) {
+    if (t1 <= t0) return CHEB_DM_OK;
+    if (P->opt.sched == CHEB_DM_SCHED_GROUPED) return launch_tasks(P, t0, t1, 1, t0, userD, ldD, st);
+    for (int t = t0; t < t1; ++t) {
+        cheb_dm_status_t s = launch_tasks(P, t, t + 1, 0, t, userD, ldD, st);
+        if (s != CHEB_DM_OK) return s;
+    }
+    return CHEB_DM_OK;
+}
+
+bool device_ok(const cheb_dm_plan_s* P) {
+    int dev = -1;
+    return cudaGetDevice(&dev) == cudaSuccess && dev == P->device;
+}
+
+}  // namespace
+
+extern "C" {
+
+cheb_dm_status_t cheb_dm_compute(cheb_dm_plan_t P, const double* dH, double* dD, void* cuda_stream) {
+    if (!P || !dH || !dD || dH == dD) return CHEB_DM_EINVAL;
+    if (!P->have_coeffs) return CHEB_DM_ESTATE;
+    if (!device_ok(P)) return CHEB_DM_ECUDA;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    P->last_launches = 0;
+    cheb_dm_status_t s = reset_counters(P, st);
+    if (s != CHEB_DM_OK) return s;
+    s = front_end(P, dH, st);
+    if (s != CHEB_DM_OK) return s;
+    s = run_tasks(P, 0, P->ntasks_solve, dD, P->N, st);
+    if (s != CHEB_DM_OK) return s;
+    P->computed = 1;
+    return CHEB_DM_OK;
+}
+
+cheb_dm_status_t cheb_dm_trace(cheb_dm_plan_t P, const double* dD, double* trace_out, void* cuda_stream) {
+    if (!P || !dD || !trace_out) return CHEB_DM_EINVAL;
+    if (!device_ok(P)) return CHEB_DM_ECUDA;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    trace_kernel<<<1, 1024, 0, st>>>(dD, P->N, P->N, trace_out);
+    CUDA_TRY(cudaGetLastError());
+    return CHEB_DM_OK;
+}
+
+cheb_dm_status_t cheb_dm_get_bounds(cheb_dm_plan_t P, double* bounds_out, void* cuda_stream) {
+    if (!P || !bounds_out) return CHEB_DM_EINVAL;
+    if (!P->computed) return CHEB_DM_ESTATE;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    DevScalars h;
+    CUDA_TRY(cudaMemcpyAsync(&h, P->sc, sizeof(h), cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(cudaStreamSynchronize(st));
+    if (h.bad_bounds || !isfinite(h.a) || !isfinite(h.b)) return CHEB_DM_EBOUNDS;
+    bounds_out[0] = h.a;
+    bounds_out[1] = h.b;
+    return CHEB_DM_OK;
+}
+
+cheb_dm_status_t cheb_dm_get_coeffs(cheb_dm_plan_t P, double* c_out, double* g_out, double* d_out, void* cuda_stream) {
+    if (!P) return CHEB_DM_EINVAL;
+    if (!P->computed) return CHEB_DM_ESTATE;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const int k = P->k, p = P->p;
+    const size_t kp = (size_t)k * p;
+    std::vector<double> tmp(kp);
+    if (c_out) CUDA_TRY(cudaMemcpyAsync(c_out, P->c, sizeof(double) * kp, cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(cudaStreamSynchronize(st));
+    for (int which = 0; which < 2; ++which) {
+        double* out = which == 0 ? g_out : d_out;
+        if (!out) continue;
+        CUDA_TRY(cudaMemcpyAsync(tmp.data(), which == 0 ? P->gT : P->dT, sizeof(double) * kp, cudaMemcpyDeviceToHost, st));
+        CUDA_TRY(cudaStreamSynchronize(st));
+        for (int l = 0; l < p; ++l)
+            for (int i = 0; i < k; ++i) out[(size_t)i * p + l] = tmp[(size_t)l * k + i];  // device layout is [l][i]
+    }
+    return CHEB_DM_OK;
+}
+
+cheb_dm_status_t cheb_dm_get_T(cheb_dm_plan_t P, int n, double* dOut, void* cuda_stream) {
+    if (!P || !dOut || n < 1 || n > P->k) return CHEB_DM_EINVAL;
+    if (!P->computed) return CHEB_DM_ESTATE;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    unpad_copy_kernel<<<P->num_sms * 4, 256, 0, st>>>(T_ptr(P, n), P->ld, P->N, dOut);
+    CUDA_TRY(cudaGetLastError());
+    CUDA_TRY(cudaStreamSynchronize(st));
+    return CHEB_DM_OK;
+}
+
+cheb_dm_status_t cheb_dm_product(cheb_dm_plan_t P, double alpha, const double* dA, const double* dB, double beta,
+                                 const double* dC, double* dOut, void* cuda_stream) {
+    if (!P || !dA || !dB || !dOut) return CHEB_DM_EINVAL;
+    if (dOut == dA || dOut == dB) return CHEB_DM_EINVAL;
+    if (!device_ok(P)) return CHEB_DM_ECUDA;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    // operands go through the TMA-described workspace buffers (this also handles odd N)
+    pad_copy_kernel<<<P->num_sms * 4, 256, 0, st>>>(dA, P->N, buf_ptr(P, 0), P->ld);
+    pad_copy_kernel<<<P->num_sms * 4, 256, 0, st>>>(dB, P->N, buf_ptr(P, 1), P->ld);
+    Task t = P->h_tasks[P->product_task];
+    t.alpha = alpha;
+    t.beta = beta;
+    t.C = dC;
+    t.ldc = P->N;
+    CUDA_TRY(cudaMemcpyAsync(P->tasks + P->product_task, &t, sizeof(Task), cudaMemcpyHostToDevice, st));
+    CUDA_TRY(cudaMemsetAsync(P->counters + P->off_work + P->product_task, 0, sizeof(int), st));
+    const int save = P->last_launches;
+    cheb_dm_status_t s = launch_tasks(P, P->product_task, P->product_task + 1, 0, P->product_task, dOut, P->N, st);
+    P->last_launches = save;
+    // the pageable-source copy above is staged by the runtime before it returns, so `t` may go out of scope
+    return s;
+}
+
+}  // extern "C"
+
+extern "C" {
+
+cheb_dm_status_t cheb_dm_moments(cheb_dm_plan_t P, const double* dH, double* tau_host, void* cuda_stream) {
+    if (!P || !dH) return CHEB_DM_EINVAL;
+    if (!P->have_coeffs) return CHEB_DM_ESTATE;
+    if (!device_ok(P)) return CHEB_DM_ECUDA;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const int k = P->k, p = P->p;
+    const int tiles = ceil_div(P->N, P->BM) * ceil_div(P->N, P->BN);
+    P->last_launches = 0;
+    cheb_dm_status_t s = reset_counters(P, st);
+    if (s != CHEB_DM_OK) return s;
+    s = front_end(P, dH, st);  // bounds + rescale (the coefficient tables it also writes are not used here)
+    if (s != CHEB_DM_OK) return s;
+    s = run_tasks(P, 0, P->nbaby, nullptr, 0, st);
+    if (s != CHEB_DM_OK) return s;
+    // j = 1: U_1 = T_k is a baby-step output, its products with T_1..T_{k-1} and all tr T_n come from one pass
+    const int nchunks = 16;
+    double* part1 = P->dots + (size_t)(p + 1) * tiles * k;  // (k-1) + 1 + k rows of nchunks partials
+    {
+        dim3 grid(2 * k, nchunks);
+        frob_partial_kernel<<<grid, 256, 0, st>>>(T_ptr(P, k), T_ptr(P, 1), (long long)P->mat_elems, P->ld, P->N, k - 1, k, part1);
+        ++P->last_launches;
+    }
+    // the chain tasks reuse group/task counters; the baby group counter is already complete
+    if (P->ntasks_all > P->ntasks_solve) {
+        if (P->opt.sched == CHEB_DM_SCHED_GROUPED)
+            s = launch_tasks(P, P->ntasks_solve, P->ntasks_all, 1, P->ntasks_solve, nullptr, 0, st);
+        else
+            s = run_tasks(P, P->ntasks_solve, P->ntasks_all, nullptr, 0, st);
+        if (s != CHEB_DM_OK) return s;
+    }
+    moments_kernel<<<1, 256, 0, st>>>(part1, nchunks, P->dots, tiles, k, p, P->N, P->tau);
+    ++P->last_launches;
+    CUDA_TRY(cudaGetLastError());
+    P->have_moments = 1;
+    P->computed = 1;
+    if (tau_host) {
+        CUDA_TRY(cudaMemcpyAsync(tau_host, P->tau, sizeof(double) * (size_t)k * p, cudaMemcpyDeviceToHost, st));
+        CUDA_TRY(cudaStreamSynchronize(st));
+    }
+    return CHEB_DM_OK;
+}
+
+cheb_dm_status_t cheb_dm_solve_mu(cheb_dm_plan_t P, double beta, double n_occ, int iters, double* mu_out,
+                                  void* cuda_stream) {
+    if (!P || !mu_out || iters < 1 || !isfinite(beta) || !(beta > 0.0) || !isfinite(n_occ)) return CHEB_DM_EINVAL;
+    if (!P->have_moments) return CHEB_DM_ESTATE;
+    if (!device_ok(P)) return CHEB_DM_ECUDA;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    mu_weights_kernel<<<P->Nq, 128, 0, st>>>(P->tau, P->costab, P->Nq, P->M, P->w);
+    mu_bisect_kernel<<<1, 1024, 0, st>>>(P->sc, beta, n_occ, iters, P->costab, P->Nq, P->w);
+    CUDA_TRY(cudaGetLastError());
+    DevScalars h;
+    CUDA_TRY(cudaMemcpyAsync(&h, P->sc, sizeof(h), cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(cudaStreamSynchronize(st));
+    if (h.bad_bounds) return CHEB_DM_EBOUNDS;
+    *mu_out = h.mu;
+    return CHEB_DM_OK;
+}
+
+}  // extern "C"

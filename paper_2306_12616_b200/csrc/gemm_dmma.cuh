@@ -1,0 +1,456 @@
+// gemm_dmma.cuh -- persistent grouped FP64 GEMM for sm_100a (north_star items 2 and 3).
+//
+// One launch runs a list of "tasks".  A task is one product of the recurrence with its fused epilogue
+//
+//     Out = alpha * (A^T B) + beta * C + sum_{i<ns} coef[i] * S_i + diag * I
+//
+// which covers  T_{a+b} = 2 T_a T_b - T_|a-b|          (Eq. 7, 22-23, Alg. 1),
+//               acc    <- S_j + T_k acc                 (Eq. 4; S_j of Eq. 21, :196-201)
+//           and B_l     = G_l + 2 T_k B_{l+1} - B_{l+2} (Clenshaw form of Eq. 4, reading A6),
+// the low-order sums S_j / G_l = sum_i coef_i T_i being formed in registers by the epilogue, so the
+// "matrix additions" of PAPER.md:234 never make a separate pass over HBM.  All operands of the method
+// are symmetric polynomials of X, so A^T = A: both operands are fetched as [k][column] tiles.
+//
+// Hardware mapping.  sm_100a has no tcgen05 kind::f64; FP64 tensor work is mma.sync.m8n8k4 -> SASS
+// DMMA.8x8x4 (measured 37.17 TFLOP/s = 64 FMA/clk/SM, one DMMA per 16 clk per SM sub-partition).
+// Operand tiles are staged by TMA (cp.async.bulk.tensor.3d, 128-byte swizzle) into a ring of shared-
+// memory stages guarded by full/empty mbarriers; one producer warp issues TMA, the consumer warps each
+// own a 32x32 accumulator tile in registers.  The swizzled layout plus an interleaved k-assignment
+// (lane t of a DMMA takes k-rows {par+2t}) makes every 64-bit ld.shared bank-conflict free.
+//
+// Scheduling.  CTAs are persistent: the producer lane claims work items (task, tile) from a global
+// counter in topological order, waits on global completion counters (whole task, one column panel of a
+// task, or a whole group of tasks), then streams the tile's K loop.  Claiming in order makes the spin
+// waits deadlock-free whatever the residency.  This replaces the paper's stream-level concurrency
+// (Alg. 1 "sync streams()").
+#pragma once
+#include "common.cuh"
+
+namespace chebdm {
+
+constexpr int BK = 16;                  // k-rows per pipeline stage
+constexpr int SLAB_BYTES = BK * 128;    // one 16-column slab: BK rows x 128 B (swizzle-128B atom rows)
+constexpr int BOX_COLS = 64;            // columns per TMA box (4 slabs)
+constexpr int BOX_BYTES = 4 * SLAB_BYTES;
+constexpr int TILE_RING = 2;            // producer run-ahead (tile descriptors in flight)
+constexpr int MAX_DEPS = 4;
+constexpr long long WATCHDOG_CLOCKS = 8000000000ll;
+
+enum DepKind : int { DEP_NONE = 0, DEP_TASK = 1, DEP_PANEL_N = 2, DEP_GROUP = 3 };
+
+struct Task {
+    // operands (indices into the tensor-map table); ktiles == 0 => no product, epilogue only
+    int mapA, mapB;
+    int ktiles;
+    int tiles_m, tiles_n;
+    int group;               // group whose counter this task's tiles increment
+    int out_is_user;         // Out = the user's D (pointer/ld come from the launch parameters)
+    int ndeps;
+    int dep_kind[MAX_DEPS];
+    int dep_idx[MAX_DEPS];   // task index (DEP_TASK, DEP_PANEL_N) or group index (DEP_GROUP)
+    int dep_target[MAX_DEPS];  // counter value that means "complete" (tiles of the task / panel / group)
+    double alpha, beta;
+    const double* C;         // nullable
+    long long ldc;
+    double* Out;
+    long long ldo;
+    const double* sum_base;  // S_i = sum_base + i * sum_stride   (same ld as the workspace)
+    long long sum_stride;
+    long long lds;
+    int sum_count;
+    int dot_count;           // moments: <Out, S_i>_F partial sums for i < dot_count (0 = off)
+    const double* coef;      // coef[i], i < sum_count (device memory, written by the coefficient kernel)
+    const double* diag_ptr;  // nullable: coefficient of T_0 = I
+    double diag_const;
+    double* dot_out;         // [tile][dot_count+1] partials (entry dot_count = partial trace of Out)
+};
+
+struct LaunchArgs {
+    const Task* tasks;
+    const int* task_first;   // prefix sums of tiles, ntasks+1 entries
+    const CUtensorMap* maps;
+    int* work_counter;       // claimed-items counter of this launch
+    int* task_done;          // [ntasks]
+    int* panel_done;         // [ntasks * panel_stride]
+    int* group_done;         // [ngroups]
+    int panel_stride;
+    int task_begin, task_end;
+    int use_deps;
+    int N;
+    double* userD;
+    long long ldD;
+    int tma2d;               // 1: operand maps are 2-D {column, row} with one 16-column box per copy
+    int* error_flag;         // set to 1 if a dependency wait exceeds the watchdog (never in a correct run)
+};
+
+template <int BM_, int BN_, int STAGES_, int MIN_CTAS_>
+struct GemmCfg {
+    static constexpr int BM = BM_, BN = BN_, STAGES = STAGES_, MIN_CTAS = MIN_CTAS_;
+    static constexpr int WARPS_M = BM / 32, WARPS_N = BN / 32;
+    static constexpr int CONSUMER_WARPS = WARPS_M * WARPS_N;
+    static constexpr int CONSUMER_THREADS = CONSUMER_WARPS * 32;
+    static constexpr int THREADS = CONSUMER_THREADS + 32;
+    static constexpr int A_BYTES = BM * BK * 8, B_BYTES = BN * BK * 8;
+    static constexpr int STAGE_BYTES = A_BYTES + B_BYTES;
+    static constexpr int BAR_OFFSET = STAGES * STAGE_BYTES;
+    static constexpr int DOT_OFFSET = BAR_OFFSET + 256;          // [CONSUMER_WARPS][32] doubles (moments epilogue)
+    static constexpr int SMEM_BYTES = DOT_OFFSET + CONSUMER_WARPS * 32 * 8 + 1024;  // + alignment slack
+};
+
+struct TileInfo {
+    int task, tm, tn, stop;
+};
+
+template <class Cfg>
+__global__ void __launch_bounds__(Cfg::THREADS, Cfg::MIN_CTAS) gemm_dmma_kernel(const LaunchArgs args) {
+    constexpr int BM = Cfg::BM, BN = Cfg::BN, STAGES = Cfg::STAGES;
+    extern __shared__ uint8_t smem_raw[];
+    // 1024-byte alignment: the 128B swizzle pattern is a function of address bits [7:9]
+    uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+    uint64_t* bars = reinterpret_cast<uint64_t*>(smem + Cfg::BAR_OFFSET);
+    // bars[0..S) full, [S..2S) empty, [2S..2S+R) tile_full, [2S+R..2S+2R) tile_empty
+    TileInfo* ring = reinterpret_cast<TileInfo*>(smem + Cfg::BAR_OFFSET + 160);
+    const uint32_t smem_base = smem_u32(smem);
+    const uint32_t bar_base = smem_u32(bars);
+    auto full_bar = [&](int s) { return bar_base + 8u * s; };
+    auto empty_bar = [&](int s) { return bar_base + 8u * (STAGES + s); };
+    auto tfull_bar = [&](int s) { return bar_base + 8u * (2 * STAGES + s); };
+    auto tempty_bar = [&](int s) { return bar_base + 8u * (2 * STAGES + TILE_RING + s); };
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < STAGES; ++s) {
+            mbar_init(full_bar(s), 1);
+            mbar_init(empty_bar(s), Cfg::CONSUMER_WARPS);
+        }
+        for (int s = 0; s < TILE_RING; ++s) {
+            mbar_init(tfull_bar(s), 1);
+            mbar_init(tempty_bar(s), Cfg::CONSUMER_WARPS);
+        }
+        fence_mbar_init();
+    }
+    __syncthreads();
+
+    const int item_begin = args.task_first[args.task_begin];
+    const int item_end = args.task_first[args.task_end];
+
+    if (warp == Cfg::CONSUMER_WARPS) {
+        // =================================== producer warp ===================================
+        if (lane == 0) {
+            int stage = 0;
+            uint32_t phase = 0;
+            int tslot = 0;
+            uint32_t tphase = 0;
+            int cur = args.task_begin;
+            unsigned long long done_tasks_lo = 0;  // cache of "task complete" observations (tasks < 64 rel.)
+            unsigned int done_groups = 0;
+            for (;;) {
+                const int item = item_begin + atomicAdd(args.work_counter, 1);
+                const bool stop = item >= item_end;
+                int tm = 0, tn = 0;
+                const Task* tk = nullptr;
+                if (!stop) {
+                    while (item >= args.task_first[cur + 1]) ++cur;
+                    tk = args.tasks + cur;
+                    const int local = item - args.task_first[cur];
+                    const int tiles_m = tk->tiles_m;
+                    tn = local / tiles_m;  // column-panel-major order: a panel's tiles are consecutive
+                    tm = local - tn * tiles_m;
+                    if (args.use_deps) {
+                        const int nd = tk->ndeps;
+                        for (int d = 0; d < nd; ++d) {
+                            const int kind = tk->dep_kind[d], idx = tk->dep_idx[d], target = tk->dep_target[d];
+                            const int* ctr;
+                            if (kind == DEP_TASK) {
+                                const int rel = idx - args.task_begin;
+                                if (rel < 64 && ((done_tasks_lo >> rel) & 1ull)) continue;
+                                ctr = args.task_done + idx;
+                            } else if (kind == DEP_PANEL_N) {
+                                ctr = args.panel_done + (size_t)idx * args.panel_stride + tn;
+                            } else {
+                                if ((done_groups >> idx) & 1u) continue;
+                                ctr = args.group_done + idx;
+                            }
+                            if (ld_acquire_gpu(ctr) < target) {
+                                const long long t0 = clock64();
+                                while (ld_acquire_gpu(ctr) < target) {
+                                    __nanosleep(32);
+                                    if (clock64() - t0 > WATCHDOG_CLOCKS) {  // ~4 s: report instead of hanging
+                                        atomicExch(args.error_flag, 1);
+                                        break;
+                                    }
+                                }
+                            }
+                            if (kind == DEP_TASK) {
+                                const int rel = idx - args.task_begin;
+                                if (rel < 64) done_tasks_lo |= 1ull << rel;
+                            } else if (kind == DEP_GROUP) {
+                                done_groups |= 1u << idx;
+                            }
+                        }
+                        fence_proxy_async();
+                    }
+                }
+                // publish the tile descriptor to the consumer warps
+                mbar_wait(tempty_bar(tslot), tphase ^ 1);
+                ring[tslot].task = cur;
+                ring[tslot].tm = tm;
+                ring[tslot].tn = tn;
+                ring[tslot].stop = stop ? 1 : 0;
+                mbar_arrive(tfull_bar(tslot));
+                if (++tslot == TILE_RING) { tslot = 0; tphase ^= 1; }
+                if (stop) break;
+
+                const int ktiles = tk->ktiles;
+                if (ktiles > 0) {
+                    const CUtensorMap* mapA = args.maps + tk->mapA;
+                    const CUtensorMap* mapB = args.maps + tk->mapB;
+                    const int slabA = tm * (BM / 16), slabB = tn * (BN / 16);
+                    for (int kt = 0; kt < ktiles; ++kt) {
+                        mbar_wait(empty_bar(stage), phase ^ 1);
+                        const uint32_t sA = smem_base + stage * Cfg::STAGE_BYTES;
+                        const uint32_t sB = sA + Cfg::A_BYTES;
+                        mbar_arrive_expect_tx(full_bar(stage), Cfg::STAGE_BYTES);
+                        if (!args.tma2d) {
+#pragma unroll
+                            for (int b = 0; b < BM / BOX_COLS; ++b)
+                                tma_load_3d(sA + b * BOX_BYTES, mapA, full_bar(stage), 0, kt * BK, slabA + 4 * b);
+#pragma unroll
+                            for (int b = 0; b < BN / BOX_COLS; ++b)
+                                tma_load_3d(sB + b * BOX_BYTES, mapB, full_bar(stage), 0, kt * BK, slabB + 4 * b);
+                        } else {
+#pragma unroll
+                            for (int b = 0; b < BM / 16; ++b)
+                                tma_load_2d(sA + b * SLAB_BYTES, mapA, full_bar(stage), (slabA + b) * 16, kt * BK);
+#pragma unroll
+                            for (int b = 0; b < BN / 16; ++b)
+                                tma_load_2d(sB + b * SLAB_BYTES, mapB, full_bar(stage), (slabB + b) * 16, kt * BK);
+                        }
+                        if (++stage == STAGES) { stage = 0; phase ^= 1; }
+                    }
+                }
+            }
+        }
+        return;
+    }
+
+    // ======================================= consumer warps =======================================
+    const int wm = warp / Cfg::WARPS_N, wn = warp % Cfg::WARPS_N;
+    const int g = lane >> 2, t = lane & 3;
+    // Per-lane fragment offsets inside a stage (see header comment).  For k4-step j: jh = j>>1, par = j&1,
+    // physical k-row r = 8*jh + par + 2t.  Column c = w*32 + i*8 + g of the operand tile lives in slab c>>4,
+    // 16-byte chunk ((c&15)>>1) ^ (r&7), half c&1.
+    uint32_t aoff[2], boff[2];
+#pragma unroll
+    for (int par = 0; par < 2; ++par) {
+        const uint32_t x = par + 2 * t;
+        const uint32_t lo = x * 128 + ((((uint32_t)g >> 1) ^ x) << 4) + (g & 1) * 8;
+        aoff[par] = (wm * 2) * SLAB_BYTES + lo;
+        boff[par] = Cfg::A_BYTES + (wn * 2) * SLAB_BYTES + lo;
+    }
+
+    int stage = 0;
+    uint32_t phase = 0;
+    int tslot = 0;
+    uint32_t tphase = 0;
+
+    for (;;) {
+        mbar_wait(tfull_bar(tslot), tphase);
+        const TileInfo ti = ring[tslot];
+        __syncwarp();
+        if (lane == 0) mbar_arrive(tempty_bar(tslot));
+        if (++tslot == TILE_RING) { tslot = 0; tphase ^= 1; }
+        if (ti.stop) break;
+        const Task* tk = args.tasks + ti.task;
+
+        double acc[4][4][2];
+#pragma unroll
+        for (int i = 0; i < 4; ++i)
+#pragma unroll
+            for (int j = 0; j < 4; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
+
+        const int ktiles = tk->ktiles;
+        for (int kt = 0; kt < ktiles; ++kt) {
+            mbar_wait(full_bar(stage), phase);
+            const uint8_t* sbase = smem + stage * Cfg::STAGE_BYTES;
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                const int jh = j >> 1, par = j & 1;
+                double a[4], b[4];
+#pragma unroll
+                for (int i = 0; i < 4; ++i) {
+                    a[i] = *reinterpret_cast<const double*>(sbase + ((aoff[par] ^ ((i & 1) << 6)) + (i >> 1) * SLAB_BYTES + jh * 1024));
+                    b[i] = *reinterpret_cast<const double*>(sbase + ((boff[par] ^ ((i & 1) << 6)) + (i >> 1) * SLAB_BYTES + jh * 1024));
+                }
+#pragma unroll
+                for (int im = 0; im < 4; ++im)
+#pragma unroll
+                    for (int jn = 0; jn < 4; ++jn) dmma_884(acc[im][jn][0], acc[im][jn][1], a[im], b[jn]);
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(empty_bar(stage));
+            if (++stage == STAGES) { stage = 0; phase ^= 1; }
+        }
+
+        // ------------------------------------ fused epilogue ------------------------------------
+        const int N = args.N;
+        const int row0 = ti.tm * BM + wm * 32 + g;
+        const int col0 = ti.tn * BN + wn * 32 + 2 * t;
+        const double alpha = tk->alpha;
+#pragma unroll
+        for (int i = 0; i < 4; ++i)
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                acc[i][j][0] *= alpha;
+                acc[i][j][1] *= alpha;
+            }
+        if (tk->C != nullptr) {
+            const double beta = tk->beta;
+            const double* C = tk->C;
+            const long long ldc = tk->ldc;
+            const bool vec = ((ldc & 1) == 0) && ((reinterpret_cast<uintptr_t>(C) & 15) == 0);
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+                const int r = row0 + i * 8;
+#pragma unroll
+                for (int j = 0; j < 4; ++j) {
+                    const int c = col0 + j * 8;
+                    if (r < N && c < N) {
+                        const double* p = C + (long long)r * ldc + c;
+                        if (vec && c + 1 < N) {
+                            const double2 v = __ldcg(reinterpret_cast<const double2*>(p));
+                            acc[i][j][0] = fma(beta, v.x, acc[i][j][0]);
+                            acc[i][j][1] = fma(beta, v.y, acc[i][j][1]);
+                        } else {
+                            acc[i][j][0] = fma(beta, __ldcg(p), acc[i][j][0]);
+                            if (c + 1 < N) acc[i][j][1] = fma(beta, __ldcg(p + 1), acc[i][j][1]);
+                        }
+                    }
+                }
+            }
+        }
+        const int ns = tk->sum_count;
+        if (ns > 0) {
+            // low-order sum  sum_i coef_i T_i  (Eq. 21): workspace matrices, even ld, 16-byte aligned rows
+            const double* coef = tk->coef;
+            const long long lds = tk->lds, sstride = tk->sum_stride;
+            const double* sb = tk->sum_base + (long long)row0 * lds + col0;
+            for (int s = 0; s < ns; ++s) {
+                const double w = coef[s];
+                const double* ps = sb + (long long)s * sstride;
+#pragma unroll
+                for (int i = 0; i < 4; ++i) {
+                    const int r = row0 + i * 8;
+#pragma unroll
+                    for (int j = 0; j < 4; ++j) {
+                        const int c = col0 + j * 8;
+                        if (r < N && c < N) {  // pad column c+1 == N (odd N) holds zeros in the workspace
+                            const double2 v = __ldcg(reinterpret_cast<const double2*>(ps + (long long)(i * 8) * lds + j * 8));
+                            acc[i][j][0] = fma(w, v.x, acc[i][j][0]);
+                            acc[i][j][1] = fma(w, v.y, acc[i][j][1]);
+                        }
+                    }
+                }
+            }
+        }
+        {
+            double diag = tk->diag_const;
+            if (tk->diag_ptr != nullptr) diag += *tk->diag_ptr;
+            if (diag != 0.0) {
+#pragma unroll
+                for (int i = 0; i < 4; ++i)
+#pragma unroll
+                    for (int j = 0; j < 4; ++j) {
+                        const int r = row0 + i * 8, c = col0 + j * 8;
+                        if (r == c) acc[i][j][0] += diag;
+                        if (r == c + 1) acc[i][j][1] += diag;
+                    }
+            }
+        }
+        {
+            double* Out = tk->out_is_user ? args.userD : tk->Out;
+            const long long ldo = tk->out_is_user ? args.ldD : tk->ldo;
+            const bool vec = ((ldo & 1) == 0) && ((reinterpret_cast<uintptr_t>(Out) & 15) == 0);
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+                const int r = row0 + i * 8;
+#pragma unroll
+                for (int j = 0; j < 4; ++j) {
+                    const int c = col0 + j * 8;
+                    if (r < N && c < N) {
+                        double* p = Out + (long long)r * ldo + c;
+                        if (vec && c + 1 < N) {
+                            __stcg(reinterpret_cast<double2*>(p), make_double2(acc[i][j][0], acc[i][j][1]));
+                        } else {
+                            __stcg(p, acc[i][j][0]);
+                            if (c + 1 < N) __stcg(p + 1, acc[i][j][1]);
+                        }
+                    }
+                }
+            }
+        }
+        // ------------- moments: Frobenius products <Out, T_i> and tr Out of this tile (reading A10) -------------
+        const int nd = tk->dot_count;
+        if (tk->dot_out != nullptr) {
+            double* s_red = reinterpret_cast<double*>(smem + Cfg::DOT_OFFSET);
+            const long long lds = tk->lds, sstride = tk->sum_stride;
+            const double* sb = tk->sum_base + (long long)row0 * lds + col0;
+            double* dst = tk->dot_out + (size_t)(ti.tn * tk->tiles_m + ti.tm) * (nd + 1);
+            for (int s0 = 0; s0 <= nd; s0 += 32) {
+                const int cnt = min(32, nd + 1 - s0);
+                for (int q = 0; q < cnt; ++q) {
+                    const int s = s0 + q;
+                    double v = 0.0;
+                    if (s < nd) {
+                        const double* ps = sb + (long long)s * sstride;
+#pragma unroll
+                        for (int i = 0; i < 4; ++i) {
+                            const int r = row0 + i * 8;
+#pragma unroll
+                            for (int j = 0; j < 4; ++j) {
+                                const int c = col0 + j * 8;
+                                if (r < N && c < N) {
+                                    const double2 w2 = __ldcg(reinterpret_cast<const double2*>(ps + (long long)(i * 8) * lds + j * 8));
+                                    v = fma(acc[i][j][0], w2.x, v);
+                                    v = fma(acc[i][j][1], w2.y, v);
+                                }
+                            }
+                        }
+                    } else {  // slot nd: trace
+#pragma unroll
+                        for (int i = 0; i < 4; ++i)
+#pragma unroll
+                            for (int j = 0; j < 4; ++j) {
+                                const int r = row0 + i * 8, c = col0 + j * 8;
+                                if (r < N && r == c) v += acc[i][j][0];
+                                if (r < N && r == c + 1) v += acc[i][j][1];
+                            }
+                    }
+#pragma unroll
+                    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+                    if (lane == 0) s_red[warp * 32 + q] = v;
+                }
+                named_bar_sync(1, Cfg::CONSUMER_THREADS);
+                if (threadIdx.x < cnt) {
+                    double v = 0.0;
+                    for (int w = 0; w < Cfg::CONSUMER_WARPS; ++w) v += s_red[w * 32 + threadIdx.x];
+                    dst[s0 + threadIdx.x] = v;
+                }
+                named_bar_sync(1, Cfg::CONSUMER_THREADS);
+            }
+        }
+        // --------------------------- publish completion of this tile ---------------------------
+        __threadfence();
+        named_bar_sync(1, Cfg::CONSUMER_THREADS);
+        if (threadIdx.x == 0) {
+            __threadfence();
+            fence_proxy_async();
+            red_release_gpu_add(args.panel_done + (size_t)ti.task * args.panel_stride + ti.tn, 1);
+            red_release_gpu_add(args.task_done + ti.task, 1);
+            red_release_gpu_add(args.group_done + tk->group, 1);
+        }
+    }
+}
+
+}  // namespace chebdm
