@@ -1,0 +1,416 @@
+#!/usr/bin/env python
+"""bench.py -- density-matrix solves/sec of the dense Chebyshev Fermi-operator path on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config cfg1] [--impl ours|reference]
+
+One "step" = one pass of the whole hot path (Gershgorin bounds + rescale, coefficient
+tables, baby steps, giant steps with fused low-order sums, trace) over one batch of synthetic input
+= one solve per seed of the workload (cfg1: seeds 0-3 -> 4 solves per step), with mu fixed beforehand
+by the (untimed, separately reported) moment/bisection path.  Everything runs through the C ABI
+(include/cheb_dm.h via the ctypes binding); torch supplies device memory, streams and events only.
+
+Prints ONE JSON line (rank 0).  `value` = solves/s with inputs resident in HBM; `e2e` = the same through
+cheb_dm_compute_host with pinned HOST buffers (H2D + D2H inside the timed region); `roofline` = the
+product kernel against the FP64 tensor (DMMA) peak; `cpu_baseline` = the oracle on the host cores.
+Multi-GPU: replicas only -- every rank runs the same workload on its own GPU, no data-path
+collective; value = all ranks' solves / max-over-ranks time.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "dm_solves_per_sec"
+UNIT = "solves/s"
+FLUSH_BYTES = 512 << 20  # > 126 MB L2
+# dram__bytes_read.sum + dram__bytes_write.sum of one product-kernel launch from the `ncu --set full`
+# captures summarised under profiles/ (per workload); None = not captured yet.
+NCU_TRAFFIC_BYTES = {}
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", default="cfg1", help="workload of the headline line (BASELINE.json configs[1] = cfg1)")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--others", default="cfg2,cfg4,cfg3", help="comma list of extra workloads reported under other_workloads ('' = none)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--sched", type=int, default=0)
+    ap.add_argument("--tile", type=int, default=0)
+    ap.add_argument("--k", type=int, default=0)
+    ap.add_argument("--p", type=int, default=0)
+    return ap.parse_args()
+
+
+# ---------------------------------------------------------------------------------------------------
+# clocks sampler (NVML in a thread; the recipe's nvidia-smi fields)
+# ---------------------------------------------------------------------------------------------------
+class ClockSampler:
+    REASONS = {0x4: "sw_power_cap", 0x8: "hw_slowdown", 0x20: "sw_thermal_slowdown", 0x40: "hw_thermal_slowdown",
+               0x80: "hw_power_brake_slowdown", 0x2: "applications_clocks_setting", 0x10: "sync_boost"}
+
+    def __init__(self, torch, device_index):
+        self.samples = []  # (t, sm_mhz, reasons_mask, power_w)
+        self.regions = []
+        self.ok = False
+        self._stop = threading.Event()
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            h = None
+            try:
+                uuid = str(torch.cuda.get_device_properties(device_index).uuid)
+                h = pynvml.nvmlDeviceGetHandleByUUID(("GPU-" + uuid) if not uuid.startswith("GPU-") else uuid)
+            except Exception:
+                vis = os.environ.get("CUDA_VISIBLE_DEVICES")
+                idx = int(vis.split(",")[device_index]) if vis and vis.split(",")[device_index].isdigit() else device_index
+                h = pynvml.nvmlDeviceGetHandleByIndex(idx)
+            self.h = h
+            self.sm_max = int(pynvml.nvmlDeviceGetMaxClockInfo(h, pynvml.NVML_CLOCK_SM))
+            self.ok = True
+        except Exception as e:  # pragma: no cover
+            self.err = repr(e)
+        if self.ok:
+            self.th = threading.Thread(target=self._run, daemon=True)
+            self.th.start()
+
+    def _run(self):
+        nv = self.nv
+        while not self._stop.is_set():
+            try:
+                sm = int(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                try:
+                    mask = int(nv.nvmlDeviceGetCurrentClocksEventReasons(self.h))
+                except Exception:
+                    mask = int(nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h))
+                pw = nv.nvmlDeviceGetPowerUsage(self.h) / 1000.0
+                self.samples.append((time.perf_counter(), sm, mask, pw))
+            except Exception:
+                pass
+            time.sleep(0.01)
+
+    def begin(self):
+        self._t0 = time.perf_counter()
+
+    def end(self):
+        self.regions.append((self._t0, time.perf_counter()))
+
+    def summary(self):
+        if not self.ok:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "note": "NVML unavailable"}
+        self._stop.set()
+        self.th.join(timeout=1.0)
+        inside = [s for s in self.samples if any(a <= s[0] <= b for a, b in self.regions)]
+        note = "sampled inside the timed regions (NVML, 10 ms period)"
+        if len(inside) < 3:
+            inside = self.samples
+            note = "timed regions shorter than the sampling period: all samples of the run"
+        sm = sorted(s[1] for s in inside)
+        mask = 0
+        for s in inside:
+            mask |= s[2]
+        reasons = [n for bit, n in self.REASONS.items() if mask & bit]
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": self.sm_max, "reasons": reasons,
+                "power_w_max": max((s[3] for s in inside), default=None), "samples": len(inside), "note": note}
+
+
+# ---------------------------------------------------------------------------------------------------
+# GPU arm
+# ---------------------------------------------------------------------------------------------------
+class Workload:
+    """Device-resident inputs + a plan for one BASELINE.json config; mu per seed from the moment path."""
+
+    def __init__(self, torch, cd, workloads, name, args):
+        self.torch, self.cd, self.name = torch, cd, name
+        self.cfg = cfg = workloads.CONFIGS[name]
+        self.N, self.M = cfg.N, cfg.M
+        self.st = torch.cuda.current_stream().cuda_stream
+        self.plan = cd.Plan(cfg.N, cfg.M, sched=args.sched, tile=args.tile, k=args.k, p=args.p)
+        self.hH, self.dH, self.dD, self.hD = [], [], [], []
+        for seed in cfg.seeds:
+            H = torch.from_numpy(workloads.hamiltonian(name, seed=seed))
+            self.hH.append(H.pin_memory())
+            self.dH.append(H.cuda())
+            self.dD.append(torch.empty((cfg.N, cfg.N), dtype=torch.float64, device="cuda"))
+            self.hD.append(torch.empty((cfg.N, cfg.N), dtype=torch.float64).pin_memory())
+        self.dtr = torch.zeros(len(cfg.seeds), dtype=torch.float64, device="cuda")
+        self.htr = torch.zeros(len(cfg.seeds), dtype=torch.float64).pin_memory()
+        # mu per seed: Gershgorin bounds -> moments -> bisection, all on the device (untimed here)
+        self.mu, self.mu_ms = [], []
+        for i in range(len(cfg.seeds)):
+            self.plan.coeffs(cfg.beta, 0.0, None)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            self.plan.moments(self.dH[i].data_ptr(), False, self.st)
+            mu = self.plan.solve_mu(cfg.beta, cfg.N_occ, 100, self.st)
+            e1.record()
+            torch.cuda.synchronize()
+            self.mu.append(mu)
+            self.mu_ms.append(e0.elapsed_time(e1))
+        self.units = len(cfg.seeds)
+        self.launches_per_step = 0
+
+    def step(self):
+        n = 0
+        for i in range(self.units):
+            self.plan.coeffs(self.cfg.beta, self.mu[i], None)
+            self.plan.compute(self.dH[i].data_ptr(), self.dD[i].data_ptr(), self.st)
+            self.plan.trace(self.dD[i].data_ptr(), self.dtr[i:].data_ptr(), self.st)
+            n += self.plan.last_launch_count() + 1
+        self.launches_per_step = n
+
+    def step_host(self):
+        for i in range(self.units):
+            self.plan.coeffs(self.cfg.beta, self.mu[i], None)
+            self.plan.compute_host(self.hH[i].data_ptr(), self.hD[i].data_ptr(), self.htr[i:].data_ptr(), self.st)
+
+    def h2d_bytes(self):
+        return self.units * 8 * self.N * self.N
+
+    def d2h_bytes(self):
+        return self.units * (8 * self.N * self.N + 8)
+
+
+def timed_steps(torch, step_fn, steps, warmup, flush, sampler=None, dist=None):
+    """W untimed steps, then K steps each bracketed by CUDA events on the launching stream with an L2 flush
+    (512 MiB memset) between them; returns total event milliseconds of the K steps."""
+    for _ in range(warmup):
+        flush.zero_()
+        step_fn()
+    torch.cuda.synchronize()
+    if dist is not None:
+        dist.barrier()
+    torch.cuda.synchronize()
+    if sampler:
+        sampler.begin()
+    evs = []
+    for _ in range(steps):
+        flush.zero_()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        step_fn()
+        e1.record()
+        evs.append((e0, e1))
+    torch.cuda.synchronize()
+    if dist is not None:
+        dist.barrier()
+    torch.cuda.synchronize()
+    if sampler:
+        sampler.end()
+    return sum(a.elapsed_time(b) for a, b in evs)
+
+
+def max_over_ranks(torch, dist, ms):
+    """Replicas only: the job's time is the slowest rank's; no data-path collective."""
+    if dist is None:
+        return ms
+    dev = "cuda" if dist.get_backend() == "nccl" else "cpu"
+    t = torch.tensor([ms], dtype=torch.float64, device=dev)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def job_value(world, units_per_step, steps, max_ms):
+    """Whole-job solves/s: every rank processed units_per_step * steps solves in max_ms (weak scaling)."""
+    return world * units_per_step * steps / (max_ms * 1e-3)
+
+
+def measure_workload(torch, cd, workloads, name, args, steps, warmup, flush, sampler, dist, peak_tf, world):
+    w = Workload(torch, cd, workloads, name, args)
+    plan = w.plan
+    # device-resident arm (timing ring on: two event records per compute, no host sync)
+    plan.set_timing(True)
+    for _ in range(warmup):
+        w.step()
+    torch.cuda.synchronize()
+    plan.set_timing(True)  # resets the ring after warm-up
+    total_ms = timed_steps(torch, w.step, steps, 0, flush, sampler, dist)
+    n_rec, prod_ms = plan.product_ms()  # the timed computes only (at most the last 256 of them)
+    plan.set_timing(False)
+    total_ms = max_over_ranks(torch, dist, total_ms)
+    flops = plan.flops_per_compute()
+    ms_per_step = total_ms / steps
+    value = job_value(world, w.units, steps, total_ms)
+    kernel_ms = prod_ms / max(n_rec, 1)
+    achieved = flops / (kernel_ms * 1e-3) * 1e-12 if kernel_ms > 0 else 0.0
+    # end-to-end arm: host buffers through cheb_dm_compute_host
+    e2e_steps = max(3, min(steps, 10))
+    e2e_ms = timed_steps(torch, w.step_host, e2e_steps, max(1, min(warmup, 3)), flush, None, dist)
+    e2e_ms = max_over_ranks(torch, dist, e2e_ms)
+    res = {
+        "workload": name, "N": w.N, "M_terms": w.M, "k": plan.k, "p": plan.p, "solves_per_step": w.units,
+        "value": value, "ms_per_step": ms_per_step, "ms_per_solve": ms_per_step / w.units,
+        "tflops_step": world * w.units * steps * flops / (total_ms * 1e-3) * 1e-12,
+        "flops_per_solve": flops, "gpu_launches_per_step": w.launches_per_step,
+        "roofline": {"bound": "tensor", "kernel": "gemm_dmma_kernel (persistent grouped FP64 DMMA GEMM, all products of one solve)",
+                     "achieved": achieved, "peak": peak_tf, "unit": "TFLOP/s", "frac": achieved / peak_tf if peak_tf else None,
+                     "traffic": NCU_TRAFFIC_BYTES.get(name), "kernel_ms": kernel_ms, "launches_timed": n_rec,
+                     "kernel_share_of_step": (kernel_ms * w.units) / ms_per_step if ms_per_step > 0 else None,
+                     "flops_per_launch": flops},
+        "e2e": {"value": world * w.units * e2e_steps / (e2e_ms * 1e-3), "unit": UNIT,
+                "h2d_bytes_per_step": w.h2d_bytes(), "d2h_bytes_per_step": w.d2h_bytes(), "steps": e2e_steps,
+                "ms_per_step": e2e_ms / e2e_steps},
+        "mu": w.mu, "mu_search_ms": w.mu_ms, "tr_D": [float(x) for x in w.dtr.cpu().tolist()], "N_occ": w.cfg.N_occ,
+        "workspace_bytes": plan.workspace_bytes(),
+    }
+    plan.destroy()
+    del w
+    torch.cuda.empty_cache()
+    return res
+
+
+# ---------------------------------------------------------------------------------------------------
+# CPU oracle arm (cpu_baseline leg and --impl reference)
+# ---------------------------------------------------------------------------------------------------
+def oracle_sample_setup(name):
+    import numpy as np
+    import oracle
+    import workloads
+    cfg = workloads.CONFIGS[name]
+    H = workloads.hamiltonian(name, seed=cfg.seeds[0])
+    a, b = oracle.gershgorin(H)
+    return oracle, np, cfg, H, a, b
+
+
+def oracle_time_terms(oracle, np, cfg, H, a, b, terms):
+    """Seconds for the first `terms` terms of the oracle's naive recurrence (terms-2 plain products)."""
+    c = np.zeros(terms)
+    c[: min(terms, cfg.M)] = oracle.cheb_coeffs(cfg.beta, 0.0, a, b, cfg.M)[:terms]
+    t0 = time.perf_counter()
+    oracle.dm_cheb(H, a, b, c)
+    return time.perf_counter() - t0
+
+
+def oracle_rate(name, budget_s):
+    """solves/s of O-cheb on this host, from a bounded sample extrapolated linearly in the product count."""
+    oracle, np, cfg, H, a, b = oracle_sample_setup(name)
+    t_probe = oracle_time_terms(oracle, np, cfg, H, a, b, 4)  # 2 products
+    per_prod = max(t_probe / 2.0, 1e-6)
+    terms = int(max(4, min(cfg.M, 2 + budget_s / per_prod)))
+    t = oracle_time_terms(oracle, np, cfg, H, a, b, terms)
+    per_prod = t / (terms - 2)
+    t_solve = per_prod * (cfg.M - 2)
+    full = terms >= cfg.M
+    sample = (f"{name} seed {cfg.seeds[0]} (N={cfg.N}, M={cfg.M}): oracle.dm_cheb, first {terms} of {cfg.M} terms "
+              f"({terms - 2} of {cfg.M - 2} naive products, {t:.2f} s)" + ("" if full else ", extrapolated linearly in the number of products"))
+    return 1.0 / t_solve, sample, oracle.num_threads(), terms
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    import workloads
+    name = args.config
+    cfg = workloads.CONFIGS[name]
+    oracle, np, cfg, H, a, b = oracle_sample_setup(name)
+    t_probe = oracle_time_terms(oracle, np, cfg, H, a, b, 4)
+    per_prod = max(t_probe / 2.0, 1e-6)
+    budget_step = min(2.0, 150.0 / max(1, args.steps + args.warmup))
+    terms = int(max(3, min(cfg.M, 2 + budget_step / per_prod)))
+    for _ in range(args.warmup):
+        oracle_time_terms(oracle, np, cfg, H, a, b, terms)
+    ts = [oracle_time_terms(oracle, np, cfg, H, a, b, terms) for _ in range(args.steps)]
+    per_prod = sum(ts) / len(ts) / (terms - 2)
+    t_solve = per_prod * (cfg.M - 2)
+    value = 1.0 / t_solve
+    sample = (f"{name} seed {cfg.seeds[0]} (N={cfg.N}, M={cfg.M}): each step = oracle.dm_cheb over the first {terms} of {cfg.M} terms "
+              f"({terms - 2} of {cfg.M - 2} naive products), solves/s extrapolated linearly in the number of products")
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": 1e3 * sum(ts) / len(ts), "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": f"{name}: {cfg.note}; beta={cfg.beta}, M={cfg.M} terms, N_occ={cfg.N_occ}", "N": cfg.N, "M_terms": cfg.M},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+    return 0
+
+
+# ---------------------------------------------------------------------------------------------------
+def main():
+    args = parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import torch
+    import paper_2306_12616_b200 as cd
+    import workloads
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (there is no CPU fallback; --impl reference times the CPU oracle)")
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist_mod
+        dist_mod.init_process_group(backend="nccl", device_id=torch.device("cuda", local))
+        dist = dist_mod
+    cd.lib()
+
+    sampler = ClockSampler(torch, local) if rank == 0 else None
+    flush = torch.empty(FLUSH_BYTES, dtype=torch.uint8, device="cuda")
+    st = torch.cuda.current_stream().cuda_stream
+    peak_tf = max(cd.dmma_peak(40000, st) for _ in range(3))
+
+    main_res = measure_workload(torch, cd, workloads, args.config, args, args.steps, args.warmup, flush, sampler, dist, peak_tf, world)
+    others = []
+    for name in [s for s in args.others.split(",") if s and s != args.config]:
+        big = workloads.CONFIGS[name].N >= 2000
+        k_steps = max(2, min(args.steps, 5 if big else 10))
+        others.append(measure_workload(torch, cd, workloads, name, args, k_steps, 3, flush, sampler, dist, peak_tf, world))
+    peak_after = cd.dmma_peak(40000, st)
+
+    if rank == 0:
+        clocks = sampler.summary() if sampler else None
+        try:
+            peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+        except Exception:
+            peaks = {}
+        cfg = workloads.CONFIGS[args.config]
+        line = {
+            "metric": METRIC, "value": main_res["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": main_res["ms_per_step"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic",
+            "config": {"workload": f"{args.config}: {cfg.note}; beta={cfg.beta}, M={cfg.M} terms, N_occ={cfg.N_occ}, seeds {list(cfg.seeds)}; "
+                                   "mu solved on the trace beforehand (device moments + bisection)",
+                       "N": cfg.N, "M_terms": cfg.M, "k": main_res["k"], "p": main_res["p"], "solves_per_step": main_res["solves_per_step"],
+                       "parallelism": "replicas only (one plan per GPU, no collective)" if world > 1 else "1 GPU",
+                       "l2": "flushed between timed steps (512 MiB device memset outside the event brackets)",
+                       "bounds": "Gershgorin on the device", "sched": "grouped persistent kernel" if args.sched == 0 else "serial launches"},
+            "ms_per_solve": main_res["ms_per_solve"], "tflops": main_res["tflops_step"],
+            "e2e": {k: main_res["e2e"][k] for k in ("value", "unit", "h2d_bytes_per_step", "d2h_bytes_per_step")},
+            "gpu_launches": main_res["gpu_launches_per_step"] * args.steps,
+            "roofline": dict(main_res["roofline"],
+                             peak_source="cheb_dm_dmma_peak: live register-resident DMMA.8x8x4 microbenchmark on this GPU (MEASURED_PEAKS.json has no FP64 entry)",
+                             peak_after_run=peak_after,
+                             peak_alt_bf16_ratio=(peaks.get("bf16_tflops") or 0) * 40.0 / 2250.0 or None),
+            "clocks": clocks,
+            "mu": main_res["mu"], "tr_D": main_res["tr_D"], "mu_search_ms": main_res["mu_search_ms"],
+            "other_workloads": others,
+        }
+        if not args.no_cpu_baseline and world == 1:
+            v, sample, cores, _ = oracle_rate(args.config, 15.0)
+            line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample}
+        print(json.dumps(line))
+    if dist is not None:
+        dist.barrier()
+        dist.destroy_process_group()
+    return 0
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -117,6 +117,14 @@ cheb_dm_status_t cheb_dm_coeffs(cheb_dm_plan_t plan, double beta, double mu, con
  * ESTATE if cheb_dm_coeffs() was never called; EINVAL on NULL/aliased pointers. */
 cheb_dm_status_t cheb_dm_compute(cheb_dm_plan_t plan, const double* dH, double* dD, void* cuda_stream);
 
+/* Host-buffer form of cheb_dm_compute (+ cheb_dm_trace): the end-to-end call a user without device
+ * memory makes.  hH, hD: HOST pointers, N*N doubles (ld N), pinned memory recommended; h_trace: HOST pointer
+ * to 1 double, or NULL.  On `cuda_stream`: copies H to a plan-owned device buffer, runs cheb_dm_compute,
+ * the trace kernel, copies D (and tr D) back and SYNCHRONISES the stream before returning, so hD is
+ * valid on return.  Same errors as cheb_dm_compute. */
+cheb_dm_status_t cheb_dm_compute_host(cheb_dm_plan_t plan, const double* hH, double* hD, double* h_trace,
+                                      void* cuda_stream);
+
 /* trace_out[0] <- tr D = sum_i D_ii (electron count, north_star item 4).  dD: device pointer (N*N,
  * ld N).  trace_out: DEVICE pointer (or pinned mapped host memory), 1 double, written
  * asynchronously on the stream in a fixed summation order (bitwise reproducible). */
@@ -171,6 +179,20 @@ cheb_dm_status_t cheb_dm_last_launch_count(cheb_dm_plan_t plan, int* launches_ou
 
 /* Executed FP64 tensor flops of one cheb_dm_compute() on this plan: 2*N^3 per product. */
 cheb_dm_status_t cheb_dm_flops_per_compute(cheb_dm_plan_t plan, double* flops_out);
+
+/* Measurement support (bench.py's roofline object).
+ * cheb_dm_set_timing(plan, 1): every following cheb_dm_compute() records a CUDA event on its stream
+ *   directly before and after the launch(es) of the product kernel (one launch in GROUPED mode).
+ *   The plan keeps a ring of 256 event pairs, so up to 256 computes can be in flight unsynchronised.
+ * cheb_dm_product_ms: waits for the recorded computes (the last min(count, 256) since timing was
+ *   switched on) and returns how many there were and the SUM of their product-launch durations in
+ *   milliseconds (host pointers).  ESTATE if timing is off or nothing ran.
+ * cheb_dm_dmma_peak: register-resident DMMA.8x8x4 issue-rate microbenchmark on all SMs (the FP64
+ *   tensor roofline of this device at its current clocks): `iters` dependent steps of 8 independent
+ *   accumulator chains per warp, 32 warps per SM; tflops_out: host pointer.  Synchronises the stream. */
+cheb_dm_status_t cheb_dm_set_timing(cheb_dm_plan_t plan, int enable);
+cheb_dm_status_t cheb_dm_product_ms(cheb_dm_plan_t plan, int* count_out, double* total_ms_out);
+cheb_dm_status_t cheb_dm_dmma_peak(int iters, double* tflops_out, void* cuda_stream);
 
 const char* cheb_dm_strerror(cheb_dm_status_t status);
 

@@ -17,6 +17,7 @@ EXPORTS = [
     "cheb_dm_trace", "cheb_dm_get_bounds", "cheb_dm_get_coeffs", "cheb_dm_get_kp", "cheb_dm_get_T",
     "cheb_dm_moments", "cheb_dm_solve_mu", "cheb_dm_product", "cheb_dm_workspace_bytes",
     "cheb_dm_last_launch_count", "cheb_dm_flops_per_compute", "cheb_dm_strerror",
+    "cheb_dm_compute_host", "cheb_dm_set_timing", "cheb_dm_product_ms", "cheb_dm_dmma_peak",
 ]
 
 
@@ -71,6 +72,10 @@ def lib():
     L.cheb_dm_workspace_bytes.argtypes = [vp, C.POINTER(C.c_size_t)]
     L.cheb_dm_last_launch_count.argtypes = [vp, ip]
     L.cheb_dm_flops_per_compute.argtypes = [vp, dp]
+    L.cheb_dm_compute_host.argtypes = [vp, vp, vp, vp, vp]
+    L.cheb_dm_set_timing.argtypes = [vp, C.c_int]
+    L.cheb_dm_product_ms.argtypes = [vp, ip, dp]
+    L.cheb_dm_dmma_peak.argtypes = [C.c_int, dp, vp]
     for n in EXPORTS:
         getattr(L, n).restype = C.c_int
     L.cheb_dm_strerror.argtypes = [C.c_int]
@@ -88,6 +93,13 @@ def _darr(a):
     import numpy as np
     a = np.ascontiguousarray(a, dtype=np.float64)
     return a, a.ctypes.data_as(C.POINTER(C.c_double))
+
+
+def dmma_peak(iters: int = 20000, stream: int = 0) -> float:
+    """FP64 tensor (DMMA.8x8x4) issue-rate peak of the current device in TFLOP/s (cheb_dm_dmma_peak)."""
+    v = C.c_double()
+    _chk(lib().cheb_dm_dmma_peak(iters, C.byref(v), stream), "cheb_dm_dmma_peak")
+    return v.value
 
 
 class Plan:
@@ -124,6 +136,18 @@ class Plan:
 
     def compute(self, dH: int, dD: int, stream: int = 0):
         _chk(lib().cheb_dm_compute(self._h, dH, dD, stream), "cheb_dm_compute")
+
+    def compute_host(self, hH: int, hD: int, h_trace: int = 0, stream: int = 0):
+        """hH, hD, h_trace: HOST addresses (e.g. of pinned torch tensors / numpy arrays)."""
+        _chk(lib().cheb_dm_compute_host(self._h, hH, hD, h_trace or None, stream), "cheb_dm_compute_host")
+
+    def set_timing(self, enable: bool):
+        _chk(lib().cheb_dm_set_timing(self._h, int(bool(enable))), "cheb_dm_set_timing")
+
+    def last_product_ms(self) -> float:
+        v = C.c_float()
+        _chk(lib().cheb_dm_last_product_ms(self._h, C.byref(v)), "cheb_dm_product_ms")
+        return v.value
 
     def trace(self, dD: int, d_out: int, stream: int = 0):
         _chk(lib().cheb_dm_trace(self._h, dD, d_out, stream), "cheb_dm_trace")

@@ -422,4 +422,24 @@ __global__ void __launch_bounds__(1024) mu_bisect_kernel(DevScalars* sc, double 
     }
 }
 
+// ---------------------------------------------------------------------------------------------------
+// Roofline denominator: register-resident DMMA.8x8x4 issue-rate microbenchmark (cheb_dm_dmma_peak).
+// Each warp runs DMMA_PEAK_CHAINS independent accumulator chains; no memory traffic in the loop.
+// ---------------------------------------------------------------------------------------------------
+constexpr int DMMA_PEAK_CHAINS = 8;
+__global__ void __launch_bounds__(512) dmma_peak_kernel(int iters, double* sink) {
+    double c[DMMA_PEAK_CHAINS][2];
+#pragma unroll
+    for (int i = 0; i < DMMA_PEAK_CHAINS; ++i) c[i][0] = c[i][1] = 0.0;
+    const double a = 1.0 + 1e-9 * threadIdx.x, b = 1.0 - 1e-9 * threadIdx.x;
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int i = 0; i < DMMA_PEAK_CHAINS; ++i) dmma_884(c[i][0], c[i][1], a, b);
+    }
+    double s = 0.0;
+#pragma unroll
+    for (int i = 0; i < DMMA_PEAK_CHAINS; ++i) s += c[i][0] + c[i][1];
+    if (s == 123.456) sink[threadIdx.x & 63] = s;  // keeps the chains alive
+}
+
 }  // namespace chebdm

@@ -48,6 +48,8 @@ struct HostTaskMeta {
 
 }  // namespace
 
+enum { TIMING_SLOTS = 256 };
+
 struct cheb_dm_plan_s {
     int N, M, k, p, Nq;
     cheb_dm_options_t opt;
@@ -83,6 +85,12 @@ struct cheb_dm_plan_s {
     int last_launches;
     double flops_per_compute;
     size_t ws_bytes;
+    // host-buffer entry point (cheb_dm_compute_host): device staging for H, D and tr D
+    double *stage_H, *stage_D, *stage_tr;
+    // optional timing of the product launches (cheb_dm_set_timing)
+    int timing;
+    cudaEvent_t ev0[TIMING_SLOTS], ev1[TIMING_SLOTS];  // ring: compute number i uses slot i % TIMING_SLOTS
+    long long ev_count;                                // computes recorded since cheb_dm_set_timing(plan, 1)
 };
 
 namespace {
@@ -464,6 +472,13 @@ cheb_dm_status_t cheb_dm_destroy(cheb_dm_plan_t P) {
     cudaFree(P->tasks);
     cudaFree(P->task_first);
     cudaFree(P->counters);
+    cudaFree(P->stage_H);
+    cudaFree(P->stage_D);
+    cudaFree(P->stage_tr);
+    for (int i = 0; i < TIMING_SLOTS; ++i) {
+        if (P->ev0[i]) cudaEventDestroy(P->ev0[i]);
+        if (P->ev1[i]) cudaEventDestroy(P->ev1[i]);
+    }
     delete P;
     return CHEB_DM_OK;
 }
@@ -515,6 +530,9 @@ cheb_dm_status_t cheb_dm_plan_ex(cheb_dm_plan_t* plan, int N, int M_terms, cheb_
     P->sc = nullptr; P->maps = nullptr; P->tasks = nullptr; P->task_first = nullptr; P->counters = nullptr;
     P->have_coeffs = P->explicit_bounds = P->have_moments = P->computed = 0;
     P->last_launches = 0;
+    P->stage_H = P->stage_D = P->stage_tr = nullptr;
+    P->timing = 0; P->ev_count = 0;
+    for (int i = 0; i < TIMING_SLOTS; ++i) P->ev0[i] = P->ev1[i] = nullptr;
 
     const int tiles = ceil_div(N, P->BM) * ceil_div(N, P->BN);
     const size_t kp = (size_t)k * p;
@@ -532,12 +550,17 @@ cheb_dm_status_t cheb_dm_plan_ex(cheb_dm_plan_t* plan, int N, int M_terms, cheb_
     ok = ok && cudaMalloc(&P->dots, sizeof(double) * ((size_t)(p + 1) * tiles * k + (size_t)2 * k * 16)) == cudaSuccess;
     ok = ok && cudaMalloc(&P->sc, sizeof(DevScalars)) == cudaSuccess;
     ok = ok && cudaMalloc(&P->maps, sizeof(CUtensorMap) * P->nmat) == cudaSuccess;
+    ok = ok && cudaMalloc(&P->stage_H, sizeof(double) * (size_t)N * N) == cudaSuccess;
+    ok = ok && cudaMalloc(&P->stage_D, sizeof(double) * (size_t)N * N) == cudaSuccess;
+    ok = ok && cudaMalloc(&P->stage_tr, sizeof(double)) == cudaSuccess;
+    for (int i = 0; i < TIMING_SLOTS && ok; ++i)
+        ok = cudaEventCreate(&P->ev0[i]) == cudaSuccess && cudaEventCreate(&P->ev1[i]) == cudaSuccess;
     if (!ok) {
         cudaGetLastError();
         cheb_dm_destroy(P);
         return CHEB_DM_EALLOC;
     }
-    P->ws_bytes += sizeof(double) * (4 * (size_t)nq + 2 * nq + 4 * kp + (size_t)p * p + (size_t)(p + 1) * tiles * k);
+    P->ws_bytes += sizeof(double) * (2 * (size_t)N * N + 4 * (size_t)nq + 2 * nq + 4 * kp + (size_t)p * p + (size_t)(p + 1) * tiles * k);
 
     cheb_dm_status_t st = CHEB_DM_OK;
     do {
@@ -706,9 +729,88 @@ cheb_dm_status_t cheb_dm_compute(cheb_dm_plan_t P, const double* dH, double* dD,
     if (s != CHEB_DM_OK) return s;
     s = front_end(P, dH, st);
     if (s != CHEB_DM_OK) return s;
+    const int slot = (int)(P->ev_count % TIMING_SLOTS);
+    if (P->timing) CUDA_TRY(cudaEventRecord(P->ev0[slot], st));
     s = run_tasks(P, 0, P->ntasks_solve, dD, P->N, st);
     if (s != CHEB_DM_OK) return s;
+    if (P->timing) {
+        CUDA_TRY(cudaEventRecord(P->ev1[slot], st));
+        ++P->ev_count;
+    }
     P->computed = 1;
+    return CHEB_DM_OK;
+}
+
+cheb_dm_status_t cheb_dm_compute_host(cheb_dm_plan_t P, const double* hH, double* hD, double* h_trace, void* cuda_stream) {
+    if (!P || !hH || !hD || hH == hD) return CHEB_DM_EINVAL;
+    if (!P->have_coeffs) return CHEB_DM_ESTATE;
+    if (!device_ok(P)) return CHEB_DM_ECUDA;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const size_t bytes = sizeof(double) * (size_t)P->N * P->N;
+    CUDA_TRY(cudaMemcpyAsync(P->stage_H, hH, bytes, cudaMemcpyHostToDevice, st));
+    cheb_dm_status_t s = cheb_dm_compute(P, P->stage_H, P->stage_D, cuda_stream);
+    if (s != CHEB_DM_OK) return s;
+    if (h_trace) {
+        trace_kernel<<<1, 1024, 0, st>>>(P->stage_D, P->N, P->N, P->stage_tr);
+        ++P->last_launches;
+        CUDA_TRY(cudaGetLastError());
+        CUDA_TRY(cudaMemcpyAsync(h_trace, P->stage_tr, sizeof(double), cudaMemcpyDeviceToHost, st));
+    }
+    CUDA_TRY(cudaMemcpyAsync(hD, P->stage_D, bytes, cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(cudaStreamSynchronize(st));
+    return CHEB_DM_OK;
+}
+
+cheb_dm_status_t cheb_dm_set_timing(cheb_dm_plan_t P, int enable) {
+    if (!P) return CHEB_DM_EINVAL;
+    P->timing = enable ? 1 : 0;
+    P->ev_count = 0;
+    return CHEB_DM_OK;
+}
+
+cheb_dm_status_t cheb_dm_product_ms(cheb_dm_plan_t P, int* count_out, double* total_ms_out) {
+    if (!P || !count_out || !total_ms_out) return CHEB_DM_EINVAL;
+    if (!P->timing || P->ev_count < 1) return CHEB_DM_ESTATE;
+    const int n = (int)(P->ev_count < TIMING_SLOTS ? P->ev_count : TIMING_SLOTS);
+    double total = 0.0;
+    for (int i = 0; i < n; ++i) {
+        const int slot = (int)((P->ev_count - 1 - i) % TIMING_SLOTS);
+        CUDA_TRY(cudaEventSynchronize(P->ev1[slot]));
+        float ms = 0.f;
+        CUDA_TRY(cudaEventElapsedTime(&ms, P->ev0[slot], P->ev1[slot]));
+        total += ms;
+    }
+    *count_out = n;
+    *total_ms_out = total;
+    return CHEB_DM_OK;
+}
+
+cheb_dm_status_t cheb_dm_dmma_peak(int iters, double* tflops_out, void* cuda_stream) {
+    if (!tflops_out || iters < 1) return CHEB_DM_EINVAL;
+    int dev = 0, ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) return CHEB_DM_ECUDA;
+    CUDA_TRY(cudaGetDevice(&dev));
+    cudaDeviceProp prop;
+    CUDA_TRY(cudaGetDeviceProperties(&prop, dev));
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    double* sink = nullptr;
+    CUDA_TRY(cudaMalloc(&sink, sizeof(double) * 64));
+    cudaEvent_t e0, e1;
+    CUDA_TRY(cudaEventCreate(&e0));
+    CUDA_TRY(cudaEventCreate(&e1));
+    const int blocks = prop.multiProcessorCount * 2, threads = 512;
+    dmma_peak_kernel<<<blocks, threads, 0, st>>>(iters / 8 + 1, sink);  // warm-up
+    CUDA_TRY(cudaEventRecord(e0, st));
+    dmma_peak_kernel<<<blocks, threads, 0, st>>>(iters, sink);
+    CUDA_TRY(cudaEventRecord(e1, st));
+    CUDA_TRY(cudaEventSynchronize(e1));
+    float ms = 0.f;
+    CUDA_TRY(cudaEventElapsedTime(&ms, e0, e1));
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    cudaFree(sink);
+    const double flops = (double)blocks * (threads / 32) * (double)iters * DMMA_PEAK_CHAINS * 512.0;
+    *tflops_out = flops / ((double)ms * 1e-3) * 1e-12;
     return CHEB_DM_OK;
 }
 

@@ -1,0 +1,328 @@
+"""`-m gpu` parity tests: the CUDA path, called through the C ABI (include/cheb_dm.h via the ctypes
+binding), against the CPU oracle on the same seeded inputs.
+
+Gates (BASELINE.json north_star):
+    max|D_gpu - D_cheb| <= 1e-10,  |tr D_gpu - tr D_cheb| <= 1e-9,
+    max|D_gpu - D_eig|  <= eps_trunc(config) + 1e-9  (eps_trunc from oracle scalars).
+Every expected value comes from oracle/ (tests/oracle_cases.py); nothing flows from the GPU into it.
+"""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+TOL_D = 1e-10
+TOL_TR = 1e-9
+
+
+def _imports():
+    import oracle
+    import paper_2306_12616_b200 as cd
+    import workloads
+    from tests import gpu_util, oracle_cases
+    return oracle, cd, workloads, gpu_util, oracle_cases
+
+
+# ----------------------------------------------------------------------------------------------
+# a-4/a-6 kernel: one product with the fused 2AB - C epilogue (Eq. 7), all tile shapes, ragged sizes
+# ----------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("tile", [1, 2, 3])
+@pytest.mark.parametrize("N", [1, 2, 7, 64, 65, 130, 200, 333])
+def test_product_2AB_minus_C(N, tile):
+    oracle, cd, workloads, gu, _ = _imports()
+    torch = gu.torch_cuda()
+    A = workloads.random_symmetric(N, seed=10 + N)
+    B = workloads.random_symmetric(N, seed=20 + N)
+    Cm = workloads.random_symmetric(N, seed=30 + N)
+    expect = 2.0 * oracle.matmul(A, B) - Cm
+    plan = cd.Plan(N, 4, tile=tile)
+    dA, dB, dC = gu.to_dev(A), gu.to_dev(B), gu.to_dev(Cm)
+    dO = torch.full((N, N), float("nan"), dtype=torch.float64, device="cuda")
+    plan.product(2.0, dA.data_ptr(), dB.data_ptr(), -1.0, dC.data_ptr(), dO.data_ptr(),
+                 torch.cuda.current_stream().cuda_stream)
+    torch.cuda.synchronize()
+    got = dO.cpu().numpy()
+    # |entries| <= 1, N-term dot products: rounding <= ~N * 2^-52 each side
+    assert np.max(np.abs(got - expect)) <= 4.0 * N * 2.0 ** -52 + 1e-15
+    plan.destroy()
+
+
+# ----------------------------------------------------------------------------------------------
+# a-1: Gershgorin bounds + rescale
+# ----------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("cfg,n", [("cfg0", 128), ("cfg1", 301), ("cfg2", 200), ("cfg3", 500), ("cfg4", 130)])
+def test_gershgorin_bounds_and_rescale(cfg, n):
+    oracle, cd, workloads, gu, _ = _imports()
+    torch = gu.torch_cuda()
+    H = workloads.hamiltonian(cfg, seed=0, n=n)
+    a, b = oracle.gershgorin(H)
+    r = gu.gpu_solve(H, 5.0, 0.0, 8, keep_plan=True)
+    ga, gb = r["bounds"]
+    scale = max(abs(a), abs(b))
+    assert abs(ga - a) <= n * 2.0 ** -52 * scale and abs(gb - b) <= n * 2.0 ** -52 * scale
+    # T_1 = X = (2H - (a+b)I)/(b-a)  (reading A1), with the GPU's own bounds
+    dX = torch.empty((n, n), dtype=torch.float64, device="cuda")
+    r["plan"].get_T(1, dX.data_ptr(), torch.cuda.current_stream().cuda_stream)
+    X = oracle.scale(H, a, b)
+    assert np.max(np.abs(dX.cpu().numpy() - X)) <= 1e-14
+    r["plan"].destroy()
+
+
+def test_gershgorin_degenerate_identity_widens():
+    _, cd, _, gu, _ = _imports()
+    H = 3.0 * np.eye(40)
+    r = gu.gpu_solve(H, 2.0, 3.0, 6)
+    assert r["bounds"] == (2.0, 4.0)
+    # X = 0 => D = p_M(0) I ~ f(mu) I = 0.5 I up to truncation
+    assert np.max(np.abs(r["D"] - np.diag(np.diag(r["D"])))) == 0.0
+
+
+# ----------------------------------------------------------------------------------------------
+# a-2 / a-3: coefficient tables computed on the device
+# ----------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("M,k,p", [(64, 0, 0), (256, 0, 0), (2048, 0, 0), (1024, 0, 0), (30, 5, 7), (7, 7, 1), (5, 1, 5)])
+def test_coefficient_tables(M, k, p):
+    oracle, cd, workloads, gu, _ = _imports()
+    H = workloads.hamiltonian("cfg1", seed=1, n=48)
+    beta, mu, bounds = 40.0, 0.07, (-20.0, 21.0)
+    outer = cd.OUTER_POWER if M <= 64 else cd.OUTER_CHEBYSHEV
+    r = gu.gpu_solve(H, beta, mu, M, bounds=bounds, keep_plan=True, k=k, p=p, outer=outer)
+    plan = r["plan"]
+    c, g, d = plan.get_coeffs()
+    kk, pp = plan.k, plan.p
+    c_or = oracle.pad_coeffs(oracle.cheb_coeffs(beta, mu, bounds[0], bounds[1], M), kk, pp)
+    assert np.max(np.abs(c - c_or)) <= 2e-15
+    g_or = oracle.g_from_c(kk, pp, c_or)
+    assert np.max(np.abs(g - g_or)) <= 1e-14
+    if outer == cd.OUTER_POWER:
+        d_or = oracle.d_from_g(kk, pp, g_or)
+        assert np.max(np.abs(d - d_or)) <= 1e-13 * max(1.0, np.max(np.abs(d_or)))
+    plan.destroy()
+
+
+# ----------------------------------------------------------------------------------------------
+# a-4: baby steps T_2..T_k (Eq. 7, 22-23, Algorithm 1) vs the three-term recurrence of the oracle
+# ----------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("pairing", [0, 1])
+@pytest.mark.parametrize("k", [2, 3, 5, 8, 11])
+def test_baby_steps_match_three_term_recurrence(k, pairing):
+    oracle, cd, workloads, gu, _ = _imports()
+    torch = gu.torch_cuda()
+    n = 150
+    H = workloads.hamiltonian("cfg1", seed=2, n=n)
+    a, b = oracle.gershgorin(H)
+    r = gu.gpu_solve(H, 10.0, 0.0, k * 3, bounds=(a, b), keep_plan=True, k=k, p=3, pairing=pairing)
+    X = oracle.scale(H, a, b)
+    Tm, Tc = np.eye(n), X
+    dT = torch.empty((n, n), dtype=torch.float64, device="cuda")
+    for j in range(2, k + 1):
+        Tn = 2.0 * oracle.matmul(X, Tc) - Tm
+        Tm, Tc = Tc, Tn
+        r["plan"].get_T(j, dT.data_ptr(), torch.cuda.current_stream().cuda_stream)
+        assert np.max(np.abs(dT.cpu().numpy() - Tc)) <= 1e-13, j
+    r["plan"].destroy()
+
+
+# ----------------------------------------------------------------------------------------------
+# whole path at reduced sizes (several tiles + ragged tail), every config kind
+# ----------------------------------------------------------------------------------------------
+SMALL = [("cfg0", 0, 128, None), ("cfg1", 0, 300, None), ("cfg1", 3, 257, None), ("cfg2", 0, 250, None),
+         ("cfg3", 0, 200, 1024), ("cfg4", 0, 200, 2048)]
+
+
+def _check(case, r):
+    dD = np.max(np.abs(r["D"] - case["D_cheb"]))
+    dtr = abs(r["trace"] - float(np.trace(case["D_cheb"])))
+    assert dD <= TOL_D, dD
+    assert dtr <= TOL_TR, dtr
+    assert abs(float(np.trace(case["D_cheb"])) - case["nocc"]) <= 1e-7  # mu solved on the trace
+    if "D_eig" in case:
+        assert np.max(np.abs(r["D"] - case["D_eig"])) <= case["eps_trunc"] + 1e-9
+    assert np.max(np.abs(r["D"] - r["D"].T)) <= 1e-11
+    return dD, dtr
+
+
+@pytest.mark.parametrize("cfg,seed,n,M", SMALL)
+def test_parity_reduced_size_device_gershgorin(cfg, seed, n, M):
+    """The hot path as bench.py runs it: bounds=None (Gershgorin on the device)."""
+    oracle, cd, workloads, gu, oc = _imports()
+    case = oc.case(cfg, seed, n, M)
+    r = gu.gpu_solve(case["H"], case["beta"], case["mu"], case["M"])
+    assert abs(r["bounds"][0] - case["a"]) <= n * 2.0 ** -52 * abs(case["a"])
+    assert abs(r["bounds"][1] - case["b"]) <= n * 2.0 ** -52 * abs(case["b"])
+    _check(case, r)
+
+
+@pytest.mark.parametrize("tile", [1, 2, 3])
+@pytest.mark.parametrize("sched", [0, 1])
+def test_parity_tiles_and_schedulers(tile, sched):
+    oracle, cd, workloads, gu, oc = _imports()
+    case = oc.case("cfg1", 0, 300, None)
+    r = gu.gpu_solve(case["H"], case["beta"], case["mu"], case["M"], bounds=(case["a"], case["b"]), tile=tile, sched=sched)
+    _check(case, r)
+
+
+def test_parity_power_outer_recursion_eq4():
+    """Eq. 4 literally (S_j + T_k acc), stable when the expansion is short (reading A6)."""
+    oracle, cd, workloads, gu, oc = _imports()
+    case = oc.case("cfg0", 0, 128, None)
+    r = gu.gpu_solve(case["H"], case["beta"], case["mu"], case["M"], bounds=(case["a"], case["b"]), outer=cd.OUTER_POWER)
+    _check(case, r)
+
+
+def test_parity_serial_pairing_and_nonsquare_kp():
+    oracle, cd, workloads, gu, oc = _imports()
+    case = oc.case("cfg2", 0, 250, None)
+    for kw in (dict(pairing=1), dict(k=32, p=8), dict(k=8, p=32), dict(k=20, p=13), dict(k=256, p=1), dict(k=1, p=256)):
+        r = gu.gpu_solve(case["H"], case["beta"], case["mu"], case["M"], bounds=(case["a"], case["b"]), **kw)
+        _check(case, r)
+
+
+def test_converged_variant_meets_1e6_vs_diagonalisation():
+    """North-star's "<= 1e-6 vs the diagonalisation DM": holds with tight bounds and enough terms
+    (SURVEY A2-iii); with Gershgorin bounds the configs' M are far from converged."""
+    oracle, cd, workloads, gu, oc = _imports()
+    case = oc.case("cfg1", 0, 300, 512, True, "tight")
+    assert case["eps_trunc"] <= 1e-6
+    r = gu.gpu_solve(case["H"], case["beta"], case["mu"], case["M"], bounds=(case["a"], case["b"]))
+    _check(case, r)
+    assert np.max(np.abs(r["D"] - case["D_eig"])) <= 1e-6
+
+
+# ----------------------------------------------------------------------------------------------
+# edge cases
+# ----------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("N,M", [(1, 1), (1, 9), (2, 2), (3, 1), (5, 3), (17, 2), (63, 10), (129, 25)])
+def test_edge_sizes(N, M):
+    oracle, cd, workloads, gu, _ = _imports()
+    H = workloads.random_symmetric(N, seed=N * 100 + M, scale=2.0)
+    a, b = oracle.gershgorin(H)
+    if a == b:
+        a, b = a - 1.0, b + 1.0
+    beta, mu = 3.0, 0.1
+    c = oracle.cheb_coeffs(beta, mu, a, b, M)
+    D = oracle.dm_cheb(H, a, b, c)
+    r = gu.gpu_solve(H, beta, mu, M)
+    assert np.max(np.abs(r["D"] - D)) <= TOL_D
+    assert abs(r["trace"] - np.trace(D)) <= TOL_TR
+
+
+def test_diagonal_H_gives_scalar_polynomial_on_diagonal():
+    oracle, cd, workloads, gu, _ = _imports()
+    eps = np.linspace(-1.7, 2.3, 70)
+    H = np.diag(eps)
+    beta, mu, M = 6.0, 0.2, 48
+    r = gu.gpu_solve(H, beta, mu, M)
+    a, b = r["bounds"]
+    assert (a, b) == (eps[0], eps[-1])  # Gershgorin is exact for diagonal H (pin P9)
+    c = oracle.cheb_coeffs(beta, mu, a, b, M)
+    want = np.array([oracle.eval_cheb_sum(c, float((2 * e - (a + b)) / (b - a))) for e in eps])
+    assert np.max(np.abs(np.diag(r["D"]) - want)) <= 1e-13
+    assert np.max(np.abs(r["D"] - np.diag(np.diag(r["D"])))) <= 1e-15
+
+
+def test_bitwise_reproducible():
+    oracle, cd, workloads, gu, oc = _imports()
+    H = workloads.hamiltonian("cfg1", seed=1, n=300)
+    r1 = gu.gpu_solve(H, 40.0, 0.01, 256)
+    r2 = gu.gpu_solve(H, 40.0, 0.01, 256)
+    assert np.array_equal(r1["D"], r2["D"]) and r1["trace"] == r2["trace"]
+
+
+def test_plan_reuse_with_new_mu_and_new_H():
+    oracle, cd, workloads, gu, oc = _imports()
+    torch = gu.torch_cuda()
+    n, M = 180, 100
+    plan = cd.Plan(n, M)
+    st = torch.cuda.current_stream().cuda_stream
+    dD = torch.empty((n, n), dtype=torch.float64, device="cuda")
+    for seed, mu in ((0, -0.2), (1, 0.3), (0, 0.05)):
+        H = workloads.hamiltonian("cfg1", seed=seed, n=n)
+        a, b = oracle.gershgorin(H)
+        dH = gu.to_dev(H)
+        plan.coeffs(25.0, mu, (a, b))
+        plan.compute(dH.data_ptr(), dD.data_ptr(), st)
+        torch.cuda.synchronize()
+        D = oracle.dm_cheb(H, a, b, oracle.cheb_coeffs(25.0, mu, a, b, M))
+        assert np.max(np.abs(dD.cpu().numpy() - D)) <= TOL_D
+    plan.destroy()
+
+
+def test_status_codes():
+    oracle, cd, workloads, gu, _ = _imports()
+    torch = gu.torch_cuda()
+    import ctypes as C
+    L = cd.lib()
+    h = C.c_void_p()
+    assert L.cheb_dm_plan(C.byref(h), 0, 4, 0) == 1          # EINVAL
+    assert L.cheb_dm_plan(C.byref(h), 8, 0, 0) == 1
+    assert L.cheb_dm_plan(C.byref(h), 8, 4, 7) == 6          # EUNSUPPORTED
+    o = cd.Options(k=2, p=1)
+    assert L.cheb_dm_plan_ex(C.byref(h), 8, 4, 0, C.byref(o)) == 1  # k*p < M
+    assert L.cheb_dm_plan(C.byref(h), 8, 4, 0) == 0
+    d = torch.zeros((8, 8), dtype=torch.float64, device="cuda")
+    e = torch.zeros((8, 8), dtype=torch.float64, device="cuda")
+    assert L.cheb_dm_compute(h, d.data_ptr(), e.data_ptr(), None) == 4   # ESTATE: no coeffs yet
+    bad = (C.c_double * 2)(1.0, 1.0)
+    assert L.cheb_dm_coeffs(h, 1.0, 0.0, bad) == 5           # EBOUNDS
+    assert L.cheb_dm_coeffs(h, -1.0, 0.0, None) == 1
+    assert L.cheb_dm_coeffs(h, float("nan"), 0.0, None) == 1
+    assert L.cheb_dm_coeffs(h, 1.0, 0.0, None) == 0
+    assert L.cheb_dm_compute(h, d.data_ptr(), d.data_ptr(), None) == 1   # aliasing
+    assert L.cheb_dm_compute(h, None, e.data_ptr(), None) == 1
+    mu = C.c_double()
+    assert L.cheb_dm_solve_mu(h, 1.0, 4.0, 50, C.byref(mu), None) == 4   # ESTATE: no moments
+    assert L.cheb_dm_destroy(h) == 0
+    # non-finite H under Gershgorin -> EBOUNDS on read-back
+    plan = cd.Plan(8, 4)
+    Hn = np.eye(8)
+    Hn[2, 3] = Hn[3, 2] = np.inf
+    dH = gu.to_dev(Hn)
+    plan.coeffs(1.0, 0.0, None)
+    plan.compute(dH.data_ptr(), e.data_ptr(), torch.cuda.current_stream().cuda_stream)
+    with pytest.raises(cd.ChebDMError) as ei:
+        plan.get_bounds()
+    assert ei.value.status == 5
+    plan.destroy()
+
+
+# ----------------------------------------------------------------------------------------------
+# a-7: trace, moments, mu
+# ----------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("cfg,n,M,kp", [("cfg0", 128, 64, (0, 0)), ("cfg1", 200, 256, (0, 0)), ("cfg2", 150, 60, (6, 10)),
+                                         ("cfg4", 130, 90, (9, 10)), ("cfg1", 64, 12, (12, 1)), ("cfg1", 64, 12, (3, 4))])
+def test_moments_and_mu(cfg, n, M, kp):
+    oracle, cd, workloads, gu, oc = _imports()
+    torch = gu.torch_cuda()
+    H = workloads.hamiltonian(cfg, seed=0, n=n)
+    beta = workloads.CONFIGS[cfg].beta
+    nocc = workloads.n_occ(cfg, n)
+    a, b = oracle.gershgorin(H)
+    _, tau_or = oracle.dm_cheb(H, a, b, np.zeros(M), want_tau=True)
+    plan = cd.Plan(n, M, k=kp[0], p=kp[1])
+    dH = gu.to_dev(H)
+    st = torch.cuda.current_stream().cuda_stream
+    plan.coeffs(beta, 0.0, (a, b))
+    tau = plan.moments(dH.data_ptr(), True, st)[:M]
+    assert np.max(np.abs(tau - tau_or)) <= 1e-10 * n
+    mu_gpu = plan.solve_mu(beta, nocc, 100, st)
+    mu_or = oracle.solve_mu(tau_or, beta, a, b, nocc, iters=100)
+    # the electron count at the GPU's mu must hit the target as well as the oracle's own root does
+    ne_gpu = oracle.electron_count(tau_or, beta, mu_gpu, a, b)
+    ne_or = oracle.electron_count(tau_or, beta, mu_or, a, b)
+    assert abs(ne_gpu - nocc) <= max(1e-8, 10 * abs(ne_or - nocc))
+    plan.destroy()
+
+
+def test_trace_kernel():
+    oracle, cd, workloads, gu, _ = _imports()
+    torch = gu.torch_cuda()
+    for n in (1, 33, 500, 1025):
+        A = workloads.random_symmetric(n, seed=n)
+        plan = cd.Plan(n, 4)
+        dA = gu.to_dev(A)
+        out = torch.zeros(1, dtype=torch.float64, device="cuda")
+        plan.trace(dA.data_ptr(), out.data_ptr(), torch.cuda.current_stream().cuda_stream)
+        torch.cuda.synchronize()
+        assert abs(out.item() - float(np.sum(np.diag(A).astype(np.longdouble)))) <= 1e-13 * n
+        plan.destroy()
