@@ -144,10 +144,11 @@ class Plan:
     def set_timing(self, enable: bool):
         _chk(lib().cheb_dm_set_timing(self._h, int(bool(enable))), "cheb_dm_set_timing")
 
-    def last_product_ms(self) -> float:
-        v = C.c_float()
-        _chk(lib().cheb_dm_last_product_ms(self._h, C.byref(v)), "cheb_dm_product_ms")
-        return v.value
+    def product_ms(self):
+        """(count, total_ms) of the product-kernel launches recorded since set_timing(True)."""
+        n, v = C.c_int(), C.c_double()
+        _chk(lib().cheb_dm_product_ms(self._h, C.byref(n), C.byref(v)), "cheb_dm_product_ms")
+        return n.value, v.value
 
     def trace(self, dD: int, d_out: int, stream: int = 0):
         _chk(lib().cheb_dm_trace(self._h, dD, d_out, stream), "cheb_dm_trace")

@@ -16,7 +16,8 @@ FULL = [("cfg1", 0), ("cfg1", 1), ("cfg1", 2), ("cfg1", 3), ("cfg2", 0), ("cfg4"
 @pytest.mark.parametrize("cfg,seed", FULL)
 def test_full_size_sampled_columns(cfg, seed):
     import oracle
-    from tests import gpu_util as gu, oracle_cases as oc
+    import gpu_util as gu
+    import oracle_cases as oc
     case = oc.case(cfg, seed, None, None, False)
     N, M = case["N"], case["M"]
     r = gu.gpu_solve(case["H"], case["beta"], case["mu"], M)

@@ -19,7 +19,8 @@ def _imports():
     import oracle
     import paper_2306_12616_b200 as cd
     import workloads
-    from tests import gpu_util, oracle_cases
+    import gpu_util
+    import oracle_cases
     return oracle, cd, workloads, gpu_util, oracle_cases
 
 
