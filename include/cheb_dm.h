@@ -82,9 +82,12 @@ typedef struct {
     int sched;   /* cheb_dm_sched_t                                                              */
     int pairing; /* cheb_dm_pairing_t                                                            */
     int tile;    /* CTA tile: 0 = auto, 1 = 128x128, 2 = 128x64, 3 = 64x64                         */
-    int fuse_sums; /* 1 (default when 0 passed via cheb_dm_plan): low-order sums G_l / S_j are
-                      formed inside the giant-step epilogues; 2: formed by separate (bandwidth-
-                      bound) passes before the giant steps -- ablation of PAPER.md:234           */
+    int fuse_sums; /* low-order sums G_l / S_j of Eq. (21).  0 = auto; 1 = formed inside the
+                      giant-step epilogues from T_1..T_{k-1} (no extra workspace; p(k-1) N^2 8 bytes of reads per
+                      solve, L2 hits while the baby block fits L2); 2 = all p sums formed in one batched pass
+                      (form_sums_kernel: each T_i read ceil(p/16) times, p extra workspace matrices), the
+                      epilogues then add one tile.  auto = 2 when k N^2 8 B > 96 MiB.  Neither mode makes the
+                      per-term AXPY passes of PAPER.md:234.                                              */
     int reserved[9];
 } cheb_dm_options_t;
 

@@ -423,6 +423,69 @@ __global__ void __launch_bounds__(1024) mu_bisect_kernel(DevScalars* sc, double 
 }
 
 // ---------------------------------------------------------------------------------------------------
+// a-5, batched form (SURVEY 8(a) option ii; Eq. 21): all low-order sums at once,
+//     G_l = coefT[l][0] I + sum_{i=1}^{k-1} coefT[l][i] T_i,   l < p   (coefT = g or d, layout [l*k + i]),
+// reading every T_i once per chunk of SUMS_CHUNK outputs instead of once per giant step: HBM bytes
+// (ceil(p/SUMS_CHUNK) (k-1) + p) mat instead of p (k-1) mat for the epilogue-fused form.  One thread owns
+// one 16-byte element pair of the padded matrices (pad columns are zero in every T_i, so they stay zero).
+//   grid = (ceil(pairs / 256), ceil(p / SUMS_CHUNK)), block = 256.
+// ---------------------------------------------------------------------------------------------------
+constexpr int SUMS_CHUNK = 16;
+__global__ void __launch_bounds__(256) form_sums_kernel(const double* __restrict__ Tbase, long long stride, long long ld, int N, int k,
+                                                        int p, const double* __restrict__ coefT, double* __restrict__ Gbase) {
+    extern __shared__ double s_coef[];  // [k][SUMS_CHUNK]
+    const int l0 = blockIdx.y * SUMS_CHUNK;
+    const int nl = min(SUMS_CHUNK, p - l0);
+    for (int e = threadIdx.x; e < k * SUMS_CHUNK; e += blockDim.x) {
+        const int i = e / SUMS_CHUNK, q = e - i * SUMS_CHUNK;
+        s_coef[e] = (q < nl) ? coefT[(size_t)(l0 + q) * k + i] : 0.0;
+    }
+    __syncthreads();
+    const long long pairs = (long long)N * ld / 2;
+    const long long pr = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (pr >= pairs) return;
+    const long long e0 = 2 * pr;
+    const int row = (int)(e0 / ld), col = (int)(e0 - (long long)row * ld);
+    double2 acc[SUMS_CHUNK];
+#pragma unroll
+    for (int q = 0; q < SUMS_CHUNK; ++q) acc[q] = make_double2(0.0, 0.0);
+    const double* src = Tbase + e0;
+    int i = 1;
+    for (; i + 3 < k; i += 4) {
+        double2 v[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) v[u] = __ldcs(reinterpret_cast<const double2*>(src + (long long)(i - 1 + u) * stride));
+#pragma unroll
+        for (int u = 0; u < 4; ++u)
+#pragma unroll
+            for (int q = 0; q < SUMS_CHUNK; ++q) {
+                const double w = s_coef[(i + u) * SUMS_CHUNK + q];
+                acc[q].x = fma(w, v[u].x, acc[q].x);
+                acc[q].y = fma(w, v[u].y, acc[q].y);
+            }
+    }
+    for (; i < k; ++i) {
+        const double2 v = __ldcs(reinterpret_cast<const double2*>(src + (long long)(i - 1) * stride));
+#pragma unroll
+        for (int q = 0; q < SUMS_CHUNK; ++q) {
+            const double w = s_coef[i * SUMS_CHUNK + q];
+            acc[q].x = fma(w, v.x, acc[q].x);
+            acc[q].y = fma(w, v.y, acc[q].y);
+        }
+    }
+    const bool d0 = (col == row), d1 = (col + 1 == row);
+#pragma unroll
+    for (int q = 0; q < SUMS_CHUNK; ++q) {
+        if (q < nl) {
+            double2 o = acc[q];
+            if (d0) o.x += s_coef[q];
+            if (d1) o.y += s_coef[q];
+            *reinterpret_cast<double2*>(Gbase + (long long)(l0 + q) * stride + e0) = o;
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------
 // Roofline denominator: register-resident DMMA.8x8x4 issue-rate microbenchmark (cheb_dm_dmma_peak).
 // Each warp runs DMMA_PEAK_CHAINS independent accumulator chains; no memory traffic in the loop.
 // ---------------------------------------------------------------------------------------------------

@@ -61,7 +61,8 @@ struct cheb_dm_plan_s {
     int nmat;            // k + 2 (+ p when the sums are pre-formed)
     double* ws;          // nmat matrices
     // scalar tables (device)
-    double *costab, *fn, *c, *gT, *dT, *Amat, *tau, *w, *dots;
+    double *costab, *fn, *c, *gT, *dT, *Amat, *tau, *w, *dots, *one;
+    int preformed;       // 1: low-order sums G_l are formed by form_sums_kernel before the giant steps
     DevScalars* sc;
     CUtensorMap* maps;   // nmat descriptors
     int tma2d;
@@ -107,6 +108,7 @@ double* T_ptr(const cheb_dm_plan_s* P, int n) {  // T_n, 1 <= n <= k
 int T_map(int n) { return n - 1; }
 double* buf_ptr(const cheb_dm_plan_s* P, int i) { return P->ws + (size_t)(P->k + i) * P->mat_elems; }
 int buf_map(const cheb_dm_plan_s* P, int i) { return P->k + i; }
+double* G_ptr(const cheb_dm_plan_s* P, int l) { return P->ws + (size_t)(P->k + 2 + l) * P->mat_elems; }
 
 // Algorithm 1, reading A7 for s = 1.  Each entry: T_n = 2 T_l T_r - T_m.
 struct BabyProd {
@@ -282,11 +284,19 @@ void build_tasks(cheb_dm_plan_s* P) {
             t.Out = buf_ptr(P, l & 1);
             t.ldo = P->ld;
         }
-        // low-order sum: T_1..T_{k-1} with coefficients row l of the table, T_0 = I through diag_ptr
-        t.sum_base = T_ptr(P, 1);
-        t.sum_count = k - 1;
-        t.coef = coefT + (size_t)l * k + 1;
-        t.diag_ptr = coefT + (size_t)l * k;
+        if (P->preformed) {
+            // G_l / S_l was formed by form_sums_kernel (diagonal term included): one extra tile, weight 1
+            t.sum_base = G_ptr(P, l);
+            t.sum_count = 1;
+            t.coef = P->one;
+            t.diag_ptr = nullptr;
+        } else {
+            // low-order sum: T_1..T_{k-1} with coefficients row l of the table, T_0 = I through diag_ptr
+            t.sum_base = T_ptr(P, 1);
+            t.sum_count = k - 1;
+            t.coef = coefT + (size_t)l * k + 1;
+            t.diag_ptr = coefT + (size_t)l * k;
+        }
         if (P->nbaby > 0) add_dep(t, DEP_GROUP, GROUP_BABY, baby_tiles);
         if (has_prod) add_dep(t, DEP_PANEL_N, (int)T.size() - 1, tiles_m);
         T.push_back(t);
@@ -347,12 +357,13 @@ void build_tasks(cheb_dm_plan_s* P) {
 cheb_dm_status_t encode_maps(cheb_dm_plan_s* P) {
     EncodeTiledFn enc = get_encode_fn();
     if (!enc) return CHEB_DM_ECUDA;
-    std::vector<CUtensorMap> h(P->nmat);
+    const int nmaps = P->k + 2;  // operands of products: T_1..T_k and the two giant-step buffers
+    std::vector<CUtensorMap> h(nmaps);
     const char* env2d = getenv("CHEB_DM_TMA2D");
     int want2d = (env2d && env2d[0] == '1') ? 1 : 0;
     for (int pass = 0; pass < 2; ++pass) {
         bool ok = true;
-        for (int i = 0; i < P->nmat && ok; ++i) {
+        for (int i = 0; i < nmaps && ok; ++i) {
             void* base = P->ws + (size_t)i * P->mat_elems;
             CUresult r;
             if (!want2d) {
@@ -378,7 +389,7 @@ cheb_dm_status_t encode_maps(cheb_dm_plan_s* P) {
         }
         if (ok) {
             P->tma2d = want2d;
-            CUDA_TRY(cudaMemcpy(P->maps, h.data(), sizeof(CUtensorMap) * P->nmat, cudaMemcpyHostToDevice));
+            CUDA_TRY(cudaMemcpy(P->maps, h.data(), sizeof(CUtensorMap) * nmaps, cudaMemcpyHostToDevice));
             return CHEB_DM_OK;
         }
         if (want2d) break;
@@ -467,6 +478,7 @@ cheb_dm_status_t cheb_dm_destroy(cheb_dm_plan_t P) {
     cudaFree(P->tau);
     cudaFree(P->w);
     cudaFree(P->dots);
+    cudaFree(P->one);
     cudaFree(P->sc);
     cudaFree(P->maps);
     cudaFree(P->tasks);
@@ -494,7 +506,7 @@ cheb_dm_status_t cheb_dm_plan_ex(cheb_dm_plan_t* plan, int N, int M_terms, cheb_
     if (o.outer != CHEB_DM_OUTER_CHEBYSHEV && o.outer != CHEB_DM_OUTER_POWER) return CHEB_DM_EINVAL;
     if (o.sched != CHEB_DM_SCHED_GROUPED && o.sched != CHEB_DM_SCHED_SERIAL) return CHEB_DM_EINVAL;
     if (o.pairing != CHEB_DM_PAIR_ALG1 && o.pairing != CHEB_DM_PAIR_SERIAL) return CHEB_DM_EINVAL;
-    if (o.fuse_sums == 0) o.fuse_sums = 1;
+    if (o.fuse_sums < 0 || o.fuse_sums > 2) return CHEB_DM_EINVAL;
     int k = o.k, p = o.p;
     if (k == 0 && p == 0) {
         k = 1;
@@ -525,8 +537,16 @@ cheb_dm_status_t cheb_dm_plan_ex(cheb_dm_plan_t* plan, int N, int M_terms, cheb_
     choose_tile(P);
     P->ld = ((long long)N + 15) / 16 * 16;
     P->mat_elems = (((size_t)N * (size_t)P->ld) + 127) / 128 * 128;
-    P->nmat = k + 2;
-    P->ws = nullptr; P->costab = P->fn = P->c = P->gT = P->dT = P->Amat = P->tau = P->w = P->dots = nullptr;
+    // a-5: fused (epilogue reads T_1..T_{k-1}: p (k-1) mat bytes per solve) while the baby block stays L2-resident,
+    // pre-formed (form_sums_kernel: (ceil(p/16) (k-1) + p) mat bytes) once it does not.
+    {
+        int mode = o.fuse_sums;
+        if (mode == 0) mode = ((double)k * (double)P->mat_elems * 8.0 > 96.0 * 1024 * 1024 && k > 2 && p > 1) ? 2 : 1;
+        P->preformed = (mode == 2) ? 1 : 0;
+        P->opt.fuse_sums = mode;
+    }
+    P->nmat = k + 2 + (P->preformed ? p : 0);
+    P->ws = nullptr; P->costab = P->fn = P->c = P->gT = P->dT = P->Amat = P->tau = P->w = P->dots = P->one = nullptr;
     P->sc = nullptr; P->maps = nullptr; P->tasks = nullptr; P->task_first = nullptr; P->counters = nullptr;
     P->have_coeffs = P->explicit_bounds = P->have_moments = P->computed = 0;
     P->last_launches = 0;
@@ -549,6 +569,7 @@ cheb_dm_status_t cheb_dm_plan_ex(cheb_dm_plan_t* plan, int N, int M_terms, cheb_
     ok = ok && cudaMalloc(&P->w, sizeof(double) * nq) == cudaSuccess;
     ok = ok && cudaMalloc(&P->dots, sizeof(double) * ((size_t)(p + 1) * tiles * k + (size_t)2 * k * 16)) == cudaSuccess;
     ok = ok && cudaMalloc(&P->sc, sizeof(DevScalars)) == cudaSuccess;
+    ok = ok && cudaMalloc(&P->one, sizeof(double)) == cudaSuccess;
     ok = ok && cudaMalloc(&P->maps, sizeof(CUtensorMap) * P->nmat) == cudaSuccess;
     ok = ok && cudaMalloc(&P->stage_H, sizeof(double) * (size_t)N * N) == cudaSuccess;
     ok = ok && cudaMalloc(&P->stage_D, sizeof(double) * (size_t)N * N) == cudaSuccess;
@@ -569,6 +590,10 @@ cheb_dm_status_t cheb_dm_plan_ex(cheb_dm_plan_t* plan, int N, int M_terms, cheb_
         cudaMemset(P->gT, 0, sizeof(double) * kp);
         cudaMemset(P->c, 0, sizeof(double) * kp);
         cudaMemset(P->sc, 0, sizeof(DevScalars));
+        {
+            const double one = 1.0;
+            cudaMemcpy(P->one, &one, sizeof(double), cudaMemcpyHostToDevice);
+        }
         std::vector<double> tab, A;
         build_costab(nq, tab);
         build_Amat(p, A);
@@ -731,7 +756,20 @@ cheb_dm_status_t cheb_dm_compute(cheb_dm_plan_t P, const double* dH, double* dD,
     if (s != CHEB_DM_OK) return s;
     const int slot = (int)(P->ev_count % TIMING_SLOTS);
     if (P->timing) CUDA_TRY(cudaEventRecord(P->ev0[slot], st));
-    s = run_tasks(P, 0, P->ntasks_solve, dD, P->N, st);
+    if (P->preformed) {
+        s = run_tasks(P, 0, P->nbaby, dD, P->N, st);
+        if (s != CHEB_DM_OK) return s;
+        const long long pairs = (long long)P->N * P->ld / 2;
+        dim3 grid((unsigned)((pairs + 255) / 256), (unsigned)ceil_div(P->p, SUMS_CHUNK));
+        const double* coefT = (P->opt.outer == CHEB_DM_OUTER_POWER) ? P->dT : P->gT;
+        form_sums_kernel<<<grid, 256, sizeof(double) * P->k * SUMS_CHUNK, st>>>(T_ptr(P, 1), (long long)P->mat_elems, P->ld, P->N, P->k,
+                                                                              P->p, coefT, G_ptr(P, 0));
+        ++P->last_launches;
+        CUDA_TRY(cudaGetLastError());
+        s = run_tasks(P, P->nbaby, P->ntasks_solve, dD, P->N, st);
+    } else {
+        s = run_tasks(P, 0, P->ntasks_solve, dD, P->N, st);
+    }
     if (s != CHEB_DM_OK) return s;
     if (P->timing) {
         CUDA_TRY(cudaEventRecord(P->ev1[slot], st));

@@ -163,6 +163,18 @@ def test_parity_tiles_and_schedulers(tile, sched):
     _check(case, r)
 
 
+@pytest.mark.parametrize("fuse", [1, 2])
+@pytest.mark.parametrize("outer", [0, 1])
+def test_parity_fused_and_preformed_sums(fuse, outer):
+    """a-5: epilogue-fused vs batched pre-formed low-order sums (Eq. 21) give the same D."""
+    oracle, cd, workloads, gu, oc = _imports()
+    case = oc.case("cfg0", 0, 128, None) if outer == 1 else oc.case("cfg2", 0, 250, None)
+    r = gu.gpu_solve(case["H"], case["beta"], case["mu"], case["M"], bounds=(case["a"], case["b"]), fuse_sums=fuse, outer=outer)
+    _check(case, r)
+    r = gu.gpu_solve(case["H"], case["beta"], case["mu"], case["M"], fuse_sums=fuse, outer=outer, k=5, p=(case["M"] + 4) // 5, tile=2)
+    _check(case, r)
+
+
 def test_parity_power_outer_recursion_eq4():
     """Eq. 4 literally (S_j + T_k acc), stable when the expansion is short (reading A6)."""
     oracle, cd, workloads, gu, oc = _imports()
