@@ -81,7 +81,9 @@ typedef struct {
     int outer;   /* cheb_dm_outer_t                                                              */
     int sched;   /* cheb_dm_sched_t                                                              */
     int pairing; /* cheb_dm_pairing_t                                                            */
-    int tile;    /* CTA tile: 0 = auto, 1 = 128x128, 2 = 128x64, 3 = 64x64                         */
+    int tile;    /* CTA tile (warp tile): 0 = auto, 1 = 128x128 (32x32), 2 = 128x64 (32x32), 3 = 64x64 (32x32),
+                    4 = 64x32 (16x16), 5 = 64x32 (32x16), 6 = 128x64 (32x16).  auto picks among 1, 6, 4 the
+                    shape with the fewest whole waves x tile area per product on this device             */
     int fuse_sums; /* low-order sums G_l / S_j of Eq. (21).  0 = auto; 1 = formed inside the
                       giant-step epilogues from T_1..T_{k-1} (no extra workspace; p(k-1) N^2 8 bytes of reads per
                       solve, L2 hits while the baby block fits L2); 2 = all p sums formed in one batched pass

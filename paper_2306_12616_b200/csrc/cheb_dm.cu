@@ -21,11 +21,36 @@ using namespace chebdm;
 
 namespace {
 
-typedef GemmCfg<128, 128, 4, 1> Cfg128x128;  // 16 consumer warps, 128 KB ring, 1 CTA/SM
-typedef GemmCfg<128, 64, 4, 2> Cfg128x64;    //  8 consumer warps,  96 KB ring, 2 CTA/SM
-typedef GemmCfg<64, 64, 6, 3> Cfg64x64;      //  4 consumer warps,  96 KB ring (6 stages), up to 3 CTA/SM
+//                 BM   BN  WM  WN  BK  stages  min CTAs/SM
+typedef GemmCfg<128, 128, 32, 32, 16, 4, 1> Cfg128x128;   // 16 consumer warps, 128 KB ring, 1 CTA/SM
+typedef GemmCfg<128, 64, 32, 32, 16, 4, 2> Cfg128x64;     //  8 consumer warps,  96 KB ring, 2 CTA/SM
+typedef GemmCfg<64, 64, 32, 32, 16, 6, 3> Cfg64x64;       //  4 consumer warps,  96 KB ring, 2 CTA/SM (smem)
+typedef GemmCfg<64, 32, 16, 16, 32, 6, 1> Cfg64x32w16;    //  8 consumer warps of 16x16, 144 KB ring, 1 CTA/SM
+typedef GemmCfg<64, 32, 32, 16, 32, 6, 1> Cfg64x32w32;    //  4 consumer warps of 32x16, 144 KB ring, 1 CTA/SM
+typedef GemmCfg<128, 64, 32, 16, 16, 6, 1> Cfg128x64w16;  // 16 consumer warps of 32x16, 144 KB ring, 1 CTA/SM
 
-enum TileSel { TILE_AUTO = 0, TILE_128x128 = 1, TILE_128x64 = 2, TILE_64x64 = 3 };
+enum TileSel { TILE_AUTO = 0, TILE_128x128 = 1, TILE_128x64 = 2, TILE_64x64 = 3, TILE_64x32_W16 = 4, TILE_64x32_W32 = 5,
+               TILE_128x64_W16 = 6, TILE_LAST = 6 };
+
+struct TileShape {
+    int BM, BN, BK, box_slabs;
+    double eff;  // main-loop efficiency used by the plan-time tile choice (fraction of the DMMA rate, measured)
+};
+template <class Cfg>
+TileShape shape_of(double eff) {
+    TileShape t = {Cfg::BM, Cfg::BN, Cfg::BK, Cfg::BOX_SLABS, eff};
+    return t;
+}
+TileShape tile_shape(int sel) {
+    switch (sel) {
+        case TILE_128x128: return shape_of<Cfg128x128>(0.85);
+        case TILE_128x64: return shape_of<Cfg128x64>(0.78);
+        case TILE_64x64: return shape_of<Cfg64x64>(0.70);
+        case TILE_64x32_W16: return shape_of<Cfg64x32w16>(0.70);
+        case TILE_64x32_W32: return shape_of<Cfg64x32w32>(0.65);
+        default: return shape_of<Cfg128x64w16>(0.80);
+    }
+}
 
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
                                   const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
@@ -55,7 +80,7 @@ struct cheb_dm_plan_s {
     cheb_dm_options_t opt;
     int device, num_sms;
     int tile;  // TileSel actually used
-    int BM, BN;
+    int BM, BN, BK, box_slabs;
     long long ld;        // padded leading dimension of workspace matrices (multiple of 16)
     size_t mat_elems;    // elements per workspace matrix
     int nmat;            // k + 2 (+ p when the sums are pre-formed)
@@ -175,29 +200,40 @@ int ceil_div(int a, int b) { return (a + b - 1) / b; }
 
 void choose_tile(cheb_dm_plan_s* P) {
     int sel = P->opt.tile;
-    if (sel < TILE_AUTO || sel > TILE_64x64) sel = TILE_AUTO;
+    if (sel < TILE_AUTO || sel > TILE_LAST) sel = TILE_AUTO;
     if (sel == TILE_AUTO) {
-        // Enough 128x128 tiles to give every SM one: large tile (least L2 traffic per flop).  Otherwise the
-        // small tile, so that the serial giant steps of small N still spread over the SMs.
-        const int t128 = ceil_div(P->N, 128) * ceil_div(P->N, 128);
-        const int t12864 = ceil_div(P->N, 128) * ceil_div(P->N, 64);
-        if (t128 >= P->num_sms) sel = TILE_128x128;
-        else if (t12864 >= 2 * P->num_sms) sel = TILE_128x64;
-        else sel = TILE_64x64;
+        // One product is the unit of the serial chain (giant steps), so pick the shape that minimises the time of
+        // one product on this device: tiles per SM (whole waves, 1 CTA per SM) x tile area / main-loop efficiency.
+        // Large N -> 128x128 (least L2 traffic per flop); N ~ 1000 -> 128x64; N ~ 500 -> 64x32 (128 tiles).
+        const int cand[3] = {TILE_128x128, TILE_128x64_W16, TILE_64x32_W16};
+        double best = 0.0;
+        for (int c = 0; c < 3; ++c) {
+            const TileShape t = tile_shape(cand[c]);
+            const int tiles = ceil_div(P->N, t.BM) * ceil_div(P->N, t.BN);
+            const double cost = (double)ceil_div(tiles, P->num_sms) * t.BM * t.BN / t.eff;
+            if (sel == TILE_AUTO || cost < best) {
+                sel = cand[c];
+                best = cost;
+            }
+        }
     }
+    const TileShape t = tile_shape(sel);
     P->tile = sel;
-    P->BM = (sel == TILE_64x64) ? 64 : 128;
-    P->BN = (sel == TILE_128x128) ? 128 : 64;
+    P->BM = t.BM;
+    P->BN = t.BN;
+    P->BK = t.BK;
+    P->box_slabs = t.box_slabs;
 }
 
 Task blank_task(const cheb_dm_plan_s* P) {
     Task t;
     memset(&t, 0, sizeof(t));
     t.mapA = t.mapB = 0;
-    t.ktiles = ceil_div(P->N, BK);
+    t.ktiles = ceil_div(P->N, P->BK);
     t.tiles_m = ceil_div(P->N, P->BM);
     t.tiles_n = ceil_div(P->N, P->BN);
     t.alpha = 1.0;
+    t.inv_alpha = 1.0;
     t.lds = P->ld;
     t.sum_stride = (long long)P->mat_elems;
     return t;
@@ -230,6 +266,7 @@ void build_tasks(cheb_dm_plan_s* P) {
         t.mapB = T_map(bp.r);
         t.group = GROUP_BABY;
         t.alpha = 2.0;
+        t.inv_alpha = 0.5;
         if (bp.m == 0) {
             t.C = nullptr;
             t.diag_const = -1.0;  // - T_0 = -I
@@ -270,6 +307,7 @@ void build_tasks(cheb_dm_plan_s* P) {
             t.mapA = T_map(k);
             t.mapB = buf_map(P, (l + 1) & 1);
             t.alpha = (power || l == 0) ? 1.0 : 2.0;
+            t.inv_alpha = 1.0 / t.alpha;
             if (!power && l + 2 <= p - 1) {
                 t.C = buf_ptr(P, (l + 2) & 1);
                 t.ldc = P->ld;
@@ -297,7 +335,9 @@ void build_tasks(cheb_dm_plan_s* P) {
             t.coef = coefT + (size_t)l * k + 1;
             t.diag_ptr = coefT + (size_t)l * k;
         }
+        // early: the baby block (operands of the low-order sum); late: the same column panel of the previous step
         if (P->nbaby > 0) add_dep(t, DEP_GROUP, GROUP_BABY, baby_tiles);
+        t.ndeps_early = t.ndeps;
         if (has_prod) add_dep(t, DEP_PANEL_N, (int)T.size() - 1, tiles_m);
         T.push_back(t);
     }
@@ -313,6 +353,7 @@ void build_tasks(cheb_dm_plan_s* P) {
         t.mapA = T_map(k);
         t.mapB = (j == 1) ? T_map(k) : buf_map(P, j & 1);
         t.alpha = 2.0;
+        t.inv_alpha = 0.5;
         if (j == 1) {
             t.diag_const = -1.0;
         } else if (j == 2) {
@@ -371,7 +412,7 @@ cheb_dm_status_t encode_maps(cheb_dm_plan_s* P) {
                 // [slab][row][128 B] with the 128-byte swizzle keyed on the row.
                 cuuint64_t dims[3] = {16, (cuuint64_t)P->N, (cuuint64_t)(P->ld / 16)};
                 cuuint64_t strides[2] = {(cuuint64_t)P->ld * 8, 128};
-                cuuint32_t box[3] = {16, (cuuint32_t)BK, 4};
+                cuuint32_t box[3] = {16, (cuuint32_t)P->BK, (cuuint32_t)P->box_slabs};
                 cuuint32_t estr[3] = {1, 1, 1};
                 r = enc(&h[i], CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, base, dims, strides, box, estr,
                         CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
@@ -379,7 +420,7 @@ cheb_dm_status_t encode_maps(cheb_dm_plan_s* P) {
             } else {
                 cuuint64_t dims[2] = {(cuuint64_t)P->ld, (cuuint64_t)P->N};
                 cuuint64_t strides[1] = {(cuuint64_t)P->ld * 8};
-                cuuint32_t box[2] = {16, (cuuint32_t)BK};
+                cuuint32_t box[2] = {16, (cuuint32_t)P->BK};
                 cuuint32_t estr[2] = {1, 1};
                 r = enc(&h[i], CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, base, dims, strides, box, estr,
                         CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
@@ -441,7 +482,10 @@ cheb_dm_status_t launch_tasks(cheb_dm_plan_s* P, int t0, int t1, int use_deps, i
     switch (P->tile) {
         case TILE_128x128: return launch_cfg<Cfg128x128>(la, items, P->num_sms, st);
         case TILE_128x64: return launch_cfg<Cfg128x64>(la, items, P->num_sms, st);
-        default: return launch_cfg<Cfg64x64>(la, items, P->num_sms, st);
+        case TILE_64x64: return launch_cfg<Cfg64x64>(la, items, P->num_sms, st);
+        case TILE_64x32_W16: return launch_cfg<Cfg64x32w16>(la, items, P->num_sms, st);
+        case TILE_64x32_W32: return launch_cfg<Cfg64x32w32>(la, items, P->num_sms, st);
+        default: return launch_cfg<Cfg128x64w16>(la, items, P->num_sms, st);
     }
 }
 
@@ -915,6 +959,7 @@ cheb_dm_status_t cheb_dm_product(cheb_dm_plan_t P, double alpha, const double* d
     pad_copy_kernel<<<P->num_sms * 4, 256, 0, st>>>(dB, P->N, buf_ptr(P, 1), P->ld);
     Task t = P->h_tasks[P->product_task];
     t.alpha = alpha;
+    t.inv_alpha = (alpha != 0.0) ? 1.0 / alpha : 0.0;  // unused: the product task has no sum / diagonal term
     t.beta = beta;
     t.C = dC;
     t.ldc = P->N;

@@ -28,10 +28,6 @@
 
 namespace chebdm {
 
-constexpr int BK = 16;                  // k-rows per pipeline stage
-constexpr int SLAB_BYTES = BK * 128;    // one 16-column slab: BK rows x 128 B (swizzle-128B atom rows)
-constexpr int BOX_COLS = 64;            // columns per TMA box (4 slabs)
-constexpr int BOX_BYTES = 4 * SLAB_BYTES;
 constexpr int TILE_RING = 2;            // producer run-ahead (tile descriptors in flight)
 constexpr int MAX_DEPS = 4;
 constexpr long long WATCHDOG_CLOCKS = 8000000000ll;
@@ -46,10 +42,14 @@ struct Task {
     int group;               // group whose counter this task's tiles increment
     int out_is_user;         // Out = the user's D (pointer/ld come from the launch parameters)
     int ndeps;
+    int ndeps_early;         // deps [0, ndeps_early) guard the operands of the low-order sum (read by the consumer
+                             // warps BEFORE the K loop); the rest guard the TMA operands and C
     int dep_kind[MAX_DEPS];
     int dep_idx[MAX_DEPS];   // task index (DEP_TASK, DEP_PANEL_N) or group index (DEP_GROUP)
     int dep_target[MAX_DEPS];  // counter value that means "complete" (tiles of the task / panel / group)
     double alpha, beta;
+    double inv_alpha;        // 1/alpha when that is exact (alpha = +-2^n): the sum and diag terms are then folded
+                             // into the accumulator before the K loop; required whenever sum_count > 0
     const double* C;         // nullable
     long long ldc;
     double* Out;
@@ -83,33 +83,59 @@ struct LaunchArgs {
     int* error_flag;         // set to 1 if a dependency wait exceeds the watchdog (never in a correct run)
 };
 
-template <int BM_, int BN_, int STAGES_, int MIN_CTAS_>
+// BM x BN CTA tile, WM x WN warp tile (multiples of 16 / 8), BK k-rows per pipeline stage.
+template <int BM_, int BN_, int WM_, int WN_, int BK_, int STAGES_, int MIN_CTAS_>
 struct GemmCfg {
-    static constexpr int BM = BM_, BN = BN_, STAGES = STAGES_, MIN_CTAS = MIN_CTAS_;
-    static constexpr int WARPS_M = BM / 32, WARPS_N = BN / 32;
+    static constexpr int BM = BM_, BN = BN_, WM = WM_, WN = WN_, BK = BK_, STAGES = STAGES_, MIN_CTAS = MIN_CTAS_;
+    static constexpr int WARPS_M = BM / WM, WARPS_N = BN / WN;
+    static constexpr int FM = WM / 8, FN = WN / 8;               // 8x8 DMMA fragments per warp tile
     static constexpr int CONSUMER_WARPS = WARPS_M * WARPS_N;
     static constexpr int CONSUMER_THREADS = CONSUMER_WARPS * 32;
     static constexpr int THREADS = CONSUMER_THREADS + 32;
+    static constexpr int SLAB_BYTES = BK * 128;                  // one 16-column slab: BK rows x 128 B
+    static constexpr int BOX_SLABS = (BM < BN ? BM : BN) >= 64 ? 4 : (BM < BN ? BM : BN) / 16;  // slabs per TMA box
+    static constexpr int BOX_BYTES = BOX_SLABS * SLAB_BYTES;
     static constexpr int A_BYTES = BM * BK * 8, B_BYTES = BN * BK * 8;
     static constexpr int STAGE_BYTES = A_BYTES + B_BYTES;
     static constexpr int BAR_OFFSET = STAGES * STAGE_BYTES;
     static constexpr int DOT_OFFSET = BAR_OFFSET + 256;          // [CONSUMER_WARPS][32] doubles (moments epilogue)
     static constexpr int SMEM_BYTES = DOT_OFFSET + CONSUMER_WARPS * 32 * 8 + 1024;  // + alignment slack
+    // small warp tiles have the registers to fetch the C tile as soon as the dependencies are known to be
+    // satisfied (first full barrier), which takes one L2 round trip off the serial chain of the giant steps
+    static constexpr bool EARLY_C = (WM * WN <= 512);
+    static_assert(WM % 16 == 0 && WN % 8 == 0 && BM % WM == 0 && BN % WN == 0, "tile shapes");
+    static_assert(WN % 16 == 0, "warp tiles are whole 16-column slabs");
+    static_assert(BK % 8 == 0 && STAGES <= 8, "pipeline");
 };
 
 struct TileInfo {
     int task, tm, tn, stop;
 };
 
+
+// Producer-side wait for one dependency counter (global memory, written by red.release.gpu).
+__device__ __forceinline__ void wait_counter(const int* ctr, int target, int* error_flag) {
+    if (ld_acquire_gpu(ctr) >= target) return;
+    const long long t0 = clock64();
+    while (ld_acquire_gpu(ctr) < target) {
+        if (clock64() - t0 > WATCHDOG_CLOCKS) {  // ~4 s: report instead of hanging
+            atomicExch(error_flag, 1);
+            break;
+        }
+    }
+}
+
 template <class Cfg>
 __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MIN_CTAS) gemm_dmma_kernel(const LaunchArgs args) {
-    constexpr int BM = Cfg::BM, BN = Cfg::BN, STAGES = Cfg::STAGES;
+    constexpr int BM = Cfg::BM, BN = Cfg::BN, BK = Cfg::BK, STAGES = Cfg::STAGES;
+    constexpr int FM = Cfg::FM, FN = Cfg::FN;
+    constexpr int SLAB_BYTES = Cfg::SLAB_BYTES;
     extern __shared__ uint8_t smem_raw[];
     // 1024-byte alignment: the 128B swizzle pattern is a function of address bits [7:9]
     uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
     uint64_t* bars = reinterpret_cast<uint64_t*>(smem + Cfg::BAR_OFFSET);
     // bars[0..S) full, [S..2S) empty, [2S..2S+R) tile_full, [2S+R..2S+2R) tile_empty
-    TileInfo* ring = reinterpret_cast<TileInfo*>(smem + Cfg::BAR_OFFSET + 160);
+    TileInfo* ring = reinterpret_cast<TileInfo*>(smem + Cfg::BAR_OFFSET + 192);
     const uint32_t smem_base = smem_u32(smem);
     const uint32_t bar_base = smem_u32(bars);
     auto full_bar = [&](int s) { return bar_base + 8u * s; };
@@ -145,6 +171,28 @@ __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MIN_CTAS) gemm_dmma_kernel(
             int cur = args.task_begin;
             unsigned long long done_tasks_lo = 0;  // cache of "task complete" observations (tasks < 64 rel.)
             unsigned int done_groups = 0;
+            // One dependency of task `tk` for column panel `tn` (no-op when already observed complete).
+            auto wait_dep = [&](const Task* tk, int d, int tn) {
+                const int kind = tk->dep_kind[d], idx = tk->dep_idx[d], target = tk->dep_target[d];
+                const int* ctr;
+                if (kind == DEP_TASK) {
+                    const int rel = idx - args.task_begin;
+                    if (rel >= 0 && rel < 64 && ((done_tasks_lo >> rel) & 1ull)) return;
+                    ctr = args.task_done + idx;
+                } else if (kind == DEP_PANEL_N) {
+                    ctr = args.panel_done + (size_t)idx * args.panel_stride + tn;
+                } else {
+                    if ((done_groups >> idx) & 1u) return;
+                    ctr = args.group_done + idx;
+                }
+                wait_counter(ctr, target, args.error_flag);
+                if (kind == DEP_TASK) {
+                    const int rel = idx - args.task_begin;
+                    if (rel >= 0 && rel < 64) done_tasks_lo |= 1ull << rel;
+                } else if (kind == DEP_GROUP) {
+                    done_groups |= 1u << idx;
+                }
+            };
             for (;;) {
                 const int item = item_begin + atomicAdd(args.work_counter, 1);
                 const bool stop = item >= item_end;
@@ -157,42 +205,11 @@ __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MIN_CTAS) gemm_dmma_kernel(
                     const int tiles_m = tk->tiles_m;
                     tn = local / tiles_m;  // column-panel-major order: a panel's tiles are consecutive
                     tm = local - tn * tiles_m;
-                    if (args.use_deps) {
-                        const int nd = tk->ndeps;
-                        for (int d = 0; d < nd; ++d) {
-                            const int kind = tk->dep_kind[d], idx = tk->dep_idx[d], target = tk->dep_target[d];
-                            const int* ctr;
-                            if (kind == DEP_TASK) {
-                                const int rel = idx - args.task_begin;
-                                if (rel < 64 && ((done_tasks_lo >> rel) & 1ull)) continue;
-                                ctr = args.task_done + idx;
-                            } else if (kind == DEP_PANEL_N) {
-                                ctr = args.panel_done + (size_t)idx * args.panel_stride + tn;
-                            } else {
-                                if ((done_groups >> idx) & 1u) continue;
-                                ctr = args.group_done + idx;
-                            }
-                            if (ld_acquire_gpu(ctr) < target) {
-                                const long long t0 = clock64();
-                                while (ld_acquire_gpu(ctr) < target) {
-                                    __nanosleep(32);
-                                    if (clock64() - t0 > WATCHDOG_CLOCKS) {  // ~4 s: report instead of hanging
-                                        atomicExch(args.error_flag, 1);
-                                        break;
-                                    }
-                                }
-                            }
-                            if (kind == DEP_TASK) {
-                                const int rel = idx - args.task_begin;
-                                if (rel < 64) done_tasks_lo |= 1ull << rel;
-                            } else if (kind == DEP_GROUP) {
-                                done_groups |= 1u << idx;
-                            }
-                        }
-                        fence_proxy_async();
-                    }
+                    // early dependencies: operands of the low-order sum, which the consumers read before the K loop
+                    if (args.use_deps)
+                        for (int d = 0; d < tk->ndeps_early; ++d) wait_dep(tk, d, tn);
                 }
-                // publish the tile descriptor to the consumer warps
+                // publish the tile descriptor to the consumer warps (mbarrier arrive = release, CTA scope)
                 mbar_wait(tempty_bar(tslot), tphase ^ 1);
                 ring[tslot].task = cur;
                 ring[tslot].tm = tm;
@@ -202,6 +219,12 @@ __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MIN_CTAS) gemm_dmma_kernel(
                 if (++tslot == TILE_RING) { tslot = 0; tphase ^= 1; }
                 if (stop) break;
 
+                // late dependencies: the TMA operands and the C tile
+                if (args.use_deps) {
+                    const int nd = tk->ndeps;
+                    for (int d = tk->ndeps_early; d < nd; ++d) wait_dep(tk, d, tn);
+                    fence_proxy_async();  // data written through the generic proxy, read next by TMA
+                }
                 const int ktiles = tk->ktiles;
                 if (ktiles > 0) {
                     const CUtensorMap* mapA = args.maps + tk->mapA;
@@ -214,11 +237,11 @@ __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MIN_CTAS) gemm_dmma_kernel(
                         mbar_arrive_expect_tx(full_bar(stage), Cfg::STAGE_BYTES);
                         if (!args.tma2d) {
 #pragma unroll
-                            for (int b = 0; b < BM / BOX_COLS; ++b)
-                                tma_load_3d(sA + b * BOX_BYTES, mapA, full_bar(stage), 0, kt * BK, slabA + 4 * b);
+                            for (int b = 0; b < BM / (16 * Cfg::BOX_SLABS); ++b)
+                                tma_load_3d(sA + b * Cfg::BOX_BYTES, mapA, full_bar(stage), 0, kt * BK, slabA + Cfg::BOX_SLABS * b);
 #pragma unroll
-                            for (int b = 0; b < BN / BOX_COLS; ++b)
-                                tma_load_3d(sB + b * BOX_BYTES, mapB, full_bar(stage), 0, kt * BK, slabB + 4 * b);
+                            for (int b = 0; b < BN / (16 * Cfg::BOX_SLABS); ++b)
+                                tma_load_3d(sB + b * Cfg::BOX_BYTES, mapB, full_bar(stage), 0, kt * BK, slabB + Cfg::BOX_SLABS * b);
                         } else {
 #pragma unroll
                             for (int b = 0; b < BM / 16; ++b)
@@ -239,21 +262,22 @@ __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MIN_CTAS) gemm_dmma_kernel(
     const int wm = warp / Cfg::WARPS_N, wn = warp % Cfg::WARPS_N;
     const int g = lane >> 2, t = lane & 3;
     // Per-lane fragment offsets inside a stage (see header comment).  For k4-step j: jh = j>>1, par = j&1,
-    // physical k-row r = 8*jh + par + 2t.  Column c = w*32 + i*8 + g of the operand tile lives in slab c>>4,
+    // physical k-row r = 8*jh + par + 2t.  Column c = w*W + i*8 + g of the operand tile lives in slab c>>4,
     // 16-byte chunk ((c&15)>>1) ^ (r&7), half c&1.
     uint32_t aoff[2], boff[2];
 #pragma unroll
     for (int par = 0; par < 2; ++par) {
         const uint32_t x = par + 2 * t;
         const uint32_t lo = x * 128 + ((((uint32_t)g >> 1) ^ x) << 4) + (g & 1) * 8;
-        aoff[par] = (wm * 2) * SLAB_BYTES + lo;
-        boff[par] = Cfg::A_BYTES + (wn * 2) * SLAB_BYTES + lo;
+        aoff[par] = (wm * (Cfg::WM / 16)) * SLAB_BYTES + lo;
+        boff[par] = Cfg::A_BYTES + (wn * (Cfg::WN / 16)) * SLAB_BYTES + lo;
     }
 
     int stage = 0;
     uint32_t phase = 0;
     int tslot = 0;
     uint32_t tphase = 0;
+    const int N = args.N;
 
     for (;;) {
         mbar_wait(tfull_bar(tslot), tphase);
@@ -263,120 +287,168 @@ __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MIN_CTAS) gemm_dmma_kernel(
         if (++tslot == TILE_RING) { tslot = 0; tphase ^= 1; }
         if (ti.stop) break;
         const Task* tk = args.tasks + ti.task;
+        const int row0 = ti.tm * BM + wm * Cfg::WM + g;
+        const int col0 = ti.tn * BN + wn * Cfg::WN + 2 * t;
 
-        double acc[4][4][2];
+        double acc[FM][FN][2];
 #pragma unroll
-        for (int i = 0; i < 4; ++i)
+        for (int i = 0; i < FM; ++i)
 #pragma unroll
-            for (int j = 0; j < 4; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
+            for (int j = 0; j < FN; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
 
-        const int ktiles = tk->ktiles;
-        for (int kt = 0; kt < ktiles; ++kt) {
-            mbar_wait(full_bar(stage), phase);
-            const uint8_t* sbase = smem + stage * Cfg::STAGE_BYTES;
-#pragma unroll
-            for (int j = 0; j < 4; ++j) {
-                const int jh = j >> 1, par = j & 1;
-                double a[4], b[4];
-#pragma unroll
-                for (int i = 0; i < 4; ++i) {
-                    a[i] = *reinterpret_cast<const double*>(sbase + ((aoff[par] ^ ((i & 1) << 6)) + (i >> 1) * SLAB_BYTES + jh * 1024));
-                    b[i] = *reinterpret_cast<const double*>(sbase + ((boff[par] ^ ((i & 1) << 6)) + (i >> 1) * SLAB_BYTES + jh * 1024));
-                }
-#pragma unroll
-                for (int im = 0; im < 4; ++im)
-#pragma unroll
-                    for (int jn = 0; jn < 4; ++jn) dmma_884(acc[im][jn][0], acc[im][jn][1], a[im], b[jn]);
-            }
-            __syncwarp();
-            if (lane == 0) mbar_arrive(empty_bar(stage));
-            if (++stage == STAGES) { stage = 0; phase ^= 1; }
-        }
-
-        // ------------------------------------ fused epilogue ------------------------------------
-        const int N = args.N;
-        const int row0 = ti.tm * BM + wm * 32 + g;
-        const int col0 = ti.tn * BN + wn * 32 + 2 * t;
-        const double alpha = tk->alpha;
-#pragma unroll
-        for (int i = 0; i < 4; ++i)
-#pragma unroll
-            for (int j = 0; j < 4; ++j) {
-                acc[i][j][0] *= alpha;
-                acc[i][j][1] *= alpha;
-            }
-        if (tk->C != nullptr) {
-            const double beta = tk->beta;
-            const double* C = tk->C;
-            const long long ldc = tk->ldc;
-            const bool vec = ((ldc & 1) == 0) && ((reinterpret_cast<uintptr_t>(C) & 15) == 0);
-#pragma unroll
-            for (int i = 0; i < 4; ++i) {
-                const int r = row0 + i * 8;
-#pragma unroll
-                for (int j = 0; j < 4; ++j) {
-                    const int c = col0 + j * 8;
-                    if (r < N && c < N) {
-                        const double* p = C + (long long)r * ldc + c;
-                        if (vec && c + 1 < N) {
-                            const double2 v = __ldcg(reinterpret_cast<const double2*>(p));
-                            acc[i][j][0] = fma(beta, v.x, acc[i][j][0]);
-                            acc[i][j][1] = fma(beta, v.y, acc[i][j][1]);
-                        } else {
-                            acc[i][j][0] = fma(beta, __ldcg(p), acc[i][j][0]);
-                            if (c + 1 < N) acc[i][j][1] = fma(beta, __ldcg(p + 1), acc[i][j][1]);
-                        }
-                    }
-                }
-            }
-        }
+        // ---- prologue: low-order sum  sum_i coef_i T_i + diag I  (Eq. 21), folded into the accumulator as
+        // (sum)/alpha before the K loop (exact: alpha = +-2^n).  Its operands are guarded by the task's early
+        // dependencies, which the producer checked before publishing this tile, so this work overlaps the wait
+        // for the previous giant step instead of extending the serial chain.
         const int ns = tk->sum_count;
+        const double inv_alpha = tk->inv_alpha;
         if (ns > 0) {
-            // low-order sum  sum_i coef_i T_i  (Eq. 21): workspace matrices, even ld, 16-byte aligned rows
             const double* coef = tk->coef;
             const long long lds = tk->lds, sstride = tk->sum_stride;
             const double* sb = tk->sum_base + (long long)row0 * lds + col0;
-            for (int s = 0; s < ns; ++s) {
-                const double w = coef[s];
-                const double* ps = sb + (long long)s * sstride;
+            int s = 0;
+            for (; (FM * FN <= 8) && s + 1 < ns; s += 2) {  // small warp tiles: two operands in flight per iteration
+                const double w0 = __ldg(coef + s) * inv_alpha, w1 = __ldg(coef + s + 1) * inv_alpha;
+                const double* p0 = sb + (long long)s * sstride;
+                const double* p1 = p0 + sstride;
+                double2 v0[FM][FN], v1[FM][FN];
 #pragma unroll
-                for (int i = 0; i < 4; ++i) {
-                    const int r = row0 + i * 8;
+                for (int i = 0; i < FM; ++i)
 #pragma unroll
-                    for (int j = 0; j < 4; ++j) {
-                        const int c = col0 + j * 8;
-                        if (r < N && c < N) {  // pad column c+1 == N (odd N) holds zeros in the workspace
-                            const double2 v = __ldcg(reinterpret_cast<const double2*>(ps + (long long)(i * 8) * lds + j * 8));
-                            acc[i][j][0] = fma(w, v.x, acc[i][j][0]);
-                            acc[i][j][1] = fma(w, v.y, acc[i][j][1]);
-                        }
+                    for (int j = 0; j < FN; ++j) {
+                        const bool in = (row0 + i * 8 < N) && (col0 + j * 8 < N);  // pad column N (odd N) holds zeros
+                        v0[i][j] = in ? __ldcg(reinterpret_cast<const double2*>(p0 + (long long)(i * 8) * lds + j * 8)) : make_double2(0.0, 0.0);
+                        v1[i][j] = in ? __ldcg(reinterpret_cast<const double2*>(p1 + (long long)(i * 8) * lds + j * 8)) : make_double2(0.0, 0.0);
                     }
-                }
+#pragma unroll
+                for (int i = 0; i < FM; ++i)
+#pragma unroll
+                    for (int j = 0; j < FN; ++j) {
+                        acc[i][j][0] = fma(w0, v0[i][j].x, acc[i][j][0]);
+                        acc[i][j][1] = fma(w0, v0[i][j].y, acc[i][j][1]);
+                        acc[i][j][0] = fma(w1, v1[i][j].x, acc[i][j][0]);
+                        acc[i][j][1] = fma(w1, v1[i][j].y, acc[i][j][1]);
+                    }
+            }
+            for (; s < ns; ++s) {
+                const double w0 = __ldg(coef + s) * inv_alpha;
+                const double* p0 = sb + (long long)s * sstride;
+#pragma unroll
+                for (int i = 0; i < FM; ++i)
+#pragma unroll
+                    for (int j = 0; j < FN; ++j)
+                        if ((row0 + i * 8 < N) && (col0 + j * 8 < N)) {
+                            const double2 v = __ldcg(reinterpret_cast<const double2*>(p0 + (long long)(i * 8) * lds + j * 8));
+                            acc[i][j][0] = fma(w0, v.x, acc[i][j][0]);
+                            acc[i][j][1] = fma(w0, v.y, acc[i][j][1]);
+                        }
             }
         }
         {
             double diag = tk->diag_const;
-            if (tk->diag_ptr != nullptr) diag += *tk->diag_ptr;
+            if (tk->diag_ptr != nullptr) diag += __ldg(tk->diag_ptr);
             if (diag != 0.0) {
+                diag *= inv_alpha;
 #pragma unroll
-                for (int i = 0; i < 4; ++i)
+                for (int i = 0; i < FM; ++i)
 #pragma unroll
-                    for (int j = 0; j < 4; ++j) {
+                    for (int j = 0; j < FN; ++j) {
                         const int r = row0 + i * 8, c = col0 + j * 8;
                         if (r == c) acc[i][j][0] += diag;
                         if (r == c + 1) acc[i][j][1] += diag;
                     }
             }
         }
+
+        // ---- C tile: fetched as soon as the first full barrier shows that the late dependencies hold ----
+        const double* Cp = tk->C;
+        const long long ldc = tk->ldc;
+        const bool cvec = ((ldc & 1) == 0) && ((reinterpret_cast<uintptr_t>(Cp) & 15) == 0);
+        double creg[Cfg::EARLY_C ? FM : 1][Cfg::EARLY_C ? FN : 1][2];
+        auto load_c = [&](int i, int j, double& c0, double& c1) {
+            const int r = row0 + i * 8, c = col0 + j * 8;
+            c0 = 0.0;
+            c1 = 0.0;
+            if (r < N && c < N) {
+                const double* p = Cp + (long long)r * ldc + c;
+                if (cvec && c + 1 < N) {
+                    const double2 v = __ldcg(reinterpret_cast<const double2*>(p));
+                    c0 = v.x;
+                    c1 = v.y;
+                } else {
+                    c0 = __ldcg(p);
+                    if (c + 1 < N) c1 = __ldcg(p + 1);
+                }
+            }
+        };
+        bool c_loaded = false;
+
+        const int ktiles = tk->ktiles;
+        for (int kt = 0; kt < ktiles; ++kt) {
+            mbar_wait(full_bar(stage), phase);
+            if (Cfg::EARLY_C && kt == 0 && Cp != nullptr) {
+#pragma unroll
+                for (int i = 0; i < FM; ++i)
+#pragma unroll
+                    for (int j = 0; j < FN; ++j) load_c(i, j, creg[Cfg::EARLY_C ? i : 0][Cfg::EARLY_C ? j : 0][0], creg[Cfg::EARLY_C ? i : 0][Cfg::EARLY_C ? j : 0][1]);
+                c_loaded = true;
+            }
+            const uint8_t* sbase = smem + stage * Cfg::STAGE_BYTES;
+#pragma unroll
+            for (int j = 0; j < BK / 4; ++j) {
+                const int jh = j >> 1, par = j & 1;
+                double a[FM], b[FN];
+#pragma unroll
+                for (int i = 0; i < FM; ++i)
+                    a[i] = *reinterpret_cast<const double*>(sbase + ((aoff[par] ^ ((i & 1) << 6)) + (i >> 1) * SLAB_BYTES + jh * 1024));
+#pragma unroll
+                for (int i = 0; i < FN; ++i)
+                    b[i] = *reinterpret_cast<const double*>(sbase + ((boff[par] ^ ((i & 1) << 6)) + (i >> 1) * SLAB_BYTES + jh * 1024));
+#pragma unroll
+                for (int im = 0; im < FM; ++im)
+#pragma unroll
+                    for (int jn = 0; jn < FN; ++jn) dmma_884(acc[im][jn][0], acc[im][jn][1], a[im], b[jn]);
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(empty_bar(stage));
+            if (++stage == STAGES) { stage = 0; phase ^= 1; }
+        }
+
+        // ------------------------------------ epilogue ------------------------------------
+        const double alpha = tk->alpha;
+#pragma unroll
+        for (int i = 0; i < FM; ++i)
+#pragma unroll
+            for (int j = 0; j < FN; ++j) {
+                acc[i][j][0] *= alpha;
+                acc[i][j][1] *= alpha;
+            }
+        if (Cp != nullptr) {
+            const double beta = tk->beta;
+#pragma unroll
+            for (int i = 0; i < FM; ++i)
+#pragma unroll
+                for (int j = 0; j < FN; ++j) {
+                    double c0, c1;
+                    if (Cfg::EARLY_C && c_loaded) {
+                        c0 = creg[Cfg::EARLY_C ? i : 0][Cfg::EARLY_C ? j : 0][0];
+                        c1 = creg[Cfg::EARLY_C ? i : 0][Cfg::EARLY_C ? j : 0][1];
+                    } else {
+                        load_c(i, j, c0, c1);
+                    }
+                    acc[i][j][0] = fma(beta, c0, acc[i][j][0]);
+                    acc[i][j][1] = fma(beta, c1, acc[i][j][1]);
+                }
+        }
         {
             double* Out = tk->out_is_user ? args.userD : tk->Out;
             const long long ldo = tk->out_is_user ? args.ldD : tk->ldo;
             const bool vec = ((ldo & 1) == 0) && ((reinterpret_cast<uintptr_t>(Out) & 15) == 0);
 #pragma unroll
-            for (int i = 0; i < 4; ++i) {
+            for (int i = 0; i < FM; ++i) {
                 const int r = row0 + i * 8;
 #pragma unroll
-                for (int j = 0; j < 4; ++j) {
+                for (int j = 0; j < FN; ++j) {
                     const int c = col0 + j * 8;
                     if (r < N && c < N) {
                         double* p = Out + (long long)r * ldo + c;
@@ -405,10 +477,10 @@ __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MIN_CTAS) gemm_dmma_kernel(
                     if (s < nd) {
                         const double* ps = sb + (long long)s * sstride;
 #pragma unroll
-                        for (int i = 0; i < 4; ++i) {
+                        for (int i = 0; i < FM; ++i) {
                             const int r = row0 + i * 8;
 #pragma unroll
-                            for (int j = 0; j < 4; ++j) {
+                            for (int j = 0; j < FN; ++j) {
                                 const int c = col0 + j * 8;
                                 if (r < N && c < N) {
                                     const double2 w2 = __ldcg(reinterpret_cast<const double2*>(ps + (long long)(i * 8) * lds + j * 8));
@@ -419,9 +491,9 @@ __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MIN_CTAS) gemm_dmma_kernel(
                         }
                     } else {  // slot nd: trace
 #pragma unroll
-                        for (int i = 0; i < 4; ++i)
+                        for (int i = 0; i < FM; ++i)
 #pragma unroll
-                            for (int j = 0; j < 4; ++j) {
+                            for (int j = 0; j < FN; ++j) {
                                 const int r = row0 + i * 8, c = col0 + j * 8;
                                 if (r < N && r == c) v += acc[i][j][0];
                                 if (r < N && r == c + 1) v += acc[i][j][1];
@@ -441,10 +513,10 @@ __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MIN_CTAS) gemm_dmma_kernel(
             }
         }
         // --------------------------- publish completion of this tile ---------------------------
-        __threadfence();
+        // CTA barrier orders every consumer thread's stores before thread 0's gpu-scope release (cumulative);
+        // the waiting producer pairs it with ld.acquire.gpu + fence.proxy.async before its TMA reads.
         named_bar_sync(1, Cfg::CONSUMER_THREADS);
         if (threadIdx.x == 0) {
-            __threadfence();
             fence_proxy_async();
             red_release_gpu_add(args.panel_done + (size_t)ti.task * args.panel_stride + ti.tn, 1);
             red_release_gpu_add(args.task_done + ti.task, 1);
