@@ -82,7 +82,7 @@ typedef struct {
     int sched;   /* cheb_dm_sched_t                                                              */
     int pairing; /* cheb_dm_pairing_t                                                            */
     int tile;    /* CTA tile (warp tile): 0 = auto, 1 = 128x128 (32x32), 2 = 128x64 (32x32), 3 = 64x64 (32x32),
-                    4 = 64x32 (16x16), 5 = 64x32 (32x16), 6 = 128x64 (32x16).  auto picks among 1, 6, 4 the
+                    4 = 64x32 (16x16), 5 = 64x32 (32x16), 6 = 128x64 (32x16), 7 = 32x32 (16x16, 2 CTAs/SM).  auto picks among 1, 6, 4 the
                     shape with the fewest whole waves x tile area per product on this device             */
     int fuse_sums; /* low-order sums G_l / S_j of Eq. (21).  0 = auto; 1 = formed inside the
                       giant-step epilogues from T_1..T_{k-1} (no extra workspace; p(k-1) N^2 8 bytes of reads per
@@ -198,6 +198,21 @@ cheb_dm_status_t cheb_dm_flops_per_compute(cheb_dm_plan_t plan, double* flops_ou
 cheb_dm_status_t cheb_dm_set_timing(cheb_dm_plan_t plan, int enable);
 cheb_dm_status_t cheb_dm_product_ms(cheb_dm_plan_t plan, int* count_out, double* total_ms_out);
 cheb_dm_status_t cheb_dm_dmma_peak(int iters, double* tflops_out, void* cuda_stream);
+
+/* Per-tile timeline of the persistent product kernel (tracing aid).
+ * cheb_dm_set_trace(plan, 1): following launches record, per work item (one output tile of one product), the
+ *   %globaltimer nanoseconds at which the producer claimed it, the consumer warps received it, its first operand
+ *   stage landed, its K loop ended and its result was published, plus the SM it ran on.  Costs a few
+ *   instructions per tile; EALLOC if the record buffer cannot be allocated.
+ * cheb_dm_get_trace: copies the records of the last cheb_dm_compute() (items in claim order: baby-step tasks
+ *   first, then giant steps; at most max_records) to HOST memory `out`, count to *count_out (host).
+ *   Synchronises the device.  ESTATE if tracing was never enabled. */
+typedef struct {
+    int task, tm, tn, sm;
+    unsigned long long t_claim, t_desc, t_first, t_kend, t_done;
+} cheb_dm_trace_rec_t;
+cheb_dm_status_t cheb_dm_set_trace(cheb_dm_plan_t plan, int enable);
+cheb_dm_status_t cheb_dm_get_trace(cheb_dm_plan_t plan, cheb_dm_trace_rec_t* out, int max_records, int* count_out);
 
 const char* cheb_dm_strerror(cheb_dm_status_t status);
 

@@ -18,7 +18,14 @@ EXPORTS = [
     "cheb_dm_moments", "cheb_dm_solve_mu", "cheb_dm_product", "cheb_dm_workspace_bytes",
     "cheb_dm_last_launch_count", "cheb_dm_flops_per_compute", "cheb_dm_strerror",
     "cheb_dm_compute_host", "cheb_dm_set_timing", "cheb_dm_product_ms", "cheb_dm_dmma_peak",
+    "cheb_dm_set_trace", "cheb_dm_get_trace",
 ]
+
+
+class TraceRec(C.Structure):
+    _fields_ = [("task", C.c_int), ("tm", C.c_int), ("tn", C.c_int), ("sm", C.c_int),
+                ("t_claim", C.c_uint64), ("t_desc", C.c_uint64), ("t_first", C.c_uint64),
+                ("t_kend", C.c_uint64), ("t_done", C.c_uint64)]
 
 
 class Options(C.Structure):
@@ -76,6 +83,8 @@ def lib():
     L.cheb_dm_set_timing.argtypes = [vp, C.c_int]
     L.cheb_dm_product_ms.argtypes = [vp, ip, dp]
     L.cheb_dm_dmma_peak.argtypes = [C.c_int, dp, vp]
+    L.cheb_dm_set_trace.argtypes = [vp, C.c_int]
+    L.cheb_dm_get_trace.argtypes = [vp, C.POINTER(TraceRec), C.c_int, ip]
     for n in EXPORTS:
         getattr(L, n).restype = C.c_int
     L.cheb_dm_strerror.argtypes = [C.c_int]
@@ -140,6 +149,16 @@ class Plan:
     def compute_host(self, hH: int, hD: int, h_trace: int = 0, stream: int = 0):
         """hH, hD, h_trace: HOST addresses (e.g. of pinned torch tensors / numpy arrays)."""
         _chk(lib().cheb_dm_compute_host(self._h, hH, hD, h_trace or None, stream), "cheb_dm_compute_host")
+
+    def set_trace(self, enable: bool):
+        _chk(lib().cheb_dm_set_trace(self._h, int(bool(enable))), "cheb_dm_set_trace")
+
+    def get_trace(self, max_records: int = 1 << 20):
+        """Per-tile timeline of the last compute: list of dicts (times in ns of %globaltimer)."""
+        buf = (TraceRec * max_records)()
+        n = C.c_int()
+        _chk(lib().cheb_dm_get_trace(self._h, buf, max_records, C.byref(n)), "cheb_dm_get_trace")
+        return [{f: getattr(buf[i], f) for f, _ in TraceRec._fields_} for i in range(n.value)]
 
     def set_timing(self, enable: bool):
         _chk(lib().cheb_dm_set_timing(self._h, int(bool(enable))), "cheb_dm_set_timing")

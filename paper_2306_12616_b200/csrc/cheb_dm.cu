@@ -28,9 +28,10 @@ typedef GemmCfg<64, 64, 32, 32, 16, 6, 3> Cfg64x64;       //  4 consumer warps, 
 typedef GemmCfg<64, 32, 16, 16, 32, 6, 1> Cfg64x32w16;    //  8 consumer warps of 16x16, 144 KB ring, 1 CTA/SM
 typedef GemmCfg<64, 32, 32, 16, 32, 6, 1> Cfg64x32w32;    //  4 consumer warps of 32x16, 144 KB ring, 1 CTA/SM
 typedef GemmCfg<128, 64, 32, 16, 16, 6, 1> Cfg128x64w16;  // 16 consumer warps of 32x16, 144 KB ring, 1 CTA/SM
+typedef GemmCfg<32, 32, 16, 16, 32, 6, 2> Cfg32x32;       //  4 consumer warps of 16x16,  96 KB ring, 2 CTA/SM
 
 enum TileSel { TILE_AUTO = 0, TILE_128x128 = 1, TILE_128x64 = 2, TILE_64x64 = 3, TILE_64x32_W16 = 4, TILE_64x32_W32 = 5,
-               TILE_128x64_W16 = 6, TILE_LAST = 6 };
+               TILE_128x64_W16 = 6, TILE_32x32 = 7, TILE_LAST = 7 };
 
 struct TileShape {
     int BM, BN, BK, box_slabs;
@@ -48,6 +49,7 @@ TileShape tile_shape(int sel) {
         case TILE_64x64: return shape_of<Cfg64x64>(0.70);
         case TILE_64x32_W16: return shape_of<Cfg64x32w16>(0.70);
         case TILE_64x32_W32: return shape_of<Cfg64x32w32>(0.65);
+        case TILE_32x32: return shape_of<Cfg32x32>(0.60);
         default: return shape_of<Cfg128x64w16>(0.80);
     }
 }
@@ -113,6 +115,9 @@ struct cheb_dm_plan_s {
     size_t ws_bytes;
     // host-buffer entry point (cheb_dm_compute_host): device staging for H, D and tr D
     double *stage_H, *stage_D, *stage_tr;
+    // optional per-tile timeline (cheb_dm_set_trace)
+    TraceRec* trace_buf;
+    int trace_on;
     // optional timing of the product launches (cheb_dm_set_timing)
     int timing;
     cudaEvent_t ev0[TIMING_SLOTS], ev1[TIMING_SLOTS];  // ring: compute number i uses slot i % TIMING_SLOTS
@@ -477,6 +482,7 @@ cheb_dm_status_t launch_tasks(cheb_dm_plan_s* P, int t0, int t1, int use_deps, i
     la.ldD = ldD;
     la.tma2d = P->tma2d;
     la.error_flag = P->counters + P->off_error;
+    la.trace = P->trace_on ? P->trace_buf : nullptr;
     const int items = P->h_first[t1] - P->h_first[t0];
     ++P->last_launches;
     switch (P->tile) {
@@ -485,6 +491,7 @@ cheb_dm_status_t launch_tasks(cheb_dm_plan_s* P, int t0, int t1, int use_deps, i
         case TILE_64x64: return launch_cfg<Cfg64x64>(la, items, P->num_sms, st);
         case TILE_64x32_W16: return launch_cfg<Cfg64x32w16>(la, items, P->num_sms, st);
         case TILE_64x32_W32: return launch_cfg<Cfg64x32w32>(la, items, P->num_sms, st);
+        case TILE_32x32: return launch_cfg<Cfg32x32>(la, items, P->num_sms, st);
         default: return launch_cfg<Cfg128x64w16>(la, items, P->num_sms, st);
     }
 }
@@ -531,6 +538,7 @@ cheb_dm_status_t cheb_dm_destroy(cheb_dm_plan_t P) {
     cudaFree(P->stage_H);
     cudaFree(P->stage_D);
     cudaFree(P->stage_tr);
+    cudaFree(P->trace_buf);
     for (int i = 0; i < TIMING_SLOTS; ++i) {
         if (P->ev0[i]) cudaEventDestroy(P->ev0[i]);
         if (P->ev1[i]) cudaEventDestroy(P->ev1[i]);
@@ -596,6 +604,7 @@ cheb_dm_status_t cheb_dm_plan_ex(cheb_dm_plan_t* plan, int N, int M_terms, cheb_
     P->last_launches = 0;
     P->stage_H = P->stage_D = P->stage_tr = nullptr;
     P->timing = 0; P->ev_count = 0;
+    P->trace_buf = nullptr; P->trace_on = 0;
     for (int i = 0; i < TIMING_SLOTS; ++i) P->ev0[i] = P->ev1[i] = nullptr;
 
     const int tiles = ceil_div(N, P->BM) * ceil_div(N, P->BN);
@@ -840,6 +849,33 @@ cheb_dm_status_t cheb_dm_compute_host(cheb_dm_plan_t P, const double* hH, double
     }
     CUDA_TRY(cudaMemcpyAsync(hD, P->stage_D, bytes, cudaMemcpyDeviceToHost, st));
     CUDA_TRY(cudaStreamSynchronize(st));
+    return CHEB_DM_OK;
+}
+
+cheb_dm_status_t cheb_dm_set_trace(cheb_dm_plan_t P, int enable) {
+    if (!P) return CHEB_DM_EINVAL;
+    if (enable && !P->trace_buf) {
+        const size_t n = (size_t)P->h_first.back();
+        if (cudaMalloc(&P->trace_buf, sizeof(TraceRec) * n) != cudaSuccess) {
+            cudaGetLastError();
+            P->trace_buf = nullptr;
+            return CHEB_DM_EALLOC;
+        }
+        CUDA_TRY(cudaMemset(P->trace_buf, 0, sizeof(TraceRec) * n));
+    }
+    P->trace_on = enable ? 1 : 0;
+    return CHEB_DM_OK;
+}
+
+cheb_dm_status_t cheb_dm_get_trace(cheb_dm_plan_t P, cheb_dm_trace_rec_t* out, int max_records, int* count_out) {
+    if (!P || !out || !count_out || max_records < 0) return CHEB_DM_EINVAL;
+    if (!P->trace_buf) return CHEB_DM_ESTATE;
+    static_assert(sizeof(cheb_dm_trace_rec_t) == sizeof(TraceRec), "trace record layout");
+    int n = P->h_first[P->ntasks_solve];  // items of one solve
+    if (n > max_records) n = max_records;
+    CUDA_TRY(cudaDeviceSynchronize());
+    CUDA_TRY(cudaMemcpy(out, P->trace_buf, sizeof(TraceRec) * (size_t)n, cudaMemcpyDeviceToHost));
+    *count_out = n;
     return CHEB_DM_OK;
 }
 

@@ -65,6 +65,8 @@ struct Task {
     double* dot_out;         // [tile][dot_count+1] partials (entry dot_count = partial trace of Out)
 };
 
+struct TraceRec;
+
 struct LaunchArgs {
     const Task* tasks;
     const int* task_first;   // prefix sums of tiles, ntasks+1 entries
@@ -81,6 +83,7 @@ struct LaunchArgs {
     long long ldD;
     int tma2d;               // 1: operand maps are 2-D {column, row} with one 16-column box per copy
     int* error_flag;         // set to 1 if a dependency wait exceeds the watchdog (never in a correct run)
+    TraceRec* trace;         // nullable: per-item timeline, indexed by the global item number
 };
 
 // BM x BN CTA tile, WM x WN warp tile (multiples of 16 / 8), BK k-rows per pipeline stage.
@@ -110,7 +113,29 @@ struct GemmCfg {
 
 struct TileInfo {
     int task, tm, tn, stop;
+    int item, pad;
+    unsigned long long t_claim;
 };
+
+// Optional per-tile timeline (cheb_dm_set_trace): one record per work item, globaltimer nanoseconds.
+struct TraceRec {
+    int task, tm, tn, sm;
+    unsigned long long t_claim;  // producer claimed the item
+    unsigned long long t_desc;   // consumers received the descriptor (early dependencies satisfied)
+    unsigned long long t_first;  // first operand stage landed (late dependencies satisfied, TMA round trip done)
+    unsigned long long t_kend;   // K loop finished
+    unsigned long long t_done;   // tile stored and published
+};
+__device__ __forceinline__ unsigned long long global_ns() {
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    return t;
+}
+__device__ __forceinline__ int sm_id() {
+    int v;
+    asm volatile("mov.u32 %0, %%smid;" : "=r"(v));
+    return v;
+}
 
 
 // Producer-side wait for one dependency counter (global memory, written by red.release.gpu).
@@ -132,7 +157,8 @@ __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MIN_CTAS) gemm_dmma_kernel(
     constexpr int SLAB_BYTES = Cfg::SLAB_BYTES;
     extern __shared__ uint8_t smem_raw[];
     // 1024-byte alignment: the 128B swizzle pattern is a function of address bits [7:9]
-    uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+    // (the pad is applied as an offset so that the pointer keeps its shared address space: LDS, not generic LD)
+    uint8_t* smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
     uint64_t* bars = reinterpret_cast<uint64_t*>(smem + Cfg::BAR_OFFSET);
     // bars[0..S) full, [S..2S) empty, [2S..2S+R) tile_full, [2S+R..2S+2R) tile_empty
     TileInfo* ring = reinterpret_cast<TileInfo*>(smem + Cfg::BAR_OFFSET + 192);
@@ -196,6 +222,7 @@ __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MIN_CTAS) gemm_dmma_kernel(
             for (;;) {
                 const int item = item_begin + atomicAdd(args.work_counter, 1);
                 const bool stop = item >= item_end;
+                const unsigned long long t_claim = args.trace ? global_ns() : 0ull;
                 int tm = 0, tn = 0;
                 const Task* tk = nullptr;
                 if (!stop) {
@@ -215,6 +242,8 @@ __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MIN_CTAS) gemm_dmma_kernel(
                 ring[tslot].tm = tm;
                 ring[tslot].tn = tn;
                 ring[tslot].stop = stop ? 1 : 0;
+                ring[tslot].item = item;
+                ring[tslot].t_claim = t_claim;
                 mbar_arrive(tfull_bar(tslot));
                 if (++tslot == TILE_RING) { tslot = 0; tphase ^= 1; }
                 if (stop) break;
@@ -287,6 +316,9 @@ __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MIN_CTAS) gemm_dmma_kernel(
         if (++tslot == TILE_RING) { tslot = 0; tphase ^= 1; }
         if (ti.stop) break;
         const Task* tk = args.tasks + ti.task;
+        const bool tracing = (args.trace != nullptr) && threadIdx.x == 0;
+        unsigned long long t_desc = 0, t_first = 0, t_kend = 0;
+        if (tracing) t_desc = global_ns();
         const int row0 = ti.tm * BM + wm * Cfg::WM + g;
         const int col0 = ti.tn * BN + wn * Cfg::WN + 2 * t;
 
@@ -386,6 +418,7 @@ __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MIN_CTAS) gemm_dmma_kernel(
         const int ktiles = tk->ktiles;
         for (int kt = 0; kt < ktiles; ++kt) {
             mbar_wait(full_bar(stage), phase);
+            if (tracing && kt == 0) t_first = global_ns();
             if (Cfg::EARLY_C && kt == 0 && Cp != nullptr) {
 #pragma unroll
                 for (int i = 0; i < FM; ++i)
@@ -415,6 +448,7 @@ __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MIN_CTAS) gemm_dmma_kernel(
         }
 
         // ------------------------------------ epilogue ------------------------------------
+        if (tracing) t_kend = global_ns();
         const double alpha = tk->alpha;
 #pragma unroll
         for (int i = 0; i < FM; ++i)
@@ -517,10 +551,16 @@ __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MIN_CTAS) gemm_dmma_kernel(
         // the waiting producer pairs it with ld.acquire.gpu + fence.proxy.async before its TMA reads.
         named_bar_sync(1, Cfg::CONSUMER_THREADS);
         if (threadIdx.x == 0) {
-            fence_proxy_async();
-            red_release_gpu_add(args.panel_done + (size_t)ti.task * args.panel_stride + ti.tn, 1);
-            red_release_gpu_add(args.task_done + ti.task, 1);
-            red_release_gpu_add(args.group_done + tk->group, 1);
+            fence_acq_rel_gpu();  // one gpu-scope fence, then three relaxed increments
+            red_relaxed_gpu_add(args.panel_done + (size_t)ti.task * args.panel_stride + ti.tn, 1);
+            red_relaxed_gpu_add(args.task_done + ti.task, 1);
+            red_relaxed_gpu_add(args.group_done + tk->group, 1);
+            if (tracing) {
+                TraceRec r;
+                r.task = ti.task; r.tm = ti.tm; r.tn = ti.tn; r.sm = sm_id();
+                r.t_claim = ti.t_claim; r.t_desc = t_desc; r.t_first = t_first; r.t_kend = t_kend; r.t_done = global_ns();
+                args.trace[ti.item] = r;
+            }
         }
     }
 }

@@ -27,7 +27,7 @@ def _imports():
 # ----------------------------------------------------------------------------------------------
 # a-4/a-6 kernel: one product with the fused 2AB - C epilogue (Eq. 7), all tile shapes, ragged sizes
 # ----------------------------------------------------------------------------------------------
-@pytest.mark.parametrize("tile", [1, 2, 3, 4, 5, 6])
+@pytest.mark.parametrize("tile", [1, 2, 3, 4, 5, 6, 7])
 @pytest.mark.parametrize("N", [1, 2, 7, 64, 65, 130, 200, 333])
 def test_product_2AB_minus_C(N, tile):
     oracle, cd, workloads, gu, _ = _imports()
@@ -154,7 +154,7 @@ def test_parity_reduced_size_device_gershgorin(cfg, seed, n, M):
     _check(case, r)
 
 
-@pytest.mark.parametrize("tile", [1, 2, 3, 4, 5, 6])
+@pytest.mark.parametrize("tile", [1, 2, 3, 4, 5, 6, 7])
 @pytest.mark.parametrize("sched", [0, 1])
 def test_parity_tiles_and_schedulers(tile, sched):
     oracle, cd, workloads, gu, oc = _imports()
