@@ -90,7 +90,10 @@ typedef struct {
                       (form_sums_kernel: each T_i read ceil(p/16) times, p extra workspace matrices), the
                       epilogues then add one tile.  auto = 2 when k N^2 8 B > 96 MiB.  Neither mode makes the
                       per-term AXPY passes of PAPER.md:234.                                              */
-    int reserved[9];
+    int giant;   /* giant steps at N <= 512: 0 = auto, 1 = generic grouped kernel, 2 = resident-multiplier kernel (each
+                    CTA keeps its 32 rows of T_k in shared memory for all p-1 products and runs two column
+                    panels as independent chains; needs tile 4, 5 or 7 and grouped scheduling, else falls back) */
+    int reserved[8];
 } cheb_dm_options_t;
 
 /* Create a plan for N x N matrices and an M_terms-term expansion.  Chooses (k,p), allocates the
@@ -145,6 +148,10 @@ cheb_dm_status_t cheb_dm_get_bounds(cheb_dm_plan_t plan, double* bounds_out, voi
  * Synchronises `cuda_stream`. */
 cheb_dm_status_t cheb_dm_get_coeffs(cheb_dm_plan_t plan, double* c_out, double* g_out, double* d_out,
                                     void* cuda_stream);
+
+/* The options the plan resolved (every "auto" replaced by the choice made: k, p, tile, fuse_sums, giant).
+ * opts_out: host pointer. */
+cheb_dm_status_t cheb_dm_get_options(cheb_dm_plan_t plan, cheb_dm_options_t* opts_out);
 
 /* The block sizes chosen by the plan. */
 cheb_dm_status_t cheb_dm_get_kp(cheb_dm_plan_t plan, int* k_out, int* p_out);

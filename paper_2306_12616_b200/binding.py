@@ -18,7 +18,7 @@ EXPORTS = [
     "cheb_dm_moments", "cheb_dm_solve_mu", "cheb_dm_product", "cheb_dm_workspace_bytes",
     "cheb_dm_last_launch_count", "cheb_dm_flops_per_compute", "cheb_dm_strerror",
     "cheb_dm_compute_host", "cheb_dm_set_timing", "cheb_dm_product_ms", "cheb_dm_dmma_peak",
-    "cheb_dm_set_trace", "cheb_dm_get_trace",
+    "cheb_dm_set_trace", "cheb_dm_get_trace", "cheb_dm_get_options",
 ]
 
 
@@ -31,7 +31,7 @@ class TraceRec(C.Structure):
 class Options(C.Structure):
     _fields_ = [("k", C.c_int), ("p", C.c_int), ("outer", C.c_int), ("sched", C.c_int),
                 ("pairing", C.c_int), ("tile", C.c_int), ("fuse_sums", C.c_int),
-                ("reserved", C.c_int * 9)]
+                ("giant", C.c_int), ("reserved", C.c_int * 8)]
 
 
 class ChebDMError(RuntimeError):
@@ -83,6 +83,7 @@ def lib():
     L.cheb_dm_set_timing.argtypes = [vp, C.c_int]
     L.cheb_dm_product_ms.argtypes = [vp, ip, dp]
     L.cheb_dm_dmma_peak.argtypes = [C.c_int, dp, vp]
+    L.cheb_dm_get_options.argtypes = [vp, C.POINTER(Options)]
     L.cheb_dm_set_trace.argtypes = [vp, C.c_int]
     L.cheb_dm_get_trace.argtypes = [vp, C.POINTER(TraceRec), C.c_int, ip]
     for n in EXPORTS:
@@ -116,14 +117,16 @@ class Plan:
 
     def __init__(self, N: int, M: int, *, k: int = 0, p: int = 0, outer: int = OUTER_CHEBYSHEV,
                  sched: int = SCHED_GROUPED, pairing: int = PAIR_ALG1, tile: int = TILE_AUTO,
-                 fuse_sums: int = 0, dtype: int = 0):
+                 fuse_sums: int = 0, giant: int = 0, dtype: int = 0):
         self._h = C.c_void_p()
         self.N, self.M = N, M
-        o = Options(k=k, p=p, outer=outer, sched=sched, pairing=pairing, tile=tile, fuse_sums=fuse_sums)
+        o = Options(k=k, p=p, outer=outer, sched=sched, pairing=pairing, tile=tile, fuse_sums=fuse_sums, giant=giant)
         _chk(lib().cheb_dm_plan_ex(C.byref(self._h), N, M, dtype, C.byref(o)), "cheb_dm_plan_ex")
         kk, pp = C.c_int(), C.c_int()
         _chk(lib().cheb_dm_get_kp(self._h, C.byref(kk), C.byref(pp)), "cheb_dm_get_kp")
         self.k, self.p = kk.value, pp.value
+        self.opts = Options()  # as resolved by the plan (tile, fuse_sums, giant, ...)
+        _chk(lib().cheb_dm_get_options(self._h, C.byref(self.opts)), "cheb_dm_get_options")
 
     def destroy(self):
         if self._h:

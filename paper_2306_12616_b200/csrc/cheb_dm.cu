@@ -16,6 +16,7 @@
 #include "aux_kernels.cuh"
 #include "common.cuh"
 #include "gemm_dmma.cuh"
+#include "giant_resident.cuh"
 
 using namespace chebdm;
 
@@ -90,6 +91,8 @@ struct cheb_dm_plan_s {
     // scalar tables (device)
     double *costab, *fn, *c, *gT, *dT, *Amat, *tau, *w, *dots, *one;
     int preformed;       // 1: low-order sums G_l are formed by form_sums_kernel before the giant steps
+    int resident;        // 1: giant steps run in giant_resident_kernel (small N), baby steps in gemm_dmma_kernel
+    int res_tiles_m, res_tiles_n, res_grid, res_smem;
     DevScalars* sc;
     CUtensorMap* maps;   // nmat descriptors
     int tma2d;
@@ -559,6 +562,7 @@ cheb_dm_status_t cheb_dm_plan_ex(cheb_dm_plan_t* plan, int N, int M_terms, cheb_
     if (o.sched != CHEB_DM_SCHED_GROUPED && o.sched != CHEB_DM_SCHED_SERIAL) return CHEB_DM_EINVAL;
     if (o.pairing != CHEB_DM_PAIR_ALG1 && o.pairing != CHEB_DM_PAIR_SERIAL) return CHEB_DM_EINVAL;
     if (o.fuse_sums < 0 || o.fuse_sums > 2) return CHEB_DM_EINVAL;
+    if (o.giant < 0 || o.giant > 2) return CHEB_DM_EINVAL;
     int k = o.k, p = o.p;
     if (k == 0 && p == 0) {
         k = 1;
@@ -597,6 +601,22 @@ cheb_dm_status_t cheb_dm_plan_ex(cheb_dm_plan_t* plan, int N, int M_terms, cheb_
         P->preformed = (mode == 2) ? 1 : 0;
         P->opt.fuse_sums = mode;
     }
+    // Giant steps in the resident-multiplier kernel: N <= 512 (32 rows of T_k fit in shared memory), operand maps
+    // with BK = 32 and 2-slab boxes (the 64x32 / 32x32 tile shapes), grouped scheduling, at least one product.
+    P->resident = 0;
+    P->res_tiles_m = P->res_tiles_n = ceil_div(N, 32);
+    P->res_grid = P->res_tiles_m * ceil_div(P->res_tiles_n, 2);
+    P->res_smem = giant_resident_smem_bytes(ceil_div(N, GR_BK));
+    if (o.giant != 1 && N <= 32 * GR_MAX_KTILES && p >= 2 && P->BK == GR_BK && P->box_slabs == 2 &&
+        o.sched == CHEB_DM_SCHED_GROUPED && P->res_grid <= P->num_sms) {
+        if (cudaFuncSetAttribute(giant_resident_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, P->res_smem) == cudaSuccess) {
+            int per_sm = 0;
+            if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, giant_resident_kernel, GR_THREADS, P->res_smem) == cudaSuccess && per_sm >= 1)
+                P->resident = 1;
+        }
+        cudaGetLastError();
+    }
+    P->opt.giant = P->resident ? 2 : 1;
     P->nmat = k + 2 + (P->preformed ? p : 0);
     P->ws = nullptr; P->costab = P->fn = P->c = P->gT = P->dT = P->Amat = P->tau = P->w = P->dots = P->one = nullptr;
     P->sc = nullptr; P->maps = nullptr; P->tasks = nullptr; P->task_first = nullptr; P->counters = nullptr;
@@ -659,7 +679,7 @@ cheb_dm_status_t cheb_dm_plan_ex(cheb_dm_plan_t* plan, int N, int M_terms, cheb_
         if (st != CHEB_DM_OK) break;
         build_tasks(P);
         const int nt = (int)P->h_tasks.size();
-        P->panel_stride = ceil_div(N, P->BN);
+        P->panel_stride = ceil_div(N, 16);  // >= the number of column panels of every kernel (narrowest panel: 16)
         P->nwork = nt + 4;
         P->off_work = 0;
         P->off_task = P->off_work + P->nwork;
@@ -708,6 +728,13 @@ cheb_dm_status_t cheb_dm_coeffs(cheb_dm_plan_t P, double beta, double mu, const 
     P->beta = beta;
     P->mu = mu;
     P->have_coeffs = 1;
+    return CHEB_DM_OK;
+}
+
+cheb_dm_status_t cheb_dm_get_options(cheb_dm_plan_t P, cheb_dm_options_t* opts_out) {
+    if (!P || !opts_out) return CHEB_DM_EINVAL;
+    *opts_out = P->opt;
+    opts_out->tile = P->tile;
     return CHEB_DM_OK;
 }
 
@@ -788,6 +815,33 @@ cheb_dm_status_t run_tasks(cheb_dm_plan_s* P, int t0, int t1, double* userD, lon
     return CHEB_DM_OK;
 }
 
+// Giant steps of the solve (tasks [nbaby, ntasks_solve)) in the resident-multiplier kernel; cooperative launch
+// because its CTAs wait on one another's panel counters.
+cheb_dm_status_t run_giant_resident(cheb_dm_plan_s* P, double* userD, long long ldD, cudaStream_t st) {
+    GiantArgs ga;
+    ga.tasks = P->tasks;
+    ga.maps = P->maps;
+    ga.first_task = P->nbaby;
+    ga.nsteps = P->ntasks_solve - P->nbaby;
+    ga.N = P->N;
+    ga.ktiles = ceil_div(P->N, GR_BK);
+    ga.tiles_m = P->res_tiles_m;
+    ga.tiles_n = P->res_tiles_n;
+    ga.panel_done = P->counters + P->off_panel;
+    ga.panel_stride = P->panel_stride;
+    ga.userD = userD;
+    ga.ldD = ldD;
+    ga.tma2d = P->tma2d;
+    ga.error_flag = P->counters + P->off_error;
+    ga.trace = P->trace_on ? P->trace_buf : nullptr;
+    ga.trace_base = P->h_first.back();
+    void* args[] = {(void*)&ga};
+    CUDA_TRY(cudaLaunchCooperativeKernel((const void*)giant_resident_kernel, dim3(P->res_grid), dim3(GR_THREADS), args,
+                                         (size_t)P->res_smem, st));
+    ++P->last_launches;
+    return CHEB_DM_OK;
+}
+
 bool device_ok(const cheb_dm_plan_s* P) {
     int dev = -1;
     return cudaGetDevice(&dev) == cudaSuccess && dev == P->device;
@@ -819,7 +873,11 @@ cheb_dm_status_t cheb_dm_compute(cheb_dm_plan_t P, const double* dH, double* dD,
                                                                               P->p, coefT, G_ptr(P, 0));
         ++P->last_launches;
         CUDA_TRY(cudaGetLastError());
-        s = run_tasks(P, P->nbaby, P->ntasks_solve, dD, P->N, st);
+        s = P->resident ? run_giant_resident(P, dD, P->N, st) : run_tasks(P, P->nbaby, P->ntasks_solve, dD, P->N, st);
+    } else if (P->resident) {
+        s = run_tasks(P, 0, P->nbaby, dD, P->N, st);
+        if (s != CHEB_DM_OK) return s;
+        s = run_giant_resident(P, dD, P->N, st);
     } else {
         s = run_tasks(P, 0, P->ntasks_solve, dD, P->N, st);
     }
@@ -855,7 +913,7 @@ cheb_dm_status_t cheb_dm_compute_host(cheb_dm_plan_t P, const double* hH, double
 cheb_dm_status_t cheb_dm_set_trace(cheb_dm_plan_t P, int enable) {
     if (!P) return CHEB_DM_EINVAL;
     if (enable && !P->trace_buf) {
-        const size_t n = (size_t)P->h_first.back();
+        const size_t n = (size_t)P->h_first.back() + (size_t)P->p * P->res_tiles_m * P->res_tiles_n;
         if (cudaMalloc(&P->trace_buf, sizeof(TraceRec) * n) != cudaSuccess) {
             cudaGetLastError();
             P->trace_buf = nullptr;
@@ -871,10 +929,16 @@ cheb_dm_status_t cheb_dm_get_trace(cheb_dm_plan_t P, cheb_dm_trace_rec_t* out, i
     if (!P || !out || !count_out || max_records < 0) return CHEB_DM_EINVAL;
     if (!P->trace_buf) return CHEB_DM_ESTATE;
     static_assert(sizeof(cheb_dm_trace_rec_t) == sizeof(TraceRec), "trace record layout");
-    int n = P->h_first[P->ntasks_solve];  // items of one solve
+    int n = P->h_first[P->resident ? P->nbaby : P->ntasks_solve];  // items of one solve (generic kernel)
     if (n > max_records) n = max_records;
     CUDA_TRY(cudaDeviceSynchronize());
     CUDA_TRY(cudaMemcpy(out, P->trace_buf, sizeof(TraceRec) * (size_t)n, cudaMemcpyDeviceToHost));
+    if (P->resident) {  // followed by the tiles of the resident giant-step kernel
+        int m = P->p * P->res_tiles_m * P->res_tiles_n;
+        if (m > max_records - n) m = max_records - n;
+        CUDA_TRY(cudaMemcpy(out + n, P->trace_buf + P->h_first.back(), sizeof(TraceRec) * (size_t)m, cudaMemcpyDeviceToHost));
+        n += m;
+    }
     *count_out = n;
     return CHEB_DM_OK;
 }

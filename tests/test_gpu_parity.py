@@ -163,6 +163,20 @@ def test_parity_tiles_and_schedulers(tile, sched):
     _check(case, r)
 
 
+@pytest.mark.parametrize("giant", [1, 2])
+@pytest.mark.parametrize("fuse", [1, 2])
+@pytest.mark.parametrize("cfg,n,outer", [("cfg1", 300, 0), ("cfg1", 257, 0), ("cfg2", 95, 0), ("cfg0", 128, 1), ("cfg1", 33, 0)])
+def test_parity_giant_generic_and_resident(giant, fuse, cfg, n, outer):
+    """a-6: the giant steps in the generic grouped kernel and in the resident-multiplier kernel (N <= 512: T_k rows
+    kept in shared memory, two column panels per CTA as independent chains), odd / ragged sizes, odd panel counts."""
+    oracle, cd, workloads, gu, oc = _imports()
+    case = oc.case(cfg, 0, n, None)
+    r = gu.gpu_solve(case["H"], case["beta"], case["mu"], case["M"], giant=giant, fuse_sums=fuse, outer=outer, keep_plan=True)
+    assert r["plan"].opts.giant == giant
+    r["plan"].destroy()
+    _check(case, r)
+
+
 @pytest.mark.parametrize("fuse", [1, 2])
 @pytest.mark.parametrize("outer", [0, 1])
 def test_parity_fused_and_preformed_sums(fuse, outer):
