@@ -13,132 +13,11 @@ namespace cg = cooperative_groups;
 // ---------------------------------------------------------------------------------------------------
 struct DevScalars {
     double a, b;                      // bounds in use (eps_a, eps_b)
-    unsigned long long enc_lo, enc_hi;  // order-preserving encodings for the atomic min / max
     int bad_bounds;                   // set when the bounds are non-finite
     int pad;
     double mu;                        // result of the device-side bisection
     double ne;                        // N_e at that mu
 };
-
-__device__ __forceinline__ unsigned long long enc_f64(double x) {
-    unsigned long long u = (unsigned long long)__double_as_longlong(x);
-    return (u & 0x8000000000000000ull) ? ~u : (u | 0x8000000000000000ull);
-}
-__device__ __forceinline__ double dec_f64(unsigned long long e) {
-    unsigned long long u = (e & 0x8000000000000000ull) ? (e & 0x7fffffffffffffffull) : ~e;
-    return __longlong_as_double((long long)u);
-}
-
-__global__ void init_scalars_kernel(DevScalars* sc, double a, double b, int explicit_bounds) {
-    sc->enc_lo = ~0ull;
-    sc->enc_hi = 0ull;
-    sc->bad_bounds = 0;
-    if (explicit_bounds) {
-        sc->a = a;
-        sc->b = b;
-    }
-}
-
-// ---------------------------------------------------------------------------------------------------
-// a-1: Gershgorin bounds + rescale, one cooperative launch (scaling of PAPER.md:96 read
-// as X = (2H - (a+b) I)/(b-a), reading A1).
-//   phase 1: one warp per row: R_i = sum_{j != i} |h_ij|; block min of h_ii - R_i / max of h_ii + R_i;
-//            one atomicMin/atomicMax per block on order-preserving integer encodings (order-independent,
-//            hence bitwise reproducible).
-//   grid sync
-//   phase 2: X[i][j] = (2 h_ij - (a+b) delta_ij) * (1/(b-a)), written with the workspace's padded leading
-//            dimension (pad columns stay zero).  For N <= ~2500 the second read of H is an L2 hit.
-// HBM bytes: 8N^2 (read) + 8N^2 (re-read, L2 for small N) + 8N^2 (write).
-// ---------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(512) bounds_rescale_kernel(const double* __restrict__ H, int N, double* __restrict__ X,
-                                                             long long ldx, DevScalars* sc, int explicit_bounds) {
-    cg::grid_group grid = cg::this_grid();
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int warps_per_block = blockDim.x >> 5;
-    __shared__ double s_lo[32], s_hi[32];
-    // 16-byte vector path: even N and aligned base make every row start 16-byte aligned
-    const bool vec = ((N & 1) == 0) && ((reinterpret_cast<uintptr_t>(H) & 15) == 0);
-    if (!explicit_bounds) {
-        double lo = INFINITY, hi = -INFINITY;
-        for (int row = blockIdx.x * warps_per_block + warp; row < N; row += gridDim.x * warps_per_block) {
-            const double* hr = H + (long long)row * N;
-            double r = 0.0, hii = 0.0;
-            if (vec) {
-                for (int j = 2 * lane; j < N; j += 64) {
-                    const double2 v = *reinterpret_cast<const double2*>(hr + j);
-                    if (j == row) hii = v.x; else r += fabs(v.x);
-                    if (j + 1 == row) hii = v.y; else r += fabs(v.y);
-                }
-            } else {
-                for (int j = lane; j < N; j += 32) {
-                    const double v = hr[j];
-                    if (j == row) hii = v; else r += fabs(v);
-                }
-            }
-#pragma unroll
-            for (int o = 16; o > 0; o >>= 1) {
-                r += __shfl_xor_sync(0xffffffffu, r, o);
-                hii += __shfl_xor_sync(0xffffffffu, hii, o);  // exactly one lane holds h_ii, the rest 0
-            }
-            lo = fmin(lo, hii - r);
-            hi = fmax(hi, hii + r);
-            if (!(isfinite(r) && isfinite(hii))) { lo = -INFINITY; hi = INFINITY; }
-        }
-        if (lane == 0) { s_lo[warp] = lo; s_hi[warp] = hi; }
-        __syncthreads();
-        if (warp == 0) {
-            lo = lane < warps_per_block ? s_lo[lane] : INFINITY;
-            hi = lane < warps_per_block ? s_hi[lane] : -INFINITY;
-#pragma unroll
-            for (int o = 16; o > 0; o >>= 1) {
-                lo = fmin(lo, __shfl_xor_sync(0xffffffffu, lo, o));
-                hi = fmax(hi, __shfl_xor_sync(0xffffffffu, hi, o));
-            }
-            if (lane == 0) {
-                atomicMin(&sc->enc_lo, enc_f64(lo));
-                atomicMax(&sc->enc_hi, enc_f64(hi));
-            }
-        }
-        __threadfence();
-        grid.sync();
-        if (blockIdx.x == 0 && threadIdx.x == 0) {
-            double a = dec_f64(sc->enc_lo), b = dec_f64(sc->enc_hi);
-            if (!(isfinite(a) && isfinite(b))) sc->bad_bounds = 1;
-            if (a == b) { a -= 1.0; b += 1.0; }  // degenerate H = cI (reading A2-iv)
-            sc->a = a;
-            sc->b = b;
-        }
-    }
-    double a, b;
-    if (explicit_bounds) {
-        a = sc->a;
-        b = sc->b;
-    } else {
-        a = dec_f64(*reinterpret_cast<volatile unsigned long long*>(&sc->enc_lo));
-        b = dec_f64(*reinterpret_cast<volatile unsigned long long*>(&sc->enc_hi));
-        if (a == b) { a -= 1.0; b += 1.0; }
-    }
-    const double inv = 1.0 / (b - a), shift = a + b;
-    for (int row = blockIdx.x * warps_per_block + warp; row < N; row += gridDim.x * warps_per_block) {
-        const double* hr = H + (long long)row * N;
-        double* xr = X + (long long)row * ldx;
-        if (vec) {
-            for (int j = 2 * lane; j < N; j += 64) {
-                const double2 v = *reinterpret_cast<const double2*>(hr + j);
-                double h0 = 2.0 * v.x, h1 = 2.0 * v.y;
-                if (j == row) h0 -= shift;
-                if (j + 1 == row) h1 -= shift;
-                *reinterpret_cast<double2*>(xr + j) = make_double2(h0 * inv, h1 * inv);
-            }
-        } else {
-            for (int j = lane; j < N; j += 32) {
-                double h = 2.0 * hr[j];
-                if (j == row) h -= shift;
-                xr[j] = h * inv;
-            }
-        }
-    }
-}
 
 // Copy a user matrix (ld N) into a padded workspace matrix (ld ldx).
 __global__ void pad_copy_kernel(const double* __restrict__ src, int N, double* __restrict__ dst, long long ldx) {
@@ -220,72 +99,213 @@ __device__ __forceinline__ double fermi_scaled(double beta_t, double mu_t, doubl
 }
 
 // ---------------------------------------------------------------------------------------------------
-// a-2: c_n by the DCT at the N_q Chebyshev nodes (cheb_dm.h, cheb_dm_coeffs).  costab[r] = cos(pi r/(2 N_q)),
-// r < 4 N_q, is built once on the host at plan time (correctly rounded), so the angle n*theta_j is reduced
-// exactly: n theta_j = pi ((n (2j+1)) mod 4N_q) / (2 N_q).
-//   fermi_nodes_kernel: fn[j] = f~(x_j), x_j = costab[2j+1]
-//   dct_kernel: block n -> c[n] (zero for n >= M), double-double accumulation, fixed order.
+// a-1 .. a-3 fused: ONE cooperative launch per solve does everything that precedes the products
+//   phase 0  zero the scheduler counters (replaces a memset node)
+//   phase 1  Gershgorin: one warp per row, per-block (min, max) partials -- no atomics, so no initialisation
+//            pass and a result that does not depend on the order of arrival
+//   -- grid sync --
+//   phase 2  every block reduces the partials to (a, b) itself; rescale H -> X = T_1 (pad columns stay zero);
+//            fn[j] = f~(x_j) at the N_q Chebyshev nodes
+//   -- grid sync --
+//   phase 3  c_n, n < k p: one warp per coefficient, double-double accumulation in a fixed order
+//   -- grid sync --
+//   phase 4  (block 0) tables g (and d) of Eq. (16)-(20).  Thread i owns the coupled chains i and k-i of
+//            g_{i,l} = 2 c_{lk+i} - g_{k-i,l+1}, so the recurrence needs no block barrier.
+// For small N the launch gaps of five separate kernels were ~10 % of a whole solve (cfg1: 39 us of 400 us).
+// HBM bytes as bounds_rescale_kernel: 8N^2 read (+ 8N^2 re-read, L2 for small N) + 8N^2 written.
 // ---------------------------------------------------------------------------------------------------
-__global__ void fermi_nodes_kernel(const DevScalars* sc, double beta, double mu, const double* __restrict__ costab, int Nq,
-                                   double* __restrict__ fn) {
-    const int j = blockIdx.x * blockDim.x + threadIdx.x;
-    if (j >= Nq) return;
-    const double a = sc->a, b = sc->b;
-    const double beta_t = beta * (b - a) * 0.5;
-    const double mu_t = (2.0 * mu - (a + b)) / (b - a);
-    fn[j] = fermi_scaled(beta_t, mu_t, costab[2 * j + 1]);
-}
+struct FrontArgs {
+    const double* H;
+    int N;
+    double* X;
+    long long ldx;
+    DevScalars* sc;
+    int explicit_bounds;
+    double a, b;             // explicit bounds
+    double* part;            // [2 * gridDim.x] per-block (lo, hi)
+    int* counters;
+    int ncounters;
+    double beta, mu;
+    const double* costab;
+    int Nq, M;
+    double* fn;
+    double* c;
+    int k, p;
+    const double* Amat;
+    int want_d;
+    double* gT;
+    double* dT;
+};
 
-__global__ void __launch_bounds__(256) dct_kernel(const double* __restrict__ fn, const double* __restrict__ costab, int Nq, int M,
-                                                  double* __restrict__ c) {
-    __shared__ dd s_buf[32];
-    const int n = blockIdx.x;
-    if (n >= M) {
-        if (threadIdx.x == 0) c[n] = 0.0;
-        return;
-    }
-    const unsigned mask = 4u * (unsigned)Nq - 1u;
-    dd s;
-    s.hi = 0.0;
-    s.lo = 0.0;
-    for (int j = threadIdx.x; j < Nq; j += blockDim.x) {
-        const unsigned r = ((unsigned)n * (2u * (unsigned)j + 1u)) & mask;
-        s = dd_add_prod(s, fn[j], costab[r]);
-    }
-    s = dd_block_reduce(s, s_buf);
-    if (threadIdx.x == 0) c[n] = ((n == 0) ? 1.0 : 2.0) * (s.hi + s.lo) / (double)Nq;
-}
-
-// ---------------------------------------------------------------------------------------------------
-// a-3: tables of Eq. (16)-(20), without forming the kp x kp matrix:
-//   g_{0,l} = c_{lk};  g_{i,p-1} = 2 c_{(p-1)k+i};  g_{i,l} = 2 c_{lk+i} - g_{k-i,l+1} (1 <= l <= p-2);
-//   g_{i,0} = c_i - g_{k-i,1}/2  (p >= 2), g_{i,0} = c_i (p == 1)                       (Eq. 16-17)
-//   d_i: back substitution of sum_{j>=l} a_{j,l} d_{i,j} = g_{i,l} (Eq. 24) with the
-//   matrix A of Eq. (10)-(11) (built on the host at plan time).
-// Output layout: gT[l*k + i] (row l is the coefficient vector of giant step l), dT likewise.
-// One block; thread i owns row i.
-// ---------------------------------------------------------------------------------------------------
-__global__ void tables_kernel(const double* __restrict__ c, int k, int p, const double* __restrict__ Amat, int want_d,
-                              double* __restrict__ gT, double* __restrict__ dT) {
-    for (int l = threadIdx.x; l < p; l += blockDim.x) gT[(size_t)l * k] = c[(size_t)l * k];
-    __syncthreads();
-    for (int l = p - 1; l >= 0; --l) {
-        for (int i = 1 + threadIdx.x; i < k; i += blockDim.x) {
-            double v;
-            if (p == 1) v = c[i];
-            else if (l == p - 1) v = 2.0 * c[(size_t)l * k + i];
-            else if (l >= 1) v = 2.0 * c[(size_t)l * k + i] - gT[(size_t)(l + 1) * k + (k - i)];
-            else v = c[i] - 0.5 * gT[(size_t)1 * k + (k - i)];
-            gT[(size_t)l * k + i] = v;
+__global__ void __launch_bounds__(512) front_end_kernel(const FrontArgs A) {
+    cg::grid_group grid = cg::this_grid();
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int warps_per_block = blockDim.x >> 5;
+    const int gwarp = blockIdx.x * warps_per_block + warp, nwarps = gridDim.x * warps_per_block;
+    const int N = A.N;
+    __shared__ double s_lo[32], s_hi[32];
+    __shared__ double s_ab[2];
+    for (int e = blockIdx.x * blockDim.x + threadIdx.x; e < A.ncounters; e += gridDim.x * blockDim.x) A.counters[e] = 0;
+    const bool vec = ((N & 1) == 0) && ((reinterpret_cast<uintptr_t>(A.H) & 15) == 0);
+    if (!A.explicit_bounds) {
+        double lo = INFINITY, hi = -INFINITY;
+        for (int row = gwarp; row < N; row += nwarps) {
+            const double* hr = A.H + (long long)row * N;
+            double r = 0.0, hii = 0.0;
+            if (vec) {
+                for (int j = 2 * lane; j < N; j += 64) {
+                    const double2 v = *reinterpret_cast<const double2*>(hr + j);
+                    if (j == row) hii = v.x; else r += fabs(v.x);
+                    if (j + 1 == row) hii = v.y; else r += fabs(v.y);
+                }
+            } else {
+                for (int j = lane; j < N; j += 32) {
+                    const double v = hr[j];
+                    if (j == row) hii = v; else r += fabs(v);
+                }
+            }
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) {
+                r += __shfl_xor_sync(0xffffffffu, r, o);
+                hii += __shfl_xor_sync(0xffffffffu, hii, o);  // exactly one lane holds h_ii, the rest 0
+            }
+            lo = fmin(lo, hii - r);
+            hi = fmax(hi, hii + r);
+            if (!(isfinite(r) && isfinite(hii))) { lo = -INFINITY; hi = INFINITY; }
+        }
+        if (lane == 0) { s_lo[warp] = lo; s_hi[warp] = hi; }
+        __syncthreads();
+        if (warp == 0) {
+            lo = lane < warps_per_block ? s_lo[lane] : INFINITY;
+            hi = lane < warps_per_block ? s_hi[lane] : -INFINITY;
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) {
+                lo = fmin(lo, __shfl_xor_sync(0xffffffffu, lo, o));
+                hi = fmax(hi, __shfl_xor_sync(0xffffffffu, hi, o));
+            }
+            if (lane == 0) {
+                A.part[2 * blockIdx.x] = lo;
+                A.part[2 * blockIdx.x + 1] = hi;
+            }
+        }
+        grid.sync();
+        if (warp == 0) {
+            lo = INFINITY;
+            hi = -INFINITY;
+            for (int bIdx = lane; bIdx < (int)gridDim.x; bIdx += 32) {
+                lo = fmin(lo, __ldcg(A.part + 2 * bIdx));
+                hi = fmax(hi, __ldcg(A.part + 2 * bIdx + 1));
+            }
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) {
+                lo = fmin(lo, __shfl_xor_sync(0xffffffffu, lo, o));
+                hi = fmax(hi, __shfl_xor_sync(0xffffffffu, hi, o));
+            }
+            if (lane == 0) {
+                s_ab[0] = lo;
+                s_ab[1] = hi;
+            }
         }
         __syncthreads();
+    } else if (threadIdx.x == 0) {
+        s_ab[0] = A.a;
+        s_ab[1] = A.b;
     }
-    if (want_d) {
-        for (int i = threadIdx.x; i < k; i += blockDim.x) {
+    __syncthreads();
+    double a = s_ab[0], b = s_ab[1];
+    const bool bad = !(isfinite(a) && isfinite(b));
+    if (a == b) { a -= 1.0; b += 1.0; }  // degenerate H = cI (reading A2-iv)
+    if (blockIdx.x == 0 && threadIdx.x == 0) {
+        A.sc->a = a;
+        A.sc->b = b;
+        A.sc->bad_bounds = bad ? 1 : 0;
+    }
+    // ---- phase 2: rescale + Fermi values at the nodes ----
+    {
+        const double inv = 1.0 / (b - a), shift = a + b;
+        for (int row = gwarp; row < N; row += nwarps) {
+            const double* hr = A.H + (long long)row * N;
+            double* xr = A.X + (long long)row * A.ldx;
+            if (vec) {
+                for (int j = 2 * lane; j < N; j += 64) {
+                    const double2 v = *reinterpret_cast<const double2*>(hr + j);
+                    double h0 = 2.0 * v.x, h1 = 2.0 * v.y;
+                    if (j == row) h0 -= shift;
+                    if (j + 1 == row) h1 -= shift;
+                    *reinterpret_cast<double2*>(xr + j) = make_double2(h0 * inv, h1 * inv);
+                }
+            } else {
+                for (int j = lane; j < N; j += 32) {
+                    double h = 2.0 * hr[j];
+                    if (j == row) h -= shift;
+                    xr[j] = h * inv;
+                }
+            }
+        }
+        const double beta_t = A.beta * (b - a) * 0.5;
+        const double mu_t = (2.0 * A.mu - (a + b)) / (b - a);
+        for (int j = blockIdx.x * blockDim.x + threadIdx.x; j < A.Nq; j += gridDim.x * blockDim.x)
+            A.fn[j] = fermi_scaled(beta_t, mu_t, A.costab[2 * j + 1]);
+    }
+    grid.sync();
+    // ---- phase 3: c_n (one warp per coefficient) ----
+    {
+        const int kp = A.k * A.p;
+        const unsigned mask = 4u * (unsigned)A.Nq - 1u;
+        for (int n = gwarp; n < kp; n += nwarps) {
+            double cn = 0.0;
+            if (n < A.M) {
+                dd s;
+                s.hi = 0.0;
+                s.lo = 0.0;
+                for (int j = lane; j < A.Nq; j += 32) {
+                    const unsigned r = ((unsigned)n * (2u * (unsigned)j + 1u)) & mask;
+                    s = dd_add_prod(s, __ldcg(A.fn + j), A.costab[r]);
+                }
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1) {
+                    dd other;
+                    other.hi = __shfl_down_sync(0xffffffffu, s.hi, o);
+                    other.lo = __shfl_down_sync(0xffffffffu, s.lo, o);
+                    s = dd_add(s, other);
+                }
+                cn = ((n == 0) ? 1.0 : 2.0) * (s.hi + s.lo) / (double)A.Nq;
+            }
+            if (lane == 0) A.c[n] = cn;
+        }
+    }
+    grid.sync();
+    // ---- phase 4: tables (block 0).  Layout gT[l*k + i], dT likewise ----
+    if (blockIdx.x != 0) return;
+    {
+        const int k = A.k, p = A.p;
+        const double* c = A.c;
+        for (int l = threadIdx.x; l < p; l += blockDim.x) A.gT[(size_t)l * k] = __ldcg(c + (size_t)l * k);
+        // pairs (i, k-i), 1 <= i <= k/2 (i == k-i when k is even and i = k/2)
+        for (int i = 1 + threadIdx.x; 2 * i <= k; i += blockDim.x) {
+            const int i2 = k - i;
+            double g1 = 0.0, g2 = 0.0;  // g_{i,l+1}, g_{k-i,l+1}
             for (int l = p - 1; l >= 0; --l) {
-                double s = gT[(size_t)l * k + i];
-                for (int j = l + 1; j < p; ++j) s -= Amat[(size_t)j * p + l] * dT[(size_t)j * k + i];
-                dT[(size_t)l * k + i] = s / Amat[(size_t)l * p + l];
+                const double c1 = __ldcg(c + (size_t)l * k + i), c2 = __ldcg(c + (size_t)l * k + i2);
+                double n1, n2;
+                if (p == 1) { n1 = c1; n2 = c2; }
+                else if (l == p - 1) { n1 = 2.0 * c1; n2 = 2.0 * c2; }
+                else if (l >= 1) { n1 = 2.0 * c1 - g2; n2 = 2.0 * c2 - g1; }
+                else { n1 = c1 - 0.5 * g2; n2 = c2 - 0.5 * g1; }
+                A.gT[(size_t)l * k + i] = n1;
+                A.gT[(size_t)l * k + i2] = n2;
+                g1 = n1;
+                g2 = n2;
+            }
+        }
+        if (A.want_d) {
+            __syncthreads();
+            for (int i = threadIdx.x; i < k; i += blockDim.x) {
+                for (int l = p - 1; l >= 0; --l) {
+                    double s = A.gT[(size_t)l * k + i];
+                    for (int j = l + 1; j < p; ++j) s -= A.Amat[(size_t)j * p + l] * A.dT[(size_t)j * k + i];
+                    A.dT[(size_t)l * k + i] = s / A.Amat[(size_t)l * p + l];
+                }
             }
         }
     }

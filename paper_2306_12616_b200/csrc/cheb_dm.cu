@@ -89,7 +89,8 @@ struct cheb_dm_plan_s {
     int nmat;            // k + 2 (+ p when the sums are pre-formed)
     double* ws;          // nmat matrices
     // scalar tables (device)
-    double *costab, *fn, *c, *gT, *dT, *Amat, *tau, *w, *dots, *one;
+    double *costab, *fn, *c, *gT, *dT, *Amat, *tau, *w, *dots, *one, *part;
+    int front_grid;      // blocks of the cooperative front_end_kernel
     int preformed;       // 1: low-order sums G_l are formed by form_sums_kernel before the giant steps
     int resident;        // 1: giant steps run in giant_resident_kernel (small N), baby steps in gemm_dmma_kernel
     int res_tiles_m, res_tiles_n, res_grid, res_smem;
@@ -241,7 +242,6 @@ Task blank_task(const cheb_dm_plan_s* P) {
     t.tiles_m = ceil_div(P->N, P->BM);
     t.tiles_n = ceil_div(P->N, P->BN);
     t.alpha = 1.0;
-    t.inv_alpha = 1.0;
     t.lds = P->ld;
     t.sum_stride = (long long)P->mat_elems;
     return t;
@@ -274,7 +274,6 @@ void build_tasks(cheb_dm_plan_s* P) {
         t.mapB = T_map(bp.r);
         t.group = GROUP_BABY;
         t.alpha = 2.0;
-        t.inv_alpha = 0.5;
         if (bp.m == 0) {
             t.C = nullptr;
             t.diag_const = -1.0;  // - T_0 = -I
@@ -315,7 +314,6 @@ void build_tasks(cheb_dm_plan_s* P) {
             t.mapA = T_map(k);
             t.mapB = buf_map(P, (l + 1) & 1);
             t.alpha = (power || l == 0) ? 1.0 : 2.0;
-            t.inv_alpha = 1.0 / t.alpha;
             if (!power && l + 2 <= p - 1) {
                 t.C = buf_ptr(P, (l + 2) & 1);
                 t.ldc = P->ld;
@@ -361,7 +359,6 @@ void build_tasks(cheb_dm_plan_s* P) {
         t.mapA = T_map(k);
         t.mapB = (j == 1) ? T_map(k) : buf_map(P, j & 1);
         t.alpha = 2.0;
-        t.inv_alpha = 0.5;
         if (j == 1) {
             t.diag_const = -1.0;
         } else if (j == 2) {
@@ -533,6 +530,7 @@ cheb_dm_status_t cheb_dm_destroy(cheb_dm_plan_t P) {
     cudaFree(P->w);
     cudaFree(P->dots);
     cudaFree(P->one);
+    cudaFree(P->part);
     cudaFree(P->sc);
     cudaFree(P->maps);
     cudaFree(P->tasks);
@@ -618,7 +616,7 @@ cheb_dm_status_t cheb_dm_plan_ex(cheb_dm_plan_t* plan, int N, int M_terms, cheb_
     }
     P->opt.giant = P->resident ? 2 : 1;
     P->nmat = k + 2 + (P->preformed ? p : 0);
-    P->ws = nullptr; P->costab = P->fn = P->c = P->gT = P->dT = P->Amat = P->tau = P->w = P->dots = P->one = nullptr;
+    P->ws = nullptr; P->costab = P->fn = P->c = P->gT = P->dT = P->Amat = P->tau = P->w = P->dots = P->one = P->part = nullptr;
     P->sc = nullptr; P->maps = nullptr; P->tasks = nullptr; P->task_first = nullptr; P->counters = nullptr;
     P->have_coeffs = P->explicit_bounds = P->have_moments = P->computed = 0;
     P->last_launches = 0;
@@ -643,6 +641,15 @@ cheb_dm_status_t cheb_dm_plan_ex(cheb_dm_plan_t* plan, int N, int M_terms, cheb_
     ok = ok && cudaMalloc(&P->dots, sizeof(double) * ((size_t)(p + 1) * tiles * k + (size_t)2 * k * 16)) == cudaSuccess;
     ok = ok && cudaMalloc(&P->sc, sizeof(DevScalars)) == cudaSuccess;
     ok = ok && cudaMalloc(&P->one, sizeof(double)) == cudaSuccess;
+    {
+        int per_sm = 0;
+        ok = ok && cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, front_end_kernel, 512, 0) == cudaSuccess && per_sm >= 1;
+        int want = ceil_div(N, 16);
+        if (ceil_div((int)kp, 16) > want) want = ceil_div((int)kp, 16);
+        if (ceil_div(nq, 512) > want) want = ceil_div(nq, 512);
+        P->front_grid = want < P->num_sms ? want : P->num_sms;
+        ok = ok && cudaMalloc(&P->part, sizeof(double) * 2 * P->num_sms) == cudaSuccess;
+    }
     ok = ok && cudaMalloc(&P->maps, sizeof(CUtensorMap) * P->nmat) == cudaSuccess;
     ok = ok && cudaMalloc(&P->stage_H, sizeof(double) * (size_t)N * N) == cudaSuccess;
     ok = ok && cudaMalloc(&P->stage_D, sizeof(double) * (size_t)N * N) == cudaSuccess;
@@ -767,41 +774,37 @@ cheb_dm_status_t cheb_dm_flops_per_compute(cheb_dm_plan_t P, double* flops_out) 
 
 namespace {
 
-// Steps a-1 .. a-3 on the stream: bounds (+ rescale of H into T_1), c_n, g (and d).
+// Steps a-1 .. a-3 on the stream, one cooperative launch: counters reset, bounds (+ rescale of H into T_1), c_n,
+// g (and d).
 cheb_dm_status_t front_end(cheb_dm_plan_s* P, const double* dH, cudaStream_t st) {
-    init_scalars_kernel<<<1, 1, 0, st>>>(P->sc, P->a, P->b, P->explicit_bounds);
+    FrontArgs fa;
+    fa.H = dH;
+    fa.N = P->N;
+    fa.X = T_ptr(P, 1);
+    fa.ldx = P->ld;
+    fa.sc = P->sc;
+    fa.explicit_bounds = P->explicit_bounds;
+    fa.a = P->a;
+    fa.b = P->b;
+    fa.part = P->part;
+    fa.counters = P->counters;
+    fa.ncounters = (int)P->counters_ints;
+    fa.beta = P->beta;
+    fa.mu = P->mu;
+    fa.costab = P->costab;
+    fa.Nq = P->Nq;
+    fa.M = P->M;
+    fa.fn = P->fn;
+    fa.c = P->c;
+    fa.k = P->k;
+    fa.p = P->p;
+    fa.Amat = P->Amat;
+    fa.want_d = (P->opt.outer == CHEB_DM_OUTER_POWER) ? 1 : 0;
+    fa.gT = P->gT;
+    fa.dT = P->dT;
+    void* args[] = {(void*)&fa};
+    CUDA_TRY(cudaLaunchCooperativeKernel((const void*)front_end_kernel, dim3(P->front_grid), dim3(512), args, 0, st));
     ++P->last_launches;
-    {
-        static int coop_blocks_per_sm = 0;
-        if (coop_blocks_per_sm == 0) {
-            CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&coop_blocks_per_sm, bounds_rescale_kernel, 512, 0));
-            if (coop_blocks_per_sm < 1) return CHEB_DM_ECUDA;
-        }
-        const int warps_per_block = 512 / 32;
-        int grid = ceil_div(P->N, warps_per_block);
-        const int cap = coop_blocks_per_sm * P->num_sms;
-        if (grid > cap) grid = cap;
-        const double* H = dH;
-        int N = P->N;
-        double* X = T_ptr(P, 1);
-        long long ldx = P->ld;
-        DevScalars* sc = P->sc;
-        int eb = P->explicit_bounds;
-        void* args[] = {(void*)&H, (void*)&N, (void*)&X, (void*)&ldx, (void*)&sc, (void*)&eb};
-        CUDA_TRY(cudaLaunchCooperativeKernel((const void*)bounds_rescale_kernel, dim3(grid), dim3(512), args, 0, st));
-        ++P->last_launches;
-    }
-    fermi_nodes_kernel<<<ceil_div(P->Nq, 256), 256, 0, st>>>(P->sc, P->beta, P->mu, P->costab, P->Nq, P->fn);
-    dct_kernel<<<P->k * P->p, 256, 0, st>>>(P->fn, P->costab, P->Nq, P->M, P->c);
-    int tb = P->k < 32 ? 32 : (P->k > 1024 ? 1024 : (P->k + 31) / 32 * 32);
-    tables_kernel<<<1, tb, 0, st>>>(P->c, P->k, P->p, P->Amat, P->opt.outer == CHEB_DM_OUTER_POWER ? 1 : 0, P->gT, P->dT);
-    P->last_launches += 3;
-    CUDA_TRY(cudaGetLastError());
-    return CHEB_DM_OK;
-}
-
-cheb_dm_status_t reset_counters(cheb_dm_plan_s* P, cudaStream_t st) {
-    CUDA_TRY(cudaMemsetAsync(P->counters, 0, sizeof(int) * P->counters_ints, st));
     return CHEB_DM_OK;
 }
 
@@ -857,9 +860,7 @@ cheb_dm_status_t cheb_dm_compute(cheb_dm_plan_t P, const double* dH, double* dD,
     if (!device_ok(P)) return CHEB_DM_ECUDA;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     P->last_launches = 0;
-    cheb_dm_status_t s = reset_counters(P, st);
-    if (s != CHEB_DM_OK) return s;
-    s = front_end(P, dH, st);
+    cheb_dm_status_t s = front_end(P, dH, st);  // also zeroes the scheduler counters
     if (s != CHEB_DM_OK) return s;
     const int slot = (int)(P->ev_count % TIMING_SLOTS);
     if (P->timing) CUDA_TRY(cudaEventRecord(P->ev0[slot], st));
@@ -1059,7 +1060,6 @@ cheb_dm_status_t cheb_dm_product(cheb_dm_plan_t P, double alpha, const double* d
     pad_copy_kernel<<<P->num_sms * 4, 256, 0, st>>>(dB, P->N, buf_ptr(P, 1), P->ld);
     Task t = P->h_tasks[P->product_task];
     t.alpha = alpha;
-    t.inv_alpha = (alpha != 0.0) ? 1.0 / alpha : 0.0;  // unused: the product task has no sum / diagonal term
     t.beta = beta;
     t.C = dC;
     t.ldc = P->N;
@@ -1084,9 +1084,7 @@ cheb_dm_status_t cheb_dm_moments(cheb_dm_plan_t P, const double* dH, double* tau
     const int k = P->k, p = P->p;
     const int tiles = ceil_div(P->N, P->BM) * ceil_div(P->N, P->BN);
     P->last_launches = 0;
-    cheb_dm_status_t s = reset_counters(P, st);
-    if (s != CHEB_DM_OK) return s;
-    s = front_end(P, dH, st);  // bounds + rescale (the coefficient tables it also writes are not used here)
+    cheb_dm_status_t s = front_end(P, dH, st);  // counters reset, bounds + rescale (its coefficient tables are not used here)
     if (s != CHEB_DM_OK) return s;
     s = run_tasks(P, 0, P->nbaby, nullptr, 0, st);
     if (s != CHEB_DM_OK) return s;

@@ -21,6 +21,12 @@ __device__ __forceinline__ void fence_mbar_init() {
 __device__ __forceinline__ void mbar_arrive(uint32_t bar) {
     asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
 }
+// Arrive that may not issue before `dep` is available in a register.  ptxas schedules SYNCS.ARRIVE independently of
+// shared-memory loads that are still in flight (it only keeps issue order), so a barrier that hands a shared-memory
+// buffer back to its writer must be tied to the loaded values, or be placed after an instruction that consumed them.
+__device__ __forceinline__ void mbar_arrive_dep(uint32_t bar, int dep) {
+    asm volatile("{\n\t.reg .b32 t;\n\tmov.b32 t, %1;\n\tmbarrier.arrive.shared::cta.b64 _, [%0];\n\t}" ::"r"(bar), "r"(dep) : "memory");
+}
 __device__ __forceinline__ void mbar_arrive_expect_tx(uint32_t bar, uint32_t bytes) {
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
 }
@@ -56,6 +62,11 @@ __device__ __forceinline__ void tma_load_2d(uint32_t dst_smem, const CUtensorMap
 }
 __device__ __forceinline__ void tma_prefetch_desc(const CUtensorMap* map) {
     asm volatile("prefetch.tensormap [%0];" ::"l"(map) : "memory");
+}
+// Tensor maps that live in global memory (written by the host with cudaMemcpy) must be acquired through the
+// tensormap proxy by every CTA before its first TMA use of them; only __grid_constant__ / __constant__ maps are exempt.
+__device__ __forceinline__ void fence_tensormap_acquire(const CUtensorMap* map) {
+    asm volatile("fence.proxy.tensormap::generic.acquire.gpu [%0], 128;" ::"l"(map) : "memory");
 }
 // generic-proxy <-> async-proxy ordering (global data written with st.global, read back by TMA)
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async;" ::: "memory"); }

@@ -48,8 +48,6 @@ struct Task {
     int dep_idx[MAX_DEPS];   // task index (DEP_TASK, DEP_PANEL_N) or group index (DEP_GROUP)
     int dep_target[MAX_DEPS];  // counter value that means "complete" (tiles of the task / panel / group)
     double alpha, beta;
-    double inv_alpha;        // 1/alpha when that is exact (alpha = +-2^n): the sum and diag terms are then folded
-                             // into the accumulator before the K loop; required whenever sum_count > 0
     const double* C;         // nullable
     long long ldc;
     double* Out;
@@ -87,14 +85,14 @@ struct LaunchArgs {
 };
 
 // BM x BN CTA tile, WM x WN warp tile (multiples of 16 / 8), BK k-rows per pipeline stage.
-template <int BM_, int BN_, int WM_, int WN_, int BK_, int STAGES_, int MIN_CTAS_>
+template <int BM_, int BN_, int WM_, int WN_, int BK_, int STAGES_, int MIN_CTAS_, int EARLYC_ = -1>
 struct GemmCfg {
     static constexpr int BM = BM_, BN = BN_, WM = WM_, WN = WN_, BK = BK_, STAGES = STAGES_, MIN_CTAS = MIN_CTAS_;
     static constexpr int WARPS_M = BM / WM, WARPS_N = BN / WN;
     static constexpr int FM = WM / 8, FN = WN / 8;               // 8x8 DMMA fragments per warp tile
     static constexpr int CONSUMER_WARPS = WARPS_M * WARPS_N;
     static constexpr int CONSUMER_THREADS = CONSUMER_WARPS * 32;
-    static constexpr int THREADS = CONSUMER_THREADS + 32;
+    static constexpr int THREADS = CONSUMER_THREADS + 64;        // + producer warp + publisher warp
     static constexpr int SLAB_BYTES = BK * 128;                  // one 16-column slab: BK rows x 128 B
     static constexpr int BOX_SLABS = (BM < BN ? BM : BN) >= 64 ? 4 : (BM < BN ? BM : BN) / 16;  // slabs per TMA box
     static constexpr int BOX_BYTES = BOX_SLABS * SLAB_BYTES;
@@ -102,10 +100,11 @@ struct GemmCfg {
     static constexpr int STAGE_BYTES = A_BYTES + B_BYTES;
     static constexpr int BAR_OFFSET = STAGES * STAGE_BYTES;
     static constexpr int DOT_OFFSET = BAR_OFFSET + 256;          // [CONSUMER_WARPS][32] doubles (moments epilogue)
-    static constexpr int SMEM_BYTES = DOT_OFFSET + CONSUMER_WARPS * 32 * 8 + 1024;  // + alignment slack
+    static constexpr int TRC_OFFSET = DOT_OFFSET + CONSUMER_WARPS * 32 * 8;  // [TILE_RING][4] u64 trace hand-off
+    static constexpr int SMEM_BYTES = TRC_OFFSET + 64 + 1024;     // + alignment slack
     // small warp tiles have the registers to fetch the C tile as soon as the dependencies are known to be
     // satisfied (first full barrier), which takes one L2 round trip off the serial chain of the giant steps
-    static constexpr bool EARLY_C = (WM * WN <= 512);
+    static constexpr bool EARLY_C = EARLYC_ < 0 ? (WM * WN <= 512) : (EARLYC_ != 0);
     static_assert(WM % 16 == 0 && WN % 8 == 0 && BM % WM == 0 && BN % WN == 0, "tile shapes");
     static_assert(WN % 16 == 0, "warp tiles are whole 16-column slabs");
     static_assert(BK % 8 == 0 && STAGES <= 8, "pipeline");
@@ -160,7 +159,7 @@ __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MIN_CTAS) gemm_dmma_kernel(
     // (the pad is applied as an offset so that the pointer keeps its shared address space: LDS, not generic LD)
     uint8_t* smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
     uint64_t* bars = reinterpret_cast<uint64_t*>(smem + Cfg::BAR_OFFSET);
-    // bars[0..S) full, [S..2S) empty, [2S..2S+R) tile_full, [2S+R..2S+2R) tile_empty
+    // bars[0..S) full, [S..2S) empty, [2S..2S+R) tile_full, [2S+R..2S+2R) tile_empty, [2S+2R] tile stored
     TileInfo* ring = reinterpret_cast<TileInfo*>(smem + Cfg::BAR_OFFSET + 192);
     const uint32_t smem_base = smem_u32(smem);
     const uint32_t bar_base = smem_u32(bars);
@@ -168,6 +167,8 @@ __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MIN_CTAS) gemm_dmma_kernel(
     auto empty_bar = [&](int s) { return bar_base + 8u * (STAGES + s); };
     auto tfull_bar = [&](int s) { return bar_base + 8u * (2 * STAGES + s); };
     auto tempty_bar = [&](int s) { return bar_base + 8u * (2 * STAGES + TILE_RING + s); };
+    const uint32_t stored_bar = bar_base + 8u * (2 * STAGES + 2 * TILE_RING);
+    unsigned long long* trc = reinterpret_cast<unsigned long long*>(smem + Cfg::TRC_OFFSET);
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
 
@@ -178,8 +179,9 @@ __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MIN_CTAS) gemm_dmma_kernel(
         }
         for (int s = 0; s < TILE_RING; ++s) {
             mbar_init(tfull_bar(s), 1);
-            mbar_init(tempty_bar(s), Cfg::CONSUMER_WARPS);
+            mbar_init(tempty_bar(s), Cfg::CONSUMER_WARPS + 1);  // consumer warps + publisher
         }
+        mbar_init(stored_bar, Cfg::CONSUMER_WARPS);
         fence_mbar_init();
     }
     __syncthreads();
@@ -196,6 +198,12 @@ __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MIN_CTAS) gemm_dmma_kernel(
             uint32_t tphase = 0;
             int cur = args.task_begin;
             unsigned long long done_tasks_lo = 0;  // cache of "task complete" observations (tasks < 64 rel.)
+            unsigned long long fenced_maps[4] = {0ull, 0ull, 0ull, 0ull};  // tensor maps this CTA has acquired
+            auto acquire_map = [&](int m) {
+                if (m < 256 && ((fenced_maps[m >> 6] >> (m & 63)) & 1ull)) return;
+                fence_tensormap_acquire(args.maps + m);
+                if (m < 256) fenced_maps[m >> 6] |= 1ull << (m & 63);
+            };
             unsigned int done_groups = 0;
             // One dependency of task `tk` for column panel `tn` (no-op when already observed complete).
             auto wait_dep = [&](const Task* tk, int d, int tn) {
@@ -258,6 +266,8 @@ __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MIN_CTAS) gemm_dmma_kernel(
                 if (ktiles > 0) {
                     const CUtensorMap* mapA = args.maps + tk->mapA;
                     const CUtensorMap* mapB = args.maps + tk->mapB;
+                    acquire_map(tk->mapA);
+                    acquire_map(tk->mapB);
                     const int slabA = tm * (BM / 16), slabB = tn * (BN / 16);
                     for (int kt = 0; kt < ktiles; ++kt) {
                         mbar_wait(empty_bar(stage), phase ^ 1);
@@ -287,6 +297,43 @@ __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MIN_CTAS) gemm_dmma_kernel(
         return;
     }
 
+    if (warp == Cfg::CONSUMER_WARPS + 1) {
+        // =================================== publisher warp ===================================
+        // Publishes the completion of each tile: waits until every consumer warp has stored its part (mbarrier
+        // arrive = release, CTA scope), makes the tile visible device-wide with ONE gpu-scope fence (cumulative over
+        // the stores it has synchronised with), then bumps the three counters.  The consumer warps meanwhile go
+        // straight on to their next tile.  Waiting producers pair this with ld.acquire.gpu + fence.proxy.async.
+        // The descriptor slot is released only after publication, so the consumers are never two tiles ahead.
+        if (lane == 0) {
+            int tslot = 0;
+            uint32_t tphase = 0, sphase = 0;
+            for (;;) {
+                mbar_wait(tfull_bar(tslot), tphase);
+                const TileInfo ti = ring[tslot];
+                if (!ti.stop) {
+                    const Task* tk = args.tasks + ti.task;
+                    mbar_wait(stored_bar, sphase);
+                    sphase ^= 1;
+                    fence_acq_rel_gpu();
+                    red_relaxed_gpu_add(args.panel_done + (size_t)ti.task * args.panel_stride + ti.tn, 1);
+                    red_relaxed_gpu_add(args.task_done + ti.task, 1);
+                    red_relaxed_gpu_add(args.group_done + tk->group, 1);
+                    if (args.trace != nullptr) {
+                        TraceRec r;
+                        r.task = ti.task; r.tm = ti.tm; r.tn = ti.tn; r.sm = sm_id();
+                        r.t_claim = ti.t_claim; r.t_desc = trc[tslot * 4 + 0]; r.t_first = trc[tslot * 4 + 1];
+                        r.t_kend = trc[tslot * 4 + 2]; r.t_done = global_ns();
+                        args.trace[ti.item] = r;
+                    }
+                }
+                mbar_arrive_dep(tempty_bar(tslot), ti.task ^ ti.tm ^ ti.tn ^ ti.stop ^ ti.item ^ (int)ti.t_claim);
+                if (ti.stop) break;
+                if (++tslot == TILE_RING) { tslot = 0; tphase ^= 1; }
+            }
+        }
+        return;
+    }
+
     // ======================================= consumer warps =======================================
     const int wm = warp / Cfg::WARPS_N, wn = warp % Cfg::WARPS_N;
     const int g = lane >> 2, t = lane & 3;
@@ -311,8 +358,12 @@ __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MIN_CTAS) gemm_dmma_kernel(
     for (;;) {
         mbar_wait(tfull_bar(tslot), tphase);
         const TileInfo ti = ring[tslot];
-        __syncwarp();
-        if (lane == 0) mbar_arrive(tempty_bar(tslot));
+        const int ti_slot = tslot;
+        // every lane must hold its copy of the descriptor before the slot is handed back (the arrive is tied to the
+        // loaded values; __syncwarp orders the other lanes' loads before lane 0's arrive)
+        const int ti_dep = ti.task ^ ti.tm ^ ti.tn ^ ti.stop ^ ti.item ^ (int)ti.t_claim ^ (int)(ti.t_claim >> 32);
+        const int ti_dep_all = (int)__reduce_xor_sync(0xffffffffu, (unsigned)ti_dep);  // needs every lane's copy
+        if (lane == 0) mbar_arrive_dep(tempty_bar(tslot), ti_dep_all);
         if (++tslot == TILE_RING) { tslot = 0; tphase ^= 1; }
         if (ti.stop) break;
         const Task* tk = args.tasks + ti.task;
@@ -328,67 +379,61 @@ __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MIN_CTAS) gemm_dmma_kernel(
 #pragma unroll
             for (int j = 0; j < FN; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
 
-        // ---- prologue: low-order sum  sum_i coef_i T_i + diag I  (Eq. 21), folded into the accumulator as
-        // (sum)/alpha before the K loop (exact: alpha = +-2^n).  Its operands are guarded by the task's early
-        // dependencies, which the producer checked before publishing this tile, so this work overlaps the wait
-        // for the previous giant step instead of extending the serial chain.
+        // ---- prologue: low-order sum  sum_i coef_i T_i  (Eq. 21).  Small warp tiles have the registers to form
+        // it BEFORE the K loop (its operands are guarded by the task's early dependencies, which the producer checked
+        // before publishing this tile), so the work overlaps the wait for the previous giant step instead of extending
+        // the serial chain.  It is kept in registers of its own and added in the epilogue: starting the accumulator
+        // from it would make every DMMA rounding relative to the (large) sum instead of the (small) running product
+        // and measurably costs accuracy (cfg4: |dtr D| 7e-10 -> 3e-9).  Large warp tiles form it in the epilogue.
+        constexpr bool PRE_SUM = (FM * FN <= 4);
+        double pre[PRE_SUM ? FM : 1][PRE_SUM ? FN : 1][2];
+#pragma unroll
+        for (int i = 0; i < (PRE_SUM ? FM : 1); ++i)
+#pragma unroll
+            for (int j = 0; j < (PRE_SUM ? FN : 1); ++j) pre[i][j][0] = pre[i][j][1] = 0.0;
         const int ns = tk->sum_count;
-        const double inv_alpha = tk->inv_alpha;
-        if (ns > 0) {
+        if (PRE_SUM && ns > 0) {
             const double* coef = tk->coef;
             const long long lds = tk->lds, sstride = tk->sum_stride;
             const double* sb = tk->sum_base + (long long)row0 * lds + col0;
             int s = 0;
-            for (; (FM * FN <= 8) && s + 1 < ns; s += 2) {  // small warp tiles: two operands in flight per iteration
-                const double w0 = __ldg(coef + s) * inv_alpha, w1 = __ldg(coef + s + 1) * inv_alpha;
-                const double* p0 = sb + (long long)s * sstride;
-                const double* p1 = p0 + sstride;
-                double2 v0[FM][FN], v1[FM][FN];
+            for (; s + 3 < ns; s += 4) {  // four operands in flight per iteration
+                double w[4];
+                double2 v[4][PRE_SUM ? FM : 1][PRE_SUM ? FN : 1];
 #pragma unroll
-                for (int i = 0; i < FM; ++i)
+                for (int u = 0; u < 4; ++u) {
+                    w[u] = __ldg(coef + s + u);
+                    const double* pu = sb + (long long)(s + u) * sstride;
 #pragma unroll
-                    for (int j = 0; j < FN; ++j) {
-                        const bool in = (row0 + i * 8 < N) && (col0 + j * 8 < N);  // pad column N (odd N) holds zeros
-                        v0[i][j] = in ? __ldcg(reinterpret_cast<const double2*>(p0 + (long long)(i * 8) * lds + j * 8)) : make_double2(0.0, 0.0);
-                        v1[i][j] = in ? __ldcg(reinterpret_cast<const double2*>(p1 + (long long)(i * 8) * lds + j * 8)) : make_double2(0.0, 0.0);
-                    }
+                    for (int i = 0; i < (PRE_SUM ? FM : 1); ++i)
 #pragma unroll
-                for (int i = 0; i < FM; ++i)
+                        for (int j = 0; j < (PRE_SUM ? FN : 1); ++j) {
+                            const bool in = (row0 + i * 8 < N) && (col0 + j * 8 < N);  // pad column N (odd N) holds zeros
+                            v[u][i][j] = in ? __ldcg(reinterpret_cast<const double2*>(pu + (long long)(i * 8) * lds + j * 8)) : make_double2(0.0, 0.0);
+                        }
+                }
 #pragma unroll
-                    for (int j = 0; j < FN; ++j) {
-                        acc[i][j][0] = fma(w0, v0[i][j].x, acc[i][j][0]);
-                        acc[i][j][1] = fma(w0, v0[i][j].y, acc[i][j][1]);
-                        acc[i][j][0] = fma(w1, v1[i][j].x, acc[i][j][0]);
-                        acc[i][j][1] = fma(w1, v1[i][j].y, acc[i][j][1]);
-                    }
-            }
-            for (; s < ns; ++s) {
-                const double w0 = __ldg(coef + s) * inv_alpha;
-                const double* p0 = sb + (long long)s * sstride;
+                for (int u = 0; u < 4; ++u)
 #pragma unroll
-                for (int i = 0; i < FM; ++i)
+                    for (int i = 0; i < (PRE_SUM ? FM : 1); ++i)
 #pragma unroll
-                    for (int j = 0; j < FN; ++j)
-                        if ((row0 + i * 8 < N) && (col0 + j * 8 < N)) {
-                            const double2 v = __ldcg(reinterpret_cast<const double2*>(p0 + (long long)(i * 8) * lds + j * 8));
-                            acc[i][j][0] = fma(w0, v.x, acc[i][j][0]);
-                            acc[i][j][1] = fma(w0, v.y, acc[i][j][1]);
+                        for (int j = 0; j < (PRE_SUM ? FN : 1); ++j) {
+                            pre[i][j][0] = fma(w[u], v[u][i][j].x, pre[i][j][0]);
+                            pre[i][j][1] = fma(w[u], v[u][i][j].y, pre[i][j][1]);
                         }
             }
-        }
-        {
-            double diag = tk->diag_const;
-            if (tk->diag_ptr != nullptr) diag += __ldg(tk->diag_ptr);
-            if (diag != 0.0) {
-                diag *= inv_alpha;
+            for (; s < ns; ++s) {
+                const double w0 = __ldg(coef + s);
+                const double* p0 = sb + (long long)s * sstride;
 #pragma unroll
-                for (int i = 0; i < FM; ++i)
+                for (int i = 0; i < (PRE_SUM ? FM : 1); ++i)
 #pragma unroll
-                    for (int j = 0; j < FN; ++j) {
-                        const int r = row0 + i * 8, c = col0 + j * 8;
-                        if (r == c) acc[i][j][0] += diag;
-                        if (r == c + 1) acc[i][j][1] += diag;
-                    }
+                    for (int j = 0; j < (PRE_SUM ? FN : 1); ++j)
+                        if ((row0 + i * 8 < N) && (col0 + j * 8 < N)) {
+                            const double2 v = __ldcg(reinterpret_cast<const double2*>(p0 + (long long)(i * 8) * lds + j * 8));
+                            pre[i][j][0] = fma(w0, v.x, pre[i][j][0]);
+                            pre[i][j][1] = fma(w0, v.y, pre[i][j][1]);
+                        }
             }
         }
 
@@ -415,9 +460,18 @@ __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MIN_CTAS) gemm_dmma_kernel(
         };
         bool c_loaded = false;
 
+        // A stage is handed back to the producer one iteration late: when the NEXT stage's full barrier has been
+        // passed, every DMMA of the previous iteration has issued, hence every ld.shared feeding them has returned.
+        // (Arriving at the end of the same iteration is not safe: the arrive can overtake loads still in flight and
+        // the producer's next TMA write then races with them.)
         const int ktiles = tk->ktiles;
+        int prev_stage = -1;
         for (int kt = 0; kt < ktiles; ++kt) {
             mbar_wait(full_bar(stage), phase);
+            if (prev_stage >= 0) {
+                __syncwarp();
+                if (lane == 0) mbar_arrive(empty_bar(prev_stage));
+            }
             if (tracing && kt == 0) t_first = global_ns();
             if (Cfg::EARLY_C && kt == 0 && Cp != nullptr) {
 #pragma unroll
@@ -442,9 +496,18 @@ __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MIN_CTAS) gemm_dmma_kernel(
 #pragma unroll
                     for (int jn = 0; jn < FN; ++jn) dmma_884(acc[im][jn][0], acc[im][jn][1], a[im], b[jn]);
             }
-            __syncwarp();
-            if (lane == 0) mbar_arrive(empty_bar(stage));
+            prev_stage = stage;
             if (++stage == STAGES) { stage = 0; phase ^= 1; }
+        }
+        if (prev_stage >= 0) {
+            // last stage of the tile: the loop-exit branch separates the arrive from the DMMAs that consumed the loads
+            __syncwarp();
+            int dep = 0;
+#pragma unroll
+            for (int i = 0; i < FM; ++i)
+#pragma unroll
+                for (int j = 0; j < FN; ++j) dep ^= __double2hiint(acc[i][j][0]) ^ __double2hiint(acc[i][j][1]);
+            if (lane == 0) mbar_arrive_dep(empty_bar(prev_stage), dep);
         }
 
         // ------------------------------------ epilogue ------------------------------------
@@ -473,6 +536,49 @@ __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MIN_CTAS) gemm_dmma_kernel(
                     acc[i][j][0] = fma(beta, c0, acc[i][j][0]);
                     acc[i][j][1] = fma(beta, c1, acc[i][j][1]);
                 }
+        }
+        if (ns > 0) {
+            if (PRE_SUM) {
+#pragma unroll
+                for (int i = 0; i < (PRE_SUM ? FM : 1); ++i)
+#pragma unroll
+                    for (int j = 0; j < (PRE_SUM ? FN : 1); ++j) {
+                        acc[PRE_SUM ? i : 0][PRE_SUM ? j : 0][0] += pre[i][j][0];
+                        acc[PRE_SUM ? i : 0][PRE_SUM ? j : 0][1] += pre[i][j][1];
+                    }
+            } else {
+                // workspace matrices: even ld, 16-byte aligned rows, zero pad columns
+                const double* coef = tk->coef;
+                const long long lds = tk->lds, sstride = tk->sum_stride;
+                const double* sb = tk->sum_base + (long long)row0 * lds + col0;
+                for (int s = 0; s < ns; ++s) {
+                    const double w = __ldg(coef + s);
+                    const double* ps = sb + (long long)s * sstride;
+#pragma unroll
+                    for (int i = 0; i < FM; ++i)
+#pragma unroll
+                        for (int j = 0; j < FN; ++j)
+                            if ((row0 + i * 8 < N) && (col0 + j * 8 < N)) {
+                                const double2 v = __ldcg(reinterpret_cast<const double2*>(ps + (long long)(i * 8) * lds + j * 8));
+                                acc[i][j][0] = fma(w, v.x, acc[i][j][0]);
+                                acc[i][j][1] = fma(w, v.y, acc[i][j][1]);
+                            }
+                }
+            }
+        }
+        {
+            double diag = tk->diag_const;
+            if (tk->diag_ptr != nullptr) diag += __ldg(tk->diag_ptr);
+            if (diag != 0.0) {
+#pragma unroll
+                for (int i = 0; i < FM; ++i)
+#pragma unroll
+                    for (int j = 0; j < FN; ++j) {
+                        const int r = row0 + i * 8, c = col0 + j * 8;
+                        if (r == c) acc[i][j][0] += diag;
+                        if (r == c + 1) acc[i][j][1] += diag;
+                    }
+            }
         }
         {
             double* Out = tk->out_is_user ? args.userD : tk->Out;
@@ -546,22 +652,14 @@ __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MIN_CTAS) gemm_dmma_kernel(
                 named_bar_sync(1, Cfg::CONSUMER_THREADS);
             }
         }
-        // --------------------------- publish completion of this tile ---------------------------
-        // CTA barrier orders every consumer thread's stores before thread 0's gpu-scope release (cumulative);
-        // the waiting producer pairs it with ld.acquire.gpu + fence.proxy.async before its TMA reads.
-        named_bar_sync(1, Cfg::CONSUMER_THREADS);
-        if (threadIdx.x == 0) {
-            fence_acq_rel_gpu();  // one gpu-scope fence, then three relaxed increments
-            red_relaxed_gpu_add(args.panel_done + (size_t)ti.task * args.panel_stride + ti.tn, 1);
-            red_relaxed_gpu_add(args.task_done + ti.task, 1);
-            red_relaxed_gpu_add(args.group_done + tk->group, 1);
-            if (tracing) {
-                TraceRec r;
-                r.task = ti.task; r.tm = ti.tm; r.tn = ti.tn; r.sm = sm_id();
-                r.t_claim = ti.t_claim; r.t_desc = t_desc; r.t_first = t_first; r.t_kend = t_kend; r.t_done = global_ns();
-                args.trace[ti.item] = r;
-            }
+        // --------------------- hand the tile over to the publisher warp ---------------------
+        if (tracing) {
+            trc[ti_slot * 4 + 0] = t_desc;
+            trc[ti_slot * 4 + 1] = t_first;
+            trc[ti_slot * 4 + 2] = t_kend;
         }
+        __syncwarp();
+        if (lane == 0) mbar_arrive(stored_bar);
     }
 }
 

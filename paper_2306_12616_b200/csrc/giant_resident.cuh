@@ -169,10 +169,15 @@ __global__ void __launch_bounds__(GR_THREADS, 1) giant_resident_kernel(const Gia
 #pragma unroll
             for (int j = 0; j < 2; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
 
-        // ---- prologue: low-order sum (Eq. 21) folded in as (sum + diag I)/alpha; the baby block is complete
-        // (stream order), so this overlaps the wait for the previous step of this panel ----
+        // ---- prologue: low-order sum (Eq. 21) into registers of its own (added in the epilogue; starting the
+        // accumulator from it costs accuracy, see gemm_dmma.cuh); the baby block is complete (stream order), so this
+        // overlaps the wait for the previous step of this panel ----
+        double pre[2][2][2];
+#pragma unroll
+        for (int i = 0; i < 2; ++i)
+#pragma unroll
+            for (int j = 0; j < 2; ++j) pre[i][j][0] = pre[i][j][1] = 0.0;
         const int ns = tk->sum_count;
-        const double inv_alpha = tk->inv_alpha;
         if (ns > 0) {
             const double* coef = tk->coef;
             const long long lds = tk->lds, sstride = tk->sum_stride;
@@ -183,7 +188,7 @@ __global__ void __launch_bounds__(GR_THREADS, 1) giant_resident_kernel(const Gia
                 double2 v[8][2][2];
 #pragma unroll
                 for (int u = 0; u < 8; ++u) {
-                    w[u] = __ldg(coef + q + u) * inv_alpha;
+                    w[u] = __ldg(coef + q + u);
                     const double* pu = sb + (long long)(q + u) * sstride;
 #pragma unroll
                     for (int i = 0; i < 2; ++i)
@@ -199,12 +204,12 @@ __global__ void __launch_bounds__(GR_THREADS, 1) giant_resident_kernel(const Gia
                     for (int i = 0; i < 2; ++i)
 #pragma unroll
                         for (int j = 0; j < 2; ++j) {
-                            acc[i][j][0] = fma(w[u], v[u][i][j].x, acc[i][j][0]);
-                            acc[i][j][1] = fma(w[u], v[u][i][j].y, acc[i][j][1]);
+                            pre[i][j][0] = fma(w[u], v[u][i][j].x, pre[i][j][0]);
+                            pre[i][j][1] = fma(w[u], v[u][i][j].y, pre[i][j][1]);
                         }
             }
             for (; q < ns; ++q) {
-                const double w0 = __ldg(coef + q) * inv_alpha;
+                const double w0 = __ldg(coef + q);
                 const double* pu = sb + (long long)q * sstride;
 #pragma unroll
                 for (int i = 0; i < 2; ++i)
@@ -212,8 +217,8 @@ __global__ void __launch_bounds__(GR_THREADS, 1) giant_resident_kernel(const Gia
                     for (int j = 0; j < 2; ++j)
                         if ((row0 + i * 8 < N) && (col0 + j * 8 < N)) {
                             const double2 v = __ldcg(reinterpret_cast<const double2*>(pu + (long long)(i * 8) * lds + j * 8));
-                            acc[i][j][0] = fma(w0, v.x, acc[i][j][0]);
-                            acc[i][j][1] = fma(w0, v.y, acc[i][j][1]);
+                            pre[i][j][0] = fma(w0, v.x, pre[i][j][0]);
+                            pre[i][j][1] = fma(w0, v.y, pre[i][j][1]);
                         }
             }
         }
@@ -221,14 +226,13 @@ __global__ void __launch_bounds__(GR_THREADS, 1) giant_resident_kernel(const Gia
             double diag = tk->diag_const;
             if (tk->diag_ptr != nullptr) diag += __ldg(tk->diag_ptr);
             if (diag != 0.0) {
-                diag *= inv_alpha;
 #pragma unroll
                 for (int i = 0; i < 2; ++i)
 #pragma unroll
                     for (int j = 0; j < 2; ++j) {
                         const int r = row0 + i * 8, c = col0 + j * 8;
-                        if (r == c) acc[i][j][0] += diag;
-                        if (r == c + 1) acc[i][j][1] += diag;
+                        if (r == c) pre[i][j][0] += diag;
+                        if (r == c + 1) pre[i][j][1] += diag;
                     }
             }
         }
@@ -247,12 +251,18 @@ __global__ void __launch_bounds__(GR_THREADS, 1) giant_resident_kernel(const Gia
         // through its own; the offset persists (the two panel families are independent chains), so from then on
         // one group's K loop covers the other's store -> flag -> poll -> TMA latency.
         if (s == 1 && g == 1 && kts > 0) mbar_wait(stagger_bar(), 0);
+        int prev_stage = -1;  // stages are released one iteration late (see gemm_dmma.cuh: the arrive must not
+                              // overtake ld.shared that are still in flight)
         for (int kt = 0; kt < kts; ++kt) {
             if (s == 1 && g == 0 && kt == kts / 2) {
                 __syncwarp();
                 if (lane == 0) mbar_arrive(stagger_bar());
             }
             mbar_wait(full_bar(g, stage), phase);
+            if (prev_stage >= 0) {
+                __syncwarp();
+                if (lane == 0) mbar_arrive(empty_bar(g, prev_stage));
+            }
             if (kt == 0) {
                 if (tracing) t_first = global_ns();
                 if (Cp != nullptr) {  // workspace matrix: even ld, 16-byte aligned rows, zero pad columns
@@ -283,9 +293,17 @@ __global__ void __launch_bounds__(GR_THREADS, 1) giant_resident_kernel(const Gia
 #pragma unroll
                     for (int jn = 0; jn < 2; ++jn) dmma_884(acc[im][jn][0], acc[im][jn][1], a[im], b[jn]);
             }
-            __syncwarp();
-            if (lane == 0) mbar_arrive(empty_bar(g, stage));
+            prev_stage = stage;
             if (++stage == GR_STAGES) { stage = 0; phase ^= 1; }
+        }
+        if (prev_stage >= 0) {
+            int dep = 0;
+#pragma unroll
+            for (int i = 0; i < 2; ++i)
+#pragma unroll
+                for (int j = 0; j < 2; ++j) dep ^= __double2hiint(acc[i][j][0]) ^ __double2hiint(acc[i][j][1]);
+            __syncwarp();
+            if (lane == 0) mbar_arrive_dep(empty_bar(g, prev_stage), dep);
         }
         if (tracing) t_kend = global_ns();
 
@@ -300,8 +318,8 @@ __global__ void __launch_bounds__(GR_THREADS, 1) giant_resident_kernel(const Gia
 #pragma unroll
             for (int j = 0; j < 2; ++j) {
                 const int c = col0 + j * 8;
-                const double o0 = fma(beta, creg[i][j][0], alpha * acc[i][j][0]);
-                const double o1 = fma(beta, creg[i][j][1], alpha * acc[i][j][1]);
+                const double o0 = fma(beta, creg[i][j][0], alpha * acc[i][j][0]) + pre[i][j][0];
+                const double o1 = fma(beta, creg[i][j][1], alpha * acc[i][j][1]) + pre[i][j][1];
                 if (r < N && c < N) {
                     double* p = Out + (long long)r * ldo + c;
                     if (vec && c + 1 < N) {

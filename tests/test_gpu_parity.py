@@ -189,6 +189,19 @@ def test_parity_fused_and_preformed_sums(fuse, outer):
     _check(case, r)
 
 
+@pytest.mark.parametrize("tile,n", [(4, 700), (5, 700), (6, 1500), (7, 700), (3, 700), (1, 1500)])
+def test_grouped_equals_serial_bitwise_many_tiles_per_task(tile, n):
+    """a-8: with more tiles per product than resident CTAs every CTA streams several tiles back to back and the
+    producer runs ahead of the consumers; the grouped schedule must reproduce the serial one bit for bit (fixed
+    summation order).  Regression test for a shared-memory stage handed back while loads were still in flight."""
+    oracle, cd, workloads, gu, oc = _imports()
+    H = workloads.hamiltonian("cfg4", seed=0, n=n)
+    ref = gu.gpu_solve(H, 200.0, 0.0, 64, tile=tile, sched=1)
+    for _ in range(3):
+        r = gu.gpu_solve(H, 200.0, 0.0, 64, tile=tile, sched=0, giant=1)
+        assert np.array_equal(r["D"], ref["D"])
+
+
 def test_parity_power_outer_recursion_eq4():
     """Eq. 4 literally (S_j + T_k acc), stable when the expansion is short (reading A6)."""
     oracle, cd, workloads, gu, oc = _imports()
