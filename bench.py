@@ -33,7 +33,12 @@ UNIT = "solves/s"
 FLUSH_BYTES = 512 << 20  # > 126 MB L2
 # dram__bytes_read.sum + dram__bytes_write.sum of one product-kernel launch from the `ncu --set full`
 # captures summarised under profiles/ (per workload); None = not captured yet.
-NCU_TRAFFIC_BYTES = {}
+# Sum over the product launches of one solve (baby-step launch + giant-step launch).  ncu replays with cold caches, so
+# for cfg1/cfg2 (working set L2-resident when warm) this is an upper bound.  cfg3: only the baby-step launch was captured.
+NCU_TRAFFIC_BYTES = {
+    "cfg1": 2.420736e6 + 0.256e3 + 32.894976e6 + 5.888e3,      # profiles/r01_ncu_cfg1_solve.txt
+    "cfg2": 60.933376e6 + 93.212416e6 + 137.357568e6 + 6.3488e6,  # profiles/r01_ncu_cfg2_solve.txt
+}
 
 
 def parse_args():
@@ -255,7 +260,10 @@ def measure_workload(torch, cd, workloads, name, args, steps, warmup, flush, sam
         "value": value, "ms_per_step": ms_per_step, "ms_per_solve": ms_per_step / w.units,
         "tflops_step": world * w.units * steps * flops / (total_ms * 1e-3) * 1e-12,
         "flops_per_solve": flops, "gpu_launches_per_step": w.launches_per_step,
-        "roofline": {"bound": "tensor", "kernel": "gemm_dmma_kernel (persistent grouped FP64 DMMA GEMM, all products of one solve)",
+        "roofline": {"bound": "tensor",
+                     "kernel": ("gemm_dmma_kernel (persistent grouped FP64 DMMA GEMM: baby steps) + giant_resident_kernel (giant steps, "
+                                "multiplier resident in shared memory)") if plan.opts.giant == 2 else
+                               "gemm_dmma_kernel (persistent grouped FP64 DMMA GEMM, all products of one solve)",
                      "achieved": achieved, "peak": peak_tf, "unit": "TFLOP/s", "frac": achieved / peak_tf if peak_tf else None,
                      "traffic": NCU_TRAFFIC_BYTES.get(name), "kernel_ms": kernel_ms, "launches_timed": n_rec,
                      "kernel_share_of_step": (kernel_ms * w.units) / ms_per_step if ms_per_step > 0 else None,
@@ -375,6 +383,11 @@ def main():
         k_steps = max(2, min(args.steps, 5 if big else 10))
         others.append(measure_workload(torch, cd, workloads, name, args, k_steps, 3, flush, sampler, dist, peak_tf, world))
     peak_after = cd.dmma_peak(40000, st)
+    # sustained DMMA peak: the same microbenchmark back to back for ~2 s (clocks settle under the power cap)
+    t_end = time.perf_counter() + 2.0
+    peak_sustained = peak_after
+    while time.perf_counter() < t_end:
+        peak_sustained = cd.dmma_peak(400000, st)
 
     if rank == 0:
         clocks = sampler.summary() if sampler else None
@@ -398,7 +411,8 @@ def main():
             "gpu_launches": main_res["gpu_launches_per_step"] * args.steps,
             "roofline": dict(main_res["roofline"],
                              peak_source="cheb_dm_dmma_peak: live register-resident DMMA.8x8x4 microbenchmark on this GPU (MEASURED_PEAKS.json has no FP64 entry)",
-                             peak_after_run=peak_after,
+                             peak_after_run=peak_after, peak_sustained=peak_sustained,
+                             frac_of_sustained=(main_res["roofline"]["achieved"] / peak_sustained) if peak_sustained else None,
                              peak_alt_bf16_ratio=(peaks.get("bf16_tflops") or 0) * 40.0 / 2250.0 or None),
             "clocks": clocks,
             "mu": main_res["mu"], "tr_D": main_res["tr_D"], "mu_search_ms": main_res["mu_search_ms"],
