@@ -26,7 +26,7 @@ namespace {
 typedef GemmCfg<128, 128, 32, 32, 16, 4, 1> Cfg128x128;   // 16 consumer warps, 128 KB ring, 1 CTA/SM
 typedef GemmCfg<128, 64, 32, 32, 16, 4, 2> Cfg128x64;     //  8 consumer warps,  96 KB ring, 2 CTA/SM
 typedef GemmCfg<64, 64, 32, 32, 16, 6, 3> Cfg64x64;       //  4 consumer warps,  96 KB ring, 2 CTA/SM (smem)
-typedef GemmCfg<64, 32, 16, 16, 32, 6, 1> Cfg64x32w16;    //  8 consumer warps of 16x16, 144 KB ring, 1 CTA/SM
+typedef GemmCfg<64, 32, 16, 16, 32, 8, 1> Cfg64x32w16;    //  8 consumer warps of 16x16, 192 KB ring, 1 CTA/SM
 typedef GemmCfg<64, 32, 32, 16, 32, 6, 1> Cfg64x32w32;    //  4 consumer warps of 32x16, 144 KB ring, 1 CTA/SM
 typedef GemmCfg<128, 64, 32, 16, 16, 6, 1> Cfg128x64w16;  // 16 consumer warps of 32x16, 144 KB ring, 1 CTA/SM
 typedef GemmCfg<32, 32, 16, 16, 32, 6, 2> Cfg32x32;       //  4 consumer warps of 16x16,  96 KB ring, 2 CTA/SM
@@ -591,14 +591,6 @@ cheb_dm_status_t cheb_dm_plan_ex(cheb_dm_plan_t* plan, int N, int M_terms, cheb_
     choose_tile(P);
     P->ld = ((long long)N + 15) / 16 * 16;
     P->mat_elems = (((size_t)N * (size_t)P->ld) + 127) / 128 * 128;
-    // a-5: fused (epilogue reads T_1..T_{k-1}: p (k-1) mat bytes per solve) while the baby block stays L2-resident,
-    // pre-formed (form_sums_kernel: (ceil(p/16) (k-1) + p) mat bytes) once it does not.
-    {
-        int mode = o.fuse_sums;
-        if (mode == 0) mode = ((double)k * (double)P->mat_elems * 8.0 > 96.0 * 1024 * 1024 && k > 2 && p > 1) ? 2 : 1;
-        P->preformed = (mode == 2) ? 1 : 0;
-        P->opt.fuse_sums = mode;
-    }
     // Giant steps in the resident-multiplier kernel: N <= 512 (32 rows of T_k fit in shared memory), operand maps
     // with BK = 32 and 2-slab boxes (the 64x32 / 32x32 tile shapes), grouped scheduling, at least one product.
     P->resident = 0;
@@ -615,6 +607,18 @@ cheb_dm_status_t cheb_dm_plan_ex(cheb_dm_plan_t* plan, int N, int M_terms, cheb_
         cudaGetLastError();
     }
     P->opt.giant = P->resident ? 2 : 1;
+    // a-5: fused (epilogue reads T_1..T_{k-1}: p (k-1) mat bytes per solve) while the baby block stays L2-resident,
+    // pre-formed (form_sums_kernel: (ceil(p/16) (k-1) + p) mat bytes) once it does not.
+    {
+        int mode = o.fuse_sums;
+        if (mode == 0) mode = ((double)k * (double)P->mat_elems * 8.0 > 96.0 * 1024 * 1024 && k > 2 && p > 1) ? 2 : 1;
+        P->preformed = (mode == 2) ? 1 : 0;
+        P->opt.fuse_sums = mode;
+    }
+    if (P->resident) {  // the resident kernel forms the sums itself (each CTA its own tiles) and parks them in G_l
+        P->preformed = 1;
+        P->opt.fuse_sums = 2;
+    }
     P->nmat = k + 2 + (P->preformed ? p : 0);
     P->ws = nullptr; P->costab = P->fn = P->c = P->gT = P->dT = P->Amat = P->tau = P->w = P->dots = P->one = P->part = nullptr;
     P->sc = nullptr; P->maps = nullptr; P->tasks = nullptr; P->task_first = nullptr; P->counters = nullptr;
@@ -838,6 +842,12 @@ cheb_dm_status_t run_giant_resident(cheb_dm_plan_s* P, double* userD, long long 
     ga.error_flag = P->counters + P->off_error;
     ga.trace = P->trace_on ? P->trace_buf : nullptr;
     ga.trace_base = P->h_first.back();
+    ga.coefT = (P->opt.outer == CHEB_DM_OUTER_POWER) ? P->dT : P->gT;
+    ga.Tbase = T_ptr(P, 1);
+    ga.Gbase = G_ptr(P, 0);
+    ga.mat_stride = (long long)P->mat_elems;
+    ga.ld = P->ld;
+    ga.k = P->k;
     void* args[] = {(void*)&ga};
     CUDA_TRY(cudaLaunchCooperativeKernel((const void*)giant_resident_kernel, dim3(P->res_grid), dim3(GR_THREADS), args,
                                          (size_t)P->res_smem, st));
@@ -864,7 +874,11 @@ cheb_dm_status_t cheb_dm_compute(cheb_dm_plan_t P, const double* dH, double* dD,
     if (s != CHEB_DM_OK) return s;
     const int slot = (int)(P->ev_count % TIMING_SLOTS);
     if (P->timing) CUDA_TRY(cudaEventRecord(P->ev0[slot], st));
-    if (P->preformed) {
+    if (P->resident) {
+        s = run_tasks(P, 0, P->nbaby, dD, P->N, st);
+        if (s != CHEB_DM_OK) return s;
+        s = run_giant_resident(P, dD, P->N, st);
+    } else if (P->preformed) {
         s = run_tasks(P, 0, P->nbaby, dD, P->N, st);
         if (s != CHEB_DM_OK) return s;
         const long long pairs = (long long)P->N * P->ld / 2;
@@ -874,11 +888,7 @@ cheb_dm_status_t cheb_dm_compute(cheb_dm_plan_t P, const double* dH, double* dD,
                                                                               P->p, coefT, G_ptr(P, 0));
         ++P->last_launches;
         CUDA_TRY(cudaGetLastError());
-        s = P->resident ? run_giant_resident(P, dD, P->N, st) : run_tasks(P, P->nbaby, P->ntasks_solve, dD, P->N, st);
-    } else if (P->resident) {
-        s = run_tasks(P, 0, P->nbaby, dD, P->N, st);
-        if (s != CHEB_DM_OK) return s;
-        s = run_giant_resident(P, dD, P->N, st);
+        s = run_tasks(P, P->nbaby, P->ntasks_solve, dD, P->N, st);
     } else {
         s = run_tasks(P, 0, P->ntasks_solve, dD, P->N, st);
     }

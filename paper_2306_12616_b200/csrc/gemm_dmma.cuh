@@ -468,10 +468,6 @@ __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MIN_CTAS) gemm_dmma_kernel(
         int prev_stage = -1;
         for (int kt = 0; kt < ktiles; ++kt) {
             mbar_wait(full_bar(stage), phase);
-            if (prev_stage >= 0) {
-                __syncwarp();
-                if (lane == 0) mbar_arrive(empty_bar(prev_stage));
-            }
             if (tracing && kt == 0) t_first = global_ns();
             if (Cfg::EARLY_C && kt == 0 && Cp != nullptr) {
 #pragma unroll
@@ -491,6 +487,10 @@ __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MIN_CTAS) gemm_dmma_kernel(
 #pragma unroll
                 for (int i = 0; i < FN; ++i)
                     b[i] = *reinterpret_cast<const double*>(sbase + ((boff[par] ^ ((i & 1) << 6)) + (i >> 1) * SLAB_BYTES + jh * 1024));
+                if (j == 0 && prev_stage >= 0) {  // previous stage back to the producer (after this stage's barrier, off the
+                    __syncwarp();                 // path from the barrier to the first loads)
+                    if (lane == 0) mbar_arrive(empty_bar(prev_stage));
+                }
 #pragma unroll
                 for (int im = 0; im < FM; ++im)
 #pragma unroll
