@@ -114,6 +114,7 @@ __device__ __forceinline__ double fermi_scaled(double beta_t, double mu_t, doubl
 // For small N the launch gaps of five separate kernels were ~10 % of a whole solve (cfg1: 39 us of 400 us).
 // HBM bytes as bounds_rescale_kernel: 8N^2 read (+ 8N^2 re-read, L2 for small N) + 8N^2 written.
 // ---------------------------------------------------------------------------------------------------
+constexpr int FRONT_SMEM_COEFS = 4608;  // 36 KB: covers k p up to 4608 (all configs; larger plans read c from L2)
 struct FrontArgs {
     const double* H;
     int N;
@@ -279,14 +280,21 @@ __global__ void __launch_bounds__(512) front_end_kernel(const FrontArgs A) {
     if (blockIdx.x != 0) return;
     {
         const int k = A.k, p = A.p;
-        const double* c = A.c;
-        for (int l = threadIdx.x; l < p; l += blockDim.x) A.gT[(size_t)l * k] = __ldcg(c + (size_t)l * k);
+        // stage c in shared memory when it fits (one coalesced pass instead of 2p dependent L2 round trips per thread)
+        __shared__ double s_c[FRONT_SMEM_COEFS];
+        const bool staged = (k * p <= FRONT_SMEM_COEFS);
+        if (staged) {
+            for (int e = threadIdx.x; e < k * p; e += blockDim.x) s_c[e] = __ldcg(A.c + e);
+            __syncthreads();
+        }
+        const double* c = staged ? s_c : A.c;
+        for (int l = threadIdx.x; l < p; l += blockDim.x) A.gT[(size_t)l * k] = c[(size_t)l * k];
         // pairs (i, k-i), 1 <= i <= k/2 (i == k-i when k is even and i = k/2)
         for (int i = 1 + threadIdx.x; 2 * i <= k; i += blockDim.x) {
             const int i2 = k - i;
             double g1 = 0.0, g2 = 0.0;  // g_{i,l+1}, g_{k-i,l+1}
             for (int l = p - 1; l >= 0; --l) {
-                const double c1 = __ldcg(c + (size_t)l * k + i), c2 = __ldcg(c + (size_t)l * k + i2);
+                const double c1 = c[(size_t)l * k + i], c2 = c[(size_t)l * k + i2];
                 double n1, n2;
                 if (p == 1) { n1 = c1; n2 = c2; }
                 else if (l == p - 1) { n1 = 2.0 * c1; n2 = 2.0 * c2; }

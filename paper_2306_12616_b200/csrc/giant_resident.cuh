@@ -197,16 +197,16 @@ __global__ void __launch_bounds__(GR_THREADS, 1) giant_resident_kernel(const Gia
                 const bool in0 = (srow0 < N) && (c < N), in1 = (srow0 + 8 < N) && (c < N);
                 const double* src = args.Tbase + (long long)srow0 * ld + c;
                 int i = 1;
-                for (; i + 3 < k; i += 4) {  // four operands (8 loads) in flight
-                    double2 v[4][2];
+                for (; i + 4 < k; i += 5) {  // five operands (10 loads) in flight
+                    double2 v[5][2];
 #pragma unroll
-                    for (int u = 0; u < 4; ++u) {
+                    for (int u = 0; u < 5; ++u) {
                         const double* pu = src + (long long)(i - 1 + u) * args.mat_stride;
                         v[u][0] = in0 ? __ldcg(reinterpret_cast<const double2*>(pu)) : make_double2(0.0, 0.0);
                         v[u][1] = in1 ? __ldcg(reinterpret_cast<const double2*>(pu + 8 * ld)) : make_double2(0.0, 0.0);
                     }
 #pragma unroll
-                    for (int u = 0; u < 4; ++u)
+                    for (int u = 0; u < 5; ++u)
 #pragma unroll
                         for (int q = 0; q < GR_SUM_CHUNK; ++q) {
                             const double w = s_coef[(i + u) * GR_SUM_CHUNK + q];
