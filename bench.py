@@ -36,8 +36,8 @@ FLUSH_BYTES = 512 << 20  # > 126 MB L2
 # Sum over the product launches of one solve (baby-step launch + giant-step launch).  ncu replays with cold caches, so
 # for cfg1/cfg2 (working set L2-resident when warm) this is an upper bound.  cfg3: only the baby-step launch was captured.
 NCU_TRAFFIC_BYTES = {
-    "cfg1": 2.420736e6 + 0.256e3 + 32.894976e6 + 5.888e3,      # profiles/r01_ncu_cfg1_solve.txt
-    "cfg2": 60.933376e6 + 93.212416e6 + 137.357568e6 + 6.3488e6,  # profiles/r01_ncu_cfg2_solve.txt
+    "cfg1": 2.460416e6 + 0.002304e6 + 32.952576e6 + 1.85728e6,       # profiles/r01_ncu_cfg1_solve.txt (baby + giant launch)
+    "cfg2": 61.915136e6 + 94.35008e6 + 137.581568e6 + 5.511936e6,     # profiles/r01_ncu_cfg2_solve.txt (two solve launches)
 }
 
 
