@@ -88,8 +88,9 @@ typedef struct {
                       giant-step epilogues from T_1..T_{k-1} (no extra workspace; p(k-1) N^2 8 bytes of reads per
                       solve, L2 hits while the baby block fits L2); 2 = all p sums formed in one batched pass
                       (form_sums_kernel: each T_i read ceil(p/16) times, p extra workspace matrices), the
-                      epilogues then add one tile.  auto = 2 when k N^2 8 B > 96 MiB.  Neither mode makes the
-                      per-term AXPY passes of PAPER.md:234.                                              */
+                      epilogues then add one tile.  auto = 2 when k N^2 8 B > 96 MiB.  With the resident giant-step
+                      kernel (giant = 2) the sums are always formed inside that kernel by the CTA that consumes
+                      them (reported as 2).  No mode makes the per-term AXPY passes of PAPER.md:234.          */
     int giant;   /* giant steps at N <= 512: 0 = auto, 1 = generic grouped kernel, 2 = resident-multiplier kernel (each
                     CTA keeps its 32 rows of T_k in shared memory for all p-1 products and runs two column
                     panels as independent chains; needs tile 4, 5 or 7 and grouped scheduling, else falls back) */
@@ -97,7 +98,8 @@ typedef struct {
 } cheb_dm_options_t;
 
 /* Create a plan for N x N matrices and an M_terms-term expansion.  Chooses (k,p), allocates the
- * workspace ((k+2) padded matrices + scalar tables) and builds the product/tile/dependency tables.
+ * workspace ((k+2) padded matrices, + p when the low-order sums are parked, + scalar tables) and builds the
+ * product/tile/dependency tables.
  * plan: host pointer, receives the handle.  EINVAL: N<1, M_terms<1, k*p<M; EUNSUPPORTED: dtype. */
 cheb_dm_status_t cheb_dm_plan(cheb_dm_plan_t* plan, int N, int M_terms, cheb_dm_dtype_t dtype);
 /* Same with explicit options (host pointer; NULL = defaults). */
@@ -194,7 +196,8 @@ cheb_dm_status_t cheb_dm_flops_per_compute(cheb_dm_plan_t plan, double* flops_ou
 
 /* Measurement support (bench.py's roofline object).
  * cheb_dm_set_timing(plan, 1): every following cheb_dm_compute() records a CUDA event on its stream
- *   directly before and after the launch(es) of the product kernel (one launch in GROUPED mode).
+ *   directly before and after the launches of the product kernels (GROUPED mode: one persistent launch, or
+ *   baby-step launch + [form_sums_kernel] + giant-step launch).
  *   The plan keeps a ring of 256 event pairs, so up to 256 computes can be in flight unsynchronised.
  * cheb_dm_product_ms: waits for the recorded computes (the last min(count, 256) since timing was
  *   switched on) and returns how many there were and the SUM of their product-launch durations in

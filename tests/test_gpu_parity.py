@@ -366,3 +366,30 @@ def test_trace_kernel():
         torch.cuda.synchronize()
         assert abs(out.item() - float(np.sum(np.diag(A).astype(np.longdouble)))) <= 1e-13 * n
         plan.destroy()
+
+
+def test_trace_records_and_resolved_options():
+    """Tracing aid (cheb_dm_set_trace / cheb_dm_get_trace) and cheb_dm_get_options: one record per work item with
+    ordered timestamps; tracing does not change the result."""
+    oracle, cd, workloads, gu, oc = _imports()
+    torch = gu.torch_cuda()
+    case = oc.case("cfg1", 0, 300, None)
+    for giant in (1, 2):
+        r = gu.gpu_solve(case["H"], case["beta"], case["mu"], case["M"], giant=giant, keep_plan=True)
+        plan, dH = r["plan"], r["dH"]
+        assert plan.opts.giant == giant and plan.opts.k == plan.k and plan.opts.tile == 4 and plan.opts.fuse_sums in (1, 2)
+        st = torch.cuda.current_stream().cuda_stream
+        dD = torch.empty_like(dH)
+        plan.set_trace(True)
+        plan.compute(dH.data_ptr(), dD.data_ptr(), st)
+        torch.cuda.synchronize()
+        recs = plan.get_trace()
+        assert np.array_equal(dD.cpu().numpy(), r["D"])
+        nbaby_items = (plan.k - 1) * 5 * 10        # 64x32 tiles of a 300x300 product
+        ngiant_items = plan.p * (10 * 10 if giant == 2 else 5 * 10)
+        assert len(recs) == nbaby_items + ngiant_items
+        for rec in recs:
+            assert 0 < rec["t_desc"] <= rec["t_kend"] <= rec["t_done"]
+            assert 0 <= rec["sm"] < 200
+        plan.set_trace(False)
+        plan.destroy()
