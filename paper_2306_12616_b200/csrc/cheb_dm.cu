@@ -30,9 +30,10 @@ typedef GemmCfg<64, 32, 16, 16, 32, 8, 1> Cfg64x32w16;    //  8 consumer warps o
 typedef GemmCfg<64, 32, 32, 16, 32, 6, 1> Cfg64x32w32;    //  4 consumer warps of 32x16, 144 KB ring, 1 CTA/SM
 typedef GemmCfg<128, 64, 32, 16, 16, 6, 1> Cfg128x64w16;  // 16 consumer warps of 32x16, 144 KB ring, 1 CTA/SM
 typedef GemmCfg<32, 32, 16, 16, 32, 6, 2> Cfg32x32;       //  4 consumer warps of 16x16,  96 KB ring, 2 CTA/SM
+typedef GemmCfg<112, 64, 16, 32, 16, 6, 1> Cfg112x64;     // 14 consumer warps of 16x32, 132 KB ring, 1 CTA/SM (N ~ 1000: 144 tiles)
 
 enum TileSel { TILE_AUTO = 0, TILE_128x128 = 1, TILE_128x64 = 2, TILE_64x64 = 3, TILE_64x32_W16 = 4, TILE_64x32_W32 = 5,
-               TILE_128x64_W16 = 6, TILE_32x32 = 7, TILE_LAST = 7 };
+               TILE_128x64_W16 = 6, TILE_32x32 = 7, TILE_112x64 = 8, TILE_LAST = 8 };
 
 struct TileShape {
     int BM, BN, BK, box_slabs;
@@ -51,6 +52,7 @@ TileShape tile_shape(int sel) {
         case TILE_64x32_W16: return shape_of<Cfg64x32w16>(0.70);
         case TILE_64x32_W32: return shape_of<Cfg64x32w32>(0.65);
         case TILE_32x32: return shape_of<Cfg32x32>(0.60);
+        case TILE_112x64: return shape_of<Cfg112x64>(0.72);  // 14 consumer warps: two sub-partitions carry 4, two carry 3
         default: return shape_of<Cfg128x64w16>(0.80);
     }
 }
@@ -214,9 +216,9 @@ void choose_tile(cheb_dm_plan_s* P) {
         // One product is the unit of the serial chain (giant steps), so pick the shape that minimises the time of
         // one product on this device: tiles per SM (whole waves, 1 CTA per SM) x tile area / main-loop efficiency.
         // Large N -> 128x128 (least L2 traffic per flop); N ~ 1000 -> 128x64; N ~ 500 -> 64x32 (128 tiles).
-        const int cand[3] = {TILE_128x128, TILE_128x64_W16, TILE_64x32_W16};
+        const int cand[4] = {TILE_128x128, TILE_128x64_W16, TILE_112x64, TILE_64x32_W16};
         double best = 0.0;
-        for (int c = 0; c < 3; ++c) {
+        for (int c = 0; c < 4; ++c) {
             const TileShape t = tile_shape(cand[c]);
             const int tiles = ceil_div(P->N, t.BM) * ceil_div(P->N, t.BN);
             const double cost = (double)ceil_div(tiles, P->num_sms) * t.BM * t.BN / t.eff;
@@ -492,6 +494,7 @@ cheb_dm_status_t launch_tasks(cheb_dm_plan_s* P, int t0, int t1, int use_deps, i
         case TILE_64x32_W16: return launch_cfg<Cfg64x32w16>(la, items, P->num_sms, st);
         case TILE_64x32_W32: return launch_cfg<Cfg64x32w32>(la, items, P->num_sms, st);
         case TILE_32x32: return launch_cfg<Cfg32x32>(la, items, P->num_sms, st);
+        case TILE_112x64: return launch_cfg<Cfg112x64>(la, items, P->num_sms, st);
         default: return launch_cfg<Cfg128x64w16>(la, items, P->num_sms, st);
     }
 }

@@ -94,7 +94,8 @@ struct GemmCfg {
     static constexpr int CONSUMER_THREADS = CONSUMER_WARPS * 32;
     static constexpr int THREADS = CONSUMER_THREADS + 64;        // + producer warp + publisher warp
     static constexpr int SLAB_BYTES = BK * 128;                  // one 16-column slab: BK rows x 128 B
-    static constexpr int BOX_SLABS = (BM < BN ? BM : BN) >= 64 ? 4 : (BM < BN ? BM : BN) / 16;  // slabs per TMA box
+    // slabs per TMA box: the largest of 4, 2, 1 that divides both operand tiles (one tensor map serves both operands)
+    static constexpr int BOX_SLABS = ((BM / 16) % 4 == 0 && (BN / 16) % 4 == 0) ? 4 : (((BM / 16) % 2 == 0 && (BN / 16) % 2 == 0) ? 2 : 1);
     static constexpr int BOX_BYTES = BOX_SLABS * SLAB_BYTES;
     static constexpr int A_BYTES = BM * BK * 8, B_BYTES = BN * BK * 8;
     static constexpr int STAGE_BYTES = A_BYTES + B_BYTES;
