@@ -54,6 +54,7 @@ def parse_args():
     ap.add_argument("--tile", type=int, default=0)
     ap.add_argument("--fuse", type=int, default=0, help="fuse_sums option of the plan (0 auto, 1 epilogue-fused, 2 pre-formed)")
     ap.add_argument("--giant", type=int, default=0, help="giant option of the plan (0 auto, 1 generic, 2 resident-multiplier kernel)")
+    ap.add_argument("--symmetric", type=int, default=0, help="symmetric-tile skipping (0 auto = on, 1 off, 2 on)")
     ap.add_argument("--k", type=int, default=0)
     ap.add_argument("--p", type=int, default=0)
     return ap.parse_args()
@@ -143,7 +144,7 @@ class Workload:
         self.cfg = cfg = workloads.CONFIGS[name]
         self.N, self.M = cfg.N, cfg.M
         self.st = torch.cuda.current_stream().cuda_stream
-        self.plan = cd.Plan(cfg.N, cfg.M, sched=args.sched, tile=args.tile, k=args.k, p=args.p, fuse_sums=args.fuse, giant=args.giant)
+        self.plan = cd.Plan(cfg.N, cfg.M, sched=args.sched, tile=args.tile, k=args.k, p=args.p, fuse_sums=args.fuse, giant=args.giant, symmetric=args.symmetric)
         self.hH, self.dH, self.dD, self.hD = [], [], [], []
         for seed in cfg.seeds:
             H = torch.from_numpy(workloads.hamiltonian(name, seed=seed))

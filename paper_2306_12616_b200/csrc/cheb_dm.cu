@@ -30,10 +30,11 @@ typedef GemmCfg<64, 32, 16, 16, 32, 8, 1> Cfg64x32w16;    //  8 consumer warps o
 typedef GemmCfg<64, 32, 32, 16, 32, 6, 1> Cfg64x32w32;    //  4 consumer warps of 32x16, 144 KB ring, 1 CTA/SM
 typedef GemmCfg<128, 64, 32, 16, 16, 6, 1> Cfg128x64w16;  // 16 consumer warps of 32x16, 144 KB ring, 1 CTA/SM
 typedef GemmCfg<32, 32, 16, 16, 32, 6, 2> Cfg32x32;       //  4 consumer warps of 16x16,  96 KB ring, 2 CTA/SM
+typedef GemmCfg<64, 64, 32, 16, 32, 6, 1> Cfg64x64w16;     //  8 consumer warps of 32x16, 192 KB ring, 1 CTA/SM
 typedef GemmCfg<112, 64, 16, 32, 16, 6, 1> Cfg112x64;     // 14 consumer warps of 16x32, 132 KB ring, 1 CTA/SM (N ~ 1000: 144 tiles)
 
 enum TileSel { TILE_AUTO = 0, TILE_128x128 = 1, TILE_128x64 = 2, TILE_64x64 = 3, TILE_64x32_W16 = 4, TILE_64x32_W32 = 5,
-               TILE_128x64_W16 = 6, TILE_32x32 = 7, TILE_112x64 = 8, TILE_LAST = 8 };
+               TILE_128x64_W16 = 6, TILE_32x32 = 7, TILE_112x64 = 8, TILE_64x64_W16 = 9, TILE_LAST = 9 };
 
 struct TileShape {
     int BM, BN, BK, box_slabs;
@@ -52,6 +53,7 @@ TileShape tile_shape(int sel) {
         case TILE_64x32_W16: return shape_of<Cfg64x32w16>(0.70);
         case TILE_64x32_W32: return shape_of<Cfg64x32w32>(0.65);
         case TILE_32x32: return shape_of<Cfg32x32>(0.60);
+        case TILE_64x64_W16: return shape_of<Cfg64x64w16>(0.76);
         case TILE_112x64: return shape_of<Cfg112x64>(0.72);  // 14 consumer warps: two sub-partitions carry 4, two carry 3
         default: return shape_of<Cfg128x64w16>(0.80);
     }
@@ -94,6 +96,8 @@ struct cheb_dm_plan_s {
     double *costab, *fn, *c, *gT, *dT, *Amat, *tau, *w, *dots, *one, *part;
     int front_grid;      // blocks of the cooperative front_end_kernel
     int preformed;       // 1: low-order sums G_l are formed by form_sums_kernel before the giant steps
+    int sym;             // 1: symmetric-tile skipping in gemm_dmma_kernel
+    int* sym_first;      // device: [tiles_n + 1] item prefix sums of a symmetric task
     int resident;        // 1: giant steps run in giant_resident_kernel (small N), baby steps in gemm_dmma_kernel
     int res_tiles_m, res_tiles_n, res_grid, res_smem;
     DevScalars* sc;
@@ -209,6 +213,19 @@ namespace {
 
 int ceil_div(int a, int b) { return (a + b - 1) / b; }
 
+// Work items of a product whose result is symmetric: tile (tm, tn) is computed iff it touches the lower triangle,
+// tm BM + BM - 1 >= tn BN, i.e. tm >= floor(tn BN / BM); the rest is filled by mirror stores.
+int sym_tm0(int tn, int BM, int BN) { return (tn * BN) / BM; }
+int sym_items(int N, int BM, int BN) {
+    const int tiles_m = ceil_div(N, BM), tiles_n = ceil_div(N, BN);
+    int n = 0;
+    for (int tn = 0; tn < tiles_n; ++tn) {
+        const int tm0 = sym_tm0(tn, BM, BN);
+        if (tm0 < tiles_m) n += tiles_m - tm0;
+    }
+    return n;
+}
+
 void choose_tile(cheb_dm_plan_s* P) {
     int sel = P->opt.tile;
     if (sel < TILE_AUTO || sel > TILE_LAST) sel = TILE_AUTO;
@@ -216,11 +233,15 @@ void choose_tile(cheb_dm_plan_s* P) {
         // One product is the unit of the serial chain (giant steps), so pick the shape that minimises the time of
         // one product on this device: tiles per SM (whole waves, 1 CTA per SM) x tile area / main-loop efficiency.
         // Large N -> 128x128 (least L2 traffic per flop); N ~ 1000 -> 128x64; N ~ 500 -> 64x32 (128 tiles).
-        const int cand[4] = {TILE_128x128, TILE_128x64_W16, TILE_112x64, TILE_64x32_W16};
+        // With symmetric-tile skipping only the lower-triangle tiles count (N <= 512: the giant steps run in the
+        // resident kernel and the tile shape only serves the throughput-bound baby phase: full count, as measured).
+        const int cand[5] = {TILE_128x128, TILE_128x64_W16, TILE_112x64, TILE_64x64_W16, TILE_64x32_W16};
         double best = 0.0;
-        for (int c = 0; c < 4; ++c) {
+        for (int c = 0; c < 5; ++c) {
             const TileShape t = tile_shape(cand[c]);
-            const int tiles = ceil_div(P->N, t.BM) * ceil_div(P->N, t.BN);
+            const bool count_sym = P->sym && P->N > 32 * GR_MAX_KTILES;
+            if (cand[c] == TILE_64x64_W16 && !count_sym) continue;
+            const int tiles = count_sym ? sym_items(P->N, t.BM, t.BN) : ceil_div(P->N, t.BM) * ceil_div(P->N, t.BN);
             const double cost = (double)ceil_div(tiles, P->num_sms) * t.BM * t.BN / t.eff;
             if (sel == TILE_AUTO || cost < best) {
                 sel = cand[c];
@@ -243,6 +264,8 @@ Task blank_task(const cheb_dm_plan_s* P) {
     t.ktiles = ceil_div(P->N, P->BK);
     t.tiles_m = ceil_div(P->N, P->BM);
     t.tiles_n = ceil_div(P->N, P->BN);
+    t.sym = 0;
+    t.nitems = t.tiles_m * t.tiles_n;
     t.alpha = 1.0;
     t.lds = P->ld;
     t.sum_stride = (long long)P->mat_elems;
@@ -266,6 +289,8 @@ void build_tasks(cheb_dm_plan_s* P) {
     T.clear();
     const int tiles = ceil_div(P->N, P->BM) * ceil_div(P->N, P->BN);
     const int tiles_m = ceil_div(P->N, P->BM);
+    // every matrix of the solve is a polynomial of X, hence symmetric: lower-triangle tiles only (option symmetric)
+    const int stiles = P->sym ? sym_items(P->N, P->BM, P->BN) : tiles;
 
     // ---- baby steps: T_n = 2 T_l T_r - T_m (Eq. 7 / 22-23 / Algorithm 1) ----
     std::vector<BabyProd> sched = baby_schedule(k, P->opt.pairing);
@@ -292,13 +317,15 @@ void build_tasks(cheb_dm_plan_s* P) {
             if (n < 2) continue;
             bool dup = false;
             for (int e = 0; e < d; ++e) dup = dup || (deps[e] == n);
-            if (!dup) add_dep(t, DEP_TASK, task_of[n], tiles);
+            if (!dup) add_dep(t, DEP_TASK, task_of[n], stiles);
         }
+        t.sym = P->sym;
+        t.nitems = stiles;
         task_of[bp.n] = (int)T.size();
         T.push_back(t);
     }
     P->nbaby = (int)T.size();
-    const int baby_tiles = P->nbaby * tiles;
+    const int baby_tiles = P->nbaby * stiles;
 
     // ---- giant steps ----
     // CHEBYSHEV: B_l = G_l + 2 Y B_{l+1} - B_{l+2} (l = p-1..1), D = G_0 + Y B_1 - B_2, G_l = sum_i g_{i,l} T_i.
@@ -346,7 +373,15 @@ void build_tasks(cheb_dm_plan_s* P) {
         // early: the baby block (operands of the low-order sum); late: the same column panel of the previous step
         if (P->nbaby > 0) add_dep(t, DEP_GROUP, GROUP_BABY, baby_tiles);
         t.ndeps_early = t.ndeps;
-        if (has_prod) add_dep(t, DEP_PANEL_N, (int)T.size() - 1, tiles_m);
+        // (symmetric tiles: a panel also receives mirrored blocks from the tiles of other panels, so the step waits
+        // for the whole previous step; the resident kernel keeps full tiles and panel chains)
+        if (P->sym && !P->resident) {
+            t.sym = 1;
+            t.nitems = stiles;
+            if (has_prod) add_dep(t, DEP_TASK, (int)T.size() - 1, stiles);
+        } else if (has_prod) {
+            add_dep(t, DEP_PANEL_N, (int)T.size() - 1, tiles_m);
+        }
         T.push_back(t);
     }
     (void)first_giant;
@@ -395,10 +430,10 @@ void build_tasks(cheb_dm_plan_s* P) {
     }
 
     P->h_first.assign(T.size() + 1, 0);
-    for (size_t i = 0; i < T.size(); ++i) P->h_first[i + 1] = P->h_first[i] + T[i].tiles_m * T[i].tiles_n;
+    for (size_t i = 0; i < T.size(); ++i) P->h_first[i + 1] = P->h_first[i] + T[i].nitems;
 
-    double nprod = 0;
-    for (int i = 0; i < P->ntasks_solve; ++i) nprod += (T[i].ktiles > 0) ? 1.0 : 0.0;
+    double nprod = 0;  // executed products, counting only the tiles that are computed
+    for (int i = 0; i < P->ntasks_solve; ++i) nprod += (T[i].ktiles > 0) ? (double)T[i].nitems / (double)tiles : 0.0;
     P->flops_per_compute = nprod * 2.0 * (double)P->N * (double)P->N * (double)P->N;
 }
 
@@ -483,6 +518,7 @@ cheb_dm_status_t launch_tasks(cheb_dm_plan_s* P, int t0, int t1, int use_deps, i
     la.userD = userD;
     la.ldD = ldD;
     la.tma2d = P->tma2d;
+    la.sym_first = P->sym_first;
     la.error_flag = P->counters + P->off_error;
     la.trace = P->trace_on ? P->trace_buf : nullptr;
     const int items = P->h_first[t1] - P->h_first[t0];
@@ -495,6 +531,7 @@ cheb_dm_status_t launch_tasks(cheb_dm_plan_s* P, int t0, int t1, int use_deps, i
         case TILE_64x32_W32: return launch_cfg<Cfg64x32w32>(la, items, P->num_sms, st);
         case TILE_32x32: return launch_cfg<Cfg32x32>(la, items, P->num_sms, st);
         case TILE_112x64: return launch_cfg<Cfg112x64>(la, items, P->num_sms, st);
+        case TILE_64x64_W16: return launch_cfg<Cfg64x64w16>(la, items, P->num_sms, st);
         default: return launch_cfg<Cfg128x64w16>(la, items, P->num_sms, st);
     }
 }
@@ -534,6 +571,7 @@ cheb_dm_status_t cheb_dm_destroy(cheb_dm_plan_t P) {
     cudaFree(P->dots);
     cudaFree(P->one);
     cudaFree(P->part);
+    cudaFree(P->sym_first);
     cudaFree(P->sc);
     cudaFree(P->maps);
     cudaFree(P->tasks);
@@ -564,6 +602,7 @@ cheb_dm_status_t cheb_dm_plan_ex(cheb_dm_plan_t* plan, int N, int M_terms, cheb_
     if (o.pairing != CHEB_DM_PAIR_ALG1 && o.pairing != CHEB_DM_PAIR_SERIAL) return CHEB_DM_EINVAL;
     if (o.fuse_sums < 0 || o.fuse_sums > 2) return CHEB_DM_EINVAL;
     if (o.giant < 0 || o.giant > 2) return CHEB_DM_EINVAL;
+    if (o.symmetric < 0 || o.symmetric > 2) return CHEB_DM_EINVAL;
     int k = o.k, p = o.p;
     if (k == 0 && p == 0) {
         k = 1;
@@ -591,6 +630,9 @@ cheb_dm_status_t cheb_dm_plan_ex(cheb_dm_plan_t* plan, int N, int M_terms, cheb_
     int nq = 1;
     while (nq < 4 * M_terms) nq <<= 1;  // N_q = 2^ceil(log2(4M)) (cheb_dm.h)
     P->Nq = nq;
+    P->sym = (o.symmetric != 1) ? 1 : 0;
+    P->opt.symmetric = P->sym ? 2 : 1;
+    P->sym_first = nullptr;
     choose_tile(P);
     P->ld = ((long long)N + 15) / 16 * 16;
     P->mat_elems = (((size_t)N * (size_t)P->ld) + 127) / 128 * 128;
@@ -688,6 +730,16 @@ cheb_dm_status_t cheb_dm_plan_ex(cheb_dm_plan_t* plan, int N, int M_terms, cheb_
             cudaMemcpy(P->Amat, A.data(), sizeof(double) * A.size(), cudaMemcpyHostToDevice) != cudaSuccess) {
             st = CHEB_DM_ECUDA;
             break;
+        }
+        {
+            const int tn_ = ceil_div(N, P->BN), tm_ = ceil_div(N, P->BM);
+            std::vector<int> pf(tn_ + 1, 0);
+            for (int tn = 0; tn < tn_; ++tn) {
+                const int tm0 = sym_tm0(tn, P->BM, P->BN);
+                pf[tn + 1] = pf[tn] + (tm0 < tm_ ? tm_ - tm0 : 0);
+            }
+            if (cudaMalloc(&P->sym_first, sizeof(int) * pf.size()) != cudaSuccess) { cudaGetLastError(); st = CHEB_DM_EALLOC; break; }
+            if (cudaMemcpy(P->sym_first, pf.data(), sizeof(int) * pf.size(), cudaMemcpyHostToDevice) != cudaSuccess) { st = CHEB_DM_ECUDA; break; }
         }
         st = encode_maps(P);
         if (st != CHEB_DM_OK) break;

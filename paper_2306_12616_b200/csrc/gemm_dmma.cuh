@@ -39,6 +39,9 @@ struct Task {
     int mapA, mapB;
     int ktiles;
     int tiles_m, tiles_n;
+    int sym;                 // 1: the result is symmetric (every operand is a polynomial of X): only the tiles that touch
+                             // the lower triangle are work items, each mirrors its blocks into the skipped tiles
+    int nitems;              // work items of this task (tiles_m * tiles_n, or the lower-triangle count when sym)
     int group;               // group whose counter this task's tiles increment
     int out_is_user;         // Out = the user's D (pointer/ld come from the launch parameters)
     int ndeps;
@@ -80,6 +83,7 @@ struct LaunchArgs {
     double* userD;
     long long ldD;
     int tma2d;               // 1: operand maps are 2-D {column, row} with one 16-column box per copy
+    const int* sym_first;    // [tiles_n + 1] prefix sums of the per-panel item counts of a symmetric task
     int* error_flag;         // set to 1 if a dependency wait exceeds the watchdog (never in a correct run)
     TraceRec* trace;         // nullable: per-item timeline, indexed by the global item number
 };
@@ -239,8 +243,19 @@ __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MIN_CTAS) gemm_dmma_kernel(
                     tk = args.tasks + cur;
                     const int local = item - args.task_first[cur];
                     const int tiles_m = tk->tiles_m;
-                    tn = local / tiles_m;  // column-panel-major order: a panel's tiles are consecutive
-                    tm = local - tn * tiles_m;
+                    if (!tk->sym) {
+                        tn = local / tiles_m;  // column-panel-major order: a panel's tiles are consecutive
+                        tm = local - tn * tiles_m;
+                    } else {
+                        // symmetric task: panel tn holds the tiles tm >= floor(tn BN / BM); find the panel by bisection
+                        int lo = 0, hi = tk->tiles_n;
+                        while (hi - lo > 1) {
+                            const int mid = (lo + hi) >> 1;
+                            if (__ldg(args.sym_first + mid) <= local) lo = mid; else hi = mid;
+                        }
+                        tn = lo;
+                        tm = (tn * BN) / BM + (local - __ldg(args.sym_first + tn));
+                    }
                     // early dependencies: operands of the low-order sum, which the consumers read before the K loop
                     if (args.use_deps)
                         for (int d = 0; d < tk->ndeps_early; ++d) wait_dep(tk, d, tn);
@@ -598,6 +613,36 @@ __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MIN_CTAS) gemm_dmma_kernel(
                         } else {
                             __stcg(p, acc[i][j][0]);
                             if (c + 1 < N) __stcg(p + 1, acc[i][j][1]);
+                        }
+                    }
+                }
+            }
+            if (tk->sym) {
+                // Mirror: an 8x8 block whose transposed position falls into a tile that is not a work item (tile
+                // (tm', tn') with tm' BM + BM - 1 < tn' BN, i.e. strictly above the diagonal) is transposed inside the
+                // warp with shuffles and stored there, row-contiguous like the direct store.  Lane (g, t) of the
+                // transposed block holds C[2t][g], C[2t+1][g], which live in lanes (2t, g>>1) and (2t+1, g>>1).
+                const int src0 = (2 * t) * 4 + (g >> 1), src1 = src0 + 4;
+#pragma unroll
+                for (int i = 0; i < FM; ++i) {
+                    const int R0 = ti.tm * BM + wm * Cfg::WM + i * 8;  // rows of the block
+#pragma unroll
+                    for (int j = 0; j < FN; ++j) {
+                        const int C0 = ti.tn * BN + wn * Cfg::WN + j * 8;  // columns of the block
+                        if ((C0 / BM) * BM + BM - 1 < (R0 / BN) * BN) {   // warp-uniform
+                            const double a0 = __shfl_sync(0xffffffffu, acc[i][j][0], src0), a1 = __shfl_sync(0xffffffffu, acc[i][j][1], src0);
+                            const double b0 = __shfl_sync(0xffffffffu, acc[i][j][0], src1), b1 = __shfl_sync(0xffffffffu, acc[i][j][1], src1);
+                            const double w0 = (g & 1) ? a1 : a0, w1 = (g & 1) ? b1 : b0;
+                            const int rr = C0 + g, cc = R0 + 2 * t;  // transposed position: row C0+g, columns R0+2t, R0+2t+1
+                            if (rr < N && cc < N) {
+                                double* p = Out + (long long)rr * ldo + cc;
+                                if (vec && cc + 1 < N) {
+                                    __stcg(reinterpret_cast<double2*>(p), make_double2(w0, w1));
+                                } else {
+                                    __stcg(p, w0);
+                                    if (cc + 1 < N) __stcg(p + 1, w1);
+                                }
+                            }
                         }
                     }
                 }

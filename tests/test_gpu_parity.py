@@ -385,11 +385,33 @@ def test_trace_records_and_resolved_options():
         torch.cuda.synchronize()
         recs = plan.get_trace()
         assert np.array_equal(dD.cpu().numpy(), r["D"])
-        nbaby_items = (plan.k - 1) * 5 * 10        # 64x32 tiles of a 300x300 product
-        ngiant_items = plan.p * (10 * 10 if giant == 2 else 5 * 10)
+        # 64x32 tiles of a 300x300 product: 5 x 10, of which 30 touch the lower triangle (symmetric-tile skipping);
+        # the resident giant-step kernel works on all 10 x 10 tiles of 32x32
+        nbaby_items = (plan.k - 1) * 30
+        ngiant_items = plan.p * (10 * 10 if giant == 2 else 30)
         assert len(recs) == nbaby_items + ngiant_items
         for rec in recs:
             assert 0 < rec["t_desc"] <= rec["t_kend"] <= rec["t_done"]
             assert 0 <= rec["sm"] < 200
         plan.set_trace(False)
         plan.destroy()
+
+
+@pytest.mark.parametrize("tile,n", [(0, 300), (0, 257), (1, 700), (6, 333), (8, 500), (9, 641), (3, 200), (7, 129)])
+def test_symmetric_tile_skipping(tile, n):
+    """Section 8(f)-3: only the tiles touching the lower triangle are computed, the rest is mirrored.  Same D as the full
+    computation up to rounding, symmetric, parity with the oracle unchanged."""
+    oracle, cd, workloads, gu, oc = _imports()
+    H = workloads.hamiltonian("cfg1", seed=1, n=n)
+    a, b = oracle.gershgorin(H)
+    M = 40
+    c = oracle.cheb_coeffs(40.0, 0.05, a, b, M)
+    D_or = oracle.dm_cheb(H, a, b, c)
+    on = gu.gpu_solve(H, 40.0, 0.05, M, tile=tile, symmetric=2, giant=1)
+    off = gu.gpu_solve(H, 40.0, 0.05, M, tile=tile, symmetric=1, giant=1)
+    assert np.max(np.abs(on["D"] - D_or)) <= TOL_D
+    assert np.max(np.abs(off["D"] - D_or)) <= TOL_D
+    assert np.max(np.abs(on["D"] - off["D"])) <= 1e-13
+    assert np.max(np.abs(on["D"] - on["D"].T)) <= 1e-14   # mirrored blocks exactly, diagonal tiles to rounding
+    res = gu.gpu_solve(H, 40.0, 0.05, M, tile=tile, symmetric=2)   # default giant kernel for this size
+    assert np.max(np.abs(res["D"] - D_or)) <= TOL_D
