@@ -459,8 +459,11 @@ __global__ void __launch_bounds__(1024) mu_bisect_kernel(DevScalars* sc, double 
 //   grid = (ceil(pairs / 256), ceil(p / SUMS_CHUNK)), block = 256.
 // ---------------------------------------------------------------------------------------------------
 constexpr int SUMS_CHUNK = 16;
+// With symmetric-tile skipping (symBM > 0) only the elements inside tiles that are work items of the giant steps are
+// formed (tile (tm, tn) of symBM x symBN with tm symBM + symBM - 1 >= tn symBN): the other tiles of G_l are never read.
 __global__ void __launch_bounds__(256) form_sums_kernel(const double* __restrict__ Tbase, long long stride, long long ld, int N, int k,
-                                                        int p, const double* __restrict__ coefT, double* __restrict__ Gbase) {
+                                                        int p, const double* __restrict__ coefT, double* __restrict__ Gbase,
+                                                        int symBM, int symBN) {
     extern __shared__ double s_coef[];  // [k][SUMS_CHUNK]
     const int l0 = blockIdx.y * SUMS_CHUNK;
     const int nl = min(SUMS_CHUNK, p - l0);
@@ -474,6 +477,7 @@ __global__ void __launch_bounds__(256) form_sums_kernel(const double* __restrict
     if (pr >= pairs) return;
     const long long e0 = 2 * pr;
     const int row = (int)(e0 / ld), col = (int)(e0 - (long long)row * ld);
+    if (symBM > 0 && (row / symBM) * symBM + symBM - 1 < (col / symBN) * symBN) return;  // tile not needed
     double2 acc[SUMS_CHUNK];
 #pragma unroll
     for (int q = 0; q < SUMS_CHUNK; ++q) acc[q] = make_double2(0.0, 0.0);

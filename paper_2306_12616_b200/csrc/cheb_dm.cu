@@ -940,7 +940,7 @@ cheb_dm_status_t cheb_dm_compute(cheb_dm_plan_t P, const double* dH, double* dD,
         dim3 grid((unsigned)((pairs + 255) / 256), (unsigned)ceil_div(P->p, SUMS_CHUNK));
         const double* coefT = (P->opt.outer == CHEB_DM_OUTER_POWER) ? P->dT : P->gT;
         form_sums_kernel<<<grid, 256, sizeof(double) * P->k * SUMS_CHUNK, st>>>(T_ptr(P, 1), (long long)P->mat_elems, P->ld, P->N, P->k,
-                                                                              P->p, coefT, G_ptr(P, 0));
+                                                                              P->p, coefT, G_ptr(P, 0), P->sym ? P->BM : 0, P->BN);
         ++P->last_launches;
         CUDA_TRY(cudaGetLastError());
         s = run_tasks(P, P->nbaby, P->ntasks_solve, dD, P->N, st);
