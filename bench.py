@@ -36,8 +36,9 @@ FLUSH_BYTES = 512 << 20  # > 126 MB L2
 # Sum over the product launches of one solve (baby-step launch + giant-step launch).  ncu replays with cold caches, so
 # for cfg1/cfg2 (working set L2-resident when warm) this is an upper bound.  cfg3: only the baby-step launch was captured.
 NCU_TRAFFIC_BYTES = {
-    "cfg1": 2.460416e6 + 0.002304e6 + 32.952576e6 + 1.85728e6,       # profiles/r01_ncu_cfg1_solve.txt (baby + giant launch)
-    "cfg2": 61.915136e6 + 94.35008e6 + 137.581568e6 + 5.511936e6,     # profiles/r01_ncu_cfg2_solve.txt (two solve launches)
+    "cfg1": 2.46656e6 + 0.002816e6 + 32.949504e6 + 1.789696e6,       # profiles/r01_ncu_cfg1_solve.txt (baby + giant launch)
+    "cfg2": 76.389888e6 + 3.767296e6 + 28.077056e6 + 75.798784e6 + 63.846912e6 + 15.08352e6,  # r01_ncu_cfg2_solve.txt
+    "cfg4": (3.075629 + 1.700576 + 3.804724 + 1.680546 + 2.296236 + 0.709022) * 1e9,        # r01_ncu_cfg4_solve.txt
 }
 
 
@@ -406,7 +407,8 @@ def main():
                        "N": cfg.N, "M_terms": cfg.M, "k": main_res["k"], "p": main_res["p"], "solves_per_step": main_res["solves_per_step"],
                        "parallelism": "replicas only (one plan per GPU, no collective)" if world > 1 else "1 GPU",
                        "l2": "flushed between timed steps (512 MiB device memset outside the event brackets)",
-                       "bounds": "Gershgorin on the device", "sched": "grouped persistent kernel" if args.sched == 0 else "serial launches"},
+                       "bounds": "Gershgorin on the device", "symmetric_tiles": bool(args.symmetric != 1),
+                       "flops": "executed tensor flops only (lower-triangle tiles when symmetric_tiles)", "sched": "grouped persistent kernel" if args.sched == 0 else "serial launches"},
             "ms_per_solve": main_res["ms_per_solve"], "tflops": main_res["tflops_step"],
             "e2e": {k: main_res["e2e"][k] for k in ("value", "unit", "h2d_bytes_per_step", "d2h_bytes_per_step")},
             "gpu_launches": main_res["gpu_launches_per_step"] * args.steps,
