@@ -433,7 +433,11 @@ void build_tasks(cheb_dm_plan_s* P) {
     for (size_t i = 0; i < T.size(); ++i) P->h_first[i + 1] = P->h_first[i] + T[i].nitems;
 
     double nprod = 0;  // executed products, counting only the tiles that are computed
-    for (int i = 0; i < P->ntasks_solve; ++i) nprod += (T[i].ktiles > 0) ? (double)T[i].nitems / (double)tiles : 0.0;
+    const double res_frac = P->sym ? (double)(P->res_tiles_m + 1) / (2.0 * P->res_tiles_m) : 1.0;  // 32x32 lower-triangle tiles
+    for (int i = 0; i < P->ntasks_solve; ++i) {
+        if (T[i].ktiles <= 0) continue;
+        nprod += (P->resident && i >= P->nbaby) ? res_frac : (double)T[i].nitems / (double)tiles;
+    }
     P->flops_per_compute = nprod * 2.0 * (double)P->N * (double)P->N * (double)P->N;
 }
 
@@ -640,7 +644,7 @@ cheb_dm_status_t cheb_dm_plan_ex(cheb_dm_plan_t* plan, int N, int M_terms, cheb_
     // with BK = 32 and 2-slab boxes (the 64x32 / 32x32 tile shapes), grouped scheduling, at least one product.
     P->resident = 0;
     P->res_tiles_m = P->res_tiles_n = ceil_div(N, 32);
-    P->res_grid = P->res_tiles_m * ceil_div(P->res_tiles_n, 2);
+    P->res_grid = P->sym ? (P->res_tiles_m * (P->res_tiles_m + 1)) / 2 : P->res_tiles_m * ceil_div(P->res_tiles_n, 2);
     P->res_smem = giant_resident_smem_bytes(ceil_div(N, GR_BK));
     if (o.giant != 1 && N <= 32 * GR_MAX_KTILES && p >= 2 && P->BK == GR_BK && P->box_slabs == 2 &&
         o.sched == CHEB_DM_SCHED_GROUPED && P->res_grid <= P->num_sms) {
@@ -903,6 +907,7 @@ cheb_dm_status_t run_giant_resident(cheb_dm_plan_s* P, double* userD, long long 
     ga.mat_stride = (long long)P->mat_elems;
     ga.ld = P->ld;
     ga.k = P->k;
+    ga.sym = P->sym;
     void* args[] = {(void*)&ga};
     CUDA_TRY(cudaLaunchCooperativeKernel((const void*)giant_resident_kernel, dim3(P->res_grid), dim3(GR_THREADS), args,
                                          (size_t)P->res_smem, st));
@@ -1001,9 +1006,13 @@ cheb_dm_status_t cheb_dm_get_trace(cheb_dm_plan_t P, cheb_dm_trace_rec_t* out, i
     CUDA_TRY(cudaMemcpy(out, P->trace_buf, sizeof(TraceRec) * (size_t)n, cudaMemcpyDeviceToHost));
     if (P->resident) {  // followed by the tiles of the resident giant-step kernel
         int m = P->p * P->res_tiles_m * P->res_tiles_n;
-        if (m > max_records - n) m = max_records - n;
-        CUDA_TRY(cudaMemcpy(out + n, P->trace_buf + P->h_first.back(), sizeof(TraceRec) * (size_t)m, cudaMemcpyDeviceToHost));
-        n += m;
+        std::vector<TraceRec> tmp((size_t)m);
+        CUDA_TRY(cudaMemcpy(tmp.data(), P->trace_buf + P->h_first.back(), sizeof(TraceRec) * (size_t)m, cudaMemcpyDeviceToHost));
+        for (int i = 0; i < m && n < max_records; ++i)
+            if (tmp[i].t_done != 0) {  // tiles above the diagonal are not work items in symmetric mode
+                memcpy(out + n, &tmp[i], sizeof(TraceRec));
+                ++n;
+            }
     }
     *count_out = n;
     return CHEB_DM_OK;

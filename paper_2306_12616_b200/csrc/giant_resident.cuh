@@ -52,6 +52,8 @@ struct GiantArgs {
     double* Gbase;           // G_0; G_l at Gbase + l * mat_stride
     long long mat_stride, ld;
     int k;
+    int sym;                 // 1: symmetric-tile skipping: grid = lower-triangle tiles (tm >= tn), one tile per CTA, the
+                             // tile is mirrored into (tn, tm), a step waits for the whole previous step
 };
 
 inline int giant_resident_smem_bytes(int ktiles) {
@@ -86,15 +88,27 @@ __global__ void __launch_bounds__(GR_THREADS, 1) giant_resident_kernel(const Gia
     }
     __syncthreads();
 
-    const int tm = blockIdx.x % args.tiles_m;
-    const int pair = blockIdx.x / args.tiles_m;
+    // tile assignment: full mode -> row block tm, panels 2 pair + {0, 1}; symmetric mode -> one lower-triangle tile
+    int tm, pair, tn_sym = 0;
+    if (!args.sym) {
+        tm = blockIdx.x % args.tiles_m;
+        pair = blockIdx.x / args.tiles_m;
+    } else {
+        int b = blockIdx.x;
+        while (b >= args.tiles_m - tn_sym) { b -= args.tiles_m - tn_sym; ++tn_sym; }  // panel-major: panel tn holds tm = tn..T-1
+        tm = tn_sym + b;
+        pair = 0;
+    }
+    const int tn_of[2] = {args.sym ? tn_sym : 2 * pair, args.sym ? args.tiles_n : 2 * pair + 1};  // panel of group g (>= tiles_n: none)
+    const int dep_target = args.sym ? (args.tiles_m * (args.tiles_m + 1)) / 2 : args.tiles_m;
     const int N = args.N;
     const int nsteps = args.nsteps;
 
     if (warp >= GR_CONSUMER_WARPS) {
         // =============================== producer warp of panel g ===============================
         const int g = warp - GR_CONSUMER_WARPS;
-        const int tn = 2 * pair + g;
+        const int tn = tn_of[g];
+        const int ctr = args.sym ? 0 : tn;  // symmetric mode: one counter per step (every tile feeds every panel)
         if (lane != 0) return;
         if (g == 0) {
             // resident A: rows [tm*32, tm*32+32) of Y = T_k as [k][column] blocks (Y is symmetric)
@@ -119,7 +133,7 @@ __global__ void __launch_bounds__(GR_THREADS, 1) giant_resident_kernel(const Gia
             const int ti = args.first_task + s;
             const Task* tk = args.tasks + ti;
             if (tk->ktiles > 0) {
-                wait_counter(args.panel_done + (size_t)(ti - 1) * args.panel_stride + tn, args.tiles_m, args.error_flag);
+                wait_counter(args.panel_done + (size_t)(ti - 1) * args.panel_stride + ctr, dep_target, args.error_flag);
                 fence_proxy_async();
                 const CUtensorMap* mapB = args.maps + tk->mapB;
                 if (s <= 2) fence_tensormap_acquire(mapB);  // the two ping-pong buffers alternate as operand B
@@ -140,7 +154,7 @@ __global__ void __launch_bounds__(GR_THREADS, 1) giant_resident_kernel(const Gia
             // tile visible device-wide, then the panel counter is bumped
             mbar_wait(stored_bar(g), (uint32_t)(s & 1));
             fence_acq_rel_gpu();
-            red_relaxed_gpu_add(args.panel_done + (size_t)ti * args.panel_stride + tn, 1);
+            red_relaxed_gpu_add(args.panel_done + (size_t)ti * args.panel_stride + ctr, 1);
         }
         return;
     }
@@ -165,10 +179,10 @@ __global__ void __launch_bounds__(GR_THREADS, 1) giant_resident_kernel(const Gia
         boff[par] = wn * GR_SLAB_BYTES + lo;
     }
     const int row0 = tm * GR_BM + wm * 16 + gq;
-    const int npanels = (2 * pair + 1 < args.tiles_n) ? 2 : 1;
+    const int npanels = (tn_of[1] < args.tiles_n) ? 2 : 1;
     int colp[2];
-    colp[0] = (2 * pair) * GR_BN + wn * 16 + 2 * t;
-    colp[1] = (2 * pair + 1) * GR_BN + wn * 16 + 2 * t;
+    colp[0] = tn_of[0] * GR_BN + wn * 16 + 2 * t;
+    colp[1] = tn_of[1] * GR_BN + wn * 16 + 2 * t;
     const bool tracing = (args.trace != nullptr) && threadIdx.x == 0;
     const long long ld = args.ld;
     double* scratch = reinterpret_cast<double*>(ring0 + 2 * GR_STAGES * GR_TILE_BYTES + 256);  // [2][128 threads][8]
@@ -180,7 +194,7 @@ __global__ void __launch_bounds__(GR_THREADS, 1) giant_resident_kernel(const Gia
         double* s_coef = reinterpret_cast<double*>(ring0);  // [k][GR_SUM_CHUNK]; the rings are idle until step 1
         const int k = args.k;
         const int srow0 = tm * GR_BM + (warp >> 2) * 16 + gq;  // 16 x 8 sub-tile of warp (warp >> 2, warp & 3)
-        const int scol[2] = {(2 * pair) * GR_BN + (warp & 3) * 8 + 2 * t, (2 * pair + 1) * GR_BN + (warp & 3) * 8 + 2 * t};
+        const int scol[2] = {tn_of[0] * GR_BN + (warp & 3) * 8 + 2 * t, tn_of[1] * GR_BN + (warp & 3) * 8 + 2 * t};
         for (int l0 = 0; l0 < nsteps; l0 += GR_SUM_CHUNK) {
             const int nl = min(GR_SUM_CHUNK, nsteps - l0);
             named_bar_sync(1, GR_CONSUMER_WARPS * 32);
@@ -295,7 +309,7 @@ __global__ void __launch_bounds__(GR_THREADS, 1) giant_resident_kernel(const Gia
 #pragma unroll
         for (int g = 0; g < 2; ++g) {
             if (g >= npanels) break;
-            const int tn = 2 * pair + g;
+            const int tn = tn_of[g];
             const int col0 = colp[g];
             unsigned long long t_desc = 0, t_first = 0, t_kend = 0;
             if (tracing) t_desc = global_ns();
@@ -382,6 +396,8 @@ __global__ void __launch_bounds__(GR_THREADS, 1) giant_resident_kernel(const Gia
                         const double2 hi = *reinterpret_cast<const double2*>(sc + (i * 2 + j) * 2);
                         const double o0 = fma(beta, creg[i][j].x, alpha * (acc[i][j][0] + hi.x)) + pre[i][j].x;
                         const double o1 = fma(beta, creg[i][j].y, alpha * (acc[i][j][1] + hi.y)) + pre[i][j].y;
+                        acc[i][j][0] = o0;
+                        acc[i][j][1] = o1;
                         if (r < N && c < N) {
                             double* p = Out + (long long)r * ldo + c;
                             if (vec && c + 1 < N) {
@@ -392,6 +408,30 @@ __global__ void __launch_bounds__(GR_THREADS, 1) giant_resident_kernel(const Gia
                             }
                         }
                     }
+                }
+                if (args.sym && tm > tn) {
+                    // mirror the tile into (tn, tm): every 8x8 block is transposed inside the warp (lane (g, t) of the
+                    // transposed block takes C[2t][g], C[2t+1][g] from lanes (2t, g>>1), (2t+1, g>>1)) and stored
+                    // row-contiguously, like the direct store
+                    const int src0 = (2 * t) * 4 + (gq >> 1), src1 = src0 + 4;
+#pragma unroll
+                    for (int i = 0; i < 2; ++i)
+#pragma unroll
+                        for (int j = 0; j < 2; ++j) {
+                            const double a0 = __shfl_sync(0xffffffffu, acc[i][j][0], src0), a1 = __shfl_sync(0xffffffffu, acc[i][j][1], src0);
+                            const double b0 = __shfl_sync(0xffffffffu, acc[i][j][0], src1), b1 = __shfl_sync(0xffffffffu, acc[i][j][1], src1);
+                            const double w0 = (gq & 1) ? a1 : a0, w1 = (gq & 1) ? b1 : b0;
+                            const int rr = tn * GR_BN + wn * 16 + j * 8 + gq, cc = tm * GR_BM + wm * 16 + i * 8 + 2 * t;
+                            if (rr < N && cc < N) {
+                                double* p = Out + (long long)rr * ldo + cc;
+                                if (vec && cc + 1 < N) {
+                                    __stcg(reinterpret_cast<double2*>(p), make_double2(w0, w1));
+                                } else {
+                                    __stcg(p, w0);
+                                    if (cc + 1 < N) __stcg(p + 1, w1);
+                                }
+                            }
+                        }
                 }
                 __syncwarp();
                 if (lane == 0) mbar_arrive(stored_bar(g));  // hand the publication over to the panel's producer warp

@@ -165,14 +165,16 @@ def test_parity_tiles_and_schedulers(tile, sched):
 
 @pytest.mark.parametrize("giant", [1, 2])
 @pytest.mark.parametrize("fuse", [1, 2])
+@pytest.mark.parametrize("symmetric", [1, 2])
 @pytest.mark.parametrize("cfg,n,outer", [("cfg1", 300, 0), ("cfg1", 257, 0), ("cfg2", 95, 0), ("cfg0", 128, 1), ("cfg1", 33, 0)])
-def test_parity_giant_generic_and_resident(giant, fuse, cfg, n, outer):
+def test_parity_giant_generic_and_resident(giant, fuse, cfg, n, outer, symmetric):
     """a-6: the giant steps in the generic grouped kernel and in the resident-multiplier kernel (N <= 512: T_k rows
     kept in shared memory, two column panels per CTA as independent chains), odd / ragged sizes, odd panel counts."""
     oracle, cd, workloads, gu, oc = _imports()
     case = oc.case(cfg, 0, n, None)
-    r = gu.gpu_solve(case["H"], case["beta"], case["mu"], case["M"], giant=giant, fuse_sums=fuse, outer=outer, keep_plan=True)
-    assert r["plan"].opts.giant == giant
+    r = gu.gpu_solve(case["H"], case["beta"], case["mu"], case["M"], giant=giant, fuse_sums=fuse, outer=outer, symmetric=symmetric,
+                     keep_plan=True)
+    assert r["plan"].opts.giant == giant and r["plan"].opts.symmetric == symmetric
     r["plan"].destroy()
     _check(case, r)
 
@@ -386,9 +388,9 @@ def test_trace_records_and_resolved_options():
         recs = plan.get_trace()
         assert np.array_equal(dD.cpu().numpy(), r["D"])
         # 64x32 tiles of a 300x300 product: 5 x 10, of which 30 touch the lower triangle (symmetric-tile skipping);
-        # the resident giant-step kernel works on all 10 x 10 tiles of 32x32
+        # the resident giant-step kernel works on the 55 lower-triangle tiles of the 10 x 10 tiles of 32x32
         nbaby_items = (plan.k - 1) * 30
-        ngiant_items = plan.p * (10 * 10 if giant == 2 else 30)
+        ngiant_items = plan.p * (55 if giant == 2 else 30)
         assert len(recs) == nbaby_items + ngiant_items
         for rec in recs:
             assert 0 < rec["t_desc"] <= rec["t_kend"] <= rec["t_done"]
@@ -413,5 +415,7 @@ def test_symmetric_tile_skipping(tile, n):
     assert np.max(np.abs(off["D"] - D_or)) <= TOL_D
     assert np.max(np.abs(on["D"] - off["D"])) <= 1e-13
     assert np.max(np.abs(on["D"] - on["D"].T)) <= 1e-14   # mirrored blocks exactly, diagonal tiles to rounding
-    res = gu.gpu_solve(H, 40.0, 0.05, M, tile=tile, symmetric=2)   # default giant kernel for this size
-    assert np.max(np.abs(res["D"] - D_or)) <= TOL_D
+    for sym in (2, 1):                                              # default giant kernel for this size (resident if N <= 512)
+        res = gu.gpu_solve(H, 40.0, 0.05, M, tile=tile, symmetric=sym)
+        assert np.max(np.abs(res["D"] - D_or)) <= TOL_D
+        assert np.max(np.abs(res["D"] - res["D"].T)) <= 1e-14
