@@ -190,6 +190,12 @@ cheb_dm_status_t cheb_dm_solve_mu(cheb_dm_plan_t plan, double beta, double n_occ
 cheb_dm_status_t cheb_dm_product(cheb_dm_plan_t plan, double alpha, const double* dA, const double* dB,
                                  double beta, const double* dC, double* dOut, void* cuda_stream);
 
+/* Synchronises `cuda_stream` and reports what the device flagged during the last compute / moments call:
+ * CHEB_DM_ECUDA if a CUDA error is pending or a dependency wait inside a persistent kernel hit its watchdog (~4 s;
+ * never in a correct run), CHEB_DM_EBOUNDS for non-finite bounds, else CHEB_DM_OK.  cheb_dm_compute_host() performs
+ * the same check before it returns. */
+cheb_dm_status_t cheb_dm_check(cheb_dm_plan_t plan, void* cuda_stream);
+
 /* Bytes of device workspace owned by the plan. */
 cheb_dm_status_t cheb_dm_workspace_bytes(cheb_dm_plan_t plan, size_t* bytes_out);
 

@@ -18,7 +18,7 @@ EXPORTS = [
     "cheb_dm_moments", "cheb_dm_solve_mu", "cheb_dm_product", "cheb_dm_workspace_bytes",
     "cheb_dm_last_launch_count", "cheb_dm_flops_per_compute", "cheb_dm_strerror",
     "cheb_dm_compute_host", "cheb_dm_set_timing", "cheb_dm_product_ms", "cheb_dm_dmma_peak",
-    "cheb_dm_set_trace", "cheb_dm_get_trace", "cheb_dm_get_options",
+    "cheb_dm_set_trace", "cheb_dm_get_trace", "cheb_dm_get_options", "cheb_dm_check",
 ]
 
 
@@ -84,6 +84,7 @@ def lib():
     L.cheb_dm_product_ms.argtypes = [vp, ip, dp]
     L.cheb_dm_dmma_peak.argtypes = [C.c_int, dp, vp]
     L.cheb_dm_get_options.argtypes = [vp, C.POINTER(Options)]
+    L.cheb_dm_check.argtypes = [vp, vp]
     L.cheb_dm_set_trace.argtypes = [vp, C.c_int]
     L.cheb_dm_get_trace.argtypes = [vp, C.POINTER(TraceRec), C.c_int, ip]
     for n in EXPORTS:
@@ -152,6 +153,10 @@ class Plan:
     def compute_host(self, hH: int, hD: int, h_trace: int = 0, stream: int = 0):
         """hH, hD, h_trace: HOST addresses (e.g. of pinned torch tensors / numpy arrays)."""
         _chk(lib().cheb_dm_compute_host(self._h, hH, hD, h_trace or None, stream), "cheb_dm_compute_host")
+
+    def check(self, stream: int = 0):
+        """Synchronise the stream and raise if the device flagged an error during the last compute."""
+        _chk(lib().cheb_dm_check(self._h, stream), "cheb_dm_check")
 
     def set_trace(self, enable: bool):
         _chk(lib().cheb_dm_set_trace(self._h, int(bool(enable))), "cheb_dm_set_trace")

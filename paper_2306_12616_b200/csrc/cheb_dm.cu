@@ -977,7 +977,21 @@ cheb_dm_status_t cheb_dm_compute_host(cheb_dm_plan_t P, const double* hH, double
         CUDA_TRY(cudaMemcpyAsync(h_trace, P->stage_tr, sizeof(double), cudaMemcpyDeviceToHost, st));
     }
     CUDA_TRY(cudaMemcpyAsync(hD, P->stage_D, bytes, cudaMemcpyDeviceToHost, st));
+    return cheb_dm_check(P, cuda_stream);  // synchronises the stream
+}
+
+cheb_dm_status_t cheb_dm_check(cheb_dm_plan_t P, void* cuda_stream) {
+    if (!P) return CHEB_DM_EINVAL;
+    if (!P->computed) return CHEB_DM_ESTATE;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    int flag = 0;
+    DevScalars h;
+    CUDA_TRY(cudaMemcpyAsync(&flag, P->counters + P->off_error, sizeof(int), cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(cudaMemcpyAsync(&h, P->sc, sizeof(h), cudaMemcpyDeviceToHost, st));
     CUDA_TRY(cudaStreamSynchronize(st));
+    CUDA_TRY(cudaGetLastError());
+    if (flag) return CHEB_DM_ECUDA;
+    if (h.bad_bounds) return CHEB_DM_EBOUNDS;
     return CHEB_DM_OK;
 }
 

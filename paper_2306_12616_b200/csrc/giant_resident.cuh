@@ -19,6 +19,12 @@
 // Work assignment is static: CTA b handles row block tm = b % tiles_m and the panels tn = 2 (b / tiles_m) + g,
 // g = 0, 1.  All CTAs must be co-resident (cooperative launch); they synchronise only through the per-panel
 // completion counters of gemm_dmma.cuh.
+//
+// Symmetric mode (args.sym, the default): every B_l is a polynomial of X, hence symmetric, so the grid
+// is the T (T + 1) / 2 lower-triangle tiles (136 at N = 500), ONE tile per CTA.  The CTA still keeps its 32 rows of
+// T_k resident and streams its panel; it mirrors its tile into (tn, tm) with an in-warp shuffle transpose, and because
+// a panel now also receives mirrored blocks from other panels a step waits for the whole previous step (one counter
+// per step).  Half the flops per step and half the sums per CTA: 12.2 -> 8.7 us per giant step at N = 500.
 #pragma once
 #include "gemm_dmma.cuh"
 
@@ -27,7 +33,7 @@ namespace chebdm {
 constexpr int GR_BM = 32, GR_BN = 32, GR_BK = 32, GR_STAGES = 5;
 constexpr int GR_SLAB_BYTES = GR_BK * 128;               // 4 KB: 16 columns x 32 k-rows
 constexpr int GR_TILE_BYTES = 2 * GR_SLAB_BYTES;         // 8 KB: one 32-column operand block of one k-tile
-constexpr int GR_CONSUMER_WARPS = 8;                     // 2 x 4 warps of 16 x 8 on a 32 x 32 tile
+constexpr int GR_CONSUMER_WARPS = 8;                     // 2 k-halves x (2 x 2 warps of 16 x 16) on a 32 x 32 tile
 constexpr int GR_THREADS = (GR_CONSUMER_WARPS + 2) * 32;   // consumer warps + one producer warp per panel
 constexpr int GR_SUM_CHUNK = 16;                         // low-order sums formed per pass over the baby block
 constexpr int GR_MAX_KTILES = 16;                        // N <= 512

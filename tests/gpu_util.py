@@ -28,6 +28,7 @@ def gpu_solve(H, beta, mu, M, bounds=None, keep_plan=False, **opts):
     plan.coeffs(beta, mu, bounds)
     plan.compute(dH.data_ptr(), dD.data_ptr(), st)
     plan.trace(dD.data_ptr(), dtr.data_ptr(), st)
+    plan.check(st)   # no watchdog / bounds flag from the device
     torch.cuda.synchronize()
     out = {"D": dD.cpu().numpy(), "trace": float(dtr.item()), "bounds": plan.get_bounds(st),
            "k": plan.k, "p": plan.p, "launches": plan.last_launch_count()}
