@@ -518,6 +518,80 @@ __global__ void __launch_bounds__(256) form_sums_kernel(const double* __restrict
 }
 
 // ---------------------------------------------------------------------------------------------------
+// a-5, batched form on the tensor cores.  The batched sums are themselves a skinny GEMM,
+//     G[e][l] = sum_i T_i[e] coefT[l][i]        (e = matrix element, K = k - 1, N = p),
+// and the scalar kernel above is bound by the FP64 FMA pipe (2 N^2 (k-1) p flops at 64 FMA/clk/SM: 1.0 ms at cfg4),
+// not by HBM.  Here one warp owns 32 consecutive elements (4 m-blocks of 8) x SUMS_CHUNK sums (2 n-blocks of 8):
+// per k4-step 4 scalar loads per lane (lane (g, t) reads element g of matrix i0 + t: 64-byte segments), 2 coefficient
+// fragments from shared memory and 8 DMMA.8x8x4.  Same skipping of unneeded tiles, same diagonal term.
+//   grid = (ceil(N ld / 32 / 8), ceil(p / SUMS_CHUNK)), block = 256 (8 warps).
+// ---------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) form_sums_dmma_kernel(const double* __restrict__ Tbase, long long stride, long long ld, int N, int k,
+                                                             int p, const double* __restrict__ coefT, double* __restrict__ Gbase,
+                                                             int symBM, int symBN) {
+    extern __shared__ double s_coef[];  // [kpad][SUMS_CHUNK], kpad = (k - 1) rounded up to 4; row i - 1 <-> T_i; + [SUMS_CHUNK] diag
+    const int l0 = blockIdx.y * SUMS_CHUNK;
+    const int nl = min(SUMS_CHUNK, p - l0);
+    const int kk = k - 1, kpad = (kk + 3) & ~3;
+    for (int e = threadIdx.x; e < (kpad + 1) * SUMS_CHUNK; e += blockDim.x) {
+        const int i = e / SUMS_CHUNK, q = e - i * SUMS_CHUNK;  // i == kpad: coefficient of T_0 = I
+        const int src_i = (i == kpad) ? 0 : i + 1;
+        s_coef[e] = (q < nl && (i == kpad || i < kk)) ? coefT[(size_t)(l0 + q) * k + src_i] : 0.0;
+    }
+    __syncthreads();
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, g = lane >> 2, t = lane & 3;
+    const long long total = (long long)N * ld;
+    const long long e0 = ((long long)blockIdx.x * 8 + warp) * 32;
+    if (e0 >= total) return;
+    bool need[4];
+    bool any = false;
+#pragma unroll
+    for (int mb = 0; mb < 4; ++mb) {
+        const long long e = e0 + mb * 8;  // an 8-block never crosses a row (ld is a multiple of 16) nor a tile
+        const int row = (int)(e / ld), col = (int)(e - (long long)row * ld);
+        need[mb] = (e < total) && !(symBM > 0 && (row / symBM) * symBM + symBM - 1 < (col / symBN) * symBN);
+        any = any || need[mb];
+    }
+    if (!any) return;
+    double acc[4][2][2];
+#pragma unroll
+    for (int mb = 0; mb < 4; ++mb)
+#pragma unroll
+        for (int nb = 0; nb < 2; ++nb) acc[mb][nb][0] = acc[mb][nb][1] = 0.0;
+    const double* src = Tbase + e0 + g;
+    for (int i0 = 0; i0 < kpad; i0 += 4) {
+        const int it = min(i0 + t, kk - 1);  // padded k-rows carry a zero coefficient; read a valid matrix
+        const double* ps = src + (long long)it * stride;
+        double a[4], b[2];
+#pragma unroll
+        for (int mb = 0; mb < 4; ++mb) a[mb] = need[mb] ? __ldcs(ps + mb * 8) : 0.0;
+#pragma unroll
+        for (int nb = 0; nb < 2; ++nb) b[nb] = s_coef[(i0 + t) * SUMS_CHUNK + nb * 8 + g];
+#pragma unroll
+        for (int mb = 0; mb < 4; ++mb)
+#pragma unroll
+            for (int nb = 0; nb < 2; ++nb) dmma_884(acc[mb][nb][0], acc[mb][nb][1], a[mb], b[nb]);
+    }
+#pragma unroll
+    for (int mb = 0; mb < 4; ++mb) {
+        if (!need[mb]) continue;
+        const long long e = e0 + mb * 8 + g;
+        const int row = (int)(e / ld), col = (int)(e - (long long)row * ld);
+#pragma unroll
+        for (int nb = 0; nb < 2; ++nb)
+#pragma unroll
+            for (int h = 0; h < 2; ++h) {
+                const int q = nb * 8 + 2 * t + h;
+                if (q < nl) {
+                    double v = acc[mb][nb][h];
+                    if (row == col) v += s_coef[kpad * SUMS_CHUNK + q];
+                    Gbase[(long long)(l0 + q) * stride + e] = v;
+                }
+            }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------
 // Roofline denominator: register-resident DMMA.8x8x4 issue-rate microbenchmark (cheb_dm_dmma_peak).
 // Each warp runs DMMA_PEAK_CHAINS independent accumulator chains; no memory traffic in the loop.
 // ---------------------------------------------------------------------------------------------------

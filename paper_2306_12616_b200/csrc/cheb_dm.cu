@@ -941,11 +941,20 @@ cheb_dm_status_t cheb_dm_compute(cheb_dm_plan_t P, const double* dH, double* dD,
     } else if (P->preformed) {
         s = run_tasks(P, 0, P->nbaby, dD, P->N, st);
         if (s != CHEB_DM_OK) return s;
-        const long long pairs = (long long)P->N * P->ld / 2;
-        dim3 grid((unsigned)((pairs + 255) / 256), (unsigned)ceil_div(P->p, SUMS_CHUNK));
         const double* coefT = (P->opt.outer == CHEB_DM_OUTER_POWER) ? P->dT : P->gT;
-        form_sums_kernel<<<grid, 256, sizeof(double) * P->k * SUMS_CHUNK, st>>>(T_ptr(P, 1), (long long)P->mat_elems, P->ld, P->N, P->k,
-                                                                              P->p, coefT, G_ptr(P, 0), P->sym ? P->BM : 0, P->BN);
+        const char* scalar_sums = getenv("CHEB_DM_SCALAR_SUMS");
+        if (scalar_sums && scalar_sums[0] == '1') {  // FP64-FMA version (ablation)
+            const long long pairs = (long long)P->N * P->ld / 2;
+            dim3 grid((unsigned)((pairs + 255) / 256), (unsigned)ceil_div(P->p, SUMS_CHUNK));
+            form_sums_kernel<<<grid, 256, sizeof(double) * P->k * SUMS_CHUNK, st>>>(T_ptr(P, 1), (long long)P->mat_elems, P->ld, P->N, P->k,
+                                                                                  P->p, coefT, G_ptr(P, 0), P->sym ? P->BM : 0, P->BN);
+        } else {
+            const long long warps = ((long long)P->N * P->ld + 31) / 32;
+            dim3 grid((unsigned)((warps + 7) / 8), (unsigned)ceil_div(P->p, SUMS_CHUNK));
+            const size_t smem = sizeof(double) * (size_t)((((P->k - 1) + 3) & ~3) + 1) * SUMS_CHUNK;
+            form_sums_dmma_kernel<<<grid, 256, smem, st>>>(T_ptr(P, 1), (long long)P->mat_elems, P->ld, P->N, P->k, P->p, coefT,
+                                                           G_ptr(P, 0), P->sym ? P->BM : 0, P->BN);
+        }
         ++P->last_launches;
         CUDA_TRY(cudaGetLastError());
         s = run_tasks(P, P->nbaby, P->ntasks_solve, dD, P->N, st);
