@@ -72,8 +72,10 @@ typedef enum { CHEB_DM_SCHED_GROUPED = 0, CHEB_DM_SCHED_SERIAL = 1 } cheb_dm_sch
 
 /* Operand pairing of the baby steps (any a+b=n is valid by Eq. 7).
  *  CHEB_DM_PAIR_ALG1 (default): Algorithm 1's pairing, ceil(log2 k) stages.
- *  CHEB_DM_PAIR_SERIAL: T_{n+1} = 2 T_1 T_n - T_{n-1} (k-1 serial products; best rounding).    */
-typedef enum { CHEB_DM_PAIR_ALG1 = 0, CHEB_DM_PAIR_SERIAL = 1 } cheb_dm_pairing_t;
+ *  CHEB_DM_PAIR_SERIAL: T_{n+1} = 2 T_1 T_n - T_{n-1} (k-1 serial products; best rounding).
+ *  CHEB_DM_PAIR_BALANCED: T_n = 2 T_ceil(n/2) T_floor(n/2) - T_{0 or 1}: same stages and concurrency as
+ *      Algorithm 1, no long chains through T_{2^j} unless n is a power of two (reading A7b).  */
+typedef enum { CHEB_DM_PAIR_ALG1 = 0, CHEB_DM_PAIR_SERIAL = 1, CHEB_DM_PAIR_BALANCED = 2 } cheb_dm_pairing_t;
 
 typedef struct {
     int k;       /* baby-step block size; 0 = auto: ceil(sqrt(M))                 */

@@ -8,7 +8,7 @@ from . import build as _build
 
 OUTER_CHEBYSHEV, OUTER_POWER = 0, 1
 SCHED_GROUPED, SCHED_SERIAL = 0, 1
-PAIR_ALG1, PAIR_SERIAL = 0, 1
+PAIR_ALG1, PAIR_SERIAL, PAIR_BALANCED = 0, 1, 2
 TILE_AUTO, TILE_128x128, TILE_128x64, TILE_64x64 = 0, 1, 2, 3
 STATUS_NAMES = ["OK", "EINVAL", "EALLOC", "ECUDA", "ESTATE", "EBOUNDS", "EUNSUPPORTED", "ENOCONV"]
 

@@ -163,6 +163,13 @@ std::vector<BabyProd> baby_schedule(int k, int pairing) {
     }
     int nstages = 0;
     while ((1 << nstages) < k) ++nstages;
+    if (pairing == CHEB_DM_PAIR_BALANCED) {
+        // T_n = 2 T_a T_b - T_{a-b}, a = ceil(n/2), b = floor(n/2): same ceil(log2 k) stages and the same concurrency
+        // as Algorithm 1 (stage s yields T_{2^{s-1}+1} .. T_{2^s}), the subtracted term is always T_0 or T_1
+        for (int s = 1; s <= nstages; ++s)
+            for (int n = (1 << (s - 1)) + 1; n <= (1 << s) && n <= k; ++n) v.push_back({n, (n + 1) / 2, n / 2, (n + 1) / 2 - n / 2, s});
+        return v;
+    }
     for (int s = 1; s <= nstages; ++s) {
         if (s == 1) {
             v.push_back({2, 1, 1, 0, 1});
@@ -603,7 +610,7 @@ cheb_dm_status_t cheb_dm_plan_ex(cheb_dm_plan_t* plan, int N, int M_terms, cheb_
     if (o.k < 0 || o.p < 0) return CHEB_DM_EINVAL;
     if (o.outer != CHEB_DM_OUTER_CHEBYSHEV && o.outer != CHEB_DM_OUTER_POWER) return CHEB_DM_EINVAL;
     if (o.sched != CHEB_DM_SCHED_GROUPED && o.sched != CHEB_DM_SCHED_SERIAL) return CHEB_DM_EINVAL;
-    if (o.pairing != CHEB_DM_PAIR_ALG1 && o.pairing != CHEB_DM_PAIR_SERIAL) return CHEB_DM_EINVAL;
+    if (o.pairing != CHEB_DM_PAIR_ALG1 && o.pairing != CHEB_DM_PAIR_SERIAL && o.pairing != CHEB_DM_PAIR_BALANCED) return CHEB_DM_EINVAL;
     if (o.fuse_sums < 0 || o.fuse_sums > 2) return CHEB_DM_EINVAL;
     if (o.giant < 0 || o.giant > 2) return CHEB_DM_EINVAL;
     if (o.symmetric < 0 || o.symmetric > 2) return CHEB_DM_EINVAL;

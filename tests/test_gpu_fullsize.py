@@ -38,3 +38,17 @@ def test_full_size_sampled_columns(cfg, seed):
     rows = cols[:2]
     comm = case["H"][rows, :] @ D - (D[rows, :] @ case["H"])
     assert np.max(np.abs(comm)) <= 1e-9 * max(1.0, np.max(np.abs(case["H"])) * N ** 0.5)
+
+
+def test_cfg4_balanced_pairing_tightens_the_trace():
+    """Reading A7b: with the balanced pairing of the baby steps (same stages and cost as Algorithm 1) the rounding left
+    by Algorithm 1's squaring chains on cfg4 (|dtr| = 7.7e-10 of the 1e-9 gate) drops by two orders of magnitude."""
+    import oracle
+    import gpu_util as gu
+    import oracle_cases as oc
+    case = oc.case("cfg4", 0, None, None, False)
+    r = gu.gpu_solve(case["H"], case["beta"], case["mu"], case["M"], pairing=2)
+    assert abs(r["trace"] - case["trace_cheb_scalar"]) <= 5e-11
+    cols = np.array([0, 777, case["N"] - 1], dtype=np.int32)
+    want = oracle.dm_cheb_columns(case["H"], case["a"], case["b"], case["c"], cols)
+    assert np.max(np.abs(r["D"][:, cols].T - want)) <= 1e-10

@@ -104,7 +104,7 @@ def test_coefficient_tables(M, k, p):
 # ----------------------------------------------------------------------------------------------
 # a-4: baby steps T_2..T_k (Eq. 7, 22-23, Algorithm 1) vs the three-term recurrence of the oracle
 # ----------------------------------------------------------------------------------------------
-@pytest.mark.parametrize("pairing", [0, 1])
+@pytest.mark.parametrize("pairing", [0, 1, 2])
 @pytest.mark.parametrize("k", [2, 3, 5, 8, 11])
 def test_baby_steps_match_three_term_recurrence(k, pairing):
     oracle, cd, workloads, gu, _ = _imports()
