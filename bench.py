@@ -180,9 +180,12 @@ class Workload:
         self.launches_per_step = n
 
     def step_host(self):
+        # the batch of the step through the pipelined host entry point: copies of neighbouring solves overlap the
+        # kernels; every H2D / D2H of the step completes inside the step (cheb_dm_wait)
         for i in range(self.units):
             self.plan.coeffs(self.cfg.beta, self.mu[i], None)
-            self.plan.compute_host(self.hH[i].data_ptr(), self.hD[i].data_ptr(), self.htr[i:].data_ptr(), self.st)
+            self.plan.compute_host_async(self.hH[i].data_ptr(), self.hD[i].data_ptr(), self.htr[i:].data_ptr(), self.st)
+        self.plan.wait(self.st)
 
     def h2d_bytes(self):
         return self.units * 8 * self.N * self.N

@@ -142,6 +142,16 @@ cheb_dm_status_t cheb_dm_compute(cheb_dm_plan_t plan, const double* dH, double* 
 cheb_dm_status_t cheb_dm_compute_host(cheb_dm_plan_t plan, const double* hH, double* hD, double* h_trace,
                                       void* cuda_stream);
 
+/* Pipelined form of cheb_dm_compute_host for a batch of solves on one plan: returns as soon as the work is queued.
+ * The H2D copy of call n+1 and the D2H copies of call n-1 run on two plan-owned copy streams and overlap the kernels
+ * of call n (two device staging slots; the kernels themselves run on `cuda_stream` in call order).  hH must stay
+ * valid and hD / h_trace must not be read until cheb_dm_wait() returns; pinned host memory is needed for the copies
+ * to be asynchronous.  The Fermi parameters are those of the last cheb_dm_coeffs() at the time of the call.
+ * cheb_dm_wait: waits for every queued call and performs cheb_dm_check(). */
+cheb_dm_status_t cheb_dm_compute_host_async(cheb_dm_plan_t plan, const double* hH, double* hD, double* h_trace,
+                                            void* cuda_stream);
+cheb_dm_status_t cheb_dm_wait(cheb_dm_plan_t plan, void* cuda_stream);
+
 /* trace_out[0] <- tr D = sum_i D_ii (electron count, north_star item 4).  dD: device pointer (N*N,
  * ld N).  trace_out: DEVICE pointer (or pinned mapped host memory), 1 double, written
  * asynchronously on the stream in a fixed summation order (bitwise reproducible). */

@@ -19,6 +19,7 @@ EXPORTS = [
     "cheb_dm_last_launch_count", "cheb_dm_flops_per_compute", "cheb_dm_strerror",
     "cheb_dm_compute_host", "cheb_dm_set_timing", "cheb_dm_product_ms", "cheb_dm_dmma_peak",
     "cheb_dm_set_trace", "cheb_dm_get_trace", "cheb_dm_get_options", "cheb_dm_check",
+    "cheb_dm_compute_host_async", "cheb_dm_wait",
 ]
 
 
@@ -85,6 +86,8 @@ def lib():
     L.cheb_dm_dmma_peak.argtypes = [C.c_int, dp, vp]
     L.cheb_dm_get_options.argtypes = [vp, C.POINTER(Options)]
     L.cheb_dm_check.argtypes = [vp, vp]
+    L.cheb_dm_compute_host_async.argtypes = [vp, vp, vp, vp, vp]
+    L.cheb_dm_wait.argtypes = [vp, vp]
     L.cheb_dm_set_trace.argtypes = [vp, C.c_int]
     L.cheb_dm_get_trace.argtypes = [vp, C.POINTER(TraceRec), C.c_int, ip]
     for n in EXPORTS:
@@ -167,6 +170,13 @@ class Plan:
         n = C.c_int()
         _chk(lib().cheb_dm_get_trace(self._h, buf, max_records, C.byref(n)), "cheb_dm_get_trace")
         return [{f: getattr(buf[i], f) for f, _ in TraceRec._fields_} for i in range(n.value)]
+
+    def compute_host_async(self, hH: int, hD: int, h_trace: int = 0, stream: int = 0):
+        """Pipelined compute_host: queue one solve (HOST addresses, pinned); results valid after wait()."""
+        _chk(lib().cheb_dm_compute_host_async(self._h, hH, hD, h_trace or None, stream), "cheb_dm_compute_host_async")
+
+    def wait(self, stream: int = 0):
+        _chk(lib().cheb_dm_wait(self._h, stream), "cheb_dm_wait")
 
     def set_timing(self, enable: bool):
         _chk(lib().cheb_dm_set_timing(self._h, int(bool(enable))), "cheb_dm_set_timing")

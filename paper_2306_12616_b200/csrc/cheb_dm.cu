@@ -125,6 +125,12 @@ struct cheb_dm_plan_s {
     size_t ws_bytes;
     // host-buffer entry point (cheb_dm_compute_host): device staging for H, D and tr D
     double *stage_H, *stage_D, *stage_tr;
+    // pipelined host entry point (cheb_dm_compute_host_async): second staging slot, copy streams, events
+    double *stage_H1, *stage_D1, *stage_tr1;
+    cudaStream_t s_in, s_out;
+    cudaEvent_t ev_in[2], ev_comp[2], ev_out[2];
+    long long n_async;
+    int pipe_ready;
     // optional per-tile timeline (cheb_dm_set_trace)
     TraceRec* trace_buf;
     int trace_on;
@@ -591,6 +597,18 @@ cheb_dm_status_t cheb_dm_destroy(cheb_dm_plan_t P) {
     cudaFree(P->stage_H);
     cudaFree(P->stage_D);
     cudaFree(P->stage_tr);
+    cudaFree(P->stage_H1);
+    cudaFree(P->stage_D1);
+    cudaFree(P->stage_tr1);
+    if (P->pipe_ready) {
+        cudaStreamDestroy(P->s_in);
+        cudaStreamDestroy(P->s_out);
+        for (int i = 0; i < 2; ++i) {
+            cudaEventDestroy(P->ev_in[i]);
+            cudaEventDestroy(P->ev_comp[i]);
+            cudaEventDestroy(P->ev_out[i]);
+        }
+    }
     cudaFree(P->trace_buf);
     for (int i = 0; i < TIMING_SLOTS; ++i) {
         if (P->ev0[i]) cudaEventDestroy(P->ev0[i]);
@@ -681,6 +699,9 @@ cheb_dm_status_t cheb_dm_plan_ex(cheb_dm_plan_t* plan, int N, int M_terms, cheb_
     P->have_coeffs = P->explicit_bounds = P->have_moments = P->computed = 0;
     P->last_launches = 0;
     P->stage_H = P->stage_D = P->stage_tr = nullptr;
+    P->stage_H1 = P->stage_D1 = P->stage_tr1 = nullptr;
+    P->pipe_ready = 0;
+    P->n_async = 0;
     P->timing = 0; P->ev_count = 0;
     P->trace_buf = nullptr; P->trace_on = 0;
     for (int i = 0; i < TIMING_SLOTS; ++i) P->ev0[i] = P->ev1[i] = nullptr;
@@ -994,6 +1015,62 @@ cheb_dm_status_t cheb_dm_compute_host(cheb_dm_plan_t P, const double* hH, double
     }
     CUDA_TRY(cudaMemcpyAsync(hD, P->stage_D, bytes, cudaMemcpyDeviceToHost, st));
     return cheb_dm_check(P, cuda_stream);  // synchronises the stream
+}
+
+cheb_dm_status_t cheb_dm_compute_host_async(cheb_dm_plan_t P, const double* hH, double* hD, double* h_trace, void* cuda_stream) {
+    if (!P || !hH || !hD || hH == hD) return CHEB_DM_EINVAL;
+    if (!P->have_coeffs) return CHEB_DM_ESTATE;
+    if (!device_ok(P)) return CHEB_DM_ECUDA;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const size_t bytes = sizeof(double) * (size_t)P->N * P->N;
+    if (!P->pipe_ready) {
+        bool ok = cudaMalloc(&P->stage_H1, bytes) == cudaSuccess && cudaMalloc(&P->stage_D1, bytes) == cudaSuccess &&
+                  cudaMalloc(&P->stage_tr1, sizeof(double)) == cudaSuccess;
+        if (!ok) { cudaGetLastError(); return CHEB_DM_EALLOC; }
+        CUDA_TRY(cudaStreamCreateWithFlags(&P->s_in, cudaStreamNonBlocking));
+        CUDA_TRY(cudaStreamCreateWithFlags(&P->s_out, cudaStreamNonBlocking));
+        for (int i = 0; i < 2; ++i) {
+            CUDA_TRY(cudaEventCreateWithFlags(&P->ev_in[i], cudaEventDisableTiming));
+            CUDA_TRY(cudaEventCreateWithFlags(&P->ev_comp[i], cudaEventDisableTiming));
+            CUDA_TRY(cudaEventCreateWithFlags(&P->ev_out[i], cudaEventDisableTiming));
+        }
+        P->pipe_ready = 1;
+    }
+    const int slot = (int)(P->n_async & 1);
+    double* sH = slot ? P->stage_H1 : P->stage_H;
+    double* sD = slot ? P->stage_D1 : P->stage_D;
+    double* sT = slot ? P->stage_tr1 : P->stage_tr;
+    // H2D of this call: the slot's previous occupant (call n-2) must have been consumed by its kernels
+    if (P->n_async >= 2) CUDA_TRY(cudaStreamWaitEvent(P->s_in, P->ev_comp[slot], 0));
+    CUDA_TRY(cudaMemcpyAsync(sH, hH, bytes, cudaMemcpyHostToDevice, P->s_in));
+    CUDA_TRY(cudaEventRecord(P->ev_in[slot], P->s_in));
+    // kernels, in call order on the caller's stream: need this call's H and the slot's D / tr copied out (call n-2)
+    CUDA_TRY(cudaStreamWaitEvent(st, P->ev_in[slot], 0));
+    if (P->n_async >= 2) CUDA_TRY(cudaStreamWaitEvent(st, P->ev_out[slot], 0));
+    cheb_dm_status_t s = cheb_dm_compute(P, sH, sD, cuda_stream);
+    if (s != CHEB_DM_OK) return s;
+    if (h_trace) {
+        trace_kernel<<<1, 1024, 0, st>>>(sD, P->N, P->N, sT);
+        ++P->last_launches;
+        CUDA_TRY(cudaGetLastError());
+    }
+    CUDA_TRY(cudaEventRecord(P->ev_comp[slot], st));
+    // D2H of this call
+    CUDA_TRY(cudaStreamWaitEvent(P->s_out, P->ev_comp[slot], 0));
+    if (h_trace) CUDA_TRY(cudaMemcpyAsync(h_trace, sT, sizeof(double), cudaMemcpyDeviceToHost, P->s_out));
+    CUDA_TRY(cudaMemcpyAsync(hD, sD, bytes, cudaMemcpyDeviceToHost, P->s_out));
+    CUDA_TRY(cudaEventRecord(P->ev_out[slot], P->s_out));
+    ++P->n_async;
+    return CHEB_DM_OK;
+}
+
+cheb_dm_status_t cheb_dm_wait(cheb_dm_plan_t P, void* cuda_stream) {
+    if (!P) return CHEB_DM_EINVAL;
+    if (P->pipe_ready) {
+        CUDA_TRY(cudaStreamSynchronize(P->s_in));
+        CUDA_TRY(cudaStreamSynchronize(P->s_out));
+    }
+    return cheb_dm_check(P, cuda_stream);
 }
 
 cheb_dm_status_t cheb_dm_check(cheb_dm_plan_t P, void* cuda_stream) {

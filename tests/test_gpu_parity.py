@@ -419,3 +419,39 @@ def test_symmetric_tile_skipping(tile, n):
         res = gu.gpu_solve(H, 40.0, 0.05, M, tile=tile, symmetric=sym)
         assert np.max(np.abs(res["D"] - D_or)) <= TOL_D
         assert np.max(np.abs(res["D"] - res["D"].T)) <= 1e-14
+
+
+def test_host_entry_points_sync_and_pipelined():
+    """cheb_dm_compute_host and the pipelined cheb_dm_compute_host_async / cheb_dm_wait (batch of 5 solves with
+    different H and mu through two staging slots) give the same D and tr D as the device-resident call."""
+    oracle, cd, workloads, gu, oc = _imports()
+    torch = gu.torch_cuda()
+    n, M = 300, 64
+    Hs = [workloads.hamiltonian("cfg1", seed=s, n=n) for s in range(5)]
+    mus = [0.01 * s for s in range(5)]
+    st = torch.cuda.current_stream().cuda_stream
+    plan = cd.Plan(n, M)
+    ref = []
+    for H, mu in zip(Hs, mus):
+        dH = gu.to_dev(H)
+        dD = torch.empty_like(dH)
+        plan.coeffs(40.0, mu, None)
+        plan.compute(dH.data_ptr(), dD.data_ptr(), st)
+        torch.cuda.synchronize()
+        ref.append(dD.cpu().numpy())
+    hH = [torch.from_numpy(H).pin_memory() for H in Hs]
+    hD = [torch.empty((n, n), dtype=torch.float64).pin_memory() for _ in Hs]
+    htr = torch.zeros(5, dtype=torch.float64).pin_memory()
+    for i in range(5):
+        plan.coeffs(40.0, mus[i], None)
+        plan.compute_host_async(hH[i].data_ptr(), hD[i].data_ptr(), htr[i:].data_ptr(), st)
+    plan.wait(st)
+    for i in range(5):
+        assert np.array_equal(hD[i].numpy(), ref[i])
+        assert abs(float(htr[i]) - float(np.trace(ref[i]))) <= 1e-10
+    out = torch.empty((n, n), dtype=torch.float64).pin_memory()
+    tr1 = torch.zeros(1, dtype=torch.float64).pin_memory()
+    plan.coeffs(40.0, mus[2], None)
+    plan.compute_host(hH[2].data_ptr(), out.data_ptr(), tr1.data_ptr(), st)
+    assert np.array_equal(out.numpy(), ref[2])
+    plan.destroy()
