@@ -36,9 +36,9 @@ FLUSH_BYTES = 512 << 20  # > 126 MB L2
 # Sum over the product launches of one solve (baby-step launch + giant-step launch).  ncu replays with cold caches, so
 # for cfg1/cfg2 (working set L2-resident when warm) this is an upper bound.  cfg3: only the baby-step launch was captured.
 NCU_TRAFFIC_BYTES = {
-    "cfg1": 2.46528e6 + 0.008448e6 + 18.194176e6 + 0.257536e6,       # profiles/r01_ncu_cfg1_solve.txt (baby + giant launch)
-    "cfg2": 76.389888e6 + 3.767296e6 + 28.077056e6 + 75.798784e6 + 63.846912e6 + 15.08352e6,  # r01_ncu_cfg2_solve.txt
-    "cfg4": (3.075629 + 1.700576 + 3.804724 + 1.680546 + 2.296236 + 0.709022) * 1e9,        # r01_ncu_cfg4_solve.txt
+    "cfg1": 2.465792e6 + 0.001024e6 + 18.196992e6 + 0.251136e6,      # profiles/r01_ncu_cfg1_solve.txt (baby + giant launch)
+    "cfg2": 76.390656e6 + 3.9296e6 + 27.222784e6 + 75.980288e6 + 63.959808e6 + 17.564416e6,  # r01_ncu_cfg2_solve.txt
+    "cfg4": (3.107274 + 1.705426 + 3.799804 + 1.681488 + 2.360649 + 0.7121) * 1e9,            # r01_ncu_cfg4_solve.txt
 }
 
 
