@@ -89,7 +89,7 @@ typedef struct {
     int fuse_sums; /* low-order sums G_l / S_j of Eq. (21).  0 = auto; 1 = formed inside the
                       giant-step epilogues from T_1..T_{k-1} (no extra workspace; p(k-1) N^2 8 bytes of reads per
                       solve, L2 hits while the baby block fits L2); 2 = all p sums formed in one batched pass
-                      (form_sums_kernel: each T_i read ceil(p/16) times, p extra workspace matrices), the
+                      (form_sums_dmma_kernel, a skinny GEMM on the tensor cores: each T_i read ceil(p/16) times, p extra workspace matrices), the
                       epilogues then add one tile.  auto = 2 when k N^2 8 B > 96 MiB.  With the resident giant-step
                       kernel (giant = 2) the sums are always formed inside that kernel by the CTA that consumes
                       them (reported as 2).  No mode makes the per-term AXPY passes of PAPER.md:234.          */
