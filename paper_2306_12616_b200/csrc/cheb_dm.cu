@@ -424,9 +424,11 @@ void build_tasks(cheb_dm_plan_s* P) {
         t.ldo = P->ld;
         t.sum_base = T_ptr(P, 1);
         t.dot_count = k - 1;  // <U_{j+1}, T_i> for i = 1..k-1; slot k-1 = tr U_{j+1} (= <U, T_0>)
-        t.dot_out = P->dots + (size_t)(j + 1) * tiles * k;
+        t.dot_out = P->dots + (size_t)(j + 1) * tiles * k;  // slots of skipped tiles stay zero (memset at plan time)
+        t.sym = P->sym;                                     // U_j = T_j(T_k) is symmetric too; dots weight mirrored blocks x2
+        t.nitems = stiles;
         if (P->nbaby > 0) add_dep(t, DEP_GROUP, GROUP_BABY, baby_tiles);
-        if (j >= 2) add_dep(t, DEP_TASK, (int)T.size() - 1, tiles);
+        if (j >= 2) add_dep(t, DEP_TASK, (int)T.size() - 1, stiles);
         T.push_back(t);
     }
     P->ntasks_all = (int)T.size();
@@ -498,22 +500,26 @@ cheb_dm_status_t encode_maps(cheb_dm_plan_s* P) {
     return CHEB_DM_ECUDA;
 }
 
-template <class Cfg>
-cheb_dm_status_t launch_cfg(const LaunchArgs& la, int items, int num_sms, cudaStream_t st) {
+template <class Cfg, bool DOTS>
+cheb_dm_status_t launch_inst(const LaunchArgs& la, int items, int num_sms, cudaStream_t st) {
     static bool attr_set = false;
     if (!attr_set) {
-        CUDA_TRY(cudaFuncSetAttribute(gemm_dmma_kernel<Cfg>, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg::SMEM_BYTES));
+        CUDA_TRY(cudaFuncSetAttribute(gemm_dmma_kernel<Cfg, DOTS>, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg::SMEM_BYTES));
         attr_set = true;
     }
     int per_sm = 1;
-    CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, gemm_dmma_kernel<Cfg>, Cfg::THREADS, Cfg::SMEM_BYTES));
+    CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, gemm_dmma_kernel<Cfg, DOTS>, Cfg::THREADS, Cfg::SMEM_BYTES));
     if (per_sm < 1) return CHEB_DM_ECUDA;
     int grid = per_sm * num_sms;
     if (grid > items) grid = items;
     if (grid < 1) grid = 1;
-    gemm_dmma_kernel<Cfg><<<grid, Cfg::THREADS, Cfg::SMEM_BYTES, st>>>(la);
+    gemm_dmma_kernel<Cfg, DOTS><<<grid, Cfg::THREADS, Cfg::SMEM_BYTES, st>>>(la);
     CUDA_TRY(cudaGetLastError());
     return CHEB_DM_OK;
+}
+template <class Cfg>
+cheb_dm_status_t launch_cfg(const LaunchArgs& la, int items, int num_sms, cudaStream_t st, bool dots) {
+    return dots ? launch_inst<Cfg, true>(la, items, num_sms, st) : launch_inst<Cfg, false>(la, items, num_sms, st);
 }
 
 // Launch tasks [t0, t1) as one persistent grid; `work_slot` selects the work counter.
@@ -540,16 +546,18 @@ cheb_dm_status_t launch_tasks(cheb_dm_plan_s* P, int t0, int t1, int use_deps, i
     la.trace = P->trace_on ? P->trace_buf : nullptr;
     const int items = P->h_first[t1] - P->h_first[t0];
     ++P->last_launches;
+    bool dots = false;  // the moments chain needs the instance whose epilogue forms the Frobenius products
+    for (int t = t0; t < t1; ++t) dots = dots || (P->h_tasks[t].dot_out != nullptr);
     switch (P->tile) {
-        case TILE_128x128: return launch_cfg<Cfg128x128>(la, items, P->num_sms, st);
-        case TILE_128x64: return launch_cfg<Cfg128x64>(la, items, P->num_sms, st);
-        case TILE_64x64: return launch_cfg<Cfg64x64>(la, items, P->num_sms, st);
-        case TILE_64x32_W16: return launch_cfg<Cfg64x32w16>(la, items, P->num_sms, st);
-        case TILE_64x32_W32: return launch_cfg<Cfg64x32w32>(la, items, P->num_sms, st);
-        case TILE_32x32: return launch_cfg<Cfg32x32>(la, items, P->num_sms, st);
-        case TILE_112x64: return launch_cfg<Cfg112x64>(la, items, P->num_sms, st);
-        case TILE_64x64_W16: return launch_cfg<Cfg64x64w16>(la, items, P->num_sms, st);
-        default: return launch_cfg<Cfg128x64w16>(la, items, P->num_sms, st);
+        case TILE_128x128: return launch_cfg<Cfg128x128>(la, items, P->num_sms, st, dots);
+        case TILE_128x64: return launch_cfg<Cfg128x64>(la, items, P->num_sms, st, dots);
+        case TILE_64x64: return launch_cfg<Cfg64x64>(la, items, P->num_sms, st, dots);
+        case TILE_64x32_W16: return launch_cfg<Cfg64x32w16>(la, items, P->num_sms, st, dots);
+        case TILE_64x32_W32: return launch_cfg<Cfg64x32w32>(la, items, P->num_sms, st, dots);
+        case TILE_32x32: return launch_cfg<Cfg32x32>(la, items, P->num_sms, st, dots);
+        case TILE_112x64: return launch_cfg<Cfg112x64>(la, items, P->num_sms, st, dots);
+        case TILE_64x64_W16: return launch_cfg<Cfg64x64w16>(la, items, P->num_sms, st, dots);
+        default: return launch_cfg<Cfg128x64w16>(la, items, P->num_sms, st, dots);
     }
 }
 
@@ -747,6 +755,7 @@ cheb_dm_status_t cheb_dm_plan_ex(cheb_dm_plan_t* plan, int N, int M_terms, cheb_
     cheb_dm_status_t st = CHEB_DM_OK;
     do {
         if (cudaMemset(P->ws, 0, sizeof(double) * P->mat_elems * P->nmat) != cudaSuccess) { st = CHEB_DM_ECUDA; break; }
+        cudaMemset(P->dots, 0, sizeof(double) * ((size_t)(p + 1) * tiles * k + (size_t)2 * k * 16));
         cudaMemset(P->dT, 0, sizeof(double) * kp);
         cudaMemset(P->gT, 0, sizeof(double) * kp);
         cudaMemset(P->c, 0, sizeof(double) * kp);

@@ -154,7 +154,9 @@ __device__ __forceinline__ void wait_counter(const int* ctr, int target, int* er
     }
 }
 
-template <class Cfg>
+// DOTS = true: the instance used by the moments chain (cheb_dm_moments), whose epilogue also forms the Frobenius
+// products; the solve uses the DOTS = false instance, which does not carry that code (and its registers).
+template <class Cfg, bool DOTS>
 __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MIN_CTAS) gemm_dmma_kernel(const LaunchArgs args) {
     constexpr int BM = Cfg::BM, BN = Cfg::BN, BK = Cfg::BK, STAGES = Cfg::STAGES;
     constexpr int FM = Cfg::FM, FN = Cfg::FN;
@@ -650,7 +652,21 @@ __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MIN_CTAS) gemm_dmma_kernel(
         }
         // ------------- moments: Frobenius products <Out, T_i> and tr Out of this tile (reading A10) -------------
         const int nd = tk->dot_count;
-        if (tk->dot_out != nullptr) {
+        if (DOTS && tk->dot_out != nullptr) {
+            if (tk->sym) {
+                // symmetric task: a block whose mirror lies in a skipped tile stands for both in the Frobenius products
+                // (the accumulators are not needed for anything else after the stores; diagonal blocks keep weight 1)
+#pragma unroll
+                for (int i = 0; i < FM; ++i)
+#pragma unroll
+                    for (int j = 0; j < FN; ++j) {
+                        const int R0 = ti.tm * BM + wm * Cfg::WM + i * 8, C0 = ti.tn * BN + wn * Cfg::WN + j * 8;
+                        if ((C0 / BM) * BM + BM - 1 < (R0 / BN) * BN) {
+                            acc[i][j][0] *= 2.0;
+                            acc[i][j][1] *= 2.0;
+                        }
+                    }
+            }
             double* s_red = reinterpret_cast<double*>(smem + Cfg::DOT_OFFSET);
             const long long lds = tk->lds, sstride = tk->sum_stride;
             const double* sb = tk->sum_base + (long long)row0 * lds + col0;
