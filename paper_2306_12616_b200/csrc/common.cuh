@@ -70,6 +70,8 @@ __device__ __forceinline__ void fence_tensormap_acquire(const CUtensorMap* map) 
 }
 // generic-proxy <-> async-proxy ordering (global data written with st.global, read back by TMA)
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async;" ::: "memory"); }
+// same, restricted to the global state space (data written with st.global by other CTAs, read next by TMA loads)
+__device__ __forceinline__ void fence_proxy_async_global() { asm volatile("fence.proxy.async.global;" ::: "memory"); }
 
 // ---- global-memory flags ------------------------------------------------------------------------
 __device__ __forceinline__ int ld_acquire_gpu(const int* p) {

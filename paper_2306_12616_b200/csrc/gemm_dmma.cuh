@@ -278,7 +278,7 @@ __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MIN_CTAS) gemm_dmma_kernel(
                 if (args.use_deps) {
                     const int nd = tk->ndeps;
                     for (int d = tk->ndeps_early; d < nd; ++d) wait_dep(tk, d, tn);
-                    fence_proxy_async();  // data written through the generic proxy, read next by TMA
+                    fence_proxy_async_global();  // data written through the generic proxy, read next by TMA
                 }
                 const int ktiles = tk->ktiles;
                 if (ktiles > 0) {

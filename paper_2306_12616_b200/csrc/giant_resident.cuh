@@ -140,7 +140,7 @@ __global__ void __launch_bounds__(GR_THREADS, 1) giant_resident_kernel(const Gia
             const Task* tk = args.tasks + ti;
             if (tk->ktiles > 0) {
                 wait_counter(args.panel_done + (size_t)(ti - 1) * args.panel_stride + ctr, dep_target, args.error_flag);
-                fence_proxy_async();
+                fence_proxy_async_global();
                 const CUtensorMap* mapB = args.maps + tk->mapB;
                 if (s <= 2) fence_tensormap_acquire(mapB);  // the two ping-pong buffers alternate as operand B
                 for (int kt = 0; kt < ktiles; ++kt) {
