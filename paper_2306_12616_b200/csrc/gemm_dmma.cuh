@@ -144,14 +144,17 @@ __device__ __forceinline__ int sm_id() {
 
 // Producer-side wait for one dependency counter (global memory, written by red.release.gpu).
 __device__ __forceinline__ void wait_counter(const int* ctr, int target, int* error_flag) {
+    // Poll with relaxed loads (an acquire load invalidates the SM's L1 on every trip, under the consumer warps' feet),
+    // then take the acquire once.
     if (ld_acquire_gpu(ctr) >= target) return;
     const long long t0 = clock64();
-    while (ld_acquire_gpu(ctr) < target) {
+    while (ld_relaxed_gpu(ctr) < target) {
         if (clock64() - t0 > WATCHDOG_CLOCKS) {  // ~4 s: report instead of hanging
             atomicExch(error_flag, 1);
             break;
         }
     }
+    (void)ld_acquire_gpu(ctr);
 }
 
 // DOTS = true: the instance used by the moments chain (cheb_dm_moments), whose epilogue also forms the Frobenius
