@@ -36,7 +36,7 @@ FLUSH_BYTES = 512 << 20  # > 126 MB L2
 # Sum over the product launches of one solve (baby-step launch + giant-step launch).  ncu replays with cold caches, so
 # for cfg1/cfg2 (working set L2-resident when warm) this is an upper bound.  cfg3: only the baby-step launch was captured.
 NCU_TRAFFIC_BYTES = {
-    "cfg1": 2.462208e6 + 0.00128e6 + 18.195968e6 + 0.31872e6,        # profiles/r01_ncu_cfg1_solve.txt (baby + giant launch)
+    "cfg1": 2.462976e6 + 0.00128e6 + 18.196224e6 + 0.335104e6,       # profiles/r01_ncu_cfg1_solve.txt (baby + giant launch)
     "cfg2": 76.414208e6 + 4.39296e6 + 29.40672e6 + 79.427328e6 + 63.915008e6 + 20.947456e6,  # r01_ncu_cfg2_solve.txt
     "cfg4": (3.049292 + 1.735402 + 3.774622 + 1.652616 + 2.360862 + 0.712185) * 1e9,         # r01_ncu_cfg4_solve.txt
 }
