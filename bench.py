@@ -272,7 +272,10 @@ def measure_workload(torch, cd, workloads, name, args, steps, warmup, flush, sam
                      "achieved": achieved, "peak": peak_tf, "unit": "TFLOP/s", "frac": achieved / peak_tf if peak_tf else None,
                      "traffic": NCU_TRAFFIC_BYTES.get(name), "kernel_ms": kernel_ms, "launches_timed": n_rec,
                      "kernel_share_of_step": (kernel_ms * w.units) / ms_per_step if ms_per_step > 0 else None,
-                     "flops_per_launch": flops},
+                     "flops_per_launch": flops,
+                     # context: what the same time would mean if every product were charged its full 2 N^3 flops
+                     # (symmetric-tile skipping executes about half of them); not the roofline figure
+                     "full_product_equivalent_tflops": ((plan.k + plan.p - 2) * 2.0 * w.N ** 3) / (kernel_ms * 1e-3) * 1e-12 if kernel_ms > 0 else None},
         "e2e": {"value": world * w.units * e2e_steps / (e2e_ms * 1e-3), "unit": UNIT,
                 "h2d_bytes_per_step": w.h2d_bytes(), "d2h_bytes_per_step": w.d2h_bytes(), "steps": e2e_steps,
                 "ms_per_step": e2e_ms / e2e_steps},
