@@ -45,6 +45,7 @@ def _load():
     lib.co_dm_cheb_columns.argtypes = [C.c_int, _dp, C.c_double, C.c_double, _dp, C.c_int,
                                        C.c_int, _ip, _dp]
     lib.co_eval_cheb_sum.restype = C.c_double
+    lib.co_dm_cheb_apply.argtypes = [C.c_int, _dp, C.c_double, C.c_double, _dp, C.c_int, C.c_int, _dp, _dp]
     lib.co_eval_cheb_sum.argtypes = [_dp, C.c_int, C.c_double]
     lib.co_a_matrix.argtypes = [C.c_int, _dp]
     lib.co_x_matrix.argtypes = [C.c_int, C.c_int, _dp, _dp]
@@ -174,6 +175,16 @@ def dm_cheb_columns(H, a, b, c, cols):
     out = np.empty((cols.shape[0], n))
     _load().co_dm_cheb_columns(n, _p(H), a, b, _p(c), c.shape[0], cols.shape[0],
                                cols.ctypes.data_as(_ip), _p(out))
+    return out
+
+
+def dm_cheb_apply(H, a, b, c, V):
+    """(sum_{n<M} c_n T_n(X)) applied to the rows of V (nvec x n) by the vector three-term recurrence."""
+    H, c, V = _f64(H), _f64(c), _f64(V)
+    n = H.shape[0]
+    V = V.reshape(-1, n)
+    out = np.empty_like(V)
+    _load().co_dm_cheb_apply(n, _p(H), a, b, _p(c), c.shape[0], V.shape[0], _p(V), _p(out))
     return out
 
 

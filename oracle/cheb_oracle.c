@@ -295,6 +295,49 @@ void co_dm_cheb_columns(int n, const double* H, double a, double b, const double
     free(X); free(vm); free(vc); free(vn);
 }
 
+/* The same M-term sum applied to arbitrary vectors: out[s] = (sum_{n<M} c_n T_n(X)) V[s], s < nvec, by the
+ * three-term recurrence of PAPER.md:91 started from v (w_0 = v, w_1 = X v, w_{n+1} = 2 X w_n - w_{n-1}); no matrix
+ * product is formed.  V and out are nvec x n row-major (one vector per row).  With V[s] = e_j this is
+ * co_dm_cheb_columns.  Used by the full-size parity tests as a probe that touches every element of D (D is symmetric,
+ * so D V[s] can be compared with the GPU's matrix times the same vector).  Pins: tests/test_oracle_matrix.py
+ * (equals co_dm_cheb times V; unit vectors reproduce the column routine; diagonal H). */
+void co_dm_cheb_apply(int n, const double* H, double a, double b, const double* c, int M,
+                      int nvec, const double* V, double* out) {
+    size_t nn = (size_t)n * n;
+    double* X = (double*)malloc(sizeof(double) * nn);
+    co_scale(n, H, a, b, X);
+    double* wm = (double*)malloc(sizeof(double) * n);
+    double* wc = (double*)malloc(sizeof(double) * n);
+    double* wn = (double*)malloc(sizeof(double) * n);
+    for (int s = 0; s < nvec; ++s) {
+        const double* v = V + (size_t)s * n;
+        double* o = out + (size_t)s * n;
+        for (int i = 0; i < n; ++i) { wm[i] = v[i]; o[i] = (M > 0) ? c[0] * v[i] : 0.0; }
+        if (M > 1) {
+#pragma omp parallel for schedule(static)
+            for (int i = 0; i < n; ++i) {
+                double acc = 0.0;
+                const double* xi = X + (size_t)i * n;
+                for (int kk = 0; kk < n; ++kk) acc += xi[kk] * v[kk];
+                wc[i] = acc;
+            }
+            for (int i = 0; i < n; ++i) o[i] += c[1] * wc[i];
+        }
+        for (int t = 2; t < M; ++t) {
+#pragma omp parallel for schedule(static)
+            for (int i = 0; i < n; ++i) {
+                double acc = 0.0;
+                const double* xi = X + (size_t)i * n;
+                for (int kk = 0; kk < n; ++kk) acc += xi[kk] * wc[kk];
+                wn[i] = 2.0 * acc - wm[i];
+            }
+            double* sw = wm; wm = wc; wc = wn; wn = sw;
+            for (int i = 0; i < n; ++i) o[i] += c[t] * wc[i];
+        }
+    }
+    free(X); free(wm); free(wc); free(wn);
+}
+
 /* Scalar M-term Chebyshev sum by the DEFINITION T_n(x) = cos(n arccos x), |x| <= 1. */
 double co_eval_cheb_sum(const double* c, int M, double x) {
     long double th = acosl((long double)x), s = 0.0L;

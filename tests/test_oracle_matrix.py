@@ -189,6 +189,34 @@ def test_dm_cheb_columns_equal_full_matrix_columns():
     assert np.max(np.abs(out - D[:, cols].T)) < 1e-13
 
 
+def test_dm_cheb_apply_equals_matrix_times_vectors_and_column_routine():
+    """oracle.dm_cheb_apply (vector three-term recurrence) against the matrix route: D_cheb @ v for
+    Gaussian and +-1 vectors, unit vectors = the column routine, M = 1 and M = 2 (no recurrence step), and a
+    diagonal H where (D v)_i = p_M(x~_i) v_i with p_M by the definition T_n = cos(n arccos x)."""
+    n = 33
+    H = workloads.hamiltonian("cfg1", seed=1, n=n)
+    a, b = oracle.gershgorin(H)
+    c = oracle.cheb_coeffs(40.0, 0.02, a, b, 50)
+    D = oracle.dm_cheb(H, a, b, c)
+    rng = np.random.default_rng(5)
+    V = np.vstack([rng.standard_normal((2, n)), rng.choice([-1.0, 1.0], size=(2, n))])
+    out = oracle.dm_cheb_apply(H, a, b, c, V)
+    assert np.max(np.abs(out - V @ D.T)) < 1e-13
+    # a dropped term / wrong sign in the recurrence shows up at O(|c_n|) ~ 1e-2
+    assert np.max(np.abs(out - V @ D.T)) < 1e-6 * np.max(np.abs(c[2:10]))
+    E = np.eye(n)[[0, 7, 32]]
+    assert np.max(np.abs(oracle.dm_cheb_apply(H, a, b, c, E) - oracle.dm_cheb_columns(H, a, b, c, [0, 7, 32]))) < 1e-14
+    for M in (1, 2, 3):
+        DM = oracle.dm_cheb(H, a, b, c[:M].copy())
+        assert np.max(np.abs(oracle.dm_cheb_apply(H, a, b, c[:M].copy(), V) - V @ DM.T)) < 1e-14
+    eps = np.linspace(-1.3, 0.9, 12)
+    Hd = np.diag(eps)
+    cd = oracle.cheb_coeffs(9.0, -0.1, -1.5, 1.0, 30)
+    pm = np.array([oracle.eval_cheb_sum(cd, float((2 * e + 0.5) / 2.5)) for e in eps])
+    v = rng.standard_normal((1, 12))
+    assert np.max(np.abs(oracle.dm_cheb_apply(Hd, -1.5, 1.0, cd, v) - pm * v)) < 1e-13
+
+
 # ---------------------------------------------------------------------------- truncation (P7)
 def test_truncation_error_bounded_by_tail_and_decays_exponentially():
     """||D_cheb - D_eig||_max <= sum_{n>=M}|c_n|, decaying like exp(-pi M / beta~)
