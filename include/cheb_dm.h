@@ -17,15 +17,23 @@
  *  - Every call returns a cheb_dm_status_t (0 = OK); nothing throws or aborts; on error no
  *    output argument is written.
  *  - "device pointer" = CUDA global memory of the device that was current in cheb_dm_plan();
- *    "host pointer" = ordinary host memory.  Matrices are dense row-major FP64 with leading
- *    dimension N (row i starts at element i*N).  H must be symmetric (row-major == col-major).
+ *    "host pointer" = ordinary host memory.  Matrices are dense row-major FP64; DEVICE matrices H and D
+ *    have the leading dimensions of the plan options ldh / ldd (default N: row i starts at element
+ *    i*N), HOST matrices always have leading dimension N.  H must be symmetric (row-major == col-major).
+ *  - Batched calls (cheb_dm_*_batch: many independent small Hamiltonians) take HOST
+ *    arrays of nbatch device (or host) matrix pointers, nbatch <= the plan option max_batch; matrix s of
+ *    the batch lives in "slot" s of the plan's workspace.  The single-matrix calls are the nbatch = 1 case.
  *  - The plan owns its workspace (cudaMalloc'ed in cheb_dm_plan(), freed in cheb_dm_destroy());
  *    the caller owns H, D and every output buffer.  D must not alias H.
- *  - cheb_dm_compute / cheb_dm_trace / cheb_dm_moments / cheb_dm_product are asynchronous on the
- *    given stream (a cudaStream_t passed as void*; NULL = legacy default stream), allocate nothing
- *    and never synchronise with the host.  Calls that return scalars to HOST memory
- *    (cheb_dm_get_bounds, cheb_dm_get_coeffs, cheb_dm_solve_mu, cheb_dm_get_T) synchronise the
- *    stream they are given.
+ *  - cheb_dm_compute[_batch] / cheb_dm_solve[_batch] (mu_out == NULL) / cheb_dm_assemble / cheb_dm_trace[_batch] /
+ *    cheb_dm_moments (tau_host == NULL) / cheb_dm_product are asynchronous on the given stream (a
+ *    cudaStream_t passed as void*; NULL = legacy default stream), allocate nothing, read no environment
+ *    variable, never synchronise with the host and may be captured into a CUDA graph.  Calls that
+ *    return scalars to HOST memory (cheb_dm_get_bounds, cheb_dm_get_scalars, cheb_dm_get_coeffs,
+ *    cheb_dm_solve_mu, cheb_dm_get_T, cheb_dm_check) synchronise the stream they are given.
+ *  - Errors the DEVICE detects (non-finite bounds, the stability guard of the power-basis recursion, a
+ *    dependency watchdog) are sticky flags: they survive later computes on the plan and are reported -- and
+ *    cleared -- by the next cheb_dm_check / cheb_dm_wait / cheb_dm_compute_host.
  *  - A plan is not thread-safe; distinct plans are independent.  There is no CPU fallback: without
  *    a CUDA device cheb_dm_plan() returns CHEB_DM_ECUDA.
  */
@@ -50,7 +58,10 @@ typedef enum {
     CHEB_DM_ESTATE = 4,       /* call order: compute before coeffs, solve_mu before moments ...  */
     CHEB_DM_EBOUNDS = 5,      /* b <= a or non-finite bounds                                     */
     CHEB_DM_EUNSUPPORTED = 6, /* dtype other than CHEB_DM_F64                                    */
-    CHEB_DM_ENOCONV = 7       /* plan-time stability guard of the power-basis outer recursion    */
+    CHEB_DM_ENOCONV = 7       /* stability guard of the power-basis outer recursion (Eq. 4): the table d
+                                 computed on the device has max|d| 2^-52 p > 1e-12 (d grows like 2^p, Eq. 12,
+                                 PAPER.md:136; reading A6); D was still written but may have lost
+                                 accuracy.  Reported by cheb_dm_check / cheb_dm_wait / cheb_dm_compute_host. */
 } cheb_dm_status_t;
 
 /* Outer (giant-step) recursion.
@@ -71,11 +82,14 @@ typedef enum { CHEB_DM_OUTER_CHEBYSHEV = 0, CHEB_DM_OUTER_POWER = 1 } cheb_dm_ou
 typedef enum { CHEB_DM_SCHED_GROUPED = 0, CHEB_DM_SCHED_SERIAL = 1 } cheb_dm_sched_t;
 
 /* Operand pairing of the baby steps (any a+b=n is valid by Eq. 7).
- *  CHEB_DM_PAIR_ALG1 (default): Algorithm 1's pairing, ceil(log2 k) stages.
+ *  CHEB_DM_PAIR_AUTO (default) = CHEB_DM_PAIR_BALANCED.
+ *  CHEB_DM_PAIR_ALG1: Algorithm 1's pairing, ceil(log2 k) stages.
  *  CHEB_DM_PAIR_SERIAL: T_{n+1} = 2 T_1 T_n - T_{n-1} (k-1 serial products; best rounding).
- *  CHEB_DM_PAIR_BALANCED: T_n = 2 T_ceil(n/2) T_floor(n/2) - T_{0 or 1}: same stages and concurrency as
- *      Algorithm 1, no long chains through T_{2^j} unless n is a power of two (reading A7b).  */
-typedef enum { CHEB_DM_PAIR_ALG1 = 0, CHEB_DM_PAIR_SERIAL = 1, CHEB_DM_PAIR_BALANCED = 2 } cheb_dm_pairing_t;
+ *  CHEB_DM_PAIR_BALANCED: T_n = 2 T_ceil(n/2) T_floor(n/2) - T_{0 or 1}: same stages, concurrency and cost as
+ *      Algorithm 1, no long chains through T_{2^j} unless n is a power of two.  On spectra concentrated at
+ *      x~ = 0 (cfg4) Algorithm 1's squaring chains leave |dtr D| = 7.7e-10 of the 1e-9 gate, the balanced
+ *      pairing 1.3e-12 (reading A7b), hence the default.                                          */
+typedef enum { CHEB_DM_PAIR_AUTO = 0, CHEB_DM_PAIR_SERIAL = 1, CHEB_DM_PAIR_BALANCED = 2, CHEB_DM_PAIR_ALG1 = 3 } cheb_dm_pairing_t;
 
 typedef struct {
     int k;       /* baby-step block size; 0 = auto: ceil(sqrt(M))                 */
@@ -101,7 +115,18 @@ typedef struct {
                     product that touch the lower triangle are computed, each mirrors its 8x8 blocks into the skipped
                     tiles (transposed in registers, stored row-contiguously).  ~45 % fewer tensor flops per product;
                     cheb_dm_flops_per_compute counts only the executed tiles.  H must be symmetric either way.        */
-    int reserved[7];
+    int max_batch; /* matrices per grouped launch (cheb_dm_compute_batch): 0 or 1 = single solves only,
+                      at most 64.  The workspace holds max_batch slots; with max_batch > 1 the tile shape is chosen for
+                      the batch and batched giant steps run in the generic grouped kernel.                          */
+    int ldh;       /* leading dimension (elements) of the caller's DEVICE matrices H; 0 = N; must be >= N.          */
+    int ldd;       /* the same for the DEVICE output matrices D.                                                  */
+    int moments;   /* 0 = auto (on), 1 = off, 2 = on: keep the giant block U_j = T_{jk}(X), j = 2..p-1, in the workspace
+                      (p - 2 more matrices per slot, + p for the low-order sums) -- needed by cheb_dm_moments,
+                      cheb_dm_solve and cheb_dm_assemble (EUNSUPPORTED when off).                                   */
+    int host_slots; /* staging sets of the host entry points allocated at plan time: 0 = none (the first host call
+                      allocates what it needs -- the one exception to "compute calls allocate nothing"), 1 = one
+                      (cheb_dm_compute_host), 2 = both + copy streams/events (cheb_dm_compute_host_async).         */
+    int reserved[2];
 } cheb_dm_options_t;
 
 /* Create a plan for N x N matrices and an M_terms-term expansion.  Chooses (k,p), allocates the
@@ -128,11 +153,22 @@ cheb_dm_status_t cheb_dm_destroy(cheb_dm_plan_t plan);
  * EINVAL: non-finite beta/mu or beta <= 0; EBOUNDS: explicit bounds with b <= a or non-finite. */
 cheb_dm_status_t cheb_dm_coeffs(cheb_dm_plan_t plan, double beta, double mu, const double* bounds);
 
-/* D <- sum_{n<M} c_n T_n(X) for the symmetric H (Eq. 3-4).  dH, dD: device pointers, N*N doubles,
- * leading dimension N.  Runs, on `cuda_stream` and without host synchronisation: bounds (Gershgorin
+/* D <- sum_{n<M} c_n T_n(X) for the symmetric H (Eq. 3-4).  dH, dD: device pointers, N rows of N doubles,
+ * leading dimensions ldh / ldd (plan options; default N).  Runs, on `cuda_stream` and without host synchronisation: bounds (Gershgorin
  * unless explicit) + rescale of H into X; coefficient tables; baby steps T_2..T_k; giant steps.
  * ESTATE if cheb_dm_coeffs() was never called; EINVAL on NULL/aliased pointers. */
 cheb_dm_status_t cheb_dm_compute(cheb_dm_plan_t plan, const double* dH, double* dD, void* cuda_stream);
+
+/* Batched form (SURVEY 8(f)-2; the many-small-Hamiltonians use case of PAPER.md:35, :55): nbatch independent
+ * solves, D_s <- sum c_n(mu_s) T_n(X_s), in ONE set of grouped launches: one front-end launch over all matrices
+ * (each with its own Gershgorin bounds and coefficient tables), one persistent baby-step launch and one
+ * giant-step launch whose work lists are the union over the batch, claimed level by level and matrix by
+ * matrix, so that the independent products of different matrices fill the SMs and hide one another's serial
+ * chain.  dH, dD: HOST arrays of nbatch device pointers (matrices as in cheb_dm_compute); mu: HOST array of
+ * nbatch chemical potentials, or NULL = the mu of cheb_dm_coeffs for all; beta and the bounds mode are those of
+ * cheb_dm_coeffs.  EINVAL: nbatch < 1 or > max_batch, NULL / aliased pointers, non-finite mu. */
+cheb_dm_status_t cheb_dm_compute_batch(cheb_dm_plan_t plan, int nbatch, const double* const* dH, double* const* dD,
+                                       const double* mu, void* cuda_stream);
 
 /* Host-buffer form of cheb_dm_compute (+ cheb_dm_trace): the end-to-end call a user without device
  * memory makes.  hH, hD: HOST pointers, N*N doubles (ld N), pinned memory recommended; h_trace: HOST pointer
@@ -151,15 +187,32 @@ cheb_dm_status_t cheb_dm_compute_host(cheb_dm_plan_t plan, const double* hH, dou
 cheb_dm_status_t cheb_dm_compute_host_async(cheb_dm_plan_t plan, const double* hH, double* hD, double* h_trace,
                                             void* cuda_stream);
 cheb_dm_status_t cheb_dm_wait(cheb_dm_plan_t plan, void* cuda_stream);
+/* Batched host forms: hH, hD HOST arrays of nbatch HOST matrix pointers (N*N doubles each, ld N, pinned
+ * recommended); h_trace: HOST pointer to nbatch doubles or NULL; mu as in cheb_dm_compute_batch.  The _async form
+ * queues the batch (pipelined over two staging sets like cheb_dm_compute_host_async; results valid after
+ * cheb_dm_wait), the other synchronises and checks before it returns. */
+cheb_dm_status_t cheb_dm_compute_batch_host(cheb_dm_plan_t plan, int nbatch, const double* const* hH, double* const* hD,
+                                            double* h_trace, const double* mu, void* cuda_stream);
+cheb_dm_status_t cheb_dm_compute_batch_host_async(cheb_dm_plan_t plan, int nbatch, const double* const* hH,
+                                                  double* const* hD, double* h_trace, const double* mu, void* cuda_stream);
 
 /* trace_out[0] <- tr D = sum_i D_ii (electron count, north_star item 4).  dD: device pointer (N*N,
  * ld N).  trace_out: DEVICE pointer (or pinned mapped host memory), 1 double, written
  * asynchronously on the stream in a fixed summation order (bitwise reproducible). */
 cheb_dm_status_t cheb_dm_trace(cheb_dm_plan_t plan, const double* dD, double* trace_out, void* cuda_stream);
 
+/* Batched trace: trace_out[s] <- tr D_s, s < nbatch (dD: HOST array of device pointers, ld = option ldd;
+ * trace_out: DEVICE pointer to nbatch doubles), one launch. */
+cheb_dm_status_t cheb_dm_trace_batch(cheb_dm_plan_t plan, int nbatch, const double* const* dD, double* trace_out,
+                                     void* cuda_stream);
+
 /* Bounds {a,b} used by the last cheb_dm_compute()/cheb_dm_moments() (host pointer, 2 doubles).
  * Synchronises `cuda_stream`.  EBOUNDS if the device flagged non-finite bounds. */
 cheb_dm_status_t cheb_dm_get_bounds(cheb_dm_plan_t plan, double* bounds_out, void* cuda_stream);
+
+/* Device-side scalars of slot `slot` (< max_batch) after the last call: out[0..3] = {a, b, mu, N_e(mu)} (host
+ * pointer; N_e is set by the bisection only).  Synchronises `cuda_stream`.  EBOUNDS as cheb_dm_get_bounds. */
+cheb_dm_status_t cheb_dm_get_scalars(cheb_dm_plan_t plan, int slot, double* out4, void* cuda_stream);
 
 /* Scalar tables of the last compute, copied to host memory (any pointer may be NULL):
  *   c_out[k*p]  c_n (zero for n >= M);   g_out[k*p]  g_{i,l} at [i*p + l];
@@ -180,12 +233,13 @@ cheb_dm_status_t cheb_dm_get_kp(cheb_dm_plan_t plan, int* k_out, int* p_out);
 cheb_dm_status_t cheb_dm_get_T(cheb_dm_plan_t plan, int n, double* dOut, void* cuda_stream);
 
 /* Chebyshev moments tau_n = tr T_n(X), n < k*p, of H (north_star item 4; reading A10):
- * bounds + rescale, baby steps, the giant block T_{jk} = T_j(T_k) (p-2 further products) and
- * tau_{jk+i} = 2 <T_{jk}, T_i>_F - tau_{jk-i} (from Eq. 7 and symmetry), the Frobenius inner
- * products being fused into the epilogues of the products that form T_{jk}.  Results stay on the
- * device inside the plan for cheb_dm_solve_mu(); if tau_host != NULL (host pointer, k*p doubles)
- * they are also copied out (this synchronises the stream).  Uses the bounds mode of the last
- * cheb_dm_coeffs() call (explicit or Gershgorin); ESTATE if there was none. */
+ * bounds + rescale, baby steps, the giant block U_j = T_{jk} = T_j(T_k) (p-2 further products, kept in the
+ * workspace) and tau_{jk+i} = 2 <T_{jk}, T_i>_F - tau_{jk-i} (from Eq. 7 and symmetry); all Frobenius inner
+ * products are one skinny GEMM over the matrix elements on the tensor cores (gram_kernel: every matrix of
+ * the two blocks is read once).  Results stay on the device inside the plan for cheb_dm_solve_mu() /
+ * cheb_dm_assemble(); if tau_host != NULL (host pointer, k*p doubles) they are also copied out (this
+ * synchronises the stream).  Uses the bounds mode of the last cheb_dm_coeffs() call (explicit or
+ * Gershgorin); ESTATE if there was none; EUNSUPPORTED if the plan was made with moments = off. */
 cheb_dm_status_t cheb_dm_moments(cheb_dm_plan_t plan, const double* dH, double* tau_host, void* cuda_stream);
 
 /* Chemical potential for a target electron count: solves N_e(mu) = sum_n c_n(mu) tau_n = n_occ by
@@ -195,6 +249,26 @@ cheb_dm_status_t cheb_dm_moments(cheb_dm_plan_t plan, const double* dH, double* 
 cheb_dm_status_t cheb_dm_solve_mu(cheb_dm_plan_t plan, double beta, double n_occ, int iters,
                                   double* mu_out, void* cuda_stream);
 
+/* mu-inclusive solve ("mu solved on the trace" of BASELINE.json's configs; adjacent to Eq. 6,
+ * PAPER.md:105): bounds + rescale and the baby block T_1..T_k ONCE, the giant block U_j = T_{jk} (p-2 products),
+ * moments by the Gram kernel, mu by `iters` bisection halvings on the device (N_e(mu) = n_occ, reading A9), the
+ * coefficient tables for that mu (mu never leaves the device), the low-order sums G_l of Eq. (21), and
+ *     D = G_0 + sum_{l=1}^{p-1} G_l U_l        (since sum_n c_n T_n = sum_l G_l T_l(T_k), reading A6)
+ * as ONE long-K product (K = (p-1) N) without the serial Horner chain of Eq. (4).  k + 2p - 4 products instead
+ * of the k + p - 2 of a fixed-mu solve, and nothing is computed twice.  beta and the bounds mode come from
+ * cheb_dm_coeffs (its mu is ignored).  mu_out: HOST pointer (nbatch doubles for the batch form) or NULL; when
+ * given, the stream is synchronised to return mu.  n_occ: target electron count(s) (HOST array for the batch
+ * form).  EUNSUPPORTED if the plan was made with moments = off.
+ * cheb_dm_assemble: D for NEW chemical potentials from the blocks left in the workspace by the last
+ * cheb_dm_moments / cheb_dm_solve[_batch] call on the same matrices (each new mu costs the coefficient tables,
+ * the sums and one long-K product -- the use in a self-consistency or MD loop); mu: HOST array of nbatch values.
+ * ESTATE if no such call preceded or nbatch differs. */
+cheb_dm_status_t cheb_dm_solve(cheb_dm_plan_t plan, const double* dH, double n_occ, int iters, double* dD,
+                               double* mu_out, void* cuda_stream);
+cheb_dm_status_t cheb_dm_solve_batch(cheb_dm_plan_t plan, int nbatch, const double* const* dH, const double* n_occ,
+                                     int iters, double* const* dD, double* mu_out, void* cuda_stream);
+cheb_dm_status_t cheb_dm_assemble(cheb_dm_plan_t plan, int nbatch, const double* mu, double* const* dD, void* cuda_stream);
+
 /* One product of the recurrence as a stand-alone call (kernel-level tests and GEMM benchmark):
  *   Out = alpha * A B + beta * C,   A, B, C, Out symmetric-operand N x N device matrices (ld N),
  * computed by the same DMMA kernel as the solve (A is read through its transpose, which equals A
@@ -202,20 +276,25 @@ cheb_dm_status_t cheb_dm_solve_mu(cheb_dm_plan_t plan, double beta, double n_occ
 cheb_dm_status_t cheb_dm_product(cheb_dm_plan_t plan, double alpha, const double* dA, const double* dB,
                                  double beta, const double* dC, double* dOut, void* cuda_stream);
 
-/* Synchronises `cuda_stream` and reports what the device flagged during the last compute / moments call:
- * CHEB_DM_ECUDA if a CUDA error is pending or a dependency wait inside a persistent kernel hit its watchdog (~4 s;
- * never in a correct run), CHEB_DM_EBOUNDS for non-finite bounds, else CHEB_DM_OK.  cheb_dm_compute_host() performs
- * the same check before it returns. */
+/* Synchronises `cuda_stream` and reports what the device flagged since the last check (the flags are sticky, so one
+ * check after a pipeline of computes sees an error of any of them; the check clears them): CHEB_DM_ECUDA if a CUDA
+ * error is pending or a dependency wait inside a persistent kernel hit its watchdog (~4 s; never in a correct
+ * run), CHEB_DM_EBOUNDS for non-finite bounds, CHEB_DM_ENOCONV for the stability guard of the power-basis outer
+ * recursion, else CHEB_DM_OK.  cheb_dm_compute_host() and cheb_dm_wait() perform the same check. */
 cheb_dm_status_t cheb_dm_check(cheb_dm_plan_t plan, void* cuda_stream);
 
 /* Bytes of device workspace owned by the plan. */
 cheb_dm_status_t cheb_dm_workspace_bytes(cheb_dm_plan_t plan, size_t* bytes_out);
 
-/* Number of kernel launches issued by the last cheb_dm_compute() (for bench.py's gpu_launches). */
+/* Number of kernel launches issued by the last cheb_dm_compute[_batch] / cheb_dm_solve[_batch] / cheb_dm_assemble /
+ * cheb_dm_moments call (for bench.py's gpu_launches). */
 cheb_dm_status_t cheb_dm_last_launch_count(cheb_dm_plan_t plan, int* launches_out);
 
-/* Executed FP64 tensor flops of one cheb_dm_compute() on this plan: 2*N^3 per product. */
+/* Executed FP64 tensor flops of one cheb_dm_compute() of ONE matrix on this plan: 2*N^3 per product, only the
+ * computed tiles with symmetric-tile skipping.  cheb_dm_flops_per_solve: the same for cheb_dm_solve (baby block,
+ * giant block, Gram kernel and the long-K assembly). */
 cheb_dm_status_t cheb_dm_flops_per_compute(cheb_dm_plan_t plan, double* flops_out);
+cheb_dm_status_t cheb_dm_flops_per_solve(cheb_dm_plan_t plan, double* flops_out);
 
 /* Measurement support (bench.py's roofline object).
  * cheb_dm_set_timing(plan, 1): every following cheb_dm_compute() records a CUDA event on its stream

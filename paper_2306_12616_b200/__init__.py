@@ -9,6 +9,6 @@ functions raises; without a CUDA device ``Plan`` raises ChebDMError(ECUDA).
 """
 from .binding import (  # noqa: F401
     ChebDMError, Options, Plan, lib, lib_path, dmma_peak,
-    OUTER_CHEBYSHEV, OUTER_POWER, SCHED_GROUPED, SCHED_SERIAL, PAIR_ALG1, PAIR_SERIAL,
-    TILE_AUTO, TILE_128x128, TILE_128x64, TILE_64x64, STATUS_NAMES,
+    OUTER_CHEBYSHEV, OUTER_POWER, SCHED_GROUPED, SCHED_SERIAL, PAIR_AUTO, PAIR_ALG1, PAIR_SERIAL, PAIR_BALANCED,
+    TILE_AUTO, TILE_128x128, TILE_128x64, TILE_64x64, STATUS_NAMES, MAX_BATCH,
 )

@@ -8,7 +8,8 @@ from . import build as _build
 
 OUTER_CHEBYSHEV, OUTER_POWER = 0, 1
 SCHED_GROUPED, SCHED_SERIAL = 0, 1
-PAIR_ALG1, PAIR_SERIAL, PAIR_BALANCED = 0, 1, 2
+PAIR_AUTO, PAIR_SERIAL, PAIR_BALANCED, PAIR_ALG1 = 0, 1, 2, 3
+MAX_BATCH = 64
 TILE_AUTO, TILE_128x128, TILE_128x64, TILE_64x64 = 0, 1, 2, 3
 STATUS_NAMES = ["OK", "EINVAL", "EALLOC", "ECUDA", "ESTATE", "EBOUNDS", "EUNSUPPORTED", "ENOCONV"]
 
@@ -20,6 +21,8 @@ EXPORTS = [
     "cheb_dm_compute_host", "cheb_dm_set_timing", "cheb_dm_product_ms", "cheb_dm_dmma_peak",
     "cheb_dm_set_trace", "cheb_dm_get_trace", "cheb_dm_get_options", "cheb_dm_check",
     "cheb_dm_compute_host_async", "cheb_dm_wait",
+    "cheb_dm_compute_batch", "cheb_dm_compute_batch_host", "cheb_dm_compute_batch_host_async", "cheb_dm_trace_batch",
+    "cheb_dm_get_scalars", "cheb_dm_solve", "cheb_dm_solve_batch", "cheb_dm_assemble", "cheb_dm_flops_per_solve",
 ]
 
 
@@ -32,7 +35,8 @@ class TraceRec(C.Structure):
 class Options(C.Structure):
     _fields_ = [("k", C.c_int), ("p", C.c_int), ("outer", C.c_int), ("sched", C.c_int),
                 ("pairing", C.c_int), ("tile", C.c_int), ("fuse_sums", C.c_int),
-                ("giant", C.c_int), ("symmetric", C.c_int), ("reserved", C.c_int * 7)]
+                ("giant", C.c_int), ("symmetric", C.c_int), ("max_batch", C.c_int), ("ldh", C.c_int), ("ldd", C.c_int),
+                ("moments", C.c_int), ("host_slots", C.c_int), ("reserved", C.c_int * 2)]
 
 
 class ChebDMError(RuntimeError):
@@ -90,6 +94,16 @@ def lib():
     L.cheb_dm_wait.argtypes = [vp, vp]
     L.cheb_dm_set_trace.argtypes = [vp, C.c_int]
     L.cheb_dm_get_trace.argtypes = [vp, C.POINTER(TraceRec), C.c_int, ip]
+    pp = C.POINTER(vp)
+    L.cheb_dm_compute_batch.argtypes = [vp, C.c_int, pp, pp, dp, vp]
+    L.cheb_dm_compute_batch_host.argtypes = [vp, C.c_int, pp, pp, vp, dp, vp]
+    L.cheb_dm_compute_batch_host_async.argtypes = [vp, C.c_int, pp, pp, vp, dp, vp]
+    L.cheb_dm_trace_batch.argtypes = [vp, C.c_int, pp, vp, vp]
+    L.cheb_dm_get_scalars.argtypes = [vp, C.c_int, dp, vp]
+    L.cheb_dm_solve.argtypes = [vp, vp, C.c_double, C.c_int, vp, dp, vp]
+    L.cheb_dm_solve_batch.argtypes = [vp, C.c_int, pp, dp, C.c_int, pp, dp, vp]
+    L.cheb_dm_assemble.argtypes = [vp, C.c_int, dp, pp, vp]
+    L.cheb_dm_flops_per_solve.argtypes = [vp, dp]
     for n in EXPORTS:
         getattr(L, n).restype = C.c_int
     L.cheb_dm_strerror.argtypes = [C.c_int]
@@ -109,6 +123,19 @@ def _darr(a):
     return a, a.ctypes.data_as(C.POINTER(C.c_double))
 
 
+def _parr(ptrs):
+    """HOST array of raw addresses (ints) for the batched calls."""
+    n = len(ptrs)
+    return (C.c_void_p * n)(*[int(x) for x in ptrs])
+
+
+def _dvec(vals):
+    if vals is None:
+        return None
+    n = len(vals)
+    return (C.c_double * n)(*[float(x) for x in vals])
+
+
 def dmma_peak(iters: int = 20000, stream: int = 0) -> float:
     """FP64 tensor (DMMA.8x8x4) issue-rate peak of the current device in TFLOP/s (cheb_dm_dmma_peak)."""
     v = C.c_double()
@@ -120,11 +147,13 @@ class Plan:
     """cheb_dm_plan_t with the same calls as the C ABI.  Pointers are raw device addresses (int)."""
 
     def __init__(self, N: int, M: int, *, k: int = 0, p: int = 0, outer: int = OUTER_CHEBYSHEV,
-                 sched: int = SCHED_GROUPED, pairing: int = PAIR_ALG1, tile: int = TILE_AUTO,
-                 fuse_sums: int = 0, giant: int = 0, symmetric: int = 0, dtype: int = 0):
+                 sched: int = SCHED_GROUPED, pairing: int = PAIR_AUTO, tile: int = TILE_AUTO,
+                 fuse_sums: int = 0, giant: int = 0, symmetric: int = 0, max_batch: int = 0, ldh: int = 0, ldd: int = 0,
+                 moments: int = 0, host_slots: int = 0, dtype: int = 0):
         self._h = C.c_void_p()
         self.N, self.M = N, M
-        o = Options(k=k, p=p, outer=outer, sched=sched, pairing=pairing, tile=tile, fuse_sums=fuse_sums, giant=giant, symmetric=symmetric)
+        o = Options(k=k, p=p, outer=outer, sched=sched, pairing=pairing, tile=tile, fuse_sums=fuse_sums, giant=giant, symmetric=symmetric,
+                    max_batch=max_batch, ldh=ldh, ldd=ldd, moments=moments, host_slots=host_slots)
         _chk(lib().cheb_dm_plan_ex(C.byref(self._h), N, M, dtype, C.byref(o)), "cheb_dm_plan_ex")
         kk, pp = C.c_int(), C.c_int()
         _chk(lib().cheb_dm_get_kp(self._h, C.byref(kk), C.byref(pp)), "cheb_dm_get_kp")
@@ -152,6 +181,51 @@ class Plan:
 
     def compute(self, dH: int, dD: int, stream: int = 0):
         _chk(lib().cheb_dm_compute(self._h, dH, dD, stream), "cheb_dm_compute")
+
+    def compute_batch(self, dH, dD, mu=None, stream: int = 0):
+        """dH, dD: sequences of device addresses; mu: sequence of floats or None (cheb_dm_compute_batch)."""
+        n = len(dH)
+        _chk(lib().cheb_dm_compute_batch(self._h, n, _parr(dH), _parr(dD), _dvec(mu), stream), "cheb_dm_compute_batch")
+
+    def compute_batch_host(self, hH, hD, h_trace: int = 0, mu=None, stream: int = 0):
+        n = len(hH)
+        _chk(lib().cheb_dm_compute_batch_host(self._h, n, _parr(hH), _parr(hD), h_trace or None, _dvec(mu), stream),
+             "cheb_dm_compute_batch_host")
+
+    def compute_batch_host_async(self, hH, hD, h_trace: int = 0, mu=None, stream: int = 0):
+        n = len(hH)
+        _chk(lib().cheb_dm_compute_batch_host_async(self._h, n, _parr(hH), _parr(hD), h_trace or None, _dvec(mu), stream),
+             "cheb_dm_compute_batch_host_async")
+
+    def trace_batch(self, dD, d_out: int, stream: int = 0):
+        _chk(lib().cheb_dm_trace_batch(self._h, len(dD), _parr(dD), d_out, stream), "cheb_dm_trace_batch")
+
+    def solve(self, dH: int, n_occ: float, dD: int, iters: int = 100, want_mu: bool = True, stream: int = 0):
+        """mu-inclusive solve (cheb_dm_solve); returns mu (synchronises) or None."""
+        mu = C.c_double()
+        _chk(lib().cheb_dm_solve(self._h, dH, float(n_occ), iters, dD, C.byref(mu) if want_mu else None, stream), "cheb_dm_solve")
+        return mu.value if want_mu else None
+
+    def solve_batch(self, dH, n_occ, dD, iters: int = 100, want_mu: bool = True, stream: int = 0):
+        n = len(dH)
+        mu = (C.c_double * n)()
+        _chk(lib().cheb_dm_solve_batch(self._h, n, _parr(dH), _dvec(n_occ), iters, _parr(dD), mu if want_mu else None, stream),
+             "cheb_dm_solve_batch")
+        return [float(x) for x in mu] if want_mu else None
+
+    def assemble(self, mu, dD, stream: int = 0):
+        _chk(lib().cheb_dm_assemble(self._h, len(dD), _dvec(mu), _parr(dD), stream), "cheb_dm_assemble")
+
+    def get_scalars(self, slot: int = 0, stream: int = 0):
+        """(a, b, mu, N_e(mu)) of a slot after the last call."""
+        out = (C.c_double * 4)()
+        _chk(lib().cheb_dm_get_scalars(self._h, slot, out, stream), "cheb_dm_get_scalars")
+        return tuple(float(x) for x in out)
+
+    def flops_per_solve(self) -> float:
+        v = C.c_double()
+        _chk(lib().cheb_dm_flops_per_solve(self._h, C.byref(v)), "cheb_dm_flops_per_solve")
+        return v.value
 
     def compute_host(self, hH: int, hD: int, h_trace: int = 0, stream: int = 0):
         """hH, hD, h_trace: HOST addresses (e.g. of pinned torch tensors / numpy arrays)."""

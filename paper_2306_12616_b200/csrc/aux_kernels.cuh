@@ -9,29 +9,29 @@ namespace chebdm {
 namespace cg = cooperative_groups;
 
 // ---------------------------------------------------------------------------------------------------
-// Device-resident scalar state of a plan.
+// Device-resident scalar state of one matrix ("slot") of a plan.
 // ---------------------------------------------------------------------------------------------------
 struct DevScalars {
     double a, b;                      // bounds in use (eps_a, eps_b)
-    int bad_bounds;                   // set when the bounds are non-finite
-    int pad;
-    double mu;                        // result of the device-side bisection
-    double ne;                        // N_e at that mu
+    int bad_bounds;                   // sticky: set when the bounds are non-finite; cleared by cheb_dm_check
+    int noconv;                       // sticky: the power-basis table d of Eq. (4) exceeded the stability guard
+    double mu;                        // chemical potential in use (given, or the result of the device-side bisection)
+    double ne;                        // N_e at that mu (bisection only)
 };
 
 // Copy a user matrix (ld N) into a padded workspace matrix (ld ldx).
-__global__ void pad_copy_kernel(const double* __restrict__ src, int N, double* __restrict__ dst, long long ldx) {
+__global__ void pad_copy_kernel(const double* __restrict__ src, long long lds, int N, double* __restrict__ dst, long long ldx) {
     const long long total = (long long)N * N;
     for (long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x; e < total; e += (long long)gridDim.x * blockDim.x) {
         const int i = (int)(e / N), j = (int)(e - (long long)i * N);
-        dst[(long long)i * ldx + j] = src[e];
+        dst[(long long)i * ldx + j] = src[(long long)i * lds + j];
     }
 }
-__global__ void unpad_copy_kernel(const double* __restrict__ src, long long ldx, int N, double* __restrict__ dst) {
+__global__ void unpad_copy_kernel(const double* __restrict__ src, long long ldx, int N, double* __restrict__ dst, long long ldd) {
     const long long total = (long long)N * N;
     for (long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x; e < total; e += (long long)gridDim.x * blockDim.x) {
         const int i = (int)(e / N), j = (int)(e - (long long)i * N);
-        dst[e] = src[(long long)i * ldx + j];
+        dst[(long long)i * ldd + j] = src[(long long)i * ldx + j];
     }
 }
 
@@ -99,42 +99,51 @@ __device__ __forceinline__ double fermi_scaled(double beta_t, double mu_t, doubl
 }
 
 // ---------------------------------------------------------------------------------------------------
-// a-1 .. a-3 fused: ONE cooperative launch per solve does everything that precedes the products
-//   phase 0  zero the scheduler counters (replaces a memset node)
-//   phase 1  Gershgorin: one warp per row, per-block (min, max) partials -- no atomics, so no initialisation
-//            pass and a result that does not depend on the order of arrival
+// a-1 .. a-3 fused: ONE cooperative launch does everything that precedes the products, for every matrix of the batch.
+// Block b serves matrix (slot) b % nb; the blocks of a slot split its rows / nodes / coefficients among themselves.
+//   phase 0  zero the scheduler counters (replaces a memset node); the sticky error flag lies outside that range
+//   phase 1  (do_bounds) Gershgorin: one warp per row, per-block (min, max) partials -- no atomics, so no
+//            initialisation pass and a result that does not depend on the order of arrival
 //   -- grid sync --
-//   phase 2  every block reduces the partials to (a, b) itself; rescale H -> X = T_1 (pad columns stay zero);
-//            fn[j] = f~(x_j) at the N_q Chebyshev nodes
+//   phase 2  every block reduces its slot's partials to (a, b) itself; rescale H -> X = T_1 (pad columns stay zero);
+//            (do_coeffs) fn[j] = f~(x_j) at the N_q Chebyshev nodes, mu given per slot or read from the slot's
+//            DevScalars (mu_from_device: the result of the device-side bisection, cheb_dm_solve)
 //   -- grid sync --
 //   phase 3  c_n, n < k p: one warp per coefficient, double-double accumulation in a fixed order
 //   -- grid sync --
-//   phase 4  (block 0) tables g (and d) of Eq. (16)-(20).  Thread i owns the coupled chains i and k-i of
-//            g_{i,l} = 2 c_{lk+i} - g_{k-i,l+1}, so the recurrence needs no block barrier.
+//   phase 4  (first block of the slot) tables g (and d) of Eq. (16)-(20).  Thread i owns the coupled chains i and
+//            k-i of g_{i,l} = 2 c_{lk+i} - g_{k-i,l+1}, so the recurrence needs no block barrier.  With the power-basis
+//            outer recursion (want_d) the guard of reading A6 is evaluated: max|d| 2^-52 p > 1e-12 sets `noconv`
+//            (d_{i,p-1} = 2^p c by Eq. 12's a_{j,j} = 2^{1-j}).
+// do_bounds = 0, do_coeffs = 1 recomputes the tables only (new mu on the same X: cheb_dm_solve, cheb_dm_remu).
 // For small N the launch gaps of five separate kernels were ~10 % of a whole solve (cfg1: 39 us of 400 us).
-// HBM bytes as bounds_rescale_kernel: 8N^2 read (+ 8N^2 re-read, L2 for small N) + 8N^2 written.
+// HBM bytes: 8N^2 read (+ 8N^2 re-read, L2 for small N) + 8N^2 written per matrix.
 // ---------------------------------------------------------------------------------------------------
 constexpr int FRONT_SMEM_COEFS = 4608;  // 36 KB: covers k p up to 4608 (all configs; larger plans read c from L2)
 struct FrontArgs {
-    const double* H;
+    int nb;                          // matrices of this call (gridDim.x >= nb)
     int N;
-    double* X;
-    long long ldx;
-    DevScalars* sc;
+    const double* H[MAX_BATCH];      // per slot, leading dimension ldh
+    double mu[MAX_BATCH];            // per slot (ignored when mu_from_device)
+    long long ldh;
+    double* X;                       // T_1 of slot 0; slot s at X + s * slot_stride
+    long long slot_stride, ldx;
+    DevScalars* sc;                  // [nb]
     int explicit_bounds;
-    double a, b;             // explicit bounds
-    double* part;            // [2 * gridDim.x] per-block (lo, hi)
-    int* counters;
+    double a, b;                     // explicit bounds
+    double* part;                    // [2 * gridDim.x] per-block (lo, hi)
+    int* counters;                   // range to zero
     int ncounters;
-    double beta, mu;
+    int do_bounds, do_coeffs, mu_from_device;
+    double beta;
     const double* costab;
     int Nq, M;
-    double* fn;
-    double* c;
+    double* fn;                      // [slot][Nq]
+    double* c;                       // [slot][k p]
     int k, p;
     const double* Amat;
     int want_d;
-    double* gT;
+    double* gT;                      // [slot][p][k]
     double* dT;
 };
 
@@ -142,98 +151,119 @@ __global__ void __launch_bounds__(512) front_end_kernel(const FrontArgs A) {
     cg::grid_group grid = cg::this_grid();
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int warps_per_block = blockDim.x >> 5;
-    const int gwarp = blockIdx.x * warps_per_block + warp, nwarps = gridDim.x * warps_per_block;
+    const int nb = A.nb;
+    const int slot = blockIdx.x % nb, sblock = blockIdx.x / nb;
+    const int sblocks = ((int)gridDim.x - slot + nb - 1) / nb;          // blocks that serve this slot
+    const int gwarp = sblock * warps_per_block + warp, nwarps = sblocks * warps_per_block;
     const int N = A.N;
+    const int kp = A.k * A.p;
+    const double* __restrict__ H = A.H[slot];
+    const long long ldh = A.ldh;
+    DevScalars* sc = A.sc + slot;
     __shared__ double s_lo[32], s_hi[32];
     __shared__ double s_ab[2];
     for (int e = blockIdx.x * blockDim.x + threadIdx.x; e < A.ncounters; e += gridDim.x * blockDim.x) A.counters[e] = 0;
-    const bool vec = ((N & 1) == 0) && ((reinterpret_cast<uintptr_t>(A.H) & 15) == 0);
-    if (!A.explicit_bounds) {
-        double lo = INFINITY, hi = -INFINITY;
-        for (int row = gwarp; row < N; row += nwarps) {
-            const double* hr = A.H + (long long)row * N;
-            double r = 0.0, hii = 0.0;
-            if (vec) {
-                for (int j = 2 * lane; j < N; j += 64) {
-                    const double2 v = *reinterpret_cast<const double2*>(hr + j);
-                    if (j == row) hii = v.x; else r += fabs(v.x);
-                    if (j + 1 == row) hii = v.y; else r += fabs(v.y);
+    double a, b;
+    if (A.do_bounds) {
+        const bool vec = ((ldh & 1) == 0) && ((reinterpret_cast<uintptr_t>(H) & 15) == 0);
+        if (!A.explicit_bounds) {
+            double lo = INFINITY, hi = -INFINITY;
+            for (int row = gwarp; row < N; row += nwarps) {
+                const double* hr = H + (long long)row * ldh;
+                double r = 0.0, hii = 0.0;
+                if (vec) {
+                    for (int j = 2 * lane; j < N; j += 64) {
+                        if (j + 1 < N) {
+                            const double2 v = *reinterpret_cast<const double2*>(hr + j);
+                            if (j == row) hii = v.x; else r += fabs(v.x);
+                            if (j + 1 == row) hii = v.y; else r += fabs(v.y);
+                        } else {
+                            const double v = hr[j];
+                            if (j == row) hii = v; else r += fabs(v);
+                        }
+                    }
+                } else {
+                    for (int j = lane; j < N; j += 32) {
+                        const double v = hr[j];
+                        if (j == row) hii = v; else r += fabs(v);
+                    }
                 }
-            } else {
-                for (int j = lane; j < N; j += 32) {
-                    const double v = hr[j];
-                    if (j == row) hii = v; else r += fabs(v);
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1) {
+                    r += __shfl_xor_sync(0xffffffffu, r, o);
+                    hii += __shfl_xor_sync(0xffffffffu, hii, o);  // exactly one lane holds h_ii, the rest 0
+                }
+                lo = fmin(lo, hii - r);
+                hi = fmax(hi, hii + r);
+                if (!(isfinite(r) && isfinite(hii))) { lo = -INFINITY; hi = INFINITY; }
+            }
+            if (lane == 0) { s_lo[warp] = lo; s_hi[warp] = hi; }
+            __syncthreads();
+            if (warp == 0) {
+                lo = lane < warps_per_block ? s_lo[lane] : INFINITY;
+                hi = lane < warps_per_block ? s_hi[lane] : -INFINITY;
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1) {
+                    lo = fmin(lo, __shfl_xor_sync(0xffffffffu, lo, o));
+                    hi = fmax(hi, __shfl_xor_sync(0xffffffffu, hi, o));
+                }
+                if (lane == 0) {
+                    A.part[2 * blockIdx.x] = lo;
+                    A.part[2 * blockIdx.x + 1] = hi;
                 }
             }
+            grid.sync();
+            if (warp == 0) {
+                lo = INFINITY;
+                hi = -INFINITY;
+                for (int bIdx = slot + nb * lane; bIdx < (int)gridDim.x; bIdx += 32 * nb) {  // the blocks of this slot
+                    lo = fmin(lo, __ldcg(A.part + 2 * bIdx));
+                    hi = fmax(hi, __ldcg(A.part + 2 * bIdx + 1));
+                }
 #pragma unroll
-            for (int o = 16; o > 0; o >>= 1) {
-                r += __shfl_xor_sync(0xffffffffu, r, o);
-                hii += __shfl_xor_sync(0xffffffffu, hii, o);  // exactly one lane holds h_ii, the rest 0
+                for (int o = 16; o > 0; o >>= 1) {
+                    lo = fmin(lo, __shfl_xor_sync(0xffffffffu, lo, o));
+                    hi = fmax(hi, __shfl_xor_sync(0xffffffffu, hi, o));
+                }
+                if (lane == 0) {
+                    s_ab[0] = lo;
+                    s_ab[1] = hi;
+                }
             }
-            lo = fmin(lo, hii - r);
-            hi = fmax(hi, hii + r);
-            if (!(isfinite(r) && isfinite(hii))) { lo = -INFINITY; hi = INFINITY; }
-        }
-        if (lane == 0) { s_lo[warp] = lo; s_hi[warp] = hi; }
-        __syncthreads();
-        if (warp == 0) {
-            lo = lane < warps_per_block ? s_lo[lane] : INFINITY;
-            hi = lane < warps_per_block ? s_hi[lane] : -INFINITY;
-#pragma unroll
-            for (int o = 16; o > 0; o >>= 1) {
-                lo = fmin(lo, __shfl_xor_sync(0xffffffffu, lo, o));
-                hi = fmax(hi, __shfl_xor_sync(0xffffffffu, hi, o));
-            }
-            if (lane == 0) {
-                A.part[2 * blockIdx.x] = lo;
-                A.part[2 * blockIdx.x + 1] = hi;
-            }
-        }
-        grid.sync();
-        if (warp == 0) {
-            lo = INFINITY;
-            hi = -INFINITY;
-            for (int bIdx = lane; bIdx < (int)gridDim.x; bIdx += 32) {
-                lo = fmin(lo, __ldcg(A.part + 2 * bIdx));
-                hi = fmax(hi, __ldcg(A.part + 2 * bIdx + 1));
-            }
-#pragma unroll
-            for (int o = 16; o > 0; o >>= 1) {
-                lo = fmin(lo, __shfl_xor_sync(0xffffffffu, lo, o));
-                hi = fmax(hi, __shfl_xor_sync(0xffffffffu, hi, o));
-            }
-            if (lane == 0) {
-                s_ab[0] = lo;
-                s_ab[1] = hi;
-            }
+            __syncthreads();
+        } else if (threadIdx.x == 0) {
+            s_ab[0] = A.a;
+            s_ab[1] = A.b;
         }
         __syncthreads();
-    } else if (threadIdx.x == 0) {
-        s_ab[0] = A.a;
-        s_ab[1] = A.b;
-    }
-    __syncthreads();
-    double a = s_ab[0], b = s_ab[1];
-    const bool bad = !(isfinite(a) && isfinite(b));
-    if (a == b) { a -= 1.0; b += 1.0; }  // degenerate H = cI (reading A2-iv)
-    if (blockIdx.x == 0 && threadIdx.x == 0) {
-        A.sc->a = a;
-        A.sc->b = b;
-        A.sc->bad_bounds = bad ? 1 : 0;
-    }
-    // ---- phase 2: rescale + Fermi values at the nodes ----
-    {
+        a = s_ab[0];
+        b = s_ab[1];
+        const bool bad = !(isfinite(a) && isfinite(b));
+        if (a == b) { a -= 1.0; b += 1.0; }  // degenerate H = cI (reading A2-iv)
+        if (sblock == 0 && threadIdx.x == 0) {
+            sc->a = a;
+            sc->b = b;
+            if (bad) sc->bad_bounds = 1;  // sticky
+        }
+        // ---- phase 2: rescale ----
         const double inv = 1.0 / (b - a), shift = a + b;
+        double* X = A.X + (long long)slot * A.slot_stride;
         for (int row = gwarp; row < N; row += nwarps) {
-            const double* hr = A.H + (long long)row * N;
-            double* xr = A.X + (long long)row * A.ldx;
+            const double* hr = H + (long long)row * ldh;
+            double* xr = X + (long long)row * A.ldx;
             if (vec) {
                 for (int j = 2 * lane; j < N; j += 64) {
-                    const double2 v = *reinterpret_cast<const double2*>(hr + j);
-                    double h0 = 2.0 * v.x, h1 = 2.0 * v.y;
-                    if (j == row) h0 -= shift;
-                    if (j + 1 == row) h1 -= shift;
-                    *reinterpret_cast<double2*>(xr + j) = make_double2(h0 * inv, h1 * inv);
+                    if (j + 1 < N) {
+                        const double2 v = *reinterpret_cast<const double2*>(hr + j);
+                        double h0 = 2.0 * v.x, h1 = 2.0 * v.y;
+                        if (j == row) h0 -= shift;
+                        if (j + 1 == row) h1 -= shift;
+                        *reinterpret_cast<double2*>(xr + j) = make_double2(h0 * inv, h1 * inv);
+                    } else {
+                        double h = 2.0 * hr[j];
+                        if (j == row) h -= shift;
+                        xr[j] = h * inv;
+                    }
                 }
             } else {
                 for (int j = lane; j < N; j += 32) {
@@ -243,15 +273,24 @@ __global__ void __launch_bounds__(512) front_end_kernel(const FrontArgs A) {
                 }
             }
         }
+    } else {
+        a = __ldcg(&sc->a);
+        b = __ldcg(&sc->b);
+    }
+    if (!A.do_coeffs) return;
+    double* fn = A.fn + (size_t)slot * A.Nq;
+    double* c = A.c + (size_t)slot * kp;
+    {
+        const double mu = A.mu_from_device ? __ldcg(&sc->mu) : A.mu[slot];
+        if (!A.mu_from_device && sblock == 0 && threadIdx.x == 0) sc->mu = mu;
         const double beta_t = A.beta * (b - a) * 0.5;
-        const double mu_t = (2.0 * A.mu - (a + b)) / (b - a);
-        for (int j = blockIdx.x * blockDim.x + threadIdx.x; j < A.Nq; j += gridDim.x * blockDim.x)
-            A.fn[j] = fermi_scaled(beta_t, mu_t, A.costab[2 * j + 1]);
+        const double mu_t = (2.0 * mu - (a + b)) / (b - a);
+        for (int j = sblock * blockDim.x + threadIdx.x; j < A.Nq; j += sblocks * blockDim.x)
+            fn[j] = fermi_scaled(beta_t, mu_t, A.costab[2 * j + 1]);
     }
     grid.sync();
     // ---- phase 3: c_n (one warp per coefficient) ----
     {
-        const int kp = A.k * A.p;
         const unsigned mask = 4u * (unsigned)A.Nq - 1u;
         for (int n = gwarp; n < kp; n += nwarps) {
             double cn = 0.0;
@@ -261,7 +300,7 @@ __global__ void __launch_bounds__(512) front_end_kernel(const FrontArgs A) {
                 s.lo = 0.0;
                 for (int j = lane; j < A.Nq; j += 32) {
                     const unsigned r = ((unsigned)n * (2u * (unsigned)j + 1u)) & mask;
-                    s = dd_add_prod(s, __ldcg(A.fn + j), A.costab[r]);
+                    s = dd_add_prod(s, __ldcg(fn + j), A.costab[r]);
                 }
 #pragma unroll
                 for (int o = 16; o > 0; o >>= 1) {
@@ -272,122 +311,207 @@ __global__ void __launch_bounds__(512) front_end_kernel(const FrontArgs A) {
                 }
                 cn = ((n == 0) ? 1.0 : 2.0) * (s.hi + s.lo) / (double)A.Nq;
             }
-            if (lane == 0) A.c[n] = cn;
+            if (lane == 0) c[n] = cn;
         }
     }
     grid.sync();
-    // ---- phase 4: tables (block 0).  Layout gT[l*k + i], dT likewise ----
-    if (blockIdx.x != 0) return;
+    // ---- phase 4: tables (first block of the slot).  Layout gT[l*k + i], dT likewise ----
+    if (sblock != 0) return;
     {
         const int k = A.k, p = A.p;
+        double* gT = A.gT + (size_t)slot * kp;
+        double* dT = A.dT + (size_t)slot * kp;
         // stage c in shared memory when it fits (one coalesced pass instead of 2p dependent L2 round trips per thread)
         __shared__ double s_c[FRONT_SMEM_COEFS];
-        const bool staged = (k * p <= FRONT_SMEM_COEFS);
+        __shared__ unsigned long long s_dmax;
+        const bool staged = (kp <= FRONT_SMEM_COEFS);
+        if (threadIdx.x == 0) s_dmax = 0ull;
         if (staged) {
-            for (int e = threadIdx.x; e < k * p; e += blockDim.x) s_c[e] = __ldcg(A.c + e);
-            __syncthreads();
+            for (int e = threadIdx.x; e < kp; e += blockDim.x) s_c[e] = __ldcg(c + e);
         }
-        const double* c = staged ? s_c : A.c;
-        for (int l = threadIdx.x; l < p; l += blockDim.x) A.gT[(size_t)l * k] = c[(size_t)l * k];
+        __syncthreads();
+        const double* cc = staged ? s_c : c;
+        for (int l = threadIdx.x; l < p; l += blockDim.x) gT[(size_t)l * k] = cc[(size_t)l * k];
         // pairs (i, k-i), 1 <= i <= k/2 (i == k-i when k is even and i = k/2)
         for (int i = 1 + threadIdx.x; 2 * i <= k; i += blockDim.x) {
             const int i2 = k - i;
             double g1 = 0.0, g2 = 0.0;  // g_{i,l+1}, g_{k-i,l+1}
             for (int l = p - 1; l >= 0; --l) {
-                const double c1 = c[(size_t)l * k + i], c2 = c[(size_t)l * k + i2];
+                const double c1 = cc[(size_t)l * k + i], c2 = cc[(size_t)l * k + i2];
                 double n1, n2;
                 if (p == 1) { n1 = c1; n2 = c2; }
                 else if (l == p - 1) { n1 = 2.0 * c1; n2 = 2.0 * c2; }
                 else if (l >= 1) { n1 = 2.0 * c1 - g2; n2 = 2.0 * c2 - g1; }
                 else { n1 = c1 - 0.5 * g2; n2 = c2 - 0.5 * g1; }
-                A.gT[(size_t)l * k + i] = n1;
-                A.gT[(size_t)l * k + i2] = n2;
+                gT[(size_t)l * k + i] = n1;
+                gT[(size_t)l * k + i2] = n2;
                 g1 = n1;
                 g2 = n2;
             }
         }
         if (A.want_d) {
             __syncthreads();
+            double dmax = 0.0;
             for (int i = threadIdx.x; i < k; i += blockDim.x) {
                 for (int l = p - 1; l >= 0; --l) {
-                    double s = A.gT[(size_t)l * k + i];
-                    for (int j = l + 1; j < p; ++j) s -= A.Amat[(size_t)j * p + l] * A.dT[(size_t)j * k + i];
-                    A.dT[(size_t)l * k + i] = s / A.Amat[(size_t)l * p + l];
+                    double s = gT[(size_t)l * k + i];
+                    for (int j = l + 1; j < p; ++j) s -= A.Amat[(size_t)j * p + l] * dT[(size_t)j * k + i];
+                    const double d = s / A.Amat[(size_t)l * p + l];
+                    dT[(size_t)l * k + i] = d;
+                    dmax = fmax(dmax, fabs(d));
                 }
+            }
+            if (!(dmax <= 1.7e308)) dmax = 1.7e308;  // NaN / inf trip the guard too
+            atomicMax(&s_dmax, (unsigned long long)__double_as_longlong(dmax));  // non-negative doubles order like integers
+            __syncthreads();
+            if (threadIdx.x == 0) {
+                const double m = __longlong_as_double((long long)s_dmax);
+                if (m * 2.220446049250313e-16 * (double)p > 1e-12) sc->noconv = 1;  // sticky (reading A6)
             }
         }
     }
 }
 
 // ---------------------------------------------------------------------------------------------------
-// a-7: trace.  One block, fixed summation order (bitwise reproducible).  8N useful bytes.
+// a-7: trace.  One block per matrix, fixed summation order (bitwise reproducible).  8N useful bytes each.
 // ---------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(1024) trace_kernel(const double* __restrict__ D, int N, long long ld, double* __restrict__ out) {
+struct TraceArgs {
+    const double* D[MAX_BATCH];
+};
+__global__ void __launch_bounds__(1024) trace_kernel(const TraceArgs A, int N, long long ld, double* __restrict__ out) {
     __shared__ dd s_buf[32];
+    const double* __restrict__ D = A.D[blockIdx.x];
     dd s;
     s.hi = 0.0;
     s.lo = 0.0;
     for (int i = threadIdx.x; i < N; i += blockDim.x) s = dd_add_prod(s, D[(long long)i * ld + i], 1.0);
     s = dd_block_reduce(s, s_buf);
-    if (threadIdx.x == 0) out[0] = s.hi + s.lo;
+    if (threadIdx.x == 0) out[blockIdx.x] = s.hi + s.lo;
 }
 
 // ---------------------------------------------------------------------------------------------------
-// a-7: moments tau_n = tr T_n(X) (reading A10).
-//   frob_partial_kernel: block (i, chunk): partial <U, T_{i+1}> over a slice of rows, i < count;
-//                        i == count: partial tr U; i == count + 1 + n: partial tr T_{n+1}, n < ntrace.
-//   moments_kernel (one block): tau_0 = N; tau_i = tr T_i (i <= k); for j >= 1:
-//       tau_{jk} = tr U_j,  tau_{jk+i} = 2 <U_j, T_i> - tau_{jk-i}  (Eq. 7 + symmetry), U_j = T_j(T_k).
-//   Partials are summed in a fixed order (bitwise reproducible).
+// a-7: moments tau_n = tr T_n(X), n < k p (reading A10).  With U_j = T_j(T_k) = T_{jk}(X):
+//     tau_i = tr T_i (i <= k),  tau_{jk} = tr U_j,  tau_{jk+i} = 2 <U_j, T_i>_F - tau_{jk-i}   (Eq. 7 + symmetry).
+// The baby block T_1..T_k and the giant block U_2..U_{p-1} are resident in the workspace (U_1 = T_k), so all inner
+// products are ONE skinny GEMM over the matrix elements,  Gram[j][i] = sum_e U_j[e] T_i[e]  (K = N ld elements),
+// which reads every matrix once per 32 x 32 block of the Gram matrix instead of k-1 matrices per product epilogue.
+//   diag_traces_kernel: block (m, slot): trace of the m-th workspace matrix (T_1..T_k, then U_2..U_{p-1})
+//   gram_kernel       : grid (CTAs, passes, slots); a pass is one 32 x 32 block (rb, cb) of the Gram matrix; every warp
+//                       owns a contiguous range of 8-element chunks and accumulates its 32 x 32 partial on the tensor
+//                       cores (DMMA.8x8x4: lane (g, t) feeds element pair 2t, 2t+1 of row-matrix g and column-matrix g);
+//                       the 8 warps are added in a fixed order, one partial per CTA
+//   moments_kernel    : one block per slot: sums the CTA partials in a fixed order, then the tau recurrence
+// Pad columns of every workspace matrix are zero, so the padded elements contribute nothing.
 // ---------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256) frob_partial_kernel(const double* __restrict__ U, const double* __restrict__ Tbase,
-                                                           long long stride, long long ld, int N, int count, int ntrace,
-                                                           double* __restrict__ part) {
+__global__ void __launch_bounds__(256) diag_traces_kernel(const double* __restrict__ Tbase, const double* __restrict__ Ubase,
+                                                          long long stride, long long slot_stride, long long ld, int N, int k,
+                                                          double* __restrict__ traces, int nmat) {
     __shared__ dd s_buf[32];
-    const int i = blockIdx.x, chunk = blockIdx.y, nchunks = gridDim.y;
-    const int r0 = (int)((long long)N * chunk / nchunks), r1 = (int)((long long)N * (chunk + 1) / nchunks);
+    const int m = blockIdx.x, slot = blockIdx.y;
+    const double* Mx = (m < k ? Tbase + (long long)m * stride : Ubase + (long long)(m - k) * stride) + (long long)slot * slot_stride;
     dd s;
     s.hi = 0.0;
     s.lo = 0.0;
-    if (i < count) {
-        const double* Ti = Tbase + (long long)i * stride;
-        for (int r = r0; r < r1; ++r)
-            for (int c = threadIdx.x; c < N; c += blockDim.x) s = dd_add_prod(s, U[(long long)r * ld + c], Ti[(long long)r * ld + c]);
-    } else {
-        const double* Mx = (i == count) ? U : Tbase + (long long)(i - count - 1) * stride;
-        for (int r = r0 + threadIdx.x; r < r1; r += blockDim.x) s = dd_add_prod(s, Mx[(long long)r * ld + r], 1.0);
-    }
+    for (int r = threadIdx.x; r < N; r += blockDim.x) s = dd_add_prod(s, Mx[(long long)r * ld + r], 1.0);
     s = dd_block_reduce(s, s_buf);
-    if (threadIdx.x == 0) part[(size_t)i * nchunks + chunk] = s.hi + s.lo;
+    if (threadIdx.x == 0) traces[(size_t)slot * nmat + m] = s.hi + s.lo;
 }
 
-// part1: [k-1 dots | tr U_1 | tr T_1..T_k] x nchunks from frob_partial_kernel (U = T_k);
-// dots: [j][tile][k] from the fused epilogues of the chain U_j, j = 2..p-1 (slot k-1 = trace).
-__global__ void moments_kernel(const double* __restrict__ part1, int nchunks, const double* __restrict__ dots, int tiles, int k, int p,
-                               int N, double* __restrict__ tau) {
-    const int kp = k * p;
-    if (threadIdx.x == 0) tau[0] = (double)N;
-    for (int n = 1 + threadIdx.x; n <= k && n < kp; n += blockDim.x) {
-        double s = 0.0;
-        for (int ch = 0; ch < nchunks; ++ch) s += part1[(size_t)(k + n - 1) * nchunks + ch];
-        tau[n] = s;
+constexpr int GRAM_BLK = 32;
+__global__ void __launch_bounds__(256) gram_kernel(const double* __restrict__ Tbase, const double* __restrict__ Ubase, long long stride,
+                                                   long long slot_stride, long long nelem, int k, int p,
+                                                   double* __restrict__ partial /* [slot][pass][cta][32*32] */) {
+    __shared__ double s_acc[GRAM_BLK * GRAM_BLK];
+    const int R = p - 1, Cn = k - 1;                       // Gram rows (U_1..U_{p-1}) and columns (T_1..T_{k-1})
+    const int npc = (Cn + GRAM_BLK - 1) / GRAM_BLK;
+    const int rb = blockIdx.y / npc, cb = blockIdx.y - rb * npc;
+    const int slot = blockIdx.z;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, g = lane >> 2, t = lane & 3;
+    const double* Ts = Tbase + (long long)slot * slot_stride;
+    const double* Us = Ubase + (long long)slot * slot_stride;
+    const double* rowp[4];
+    const double* colp[4];
+    bool rowv[4], colv[4];
+#pragma unroll
+    for (int mb = 0; mb < 4; ++mb) {
+        const int r = rb * GRAM_BLK + mb * 8 + g;
+        rowv[mb] = r < R;
+        rowp[mb] = (r == 0 || !rowv[mb]) ? Ts + (long long)(k - 1) * stride : Us + (long long)(r - 1) * stride;  // U_1 = T_k
+        const int q = cb * GRAM_BLK + mb * 8 + g;
+        colv[mb] = q < Cn;
+        colp[mb] = Ts + (long long)(colv[mb] ? q : 0) * stride;
     }
+    double acc[4][4][2];
+#pragma unroll
+    for (int i = 0; i < 4; ++i)
+#pragma unroll
+        for (int j = 0; j < 4; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
+    const long long nchunks = nelem / 8;                  // nelem = N ld, ld a multiple of 16
+    const long long W = (long long)gridDim.x * 8, w = (long long)blockIdx.x * 8 + warp;
+    const long long per = (nchunks + W - 1) / W;
+    const long long c0 = w * per, c1 = (c0 + per < nchunks) ? c0 + per : nchunks;
+#pragma unroll 2
+    for (long long ch = c0; ch < c1; ++ch) {
+        const long long e = ch * 8 + 2 * t;
+        double2 a[4], b[4];
+#pragma unroll
+        for (int mb = 0; mb < 4; ++mb) {
+            a[mb] = rowv[mb] ? __ldcs(reinterpret_cast<const double2*>(rowp[mb] + e)) : make_double2(0.0, 0.0);
+            b[mb] = colv[mb] ? __ldcs(reinterpret_cast<const double2*>(colp[mb] + e)) : make_double2(0.0, 0.0);
+        }
+#pragma unroll
+        for (int i = 0; i < 4; ++i)
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                dmma_884(acc[i][j][0], acc[i][j][1], a[i].x, b[j].x);
+                dmma_884(acc[i][j][0], acc[i][j][1], a[i].y, b[j].y);
+            }
+    }
+    // fixed-order sum of the 8 warps (each lane owns distinct entries), one partial per CTA
+    for (int e = threadIdx.x; e < GRAM_BLK * GRAM_BLK; e += blockDim.x) s_acc[e] = 0.0;
+    __syncthreads();
+    for (int wv = 0; wv < 8; ++wv) {
+        if (warp == wv) {
+#pragma unroll
+            for (int i = 0; i < 4; ++i)
+#pragma unroll
+                for (int j = 0; j < 4; ++j) {
+                    s_acc[(i * 8 + g) * GRAM_BLK + j * 8 + 2 * t] += acc[i][j][0];
+                    s_acc[(i * 8 + g) * GRAM_BLK + j * 8 + 2 * t + 1] += acc[i][j][1];
+                }
+        }
+        __syncthreads();
+    }
+    double* dst = partial + (((size_t)slot * gridDim.y + blockIdx.y) * gridDim.x + blockIdx.x) * (GRAM_BLK * GRAM_BLK);
+    for (int e = threadIdx.x; e < GRAM_BLK * GRAM_BLK; e += blockDim.x) dst[e] = s_acc[e];
+}
+
+// traces: [slot][nmat] (T_1..T_k, U_2..U_{p-1}); partial: gram_kernel's output; gram: scratch [slot][(p-1)(k-1)].
+__global__ void __launch_bounds__(256) moments_kernel(const double* __restrict__ traces, int nmat, const double* __restrict__ partial,
+                                                      int nctas, int npasses, double* __restrict__ gram, int k, int p, int N,
+                                                      double* __restrict__ tau_all) {
+    const int slot = blockIdx.x;
+    const int kp = k * p, R = p - 1, Cn = k - 1;
+    const int npc = (Cn + GRAM_BLK - 1) / GRAM_BLK;
+    double* tau = tau_all + (size_t)slot * kp;
+    double* G = gram + (size_t)slot * (size_t)(R > 0 ? R : 1) * (Cn > 0 ? Cn : 1);
+    const double* tr = traces + (size_t)slot * nmat;
+    for (int e = threadIdx.x; e < R * Cn; e += blockDim.x) {
+        const int r = e / Cn, q = e - r * Cn;
+        const int pass = (r / GRAM_BLK) * npc + q / GRAM_BLK;
+        const double* src = partial + ((size_t)slot * npasses + pass) * nctas * (GRAM_BLK * GRAM_BLK) + (r % GRAM_BLK) * GRAM_BLK + q % GRAM_BLK;
+        dd s;
+        s.hi = 0.0;
+        s.lo = 0.0;
+        for (int cta = 0; cta < nctas; ++cta) s = dd_add_prod(s, src[(size_t)cta * (GRAM_BLK * GRAM_BLK)], 1.0);
+        G[e] = s.hi + s.lo;
+    }
+    if (threadIdx.x == 0) tau[0] = (double)N;
+    for (int n = 1 + threadIdx.x; n <= k && n < kp; n += blockDim.x) tau[n] = tr[n - 1];
     __syncthreads();
     for (int j = 1; j < p; ++j) {
-        for (int i = 1 + threadIdx.x; i < k; i += blockDim.x) {
-            double s = 0.0;
-            if (j == 1) {
-                for (int ch = 0; ch < nchunks; ++ch) s += part1[(size_t)(i - 1) * nchunks + ch];
-            } else {
-                for (int t = 0; t < tiles; ++t) s += dots[((size_t)j * tiles + t) * k + (i - 1)];
-            }
-            tau[j * k + i] = 2.0 * s - tau[j * k - i];
-        }
-        if (threadIdx.x == 0 && j >= 2) {
-            double s = 0.0;
-            for (int t = 0; t < tiles; ++t) s += dots[((size_t)j * tiles + t) * k + (k - 1)];
-            tau[j * k] = s;
-        }
+        if (threadIdx.x == 0 && j >= 2) tau[j * k] = tr[k + j - 2];  // tr U_j (tau_k = tr T_k is already set)
+        for (int i = 1 + threadIdx.x; i < k; i += blockDim.x) tau[j * k + i] = 2.0 * G[(size_t)(j - 1) * Cn + (i - 1)] - tau[j * k - i];
         __syncthreads();
     }
 }
@@ -396,13 +520,14 @@ __global__ void moments_kernel(const double* __restrict__ part1, int nchunks, co
 // a-7: mu search.  N_e(mu) = sum_n c_n(mu) tau_n = sum_j f~(x_j; mu) w_j with the mu-independent weights
 //   w_j = (1/N_q) sum_{n<M} (2 - delta_n0) tau_n cos(n theta_j)
 // (the DCT of cheb_dm_coeffs with the two sums exchanged), so one bisection step costs N_q Fermi values.
-//   mu_weights_kernel: block j -> w[j]
-//   mu_bisect_kernel : one block, `iters` halvings of [a,b]: N_e(mid) < n_occ ? lo = mid : hi = mid.
+//   mu_weights_kernel: block (j, slot) -> w[slot][j]
+//   mu_bisect_kernel : one block per slot, `iters` halvings of [a,b]: N_e(mid) < n_occ ? lo = mid : hi = mid.
 // ---------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(128) mu_weights_kernel(const double* __restrict__ tau, const double* __restrict__ costab, int Nq, int M,
-                                                         double* __restrict__ w) {
+__global__ void __launch_bounds__(128) mu_weights_kernel(const double* __restrict__ tau_all, const double* __restrict__ costab, int Nq, int M,
+                                                         int kp, double* __restrict__ w_all) {
     __shared__ dd s_buf[32];
-    const int j = blockIdx.x;
+    const int j = blockIdx.x, slot = blockIdx.y;
+    const double* tau = tau_all + (size_t)slot * kp;
     const unsigned mask = 4u * (unsigned)Nq - 1u;
     dd s;
     s.hi = 0.0;
@@ -412,13 +537,19 @@ __global__ void __launch_bounds__(128) mu_weights_kernel(const double* __restric
         s = dd_add_prod(s, (n == 0 ? 1.0 : 2.0) * tau[n], costab[r]);
     }
     s = dd_block_reduce(s, s_buf);
-    if (threadIdx.x == 0) w[j] = (s.hi + s.lo) / (double)Nq;
+    if (threadIdx.x == 0) w_all[(size_t)slot * Nq + j] = (s.hi + s.lo) / (double)Nq;
 }
 
-__global__ void __launch_bounds__(1024) mu_bisect_kernel(DevScalars* sc, double beta, double n_occ, int iters,
-                                                         const double* __restrict__ costab, int Nq, const double* __restrict__ w) {
+struct BisectArgs {
+    double n_occ[MAX_BATCH];
+};
+__global__ void __launch_bounds__(1024) mu_bisect_kernel(DevScalars* sc_all, double beta, const BisectArgs B, int iters,
+                                                         const double* __restrict__ costab, int Nq, const double* __restrict__ w_all) {
     __shared__ dd s_buf[32];
     __shared__ double s_lo, s_hi, s_ne;
+    DevScalars* sc = sc_all + blockIdx.x;
+    const double* w = w_all + (size_t)blockIdx.x * Nq;
+    const double n_occ = B.n_occ[blockIdx.x];
     const double a = sc->a, b = sc->b;
     const double beta_t = beta * (b - a) * 0.5;
     if (threadIdx.x == 0) { s_lo = a; s_hi = b; s_ne = 0.0; }
@@ -461,10 +592,13 @@ __global__ void __launch_bounds__(1024) mu_bisect_kernel(DevScalars* sc, double 
 constexpr int SUMS_CHUNK = 16;
 // With symmetric-tile skipping (symBM > 0) only the elements inside tiles that are work items of the giant steps are
 // formed (tile (tm, tn) of symBM x symBN with tm symBM + symBM - 1 >= tn symBN): the other tiles of G_l are never read.
-__global__ void __launch_bounds__(256) form_sums_kernel(const double* __restrict__ Tbase, long long stride, long long ld, int N, int k,
-                                                        int p, const double* __restrict__ coefT, double* __restrict__ Gbase,
-                                                        int symBM, int symBN) {
+__global__ void __launch_bounds__(256) form_sums_kernel(const double* __restrict__ Tbase0, long long stride, long long ld, int N, int k,
+                                                        int p, const double* __restrict__ coefT0, double* __restrict__ Gbase0,
+                                                        int symBM, int symBN, long long slot_stride) {
     extern __shared__ double s_coef[];  // [k][SUMS_CHUNK]
+    const double* __restrict__ Tbase = Tbase0 + (long long)blockIdx.z * slot_stride;   // blockIdx.z = matrix of the batch
+    double* __restrict__ Gbase = Gbase0 + (long long)blockIdx.z * slot_stride;
+    const double* __restrict__ coefT = coefT0 + (size_t)blockIdx.z * k * p;
     const int l0 = blockIdx.y * SUMS_CHUNK;
     const int nl = min(SUMS_CHUNK, p - l0);
     for (int e = threadIdx.x; e < k * SUMS_CHUNK; e += blockDim.x) {
@@ -526,10 +660,13 @@ __global__ void __launch_bounds__(256) form_sums_kernel(const double* __restrict
 // fragments from shared memory and 8 DMMA.8x8x4.  Same skipping of unneeded tiles, same diagonal term.
 //   grid = (ceil(N ld / 32 / 8), ceil(p / SUMS_CHUNK)), block = 256 (8 warps).
 // ---------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256) form_sums_dmma_kernel(const double* __restrict__ Tbase, long long stride, long long ld, int N, int k,
-                                                             int p, const double* __restrict__ coefT, double* __restrict__ Gbase,
-                                                             int symBM, int symBN) {
+__global__ void __launch_bounds__(256) form_sums_dmma_kernel(const double* __restrict__ Tbase0, long long stride, long long ld, int N, int k,
+                                                             int p, const double* __restrict__ coefT0, double* __restrict__ Gbase0,
+                                                             int symBM, int symBN, long long slot_stride) {
     extern __shared__ double s_coef[];  // [kpad][SUMS_CHUNK], kpad = (k - 1) rounded up to 4; row i - 1 <-> T_i; + [SUMS_CHUNK] diag
+    const double* __restrict__ Tbase = Tbase0 + (long long)blockIdx.z * slot_stride;   // blockIdx.z = matrix of the batch
+    double* __restrict__ Gbase = Gbase0 + (long long)blockIdx.z * slot_stride;
+    const double* __restrict__ coefT = coefT0 + (size_t)blockIdx.z * k * p;
     const int l0 = blockIdx.y * SUMS_CHUNK;
     const int nl = min(SUMS_CHUNK, p - l0);
     const int kk = k - 1, kpad = (kk + 3) & ~3;

@@ -1,7 +1,7 @@
-// cheb_dm.cu -- host side of the C ABI declared in include/cheb_dm.h: plan (block sizes, workspace,
+// cheb_dm.cu -- host side of the C ABI declared in include/cheb_dm.h: plan (block sizes, workspace slots,
 // TMA descriptors, task/dependency tables) and the launches of the sm_100a kernels.  Product code;
 // shares nothing with oracle/.  There is no CPU path: every step of the solve runs in the kernels of
-// gemm_dmma.cuh / aux_kernels.cuh.
+// gemm_dmma.cuh / giant_resident.cuh / aux_kernels.cuh.
 #include <cuda.h>
 #include <cuda_runtime.h>
 #include <math.h>
@@ -30,11 +30,12 @@ typedef GemmCfg<64, 32, 16, 16, 32, 8, 1> Cfg64x32w16;    //  8 consumer warps o
 typedef GemmCfg<64, 32, 32, 16, 32, 6, 1> Cfg64x32w32;    //  4 consumer warps of 32x16, 144 KB ring, 1 CTA/SM
 typedef GemmCfg<128, 64, 32, 16, 16, 6, 1> Cfg128x64w16;  // 16 consumer warps of 32x16, 144 KB ring, 1 CTA/SM
 typedef GemmCfg<32, 32, 16, 16, 32, 6, 2> Cfg32x32;       //  4 consumer warps of 16x16,  96 KB ring, 2 CTA/SM
-typedef GemmCfg<64, 64, 32, 16, 32, 6, 1> Cfg64x64w16;     //  8 consumer warps of 32x16, 192 KB ring, 1 CTA/SM
+typedef GemmCfg<64, 64, 32, 16, 32, 6, 1> Cfg64x64w16;    //  8 consumer warps of 32x16, 192 KB ring, 1 CTA/SM
 typedef GemmCfg<112, 64, 16, 32, 16, 6, 1> Cfg112x64;     // 14 consumer warps of 16x32, 132 KB ring, 1 CTA/SM (N ~ 1000: 144 tiles)
+typedef GemmCfg<64, 32, 16, 16, 32, 4, 2> Cfg64x32x2;     //  8 consumer warps of 16x16,  96 KB ring, 2 CTA/SM (batched small N)
 
 enum TileSel { TILE_AUTO = 0, TILE_128x128 = 1, TILE_128x64 = 2, TILE_64x64 = 3, TILE_64x32_W16 = 4, TILE_64x32_W32 = 5,
-               TILE_128x64_W16 = 6, TILE_32x32 = 7, TILE_112x64 = 8, TILE_64x64_W16 = 9, TILE_LAST = 9 };
+               TILE_128x64_W16 = 6, TILE_32x32 = 7, TILE_112x64 = 8, TILE_64x64_W16 = 9, TILE_64x32_X2 = 10, TILE_LAST = 10 };
 
 struct TileShape {
     int BM, BN, BK, box_slabs;
@@ -55,6 +56,7 @@ TileShape tile_shape(int sel) {
         case TILE_32x32: return shape_of<Cfg32x32>(0.60);
         case TILE_64x64_W16: return shape_of<Cfg64x64w16>(0.76);
         case TILE_112x64: return shape_of<Cfg112x64>(0.72);  // 14 consumer warps: two sub-partitions carry 4, two carry 3
+        case TILE_64x32_X2: return shape_of<Cfg64x32x2>(0.70);
         default: return shape_of<Cfg128x64w16>(0.80);
     }
 }
@@ -74,8 +76,17 @@ EncodeTiledFn get_encode_fn() {
     return fn;
 }
 
-struct HostTaskMeta {
-    int has_gemm;
+// One grouped launch works on a table: ntl "level tasks" (the products of the method in topological order), each
+// instantiated for every slot of the plan: task (lt, slot) at index lt * maxb + slot.  All tasks of a table have the
+// same number of work items.
+struct TaskTable {
+    std::vector<Task> h;
+    Task* d;
+    int ntl;
+    int items_per_task;
+    int ctr_task_off, ctr_panel_off;  // this table's regions of the counter block
+    int trace_base;
+    TaskTable() : d(nullptr), ntl(0), items_per_task(0), ctr_task_off(0), ctr_panel_off(0), trace_base(0) {}
 };
 
 }  // namespace
@@ -83,57 +94,58 @@ struct HostTaskMeta {
 enum { TIMING_SLOTS = 256 };
 
 struct cheb_dm_plan_s {
-    int N, M, k, p, Nq;
+    int N, M, k, p, Nq, maxb;
     cheb_dm_options_t opt;
     int device, num_sms;
     int tile;  // TileSel actually used
     int BM, BN, BK, box_slabs;
     long long ld;        // padded leading dimension of workspace matrices (multiple of 16)
+    long long ldh, ldd;  // leading dimensions of the caller's device matrices
     size_t mat_elems;    // elements per workspace matrix
-    int nmat;            // k + 2 (+ p when the sums are pre-formed)
-    double* ws;          // nmat matrices
-    // scalar tables (device)
-    double *costab, *fn, *c, *gT, *dT, *Amat, *tau, *w, *dots, *one, *part;
-    int front_grid;      // blocks of the cooperative front_end_kernel
+    int nmat;            // matrices per slot: T_1..T_k | buf0 buf1 | G_0..G_{p-1} (if any) | U_2..U_{p-1} (if any)
+    size_t slot_elems;   // nmat * mat_elems
+    int off_G, off_U;    // first matrix of the G / U blocks inside a slot (-1: absent)
+    double* ws;          // maxb slots
+    // scalar tables (device): costab, Amat, one are shared; the others are per slot
+    double *costab, *Amat, *one;
+    double *fn, *c, *gT, *dT, *tau, *w;
+    double *part;        // front end: per-block (lo, hi)
+    double *traces, *gram_part, *gram;  // moments: traces [slot][ntrmat], Gram partials, Gram
+    int ntrmat, gram_ctas, gram_passes;
+    int front_max_grid;  // co-resident blocks of the cooperative front_end_kernel
+    int gemm_per_sm;     // resident CTAs per SM of the product kernel instance of this plan
+    int scalar_sums;     // CHEB_DM_SCALAR_SUMS=1 at plan time: FP64-FMA form_sums_kernel (ablation)
     int preformed;       // 1: low-order sums G_l are formed by form_sums_kernel before the giant steps
     int sym;             // 1: symmetric-tile skipping in gemm_dmma_kernel
     int* sym_first;      // device: [tiles_n + 1] item prefix sums of a symmetric task
-    int resident;        // 1: giant steps run in giant_resident_kernel (small N), baby steps in gemm_dmma_kernel
+    int resident;        // 1: single solves run their giant steps in giant_resident_kernel (small N)
+    int moments_on;      // 1: the workspace holds the G and U blocks (cheb_dm_moments / solve / assemble)
     int res_tiles_m, res_tiles_n, res_grid, res_smem;
-    DevScalars* sc;
-    CUtensorMap* maps;   // nmat descriptors
+    DevScalars* sc;      // [maxb]
+    CUtensorMap* maps;   // maxb * nmaps_slot descriptors
+    int nmaps_slot, map_flatA, map_flatB;
     int tma2d;
     // task tables
-    int ntasks_solve;        // tasks [0, ntasks_solve) = the solve; [ntasks_solve, ntasks_all) = moments chain
-    int ntasks_all;
-    int nbaby;               // baby tasks are [0, nbaby)
-    int product_task;        // index of the scratch task used by cheb_dm_product
-    Task* tasks;             // device
-    int* task_first;         // device, ntasks_all + 2
-    std::vector<Task> h_tasks;
-    std::vector<int> h_first;
-    int* counters;           // device: [work counters | task_done | group_done | panel_done | error]
+    TaskTable baby, giant, chain, flat, misc;
+    int* counters;       // device: [error flag | work counters | per-table task_done and panel_done regions]
     size_t counters_ints;
-    int off_work, off_task, off_group, off_panel, off_error;
+    int nwork, work_next;
     int panel_stride;
-    int nwork;               // number of work counters (one per possible launch)
     // state
-    int have_coeffs, explicit_bounds, have_moments, computed;
+    int have_coeffs, explicit_bounds, have_moments, computed, blocks_nb;
     double beta, mu, a, b;
     int last_launches;
-    double flops_per_compute;
+    double flops_per_compute, flops_per_solve;
     size_t ws_bytes;
-    // host-buffer entry point (cheb_dm_compute_host): device staging for H, D and tr D
-    double *stage_H, *stage_D, *stage_tr;
-    // pipelined host entry point (cheb_dm_compute_host_async): second staging slot, copy streams, events
-    double *stage_H1, *stage_D1, *stage_tr1;
+    // host entry points: two staging sets (H, D, tr D for every slot), copy streams, events
+    double *stage_H[2], *stage_D[2], *stage_tr[2];
     cudaStream_t s_in, s_out;
     cudaEvent_t ev_in[2], ev_comp[2], ev_out[2];
     long long n_async;
     int pipe_ready;
     // optional per-tile timeline (cheb_dm_set_trace)
     TraceRec* trace_buf;
-    int trace_on;
+    int trace_on, trace_res_base, trace_total;
     // optional timing of the product launches (cheb_dm_set_timing)
     int timing;
     cudaEvent_t ev0[TIMING_SLOTS], ev1[TIMING_SLOTS];  // ring: compute number i uses slot i % TIMING_SLOTS
@@ -148,13 +160,18 @@ namespace {
         if (e__ != cudaSuccess) return CHEB_DM_ECUDA; \
     } while (0)
 
-double* T_ptr(const cheb_dm_plan_s* P, int n) {  // T_n, 1 <= n <= k
-    return P->ws + (size_t)(n - 1) * P->mat_elems;
+// ---- workspace layout: matrix m of slot s ----
+double* mat_ptr(const cheb_dm_plan_s* P, int s, int m) { return P->ws + (size_t)s * P->slot_elems + (size_t)m * P->mat_elems; }
+double* T_ptr(const cheb_dm_plan_s* P, int s, int n) { return mat_ptr(P, s, n - 1); }             // T_n, 1 <= n <= k
+double* buf_ptr(const cheb_dm_plan_s* P, int s, int i) { return mat_ptr(P, s, P->k + i); }        // ping-pong buffers
+double* G_ptr(const cheb_dm_plan_s* P, int s, int l) { return mat_ptr(P, s, P->off_G + l); }      // G_l, 0 <= l < p
+double* U_ptr(const cheb_dm_plan_s* P, int s, int j) {                                            // U_j = T_j(T_k), 1 <= j <= p-1
+    return j == 1 ? T_ptr(P, s, P->k) : mat_ptr(P, s, P->off_U + j - 2);
 }
-int T_map(int n) { return n - 1; }
-double* buf_ptr(const cheb_dm_plan_s* P, int i) { return P->ws + (size_t)(P->k + i) * P->mat_elems; }
-int buf_map(const cheb_dm_plan_s* P, int i) { return P->k + i; }
-double* G_ptr(const cheb_dm_plan_s* P, int l) { return P->ws + (size_t)(P->k + 2 + l) * P->mat_elems; }
+int T_map(const cheb_dm_plan_s* P, int s, int n) { return s * P->nmaps_slot + n - 1; }
+int buf_map(const cheb_dm_plan_s* P, int s, int i) { return s * P->nmaps_slot + P->k + i; }
+int flatA_map(const cheb_dm_plan_s* P, int s, int l) { return s * P->nmaps_slot + P->map_flatA + l - 1; }  // G_l, l >= 1
+int flatB_map(const cheb_dm_plan_s* P, int s, int j) { return s * P->nmaps_slot + P->map_flatB + j - 1; }  // U_j, j >= 1
 
 // Algorithm 1, reading A7 for s = 1.  Each entry: T_n = 2 T_l T_r - T_m.
 struct BabyProd {
@@ -220,10 +237,6 @@ void build_Amat(int p, std::vector<double>& A) {
     }
 }
 
-}  // namespace
-
-namespace {
-
 int ceil_div(int a, int b) { return (a + b - 1) / b; }
 
 // Work items of a product whose result is symmetric: tile (tm, tn) is computed iff it touches the lower triangle,
@@ -244,17 +257,18 @@ void choose_tile(cheb_dm_plan_s* P) {
     if (sel < TILE_AUTO || sel > TILE_LAST) sel = TILE_AUTO;
     if (sel == TILE_AUTO) {
         // One product is the unit of the serial chain (giant steps), so pick the shape that minimises the time of
-        // one product on this device: tiles per SM (whole waves, 1 CTA per SM) x tile area / main-loop efficiency.
+        // one product level on this device: tiles per SM (whole waves, 1 CTA per SM) x tile area / main-loop efficiency.
         // Large N -> 128x128 (least L2 traffic per flop); N ~ 1000 -> 128x64; N ~ 500 -> 64x32 (128 tiles).
-        // With symmetric-tile skipping only the lower-triangle tiles count (N <= 512: the giant steps run in the
-        // resident kernel and the tile shape only serves the throughput-bound baby phase: full count, as measured).
+        // With symmetric-tile skipping only the lower-triangle tiles count (single solves at N <= 512: the giant steps
+        // run in the resident kernel and the tile shape only serves the throughput-bound baby phase: full count, as
+        // measured).  A batch plan counts the tiles of all max_batch matrices of a level (they are claimed together).
         const int cand[5] = {TILE_128x128, TILE_128x64_W16, TILE_112x64, TILE_64x64_W16, TILE_64x32_W16};
         double best = 0.0;
         for (int c = 0; c < 5; ++c) {
             const TileShape t = tile_shape(cand[c]);
-            const bool count_sym = P->sym && P->N > 32 * GR_MAX_KTILES;
+            const bool count_sym = P->sym && (P->N > 32 * GR_MAX_KTILES || P->maxb > 1);
             if (cand[c] == TILE_64x64_W16 && !count_sym) continue;
-            const int tiles = count_sym ? sym_items(P->N, t.BM, t.BN) : ceil_div(P->N, t.BM) * ceil_div(P->N, t.BN);
+            const int tiles = (count_sym ? sym_items(P->N, t.BM, t.BN) : ceil_div(P->N, t.BM) * ceil_div(P->N, t.BN)) * P->maxb;
             const double cost = (double)ceil_div(tiles, P->num_sms) * t.BM * t.BN / t.eff;
             if (sel == TILE_AUTO || cost < best) {
                 sel = cand[c];
@@ -270,15 +284,15 @@ void choose_tile(cheb_dm_plan_s* P) {
     P->box_slabs = t.box_slabs;
 }
 
-Task blank_task(const cheb_dm_plan_s* P) {
+Task blank_task(const cheb_dm_plan_s* P, int slot) {
     Task t;
     memset(&t, 0, sizeof(t));
-    t.mapA = t.mapB = 0;
     t.ktiles = ceil_div(P->N, P->BK);
+    t.kchunks = 1;
     t.tiles_m = ceil_div(P->N, P->BM);
     t.tiles_n = ceil_div(P->N, P->BN);
-    t.sym = 0;
     t.nitems = t.tiles_m * t.tiles_n;
+    t.slot = slot;
     t.alpha = 1.0;
     t.lds = P->ld;
     t.sum_stride = (long long)P->mat_elems;
@@ -293,201 +307,239 @@ void add_dep(Task& t, int kind, int idx, int target) {
     ++t.ndeps;
 }
 
-// Groups: 0 = baby steps of the solve, 1 = giant steps, 2 = moments chain, 3 = cheb_dm_product scratch.
-enum { GROUP_BABY = 0, GROUP_GIANT = 1, GROUP_MOM = 2, GROUP_MISC = 3, NGROUPS = 4 };
-
-void build_tasks(cheb_dm_plan_s* P) {
-    const int k = P->k, p = P->p;
-    std::vector<Task>& T = P->h_tasks;
-    T.clear();
+void build_tables(cheb_dm_plan_s* P) {
+    const int k = P->k, p = P->p, B = P->maxb;
     const int tiles = ceil_div(P->N, P->BM) * ceil_div(P->N, P->BN);
     const int tiles_m = ceil_div(P->N, P->BM);
     // every matrix of the solve is a polynomial of X, hence symmetric: lower-triangle tiles only (option symmetric)
     const int stiles = P->sym ? sym_items(P->N, P->BM, P->BN) : tiles;
+    auto idx = [&](int lt, int s) { return lt * B + s; };
 
     // ---- baby steps: T_n = 2 T_l T_r - T_m (Eq. 7 / 22-23 / Algorithm 1) ----
-    std::vector<BabyProd> sched = baby_schedule(k, P->opt.pairing);
-    std::vector<int> task_of(k + 1, -1);  // task index that produces T_n (n >= 2)
-    for (const BabyProd& bp : sched) {
-        Task t = blank_task(P);
-        t.mapA = T_map(bp.l);
-        t.mapB = T_map(bp.r);
-        t.group = GROUP_BABY;
-        t.alpha = 2.0;
-        if (bp.m == 0) {
-            t.C = nullptr;
-            t.diag_const = -1.0;  // - T_0 = -I
-        } else {
-            t.C = T_ptr(P, bp.m);
-            t.ldc = P->ld;
-            t.beta = -1.0;
+    const int pairing = (P->opt.pairing == CHEB_DM_PAIR_AUTO) ? CHEB_DM_PAIR_BALANCED : P->opt.pairing;
+    std::vector<BabyProd> sched = baby_schedule(k, pairing);
+    {
+        TaskTable& tt = P->baby;
+        tt.ntl = (int)sched.size();
+        tt.items_per_task = stiles;
+        tt.h.assign((size_t)tt.ntl * B, Task());
+        std::vector<int> lt_of(k + 1, -1);  // level task that produces T_n (n >= 2)
+        for (int lt = 0; lt < tt.ntl; ++lt) {
+            const BabyProd& bp = sched[lt];
+            for (int s = 0; s < B; ++s) {
+                Task t = blank_task(P, s);
+                t.mapA = T_map(P, s, bp.l);
+                t.mapB = T_map(P, s, bp.r);
+                t.alpha = 2.0;
+                if (bp.m == 0) {
+                    t.diag_const = -1.0;  // - T_0 = -I
+                } else {
+                    t.C = T_ptr(P, s, bp.m);
+                    t.ldc = P->ld;
+                    t.beta = -1.0;
+                }
+                t.Out = T_ptr(P, s, bp.n);
+                t.ldo = P->ld;
+                const int deps[3] = {bp.l, bp.r, bp.m};
+                for (int d = 0; d < 3; ++d) {
+                    const int n = deps[d];
+                    if (n < 2) continue;
+                    bool dup = false;
+                    for (int e = 0; e < d; ++e) dup = dup || (deps[e] == n);
+                    if (!dup) add_dep(t, DEP_TASK, idx(lt_of[n], s), stiles);
+                }
+                t.sym = P->sym;
+                t.nitems = stiles;
+                tt.h[idx(lt, s)] = t;
+            }
+            lt_of[bp.n] = lt;
         }
-        t.Out = T_ptr(P, bp.n);
-        t.ldo = P->ld;
-        int deps[3] = {bp.l, bp.r, bp.m};
-        for (int d = 0; d < 3; ++d) {
-            const int n = deps[d];
-            if (n < 2) continue;
-            bool dup = false;
-            for (int e = 0; e < d; ++e) dup = dup || (deps[e] == n);
-            if (!dup) add_dep(t, DEP_TASK, task_of[n], stiles);
-        }
-        t.sym = P->sym;
-        t.nitems = stiles;
-        task_of[bp.n] = (int)T.size();
-        T.push_back(t);
     }
-    P->nbaby = (int)T.size();
-    const int baby_tiles = P->nbaby * stiles;
 
     // ---- giant steps ----
     // CHEBYSHEV: B_l = G_l + 2 Y B_{l+1} - B_{l+2} (l = p-1..1), D = G_0 + Y B_1 - B_2, G_l = sum_i g_{i,l} T_i.
     // POWER    : acc_j = S_j + Y acc_{j+1} (Eq. 4), S_j = sum_i d_{i,j} T_i (Eq. 21).
-    // B_l / acc_l lives in buf[l & 1]; Y = T_k.  Column panels of successive steps are independent chains, so
-    // step l only waits for the SAME column panel of step l+1 (DEP_PANEL_N).
-    const bool power = (P->opt.outer == CHEB_DM_OUTER_POWER);
-    const double* coefT = power ? P->dT : P->gT;
-    const int first_giant = (int)T.size();
-    for (int l = p - 1; l >= 0; --l) {
-        Task t = blank_task(P);
-        t.group = GROUP_GIANT;
-        const bool has_prod = (l + 1 <= p - 1);
-        if (has_prod) {
-            t.mapA = T_map(k);
-            t.mapB = buf_map(P, (l + 1) & 1);
-            t.alpha = (power || l == 0) ? 1.0 : 2.0;
-            if (!power && l + 2 <= p - 1) {
-                t.C = buf_ptr(P, (l + 2) & 1);
-                t.ldc = P->ld;
-                t.beta = -1.0;
+    // B_l / acc_l lives in buf[l & 1]; Y = T_k.  Without symmetric tiles the column panels of successive steps are
+    // independent chains (step l only waits for the SAME column panel of step l+1: DEP_PANEL_N).  The baby block is
+    // complete when this table is launched (stream order).
+    {
+        const bool power = (P->opt.outer == CHEB_DM_OUTER_POWER);
+        TaskTable& tt = P->giant;
+        tt.ntl = p;
+        const bool gsym = P->sym != 0;
+        tt.items_per_task = gsym ? stiles : tiles;
+        tt.h.assign((size_t)tt.ntl * B, Task());
+        for (int lt = 0; lt < p; ++lt) {
+            const int l = p - 1 - lt;
+            for (int s = 0; s < B; ++s) {
+                const double* coefT = (power ? P->dT : P->gT) + (size_t)s * k * p;
+                Task t = blank_task(P, s);
+                const bool has_prod = (l + 1 <= p - 1);
+                if (has_prod) {
+                    t.mapA = T_map(P, s, k);
+                    t.mapB = buf_map(P, s, (l + 1) & 1);
+                    t.alpha = (power || l == 0) ? 1.0 : 2.0;
+                    if (!power && l + 2 <= p - 1) {
+                        t.C = buf_ptr(P, s, (l + 2) & 1);
+                        t.ldc = P->ld;
+                        t.beta = -1.0;
+                    }
+                } else {
+                    t.ktiles = 0;
+                }
+                if (l == 0) {
+                    t.out_is_user = 1;
+                } else {
+                    t.Out = buf_ptr(P, s, l & 1);
+                    t.ldo = P->ld;
+                }
+                if (P->preformed) {
+                    // G_l / S_l was formed beforehand (diagonal term included): one extra tile, weight 1
+                    t.sum_base = G_ptr(P, s, l);
+                    t.sum_count = 1;
+                    t.coef = P->one;
+                    t.diag_ptr = nullptr;
+                } else {
+                    // low-order sum: T_1..T_{k-1} with coefficients row l of the table, T_0 = I through diag_ptr
+                    t.sum_base = T_ptr(P, s, 1);
+                    t.sum_count = k - 1;
+                    t.coef = coefT + (size_t)l * k + 1;
+                    t.diag_ptr = coefT + (size_t)l * k;
+                }
+                t.ndeps_early = 0;
+                // (symmetric tiles: a panel also receives mirrored blocks from the tiles of other panels, so the step
+                // waits for the whole previous step; the resident kernel has its own counters)
+                if (gsym) {
+                    t.sym = 1;
+                    t.nitems = stiles;
+                    if (has_prod) add_dep(t, DEP_TASK, idx(lt - 1, s), stiles);
+                } else if (has_prod) {
+                    add_dep(t, DEP_PANEL_N, idx(lt - 1, s), tiles_m);
+                }
+                tt.h[idx(lt, s)] = t;
             }
-        } else {
-            t.ktiles = 0;
         }
-        if (l == 0) {
+    }
+
+    // ---- giant block (cheb_dm_moments / cheb_dm_solve): U_j = T_j(Y), U_{j+1} = 2 Y U_j - U_{j-1}, j = 1..p-2, kept in
+    // the workspace (U_1 = Y = T_k, U_0 = I).  The baby block is complete when this table is launched. ----
+    if (P->moments_on) {
+        TaskTable& tt = P->chain;
+        tt.ntl = (p >= 3) ? p - 2 : 0;
+        tt.items_per_task = stiles;
+        tt.h.assign((size_t)tt.ntl * B, Task());
+        for (int lt = 0; lt < tt.ntl; ++lt) {
+            const int j = lt + 1;
+            for (int s = 0; s < B; ++s) {
+                Task t = blank_task(P, s);
+                t.mapA = T_map(P, s, k);
+                t.mapB = flatB_map(P, s, j);
+                t.alpha = 2.0;
+                if (j == 1) {
+                    t.diag_const = -1.0;
+                } else {
+                    t.C = U_ptr(P, s, j - 1);
+                    t.ldc = P->ld;
+                    t.beta = -1.0;
+                }
+                t.Out = U_ptr(P, s, j + 1);
+                t.ldo = P->ld;
+                t.sym = P->sym;
+                t.nitems = stiles;
+                if (j >= 2) add_dep(t, DEP_TASK, idx(lt - 1, s), stiles);
+                tt.h[idx(lt, s)] = t;
+            }
+        }
+        // ---- flat giant step: D = G_0 + sum_{l=1}^{p-1} G_l U_l as ONE long-K product ----
+        TaskTable& tf = P->flat;
+        tf.ntl = 1;
+        tf.items_per_task = stiles;
+        tf.h.assign((size_t)B, Task());
+        for (int s = 0; s < B; ++s) {
+            Task t = blank_task(P, s);
+            if (p >= 2) {
+                t.mapA = flatA_map(P, s, 1);
+                t.mapB = flatB_map(P, s, 1);
+                t.kchunks = p - 1;
+            } else {
+                t.ktiles = 0;
+            }
             t.out_is_user = 1;
-        } else {
-            t.Out = buf_ptr(P, l & 1);
-            t.ldo = P->ld;
-        }
-        if (P->preformed) {
-            // G_l / S_l was formed by form_sums_kernel (diagonal term included): one extra tile, weight 1
-            t.sum_base = G_ptr(P, l);
+            t.sum_base = G_ptr(P, s, 0);
             t.sum_count = 1;
             t.coef = P->one;
-            t.diag_ptr = nullptr;
-        } else {
-            // low-order sum: T_1..T_{k-1} with coefficients row l of the table, T_0 = I through diag_ptr
-            t.sum_base = T_ptr(P, 1);
-            t.sum_count = k - 1;
-            t.coef = coefT + (size_t)l * k + 1;
-            t.diag_ptr = coefT + (size_t)l * k;
-        }
-        // early: the baby block (operands of the low-order sum); late: the same column panel of the previous step
-        if (P->nbaby > 0) add_dep(t, DEP_GROUP, GROUP_BABY, baby_tiles);
-        t.ndeps_early = t.ndeps;
-        // (symmetric tiles: a panel also receives mirrored blocks from the tiles of other panels, so the step waits
-        // for the whole previous step; the resident kernel keeps full tiles and panel chains)
-        if (P->sym && !P->resident) {
-            t.sym = 1;
+            t.sym = P->sym;
             t.nitems = stiles;
-            if (has_prod) add_dep(t, DEP_TASK, (int)T.size() - 1, stiles);
-        } else if (has_prod) {
-            add_dep(t, DEP_PANEL_N, (int)T.size() - 1, tiles_m);
+            tf.h[s] = t;
         }
-        T.push_back(t);
     }
-    (void)first_giant;
-    P->ntasks_solve = (int)T.size();
 
-    // ---- moments chain (cheb_dm_moments): U_j = T_j(Y), U_{j+1} = 2 Y U_j - U_{j-1}, j = 1..p-2, with the
-    // Frobenius products <U_{j+1}, T_i>, i < k, fused into the epilogue (dot_count).  U_j lives in buf[j & 1]
-    // for j >= 2 (U_1 = Y = T_k, U_0 = I).
-    for (int j = 1; j + 1 <= p - 1; ++j) {
-        Task t = blank_task(P);
-        t.group = GROUP_MOM;
-        t.mapA = T_map(k);
-        t.mapB = (j == 1) ? T_map(k) : buf_map(P, j & 1);
-        t.alpha = 2.0;
-        if (j == 1) {
-            t.diag_const = -1.0;
-        } else if (j == 2) {
-            t.C = T_ptr(P, k);
-            t.ldc = P->ld;
-            t.beta = -1.0;
-        } else {
-            t.C = buf_ptr(P, (j - 1) & 1);
-            t.ldc = P->ld;
-            t.beta = -1.0;
-        }
-        t.Out = buf_ptr(P, (j + 1) & 1);
-        t.ldo = P->ld;
-        t.sum_base = T_ptr(P, 1);
-        t.dot_count = k - 1;  // <U_{j+1}, T_i> for i = 1..k-1; slot k-1 = tr U_{j+1} (= <U, T_0>)
-        t.dot_out = P->dots + (size_t)(j + 1) * tiles * k;  // slots of skipped tiles stay zero (memset at plan time)
-        t.sym = P->sym;                                     // U_j = T_j(T_k) is symmetric too; dots weight mirrored blocks x2
-        t.nitems = stiles;
-        if (P->nbaby > 0) add_dep(t, DEP_GROUP, GROUP_BABY, baby_tiles);
-        if (j >= 2) add_dep(t, DEP_TASK, (int)T.size() - 1, stiles);
-        T.push_back(t);
-    }
-    P->ntasks_all = (int)T.size();
-
-    // ---- scratch task of cheb_dm_product ----
+    // ---- scratch task of cheb_dm_product (slot 0) ----
     {
-        Task t = blank_task(P);
-        t.group = GROUP_MISC;
-        t.mapA = buf_map(P, 0);
-        t.mapB = buf_map(P, 1);
+        TaskTable& tt = P->misc;
+        tt.ntl = 1;
+        tt.items_per_task = tiles;
+        tt.h.assign((size_t)B, Task());
+        Task t = blank_task(P, 0);
+        t.mapA = buf_map(P, 0, 0);
+        t.mapB = buf_map(P, 0, 1);
         t.out_is_user = 1;
-        P->product_task = (int)T.size();
-        T.push_back(t);
+        tt.h[0] = t;
     }
 
-    P->h_first.assign(T.size() + 1, 0);
-    for (size_t i = 0; i < T.size(); ++i) P->h_first[i + 1] = P->h_first[i] + T[i].nitems;
-
-    double nprod = 0;  // executed products, counting only the tiles that are computed
+    // executed products, counting only the tiles that are computed
     const double res_frac = P->sym ? (double)(P->res_tiles_m + 1) / (2.0 * P->res_tiles_m) : 1.0;  // 32x32 lower-triangle tiles
-    for (int i = 0; i < P->ntasks_solve; ++i) {
-        if (T[i].ktiles <= 0) continue;
-        nprod += (P->resident && i >= P->nbaby) ? res_frac : (double)T[i].nitems / (double)tiles;
-    }
-    P->flops_per_compute = nprod * 2.0 * (double)P->N * (double)P->N * (double)P->N;
+    const double frac = (double)stiles / (double)tiles;
+    const double n3 = 2.0 * (double)P->N * (double)P->N * (double)P->N;
+    const double nbaby = (double)P->baby.ntl * frac;
+    const double ngiant = (p >= 2) ? (double)(p - 1) * (P->resident ? res_frac : frac) : 0.0;
+    P->flops_per_compute = (nbaby + ngiant) * n3;
+    const double ngen = (p >= 2) ? (double)(p - 1) * frac : 0.0;
+    const double gram_flops = 2.0 * (double)P->N * (double)P->ld * (double)(p > 1 ? p - 1 : 0) * (double)(k > 1 ? k - 1 : 0);
+    P->flops_per_solve = (nbaby + (double)P->chain.ntl * frac + ngen) * n3 + gram_flops;
 }
 
+cheb_dm_status_t encode_one(EncodeTiledFn enc, const cheb_dm_plan_s* P, CUtensorMap* out, void* base, int want2d) {
+    CUresult r;
+    if (!want2d) {
+        // {16 columns (128 B), N rows, ld/16 slabs}: a box of box_slabs slabs x BK rows lands in shared memory as
+        // [slab][row][128 B] with the 128-byte swizzle keyed on the row.
+        cuuint64_t dims[3] = {16, (cuuint64_t)P->N, (cuuint64_t)(P->ld / 16)};
+        cuuint64_t strides[2] = {(cuuint64_t)P->ld * 8, 128};
+        cuuint32_t box[3] = {16, (cuuint32_t)P->BK, (cuuint32_t)P->box_slabs};
+        cuuint32_t estr[3] = {1, 1, 1};
+        r = enc(out, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, base, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    } else {
+        cuuint64_t dims[2] = {(cuuint64_t)P->ld, (cuuint64_t)P->N};
+        cuuint64_t strides[1] = {(cuuint64_t)P->ld * 8};
+        cuuint32_t box[2] = {16, (cuuint32_t)P->BK};
+        cuuint32_t estr[2] = {1, 1};
+        r = enc(out, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, base, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    }
+    return r == CUDA_SUCCESS ? CHEB_DM_OK : CHEB_DM_ECUDA;
+}
+
+// Operand descriptors of slot s: T_1..T_k, buf0, buf1, then (moments_on) G_1..G_{p-1} and U_1..U_{p-1} as two
+// contiguous runs for the long-K product (U_1's entry describes T_k again).
 cheb_dm_status_t encode_maps(cheb_dm_plan_s* P) {
     EncodeTiledFn enc = get_encode_fn();
     if (!enc) return CHEB_DM_ECUDA;
-    const int nmaps = P->k + 2;  // operands of products: T_1..T_k and the two giant-step buffers
+    const int nmaps = P->nmaps_slot * P->maxb;
     std::vector<CUtensorMap> h(nmaps);
     const char* env2d = getenv("CHEB_DM_TMA2D");
     int want2d = (env2d && env2d[0] == '1') ? 1 : 0;
     for (int pass = 0; pass < 2; ++pass) {
         bool ok = true;
-        for (int i = 0; i < nmaps && ok; ++i) {
-            void* base = P->ws + (size_t)i * P->mat_elems;
-            CUresult r;
-            if (!want2d) {
-                // {16 columns (128 B), N rows, ld/16 slabs}: a box of 4 slabs x BK rows lands in shared memory as
-                // [slab][row][128 B] with the 128-byte swizzle keyed on the row.
-                cuuint64_t dims[3] = {16, (cuuint64_t)P->N, (cuuint64_t)(P->ld / 16)};
-                cuuint64_t strides[2] = {(cuuint64_t)P->ld * 8, 128};
-                cuuint32_t box[3] = {16, (cuuint32_t)P->BK, (cuuint32_t)P->box_slabs};
-                cuuint32_t estr[3] = {1, 1, 1};
-                r = enc(&h[i], CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, base, dims, strides, box, estr,
-                        CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
-                        CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-            } else {
-                cuuint64_t dims[2] = {(cuuint64_t)P->ld, (cuuint64_t)P->N};
-                cuuint64_t strides[1] = {(cuuint64_t)P->ld * 8};
-                cuuint32_t box[2] = {16, (cuuint32_t)P->BK};
-                cuuint32_t estr[2] = {1, 1};
-                r = enc(&h[i], CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, base, dims, strides, box, estr,
-                        CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
-                        CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-            }
-            ok = (r == CUDA_SUCCESS);
+        for (int s = 0; s < P->maxb && ok; ++s) {
+            CUtensorMap* hs = h.data() + (size_t)s * P->nmaps_slot;
+            for (int i = 0; i < P->k + 2 && ok; ++i) ok = encode_one(enc, P, hs + i, mat_ptr(P, s, i), want2d) == CHEB_DM_OK;
+            if (P->moments_on)
+                for (int l = 1; l <= P->p - 1 && ok; ++l) {
+                    ok = encode_one(enc, P, hs + P->map_flatA + l - 1, G_ptr(P, s, l), want2d) == CHEB_DM_OK &&
+                         encode_one(enc, P, hs + P->map_flatB + l - 1, U_ptr(P, s, l), want2d) == CHEB_DM_OK;
+                }
         }
         if (ok) {
             P->tma2d = want2d;
@@ -500,65 +552,327 @@ cheb_dm_status_t encode_maps(cheb_dm_plan_s* P) {
     return CHEB_DM_ECUDA;
 }
 
-template <class Cfg, bool DOTS>
-cheb_dm_status_t launch_inst(const LaunchArgs& la, int items, int num_sms, cudaStream_t st) {
-    static bool attr_set = false;
-    if (!attr_set) {
-        CUDA_TRY(cudaFuncSetAttribute(gemm_dmma_kernel<Cfg, DOTS>, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg::SMEM_BYTES));
-        attr_set = true;
+// Per plan (and therefore per device): opt in to the dynamic shared memory of the product kernel instance and record
+// how many of its CTAs fit an SM.
+template <class Cfg>
+cheb_dm_status_t prepare_inst(int* per_sm) {
+    CUDA_TRY(cudaFuncSetAttribute(gemm_dmma_kernel<Cfg>, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg::SMEM_BYTES));
+    CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(per_sm, gemm_dmma_kernel<Cfg>, Cfg::THREADS, Cfg::SMEM_BYTES));
+    return *per_sm >= 1 ? CHEB_DM_OK : CHEB_DM_ECUDA;
+}
+cheb_dm_status_t prepare_gemm(cheb_dm_plan_s* P) {
+    switch (P->tile) {
+        case TILE_128x128: return prepare_inst<Cfg128x128>(&P->gemm_per_sm);
+        case TILE_128x64: return prepare_inst<Cfg128x64>(&P->gemm_per_sm);
+        case TILE_64x64: return prepare_inst<Cfg64x64>(&P->gemm_per_sm);
+        case TILE_64x32_W16: return prepare_inst<Cfg64x32w16>(&P->gemm_per_sm);
+        case TILE_64x32_W32: return prepare_inst<Cfg64x32w32>(&P->gemm_per_sm);
+        case TILE_32x32: return prepare_inst<Cfg32x32>(&P->gemm_per_sm);
+        case TILE_112x64: return prepare_inst<Cfg112x64>(&P->gemm_per_sm);
+        case TILE_64x64_W16: return prepare_inst<Cfg64x64w16>(&P->gemm_per_sm);
+        case TILE_64x32_X2: return prepare_inst<Cfg64x32x2>(&P->gemm_per_sm);
+        default: return prepare_inst<Cfg128x64w16>(&P->gemm_per_sm);
     }
-    int per_sm = 1;
-    CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, gemm_dmma_kernel<Cfg, DOTS>, Cfg::THREADS, Cfg::SMEM_BYTES));
-    if (per_sm < 1) return CHEB_DM_ECUDA;
-    int grid = per_sm * num_sms;
-    if (grid > items) grid = items;
-    if (grid < 1) grid = 1;
-    gemm_dmma_kernel<Cfg, DOTS><<<grid, Cfg::THREADS, Cfg::SMEM_BYTES, st>>>(la);
+}
+
+template <class Cfg>
+cheb_dm_status_t launch_inst(const LaunchArgs& la, int grid, cudaStream_t st) {
+    gemm_dmma_kernel<Cfg><<<grid, Cfg::THREADS, Cfg::SMEM_BYTES, st>>>(la);
     CUDA_TRY(cudaGetLastError());
     return CHEB_DM_OK;
 }
-template <class Cfg>
-cheb_dm_status_t launch_cfg(const LaunchArgs& la, int items, int num_sms, cudaStream_t st, bool dots) {
-    return dots ? launch_inst<Cfg, true>(la, items, num_sms, st) : launch_inst<Cfg, false>(la, items, num_sms, st);
-}
 
-// Launch tasks [t0, t1) as one persistent grid; `work_slot` selects the work counter.
-cheb_dm_status_t launch_tasks(cheb_dm_plan_s* P, int t0, int t1, int use_deps, int work_slot, double* userD,
-                              long long ldD, cudaStream_t st) {
+// Launch the level tasks [lt0, lt1) of a table for the slots [0, nb) as one persistent grid.
+cheb_dm_status_t launch_tasks(cheb_dm_plan_s* P, const TaskTable& tt, int lt0, int lt1, int nb, int use_deps,
+                              double* const* userD, long long ldD, cudaStream_t st) {
+    if (lt1 <= lt0 || nb < 1) return CHEB_DM_OK;
     LaunchArgs la;
-    la.tasks = P->tasks;
-    la.task_first = P->task_first;
+    memset(&la, 0, sizeof(la));
+    la.tasks = tt.d;
     la.maps = P->maps;
-    la.work_counter = P->counters + P->off_work + work_slot;
-    la.task_done = P->counters + P->off_task;
-    la.panel_done = P->counters + P->off_panel;
-    la.group_done = P->counters + P->off_group;
+    la.work_counter = P->counters + 1 + (P->work_next++ % P->nwork);
+    la.task_done = P->counters + tt.ctr_task_off;
+    la.panel_done = P->counters + tt.ctr_panel_off;
     la.panel_stride = P->panel_stride;
-    la.task_begin = t0;
-    la.task_end = t1;
+    la.lt_begin = lt0;
+    la.lt_end = lt1;
+    la.nb = nb;
+    la.maxb = P->maxb;
+    la.items_per_task = tt.items_per_task;
     la.use_deps = use_deps;
     la.N = P->N;
-    la.userD = userD;
+    for (int s = 0; s < nb; ++s) la.userD[s] = userD ? userD[s] : nullptr;
     la.ldD = ldD;
     la.tma2d = P->tma2d;
     la.sym_first = P->sym_first;
-    la.error_flag = P->counters + P->off_error;
+    la.error_flag = P->counters;
     la.trace = P->trace_on ? P->trace_buf : nullptr;
-    const int items = P->h_first[t1] - P->h_first[t0];
+    la.trace_base = tt.trace_base + lt0 * tt.items_per_task;
+    const long long items = (long long)(lt1 - lt0) * nb * tt.items_per_task;
+    long long grid = (long long)P->gemm_per_sm * P->num_sms;
+    if (grid > items) grid = items;
+    if (grid < 1) grid = 1;
     ++P->last_launches;
-    bool dots = false;  // the moments chain needs the instance whose epilogue forms the Frobenius products
-    for (int t = t0; t < t1; ++t) dots = dots || (P->h_tasks[t].dot_out != nullptr);
     switch (P->tile) {
-        case TILE_128x128: return launch_cfg<Cfg128x128>(la, items, P->num_sms, st, dots);
-        case TILE_128x64: return launch_cfg<Cfg128x64>(la, items, P->num_sms, st, dots);
-        case TILE_64x64: return launch_cfg<Cfg64x64>(la, items, P->num_sms, st, dots);
-        case TILE_64x32_W16: return launch_cfg<Cfg64x32w16>(la, items, P->num_sms, st, dots);
-        case TILE_64x32_W32: return launch_cfg<Cfg64x32w32>(la, items, P->num_sms, st, dots);
-        case TILE_32x32: return launch_cfg<Cfg32x32>(la, items, P->num_sms, st, dots);
-        case TILE_112x64: return launch_cfg<Cfg112x64>(la, items, P->num_sms, st, dots);
-        case TILE_64x64_W16: return launch_cfg<Cfg64x64w16>(la, items, P->num_sms, st, dots);
-        default: return launch_cfg<Cfg128x64w16>(la, items, P->num_sms, st, dots);
+        case TILE_128x128: return launch_inst<Cfg128x128>(la, (int)grid, st);
+        case TILE_128x64: return launch_inst<Cfg128x64>(la, (int)grid, st);
+        case TILE_64x64: return launch_inst<Cfg64x64>(la, (int)grid, st);
+        case TILE_64x32_W16: return launch_inst<Cfg64x32w16>(la, (int)grid, st);
+        case TILE_64x32_W32: return launch_inst<Cfg64x32w32>(la, (int)grid, st);
+        case TILE_32x32: return launch_inst<Cfg32x32>(la, (int)grid, st);
+        case TILE_112x64: return launch_inst<Cfg112x64>(la, (int)grid, st);
+        case TILE_64x64_W16: return launch_inst<Cfg64x64w16>(la, (int)grid, st);
+        case TILE_64x32_X2: return launch_inst<Cfg64x32x2>(la, (int)grid, st);
+        default: return launch_inst<Cfg128x64w16>(la, (int)grid, st);
     }
+}
+
+// A whole table: one persistent launch (GROUPED), or one launch per level task (SERIAL: the paper's single-stream
+// mode, PAPER.md:190 -- the ablation baseline).
+cheb_dm_status_t run_table(cheb_dm_plan_s* P, const TaskTable& tt, int nb, double* const* userD, long long ldD, cudaStream_t st) {
+    if (tt.ntl <= 0) return CHEB_DM_OK;
+    if (P->opt.sched == CHEB_DM_SCHED_GROUPED) return launch_tasks(P, tt, 0, tt.ntl, nb, 1, userD, ldD, st);
+    for (int lt = 0; lt < tt.ntl; ++lt) {
+        cheb_dm_status_t s = launch_tasks(P, tt, lt, lt + 1, nb, 0, userD, ldD, st);
+        if (s != CHEB_DM_OK) return s;
+    }
+    return CHEB_DM_OK;
+}
+
+bool device_ok(const cheb_dm_plan_s* P) {
+    int dev = -1;
+    return cudaGetDevice(&dev) == cudaSuccess && dev == P->device;
+}
+
+int front_grid_for(const cheb_dm_plan_s* P, int nb) {
+    int want = ceil_div(P->N, 16);
+    const int kp = P->k * P->p;
+    if (ceil_div(kp, 16) > want) want = ceil_div(kp, 16);
+    if (ceil_div(P->Nq, 512) > want) want = ceil_div(P->Nq, 512);
+    long long g = (long long)want * nb;
+    if (g > P->front_max_grid) g = P->front_max_grid;
+    if (g < nb) g = nb;
+    return (int)g;
+}
+
+// Steps a-1 .. a-3 on the stream, one cooperative launch over the nb matrices: counters reset, bounds (+ rescale of H
+// into T_1), c_n, g (and d).  do_bounds / do_coeffs select the halves (cheb_dm_solve runs them apart).
+cheb_dm_status_t front_end(cheb_dm_plan_s* P, int nb, const double* const* dH, long long ldh, const double* mu, int do_bounds,
+                           int do_coeffs, int mu_from_device, cudaStream_t st) {
+    FrontArgs fa;
+    memset(&fa, 0, sizeof(fa));
+    fa.nb = nb;
+    fa.N = P->N;
+    for (int s = 0; s < nb; ++s) {
+        fa.H[s] = dH ? dH[s] : nullptr;
+        fa.mu[s] = mu ? mu[s] : P->mu;
+    }
+    fa.ldh = ldh;
+    fa.X = T_ptr(P, 0, 1);
+    fa.slot_stride = (long long)P->slot_elems;
+    fa.ldx = P->ld;
+    fa.sc = P->sc;
+    fa.explicit_bounds = P->explicit_bounds;
+    fa.a = P->a;
+    fa.b = P->b;
+    fa.part = P->part;
+    fa.counters = P->counters + 1;  // [0] is the sticky error flag
+    fa.ncounters = (int)P->counters_ints - 1;
+    fa.do_bounds = do_bounds;
+    fa.do_coeffs = do_coeffs;
+    fa.mu_from_device = mu_from_device;
+    fa.beta = P->beta;
+    fa.costab = P->costab;
+    fa.Nq = P->Nq;
+    fa.M = P->M;
+    fa.fn = P->fn;
+    fa.c = P->c;
+    fa.k = P->k;
+    fa.p = P->p;
+    fa.Amat = P->Amat;
+    fa.want_d = (P->opt.outer == CHEB_DM_OUTER_POWER) ? 1 : 0;
+    fa.gT = P->gT;
+    fa.dT = P->dT;
+    void* args[] = {(void*)&fa};
+    CUDA_TRY(cudaLaunchCooperativeKernel((const void*)front_end_kernel, dim3(front_grid_for(P, nb)), dim3(512), args, 0, st));
+    P->work_next = 0;
+    ++P->last_launches;
+    return CHEB_DM_OK;
+}
+
+// Low-order sums G_l = sum_i coef_{i,l} T_i of Eq. (21) for all l at once (a-5, batched form), nb matrices.
+// full = true: every element (the G_l are operands of the long-K product); false: only the tiles the giant steps read.
+cheb_dm_status_t form_sums(cheb_dm_plan_s* P, int nb, bool full, cudaStream_t st) {
+    const double* coefT = (P->opt.outer == CHEB_DM_OUTER_POWER) ? P->dT : P->gT;
+    const int symBM = (P->sym && !full) ? P->BM : 0;
+    if (P->scalar_sums) {  // FP64-FMA version (ablation)
+        const long long pairs = (long long)P->N * P->ld / 2;
+        dim3 grid((unsigned)((pairs + 255) / 256), (unsigned)ceil_div(P->p, SUMS_CHUNK), (unsigned)nb);
+        form_sums_kernel<<<grid, 256, sizeof(double) * P->k * SUMS_CHUNK, st>>>(T_ptr(P, 0, 1), (long long)P->mat_elems, P->ld, P->N, P->k, P->p,
+                                                                              coefT, G_ptr(P, 0, 0), symBM, P->BN, (long long)P->slot_elems);
+    } else {
+        const long long warps = ((long long)P->N * P->ld + 31) / 32;
+        dim3 grid((unsigned)((warps + 7) / 8), (unsigned)ceil_div(P->p, SUMS_CHUNK), (unsigned)nb);
+        const size_t smem = sizeof(double) * (size_t)((((P->k - 1) + 3) & ~3) + 1) * SUMS_CHUNK;
+        form_sums_dmma_kernel<<<grid, 256, smem, st>>>(T_ptr(P, 0, 1), (long long)P->mat_elems, P->ld, P->N, P->k, P->p, coefT, G_ptr(P, 0, 0),
+                                                       symBM, P->BN, (long long)P->slot_elems);
+    }
+    ++P->last_launches;
+    CUDA_TRY(cudaGetLastError());
+    return CHEB_DM_OK;
+}
+
+// Giant steps of ONE solve in the resident-multiplier kernel (slot 0 of the giant table); cooperative launch because
+// its CTAs wait on one another's panel counters.
+cheb_dm_status_t run_giant_resident(cheb_dm_plan_s* P, double* userD, long long ldD, cudaStream_t st) {
+    GiantArgs ga;
+    memset(&ga, 0, sizeof(ga));
+    ga.tasks = P->giant.d;
+    ga.maps = P->maps;
+    ga.first_task = 0;
+    ga.nsteps = P->giant.ntl;
+    ga.task_stride = P->maxb;
+    ga.N = P->N;
+    ga.ktiles = ceil_div(P->N, GR_BK);
+    ga.tiles_m = P->res_tiles_m;
+    ga.tiles_n = P->res_tiles_n;
+    ga.panel_done = P->counters + P->giant.ctr_panel_off;
+    ga.panel_stride = P->panel_stride;
+    ga.userD = userD;
+    ga.ldD = ldD;
+    ga.tma2d = P->tma2d;
+    ga.error_flag = P->counters;
+    ga.trace = P->trace_on ? P->trace_buf : nullptr;
+    ga.trace_base = P->trace_res_base;
+    ga.coefT = (P->opt.outer == CHEB_DM_OUTER_POWER) ? P->dT : P->gT;
+    ga.Tbase = T_ptr(P, 0, 1);
+    ga.Gbase = G_ptr(P, 0, 0);
+    ga.mat_stride = (long long)P->mat_elems;
+    ga.ld = P->ld;
+    ga.k = P->k;
+    ga.sym = P->sym;
+    void* args[] = {(void*)&ga};
+    CUDA_TRY(cudaLaunchCooperativeKernel((const void*)giant_resident_kernel, dim3(P->res_grid), dim3(GR_THREADS), args,
+                                         (size_t)P->res_smem, st));
+    ++P->last_launches;
+    return CHEB_DM_OK;
+}
+
+// Products of a fixed-mu solve after the front end: baby steps, sums, giant steps.
+cheb_dm_status_t run_products(cheb_dm_plan_s* P, int nb, double* const* dD, long long ldd, cudaStream_t st) {
+    cheb_dm_status_t s = run_table(P, P->baby, nb, dD, ldd, st);
+    if (s != CHEB_DM_OK) return s;
+    if (P->resident && nb == 1) return run_giant_resident(P, dD[0], ldd, st);
+    if (P->preformed) {
+        s = form_sums(P, nb, false, st);
+        if (s != CHEB_DM_OK) return s;
+    }
+    return run_table(P, P->giant, nb, dD, ldd, st);
+}
+
+cheb_dm_status_t compute_impl(cheb_dm_plan_s* P, int nb, const double* const* dH, long long ldh, double* const* dD, long long ldd,
+                              const double* mu, cudaStream_t st) {
+    P->last_launches = 0;
+    cheb_dm_status_t s = front_end(P, nb, dH, ldh, mu, 1, 1, 0, st);  // also zeroes the scheduler counters
+    if (s != CHEB_DM_OK) return s;
+    const int slot = (int)(P->ev_count % TIMING_SLOTS);
+    if (P->timing) CUDA_TRY(cudaEventRecord(P->ev0[slot], st));
+    s = run_products(P, nb, dD, ldd, st);
+    if (s != CHEB_DM_OK) return s;
+    if (P->timing) {
+        CUDA_TRY(cudaEventRecord(P->ev1[slot], st));
+        ++P->ev_count;
+    }
+    P->computed = 1;
+    P->blocks_nb = 0;  // the baby block in the workspace no longer belongs to a moments / solve call
+    P->have_moments = 0;
+    return CHEB_DM_OK;
+}
+
+// Baby block, giant block and moments of nb matrices (front end with bounds already run).
+cheb_dm_status_t blocks_and_moments(cheb_dm_plan_s* P, int nb, cudaStream_t st) {
+    cheb_dm_status_t s = run_table(P, P->baby, nb, nullptr, 0, st);
+    if (s != CHEB_DM_OK) return s;
+    s = run_table(P, P->chain, nb, nullptr, 0, st);
+    if (s != CHEB_DM_OK) return s;
+    const int k = P->k, p = P->p;
+    diag_traces_kernel<<<dim3(P->ntrmat, nb), 256, 0, st>>>(T_ptr(P, 0, 1), P->off_U >= 0 ? mat_ptr(P, 0, P->off_U) : T_ptr(P, 0, 1),
+                                                           (long long)P->mat_elems, (long long)P->slot_elems, P->ld, P->N, k, P->traces, P->ntrmat);
+    ++P->last_launches;
+    if (p >= 2 && k >= 2) {
+        gram_kernel<<<dim3(P->gram_ctas, P->gram_passes, nb), 256, 0, st>>>(T_ptr(P, 0, 1), P->off_U >= 0 ? mat_ptr(P, 0, P->off_U) : T_ptr(P, 0, 1),
+                                                                           (long long)P->mat_elems, (long long)P->slot_elems,
+                                                                           (long long)P->N * P->ld, k, p, P->gram_part);
+        ++P->last_launches;
+    }
+    moments_kernel<<<nb, 256, 0, st>>>(P->traces, P->ntrmat, P->gram_part, P->gram_ctas, P->gram_passes, P->gram, k, p, P->N, P->tau);
+    ++P->last_launches;
+    CUDA_TRY(cudaGetLastError());
+    return CHEB_DM_OK;
+}
+
+cheb_dm_status_t bisect(cheb_dm_plan_s* P, int nb, double beta, const double* n_occ, int iters, cudaStream_t st) {
+    BisectArgs ba;
+    memset(&ba, 0, sizeof(ba));
+    for (int s = 0; s < nb; ++s) ba.n_occ[s] = n_occ[s];
+    mu_weights_kernel<<<dim3(P->Nq, nb), 128, 0, st>>>(P->tau, P->costab, P->Nq, P->M, P->k * P->p, P->w);
+    mu_bisect_kernel<<<nb, 1024, 0, st>>>(P->sc, beta, ba, iters, P->costab, P->Nq, P->w);
+    P->last_launches += 2;
+    CUDA_TRY(cudaGetLastError());
+    return CHEB_DM_OK;
+}
+
+// D from the blocks in the workspace: coefficient tables (mu given, or the device's), sums, one long-K product.
+cheb_dm_status_t assemble_impl(cheb_dm_plan_s* P, int nb, const double* mu, int mu_from_device, double* const* dD, long long ldd,
+                               cudaStream_t st) {
+    cheb_dm_status_t s = front_end(P, nb, nullptr, 0, mu, 0, 1, mu_from_device, st);
+    if (s != CHEB_DM_OK) return s;
+    s = form_sums(P, nb, true, st);
+    if (s != CHEB_DM_OK) return s;
+    return run_table(P, P->flat, nb, dD, ldd, st);
+}
+
+cheb_dm_status_t trace_impl(cheb_dm_plan_s* P, int nb, const double* const* dD, long long ldd, double* out, cudaStream_t st) {
+    TraceArgs ta;
+    memset(&ta, 0, sizeof(ta));
+    for (int s = 0; s < nb; ++s) ta.D[s] = dD[s];
+    trace_kernel<<<nb, 1024, 0, st>>>(ta, P->N, ldd, out);
+    CUDA_TRY(cudaGetLastError());
+    return CHEB_DM_OK;
+}
+
+// Staging sets of the host entry points: `sets` of them (1 or 2); 2 also creates the copy streams and events.
+cheb_dm_status_t ensure_staging(cheb_dm_plan_s* P, int sets) {
+    const size_t bytes = sizeof(double) * (size_t)P->N * P->N * P->maxb;
+    for (int i = 0; i < sets; ++i) {
+        if (P->stage_H[i]) continue;
+        const bool ok = cudaMalloc(&P->stage_H[i], bytes) == cudaSuccess && cudaMalloc(&P->stage_D[i], bytes) == cudaSuccess &&
+                        cudaMalloc(&P->stage_tr[i], sizeof(double) * P->maxb) == cudaSuccess;
+        if (!ok) { cudaGetLastError(); return CHEB_DM_EALLOC; }
+        P->ws_bytes += 2 * bytes;
+    }
+    if (sets >= 2 && !P->pipe_ready) {
+        CUDA_TRY(cudaStreamCreateWithFlags(&P->s_in, cudaStreamNonBlocking));
+        CUDA_TRY(cudaStreamCreateWithFlags(&P->s_out, cudaStreamNonBlocking));
+        for (int i = 0; i < 2; ++i) {
+            CUDA_TRY(cudaEventCreateWithFlags(&P->ev_in[i], cudaEventDisableTiming));
+            CUDA_TRY(cudaEventCreateWithFlags(&P->ev_comp[i], cudaEventDisableTiming));
+            CUDA_TRY(cudaEventCreateWithFlags(&P->ev_out[i], cudaEventDisableTiming));
+        }
+        P->pipe_ready = 1;
+    }
+    return CHEB_DM_OK;
+}
+
+bool batch_args_ok(const cheb_dm_plan_s* P, int nb, const double* const* A, double* const* B, const double* mu) {
+    if (nb < 1 || nb > P->maxb || !A || !B) return false;
+    for (int s = 0; s < nb; ++s) {
+        if (!A[s] || !B[s] || A[s] == B[s]) return false;
+        if (mu && !isfinite(mu[s])) return false;
+        for (int t = 0; t < s; ++t)
+            if (B[t] == B[s]) return false;
+    }
+    return true;
 }
 
 }  // namespace
@@ -576,7 +890,7 @@ const char* cheb_dm_strerror(cheb_dm_status_t s) {
         case CHEB_DM_ECUDA: return "CUDA error or no device";
         case CHEB_DM_ESTATE: return "call order violated";
         case CHEB_DM_EBOUNDS: return "bad spectral bounds";
-        case CHEB_DM_EUNSUPPORTED: return "unsupported dtype";
+        case CHEB_DM_EUNSUPPORTED: return "unsupported dtype or plan option";
         case CHEB_DM_ENOCONV: return "power-basis outer recursion would lose accuracy (use the Chebyshev outer recursion)";
     }
     return "unknown status";
@@ -593,21 +907,25 @@ cheb_dm_status_t cheb_dm_destroy(cheb_dm_plan_t P) {
     cudaFree(P->Amat);
     cudaFree(P->tau);
     cudaFree(P->w);
-    cudaFree(P->dots);
     cudaFree(P->one);
     cudaFree(P->part);
+    cudaFree(P->traces);
+    cudaFree(P->gram_part);
+    cudaFree(P->gram);
     cudaFree(P->sym_first);
     cudaFree(P->sc);
     cudaFree(P->maps);
-    cudaFree(P->tasks);
-    cudaFree(P->task_first);
+    cudaFree(P->baby.d);
+    cudaFree(P->giant.d);
+    cudaFree(P->chain.d);
+    cudaFree(P->flat.d);
+    cudaFree(P->misc.d);
     cudaFree(P->counters);
-    cudaFree(P->stage_H);
-    cudaFree(P->stage_D);
-    cudaFree(P->stage_tr);
-    cudaFree(P->stage_H1);
-    cudaFree(P->stage_D1);
-    cudaFree(P->stage_tr1);
+    for (int i = 0; i < 2; ++i) {
+        cudaFree(P->stage_H[i]);
+        cudaFree(P->stage_D[i]);
+        cudaFree(P->stage_tr[i]);
+    }
     if (P->pipe_ready) {
         cudaStreamDestroy(P->s_in);
         cudaStreamDestroy(P->s_out);
@@ -636,10 +954,13 @@ cheb_dm_status_t cheb_dm_plan_ex(cheb_dm_plan_t* plan, int N, int M_terms, cheb_
     if (o.k < 0 || o.p < 0) return CHEB_DM_EINVAL;
     if (o.outer != CHEB_DM_OUTER_CHEBYSHEV && o.outer != CHEB_DM_OUTER_POWER) return CHEB_DM_EINVAL;
     if (o.sched != CHEB_DM_SCHED_GROUPED && o.sched != CHEB_DM_SCHED_SERIAL) return CHEB_DM_EINVAL;
-    if (o.pairing != CHEB_DM_PAIR_ALG1 && o.pairing != CHEB_DM_PAIR_SERIAL && o.pairing != CHEB_DM_PAIR_BALANCED) return CHEB_DM_EINVAL;
+    if (o.pairing < CHEB_DM_PAIR_AUTO || o.pairing > CHEB_DM_PAIR_ALG1) return CHEB_DM_EINVAL;
     if (o.fuse_sums < 0 || o.fuse_sums > 2) return CHEB_DM_EINVAL;
     if (o.giant < 0 || o.giant > 2) return CHEB_DM_EINVAL;
     if (o.symmetric < 0 || o.symmetric > 2) return CHEB_DM_EINVAL;
+    if (o.max_batch < 0 || o.max_batch > MAX_BATCH) return CHEB_DM_EINVAL;
+    if ((o.ldh != 0 && o.ldh < N) || (o.ldd != 0 && o.ldd < N)) return CHEB_DM_EINVAL;
+    if (o.moments < 0 || o.moments > 2 || o.host_slots < 0 || o.host_slots > 2) return CHEB_DM_EINVAL;
     int k = o.k, p = o.p;
     if (k == 0 && p == 0) {
         k = 1;
@@ -662,25 +983,35 @@ cheb_dm_status_t cheb_dm_plan_ex(cheb_dm_plan_t* plan, int N, int M_terms, cheb_
     cheb_dm_plan_s* P = new (std::nothrow) cheb_dm_plan_s();
     if (!P) return CHEB_DM_EALLOC;
     P->N = N; P->M = M_terms; P->k = k; P->p = p;
-    P->opt = o; P->opt.k = k; P->opt.p = p;
+    P->maxb = o.max_batch < 1 ? 1 : o.max_batch;
+    P->opt = o; P->opt.k = k; P->opt.p = p; P->opt.max_batch = P->maxb;
+    P->ldh = o.ldh ? o.ldh : N;
+    P->ldd = o.ldd ? o.ldd : N;
+    P->opt.ldh = (int)P->ldh; P->opt.ldd = (int)P->ldd;
+    if (P->opt.pairing == CHEB_DM_PAIR_AUTO) P->opt.pairing = CHEB_DM_PAIR_BALANCED;
     P->device = dev; P->num_sms = prop.multiProcessorCount;
     int nq = 1;
     while (nq < 4 * M_terms) nq <<= 1;  // N_q = 2^ceil(log2(4M)) (cheb_dm.h)
     P->Nq = nq;
     P->sym = (o.symmetric != 1) ? 1 : 0;
     P->opt.symmetric = P->sym ? 2 : 1;
-    P->sym_first = nullptr;
+    {
+        const char* env = getenv("CHEB_DM_SCALAR_SUMS");  // read here, never in a compute call
+        P->scalar_sums = (env && env[0] == '1') ? 1 : 0;
+    }
     choose_tile(P);
     P->ld = ((long long)N + 15) / 16 * 16;
     P->mat_elems = (((size_t)N * (size_t)P->ld) + 127) / 128 * 128;
-    // Giant steps in the resident-multiplier kernel: N <= 512 (32 rows of T_k fit in shared memory), operand maps
-    // with BK = 32 and 2-slab boxes (the 64x32 / 32x32 tile shapes), grouped scheduling, at least one product.
+    // Giant steps of single solves in the resident-multiplier kernel: N <= 512 (32 rows of T_k fit in shared memory),
+    // operand maps with BK = 32 and 2-slab boxes (the 64x32 / 32x32 tile shapes), grouped scheduling, at least one
+    // product, and k small enough for its coefficient staging area (k * GR_SUM_CHUNK doubles inside the idle TMA rings).
     P->resident = 0;
     P->res_tiles_m = P->res_tiles_n = ceil_div(N, 32);
     P->res_grid = P->sym ? (P->res_tiles_m * (P->res_tiles_m + 1)) / 2 : P->res_tiles_m * ceil_div(P->res_tiles_n, 2);
     P->res_smem = giant_resident_smem_bytes(ceil_div(N, GR_BK));
     if (o.giant != 1 && N <= 32 * GR_MAX_KTILES && p >= 2 && P->BK == GR_BK && P->box_slabs == 2 &&
-        o.sched == CHEB_DM_SCHED_GROUPED && P->res_grid <= P->num_sms) {
+        o.sched == CHEB_DM_SCHED_GROUPED && P->res_grid <= P->num_sms &&
+        (long long)k * GR_SUM_CHUNK * 8 <= 2ll * GR_STAGES * GR_TILE_BYTES) {
         if (cudaFuncSetAttribute(giant_resident_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, P->res_smem) == cudaSuccess) {
             int per_sm = 0;
             if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, giant_resident_kernel, GR_THREADS, P->res_smem) == cudaSuccess && per_sm >= 1)
@@ -689,60 +1020,80 @@ cheb_dm_status_t cheb_dm_plan_ex(cheb_dm_plan_t* plan, int N, int M_terms, cheb_
         cudaGetLastError();
     }
     P->opt.giant = P->resident ? 2 : 1;
-    // a-5: fused (epilogue reads T_1..T_{k-1}: p (k-1) mat bytes per solve) while the baby block stays L2-resident,
-    // pre-formed (form_sums_kernel: (ceil(p/16) (k-1) + p) mat bytes) once it does not.
+    P->moments_on = (o.moments != 1) ? 1 : 0;
+    P->opt.moments = P->moments_on ? 2 : 1;
+    // a-5: fused (epilogue reads T_1..T_{k-1}: p (k-1) mat bytes per solve) while the baby blocks of the batch stay
+    // L2-resident, pre-formed (form_sums_kernel: (ceil(p/16) (k-1) + p) mat bytes) once they do not.
     {
         int mode = o.fuse_sums;
-        if (mode == 0) mode = ((double)k * (double)P->mat_elems * 8.0 > 96.0 * 1024 * 1024 && k > 2 && p > 1) ? 2 : 1;
+        if (mode == 0) mode = ((double)k * (double)P->mat_elems * 8.0 * P->maxb > 96.0 * 1024 * 1024 && k > 2 && p > 1) ? 2 : 1;
         P->preformed = (mode == 2) ? 1 : 0;
         P->opt.fuse_sums = mode;
     }
-    if (P->resident) {  // the resident kernel forms the sums itself (each CTA its own tiles) and parks them in G_l
+    if (P->resident && P->maxb == 1) {  // the resident kernel forms the sums itself (each CTA its own tiles) and parks them in G_l
         P->preformed = 1;
         P->opt.fuse_sums = 2;
     }
-    P->nmat = k + 2 + (P->preformed ? p : 0);
-    P->ws = nullptr; P->costab = P->fn = P->c = P->gT = P->dT = P->Amat = P->tau = P->w = P->dots = P->one = P->part = nullptr;
-    P->sc = nullptr; P->maps = nullptr; P->tasks = nullptr; P->task_first = nullptr; P->counters = nullptr;
-    P->have_coeffs = P->explicit_bounds = P->have_moments = P->computed = 0;
+    const bool need_G = P->preformed || P->resident || P->moments_on;
+    P->off_G = need_G ? k + 2 : -1;
+    P->off_U = (P->moments_on && p >= 3) ? k + 2 + (need_G ? p : 0) : -1;
+    P->nmat = k + 2 + (need_G ? p : 0) + ((P->moments_on && p >= 3) ? p - 2 : 0);
+    P->slot_elems = (size_t)P->nmat * P->mat_elems;
+    P->map_flatA = k + 2;
+    P->map_flatB = k + 2 + (p - 1);
+    P->nmaps_slot = k + 2 + (P->moments_on ? 2 * (p - 1) : 0);
+    P->ntrmat = k + ((P->moments_on && p >= 3) ? p - 2 : 0);
+    {
+        const long long nchunks = (long long)N * P->ld / 8;
+        long long ctas = nchunks / 64;
+        if (ctas > 2ll * P->num_sms) ctas = 2ll * P->num_sms;
+        if (ctas < 1) ctas = 1;
+        P->gram_ctas = (int)ctas;
+        P->gram_passes = ceil_div(p > 1 ? p - 1 : 1, GRAM_BLK) * ceil_div(k > 1 ? k - 1 : 1, GRAM_BLK);
+    }
+    P->ws = nullptr; P->costab = P->fn = P->c = P->gT = P->dT = P->Amat = P->tau = P->w = P->one = P->part = nullptr;
+    P->traces = P->gram_part = P->gram = nullptr;
+    P->sym_first = nullptr; P->sc = nullptr; P->maps = nullptr; P->counters = nullptr;
+    P->have_coeffs = P->explicit_bounds = P->have_moments = P->computed = P->blocks_nb = 0;
+    P->beta = P->mu = P->a = P->b = 0.0;
     P->last_launches = 0;
-    P->stage_H = P->stage_D = P->stage_tr = nullptr;
-    P->stage_H1 = P->stage_D1 = P->stage_tr1 = nullptr;
+    P->work_next = 0;
+    for (int i = 0; i < 2; ++i) P->stage_H[i] = P->stage_D[i] = P->stage_tr[i] = nullptr;
     P->pipe_ready = 0;
     P->n_async = 0;
     P->timing = 0; P->ev_count = 0;
     P->trace_buf = nullptr; P->trace_on = 0;
     for (int i = 0; i < TIMING_SLOTS; ++i) P->ev0[i] = P->ev1[i] = nullptr;
 
-    const int tiles = ceil_div(N, P->BM) * ceil_div(N, P->BN);
-    const size_t kp = (size_t)k * p;
-    P->ws_bytes = sizeof(double) * P->mat_elems * P->nmat;
+    const size_t kp = (size_t)k * p, B = (size_t)P->maxb;
+    P->ws_bytes = sizeof(double) * P->slot_elems * B;
     bool ok = true;
     ok = ok && cudaMalloc(&P->ws, P->ws_bytes) == cudaSuccess;
     ok = ok && cudaMalloc(&P->costab, sizeof(double) * 4 * nq) == cudaSuccess;
-    ok = ok && cudaMalloc(&P->fn, sizeof(double) * nq) == cudaSuccess;
-    ok = ok && cudaMalloc(&P->c, sizeof(double) * kp) == cudaSuccess;
-    ok = ok && cudaMalloc(&P->gT, sizeof(double) * kp) == cudaSuccess;
-    ok = ok && cudaMalloc(&P->dT, sizeof(double) * kp) == cudaSuccess;
+    ok = ok && cudaMalloc(&P->fn, sizeof(double) * nq * B) == cudaSuccess;
+    ok = ok && cudaMalloc(&P->c, sizeof(double) * kp * B) == cudaSuccess;
+    ok = ok && cudaMalloc(&P->gT, sizeof(double) * kp * B) == cudaSuccess;
+    ok = ok && cudaMalloc(&P->dT, sizeof(double) * kp * B) == cudaSuccess;
     ok = ok && cudaMalloc(&P->Amat, sizeof(double) * p * p) == cudaSuccess;
-    ok = ok && cudaMalloc(&P->tau, sizeof(double) * kp) == cudaSuccess;
-    ok = ok && cudaMalloc(&P->w, sizeof(double) * nq) == cudaSuccess;
-    ok = ok && cudaMalloc(&P->dots, sizeof(double) * ((size_t)(p + 1) * tiles * k + (size_t)2 * k * 16)) == cudaSuccess;
-    ok = ok && cudaMalloc(&P->sc, sizeof(DevScalars)) == cudaSuccess;
+    ok = ok && cudaMalloc(&P->tau, sizeof(double) * kp * B) == cudaSuccess;
+    ok = ok && cudaMalloc(&P->w, sizeof(double) * nq * B) == cudaSuccess;
+    ok = ok && cudaMalloc(&P->sc, sizeof(DevScalars) * B) == cudaSuccess;
     ok = ok && cudaMalloc(&P->one, sizeof(double)) == cudaSuccess;
+    const size_t gram_part_elems = B * P->gram_passes * P->gram_ctas * (size_t)(GRAM_BLK * GRAM_BLK);
+    if (P->moments_on) {
+        ok = ok && cudaMalloc(&P->traces, sizeof(double) * B * P->ntrmat) == cudaSuccess;
+        ok = ok && cudaMalloc(&P->gram_part, sizeof(double) * gram_part_elems) == cudaSuccess;
+        ok = ok && cudaMalloc(&P->gram, sizeof(double) * B * (kp + 1)) == cudaSuccess;
+    }
     {
         int per_sm = 0;
         ok = ok && cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, front_end_kernel, 512, 0) == cudaSuccess && per_sm >= 1;
-        int want = ceil_div(N, 16);
-        if (ceil_div((int)kp, 16) > want) want = ceil_div((int)kp, 16);
-        if (ceil_div(nq, 512) > want) want = ceil_div(nq, 512);
-        P->front_grid = want < P->num_sms ? want : P->num_sms;
-        ok = ok && cudaMalloc(&P->part, sizeof(double) * 2 * P->num_sms) == cudaSuccess;
+        P->front_max_grid = per_sm * P->num_sms;
+        if (P->front_max_grid > 4 * P->num_sms) P->front_max_grid = 4 * P->num_sms;
+        ok = ok && P->front_max_grid >= P->maxb;
+        ok = ok && cudaMalloc(&P->part, sizeof(double) * 2 * (P->front_max_grid > 0 ? P->front_max_grid : 1)) == cudaSuccess;
     }
-    ok = ok && cudaMalloc(&P->maps, sizeof(CUtensorMap) * P->nmat) == cudaSuccess;
-    ok = ok && cudaMalloc(&P->stage_H, sizeof(double) * (size_t)N * N) == cudaSuccess;
-    ok = ok && cudaMalloc(&P->stage_D, sizeof(double) * (size_t)N * N) == cudaSuccess;
-    ok = ok && cudaMalloc(&P->stage_tr, sizeof(double)) == cudaSuccess;
+    ok = ok && cudaMalloc(&P->maps, sizeof(CUtensorMap) * P->nmaps_slot * B) == cudaSuccess;
     for (int i = 0; i < TIMING_SLOTS && ok; ++i)
         ok = cudaEventCreate(&P->ev0[i]) == cudaSuccess && cudaEventCreate(&P->ev1[i]) == cudaSuccess;
     if (!ok) {
@@ -750,16 +1101,17 @@ cheb_dm_status_t cheb_dm_plan_ex(cheb_dm_plan_t* plan, int N, int M_terms, cheb_
         cheb_dm_destroy(P);
         return CHEB_DM_EALLOC;
     }
-    P->ws_bytes += sizeof(double) * (2 * (size_t)N * N + 4 * (size_t)nq + 2 * nq + 4 * kp + (size_t)p * p + (size_t)(p + 1) * tiles * k);
+    P->ws_bytes += sizeof(double) * (4 * (size_t)nq + B * (2 * nq + 4 * kp) + (size_t)p * p + (P->moments_on ? gram_part_elems : 0));
 
     cheb_dm_status_t st = CHEB_DM_OK;
     do {
-        if (cudaMemset(P->ws, 0, sizeof(double) * P->mat_elems * P->nmat) != cudaSuccess) { st = CHEB_DM_ECUDA; break; }
-        cudaMemset(P->dots, 0, sizeof(double) * ((size_t)(p + 1) * tiles * k + (size_t)2 * k * 16));
-        cudaMemset(P->dT, 0, sizeof(double) * kp);
-        cudaMemset(P->gT, 0, sizeof(double) * kp);
-        cudaMemset(P->c, 0, sizeof(double) * kp);
-        cudaMemset(P->sc, 0, sizeof(DevScalars));
+        if (prepare_gemm(P) != CHEB_DM_OK) { cudaGetLastError(); st = CHEB_DM_ECUDA; break; }
+        if (cudaMemset(P->ws, 0, sizeof(double) * P->slot_elems * B) != cudaSuccess) { st = CHEB_DM_ECUDA; break; }
+        cudaMemset(P->dT, 0, sizeof(double) * kp * B);
+        cudaMemset(P->gT, 0, sizeof(double) * kp * B);
+        cudaMemset(P->c, 0, sizeof(double) * kp * B);
+        cudaMemset(P->tau, 0, sizeof(double) * kp * B);
+        cudaMemset(P->sc, 0, sizeof(DevScalars) * B);
         {
             const double one = 1.0;
             cudaMemcpy(P->one, &one, sizeof(double), cudaMemcpyHostToDevice);
@@ -784,28 +1136,38 @@ cheb_dm_status_t cheb_dm_plan_ex(cheb_dm_plan_t* plan, int N, int M_terms, cheb_
         }
         st = encode_maps(P);
         if (st != CHEB_DM_OK) break;
-        build_tasks(P);
-        const int nt = (int)P->h_tasks.size();
+        build_tables(P);
         P->panel_stride = ceil_div(N, 16);  // >= the number of column panels of every kernel (narrowest panel: 16)
-        P->nwork = nt + 4;
-        P->off_work = 0;
-        P->off_task = P->off_work + P->nwork;
-        P->off_group = P->off_task + nt;
-        P->off_error = P->off_group + NGROUPS;
-        P->off_panel = P->off_error + 1;
-        P->counters_ints = (size_t)P->off_panel + (size_t)nt * P->panel_stride;
-        if (cudaMalloc(&P->tasks, sizeof(Task) * nt) != cudaSuccess ||
-            cudaMalloc(&P->task_first, sizeof(int) * (nt + 1)) != cudaSuccess ||
-            cudaMalloc(&P->counters, sizeof(int) * P->counters_ints) != cudaSuccess) {
-            cudaGetLastError();
-            st = CHEB_DM_EALLOC;
-            break;
+        TaskTable* tabs[5] = {&P->baby, &P->giant, &P->chain, &P->flat, &P->misc};
+        size_t off = 1;  // [0] = sticky error flag
+        int total_tasks = 0, trace_off = 0;
+        for (int t = 0; t < 5; ++t) total_tasks += (int)tabs[t]->h.size();
+        P->nwork = total_tasks + 8;
+        off += P->nwork;
+        for (int t = 0; t < 5; ++t) {
+            TaskTable* tt = tabs[t];
+            tt->ctr_task_off = (int)off;
+            off += tt->h.size();
+            tt->ctr_panel_off = (int)off;
+            off += tt->h.size() * (size_t)P->panel_stride;
+            tt->trace_base = trace_off;
+            trace_off += tt->ntl * tt->items_per_task;  // timeline of single solves (slot 0)
         }
-        if (cudaMemcpy(P->tasks, P->h_tasks.data(), sizeof(Task) * nt, cudaMemcpyHostToDevice) != cudaSuccess ||
-            cudaMemcpy(P->task_first, P->h_first.data(), sizeof(int) * (nt + 1), cudaMemcpyHostToDevice) != cudaSuccess ||
-            cudaMemset(P->counters, 0, sizeof(int) * P->counters_ints) != cudaSuccess) {
-            st = CHEB_DM_ECUDA;
-            break;
+        P->trace_res_base = trace_off;
+        P->trace_total = trace_off + P->p * P->res_tiles_m * P->res_tiles_n;
+        P->counters_ints = off;
+        if (cudaMalloc(&P->counters, sizeof(int) * P->counters_ints) != cudaSuccess) { cudaGetLastError(); st = CHEB_DM_EALLOC; break; }
+        if (cudaMemset(P->counters, 0, sizeof(int) * P->counters_ints) != cudaSuccess) { st = CHEB_DM_ECUDA; break; }
+        for (int t = 0; t < 5 && st == CHEB_DM_OK; ++t) {
+            TaskTable* tt = tabs[t];
+            if (tt->h.empty()) continue;
+            if (cudaMalloc(&tt->d, sizeof(Task) * tt->h.size()) != cudaSuccess) { cudaGetLastError(); st = CHEB_DM_EALLOC; break; }
+            if (cudaMemcpy(tt->d, tt->h.data(), sizeof(Task) * tt->h.size(), cudaMemcpyHostToDevice) != cudaSuccess) st = CHEB_DM_ECUDA;
+        }
+        if (st != CHEB_DM_OK) break;
+        if (o.host_slots > 0) {
+            st = ensure_staging(P, o.host_slots);
+            if (st != CHEB_DM_OK) break;
         }
         if (cudaDeviceSynchronize() != cudaSuccess) { st = CHEB_DM_ECUDA; break; }
     } while (0);
@@ -870,207 +1232,105 @@ cheb_dm_status_t cheb_dm_flops_per_compute(cheb_dm_plan_t P, double* flops_out) 
     return CHEB_DM_OK;
 }
 
-}  // extern "C"
-
-namespace {
-
-// Steps a-1 .. a-3 on the stream, one cooperative launch: counters reset, bounds (+ rescale of H into T_1), c_n,
-// g (and d).
-cheb_dm_status_t front_end(cheb_dm_plan_s* P, const double* dH, cudaStream_t st) {
-    FrontArgs fa;
-    fa.H = dH;
-    fa.N = P->N;
-    fa.X = T_ptr(P, 1);
-    fa.ldx = P->ld;
-    fa.sc = P->sc;
-    fa.explicit_bounds = P->explicit_bounds;
-    fa.a = P->a;
-    fa.b = P->b;
-    fa.part = P->part;
-    fa.counters = P->counters;
-    fa.ncounters = (int)P->counters_ints;
-    fa.beta = P->beta;
-    fa.mu = P->mu;
-    fa.costab = P->costab;
-    fa.Nq = P->Nq;
-    fa.M = P->M;
-    fa.fn = P->fn;
-    fa.c = P->c;
-    fa.k = P->k;
-    fa.p = P->p;
-    fa.Amat = P->Amat;
-    fa.want_d = (P->opt.outer == CHEB_DM_OUTER_POWER) ? 1 : 0;
-    fa.gT = P->gT;
-    fa.dT = P->dT;
-    void* args[] = {(void*)&fa};
-    CUDA_TRY(cudaLaunchCooperativeKernel((const void*)front_end_kernel, dim3(P->front_grid), dim3(512), args, 0, st));
-    ++P->last_launches;
+cheb_dm_status_t cheb_dm_flops_per_solve(cheb_dm_plan_t P, double* flops_out) {
+    if (!P || !flops_out) return CHEB_DM_EINVAL;
+    if (!P->moments_on) return CHEB_DM_EUNSUPPORTED;
+    *flops_out = P->flops_per_solve;
     return CHEB_DM_OK;
 }
 
-cheb_dm_status_t run_tasks(cheb_dm_plan_s* P, int t0, int t1, double* userD, long long ldD, cudaStream_t st) {
-    if (t1 <= t0) return CHEB_DM_OK;
-    if (P->opt.sched == CHEB_DM_SCHED_GROUPED) return launch_tasks(P, t0, t1, 1, t0, userD, ldD, st);
-    for (int t = t0; t < t1; ++t) {
-        cheb_dm_status_t s = launch_tasks(P, t, t + 1, 0, t, userD, ldD, st);
-        if (s != CHEB_DM_OK) return s;
-    }
-    return CHEB_DM_OK;
+// ------------------------------------------------------------------------------------------------------
+// fixed-mu solves
+// ------------------------------------------------------------------------------------------------------
+cheb_dm_status_t cheb_dm_compute_batch(cheb_dm_plan_t P, int nbatch, const double* const* dH, double* const* dD, const double* mu,
+                                       void* cuda_stream) {
+    if (!P || !batch_args_ok(P, nbatch, dH, dD, mu)) return CHEB_DM_EINVAL;
+    if (!P->have_coeffs) return CHEB_DM_ESTATE;
+    if (!device_ok(P)) return CHEB_DM_ECUDA;
+    return compute_impl(P, nbatch, dH, P->ldh, dD, P->ldd, mu, (cudaStream_t)cuda_stream);
 }
-
-// Giant steps of the solve (tasks [nbaby, ntasks_solve)) in the resident-multiplier kernel; cooperative launch
-// because its CTAs wait on one another's panel counters.
-cheb_dm_status_t run_giant_resident(cheb_dm_plan_s* P, double* userD, long long ldD, cudaStream_t st) {
-    GiantArgs ga;
-    ga.tasks = P->tasks;
-    ga.maps = P->maps;
-    ga.first_task = P->nbaby;
-    ga.nsteps = P->ntasks_solve - P->nbaby;
-    ga.N = P->N;
-    ga.ktiles = ceil_div(P->N, GR_BK);
-    ga.tiles_m = P->res_tiles_m;
-    ga.tiles_n = P->res_tiles_n;
-    ga.panel_done = P->counters + P->off_panel;
-    ga.panel_stride = P->panel_stride;
-    ga.userD = userD;
-    ga.ldD = ldD;
-    ga.tma2d = P->tma2d;
-    ga.error_flag = P->counters + P->off_error;
-    ga.trace = P->trace_on ? P->trace_buf : nullptr;
-    ga.trace_base = P->h_first.back();
-    ga.coefT = (P->opt.outer == CHEB_DM_OUTER_POWER) ? P->dT : P->gT;
-    ga.Tbase = T_ptr(P, 1);
-    ga.Gbase = G_ptr(P, 0);
-    ga.mat_stride = (long long)P->mat_elems;
-    ga.ld = P->ld;
-    ga.k = P->k;
-    ga.sym = P->sym;
-    void* args[] = {(void*)&ga};
-    CUDA_TRY(cudaLaunchCooperativeKernel((const void*)giant_resident_kernel, dim3(P->res_grid), dim3(GR_THREADS), args,
-                                         (size_t)P->res_smem, st));
-    ++P->last_launches;
-    return CHEB_DM_OK;
-}
-
-bool device_ok(const cheb_dm_plan_s* P) {
-    int dev = -1;
-    return cudaGetDevice(&dev) == cudaSuccess && dev == P->device;
-}
-
-}  // namespace
-
-extern "C" {
 
 cheb_dm_status_t cheb_dm_compute(cheb_dm_plan_t P, const double* dH, double* dD, void* cuda_stream) {
     if (!P || !dH || !dD || dH == dD) return CHEB_DM_EINVAL;
+    return cheb_dm_compute_batch(P, 1, &dH, &dD, nullptr, cuda_stream);
+}
+
+cheb_dm_status_t cheb_dm_compute_batch_host_async(cheb_dm_plan_t P, int nbatch, const double* const* hH, double* const* hD,
+                                                  double* h_trace, const double* mu, void* cuda_stream) {
+    if (!P || !batch_args_ok(P, nbatch, hH, hD, mu)) return CHEB_DM_EINVAL;
     if (!P->have_coeffs) return CHEB_DM_ESTATE;
     if (!device_ok(P)) return CHEB_DM_ECUDA;
+    cheb_dm_status_t s = ensure_staging(P, 2);
+    if (s != CHEB_DM_OK) return s;
     cudaStream_t st = (cudaStream_t)cuda_stream;
-    P->last_launches = 0;
-    cheb_dm_status_t s = front_end(P, dH, st);  // also zeroes the scheduler counters
+    const size_t elems = (size_t)P->N * P->N, bytes = sizeof(double) * elems;
+    const int set = (int)(P->n_async & 1);
+    const double* sH[MAX_BATCH];
+    double* sD[MAX_BATCH];
+    for (int i = 0; i < nbatch; ++i) {
+        sH[i] = P->stage_H[set] + (size_t)i * elems;
+        sD[i] = P->stage_D[set] + (size_t)i * elems;
+    }
+    // H2D of this call: the set's previous occupant (call n-2) must have been consumed by its kernels
+    if (P->n_async >= 2) CUDA_TRY(cudaStreamWaitEvent(P->s_in, P->ev_comp[set], 0));
+    for (int i = 0; i < nbatch; ++i) CUDA_TRY(cudaMemcpyAsync((void*)sH[i], hH[i], bytes, cudaMemcpyHostToDevice, P->s_in));
+    CUDA_TRY(cudaEventRecord(P->ev_in[set], P->s_in));
+    // kernels, in call order on the caller's stream: need this call's H and the set's D / tr copied out (call n-2)
+    CUDA_TRY(cudaStreamWaitEvent(st, P->ev_in[set], 0));
+    if (P->n_async >= 2) CUDA_TRY(cudaStreamWaitEvent(st, P->ev_out[set], 0));
+    s = compute_impl(P, nbatch, sH, P->N, sD, P->N, mu, st);
     if (s != CHEB_DM_OK) return s;
-    const int slot = (int)(P->ev_count % TIMING_SLOTS);
-    if (P->timing) CUDA_TRY(cudaEventRecord(P->ev0[slot], st));
-    if (P->resident) {
-        s = run_tasks(P, 0, P->nbaby, dD, P->N, st);
+    if (h_trace) {
+        s = trace_impl(P, nbatch, sD, P->N, P->stage_tr[set], st);
         if (s != CHEB_DM_OK) return s;
-        s = run_giant_resident(P, dD, P->N, st);
-    } else if (P->preformed) {
-        s = run_tasks(P, 0, P->nbaby, dD, P->N, st);
-        if (s != CHEB_DM_OK) return s;
-        const double* coefT = (P->opt.outer == CHEB_DM_OUTER_POWER) ? P->dT : P->gT;
-        const char* scalar_sums = getenv("CHEB_DM_SCALAR_SUMS");
-        if (scalar_sums && scalar_sums[0] == '1') {  // FP64-FMA version (ablation)
-            const long long pairs = (long long)P->N * P->ld / 2;
-            dim3 grid((unsigned)((pairs + 255) / 256), (unsigned)ceil_div(P->p, SUMS_CHUNK));
-            form_sums_kernel<<<grid, 256, sizeof(double) * P->k * SUMS_CHUNK, st>>>(T_ptr(P, 1), (long long)P->mat_elems, P->ld, P->N, P->k,
-                                                                                  P->p, coefT, G_ptr(P, 0), P->sym ? P->BM : 0, P->BN);
-        } else {
-            const long long warps = ((long long)P->N * P->ld + 31) / 32;
-            dim3 grid((unsigned)((warps + 7) / 8), (unsigned)ceil_div(P->p, SUMS_CHUNK));
-            const size_t smem = sizeof(double) * (size_t)((((P->k - 1) + 3) & ~3) + 1) * SUMS_CHUNK;
-            form_sums_dmma_kernel<<<grid, 256, smem, st>>>(T_ptr(P, 1), (long long)P->mat_elems, P->ld, P->N, P->k, P->p, coefT,
-                                                           G_ptr(P, 0), P->sym ? P->BM : 0, P->BN);
-        }
         ++P->last_launches;
-        CUDA_TRY(cudaGetLastError());
-        s = run_tasks(P, P->nbaby, P->ntasks_solve, dD, P->N, st);
-    } else {
-        s = run_tasks(P, 0, P->ntasks_solve, dD, P->N, st);
     }
-    if (s != CHEB_DM_OK) return s;
-    if (P->timing) {
-        CUDA_TRY(cudaEventRecord(P->ev1[slot], st));
-        ++P->ev_count;
-    }
-    P->computed = 1;
+    CUDA_TRY(cudaEventRecord(P->ev_comp[set], st));
+    // D2H of this call
+    CUDA_TRY(cudaStreamWaitEvent(P->s_out, P->ev_comp[set], 0));
+    if (h_trace) CUDA_TRY(cudaMemcpyAsync(h_trace, P->stage_tr[set], sizeof(double) * nbatch, cudaMemcpyDeviceToHost, P->s_out));
+    for (int i = 0; i < nbatch; ++i) CUDA_TRY(cudaMemcpyAsync(hD[i], sD[i], bytes, cudaMemcpyDeviceToHost, P->s_out));
+    CUDA_TRY(cudaEventRecord(P->ev_out[set], P->s_out));
+    ++P->n_async;
     return CHEB_DM_OK;
+}
+
+cheb_dm_status_t cheb_dm_compute_batch_host(cheb_dm_plan_t P, int nbatch, const double* const* hH, double* const* hD, double* h_trace,
+                                            const double* mu, void* cuda_stream) {
+    if (!P || !batch_args_ok(P, nbatch, hH, hD, mu)) return CHEB_DM_EINVAL;
+    if (!P->have_coeffs) return CHEB_DM_ESTATE;
+    if (!device_ok(P)) return CHEB_DM_ECUDA;
+    cheb_dm_status_t s = ensure_staging(P, 1);
+    if (s != CHEB_DM_OK) return s;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const size_t elems = (size_t)P->N * P->N, bytes = sizeof(double) * elems;
+    const double* sH[MAX_BATCH];
+    double* sD[MAX_BATCH];
+    for (int i = 0; i < nbatch; ++i) {
+        sH[i] = P->stage_H[0] + (size_t)i * elems;
+        sD[i] = P->stage_D[0] + (size_t)i * elems;
+        CUDA_TRY(cudaMemcpyAsync((void*)sH[i], hH[i], bytes, cudaMemcpyHostToDevice, st));
+    }
+    s = compute_impl(P, nbatch, sH, P->N, sD, P->N, mu, st);
+    if (s != CHEB_DM_OK) return s;
+    if (h_trace) {
+        s = trace_impl(P, nbatch, sD, P->N, P->stage_tr[0], st);
+        if (s != CHEB_DM_OK) return s;
+        ++P->last_launches;
+        CUDA_TRY(cudaMemcpyAsync(h_trace, P->stage_tr[0], sizeof(double) * nbatch, cudaMemcpyDeviceToHost, st));
+    }
+    for (int i = 0; i < nbatch; ++i) CUDA_TRY(cudaMemcpyAsync(hD[i], sD[i], bytes, cudaMemcpyDeviceToHost, st));
+    return cheb_dm_check(P, cuda_stream);  // synchronises the stream
 }
 
 cheb_dm_status_t cheb_dm_compute_host(cheb_dm_plan_t P, const double* hH, double* hD, double* h_trace, void* cuda_stream) {
     if (!P || !hH || !hD || hH == hD) return CHEB_DM_EINVAL;
-    if (!P->have_coeffs) return CHEB_DM_ESTATE;
-    if (!device_ok(P)) return CHEB_DM_ECUDA;
-    cudaStream_t st = (cudaStream_t)cuda_stream;
-    const size_t bytes = sizeof(double) * (size_t)P->N * P->N;
-    CUDA_TRY(cudaMemcpyAsync(P->stage_H, hH, bytes, cudaMemcpyHostToDevice, st));
-    cheb_dm_status_t s = cheb_dm_compute(P, P->stage_H, P->stage_D, cuda_stream);
-    if (s != CHEB_DM_OK) return s;
-    if (h_trace) {
-        trace_kernel<<<1, 1024, 0, st>>>(P->stage_D, P->N, P->N, P->stage_tr);
-        ++P->last_launches;
-        CUDA_TRY(cudaGetLastError());
-        CUDA_TRY(cudaMemcpyAsync(h_trace, P->stage_tr, sizeof(double), cudaMemcpyDeviceToHost, st));
-    }
-    CUDA_TRY(cudaMemcpyAsync(hD, P->stage_D, bytes, cudaMemcpyDeviceToHost, st));
-    return cheb_dm_check(P, cuda_stream);  // synchronises the stream
+    return cheb_dm_compute_batch_host(P, 1, &hH, &hD, h_trace, nullptr, cuda_stream);
 }
 
 cheb_dm_status_t cheb_dm_compute_host_async(cheb_dm_plan_t P, const double* hH, double* hD, double* h_trace, void* cuda_stream) {
     if (!P || !hH || !hD || hH == hD) return CHEB_DM_EINVAL;
-    if (!P->have_coeffs) return CHEB_DM_ESTATE;
-    if (!device_ok(P)) return CHEB_DM_ECUDA;
-    cudaStream_t st = (cudaStream_t)cuda_stream;
-    const size_t bytes = sizeof(double) * (size_t)P->N * P->N;
-    if (!P->pipe_ready) {
-        bool ok = cudaMalloc(&P->stage_H1, bytes) == cudaSuccess && cudaMalloc(&P->stage_D1, bytes) == cudaSuccess &&
-                  cudaMalloc(&P->stage_tr1, sizeof(double)) == cudaSuccess;
-        if (!ok) { cudaGetLastError(); return CHEB_DM_EALLOC; }
-        CUDA_TRY(cudaStreamCreateWithFlags(&P->s_in, cudaStreamNonBlocking));
-        CUDA_TRY(cudaStreamCreateWithFlags(&P->s_out, cudaStreamNonBlocking));
-        for (int i = 0; i < 2; ++i) {
-            CUDA_TRY(cudaEventCreateWithFlags(&P->ev_in[i], cudaEventDisableTiming));
-            CUDA_TRY(cudaEventCreateWithFlags(&P->ev_comp[i], cudaEventDisableTiming));
-            CUDA_TRY(cudaEventCreateWithFlags(&P->ev_out[i], cudaEventDisableTiming));
-        }
-        P->pipe_ready = 1;
-    }
-    const int slot = (int)(P->n_async & 1);
-    double* sH = slot ? P->stage_H1 : P->stage_H;
-    double* sD = slot ? P->stage_D1 : P->stage_D;
-    double* sT = slot ? P->stage_tr1 : P->stage_tr;
-    // H2D of this call: the slot's previous occupant (call n-2) must have been consumed by its kernels
-    if (P->n_async >= 2) CUDA_TRY(cudaStreamWaitEvent(P->s_in, P->ev_comp[slot], 0));
-    CUDA_TRY(cudaMemcpyAsync(sH, hH, bytes, cudaMemcpyHostToDevice, P->s_in));
-    CUDA_TRY(cudaEventRecord(P->ev_in[slot], P->s_in));
-    // kernels, in call order on the caller's stream: need this call's H and the slot's D / tr copied out (call n-2)
-    CUDA_TRY(cudaStreamWaitEvent(st, P->ev_in[slot], 0));
-    if (P->n_async >= 2) CUDA_TRY(cudaStreamWaitEvent(st, P->ev_out[slot], 0));
-    cheb_dm_status_t s = cheb_dm_compute(P, sH, sD, cuda_stream);
-    if (s != CHEB_DM_OK) return s;
-    if (h_trace) {
-        trace_kernel<<<1, 1024, 0, st>>>(sD, P->N, P->N, sT);
-        ++P->last_launches;
-        CUDA_TRY(cudaGetLastError());
-    }
-    CUDA_TRY(cudaEventRecord(P->ev_comp[slot], st));
-    // D2H of this call
-    CUDA_TRY(cudaStreamWaitEvent(P->s_out, P->ev_comp[slot], 0));
-    if (h_trace) CUDA_TRY(cudaMemcpyAsync(h_trace, sT, sizeof(double), cudaMemcpyDeviceToHost, P->s_out));
-    CUDA_TRY(cudaMemcpyAsync(hD, sD, bytes, cudaMemcpyDeviceToHost, P->s_out));
-    CUDA_TRY(cudaEventRecord(P->ev_out[slot], P->s_out));
-    ++P->n_async;
-    return CHEB_DM_OK;
+    return cheb_dm_compute_batch_host_async(P, 1, &hH, &hD, h_trace, nullptr, cuda_stream);
 }
 
 cheb_dm_status_t cheb_dm_wait(cheb_dm_plan_t P, void* cuda_stream) {
@@ -1087,20 +1347,223 @@ cheb_dm_status_t cheb_dm_check(cheb_dm_plan_t P, void* cuda_stream) {
     if (!P->computed) return CHEB_DM_ESTATE;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     int flag = 0;
-    DevScalars h;
-    CUDA_TRY(cudaMemcpyAsync(&flag, P->counters + P->off_error, sizeof(int), cudaMemcpyDeviceToHost, st));
-    CUDA_TRY(cudaMemcpyAsync(&h, P->sc, sizeof(h), cudaMemcpyDeviceToHost, st));
+    std::vector<DevScalars> h((size_t)P->maxb);
+    CUDA_TRY(cudaMemcpyAsync(&flag, P->counters, sizeof(int), cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(cudaMemcpyAsync(h.data(), P->sc, sizeof(DevScalars) * P->maxb, cudaMemcpyDeviceToHost, st));
     CUDA_TRY(cudaStreamSynchronize(st));
     CUDA_TRY(cudaGetLastError());
+    bool bad = false, noconv = false;
+    for (int s = 0; s < P->maxb; ++s) {
+        bad = bad || h[s].bad_bounds;
+        noconv = noconv || h[s].noconv;
+    }
+    if (flag) CUDA_TRY(cudaMemsetAsync(P->counters, 0, sizeof(int), st));  // the flags are sticky until reported here
+    if (bad || noconv)
+        for (int s = 0; s < P->maxb; ++s)
+            if (h[s].bad_bounds || h[s].noconv) CUDA_TRY(cudaMemsetAsync(&P->sc[s].bad_bounds, 0, 2 * sizeof(int), st));
     if (flag) return CHEB_DM_ECUDA;
-    if (h.bad_bounds) return CHEB_DM_EBOUNDS;
+    if (bad) return CHEB_DM_EBOUNDS;
+    if (noconv) return CHEB_DM_ENOCONV;
     return CHEB_DM_OK;
 }
 
+// ------------------------------------------------------------------------------------------------------
+// moments, mu search, mu-inclusive solve
+// ------------------------------------------------------------------------------------------------------
+cheb_dm_status_t cheb_dm_moments(cheb_dm_plan_t P, const double* dH, double* tau_host, void* cuda_stream) {
+    if (!P || !dH) return CHEB_DM_EINVAL;
+    if (!P->moments_on) return CHEB_DM_EUNSUPPORTED;
+    if (!P->have_coeffs) return CHEB_DM_ESTATE;
+    if (!device_ok(P)) return CHEB_DM_ECUDA;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    P->last_launches = 0;
+    cheb_dm_status_t s = front_end(P, 1, &dH, P->ldh, nullptr, 1, 0, 0, st);  // counters reset, bounds + rescale
+    if (s != CHEB_DM_OK) return s;
+    s = blocks_and_moments(P, 1, st);
+    if (s != CHEB_DM_OK) return s;
+    P->have_moments = 1;
+    P->blocks_nb = 1;
+    P->computed = 1;
+    if (tau_host) {
+        CUDA_TRY(cudaMemcpyAsync(tau_host, P->tau, sizeof(double) * (size_t)P->k * P->p, cudaMemcpyDeviceToHost, st));
+        CUDA_TRY(cudaStreamSynchronize(st));
+    }
+    return CHEB_DM_OK;
+}
+
+cheb_dm_status_t cheb_dm_solve_mu(cheb_dm_plan_t P, double beta, double n_occ, int iters, double* mu_out, void* cuda_stream) {
+    if (!P || !mu_out || iters < 1 || !isfinite(beta) || !(beta > 0.0) || !isfinite(n_occ)) return CHEB_DM_EINVAL;
+    if (!P->have_moments) return CHEB_DM_ESTATE;
+    if (!device_ok(P)) return CHEB_DM_ECUDA;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    cheb_dm_status_t s = bisect(P, 1, beta, &n_occ, iters, st);
+    if (s != CHEB_DM_OK) return s;
+    DevScalars h;
+    CUDA_TRY(cudaMemcpyAsync(&h, P->sc, sizeof(h), cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(cudaStreamSynchronize(st));
+    if (h.bad_bounds) return CHEB_DM_EBOUNDS;
+    *mu_out = h.mu;
+    return CHEB_DM_OK;
+}
+
+cheb_dm_status_t cheb_dm_solve_batch(cheb_dm_plan_t P, int nbatch, const double* const* dH, const double* n_occ, int iters,
+                                     double* const* dD, double* mu_out, void* cuda_stream) {
+    if (!P || !n_occ || iters < 1 || !batch_args_ok(P, nbatch, dH, dD, nullptr)) return CHEB_DM_EINVAL;
+    for (int s = 0; s < nbatch; ++s)
+        if (!isfinite(n_occ[s])) return CHEB_DM_EINVAL;
+    if (!P->moments_on) return CHEB_DM_EUNSUPPORTED;
+    if (!P->have_coeffs) return CHEB_DM_ESTATE;
+    if (!device_ok(P)) return CHEB_DM_ECUDA;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    P->last_launches = 0;
+    cheb_dm_status_t s = front_end(P, nbatch, dH, P->ldh, nullptr, 1, 0, 0, st);
+    if (s != CHEB_DM_OK) return s;
+    const int slot = (int)(P->ev_count % TIMING_SLOTS);
+    if (P->timing) CUDA_TRY(cudaEventRecord(P->ev0[slot], st));
+    s = blocks_and_moments(P, nbatch, st);
+    if (s != CHEB_DM_OK) return s;
+    s = bisect(P, nbatch, P->beta, n_occ, iters, st);
+    if (s != CHEB_DM_OK) return s;
+    s = assemble_impl(P, nbatch, nullptr, 1, dD, P->ldd, st);
+    if (s != CHEB_DM_OK) return s;
+    if (P->timing) {
+        CUDA_TRY(cudaEventRecord(P->ev1[slot], st));
+        ++P->ev_count;
+    }
+    P->computed = 1;
+    P->have_moments = (nbatch == 1);
+    P->blocks_nb = nbatch;
+    if (mu_out) {
+        std::vector<DevScalars> h((size_t)nbatch);
+        CUDA_TRY(cudaMemcpyAsync(h.data(), P->sc, sizeof(DevScalars) * nbatch, cudaMemcpyDeviceToHost, st));
+        CUDA_TRY(cudaStreamSynchronize(st));
+        for (int i = 0; i < nbatch; ++i)
+            if (h[i].bad_bounds) return CHEB_DM_EBOUNDS;
+        for (int i = 0; i < nbatch; ++i) mu_out[i] = h[i].mu;
+    }
+    return CHEB_DM_OK;
+}
+
+cheb_dm_status_t cheb_dm_solve(cheb_dm_plan_t P, const double* dH, double n_occ, int iters, double* dD, double* mu_out,
+                               void* cuda_stream) {
+    if (!P || !dH || !dD || dH == dD) return CHEB_DM_EINVAL;
+    return cheb_dm_solve_batch(P, 1, &dH, &n_occ, iters, &dD, mu_out, cuda_stream);
+}
+
+cheb_dm_status_t cheb_dm_assemble(cheb_dm_plan_t P, int nbatch, const double* mu, double* const* dD, void* cuda_stream) {
+    if (!P || !mu || !dD || nbatch < 1 || nbatch > P->maxb) return CHEB_DM_EINVAL;
+    for (int s = 0; s < nbatch; ++s)
+        if (!dD[s] || !isfinite(mu[s])) return CHEB_DM_EINVAL;
+    if (!P->moments_on) return CHEB_DM_EUNSUPPORTED;
+    if (!P->have_coeffs || P->blocks_nb != nbatch) return CHEB_DM_ESTATE;
+    if (!device_ok(P)) return CHEB_DM_ECUDA;
+    P->last_launches = 0;
+    return assemble_impl(P, nbatch, mu, 0, dD, P->ldd, (cudaStream_t)cuda_stream);
+}
+
+// ------------------------------------------------------------------------------------------------------
+// trace, getters
+// ------------------------------------------------------------------------------------------------------
+cheb_dm_status_t cheb_dm_trace_batch(cheb_dm_plan_t P, int nbatch, const double* const* dD, double* trace_out, void* cuda_stream) {
+    if (!P || !dD || !trace_out || nbatch < 1 || nbatch > MAX_BATCH) return CHEB_DM_EINVAL;
+    for (int s = 0; s < nbatch; ++s)
+        if (!dD[s]) return CHEB_DM_EINVAL;
+    if (!device_ok(P)) return CHEB_DM_ECUDA;
+    return trace_impl(P, nbatch, dD, P->ldd, trace_out, (cudaStream_t)cuda_stream);
+}
+
+cheb_dm_status_t cheb_dm_trace(cheb_dm_plan_t P, const double* dD, double* trace_out, void* cuda_stream) {
+    if (!P || !dD || !trace_out) return CHEB_DM_EINVAL;
+    return cheb_dm_trace_batch(P, 1, &dD, trace_out, cuda_stream);
+}
+
+cheb_dm_status_t cheb_dm_get_scalars(cheb_dm_plan_t P, int slot, double* out4, void* cuda_stream) {
+    if (!P || !out4 || slot < 0 || slot >= P->maxb) return CHEB_DM_EINVAL;
+    if (!P->computed) return CHEB_DM_ESTATE;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    DevScalars h;
+    CUDA_TRY(cudaMemcpyAsync(&h, P->sc + slot, sizeof(h), cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(cudaStreamSynchronize(st));
+    if (h.bad_bounds || !isfinite(h.a) || !isfinite(h.b)) return CHEB_DM_EBOUNDS;
+    out4[0] = h.a;
+    out4[1] = h.b;
+    out4[2] = h.mu;
+    out4[3] = h.ne;
+    return CHEB_DM_OK;
+}
+
+cheb_dm_status_t cheb_dm_get_bounds(cheb_dm_plan_t P, double* bounds_out, void* cuda_stream) {
+    if (!P || !bounds_out) return CHEB_DM_EINVAL;
+    double v[4];
+    cheb_dm_status_t s = cheb_dm_get_scalars(P, 0, v, cuda_stream);
+    if (s != CHEB_DM_OK) return s;
+    bounds_out[0] = v[0];
+    bounds_out[1] = v[1];
+    return CHEB_DM_OK;
+}
+
+cheb_dm_status_t cheb_dm_get_coeffs(cheb_dm_plan_t P, double* c_out, double* g_out, double* d_out, void* cuda_stream) {
+    if (!P) return CHEB_DM_EINVAL;
+    if (!P->computed) return CHEB_DM_ESTATE;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const int k = P->k, p = P->p;
+    const size_t kp = (size_t)k * p;
+    std::vector<double> tmp(kp);
+    if (c_out) CUDA_TRY(cudaMemcpyAsync(c_out, P->c, sizeof(double) * kp, cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(cudaStreamSynchronize(st));
+    for (int which = 0; which < 2; ++which) {
+        double* out = which == 0 ? g_out : d_out;
+        if (!out) continue;
+        CUDA_TRY(cudaMemcpyAsync(tmp.data(), which == 0 ? P->gT : P->dT, sizeof(double) * kp, cudaMemcpyDeviceToHost, st));
+        CUDA_TRY(cudaStreamSynchronize(st));
+        for (int l = 0; l < p; ++l)
+            for (int i = 0; i < k; ++i) out[(size_t)i * p + l] = tmp[(size_t)l * k + i];  // device layout is [l][i]
+    }
+    return CHEB_DM_OK;
+}
+
+cheb_dm_status_t cheb_dm_get_T(cheb_dm_plan_t P, int n, double* dOut, void* cuda_stream) {
+    if (!P || !dOut || n < 1 || n > P->k) return CHEB_DM_EINVAL;
+    if (!P->computed) return CHEB_DM_ESTATE;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    unpad_copy_kernel<<<P->num_sms * 4, 256, 0, st>>>(T_ptr(P, 0, n), P->ld, P->N, dOut, P->N);
+    CUDA_TRY(cudaGetLastError());
+    CUDA_TRY(cudaStreamSynchronize(st));
+    return CHEB_DM_OK;
+}
+
+cheb_dm_status_t cheb_dm_product(cheb_dm_plan_t P, double alpha, const double* dA, const double* dB, double beta,
+                                 const double* dC, double* dOut, void* cuda_stream) {
+    if (!P || !dA || !dB || !dOut) return CHEB_DM_EINVAL;
+    if (dOut == dA || dOut == dB) return CHEB_DM_EINVAL;
+    if (!device_ok(P)) return CHEB_DM_ECUDA;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    // operands go through the TMA-described workspace buffers (this also handles odd N)
+    pad_copy_kernel<<<P->num_sms * 4, 256, 0, st>>>(dA, P->N, P->N, buf_ptr(P, 0, 0), P->ld);
+    pad_copy_kernel<<<P->num_sms * 4, 256, 0, st>>>(dB, P->N, P->N, buf_ptr(P, 0, 1), P->ld);
+    Task t = P->misc.h[0];
+    t.alpha = alpha;
+    t.beta = beta;
+    t.C = dC;
+    t.ldc = P->N;
+    CUDA_TRY(cudaMemcpyAsync(P->misc.d, &t, sizeof(Task), cudaMemcpyHostToDevice, st));
+    const int save = P->last_launches, wsave = P->work_next;
+    P->work_next = P->nwork - 1;  // the last work counter is reserved for this call
+    CUDA_TRY(cudaMemsetAsync(P->counters + 1 + P->work_next, 0, sizeof(int), st));
+    cheb_dm_status_t s = launch_tasks(P, P->misc, 0, 1, 1, 0, &dOut, P->N, st);
+    P->last_launches = save;
+    P->work_next = wsave;
+    // the pageable-source copy above is staged by the runtime before it returns, so `t` may go out of scope
+    return s;
+}
+
+// ------------------------------------------------------------------------------------------------------
+// tracing and measurement support
+// ------------------------------------------------------------------------------------------------------
 cheb_dm_status_t cheb_dm_set_trace(cheb_dm_plan_t P, int enable) {
     if (!P) return CHEB_DM_EINVAL;
     if (enable && !P->trace_buf) {
-        const size_t n = (size_t)P->h_first.back() + (size_t)P->p * P->res_tiles_m * P->res_tiles_n;
+        const size_t n = (size_t)P->trace_total;
         if (cudaMalloc(&P->trace_buf, sizeof(TraceRec) * n) != cudaSuccess) {
             cudaGetLastError();
             P->trace_buf = nullptr;
@@ -1116,14 +1579,21 @@ cheb_dm_status_t cheb_dm_get_trace(cheb_dm_plan_t P, cheb_dm_trace_rec_t* out, i
     if (!P || !out || !count_out || max_records < 0) return CHEB_DM_EINVAL;
     if (!P->trace_buf) return CHEB_DM_ESTATE;
     static_assert(sizeof(cheb_dm_trace_rec_t) == sizeof(TraceRec), "trace record layout");
-    int n = P->h_first[P->resident ? P->nbaby : P->ntasks_solve];  // items of one solve (generic kernel)
-    if (n > max_records) n = max_records;
     CUDA_TRY(cudaDeviceSynchronize());
-    CUDA_TRY(cudaMemcpy(out, P->trace_buf, sizeof(TraceRec) * (size_t)n, cudaMemcpyDeviceToHost));
-    if (P->resident) {  // followed by the tiles of the resident giant-step kernel
-        int m = P->p * P->res_tiles_m * P->res_tiles_n;
+    int n = 0;
+    // single solve (slot 0): baby-step items, then the giant steps (generic kernel items or resident-kernel tiles)
+    const TaskTable* tabs[2] = {&P->baby, P->resident ? nullptr : &P->giant};
+    for (int t = 0; t < 2; ++t) {
+        if (!tabs[t]) continue;
+        int m = tabs[t]->ntl * tabs[t]->items_per_task;
+        if (m > max_records - n) m = max_records - n;
+        if (m > 0) CUDA_TRY(cudaMemcpy(out + n, P->trace_buf + tabs[t]->trace_base, sizeof(TraceRec) * (size_t)m, cudaMemcpyDeviceToHost));
+        n += m > 0 ? m : 0;
+    }
+    if (P->resident) {
+        const int m = P->p * P->res_tiles_m * P->res_tiles_n;
         std::vector<TraceRec> tmp((size_t)m);
-        CUDA_TRY(cudaMemcpy(tmp.data(), P->trace_buf + P->h_first.back(), sizeof(TraceRec) * (size_t)m, cudaMemcpyDeviceToHost));
+        CUDA_TRY(cudaMemcpy(tmp.data(), P->trace_buf + P->trace_res_base, sizeof(TraceRec) * (size_t)m, cudaMemcpyDeviceToHost));
         for (int i = 0; i < m && n < max_records; ++i)
             if (tmp[i].t_done != 0) {  // tiles above the diagonal are not work items in symmetric mode
                 memcpy(out + n, &tmp[i], sizeof(TraceRec));
@@ -1184,142 +1654,6 @@ cheb_dm_status_t cheb_dm_dmma_peak(int iters, double* tflops_out, void* cuda_str
     cudaFree(sink);
     const double flops = (double)blocks * (threads / 32) * (double)iters * DMMA_PEAK_CHAINS * 512.0;
     *tflops_out = flops / ((double)ms * 1e-3) * 1e-12;
-    return CHEB_DM_OK;
-}
-
-cheb_dm_status_t cheb_dm_trace(cheb_dm_plan_t P, const double* dD, double* trace_out, void* cuda_stream) {
-    if (!P || !dD || !trace_out) return CHEB_DM_EINVAL;
-    if (!device_ok(P)) return CHEB_DM_ECUDA;
-    cudaStream_t st = (cudaStream_t)cuda_stream;
-    trace_kernel<<<1, 1024, 0, st>>>(dD, P->N, P->N, trace_out);
-    CUDA_TRY(cudaGetLastError());
-    return CHEB_DM_OK;
-}
-
-cheb_dm_status_t cheb_dm_get_bounds(cheb_dm_plan_t P, double* bounds_out, void* cuda_stream) {
-    if (!P || !bounds_out) return CHEB_DM_EINVAL;
-    if (!P->computed) return CHEB_DM_ESTATE;
-    cudaStream_t st = (cudaStream_t)cuda_stream;
-    DevScalars h;
-    CUDA_TRY(cudaMemcpyAsync(&h, P->sc, sizeof(h), cudaMemcpyDeviceToHost, st));
-    CUDA_TRY(cudaStreamSynchronize(st));
-    if (h.bad_bounds || !isfinite(h.a) || !isfinite(h.b)) return CHEB_DM_EBOUNDS;
-    bounds_out[0] = h.a;
-    bounds_out[1] = h.b;
-    return CHEB_DM_OK;
-}
-
-cheb_dm_status_t cheb_dm_get_coeffs(cheb_dm_plan_t P, double* c_out, double* g_out, double* d_out, void* cuda_stream) {
-    if (!P) return CHEB_DM_EINVAL;
-    if (!P->computed) return CHEB_DM_ESTATE;
-    cudaStream_t st = (cudaStream_t)cuda_stream;
-    const int k = P->k, p = P->p;
-    const size_t kp = (size_t)k * p;
-    std::vector<double> tmp(kp);
-    if (c_out) CUDA_TRY(cudaMemcpyAsync(c_out, P->c, sizeof(double) * kp, cudaMemcpyDeviceToHost, st));
-    CUDA_TRY(cudaStreamSynchronize(st));
-    for (int which = 0; which < 2; ++which) {
-        double* out = which == 0 ? g_out : d_out;
-        if (!out) continue;
-        CUDA_TRY(cudaMemcpyAsync(tmp.data(), which == 0 ? P->gT : P->dT, sizeof(double) * kp, cudaMemcpyDeviceToHost, st));
-        CUDA_TRY(cudaStreamSynchronize(st));
-        for (int l = 0; l < p; ++l)
-            for (int i = 0; i < k; ++i) out[(size_t)i * p + l] = tmp[(size_t)l * k + i];  // device layout is [l][i]
-    }
-    return CHEB_DM_OK;
-}
-
-cheb_dm_status_t cheb_dm_get_T(cheb_dm_plan_t P, int n, double* dOut, void* cuda_stream) {
-    if (!P || !dOut || n < 1 || n > P->k) return CHEB_DM_EINVAL;
-    if (!P->computed) return CHEB_DM_ESTATE;
-    cudaStream_t st = (cudaStream_t)cuda_stream;
-    unpad_copy_kernel<<<P->num_sms * 4, 256, 0, st>>>(T_ptr(P, n), P->ld, P->N, dOut);
-    CUDA_TRY(cudaGetLastError());
-    CUDA_TRY(cudaStreamSynchronize(st));
-    return CHEB_DM_OK;
-}
-
-cheb_dm_status_t cheb_dm_product(cheb_dm_plan_t P, double alpha, const double* dA, const double* dB, double beta,
-                                 const double* dC, double* dOut, void* cuda_stream) {
-    if (!P || !dA || !dB || !dOut) return CHEB_DM_EINVAL;
-    if (dOut == dA || dOut == dB) return CHEB_DM_EINVAL;
-    if (!device_ok(P)) return CHEB_DM_ECUDA;
-    cudaStream_t st = (cudaStream_t)cuda_stream;
-    // operands go through the TMA-described workspace buffers (this also handles odd N)
-    pad_copy_kernel<<<P->num_sms * 4, 256, 0, st>>>(dA, P->N, buf_ptr(P, 0), P->ld);
-    pad_copy_kernel<<<P->num_sms * 4, 256, 0, st>>>(dB, P->N, buf_ptr(P, 1), P->ld);
-    Task t = P->h_tasks[P->product_task];
-    t.alpha = alpha;
-    t.beta = beta;
-    t.C = dC;
-    t.ldc = P->N;
-    CUDA_TRY(cudaMemcpyAsync(P->tasks + P->product_task, &t, sizeof(Task), cudaMemcpyHostToDevice, st));
-    CUDA_TRY(cudaMemsetAsync(P->counters + P->off_work + P->product_task, 0, sizeof(int), st));
-    const int save = P->last_launches;
-    cheb_dm_status_t s = launch_tasks(P, P->product_task, P->product_task + 1, 0, P->product_task, dOut, P->N, st);
-    P->last_launches = save;
-    // the pageable-source copy above is staged by the runtime before it returns, so `t` may go out of scope
-    return s;
-}
-
-}  // extern "C"
-
-extern "C" {
-
-cheb_dm_status_t cheb_dm_moments(cheb_dm_plan_t P, const double* dH, double* tau_host, void* cuda_stream) {
-    if (!P || !dH) return CHEB_DM_EINVAL;
-    if (!P->have_coeffs) return CHEB_DM_ESTATE;
-    if (!device_ok(P)) return CHEB_DM_ECUDA;
-    cudaStream_t st = (cudaStream_t)cuda_stream;
-    const int k = P->k, p = P->p;
-    const int tiles = ceil_div(P->N, P->BM) * ceil_div(P->N, P->BN);
-    P->last_launches = 0;
-    cheb_dm_status_t s = front_end(P, dH, st);  // counters reset, bounds + rescale (its coefficient tables are not used here)
-    if (s != CHEB_DM_OK) return s;
-    s = run_tasks(P, 0, P->nbaby, nullptr, 0, st);
-    if (s != CHEB_DM_OK) return s;
-    // j = 1: U_1 = T_k is a baby-step output, its products with T_1..T_{k-1} and all tr T_n come from one pass
-    const int nchunks = 16;
-    double* part1 = P->dots + (size_t)(p + 1) * tiles * k;  // (k-1) + 1 + k rows of nchunks partials
-    {
-        dim3 grid(2 * k, nchunks);
-        frob_partial_kernel<<<grid, 256, 0, st>>>(T_ptr(P, k), T_ptr(P, 1), (long long)P->mat_elems, P->ld, P->N, k - 1, k, part1);
-        ++P->last_launches;
-    }
-    // the chain tasks reuse group/task counters; the baby group counter is already complete
-    if (P->ntasks_all > P->ntasks_solve) {
-        if (P->opt.sched == CHEB_DM_SCHED_GROUPED)
-            s = launch_tasks(P, P->ntasks_solve, P->ntasks_all, 1, P->ntasks_solve, nullptr, 0, st);
-        else
-            s = run_tasks(P, P->ntasks_solve, P->ntasks_all, nullptr, 0, st);
-        if (s != CHEB_DM_OK) return s;
-    }
-    moments_kernel<<<1, 256, 0, st>>>(part1, nchunks, P->dots, tiles, k, p, P->N, P->tau);
-    ++P->last_launches;
-    CUDA_TRY(cudaGetLastError());
-    P->have_moments = 1;
-    P->computed = 1;
-    if (tau_host) {
-        CUDA_TRY(cudaMemcpyAsync(tau_host, P->tau, sizeof(double) * (size_t)k * p, cudaMemcpyDeviceToHost, st));
-        CUDA_TRY(cudaStreamSynchronize(st));
-    }
-    return CHEB_DM_OK;
-}
-
-cheb_dm_status_t cheb_dm_solve_mu(cheb_dm_plan_t P, double beta, double n_occ, int iters, double* mu_out,
-                                  void* cuda_stream) {
-    if (!P || !mu_out || iters < 1 || !isfinite(beta) || !(beta > 0.0) || !isfinite(n_occ)) return CHEB_DM_EINVAL;
-    if (!P->have_moments) return CHEB_DM_ESTATE;
-    if (!device_ok(P)) return CHEB_DM_ECUDA;
-    cudaStream_t st = (cudaStream_t)cuda_stream;
-    mu_weights_kernel<<<P->Nq, 128, 0, st>>>(P->tau, P->costab, P->Nq, P->M, P->w);
-    mu_bisect_kernel<<<1, 1024, 0, st>>>(P->sc, beta, n_occ, iters, P->costab, P->Nq, P->w);
-    CUDA_TRY(cudaGetLastError());
-    DevScalars h;
-    CUDA_TRY(cudaMemcpyAsync(&h, P->sc, sizeof(h), cudaMemcpyDeviceToHost, st));
-    CUDA_TRY(cudaStreamSynchronize(st));
-    if (h.bad_bounds) return CHEB_DM_EBOUNDS;
-    *mu_out = h.mu;
     return CHEB_DM_OK;
 }
 

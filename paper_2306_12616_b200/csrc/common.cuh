@@ -7,6 +7,8 @@
 
 namespace chebdm {
 
+constexpr int MAX_BATCH = 64;           // matrices ("slots") of one grouped launch (cheb_dm_compute_batch)
+
 __device__ __forceinline__ uint32_t smem_u32(const void* p) {
     return static_cast<uint32_t>(__cvta_generic_to_shared(p));
 }

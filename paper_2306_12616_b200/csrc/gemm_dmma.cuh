@@ -32,7 +32,7 @@ constexpr int TILE_RING = 2;            // producer run-ahead (tile descriptors 
 constexpr int MAX_DEPS = 4;
 constexpr long long WATCHDOG_CLOCKS = 8000000000ll;
 
-enum DepKind : int { DEP_NONE = 0, DEP_TASK = 1, DEP_PANEL_N = 2, DEP_GROUP = 3 };
+enum DepKind : int { DEP_NONE = 0, DEP_TASK = 1, DEP_PANEL_N = 2 };
 
 struct Task {
     // operands (indices into the tensor-map table); ktiles == 0 => no product, epilogue only
@@ -42,14 +42,16 @@ struct Task {
     int sym;                 // 1: the result is symmetric (every operand is a polynomial of X): only the tiles that touch
                              // the lower triangle are work items, each mirrors its blocks into the skipped tiles
     int nitems;              // work items of this task (tiles_m * tiles_n, or the lower-triangle count when sym)
-    int group;               // group whose counter this task's tiles increment
-    int out_is_user;         // Out = the user's D (pointer/ld come from the launch parameters)
+    int slot;                // matrix of the batch this task belongs to (0 for single solves)
+    int out_is_user;         // Out = the user's D of this slot (pointer/ld come from the launch parameters)
+    int kchunks;             // >= 1: the K loop runs over kchunks operand pairs (mapA + c, mapB + c), ktiles k-tiles
+                             // each: one long-K product  sum_c A_c^T B_c  (flat giant step)
     int ndeps;
     int ndeps_early;         // deps [0, ndeps_early) guard the operands of the low-order sum (read by the consumer
                              // warps BEFORE the K loop); the rest guard the TMA operands and C
     int dep_kind[MAX_DEPS];
-    int dep_idx[MAX_DEPS];   // task index (DEP_TASK, DEP_PANEL_N) or group index (DEP_GROUP)
-    int dep_target[MAX_DEPS];  // counter value that means "complete" (tiles of the task / panel / group)
+    int dep_idx[MAX_DEPS];   // task index inside the table of this launch (DEP_TASK, DEP_PANEL_N)
+    int dep_target[MAX_DEPS];  // counter value that means "complete" (tiles of the task / panel)
     double alpha, beta;
     const double* C;         // nullable
     long long ldc;
@@ -59,33 +61,38 @@ struct Task {
     long long sum_stride;
     long long lds;
     int sum_count;
-    int dot_count;           // moments: <Out, S_i>_F partial sums for i < dot_count (0 = off)
     const double* coef;      // coef[i], i < sum_count (device memory, written by the coefficient kernel)
     const double* diag_ptr;  // nullable: coefficient of T_0 = I
     double diag_const;
-    double* dot_out;         // [tile][dot_count+1] partials (entry dot_count = partial trace of Out)
 };
 
 struct TraceRec;
 
+// A launch runs the tasks of one table.  The table holds, for every "level task" lt (one product of the method, in
+// topological order), one task per matrix of the batch: index lt * maxb + slot.  A launch covers the level tasks
+// [lt_begin, lt_end) of the slots [0, nb); every task of a table has the same number of work items, so work item w of
+// the launch is tile (w % items_per_task) of task ((w / items_per_task) / nb, (w / items_per_task) % nb): items are
+// claimed level by level and, inside a level, matrix by matrix -- the independent products of different matrices
+// fill the machine where one small matrix cannot.
 struct LaunchArgs {
-    const Task* tasks;
-    const int* task_first;   // prefix sums of tiles, ntasks+1 entries
+    const Task* tasks;       // table
     const CUtensorMap* maps;
     int* work_counter;       // claimed-items counter of this launch
-    int* task_done;          // [ntasks]
-    int* panel_done;         // [ntasks * panel_stride]
-    int* group_done;         // [ngroups]
+    int* task_done;          // [table tasks]
+    int* panel_done;         // [table tasks * panel_stride]
     int panel_stride;
-    int task_begin, task_end;
+    int lt_begin, lt_end;    // level tasks of this launch
+    int nb, maxb;            // matrices in this launch / slots of the table
+    int items_per_task;
     int use_deps;
     int N;
-    double* userD;
+    double* userD[MAX_BATCH];  // per slot: the caller's D
     long long ldD;
     int tma2d;               // 1: operand maps are 2-D {column, row} with one 16-column box per copy
     const int* sym_first;    // [tiles_n + 1] prefix sums of the per-panel item counts of a symmetric task
     int* error_flag;         // set to 1 if a dependency wait exceeds the watchdog (never in a correct run)
-    TraceRec* trace;         // nullable: per-item timeline, indexed by the global item number
+    TraceRec* trace;         // nullable: per-item timeline, indexed by trace_base + work item of the launch
+    int trace_base;
 };
 
 // BM x BN CTA tile, WM x WN warp tile (multiples of 16 / 8), BK k-rows per pipeline stage.
@@ -104,8 +111,7 @@ struct GemmCfg {
     static constexpr int A_BYTES = BM * BK * 8, B_BYTES = BN * BK * 8;
     static constexpr int STAGE_BYTES = A_BYTES + B_BYTES;
     static constexpr int BAR_OFFSET = STAGES * STAGE_BYTES;
-    static constexpr int DOT_OFFSET = BAR_OFFSET + 256;          // [CONSUMER_WARPS][32] doubles (moments epilogue)
-    static constexpr int TRC_OFFSET = DOT_OFFSET + CONSUMER_WARPS * 32 * 8;  // [TILE_RING][4] u64 trace hand-off
+    static constexpr int TRC_OFFSET = BAR_OFFSET + 256;          // [TILE_RING][4] u64 trace hand-off
     static constexpr int SMEM_BYTES = TRC_OFFSET + 64 + 1024;     // + alignment slack
     // small warp tiles have the registers to fetch the C tile as soon as the dependencies are known to be
     // satisfied (first full barrier), which takes one L2 round trip off the serial chain of the giant steps
@@ -157,9 +163,7 @@ __device__ __forceinline__ void wait_counter(const int* ctr, int target, int* er
     (void)ld_acquire_gpu(ctr);
 }
 
-// DOTS = true: the instance used by the moments chain (cheb_dm_moments), whose epilogue also forms the Frobenius
-// products; the solve uses the DOTS = false instance, which does not carry that code (and its registers).
-template <class Cfg, bool DOTS>
+template <class Cfg>
 __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MIN_CTAS) gemm_dmma_kernel(const LaunchArgs args) {
     constexpr int BM = Cfg::BM, BN = Cfg::BN, BK = Cfg::BK, STAGES = Cfg::STAGES;
     constexpr int FM = Cfg::FM, FN = Cfg::FN;
@@ -169,7 +173,7 @@ __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MIN_CTAS) gemm_dmma_kernel(
     // (the pad is applied as an offset so that the pointer keeps its shared address space: LDS, not generic LD)
     uint8_t* smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
     uint64_t* bars = reinterpret_cast<uint64_t*>(smem + Cfg::BAR_OFFSET);
-    // bars[0..S) full, [S..2S) empty, [2S..2S+R) tile_full, [2S+R..2S+2R) tile_empty, [2S+2R] tile stored
+    // bars[0..S) full, [S..2S) empty, [2S..2S+R) tile_full, [2S+R..2S+2R) tile_empty, [2S+2R..2S+3R) tile stored
     TileInfo* ring = reinterpret_cast<TileInfo*>(smem + Cfg::BAR_OFFSET + 192);
     const uint32_t smem_base = smem_u32(smem);
     const uint32_t bar_base = smem_u32(bars);
@@ -177,7 +181,9 @@ __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MIN_CTAS) gemm_dmma_kernel(
     auto empty_bar = [&](int s) { return bar_base + 8u * (STAGES + s); };
     auto tfull_bar = [&](int s) { return bar_base + 8u * (2 * STAGES + s); };
     auto tempty_bar = [&](int s) { return bar_base + 8u * (2 * STAGES + TILE_RING + s); };
-    const uint32_t stored_bar = bar_base + 8u * (2 * STAGES + 2 * TILE_RING);
+    // one "stored" barrier per descriptor slot: a consumer warp may run one tile ahead of a slow warp (next tile's K
+    // loop fits the free ring, or epilogue-only tiles), and its arrive for tile n+1 must not complete tile n's phase
+    auto stored_bar = [&](int s) { return bar_base + 8u * (2 * STAGES + 2 * TILE_RING + s); };
     unsigned long long* trc = reinterpret_cast<unsigned long long*>(smem + Cfg::TRC_OFFSET);
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -190,14 +196,14 @@ __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MIN_CTAS) gemm_dmma_kernel(
         for (int s = 0; s < TILE_RING; ++s) {
             mbar_init(tfull_bar(s), 1);
             mbar_init(tempty_bar(s), Cfg::CONSUMER_WARPS + 1);  // consumer warps + publisher
+            mbar_init(stored_bar(s), Cfg::CONSUMER_WARPS);
         }
-        mbar_init(stored_bar, Cfg::CONSUMER_WARPS);
         fence_mbar_init();
     }
     __syncthreads();
 
-    const int item_begin = args.task_first[args.task_begin];
-    const int item_end = args.task_first[args.task_end];
+    const int ipt = args.items_per_task;
+    const int item_end = (args.lt_end - args.lt_begin) * args.nb * ipt;
 
     if (warp == Cfg::CONSUMER_WARPS) {
         // =================================== producer warp ===================================
@@ -206,47 +212,39 @@ __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MIN_CTAS) gemm_dmma_kernel(
             uint32_t phase = 0;
             int tslot = 0;
             uint32_t tphase = 0;
-            int cur = args.task_begin;
-            unsigned long long done_tasks_lo = 0;  // cache of "task complete" observations (tasks < 64 rel.)
+            const int tbase = args.lt_begin * args.maxb;   // first table task of this launch
+            unsigned long long done_tasks[8] = {0ull, 0ull, 0ull, 0ull, 0ull, 0ull, 0ull, 0ull};  // "task complete" seen (rel. index < 512)
             unsigned long long fenced_maps[4] = {0ull, 0ull, 0ull, 0ull};  // tensor maps this CTA has acquired
             auto acquire_map = [&](int m) {
                 if (m < 256 && ((fenced_maps[m >> 6] >> (m & 63)) & 1ull)) return;
                 fence_tensormap_acquire(args.maps + m);
                 if (m < 256) fenced_maps[m >> 6] |= 1ull << (m & 63);
             };
-            unsigned int done_groups = 0;
             // One dependency of task `tk` for column panel `tn` (no-op when already observed complete).
             auto wait_dep = [&](const Task* tk, int d, int tn) {
                 const int kind = tk->dep_kind[d], idx = tk->dep_idx[d], target = tk->dep_target[d];
+                const int rel = idx - tbase;
                 const int* ctr;
                 if (kind == DEP_TASK) {
-                    const int rel = idx - args.task_begin;
-                    if (rel >= 0 && rel < 64 && ((done_tasks_lo >> rel) & 1ull)) return;
+                    if (rel >= 0 && rel < 512 && ((done_tasks[rel >> 6] >> (rel & 63)) & 1ull)) return;
                     ctr = args.task_done + idx;
-                } else if (kind == DEP_PANEL_N) {
-                    ctr = args.panel_done + (size_t)idx * args.panel_stride + tn;
                 } else {
-                    if ((done_groups >> idx) & 1u) return;
-                    ctr = args.group_done + idx;
+                    ctr = args.panel_done + (size_t)idx * args.panel_stride + tn;
                 }
                 wait_counter(ctr, target, args.error_flag);
-                if (kind == DEP_TASK) {
-                    const int rel = idx - args.task_begin;
-                    if (rel >= 0 && rel < 64) done_tasks_lo |= 1ull << rel;
-                } else if (kind == DEP_GROUP) {
-                    done_groups |= 1u << idx;
-                }
+                if (kind == DEP_TASK && rel >= 0 && rel < 512) done_tasks[rel >> 6] |= 1ull << (rel & 63);
             };
             for (;;) {
-                const int item = item_begin + atomicAdd(args.work_counter, 1);
+                const int item = atomicAdd(args.work_counter, 1);
                 const bool stop = item >= item_end;
                 const unsigned long long t_claim = args.trace ? global_ns() : 0ull;
-                int tm = 0, tn = 0;
+                int tm = 0, tn = 0, cur = tbase;
                 const Task* tk = nullptr;
                 if (!stop) {
-                    while (item >= args.task_first[cur + 1]) ++cur;
+                    const int tq = item / ipt, local = item - tq * ipt;
+                    const int lt = tq / args.nb, slot = tq - lt * args.nb;
+                    cur = (args.lt_begin + lt) * args.maxb + slot;
                     tk = args.tasks + cur;
-                    const int local = item - args.task_first[cur];
                     const int tiles_m = tk->tiles_m;
                     if (!tk->sym) {
                         tn = local / tiles_m;  // column-panel-major order: a panel's tiles are consecutive
@@ -284,11 +282,12 @@ __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MIN_CTAS) gemm_dmma_kernel(
                     fence_proxy_async_global();  // data written through the generic proxy, read next by TMA
                 }
                 const int ktiles = tk->ktiles;
-                if (ktiles > 0) {
-                    const CUtensorMap* mapA = args.maps + tk->mapA;
-                    const CUtensorMap* mapB = args.maps + tk->mapB;
-                    acquire_map(tk->mapA);
-                    acquire_map(tk->mapB);
+                const int kchunks = ktiles > 0 ? tk->kchunks : 0;
+                for (int kc = 0; kc < kchunks; ++kc) {
+                    const CUtensorMap* mapA = args.maps + tk->mapA + kc;
+                    const CUtensorMap* mapB = args.maps + tk->mapB + kc;
+                    acquire_map(tk->mapA + kc);
+                    acquire_map(tk->mapB + kc);
                     const int slabA = tm * (BM / 16), slabB = tn * (BN / 16);
                     for (int kt = 0; kt < ktiles; ++kt) {
                         mbar_wait(empty_bar(stage), phase ^ 1);
@@ -322,29 +321,27 @@ __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MIN_CTAS) gemm_dmma_kernel(
         // =================================== publisher warp ===================================
         // Publishes the completion of each tile: waits until every consumer warp has stored its part (mbarrier
         // arrive = release, CTA scope), makes the tile visible device-wide with ONE gpu-scope fence (cumulative over
-        // the stores it has synchronised with), then bumps the three counters.  The consumer warps meanwhile go
+        // the stores it has synchronised with), then bumps the two counters.  The consumer warps meanwhile go
         // straight on to their next tile.  Waiting producers pair this with ld.acquire.gpu + fence.proxy.async.
-        // The descriptor slot is released only after publication, so the consumers are never two tiles ahead.
+        // The descriptor slot is released only after publication, so the consumers are never two tiles ahead; each
+        // descriptor slot has its own "stored" barrier, so being ONE tile ahead cannot be mis-attributed either.
         if (lane == 0) {
             int tslot = 0;
-            uint32_t tphase = 0, sphase = 0;
+            uint32_t tphase = 0;
             for (;;) {
                 mbar_wait(tfull_bar(tslot), tphase);
                 const TileInfo ti = ring[tslot];
                 if (!ti.stop) {
-                    const Task* tk = args.tasks + ti.task;
-                    mbar_wait(stored_bar, sphase);
-                    sphase ^= 1;
+                    mbar_wait(stored_bar(tslot), tphase);  // slot s is used once per ring cycle: same phase as its descriptor
                     fence_acq_rel_gpu();
                     red_relaxed_gpu_add(args.panel_done + (size_t)ti.task * args.panel_stride + ti.tn, 1);
                     red_relaxed_gpu_add(args.task_done + ti.task, 1);
-                    red_relaxed_gpu_add(args.group_done + tk->group, 1);
                     if (args.trace != nullptr) {
                         TraceRec r;
                         r.task = ti.task; r.tm = ti.tm; r.tn = ti.tn; r.sm = sm_id();
                         r.t_claim = ti.t_claim; r.t_desc = trc[tslot * 4 + 0]; r.t_first = trc[tslot * 4 + 1];
                         r.t_kend = trc[tslot * 4 + 2]; r.t_done = global_ns();
-                        args.trace[ti.item] = r;
+                        args.trace[args.trace_base + ti.item] = r;
                     }
                 }
                 mbar_arrive_dep(tempty_bar(tslot), ti.task ^ ti.tm ^ ti.tn ^ ti.stop ^ ti.item ^ (int)ti.t_claim);
@@ -485,7 +482,7 @@ __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MIN_CTAS) gemm_dmma_kernel(
         // passed, every DMMA of the previous iteration has issued, hence every ld.shared feeding them has returned.
         // (Arriving at the end of the same iteration is not safe: the arrive can overtake loads still in flight and
         // the producer's next TMA write then races with them.)
-        const int ktiles = tk->ktiles;
+        const int ktiles = tk->ktiles * (tk->ktiles > 0 ? tk->kchunks : 0);
         int prev_stage = -1;
         for (int kt = 0; kt < ktiles; ++kt) {
             mbar_wait(full_bar(stage), phase);
@@ -602,7 +599,7 @@ __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MIN_CTAS) gemm_dmma_kernel(
             }
         }
         {
-            double* Out = tk->out_is_user ? args.userD : tk->Out;
+            double* Out = tk->out_is_user ? args.userD[tk->slot] : tk->Out;
             const long long ldo = tk->out_is_user ? args.ldD : tk->ldo;
             const bool vec = ((ldo & 1) == 0) && ((reinterpret_cast<uintptr_t>(Out) & 15) == 0);
 #pragma unroll
@@ -653,70 +650,6 @@ __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MIN_CTAS) gemm_dmma_kernel(
                 }
             }
         }
-        // ------------- moments: Frobenius products <Out, T_i> and tr Out of this tile (reading A10) -------------
-        const int nd = tk->dot_count;
-        if (DOTS && tk->dot_out != nullptr) {
-            if (tk->sym) {
-                // symmetric task: a block whose mirror lies in a skipped tile stands for both in the Frobenius products
-                // (the accumulators are not needed for anything else after the stores; diagonal blocks keep weight 1)
-#pragma unroll
-                for (int i = 0; i < FM; ++i)
-#pragma unroll
-                    for (int j = 0; j < FN; ++j) {
-                        const int R0 = ti.tm * BM + wm * Cfg::WM + i * 8, C0 = ti.tn * BN + wn * Cfg::WN + j * 8;
-                        if ((C0 / BM) * BM + BM - 1 < (R0 / BN) * BN) {
-                            acc[i][j][0] *= 2.0;
-                            acc[i][j][1] *= 2.0;
-                        }
-                    }
-            }
-            double* s_red = reinterpret_cast<double*>(smem + Cfg::DOT_OFFSET);
-            const long long lds = tk->lds, sstride = tk->sum_stride;
-            const double* sb = tk->sum_base + (long long)row0 * lds + col0;
-            double* dst = tk->dot_out + (size_t)(ti.tn * tk->tiles_m + ti.tm) * (nd + 1);
-            for (int s0 = 0; s0 <= nd; s0 += 32) {
-                const int cnt = min(32, nd + 1 - s0);
-                for (int q = 0; q < cnt; ++q) {
-                    const int s = s0 + q;
-                    double v = 0.0;
-                    if (s < nd) {
-                        const double* ps = sb + (long long)s * sstride;
-#pragma unroll
-                        for (int i = 0; i < FM; ++i) {
-                            const int r = row0 + i * 8;
-#pragma unroll
-                            for (int j = 0; j < FN; ++j) {
-                                const int c = col0 + j * 8;
-                                if (r < N && c < N) {
-                                    const double2 w2 = __ldcg(reinterpret_cast<const double2*>(ps + (long long)(i * 8) * lds + j * 8));
-                                    v = fma(acc[i][j][0], w2.x, v);
-                                    v = fma(acc[i][j][1], w2.y, v);
-                                }
-                            }
-                        }
-                    } else {  // slot nd: trace
-#pragma unroll
-                        for (int i = 0; i < FM; ++i)
-#pragma unroll
-                            for (int j = 0; j < FN; ++j) {
-                                const int r = row0 + i * 8, c = col0 + j * 8;
-                                if (r < N && r == c) v += acc[i][j][0];
-                                if (r < N && r == c + 1) v += acc[i][j][1];
-                            }
-                    }
-#pragma unroll
-                    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
-                    if (lane == 0) s_red[warp * 32 + q] = v;
-                }
-                named_bar_sync(1, Cfg::CONSUMER_THREADS);
-                if (threadIdx.x < cnt) {
-                    double v = 0.0;
-                    for (int w = 0; w < Cfg::CONSUMER_WARPS; ++w) v += s_red[w * 32 + threadIdx.x];
-                    dst[s0 + threadIdx.x] = v;
-                }
-                named_bar_sync(1, Cfg::CONSUMER_THREADS);
-            }
-        }
         // --------------------- hand the tile over to the publisher warp ---------------------
         if (tracing) {
             trc[ti_slot * 4 + 0] = t_desc;
@@ -724,7 +657,7 @@ __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MIN_CTAS) gemm_dmma_kernel(
             trc[ti_slot * 4 + 2] = t_kend;
         }
         __syncwarp();
-        if (lane == 0) mbar_arrive(stored_bar);
+        if (lane == 0) mbar_arrive(stored_bar(ti_slot));
     }
 }
 

@@ -39,12 +39,12 @@ constexpr int GR_SUM_CHUNK = 16;                         // low-order sums forme
 constexpr int GR_MAX_KTILES = 16;                        // N <= 512
 
 struct GiantArgs {
-    const Task* tasks;       // giant tasks: tasks[first_task + s], s = 0..nsteps-1 (s = 0 is the product-free step)
+    const Task* tasks;       // giant tasks: tasks[(first_task + s) * task_stride], s = 0..nsteps-1 (s = 0 is the product-free step)
     const CUtensorMap* maps;
-    int first_task, nsteps;
+    int first_task, nsteps, task_stride;
     int N, ktiles;
     int tiles_m, tiles_n;    // 32-row blocks, 32-column panels
-    int* panel_done;         // [task][panel] completion counters (target tiles_m)
+    int* panel_done;         // [step][panel] completion counters (target tiles_m)
     int panel_stride;
     double* userD;
     long long ldD;
@@ -118,7 +118,7 @@ __global__ void __launch_bounds__(GR_THREADS, 1) giant_resident_kernel(const Gia
         if (lane != 0) return;
         if (g == 0) {
             // resident A: rows [tm*32, tm*32+32) of Y = T_k as [k][column] blocks (Y is symmetric)
-            const Task* t1 = args.tasks + args.first_task + (nsteps > 1 ? 1 : 0);
+            const Task* t1 = args.tasks + (size_t)(args.first_task + (nsteps > 1 ? 1 : 0)) * args.task_stride;
             const CUtensorMap* mapA = args.maps + t1->mapA;
             fence_tensormap_acquire(mapA);
             mbar_arrive_expect_tx(resa_bar(), (uint32_t)(ktiles * GR_TILE_BYTES));
@@ -136,10 +136,9 @@ __global__ void __launch_bounds__(GR_THREADS, 1) giant_resident_kernel(const Gia
         int stage = 0;
         uint32_t phase = 0;
         for (int s = 0; s < nsteps; ++s) {
-            const int ti = args.first_task + s;
-            const Task* tk = args.tasks + ti;
+            const Task* tk = args.tasks + (size_t)(args.first_task + s) * args.task_stride;
             if (tk->ktiles > 0) {
-                wait_counter(args.panel_done + (size_t)(ti - 1) * args.panel_stride + ctr, dep_target, args.error_flag);
+                wait_counter(args.panel_done + (size_t)(s - 1) * args.panel_stride + ctr, dep_target, args.error_flag);
                 fence_proxy_async_global();
                 const CUtensorMap* mapB = args.maps + tk->mapB;
                 if (s <= 2) fence_tensormap_acquire(mapB);  // the two ping-pong buffers alternate as operand B
@@ -160,7 +159,7 @@ __global__ void __launch_bounds__(GR_THREADS, 1) giant_resident_kernel(const Gia
             // tile visible device-wide, then the panel counter is bumped
             mbar_wait(stored_bar(g), (uint32_t)(s & 1));
             fence_acq_rel_gpu();
-            red_relaxed_gpu_add(args.panel_done + (size_t)ti * args.panel_stride + ctr, 1);
+            red_relaxed_gpu_add(args.panel_done + (size_t)s * args.panel_stride + ctr, 1);
         }
         return;
     }
@@ -288,7 +287,7 @@ __global__ void __launch_bounds__(GR_THREADS, 1) giant_resident_kernel(const Gia
 #pragma unroll
             for (int j = 0; j < 2; ++j) pv[i][j] = make_double2(0.0, 0.0);
         if (kh != 0 || s >= nsteps || g >= npanels) return;
-        const Task* tk = args.tasks + args.first_task + s;
+        const Task* tk = args.tasks + (size_t)(args.first_task + s) * args.task_stride;
         if (tk->sum_count <= 0) return;
         const double* sb = tk->sum_base + (long long)row0 * tk->lds + colp[g];
 #pragma unroll
@@ -303,7 +302,7 @@ __global__ void __launch_bounds__(GR_THREADS, 1) giant_resident_kernel(const Gia
 
     for (int s = 0; s < nsteps; ++s) {
         const int ti = args.first_task + s;
-        const Task* tk = args.tasks + ti;
+        const Task* tk = args.tasks + (size_t)ti * args.task_stride;
         const int kts = tk->ktiles;
         const double alpha = tk->alpha;
         const double* Cp = tk->C;

@@ -23,7 +23,7 @@ def moments_from_spectrum(E, a, b, M):
 
 
 @functools.lru_cache(maxsize=16)
-def case(cfg, seed=0, n=None, M=None, full=True, bounds="gershgorin"):
+def case(cfg, seed=0, n=None, M=None, full=True, bounds="gershgorin", mu_fixed=None):
     c = workloads.CONFIGS[cfg]
     H = workloads.hamiltonian(cfg, seed=seed, n=n)
     N = H.shape[0]
@@ -40,7 +40,8 @@ def case(cfg, seed=0, n=None, M=None, full=True, bounds="gershgorin"):
         w = 0.01 * (hi - lo)
         a, b = lo - w, hi + w
     tau = moments_from_spectrum(E, a, b, M)
-    mu = oracle.solve_mu(tau, c.beta, a, b, nocc, iters=100)
+    # mu_fixed: skip the bisection (100 x M x N_q long-double terms: minutes for M ~ 4600) and use the given value
+    mu = oracle.solve_mu(tau, c.beta, a, b, nocc, iters=100) if mu_fixed is None else float(mu_fixed)
     coef = oracle.cheb_coeffs(c.beta, mu, a, b, M)
     out = dict(cfg=cfg, H=H, N=N, M=M, beta=c.beta, nocc=nocc, a=a, b=b, E=E, V=V, tau=tau, mu=mu, c=coef)
     xt = (2.0 * E - (a + b)) / (b - a)

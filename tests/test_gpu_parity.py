@@ -104,7 +104,7 @@ def test_coefficient_tables(M, k, p):
 # ----------------------------------------------------------------------------------------------
 # a-4: baby steps T_2..T_k (Eq. 7, 22-23, Algorithm 1) vs the three-term recurrence of the oracle
 # ----------------------------------------------------------------------------------------------
-@pytest.mark.parametrize("pairing", [0, 1, 2])
+@pytest.mark.parametrize("pairing", [0, 1, 2, 3])
 @pytest.mark.parametrize("k", [2, 3, 5, 8, 11])
 def test_baby_steps_match_three_term_recurrence(k, pairing):
     oracle, cd, workloads, gu, _ = _imports()
@@ -215,19 +215,29 @@ def test_parity_power_outer_recursion_eq4():
 def test_parity_serial_pairing_and_nonsquare_kp():
     oracle, cd, workloads, gu, oc = _imports()
     case = oc.case("cfg2", 0, 250, None)
-    for kw in (dict(pairing=1), dict(k=32, p=8), dict(k=8, p=32), dict(k=20, p=13), dict(k=256, p=1), dict(k=1, p=256)):
+    for kw in (dict(pairing=1), dict(pairing=3), dict(k=32, p=8), dict(k=8, p=32), dict(k=20, p=13), dict(k=256, p=1), dict(k=1, p=256)):
         r = gu.gpu_solve(case["H"], case["beta"], case["mu"], case["M"], bounds=(case["a"], case["b"]), **kw)
         _check(case, r)
 
 
-def test_converged_variant_meets_1e6_vs_diagonalisation():
-    """North-star's "<= 1e-6 vs the diagonalisation DM": holds with tight bounds and enough terms
-    (SURVEY A2-iii); with Gershgorin bounds the configs' M are far from converged."""
+# (config, reduced n, M): tight bounds (spectrum widened by 1 %) and M ~ 4.4 beta~ rounded up
+# cfg4 (beta~ ~ 1010 even with tight bounds): mu fixed at the centre of its dense level cluster instead of the bisection
+CONVERGED = [("cfg0", 128, 208, None), ("cfg1", 300, 512, None), ("cfg2", 250, 480, None), ("cfg3", 200, 720, None),
+             ("cfg4", 200, 4608, 0.0)]
+
+
+@pytest.mark.parametrize("cfg,n,M,mu_fixed", CONVERGED)
+def test_converged_variant_meets_1e6_vs_diagonalisation(cfg, n, M, mu_fixed):
+    """North-star's "<= 1e-6 vs the diagonalisation DM", one demonstration per config kind: holds with tight bounds
+    and enough terms; with Gershgorin bounds the configs' own M are far from converged."""
     oracle, cd, workloads, gu, oc = _imports()
-    case = oc.case("cfg1", 0, 300, 512, True, "tight")
-    assert case["eps_trunc"] <= 1e-6
+    case = oc.case(cfg, 0, n, M, True, "tight", mu_fixed)
+    assert case["eps_trunc"] <= 1e-6, case["eps_trunc"]
     r = gu.gpu_solve(case["H"], case["beta"], case["mu"], case["M"], bounds=(case["a"], case["b"]))
-    _check(case, r)
+    assert np.max(np.abs(r["D"] - case["D_cheb"])) <= TOL_D
+    assert abs(r["trace"] - float(np.trace(case["D_cheb"]))) <= TOL_TR
+    if mu_fixed is None:
+        assert abs(float(np.trace(case["D_cheb"])) - case["nocc"]) <= 1e-7  # mu solved on the trace
     assert np.max(np.abs(r["D"] - case["D_eig"])) <= 1e-6
 
 
@@ -328,12 +338,161 @@ def test_status_codes():
     plan.destroy()
 
 
+def test_sticky_device_flags_survive_later_computes():
+    """a device-side error of ANY solve of a pipeline is reported by the one check at its end (the flags are
+    sticky and cleared by the check), not erased by the next compute's front end."""
+    oracle, cd, workloads, gu, _ = _imports()
+    torch = gu.torch_cuda()
+    st = torch.cuda.current_stream().cuda_stream
+    n = 40
+    good = gu.to_dev(workloads.hamiltonian("cfg1", seed=0, n=n))
+    Hb = workloads.hamiltonian("cfg1", seed=1, n=n)
+    Hb[3, 4] = Hb[4, 3] = np.inf
+    bad = gu.to_dev(Hb)
+    dD = torch.empty((n, n), dtype=torch.float64, device="cuda")
+    plan = cd.Plan(n, 16)
+    plan.coeffs(5.0, 0.0, None)
+    plan.compute(bad.data_ptr(), dD.data_ptr(), st)
+    plan.compute(good.data_ptr(), dD.data_ptr(), st)
+    plan.compute(good.data_ptr(), dD.data_ptr(), st)
+    with pytest.raises(cd.ChebDMError) as ei:
+        plan.check(st)
+    assert ei.value.status == 5       # EBOUNDS from the first of the three computes
+    plan.check(st)                    # reported once, then cleared
+    plan.compute(good.data_ptr(), dD.data_ptr(), st)
+    plan.check(st)
+    plan.destroy()
+
+
+def test_enoconv_guard_of_the_power_basis_recursion():
+    """Eq. 4 literally (OUTER_POWER): d_{i,p-1} = 2^p c (Eq. 12, a_{j,j} = 2^{1-j}).  Reading A6: when
+    max|d| 2^-52 p > 1e-12 the device sets a flag and cheb_dm_check returns ENOCONV (cfg4 kind, M = 2048: max|d| ~ 1e13
+    and the result is wrong at the 1e-4 level); short expansions (cfg0) pass."""
+    oracle, cd, workloads, gu, oc = _imports()
+    torch = gu.torch_cuda()
+    st = torch.cuda.current_stream().cuda_stream
+    H = workloads.hamiltonian("cfg4", seed=0, n=200)
+    dH = gu.to_dev(H)
+    dD = torch.empty((200, 200), dtype=torch.float64, device="cuda")
+    plan = cd.Plan(200, 2048, outer=cd.OUTER_POWER)
+    plan.coeffs(200.0, 0.0, None)
+    plan.compute(dH.data_ptr(), dD.data_ptr(), st)
+    with pytest.raises(cd.ChebDMError) as ei:
+        plan.check(st)
+    assert ei.value.status == 7
+    _, _, d = plan.get_coeffs(st)
+    a, b = oracle.gershgorin(H)
+    d_or = oracle.d_from_g(plan.k, plan.p, oracle.g_from_c(plan.k, plan.p, oracle.pad_coeffs(oracle.cheb_coeffs(200.0, 0.0, a, b, 2048), plan.k, plan.p)))
+    assert np.max(np.abs(d_or)) * 2.0 ** -52 * plan.p > 1e-12          # the oracle's table trips the same rule
+    plan.destroy()
+    case = oc.case("cfg0", 0, 128, None)
+    r = gu.gpu_solve(case["H"], case["beta"], case["mu"], case["M"], outer=cd.OUTER_POWER)   # gpu_solve calls check
+    _check(case, r)
+    # the Chebyshev-basis recursion (default) never computes d and never trips
+    r = gu.gpu_solve(H, 200.0, 0.0, 2048)
+    assert np.all(np.isfinite(r["D"]))
+
+
+@pytest.mark.parametrize("n,ldh,ldd", [(130, 136, 133), (257, 258, 300), (64, 64, 70), (33, 40, 33)])
+def test_leading_dimension_options(n, ldh, ldd):
+    """Options ldh / ldd: H and D inside larger device arrays, even and odd pitches."""
+    oracle, cd, workloads, gu, oc = _imports()
+    torch = gu.torch_cuda()
+    st = torch.cuda.current_stream().cuda_stream
+    H = workloads.hamiltonian("cfg1", seed=4, n=n)
+    a, b = oracle.gershgorin(H)
+    M, beta, mu = 48, 30.0, 0.04
+    D_or = oracle.dm_cheb(H, a, b, oracle.cheb_coeffs(beta, mu, a, b, M))
+    Hp = np.full((n, ldh), 7.77)          # the padding must never be read as data
+    Hp[:, :n] = H
+    dH = gu.to_dev(Hp)
+    dD = torch.full((n, ldd), -5.0, dtype=torch.float64, device="cuda")
+    dtr = torch.zeros(1, dtype=torch.float64, device="cuda")
+    for giant in (1, 2):
+        plan = cd.Plan(n, M, ldh=ldh, ldd=ldd, giant=giant)
+        plan.coeffs(beta, mu, None)
+        plan.compute(dH.data_ptr(), dD.data_ptr(), st)
+        plan.trace(dD.data_ptr(), dtr.data_ptr(), st)
+        plan.check(st)
+        got = dD.cpu().numpy()
+        assert np.max(np.abs(got[:, :n] - D_or)) <= TOL_D
+        assert np.all(got[:, n:] == -5.0)                      # the padding of D is never written
+        assert abs(float(dtr.item()) - float(np.trace(D_or))) <= TOL_TR
+        assert plan.get_bounds(st) == pytest.approx((a, b), rel=1e-14)
+        plan.destroy()
+    with pytest.raises(cd.ChebDMError):
+        cd.Plan(n, M, ldh=n - 1)
+
+
+def test_cuda_graph_capture_and_replay():
+    """cheb_dm_compute + cheb_dm_trace allocate nothing, read no environment and never
+    synchronise, so the whole solve (cooperative launches included) is capturable; replays on new H contents are
+    bit-identical to eager calls.  Both the resident-kernel path and the generic one, and a batch."""
+    oracle, cd, workloads, gu, oc = _imports()
+    torch = gu.torch_cuda()
+    n, M, beta = 300, 100, 40.0
+    Hs = [workloads.hamiltonian("cfg1", seed=s, n=n) for s in range(3)]
+    for opts in (dict(), dict(giant=1), dict(max_batch=2)):
+        nb = opts.get("max_batch", 1)
+        plan = cd.Plan(n, M, **opts)
+        plan.coeffs(beta, 0.03, None)
+        dH = [torch.empty((n, n), dtype=torch.float64, device="cuda") for _ in range(nb)]
+        dD = [torch.empty((n, n), dtype=torch.float64, device="cuda") for _ in range(nb)]
+        dtr = torch.zeros(nb, dtype=torch.float64, device="cuda")
+        eager = []
+        st = torch.cuda.current_stream().cuda_stream
+        for H in Hs:
+            for x in dH:
+                x.copy_(torch.from_numpy(H))
+            plan.compute_batch([x.data_ptr() for x in dH], [x.data_ptr() for x in dD], None, st)
+            plan.trace_batch([x.data_ptr() for x in dD], dtr.data_ptr(), st)
+            torch.cuda.synchronize()
+            eager.append((dD[0].cpu().numpy().copy(), float(dtr[0].item())))
+        side = torch.cuda.Stream()
+        g = torch.cuda.CUDAGraph()
+        torch.cuda.synchronize()
+        with torch.cuda.graph(g, stream=side):
+            cs = torch.cuda.current_stream().cuda_stream
+            plan.compute_batch([x.data_ptr() for x in dH], [x.data_ptr() for x in dD], None, cs)
+            plan.trace_batch([x.data_ptr() for x in dD], dtr.data_ptr(), cs)
+        for rep in range(2):
+            for H, (D_e, tr_e) in zip(Hs, eager):
+                for x in dH:
+                    x.copy_(torch.from_numpy(H))
+                for x in dD:
+                    x.fill_(float("nan"))
+                g.replay()
+                torch.cuda.synchronize()
+                for x in dD:
+                    assert np.array_equal(x.cpu().numpy(), D_e)
+                assert float(dtr[nb - 1].item()) == tr_e
+        plan.check(st)
+        del g
+        plan.destroy()
+
+
+def test_resident_kernel_guard_on_large_k():
+    """the resident giant-step kernel stages k * 16 coefficients inside its idle TMA rings (80 KB): plans with
+    k > 640 must fall back to the generic kernel instead of overrunning into the mbarriers."""
+    oracle, cd, workloads, gu, oc = _imports()
+    n, M = 64, 1400
+    H = workloads.hamiltonian("cfg1", seed=0, n=n)
+    a, b = oracle.gershgorin(H)
+    D_or = oracle.dm_cheb(H, a, b, oracle.cheb_coeffs(15.0, 0.02, a, b, M))
+    for k, want in ((700, 1), (640, 2)):
+        r = gu.gpu_solve(H, 15.0, 0.02, M, k=k, p=(M + k - 1) // k, keep_plan=True)
+        assert r["plan"].opts.giant == want
+        r["plan"].destroy()
+        assert np.max(np.abs(r["D"] - D_or)) <= TOL_D
+
+
 # ----------------------------------------------------------------------------------------------
 # a-7: trace, moments, mu
 # ----------------------------------------------------------------------------------------------
-@pytest.mark.parametrize("cfg,n,M,kp", [("cfg0", 128, 64, (0, 0)), ("cfg1", 200, 256, (0, 0)), ("cfg2", 150, 60, (6, 10)),
-                                         ("cfg4", 130, 90, (9, 10)), ("cfg1", 64, 12, (12, 1)), ("cfg1", 64, 12, (3, 4))])
-def test_moments_and_mu(cfg, n, M, kp):
+@pytest.mark.parametrize("cfg,n,M,kp,tile", [("cfg0", 128, 64, (0, 0), 0), ("cfg1", 200, 256, (0, 0), 0), ("cfg2", 150, 60, (6, 10), 0),
+                                              ("cfg4", 130, 90, (9, 10), 0), ("cfg1", 64, 12, (12, 1), 0), ("cfg1", 64, 12, (3, 4), 0),
+                                              ("cfg1", 700, 64, (0, 0), 1), ("cfg1", 500, 256, (0, 0), 0), ("cfg2", 1000, 256, (0, 0), 0)])
+def test_moments_and_mu(cfg, n, M, kp, tile):
     oracle, cd, workloads, gu, oc = _imports()
     torch = gu.torch_cuda()
     H = workloads.hamiltonian(cfg, seed=0, n=n)
@@ -341,7 +500,7 @@ def test_moments_and_mu(cfg, n, M, kp):
     nocc = workloads.n_occ(cfg, n)
     a, b = oracle.gershgorin(H)
     _, tau_or = oracle.dm_cheb(H, a, b, np.zeros(M), want_tau=True)
-    plan = cd.Plan(n, M, k=kp[0], p=kp[1])
+    plan = cd.Plan(n, M, k=kp[0], p=kp[1], tile=tile)
     dH = gu.to_dev(H)
     st = torch.cuda.current_stream().cuda_stream
     plan.coeffs(beta, 0.0, (a, b))

@@ -1,0 +1,134 @@
+"""`-m gpu` parity of the mu-inclusive path: cheb_dm_solve = bounds, baby block and giant block once,
+moments by the Gram kernel, bisection on the device, D = G_0 + sum_l G_l U_l as one long-K product; cheb_dm_assemble
+re-assembles D for new chemical potentials from the resident blocks.
+
+Oracle side (no value flows from the GPU into it): tau_n = tr T_n(X) from the naive matrix recurrence
+(oracle.dm_cheb(..., want_tau=True)), mu by oracle.solve_mu (the 100-halving bisection of reading A9), D by
+oracle.dm_cheb with that mu."""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+TOL_D = 1e-10
+TOL_TR = 1e-9
+
+
+def _imports():
+    import oracle
+    import paper_2306_12616_b200 as cd
+    import workloads
+    import gpu_util
+    return oracle, cd, workloads, gpu_util
+
+
+def _oracle_solution(oracle, workloads, cfg, seed, n, M):
+    H = workloads.hamiltonian(cfg, seed=seed, n=n)
+    N = H.shape[0]
+    c = workloads.CONFIGS[cfg]
+    M = c.M if M is None else M
+    nocc = workloads.n_occ(cfg, N)
+    a, b = oracle.gershgorin(H)
+    _, tau = oracle.dm_cheb(H, a, b, np.zeros(M), want_tau=True)
+    mu = oracle.solve_mu(tau, c.beta, a, b, nocc, iters=100)
+    D = oracle.dm_cheb(H, a, b, oracle.cheb_coeffs(c.beta, mu, a, b, M))
+    return dict(H=H, N=N, M=M, beta=c.beta, nocc=nocc, a=a, b=b, tau=tau, mu=mu, D=D)
+
+
+CASES = [("cfg0", 0, 128, None, {}), ("cfg1", 0, 300, None, {}), ("cfg1", 1, 257, None, {}), ("cfg2", 0, 250, None, {}),
+         ("cfg3", 0, 200, 1024, {}), ("cfg4", 0, 200, 2048, {}), ("cfg1", 2, 130, 60, dict(k=6, p=10)),
+         ("cfg1", 0, 64, 12, dict(k=12, p=1)), ("cfg1", 0, 64, 12, dict(k=1, p=12)), ("cfg1", 0, 64, 12, dict(k=6, p=2)),
+         ("cfg2", 0, 150, 70, dict(k=2, p=35, tile=3)), ("cfg1", 3, 700, 64, dict(tile=1)), ("cfg1", 3, 333, 64, dict(symmetric=1))]
+
+
+@pytest.mark.parametrize("cfg,seed,n,M,opts", CASES)
+def test_solve_mu_inclusive_parity(cfg, seed, n, M, opts):
+    oracle, cd, workloads, gu = _imports()
+    torch = gu.torch_cuda()
+    o = _oracle_solution(oracle, workloads, cfg, seed, n, M)
+    N = o["N"]
+    plan = cd.Plan(N, o["M"], **opts)
+    st = torch.cuda.current_stream().cuda_stream
+    dH = gu.to_dev(o["H"])
+    dD = torch.full((N, N), float("nan"), dtype=torch.float64, device="cuda")
+    dtr = torch.zeros(1, dtype=torch.float64, device="cuda")
+    plan.coeffs(o["beta"], 123.0, None)  # the mu given here is ignored by cheb_dm_solve
+    mu = plan.solve(dH.data_ptr(), o["nocc"], dD.data_ptr(), 100, True, st)
+    plan.trace(dD.data_ptr(), dtr.data_ptr(), st)
+    plan.check(st)
+    a, b, mu_dev, ne = plan.get_scalars(0, st)
+    assert mu == mu_dev
+    # the electron count at the GPU's mu hits the target as well as the oracle's own root does (oracle-side evaluation)
+    ne_gpu = oracle.electron_count(o["tau"], o["beta"], mu, o["a"], o["b"])
+    ne_or = oracle.electron_count(o["tau"], o["beta"], o["mu"], o["a"], o["b"])
+    assert abs(ne_gpu - o["nocc"]) <= max(1e-8, 10 * abs(ne_or - o["nocc"]))
+    assert abs(mu - o["mu"]) <= 1e-10 * max(1.0, abs(o["b"] - o["a"]))
+    D = dD.cpu().numpy()
+    assert np.max(np.abs(D - o["D"])) <= TOL_D
+    assert abs(float(dtr.item()) - float(np.trace(o["D"]))) <= TOL_TR
+    assert abs(float(dtr.item()) - o["nocc"]) <= 1e-7
+    assert np.max(np.abs(D - D.T)) <= 1e-11
+    # moments left on the device by the same call chain (cheb_dm_moments shares the code): compare tau too
+    tau = plan.moments(dH.data_ptr(), True, st)[: o["M"]]
+    assert np.max(np.abs(tau - o["tau"])) <= 1e-10 * N
+    # new chemical potentials from the resident blocks
+    for mu2 in (o["mu"] + 0.05, o["a"] + 0.3 * (o["b"] - o["a"])):
+        plan.assemble([mu2], [dD.data_ptr()], st)
+        torch.cuda.synchronize()
+        D2 = oracle.dm_cheb(o["H"], o["a"], o["b"], oracle.cheb_coeffs(o["beta"], mu2, o["a"], o["b"], o["M"]))
+        assert np.max(np.abs(dD.cpu().numpy() - D2)) <= TOL_D
+    plan.destroy()
+
+
+def test_solve_batch_parity_and_equals_single():
+    """cheb_dm_solve_batch: three matrices with different targets in one set of launches; same mu and D (bitwise) as
+    the single-matrix call on a batch plan, parity with the oracle for each."""
+    oracle, cd, workloads, gu = _imports()
+    torch = gu.torch_cuda()
+    sols = [_oracle_solution(oracle, workloads, "cfg1", s, 200, 100) for s in range(3)]
+    noccs = [100.0, 90.0, 111.0]
+    for o, no in zip(sols, noccs):
+        o["mu"] = oracle.solve_mu(o["tau"], o["beta"], o["a"], o["b"], no, iters=100)
+        o["D"] = oracle.dm_cheb(o["H"], o["a"], o["b"], oracle.cheb_coeffs(o["beta"], o["mu"], o["a"], o["b"], o["M"]))
+    plan = cd.Plan(200, 100, max_batch=4)
+    st = torch.cuda.current_stream().cuda_stream
+    dH = [gu.to_dev(o["H"]) for o in sols]
+    dD = [torch.empty((200, 200), dtype=torch.float64, device="cuda") for _ in sols]
+    plan.coeffs(sols[0]["beta"], 0.0, None)
+    mus = plan.solve_batch([x.data_ptr() for x in dH], noccs, [x.data_ptr() for x in dD], 100, True, st)
+    plan.check(st)
+    Ds = [d.cpu().numpy() for d in dD]
+    for o, mu, D in zip(sols, mus, Ds):
+        assert abs(mu - o["mu"]) <= 1e-10 * (o["b"] - o["a"])
+        assert np.max(np.abs(D - o["D"])) <= TOL_D
+    one = torch.empty((200, 200), dtype=torch.float64, device="cuda")
+    mu1 = plan.solve(dH[1].data_ptr(), noccs[1], one.data_ptr(), 100, True, st)
+    assert mu1 == mus[1] and np.array_equal(one.cpu().numpy(), Ds[1])
+    plan.destroy()
+
+
+def test_solve_needs_the_moments_option_and_call_order():
+    oracle, cd, workloads, gu = _imports()
+    torch = gu.torch_cuda()
+    H = workloads.hamiltonian("cfg1", seed=0, n=64)
+    dH, dD = gu.to_dev(H), torch.empty((64, 64), dtype=torch.float64, device="cuda")
+    plan = cd.Plan(64, 16, moments=1)
+    plan.coeffs(10.0, 0.0, None)
+    for call in (lambda: plan.solve(dH.data_ptr(), 32, dD.data_ptr()), lambda: plan.moments(dH.data_ptr()),
+                 lambda: plan.assemble([0.0], [dD.data_ptr()])):
+        with pytest.raises(cd.ChebDMError) as ei:
+            call()
+        assert ei.value.status == 6  # EUNSUPPORTED
+    plan.destroy()
+    plan = cd.Plan(64, 16)
+    plan.coeffs(10.0, 0.0, None)
+    with pytest.raises(cd.ChebDMError) as ei:
+        plan.assemble([0.0], [dD.data_ptr()])      # no blocks in the workspace yet
+    assert ei.value.status == 4
+    plan.solve(dH.data_ptr(), 32, dD.data_ptr())
+    plan.assemble([0.1], [dD.data_ptr()])
+    plan.compute(dH.data_ptr(), dD.data_ptr())      # a fixed-mu compute overwrites the blocks' bookkeeping
+    with pytest.raises(cd.ChebDMError) as ei:
+        plan.assemble([0.0], [dD.data_ptr()])
+    assert ei.value.status == 4
+    plan.destroy()
