@@ -5,13 +5,15 @@
 
 One "step" = one pass of the whole hot path (Gershgorin bounds + rescale, coefficient
 tables, baby steps, giant steps with fused low-order sums, trace) over one batch of synthetic input
-= one solve per seed of the workload (cfg1: seeds 0-3 -> 4 solves per step), with mu fixed beforehand
-by the (untimed, separately reported) moment/bisection path.  Everything runs through the C ABI
+= one solve per seed of the workload (cfg1: seeds 0-3 -> a batch of 4 solves per step, ONE set of grouped
+launches through cheb_dm_compute_batch), with mu fixed beforehand by the device's own mu-inclusive path.
+That path (cheb_dm_solve_batch: baby block once, giant block, Gram-kernel moments, bisection on the device,
+long-K assembly) is timed too and reported beside it (`mu_inclusive`).  Everything runs through the C ABI
 (include/cheb_dm.h via the ctypes binding); torch supplies device memory, streams and events only.
 
 Prints ONE JSON line (rank 0).  `value` = solves/s with inputs resident in HBM; `e2e` = the same through
-cheb_dm_compute_host with pinned HOST buffers (H2D + D2H inside the timed region); `roofline` = the
-product kernel against the FP64 tensor (DMMA) peak; `cpu_baseline` = the oracle on the host cores.
+cheb_dm_compute_batch_host_async with pinned HOST buffers (H2D + D2H inside the timed region); `roofline` = the
+product kernels against the FP64 tensor (DMMA) peak; `cpu_baseline` = the oracle on the host cores.
 Multi-GPU: replicas only -- every rank runs the same workload on its own GPU, no data-path
 collective; value = all ranks' solves / max-over-ranks time.
 """
@@ -31,15 +33,18 @@ if ROOT not in sys.path:
 METRIC = "dm_solves_per_sec"
 UNIT = "solves/s"
 FLUSH_BYTES = 512 << 20  # > 126 MB L2
-# dram__bytes_read.sum + dram__bytes_write.sum of one product-kernel launch from the `ncu --set full`
-# captures summarised under profiles/ (per workload); None = not captured yet.
-# Sum over the product launches of one solve (baby-step launch + giant-step launch).  ncu replays with cold caches, so
-# for cfg1/cfg2 (working set L2-resident when warm) this is an upper bound.  cfg3: only the baby-step launch was captured.
-NCU_TRAFFIC_BYTES = {
-    "cfg1": 2.462976e6 + 0.00128e6 + 18.196224e6 + 0.335104e6,       # profiles/r01_ncu_cfg1_solve.txt (baby + giant launch)
-    "cfg2": 76.414208e6 + 4.39296e6 + 29.40672e6 + 79.427328e6 + 63.915008e6 + 20.947456e6,  # r01_ncu_cfg2_solve.txt
-    "cfg4": (3.049292 + 1.735402 + 3.774622 + 1.652616 + 2.360862 + 0.712185) * 1e9,         # r01_ncu_cfg4_solve.txt
-}
+# dram__bytes_read.sum + dram__bytes_write.sum of the product launches of one step, from the `ncu --set full` captures
+# summarised under profiles/: read from the data file the capture step writes (never typed here).
+TRAFFIC_FILE = os.path.join(ROOT, "profiles", "r02_traffic.json")
+
+
+def ncu_traffic(name):
+    try:
+        with open(TRAFFIC_FILE) as f:
+            ent = json.load(f).get(name)
+        return (float(ent["dram_bytes_per_step"]), ent.get("source")) if ent else (None, None)
+    except Exception:
+        return None, None
 
 
 def parse_args():
@@ -49,7 +54,9 @@ def parse_args():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", default="cfg1", help="workload of the headline line (BASELINE.json configs[1] = cfg1)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--others", default="cfg2,cfg4,cfg3", help="comma list of extra workloads reported under other_workloads ('' = none)")
+    ap.add_argument("--others", default="cfg0,cfg2,cfg4,cfg3", help="comma list of extra workloads reported under other_workloads ('' = none)")
+    ap.add_argument("--batch", type=int, default=0, help="matrices per step (0 = the workload's seeds; cfg0: 16 seeds)")
+    ap.add_argument("--no-batch", action="store_true", help="ablation: the step's solves as serial cheb_dm_compute calls")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--sched", type=int, default=0)
     ap.add_argument("--tile", type=int, default=0)
@@ -137,54 +144,80 @@ class ClockSampler:
 # ---------------------------------------------------------------------------------------------------
 # GPU arm
 # ---------------------------------------------------------------------------------------------------
+def workload_seeds(cfg, name, args):
+    """cfg1: the four seeds of BASELINE.json; cfg0 (one tile per product): 16 seeded matrices of the same recipe
+    form the batch; the others: their one seed."""
+    n = args.batch if args.batch > 0 else (16 if name == "cfg0" else len(cfg.seeds))
+    return tuple(cfg.seeds) if n == len(cfg.seeds) else tuple(range(n))
+
+
 class Workload:
-    """Device-resident inputs + a plan for one BASELINE.json config; mu per seed from the moment path."""
+    """Device-resident inputs + a plan for one BASELINE.json config; mu per seed from the device's mu-inclusive path."""
 
     def __init__(self, torch, cd, workloads, name, args):
         self.torch, self.cd, self.name = torch, cd, name
         self.cfg = cfg = workloads.CONFIGS[name]
         self.N, self.M = cfg.N, cfg.M
+        self.seeds = workload_seeds(cfg, name, args)
+        self.units = len(self.seeds)
+        self.batched = not args.no_batch
         self.st = torch.cuda.current_stream().cuda_stream
-        self.plan = cd.Plan(cfg.N, cfg.M, sched=args.sched, tile=args.tile, k=args.k, p=args.p, fuse_sums=args.fuse, giant=args.giant, symmetric=args.symmetric)
+        self.plan = cd.Plan(cfg.N, cfg.M, sched=args.sched, tile=args.tile, k=args.k, p=args.p, fuse_sums=args.fuse, giant=args.giant,
+                            symmetric=args.symmetric, max_batch=self.units if self.batched else 1, host_slots=2)
         self.hH, self.dH, self.dD, self.hD = [], [], [], []
-        for seed in cfg.seeds:
+        for seed in self.seeds:
             H = torch.from_numpy(workloads.hamiltonian(name, seed=seed))
             self.hH.append(H.pin_memory())
             self.dH.append(H.cuda())
             self.dD.append(torch.empty((cfg.N, cfg.N), dtype=torch.float64, device="cuda"))
             self.hD.append(torch.empty((cfg.N, cfg.N), dtype=torch.float64).pin_memory())
-        self.dtr = torch.zeros(len(cfg.seeds), dtype=torch.float64, device="cuda")
-        self.htr = torch.zeros(len(cfg.seeds), dtype=torch.float64).pin_memory()
-        # mu per seed: Gershgorin bounds -> moments -> bisection, all on the device (untimed here)
-        self.mu, self.mu_ms = [], []
-        for i in range(len(cfg.seeds)):
-            self.plan.coeffs(cfg.beta, 0.0, None)
-            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            e0.record()
-            self.plan.moments(self.dH[i].data_ptr(), False, self.st)
-            mu = self.plan.solve_mu(cfg.beta, cfg.N_occ, 100, self.st)
-            e1.record()
-            torch.cuda.synchronize()
-            self.mu.append(mu)
-            self.mu_ms.append(e0.elapsed_time(e1))
-        self.units = len(cfg.seeds)
+        self.pH, self.pD = [x.data_ptr() for x in self.dH], [x.data_ptr() for x in self.dD]
+        self.phH, self.phD = [x.data_ptr() for x in self.hH], [x.data_ptr() for x in self.hD]
+        self.dtr = torch.zeros(self.units, dtype=torch.float64, device="cuda")
+        self.htr = torch.zeros(self.units, dtype=torch.float64).pin_memory()
+        self.nocc = [float(cfg.N_occ)] * self.units
+        # mu per seed: Gershgorin bounds -> blocks -> moments -> bisection, all on the device (cheb_dm_solve_batch)
+        self.plan.coeffs(cfg.beta, 0.0, None)
+        if self.batched:
+            self.mu = self.plan.solve_batch(self.pH, self.nocc, self.pD, 100, True, self.st)
+        else:
+            self.mu = [self.plan.solve(self.pH[i], self.nocc[i], self.pD[i], 100, True, self.st) for i in range(self.units)]
+        self.plan.check(self.st)
         self.launches_per_step = 0
 
     def step(self):
+        if self.batched:
+            self.plan.compute_batch(self.pH, self.pD, self.mu, self.st)
+            self.plan.trace_batch(self.pD, self.dtr.data_ptr(), self.st)
+            self.launches_per_step = self.plan.last_launch_count() + 1
+            return
         n = 0
         for i in range(self.units):
             self.plan.coeffs(self.cfg.beta, self.mu[i], None)
-            self.plan.compute(self.dH[i].data_ptr(), self.dD[i].data_ptr(), self.st)
-            self.plan.trace(self.dD[i].data_ptr(), self.dtr[i:].data_ptr(), self.st)
+            self.plan.compute(self.pH[i], self.pD[i], self.st)
+            self.plan.trace(self.pD[i], self.dtr[i:].data_ptr(), self.st)
             n += self.plan.last_launch_count() + 1
         self.launches_per_step = n
 
+    def step_mu_inclusive(self):
+        # the whole "mu solved on the trace" path: nothing is known beforehand but beta and N_occ
+        if self.batched:
+            self.plan.solve_batch(self.pH, self.nocc, self.pD, 100, False, self.st)
+            self.plan.trace_batch(self.pD, self.dtr.data_ptr(), self.st)
+        else:
+            for i in range(self.units):
+                self.plan.solve(self.pH[i], self.nocc[i], self.pD[i], 100, False, self.st)
+                self.plan.trace(self.pD[i], self.dtr[i:].data_ptr(), self.st)
+
     def step_host(self):
-        # the batch of the step through the pipelined host entry point: copies of neighbouring solves overlap the
-        # kernels; every H2D / D2H of the step completes inside the step (cheb_dm_wait)
-        for i in range(self.units):
-            self.plan.coeffs(self.cfg.beta, self.mu[i], None)
-            self.plan.compute_host_async(self.hH[i].data_ptr(), self.hD[i].data_ptr(), self.htr[i:].data_ptr(), self.st)
+        # the batch of the step through the pipelined host entry point; every H2D / D2H of the step completes inside the
+        # step (cheb_dm_wait)
+        if self.batched:
+            self.plan.compute_batch_host_async(self.phH, self.phD, self.htr.data_ptr(), self.mu, self.st)
+        else:
+            for i in range(self.units):
+                self.plan.coeffs(self.cfg.beta, self.mu[i], None)
+                self.plan.compute_host_async(self.phH[i], self.phD[i], self.htr[i:].data_ptr(), self.st)
         self.plan.wait(self.st)
 
     def h2d_bytes(self):
@@ -241,45 +274,60 @@ def job_value(world, units_per_step, steps, max_ms):
 def measure_workload(torch, cd, workloads, name, args, steps, warmup, flush, sampler, dist, peak_tf, world):
     w = Workload(torch, cd, workloads, name, args)
     plan = w.plan
-    # device-resident arm (timing ring on: two event records per compute, no host sync)
+    # device-resident arm (timing ring on: two event records per compute call, no host sync)
     plan.set_timing(True)
     for _ in range(warmup):
         w.step()
     torch.cuda.synchronize()
     plan.set_timing(True)  # resets the ring after warm-up
     total_ms = timed_steps(torch, w.step, steps, 0, flush, sampler, dist)
-    n_rec, prod_ms = plan.product_ms()  # the timed computes only (at most the last 256 of them)
+    n_rec, prod_ms = plan.product_ms()  # the timed compute calls only (at most the last 256 of them)
     plan.set_timing(False)
+    plan.check(w.st)                     # sticky device flags of the whole timed region
     total_ms = max_over_ranks(torch, dist, total_ms)
-    flops = plan.flops_per_compute()
+    flops = plan.flops_per_compute()     # per matrix
+    per_call = w.units if w.batched else 1
     ms_per_step = total_ms / steps
     value = job_value(world, w.units, steps, total_ms)
-    kernel_ms = prod_ms / max(n_rec, 1)
-    achieved = flops / (kernel_ms * 1e-3) * 1e-12 if kernel_ms > 0 else 0.0
-    # end-to-end arm: host buffers through cheb_dm_compute_host
+    kernel_ms = prod_ms / max(n_rec, 1)  # product launches of one compute call (a whole batch when batched)
+    achieved = per_call * flops / (kernel_ms * 1e-3) * 1e-12 if kernel_ms > 0 else 0.0
+    tr_D = [float(x) for x in w.dtr.cpu().tolist()]
+    # mu-inclusive arm: cheb_dm_solve[_batch] (bounds, blocks, moments, bisection, assembly) + trace
+    mi_steps = max(3, min(steps, 10))
+    mi_ms = timed_steps(torch, w.step_mu_inclusive, mi_steps, max(1, min(warmup, 3)), flush, None, dist)
+    mi_ms = max_over_ranks(torch, dist, mi_ms) / mi_steps
+    plan.check(w.st)
+    tr_D_mi = [float(x) for x in w.dtr.cpu().tolist()]
+    # end-to-end arm: host buffers through the pipelined host entry point
     e2e_steps = max(3, min(steps, 10))
     e2e_ms = timed_steps(torch, w.step_host, e2e_steps, max(1, min(warmup, 3)), flush, None, dist)
     e2e_ms = max_over_ranks(torch, dist, e2e_ms)
+    traffic, traffic_src = ncu_traffic(name)
     res = {
         "workload": name, "N": w.N, "M_terms": w.M, "k": plan.k, "p": plan.p, "solves_per_step": w.units,
+        "batched": bool(w.batched and w.units > 1), "tile": plan.opts.tile, "giant_kernel": "resident" if (plan.opts.giant == 2 and per_call == 1) else "generic",
         "value": value, "ms_per_step": ms_per_step, "ms_per_solve": ms_per_step / w.units,
         "tflops_step": world * w.units * steps * flops / (total_ms * 1e-3) * 1e-12,
         "flops_per_solve": flops, "gpu_launches_per_step": w.launches_per_step,
         "roofline": {"bound": "tensor",
                      "kernel": ("gemm_dmma_kernel (persistent grouped FP64 DMMA GEMM: baby steps) + giant_resident_kernel (giant steps, "
-                                "multiplier resident in shared memory)") if plan.opts.giant == 2 else
-                               "gemm_dmma_kernel (persistent grouped FP64 DMMA GEMM, all products of one solve)",
+                                "multiplier resident in shared memory)") if (plan.opts.giant == 2 and per_call == 1) else
+                               "gemm_dmma_kernel (persistent grouped FP64 DMMA GEMM: baby-step launch + giant-step launch over the whole batch)",
                      "achieved": achieved, "peak": peak_tf, "unit": "TFLOP/s", "frac": achieved / peak_tf if peak_tf else None,
-                     "traffic": NCU_TRAFFIC_BYTES.get(name), "kernel_ms": kernel_ms, "launches_timed": n_rec,
-                     "kernel_share_of_step": (kernel_ms * w.units) / ms_per_step if ms_per_step > 0 else None,
-                     "flops_per_launch": flops,
+                     "traffic": traffic, "traffic_source": traffic_src, "kernel_ms": kernel_ms, "launches_timed": n_rec,
+                     "kernel_share_of_step": (kernel_ms * (w.units / per_call)) / ms_per_step if ms_per_step > 0 else None,
+                     "flops_per_launch": per_call * flops,
                      # context: what the same time would mean if every product were charged its full 2 N^3 flops
                      # (symmetric-tile skipping executes about half of them); not the roofline figure
-                     "full_product_equivalent_tflops": ((plan.k + plan.p - 2) * 2.0 * w.N ** 3) / (kernel_ms * 1e-3) * 1e-12 if kernel_ms > 0 else None},
+                     "full_product_equivalent_tflops": (per_call * (plan.k + plan.p - 2) * 2.0 * w.N ** 3) / (kernel_ms * 1e-3) * 1e-12 if kernel_ms > 0 else None},
         "e2e": {"value": world * w.units * e2e_steps / (e2e_ms * 1e-3), "unit": UNIT,
                 "h2d_bytes_per_step": w.h2d_bytes(), "d2h_bytes_per_step": w.d2h_bytes(), "steps": e2e_steps,
                 "ms_per_step": e2e_ms / e2e_steps},
-        "mu": w.mu, "mu_search_ms": w.mu_ms, "tr_D": [float(x) for x in w.dtr.cpu().tolist()], "N_occ": w.cfg.N_occ,
+        "mu_inclusive": {"call": "cheb_dm_solve_batch" if w.batched else "cheb_dm_solve", "ms_per_step": mi_ms, "ms_per_solve": mi_ms / w.units,
+                         "value": world * w.units / (mi_ms * 1e-3), "unit": UNIT, "vs_fixed_mu": mi_ms / ms_per_step if ms_per_step > 0 else None,
+                         "flops_per_solve": plan.flops_per_solve(), "tflops": w.units * plan.flops_per_solve() / (mi_ms * 1e-3) * 1e-12,
+                         "products": plan.k + 2 * plan.p - 4, "tr_D": tr_D_mi},
+        "mu": w.mu, "tr_D": tr_D, "N_occ": w.cfg.N_occ, "seeds": list(w.seeds),
         "workspace_bytes": plan.workspace_bytes(),
     }
     plan.destroy()
@@ -323,6 +371,49 @@ def oracle_rate(name, budget_s):
     sample = (f"{name} seed {cfg.seeds[0]} (N={cfg.N}, M={cfg.M}): oracle.dm_cheb, first {terms} of {cfg.M} terms "
               f"({terms - 2} of {cfg.M - 2} naive products, {t:.2f} s)" + ("" if full else ", extrapolated linearly in the number of products"))
     return 1.0 / t_solve, sample, oracle.num_threads(), terms
+
+
+def oracle_eig_rate(name, ref_sweep=None):
+    """solves/s of O-eig (cyclic Jacobi + Eq. 1-2) on this host.  N <= 1000: ONE sweep is timed and multiplied by the
+    sweeps a full run needs (counted on a 200 x 200 sample of the same kind); larger N: extrapolated from the
+    N = 1000 sweep by (N/1000)^3.  Labelled accordingly."""
+    import numpy as np
+    import oracle
+    import workloads
+    cfg = workloads.CONFIGS[name]
+    Hs = workloads.hamiltonian(name, seed=cfg.seeds[0], n=min(200, cfg.N))
+    sweeps = max(1, oracle.jacobi_sweeps(Hs, 60, 1e-14))  # sweeps to off(H) <= 1e-14 |H|_F on the sample
+    if cfg.N <= 1000:
+        H = workloads.hamiltonian(name, seed=cfg.seeds[0])
+        t0 = time.perf_counter()
+        oracle.jacobi_sweeps(H, 1, 1e-14)
+        t_sweep = time.perf_counter() - t0
+        how = f"one Jacobi sweep at N={cfg.N} timed ({t_sweep:.2f} s) x {sweeps} sweeps (count from a 200x200 sample of the same kind)"
+    else:
+        t_sweep = (ref_sweep or 0.0) * (cfg.N / 1000.0) ** 3
+        how = f"EXTRAPOLATED: one sweep at N=1000 ({ref_sweep:.2f} s) x (N/1000)^3 x {sweeps} sweeps"
+    t = t_sweep * sweeps
+    return (1.0 / t if t > 0 else None), how, t_sweep
+
+
+def cpu_baselines(names, budget_s):
+    """O-cheb (bounded sample, linear in the product count) and O-eig per workload, as SURVEY 8(d) specifies."""
+    out, ref_sweep = {}, None
+    for name in names:
+        try:
+            v, sample, cores, _ = oracle_rate(name, budget_s)
+            ent = {"o_cheb": {"value": v, "unit": UNIT, "cores": cores, "sample": sample}}
+            import workloads
+            if workloads.CONFIGS[name].N == 1000 or ref_sweep is None:
+                pass
+            ve, how, t_sweep = oracle_eig_rate(name, ref_sweep)
+            if workloads.CONFIGS[name].N == 1000:
+                ref_sweep = t_sweep
+            ent["o_eig"] = {"value": ve, "unit": UNIT, "cores": cores, "sample": how}
+            out[name] = ent
+        except Exception as e:  # pragma: no cover
+            out[name] = {"error": repr(e)}
+    return out
 
 
 def run_reference(args):
@@ -409,8 +500,9 @@ def main():
             "ms_per_step": main_res["ms_per_step"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f64", "data": "synthetic",
             "config": {"workload": f"{args.config}: {cfg.note}; beta={cfg.beta}, M={cfg.M} terms, N_occ={cfg.N_occ}, seeds {list(cfg.seeds)}; "
-                                   "mu solved on the trace beforehand (device moments + bisection)",
+                                   "mu solved on the trace beforehand by cheb_dm_solve_batch (device moments + bisection); the step's solves run as one batch (cheb_dm_compute_batch)",
                        "N": cfg.N, "M_terms": cfg.M, "k": main_res["k"], "p": main_res["p"], "solves_per_step": main_res["solves_per_step"],
+                       "batched": main_res["batched"], "tile": main_res["tile"], "giant_kernel": main_res["giant_kernel"],
                        "parallelism": "replicas only (one plan per GPU, no collective)" if world > 1 else "1 GPU",
                        "l2": "flushed between timed steps (512 MiB device memset outside the event brackets)",
                        "bounds": "Gershgorin on the device", "symmetric_tiles": bool(args.symmetric != 1),
@@ -424,12 +516,17 @@ def main():
                              frac_of_sustained=(main_res["roofline"]["achieved"] / peak_sustained) if peak_sustained else None,
                              peak_alt_bf16_ratio=(peaks.get("bf16_tflops") or 0) * 40.0 / 2250.0 or None),
             "clocks": clocks,
-            "mu": main_res["mu"], "tr_D": main_res["tr_D"], "mu_search_ms": main_res["mu_search_ms"],
+            "mu": main_res["mu"], "tr_D": main_res["tr_D"], "mu_inclusive": main_res["mu_inclusive"],
             "other_workloads": others,
         }
         if not args.no_cpu_baseline and world == 1:
-            v, sample, cores, _ = oracle_rate(args.config, 15.0)
+            v, sample, cores, _ = oracle_rate(args.config, 12.0)
             line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample}
+            # per workload: O-cheb and O-eig; N = 1000 first so that the larger sizes can extrapolate its sweep
+            names = [args.config] + [o["workload"] for o in others]
+            order = sorted(names, key=lambda n: (workloads.CONFIGS[n].N != 1000, workloads.CONFIGS[n].N))
+            per = cpu_baselines(order, 4.0)
+            line["cpu_baseline"]["per_workload"] = {n: per[n] for n in names}
         print(json.dumps(line))
     if dist is not None:
         dist.barrier()

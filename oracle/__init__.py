@@ -129,6 +129,16 @@ def jacobi_eig(H, max_sweeps=60, tol=1e-14):
     return E, Vt.T.copy()
 
 
+def jacobi_sweeps(H, max_sweeps=60, tol=1e-14) -> int:
+    """Runs co_jacobi_eig and returns its sweep count (-1: stopped at max_sweeps before off(H) <= tol |H|_F).
+    For timing the eigensolver (bench.py's cpu_baseline): max_sweeps = 1 times one sweep."""
+    H = _f64(H)
+    n = H.shape[0]
+    E = np.empty(n)
+    Vt = np.empty((n, n))
+    return int(_load().co_jacobi_eig(n, _p(H), _p(E), _p(Vt), max_sweeps, tol))
+
+
 def dm_from_eig(E, V, beta, mu):
     E = _f64(E)
     Vt = _f64(np.asarray(V).T)
