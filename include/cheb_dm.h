@@ -98,8 +98,11 @@ typedef struct {
     int sched;   /* cheb_dm_sched_t                                                              */
     int pairing; /* cheb_dm_pairing_t                                                            */
     int tile;    /* CTA tile (warp tile): 0 = auto, 1 = 128x128 (32x32), 2 = 128x64 (32x32), 3 = 64x64 (32x32),
-                    4 = 64x32 (16x16), 5 = 64x32 (32x16), 6 = 128x64 (32x16), 7 = 32x32 (16x16, 2 CTAs/SM), 8 = 112x64 (16x32).  auto picks among 1, 6, 8, 4 the
-                    shape with the fewest whole waves x tile area per product on this device             */
+                    4 = 64x32 (16x16), 5 = 64x32 (32x16), 6 = 128x64 (32x16), 7 = 32x32 (16x16, 2 CTAs/SM), 8 = 112x64 (16x32),
+                    9 = 64x64 (32x16), 10 = 64x32 (16x16, 2 CTAs/SM); 11 = 64x32 and 12 = 64x64 in the kernel with specialised
+                    epilogue warps (the consumer warps park a finished tile in shared memory and start the next item while
+                    four epilogue warps combine, store, mirror and publish it).  auto: 11 or 12 for N >= 450 (whichever needs
+                    fewer whole waves x tile area per product level on this device), 4 or 7 below               */
     int fuse_sums; /* low-order sums G_l / S_j of Eq. (21).  0 = auto; 1 = formed inside the
                       giant-step epilogues from T_1..T_{k-1} (no extra workspace; p(k-1) N^2 8 bytes of reads per
                       solve, L2 hits while the baby block fits L2); 2 = all p sums formed in one batched pass

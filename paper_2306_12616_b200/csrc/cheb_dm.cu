@@ -16,6 +16,7 @@
 #include "aux_kernels.cuh"
 #include "common.cuh"
 #include "gemm_dmma.cuh"
+#include "gemm_epi.cuh"
 #include "giant_resident.cuh"
 
 using namespace chebdm;
@@ -33,9 +34,13 @@ typedef GemmCfg<32, 32, 16, 16, 32, 6, 2> Cfg32x32;       //  4 consumer warps o
 typedef GemmCfg<64, 64, 32, 16, 32, 6, 1> Cfg64x64w16;    //  8 consumer warps of 32x16, 192 KB ring, 1 CTA/SM
 typedef GemmCfg<112, 64, 16, 32, 16, 6, 1> Cfg112x64;     // 14 consumer warps of 16x32, 132 KB ring, 1 CTA/SM (N ~ 1000: 144 tiles)
 typedef GemmCfg<64, 32, 16, 16, 32, 4, 2> Cfg64x32x2;     //  8 consumer warps of 16x16,  96 KB ring, 2 CTA/SM (batched small N)
+//                BM  BN  WM  WN  k-split BK stages      (gemm_epi.cuh: 8 consumer warps + 4 epilogue warps, 1 CTA/SM)
+typedef EpiCfg<64, 32, 32, 16, 2, 32, 7> CfgE64x32;       //  2 k-halves x (2 x 2 warps of 32x16), 168 KB ring + 40 KB staging tile
+typedef EpiCfg<64, 64, 32, 16, 1, 32, 5> CfgE64x64;       //  2 x 4 warps of 32x16, 160 KB ring + 36 KB staging tile
 
 enum TileSel { TILE_AUTO = 0, TILE_128x128 = 1, TILE_128x64 = 2, TILE_64x64 = 3, TILE_64x32_W16 = 4, TILE_64x32_W32 = 5,
-               TILE_128x64_W16 = 6, TILE_32x32 = 7, TILE_112x64 = 8, TILE_64x64_W16 = 9, TILE_64x32_X2 = 10, TILE_LAST = 10 };
+               TILE_128x64_W16 = 6, TILE_32x32 = 7, TILE_112x64 = 8, TILE_64x64_W16 = 9, TILE_64x32_X2 = 10, TILE_E64x32 = 11, TILE_E64x64 = 12,
+               TILE_LAST = 12 };
 
 struct TileShape {
     int BM, BN, BK, box_slabs;
@@ -57,6 +62,8 @@ TileShape tile_shape(int sel) {
         case TILE_64x64_W16: return shape_of<Cfg64x64w16>(0.76);
         case TILE_112x64: return shape_of<Cfg112x64>(0.72);  // 14 consumer warps: two sub-partitions carry 4, two carry 3
         case TILE_64x32_X2: return shape_of<Cfg64x32x2>(0.70);
+        case TILE_E64x32: return shape_of<CfgE64x32>(0.88);
+        case TILE_E64x64: return shape_of<CfgE64x64>(0.90);
         default: return shape_of<Cfg128x64w16>(0.80);
     }
 }
@@ -145,7 +152,7 @@ struct cheb_dm_plan_s {
     int pipe_ready;
     // optional per-tile timeline (cheb_dm_set_trace)
     TraceRec* trace_buf;
-    int trace_on, trace_res_base, trace_total;
+    int trace_on, trace_res_base, trace_total, trace_nb;  // trace_nb: matrices of the last traced launch
     // optional timing of the product launches (cheb_dm_set_timing)
     int timing;
     cudaEvent_t ev0[TIMING_SLOTS], ev1[TIMING_SLOTS];  // ring: compute number i uses slot i % TIMING_SLOTS
@@ -252,27 +259,53 @@ int sym_items(int N, int BM, int BN) {
     return n;
 }
 
+bool is_epi_tile(int sel) { return sel == TILE_E64x32 || sel == TILE_E64x64; }
+
 void choose_tile(cheb_dm_plan_s* P) {
     int sel = P->opt.tile;
     if (sel < TILE_AUTO || sel > TILE_LAST) sel = TILE_AUTO;
     if (sel == TILE_AUTO) {
-        // One product is the unit of the serial chain (giant steps), so pick the shape that minimises the time of
-        // one product level on this device: tiles per SM (whole waves, 1 CTA per SM) x tile area / main-loop efficiency.
-        // Large N -> 128x128 (least L2 traffic per flop); N ~ 1000 -> 128x64; N ~ 500 -> 64x32 (128 tiles).
-        // With symmetric-tile skipping only the lower-triangle tiles count (single solves at N <= 512: the giant steps
-        // run in the resident kernel and the tile shape only serves the throughput-bound baby phase: full count, as
-        // measured).  A batch plan counts the tiles of all max_batch matrices of a level (they are claimed together).
-        const int cand[5] = {TILE_128x128, TILE_128x64_W16, TILE_112x64, TILE_64x64_W16, TILE_64x32_W16};
-        double best = 0.0;
-        for (int c = 0; c < 5; ++c) {
-            const TileShape t = tile_shape(cand[c]);
-            const bool count_sym = P->sym && (P->N > 32 * GR_MAX_KTILES || P->maxb > 1);
-            if (cand[c] == TILE_64x64_W16 && !count_sym) continue;
-            const int tiles = (count_sym ? sym_items(P->N, t.BM, t.BN) : ceil_div(P->N, t.BM) * ceil_div(P->N, t.BN)) * P->maxb;
-            const double cost = (double)ceil_div(tiles, P->num_sms) * t.BM * t.BN / t.eff;
-            if (sel == TILE_AUTO || cost < best) {
-                sel = cand[c];
-                best = cost;
+        // One product level is the unit of the serial chain (giant steps), so pick the shape that minimises the time of a
+        // level on this device: whole waves of work items (all matrices of a batch are claimed together) x tile area /
+        // measured main-loop efficiency.  Measured on B200 (profiles/r02_ablations.md):
+        //  * the kernel with specialised epilogue warps (gemm_epi.cuh, 64x32 and 64x64 tiles) wins from N ~ 450 up to
+        //    N = 5000 (cfg3: 0.90 of the DMMA peak against 0.84 with 128x128 tiles of the generic kernel, whose 18 warps
+        //    leave 96 registers per thread): its consumers never wait for an epilogue;
+        //  * below that the K loop of an item is shorter than the epilogue warps' work on it: 64x32 tiles of the generic
+        //    kernel, or 32x32 tiles with 2 CTAs per SM when a batch level has enough items to fill them;
+        //  * single solves at N <= 512 run their giant steps in the resident kernel; the shape only serves the baby steps.
+        const bool single_small = (P->maxb == 1 && P->N <= 32 * GR_MAX_KTILES);
+        if (single_small) {
+            sel = (P->N >= 450) ? TILE_E64x32 : TILE_64x32_W16;
+        } else {
+            int cand[3], ncand = 0;
+            if (P->N >= 450) {
+                cand[ncand++] = TILE_E64x32;
+                cand[ncand++] = TILE_E64x64;
+                if (P->N >= 3000) cand[ncand++] = TILE_128x128;
+            } else {
+                cand[ncand++] = TILE_64x32_W16;
+                if (P->maxb > 1) cand[ncand++] = TILE_32x32;
+            }
+            // time of one product level in microseconds: whole waves x (K loop of an item at 250 GFLOP/s per SM / measured
+            // main-loop efficiency + what is not overlapped per item: 0.3 us with epilogue warps, ~3 us without), plus, when a
+            // level is a single wave, the epilogue -> publish -> poll -> TMA tail that no second wave hides
+            double best = 0.0;
+            for (int c = 0; c < ncand; ++c) {
+                const TileShape t = tile_shape(cand[c]);
+                const int per_sm = (cand[c] == TILE_32x32) ? 2 : 1;
+                const bool epi = is_epi_tile(cand[c]);
+                const long long tiles = (long long)(P->sym ? sym_items(P->N, t.BM, t.BN) : ceil_div(P->N, t.BM) * ceil_div(P->N, t.BN)) * P->maxb;
+                const long long waves = (tiles + (long long)P->num_sms * per_sm - 1) / ((long long)P->num_sms * per_sm);
+                double eff = t.eff;
+                if (cand[c] == TILE_E64x32 && P->N > 2500) eff -= 0.03;  // L2 -> SM operand traffic of the narrow tile
+                const double kloop = 2.0 * t.BM * t.BN * (double)P->N / 250e3 * per_sm / eff;
+                double cost = (double)waves * (kloop + (epi ? 0.3 : 3.0));
+                if (waves == 1) cost += epi ? 6.3 : 1.6;
+                if (c == 0 || cost < best) {
+                    sel = cand[c];
+                    best = cost;
+                }
             }
         }
     }
@@ -560,8 +593,16 @@ cheb_dm_status_t prepare_inst(int* per_sm) {
     CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(per_sm, gemm_dmma_kernel<Cfg>, Cfg::THREADS, Cfg::SMEM_BYTES));
     return *per_sm >= 1 ? CHEB_DM_OK : CHEB_DM_ECUDA;
 }
+template <class Cfg>
+cheb_dm_status_t prepare_epi(int* per_sm) {
+    CUDA_TRY(cudaFuncSetAttribute(gemm_epi_kernel<Cfg>, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg::SMEM_BYTES));
+    CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(per_sm, gemm_epi_kernel<Cfg>, Cfg::THREADS, Cfg::SMEM_BYTES));
+    return *per_sm >= 1 ? CHEB_DM_OK : CHEB_DM_ECUDA;
+}
 cheb_dm_status_t prepare_gemm(cheb_dm_plan_s* P) {
     switch (P->tile) {
+        case TILE_E64x32: return prepare_epi<CfgE64x32>(&P->gemm_per_sm);
+        case TILE_E64x64: return prepare_epi<CfgE64x64>(&P->gemm_per_sm);
         case TILE_128x128: return prepare_inst<Cfg128x128>(&P->gemm_per_sm);
         case TILE_128x64: return prepare_inst<Cfg128x64>(&P->gemm_per_sm);
         case TILE_64x64: return prepare_inst<Cfg64x64>(&P->gemm_per_sm);
@@ -578,6 +619,13 @@ cheb_dm_status_t prepare_gemm(cheb_dm_plan_s* P) {
 template <class Cfg>
 cheb_dm_status_t launch_inst(const LaunchArgs& la, int grid, cudaStream_t st) {
     gemm_dmma_kernel<Cfg><<<grid, Cfg::THREADS, Cfg::SMEM_BYTES, st>>>(la);
+    CUDA_TRY(cudaGetLastError());
+    return CHEB_DM_OK;
+}
+
+template <class Cfg>
+cheb_dm_status_t launch_epi(const LaunchArgs& la, int grid, cudaStream_t st) {
+    gemm_epi_kernel<Cfg><<<grid, Cfg::THREADS, Cfg::SMEM_BYTES, st>>>(la);
     CUDA_TRY(cudaGetLastError());
     return CHEB_DM_OK;
 }
@@ -607,13 +655,16 @@ cheb_dm_status_t launch_tasks(cheb_dm_plan_s* P, const TaskTable& tt, int lt0, i
     la.sym_first = P->sym_first;
     la.error_flag = P->counters;
     la.trace = P->trace_on ? P->trace_buf : nullptr;
-    la.trace_base = tt.trace_base + lt0 * tt.items_per_task;
+    la.trace_base = tt.trace_base + lt0 * tt.items_per_task * nb;  // a table's region holds ntl * maxb * items records
+    if (P->trace_on) P->trace_nb = nb;
     const long long items = (long long)(lt1 - lt0) * nb * tt.items_per_task;
     long long grid = (long long)P->gemm_per_sm * P->num_sms;
     if (grid > items) grid = items;
     if (grid < 1) grid = 1;
     ++P->last_launches;
     switch (P->tile) {
+        case TILE_E64x32: return launch_epi<CfgE64x32>(la, (int)grid, st);
+        case TILE_E64x64: return launch_epi<CfgE64x64>(la, (int)grid, st);
         case TILE_128x128: return launch_inst<Cfg128x128>(la, (int)grid, st);
         case TILE_128x64: return launch_inst<Cfg128x64>(la, (int)grid, st);
         case TILE_64x64: return launch_inst<Cfg64x64>(la, (int)grid, st);
@@ -1026,7 +1077,9 @@ cheb_dm_status_t cheb_dm_plan_ex(cheb_dm_plan_t* plan, int N, int M_terms, cheb_
     // L2-resident, pre-formed (form_sums_kernel: (ceil(p/16) (k-1) + p) mat bytes) once they do not.
     {
         int mode = o.fuse_sums;
-        if (mode == 0) mode = ((double)k * (double)P->mat_elems * 8.0 * P->maxb > 96.0 * 1024 * 1024 && k > 2 && p > 1) ? 2 : 1;
+        // (the epilogue warps of gemm_epi.cuh cannot gather k-1 tiles per item as fast as the consumers finish small-N
+        // items: with those tile shapes the sums are always pre-formed)
+        if (mode == 0) mode = (((double)k * (double)P->mat_elems * 8.0 * P->maxb > 96.0 * 1024 * 1024 || is_epi_tile(P->tile)) && k > 2 && p > 1) ? 2 : 1;
         P->preformed = (mode == 2) ? 1 : 0;
         P->opt.fuse_sums = mode;
     }
@@ -1062,7 +1115,7 @@ cheb_dm_status_t cheb_dm_plan_ex(cheb_dm_plan_t* plan, int N, int M_terms, cheb_
     P->pipe_ready = 0;
     P->n_async = 0;
     P->timing = 0; P->ev_count = 0;
-    P->trace_buf = nullptr; P->trace_on = 0;
+    P->trace_buf = nullptr; P->trace_on = 0; P->trace_nb = 1;
     for (int i = 0; i < TIMING_SLOTS; ++i) P->ev0[i] = P->ev1[i] = nullptr;
 
     const size_t kp = (size_t)k * p, B = (size_t)P->maxb;
@@ -1151,7 +1204,7 @@ cheb_dm_status_t cheb_dm_plan_ex(cheb_dm_plan_t* plan, int N, int M_terms, cheb_
             tt->ctr_panel_off = (int)off;
             off += tt->h.size() * (size_t)P->panel_stride;
             tt->trace_base = trace_off;
-            trace_off += tt->ntl * tt->items_per_task;  // timeline of single solves (slot 0)
+            trace_off += tt->ntl * tt->items_per_task * P->maxb;
         }
         P->trace_res_base = trace_off;
         P->trace_total = trace_off + P->p * P->res_tiles_m * P->res_tiles_n;
@@ -1581,16 +1634,19 @@ cheb_dm_status_t cheb_dm_get_trace(cheb_dm_plan_t P, cheb_dm_trace_rec_t* out, i
     static_assert(sizeof(cheb_dm_trace_rec_t) == sizeof(TraceRec), "trace record layout");
     CUDA_TRY(cudaDeviceSynchronize());
     int n = 0;
-    // single solve (slot 0): baby-step items, then the giant steps (generic kernel items or resident-kernel tiles)
-    const TaskTable* tabs[2] = {&P->baby, P->resident ? nullptr : &P->giant};
+    // baby-step items, then the giant steps (generic kernel items or resident-kernel tiles), of the nb matrices of the
+    // last traced call, in claim order (level by level, matrix by matrix)
+    const int tnb = P->trace_nb > 0 ? P->trace_nb : 1;
+    const bool res = P->resident && tnb == 1;
+    const TaskTable* tabs[2] = {&P->baby, res ? nullptr : &P->giant};
     for (int t = 0; t < 2; ++t) {
         if (!tabs[t]) continue;
-        int m = tabs[t]->ntl * tabs[t]->items_per_task;
+        int m = tabs[t]->ntl * tabs[t]->items_per_task * tnb;
         if (m > max_records - n) m = max_records - n;
         if (m > 0) CUDA_TRY(cudaMemcpy(out + n, P->trace_buf + tabs[t]->trace_base, sizeof(TraceRec) * (size_t)m, cudaMemcpyDeviceToHost));
         n += m > 0 ? m : 0;
     }
-    if (P->resident) {
+    if (res) {
         const int m = P->p * P->res_tiles_m * P->res_tiles_n;
         std::vector<TraceRec> tmp((size_t)m);
         CUDA_TRY(cudaMemcpy(tmp.data(), P->trace_buf + P->trace_res_base, sizeof(TraceRec) * (size_t)m, cudaMemcpyDeviceToHost));

@@ -403,7 +403,8 @@ __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MIN_CTAS) gemm_dmma_kernel(
         // the serial chain.  It is kept in registers of its own and added in the epilogue: starting the accumulator
         // from it would make every DMMA rounding relative to the (large) sum instead of the (small) running product
         // and measurably costs accuracy (cfg4: |dtr D| 7e-10 -> 3e-9).  Large warp tiles form it in the epilogue.
-        constexpr bool PRE_SUM = (FM * FN <= 4);
+        constexpr bool PRE_SUM = (FM * FN <= 4) || (FM * FN <= 8 && Cfg::THREADS <= 320);  // 18-warp CTAs have 96 registers per thread
+        constexpr int PRE_U = (FM * FN <= 4) ? 4 : 2;  // operands in flight per iteration (register budget)
         double pre[PRE_SUM ? FM : 1][PRE_SUM ? FN : 1][2];
 #pragma unroll
         for (int i = 0; i < (PRE_SUM ? FM : 1); ++i)
@@ -415,11 +416,11 @@ __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MIN_CTAS) gemm_dmma_kernel(
             const long long lds = tk->lds, sstride = tk->sum_stride;
             const double* sb = tk->sum_base + (long long)row0 * lds + col0;
             int s = 0;
-            for (; s + 3 < ns; s += 4) {  // four operands in flight per iteration
-                double w[4];
-                double2 v[4][PRE_SUM ? FM : 1][PRE_SUM ? FN : 1];
+            for (; s + PRE_U - 1 < ns; s += PRE_U) {  // PRE_U operands in flight per iteration
+                double w[PRE_U];
+                double2 v[PRE_U][PRE_SUM ? FM : 1][PRE_SUM ? FN : 1];
 #pragma unroll
-                for (int u = 0; u < 4; ++u) {
+                for (int u = 0; u < PRE_U; ++u) {
                     w[u] = __ldg(coef + s + u);
                     const double* pu = sb + (long long)(s + u) * sstride;
 #pragma unroll
@@ -431,7 +432,7 @@ __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MIN_CTAS) gemm_dmma_kernel(
                         }
                 }
 #pragma unroll
-                for (int u = 0; u < 4; ++u)
+                for (int u = 0; u < PRE_U; ++u)
 #pragma unroll
                     for (int i = 0; i < (PRE_SUM ? FM : 1); ++i)
 #pragma unroll

@@ -60,7 +60,7 @@ def test_batch_cfg1_four_seeds_full_size_full_matrix():
     plan.destroy()
 
 
-@pytest.mark.parametrize("tile", [0, 3, 4, 5, 7, 9, 10])
+@pytest.mark.parametrize("tile", [0, 3, 4, 5, 7, 9, 10, 11, 12])
 def test_batch_ragged_n257_three_of_four_slots(tile):
     """nbatch < max_batch, odd N (ragged tiles, padded leading dimension), a different mu per matrix."""
     oracle, cd, workloads, gu, oc = _imports()

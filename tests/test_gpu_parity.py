@@ -27,7 +27,7 @@ def _imports():
 # ----------------------------------------------------------------------------------------------
 # a-4/a-6 kernel: one product with the fused 2AB - C epilogue (Eq. 7), all tile shapes, ragged sizes
 # ----------------------------------------------------------------------------------------------
-@pytest.mark.parametrize("tile", [1, 2, 3, 4, 5, 6, 7, 8])
+@pytest.mark.parametrize("tile", [1, 2, 3, 4, 5, 6, 7, 8, 9, 10, 11, 12])
 @pytest.mark.parametrize("N", [1, 2, 7, 64, 65, 130, 200, 333])
 def test_product_2AB_minus_C(N, tile):
     oracle, cd, workloads, gu, _ = _imports()
@@ -154,7 +154,7 @@ def test_parity_reduced_size_device_gershgorin(cfg, seed, n, M):
     _check(case, r)
 
 
-@pytest.mark.parametrize("tile", [1, 2, 3, 4, 5, 6, 7, 8])
+@pytest.mark.parametrize("tile", [1, 2, 3, 4, 5, 6, 7, 8, 9, 10, 11, 12])
 @pytest.mark.parametrize("sched", [0, 1])
 def test_parity_tiles_and_schedulers(tile, sched):
     oracle, cd, workloads, gu, oc = _imports()
@@ -191,7 +191,7 @@ def test_parity_fused_and_preformed_sums(fuse, outer):
     _check(case, r)
 
 
-@pytest.mark.parametrize("tile,n", [(4, 700), (5, 700), (6, 1500), (7, 700), (3, 700), (1, 1500), (8, 1500)])
+@pytest.mark.parametrize("tile,n", [(4, 700), (5, 700), (6, 1500), (7, 700), (3, 700), (1, 1500), (8, 1500), (11, 700), (12, 700), (11, 257), (12, 129)])
 def test_grouped_equals_serial_bitwise_many_tiles_per_task(tile, n):
     """a-8: with more tiles per product than resident CTAs every CTA streams several tiles back to back and the
     producer runs ahead of the consumers; the grouped schedule must reproduce the serial one bit for bit (fixed
@@ -558,7 +558,7 @@ def test_trace_records_and_resolved_options():
         plan.destroy()
 
 
-@pytest.mark.parametrize("tile,n", [(0, 300), (0, 257), (1, 700), (6, 333), (8, 500), (9, 641), (3, 200), (7, 129)])
+@pytest.mark.parametrize("tile,n", [(0, 300), (0, 257), (1, 700), (6, 333), (8, 500), (9, 641), (3, 200), (7, 129), (11, 300), (11, 257), (12, 641), (12, 129)])
 def test_symmetric_tile_skipping(tile, n):
     """Section 8(f)-3: only the tiles touching the lower triangle are computed, the rest is mirrored.  Same D as the full
     computation up to rounding, symmetric, parity with the oracle unchanged."""
