@@ -129,7 +129,9 @@ typedef struct {
     int host_slots; /* staging sets of the host entry points allocated at plan time: 0 = none (the first host call
                       allocates what it needs -- the one exception to "compute calls allocate nothing"), 1 = one
                       (cheb_dm_compute_host), 2 = both + copy streams/events (cheb_dm_compute_host_async).         */
-    int reserved[2];
+    int sliced;     /* digits S of cheb_dm_product_sliced: 0 = off, 2..8: the plan allocates the int8 digit
+                      planes of two operands (2 S N kpad bytes, kpad = N rounded up to 64) and their scale vectors.        */
+    int reserved[1];
 } cheb_dm_options_t;
 
 /* Create a plan for N x N matrices and an M_terms-term expansion.  Chooses (k,p), allocates the
@@ -278,6 +280,17 @@ cheb_dm_status_t cheb_dm_assemble(cheb_dm_plan_t plan, int nbatch, const double*
  * for the symmetric operands of this method).  C may be NULL (beta ignored).  Out may alias C. */
 cheb_dm_status_t cheb_dm_product(cheb_dm_plan_t plan, double alpha, const double* dA, const double* dB,
                                  double beta, const double* dC, double* dOut, void* cuda_stream);
+
+/* The same product on the Blackwell tensor path proper: sm_100a has no FP64 tcgen05 MMA, so the
+ * FP64 operands are sliced error-free into S int8 digits per element (row-wise power-of-two scales), the S (S+1)/2
+ * leading digit products run on tcgen05.mma kind::i8 with int32 accumulators in tensor memory, and the result is
+ * recombined in FP64:  Out = alpha * A B + beta * C  with  |error_ij| <= K (S+1) 2^{-7S} max_k|a_ik| max_k|b_kj| 4
+ * plus FP64 rounding of the recombination; S = 8 (36 int8 products) is below the rounding error of an FP64 dot
+ * product.  A, B symmetric N x N device matrices (ld N; B may equal A), C nullable (ld N), Out must not alias A or B.
+ * Stand-alone call (kernel-level tests and benchmark against the DMMA product); the solve does not use it.
+ * EUNSUPPORTED unless the plan was made with the option sliced = S. */
+cheb_dm_status_t cheb_dm_product_sliced(cheb_dm_plan_t plan, double alpha, const double* dA, const double* dB,
+                                        double beta, const double* dC, double* dOut, void* cuda_stream);
 
 /* Synchronises `cuda_stream` and reports what the device flagged since the last check (the flags are sticky, so one
  * check after a pipeline of computes sees an error of any of them; the check clears them): CHEB_DM_ECUDA if a CUDA

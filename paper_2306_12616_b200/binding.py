@@ -23,6 +23,7 @@ EXPORTS = [
     "cheb_dm_compute_host_async", "cheb_dm_wait",
     "cheb_dm_compute_batch", "cheb_dm_compute_batch_host", "cheb_dm_compute_batch_host_async", "cheb_dm_trace_batch",
     "cheb_dm_get_scalars", "cheb_dm_solve", "cheb_dm_solve_batch", "cheb_dm_assemble", "cheb_dm_flops_per_solve",
+    "cheb_dm_product_sliced",
 ]
 
 
@@ -36,7 +37,7 @@ class Options(C.Structure):
     _fields_ = [("k", C.c_int), ("p", C.c_int), ("outer", C.c_int), ("sched", C.c_int),
                 ("pairing", C.c_int), ("tile", C.c_int), ("fuse_sums", C.c_int),
                 ("giant", C.c_int), ("symmetric", C.c_int), ("max_batch", C.c_int), ("ldh", C.c_int), ("ldd", C.c_int),
-                ("moments", C.c_int), ("host_slots", C.c_int), ("reserved", C.c_int * 2)]
+                ("moments", C.c_int), ("host_slots", C.c_int), ("sliced", C.c_int), ("reserved", C.c_int * 1)]
 
 
 class ChebDMError(RuntimeError):
@@ -104,6 +105,7 @@ def lib():
     L.cheb_dm_solve_batch.argtypes = [vp, C.c_int, pp, dp, C.c_int, pp, dp, vp]
     L.cheb_dm_assemble.argtypes = [vp, C.c_int, dp, pp, vp]
     L.cheb_dm_flops_per_solve.argtypes = [vp, dp]
+    L.cheb_dm_product_sliced.argtypes = [vp, C.c_double, vp, vp, C.c_double, vp, vp, vp]
     for n in EXPORTS:
         getattr(L, n).restype = C.c_int
     L.cheb_dm_strerror.argtypes = [C.c_int]
@@ -149,11 +151,11 @@ class Plan:
     def __init__(self, N: int, M: int, *, k: int = 0, p: int = 0, outer: int = OUTER_CHEBYSHEV,
                  sched: int = SCHED_GROUPED, pairing: int = PAIR_AUTO, tile: int = TILE_AUTO,
                  fuse_sums: int = 0, giant: int = 0, symmetric: int = 0, max_batch: int = 0, ldh: int = 0, ldd: int = 0,
-                 moments: int = 0, host_slots: int = 0, dtype: int = 0):
+                 moments: int = 0, host_slots: int = 0, sliced: int = 0, dtype: int = 0):
         self._h = C.c_void_p()
         self.N, self.M = N, M
         o = Options(k=k, p=p, outer=outer, sched=sched, pairing=pairing, tile=tile, fuse_sums=fuse_sums, giant=giant, symmetric=symmetric,
-                    max_batch=max_batch, ldh=ldh, ldd=ldd, moments=moments, host_slots=host_slots)
+                    max_batch=max_batch, ldh=ldh, ldd=ldd, moments=moments, host_slots=host_slots, sliced=sliced)
         _chk(lib().cheb_dm_plan_ex(C.byref(self._h), N, M, dtype, C.byref(o)), "cheb_dm_plan_ex")
         kk, pp = C.c_int(), C.c_int()
         _chk(lib().cheb_dm_get_kp(self._h, C.byref(kk), C.byref(pp)), "cheb_dm_get_kp")
@@ -298,6 +300,9 @@ class Plan:
 
     def product(self, alpha: float, dA: int, dB: int, beta: float, dC, d_out: int, stream: int = 0):
         _chk(lib().cheb_dm_product(self._h, alpha, dA, dB, beta, dC, d_out, stream), "cheb_dm_product")
+
+    def product_sliced(self, alpha: float, dA: int, dB: int, beta: float, dC, d_out: int, stream: int = 0):
+        _chk(lib().cheb_dm_product_sliced(self._h, alpha, dA, dB, beta, dC, d_out, stream), "cheb_dm_product_sliced")
 
     def workspace_bytes(self) -> int:
         v = C.c_size_t()

@@ -8,7 +8,7 @@ import subprocess
 _HERE = os.path.dirname(os.path.abspath(__file__))
 SRC = os.path.join(_HERE, "csrc", "cheb_dm.cu")
 LIB_PATH = os.path.join(_HERE, "libcheb_dm.so")
-_DEPS = [os.path.join(_HERE, "csrc", f) for f in ("cheb_dm.cu", "common.cuh", "gemm_dmma.cuh", "giant_resident.cuh", "aux_kernels.cuh")]
+_DEPS = [os.path.join(_HERE, "csrc", f) for f in ("cheb_dm.cu", "common.cuh", "gemm_dmma.cuh", "gemm_epi.cuh", "giant_resident.cuh", "aux_kernels.cuh", "ozaki.cuh")]
 _DEPS.append(os.path.join(os.path.dirname(_HERE), "include", "cheb_dm.h"))
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",

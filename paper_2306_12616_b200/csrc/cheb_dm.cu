@@ -18,6 +18,7 @@
 #include "gemm_dmma.cuh"
 #include "gemm_epi.cuh"
 #include "giant_resident.cuh"
+#include "ozaki.cuh"
 
 using namespace chebdm;
 
@@ -150,6 +151,12 @@ struct cheb_dm_plan_s {
     cudaEvent_t ev_in[2], ev_comp[2], ev_out[2];
     long long n_async;
     int pipe_ready;
+    // digit planes of cheb_dm_product_sliced (option sliced = S): [operand][digit][N][oz_kpad] int8, scales [operand][N]
+    int oz_S;
+    long long oz_kpad;
+    int8_t* oz_digits;
+    double* oz_scale;
+    CUtensorMap oz_map[2][2];  // [operand][0: 128-row boxes (left factor), 1: 64-row boxes (right factor)]
     // optional per-tile timeline (cheb_dm_set_trace)
     TraceRec* trace_buf;
     int trace_on, trace_res_base, trace_total, trace_nb;  // trace_nb: matrices of the last traced launch
@@ -926,6 +933,33 @@ bool batch_args_ok(const cheb_dm_plan_s* P, int nb, const double* const* A, doub
     return true;
 }
 
+// Digit planes, scales and TMA descriptors of cheb_dm_product_sliced.
+cheb_dm_status_t prepare_sliced(cheb_dm_plan_s* P) {
+    const size_t plane = (size_t)P->N * (size_t)P->oz_kpad;
+    const size_t bytes = 2 * (size_t)P->oz_S * plane;
+    if (cudaMalloc(&P->oz_digits, bytes) != cudaSuccess || cudaMalloc(&P->oz_scale, sizeof(double) * 2 * P->N) != cudaSuccess) {
+        cudaGetLastError();
+        return CHEB_DM_EALLOC;
+    }
+    P->ws_bytes += bytes + sizeof(double) * 2 * P->N;
+    EncodeTiledFn enc = get_encode_fn();
+    if (!enc) return CHEB_DM_ECUDA;
+    for (int op = 0; op < 2; ++op)
+        for (int role = 0; role < 2; ++role) {
+            // {k (bytes), row, digit}: a box is one k-block of 64 int8 x 128 (or 64) rows of one digit plane, 64-byte swizzle
+            cuuint64_t dims[3] = {(cuuint64_t)P->oz_kpad, (cuuint64_t)P->N, (cuuint64_t)P->oz_S};
+            cuuint64_t strides[2] = {(cuuint64_t)P->oz_kpad, (cuuint64_t)plane};
+            cuuint32_t box[3] = {(cuuint32_t)OZ_BK, (cuuint32_t)(role == 0 ? OZ_BM : OZ_BN), 1};
+            cuuint32_t estr[3] = {1, 1, 1};
+            CUresult r = enc(&P->oz_map[op][role], CU_TENSOR_MAP_DATA_TYPE_UINT8, 3, P->oz_digits + (size_t)op * P->oz_S * plane, dims, strides, box,
+                             estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_64B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                             CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+            if (r != CUDA_SUCCESS) return CHEB_DM_ECUDA;
+        }
+    CUDA_TRY(cudaFuncSetAttribute(oz_gemm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, oz_smem_bytes()));
+    return CHEB_DM_OK;
+}
+
 }  // namespace
 
 // =====================================================================================================
@@ -986,6 +1020,8 @@ cheb_dm_status_t cheb_dm_destroy(cheb_dm_plan_t P) {
             cudaEventDestroy(P->ev_out[i]);
         }
     }
+    cudaFree(P->oz_digits);
+    cudaFree(P->oz_scale);
     cudaFree(P->trace_buf);
     for (int i = 0; i < TIMING_SLOTS; ++i) {
         if (P->ev0[i]) cudaEventDestroy(P->ev0[i]);
@@ -1012,6 +1048,7 @@ cheb_dm_status_t cheb_dm_plan_ex(cheb_dm_plan_t* plan, int N, int M_terms, cheb_
     if (o.max_batch < 0 || o.max_batch > MAX_BATCH) return CHEB_DM_EINVAL;
     if ((o.ldh != 0 && o.ldh < N) || (o.ldd != 0 && o.ldd < N)) return CHEB_DM_EINVAL;
     if (o.moments < 0 || o.moments > 2 || o.host_slots < 0 || o.host_slots > 2) return CHEB_DM_EINVAL;
+    if (o.sliced != 0 && (o.sliced < 2 || o.sliced > OZ_MAX_S || N > 65535)) return CHEB_DM_EINVAL;
     int k = o.k, p = o.p;
     if (k == 0 && p == 0) {
         k = 1;
@@ -1116,6 +1153,7 @@ cheb_dm_status_t cheb_dm_plan_ex(cheb_dm_plan_t* plan, int N, int M_terms, cheb_
     P->n_async = 0;
     P->timing = 0; P->ev_count = 0;
     P->trace_buf = nullptr; P->trace_on = 0; P->trace_nb = 1;
+    P->oz_S = o.sliced; P->oz_kpad = ((long long)N + OZ_BK - 1) / OZ_BK * OZ_BK; P->oz_digits = nullptr; P->oz_scale = nullptr;
     for (int i = 0; i < TIMING_SLOTS; ++i) P->ev0[i] = P->ev1[i] = nullptr;
 
     const size_t kp = (size_t)k * p, B = (size_t)P->maxb;
@@ -1220,6 +1258,10 @@ cheb_dm_status_t cheb_dm_plan_ex(cheb_dm_plan_t* plan, int N, int M_terms, cheb_
         if (st != CHEB_DM_OK) break;
         if (o.host_slots > 0) {
             st = ensure_staging(P, o.host_slots);
+            if (st != CHEB_DM_OK) break;
+        }
+        if (P->oz_S > 0) {
+            st = prepare_sliced(P);
             if (st != CHEB_DM_OK) break;
         }
         if (cudaDeviceSynchronize() != cudaSuccess) { st = CHEB_DM_ECUDA; break; }
@@ -1608,6 +1650,41 @@ cheb_dm_status_t cheb_dm_product(cheb_dm_plan_t P, double alpha, const double* d
     P->work_next = wsave;
     // the pageable-source copy above is staged by the runtime before it returns, so `t` may go out of scope
     return s;
+}
+
+cheb_dm_status_t cheb_dm_product_sliced(cheb_dm_plan_t P, double alpha, const double* dA, const double* dB, double beta,
+                                        const double* dC, double* dOut, void* cuda_stream) {
+    if (!P || !dA || !dB || !dOut) return CHEB_DM_EINVAL;
+    if (dOut == dA || dOut == dB) return CHEB_DM_EINVAL;
+    if (P->oz_S < 2) return CHEB_DM_EUNSUPPORTED;
+    if (!device_ok(P)) return CHEB_DM_ECUDA;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const int N = P->N, S = P->oz_S;
+    const size_t plane = (size_t)N * (size_t)P->oz_kpad;
+    const int same = (dA == dB) ? 1 : 0;
+    const int split_blocks = ceil_div(N * 32, 256);
+    oz_split_kernel<<<split_blocks, 256, 0, st>>>(dA, N, N, S, P->oz_digits, P->oz_kpad, P->oz_scale);
+    if (!same) oz_split_kernel<<<split_blocks, 256, 0, st>>>(dB, N, N, S, P->oz_digits + (size_t)S * plane, P->oz_kpad, P->oz_scale + N);
+    OzArgs oa;
+    memset(&oa, 0, sizeof(oa));
+    oa.N = N;
+    oa.S = S;
+    oa.kblocks = (int)(P->oz_kpad / OZ_BK);
+    oa.tiles_m = ceil_div(N, OZ_BM);
+    oa.tiles_n = ceil_div(N, OZ_BN);
+    oa.scaleA = P->oz_scale;
+    oa.scaleB = P->oz_scale + (same ? 0 : N);
+    oa.alpha = alpha;
+    oa.beta = dC ? beta : 0.0;
+    oa.C = dC;
+    oa.ldc = N;
+    oa.Out = dOut;
+    oa.ldo = N;
+    int grid = oa.tiles_m * oa.tiles_n;
+    if (grid > P->num_sms) grid = P->num_sms;
+    oz_gemm_kernel<<<grid, OZ_THREADS, oz_smem_bytes(), st>>>(P->oz_map[0][0], P->oz_map[same ? 0 : 1][1], oa);
+    CUDA_TRY(cudaGetLastError());
+    return CHEB_DM_OK;
 }
 
 // ------------------------------------------------------------------------------------------------------

@@ -1,0 +1,276 @@
+// ozaki.cuh -- FP64-accurate product of two symmetric matrices on the Blackwell tensor path proper
+// (SURVEY 8(f)-4): error-free slicing of the FP64 operands into int8 digits, the digit products on
+// tcgen05.mma kind::i8 (SASS UTCIMMA) with int32 accumulators in tensor memory, recombination in FP64.
+// sm_100a has no tcgen05 kind::f64 (the products of the solve run on DMMA.8x8x4, gemm_dmma.cuh); this is the
+// only route past the DMMA issue rate for the products  T_{a+b} = 2 T_a T_b - T_|a-b|  (Eq. 7) and
+// the Horner steps of Eq. (4).  Stand-alone product (cheb_dm_product_sliced); not wired into
+// the solve.  Product code; shares nothing with oracle/.
+//
+// Slicing (per row i of a symmetric operand; the row of B^T = B is the column of B):
+//     a_ik = 2^{e_i} ( sum_{s<S} q_s[i][k] 2^{-6-7s} + rho ),   q_s in [-64, 64] (int8),  |rho| <= 2^{-7S},
+// with 2^{e_i} > max_k |a_ik|:  t_0 = a 2^{6-e},  q_s = rint(t_s),  t_{s+1} = (t_s - q_s) 2^7  -- every step exact.
+// Product:  (A B)_ij = 2^{e_i+f_j-12} sum_{d} 2^{-7d} P_d[i][j] + O(K 2^{e_i+f_j-7S}),
+//     P_d = sum_{s+t=d} sum_k q^A_s[i][k] q^B_t[j][k]      exactly in int32:  |P_d| <= (d+1) K 64^2 < 2^31 for K <= 65535,
+// keeping d < S (the dropped digit products are below the slicing error).  S(S+1)/2 int8 products: 36 for S = 8,
+// for which the error bound K (S+1) 2^{-7S} 2^{e_i+f_j} is below the rounding error of an FP64 dot product.
+//
+// Kernel: one CTA per 128 x 64 output tile (persistent, static tile order), cta_group::1.  ALL S accumulators
+// P_0..P_{S-1} live in tensor memory at once (S x 64 columns <= 512), so every digit tile is fetched once per k-block
+// and used by up to S MMAs: S(S+1)/2 MMA blocks per 2S tile loads (a plain int8 GEMM loads 2 per block and is
+// L2-bound on this part).  k-block = 64 int8 (64-byte swizzle rows), stage = S A-tiles (128 x 64 B) + S B-tiles
+// (64 x 64 B), two stages.  Warp 0: TMA producer, warp 1: MMA issuer (one lane), warp 2: TMEM allocator, warps 4-7:
+// epilogue (tcgen05.ld of the S accumulators, Horner recombination in FP64, scaling, alpha/beta, store).
+#pragma once
+#include "common.cuh"
+
+namespace chebdm {
+
+constexpr int OZ_MAX_S = 8;
+constexpr int OZ_BM = 128, OZ_BN = 64, OZ_BK = 64;          // output tile, k-block in int8 elements (= bytes)
+constexpr int OZ_A_TILE = OZ_BM * OZ_BK, OZ_B_TILE = OZ_BN * OZ_BK;   // 8 KB, 4 KB
+constexpr int OZ_STAGES = 2;
+constexpr int OZ_THREADS = 256;
+constexpr int OZ_BAND = 16;                                  // column tiles per raster band (L2 reuse of the digit strips)
+
+// ---- tcgen05 wrappers ----
+__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_alloc512(uint32_t smem_slot) {
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 512;" ::"r"(smem_slot) : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+}
+__device__ __forceinline__ void tc_dealloc512(uint32_t taddr) {
+    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 512;" ::"r"(taddr) : "memory");
+}
+// D[tmem] (+)= A[smem] * B[smem]^T, int8 x int8 -> int32, M = 128, N = 64, K = 32 per instruction
+__device__ __forceinline__ void tc_mma_i8(uint32_t d_tmem, uint64_t adesc, uint64_t bdesc, uint32_t idesc, uint32_t accumulate) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+        "tcgen05.mma.cta_group::1.kind::i8 [%0], %1, %2, %3, p;\n\t}"
+        ::"r"(d_tmem), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate)
+        : "memory");
+}
+// arrive on an mbarrier when every MMA issued so far by this thread has completed (implies fence::before_thread_sync)
+__device__ __forceinline__ void tc_commit(uint32_t bar) {
+    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void tc_ld8(uint32_t taddr, int (&v)[8]) {
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+                 : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7])
+                 : "r"(taddr)
+                 : "memory");
+}
+__device__ __forceinline__ void tc_wait_ld() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
+
+// Shared-memory matrix descriptor, K-major operand tile of 64-byte rows with the 64-byte swizzle: 8-row groups are
+// 512 bytes apart (stride byte offset), the leading byte offset is unused for swizzled K-major tiles, descriptor
+// version 1 (sm_100), layout type 4 = SWIZZLE_64B.  Advancing by one K = 32 instruction adds 32 bytes to the start.
+__device__ __forceinline__ uint64_t oz_smem_desc(uint32_t saddr) {
+    uint64_t d = 0;
+    d |= (uint64_t)((saddr & 0x3FFFFu) >> 4);      // [0,14)  start address >> 4
+    d |= (uint64_t)1 << 16;                         // [16,30) leading byte offset >> 4 (ignored)
+    d |= (uint64_t)(512 >> 4) << 32;                // [32,46) stride byte offset >> 4
+    d |= (uint64_t)1 << 46;                         // [46,48) descriptor version
+    d |= (uint64_t)4 << 61;                         // [61,64) swizzle mode: 64 B
+    return d;
+}
+// Instruction descriptor of kind::i8: D = S32 (2 at [4,6)), A and B signed int8 (1 at [7,10), [10,13)), both K-major,
+// N >> 3 at [17,23), M >> 4 at [24,29), dense, no saturation.
+__host__ __device__ constexpr uint32_t oz_idesc() {
+    return (2u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(OZ_BN >> 3) << 17) | ((uint32_t)(OZ_BM >> 4) << 24);
+}
+
+// ---------------------------------------------------------------------------------------------------
+// Slicing: one warp per row.  digits[s][row][k] (int8, row pitch kpad, zero beyond N), scale[row] = 2^{e_row}.
+// ---------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) oz_split_kernel(const double* __restrict__ A, long long lda, int N, int S, int8_t* __restrict__ digits,
+                                                       long long kpad, double* __restrict__ scale) {
+    const int warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
+    if (warp >= N) return;
+    const double* row = A + (long long)warp * lda;
+    double m = 0.0;
+    for (int k = lane; k < N; k += 32) m = fmax(m, fabs(row[k]));
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) m = fmax(m, __shfl_xor_sync(0xffffffffu, m, o));
+    int e = 0;
+    if (m > 0.0 && isfinite(m)) {
+        (void)frexp(m, &e);                 // m = f 2^e, f in [0.5, 1)  =>  |a| 2^-e < 1
+    }
+    if (lane == 0) scale[warp] = ldexp(1.0, e);
+    const long long plane = (long long)N * kpad;
+    for (long long k = lane; k < kpad; k += 32) {
+        double t = (k < N) ? ldexp(row[k], 6 - e) : 0.0;   // |t| < 64
+        int8_t* dst = digits + (long long)warp * kpad + k;
+        for (int s = 0; s < S; ++s) {
+            const double q = rint(t);
+            dst[(long long)s * plane] = (int8_t)(int)q;
+            t = (t - q) * 128.0;                            // exact: |t - q| <= 1/2
+        }
+    }
+}
+
+struct OzArgs {
+    int N, S;
+    int kblocks;                 // kpad / OZ_BK
+    int tiles_m, tiles_n;
+    const double* scaleA;        // [N] 2^{e_i}
+    const double* scaleB;        // [N] 2^{f_j}
+    double alpha, beta;
+    const double* C;             // nullable, leading dimension ldc
+    long long ldc;
+    double* Out;
+    long long ldo;
+};
+
+__device__ __forceinline__ void oz_tile_of(int t, int tiles_m, int tiles_n, int& tm, int& tn) {
+    // column bands of OZ_BAND tiles, row-major inside a band: the CTAs of a wave share few A and B strips
+    const int band_tiles = tiles_m * OZ_BAND;
+    const int band = t / band_tiles;
+    const int r = t - band * band_tiles;
+    const int width = min(OZ_BAND, tiles_n - band * OZ_BAND);
+    tm = r / width;
+    tn = band * OZ_BAND + (r - tm * width);
+}
+
+__global__ void __launch_bounds__(OZ_THREADS, 1) oz_gemm_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUtensorMap mapB,
+                                                                const OzArgs args) {
+    extern __shared__ uint8_t smem_raw[];
+    uint8_t* smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
+    const int S = args.S;
+    const uint32_t stage_bytes = (uint32_t)S * (OZ_A_TILE + OZ_B_TILE);
+    const uint32_t ring_bytes = OZ_STAGES * OZ_MAX_S * (OZ_A_TILE + OZ_B_TILE);
+    uint64_t* bars = reinterpret_cast<uint64_t*>(smem + ring_bytes);
+    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(smem + ring_bytes + 64);
+    const uint32_t smem_base = smem_u32(smem);
+    const uint32_t bar_base = smem_u32(bars);
+    auto full_bar = [&](int s) { return bar_base + 8u * s; };
+    auto empty_bar = [&](int s) { return bar_base + 8u * (OZ_STAGES + s); };
+    const uint32_t tfull_bar = bar_base + 8u * (2 * OZ_STAGES);
+    const uint32_t tempty_bar = tfull_bar + 8u;
+    auto a_tile = [&](int stage, int s) { return smem_base + (uint32_t)stage * (OZ_MAX_S * (OZ_A_TILE + OZ_B_TILE)) + (uint32_t)s * OZ_A_TILE; };
+    auto b_tile = [&](int stage, int t) { return smem_base + (uint32_t)stage * (OZ_MAX_S * (OZ_A_TILE + OZ_B_TILE)) + OZ_MAX_S * OZ_A_TILE + (uint32_t)t * OZ_B_TILE; };
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < OZ_STAGES; ++s) {
+            mbar_init(full_bar(s), 1);
+            mbar_init(empty_bar(s), 1);
+        }
+        mbar_init(tfull_bar, 1);
+        mbar_init(tempty_bar, 4);   // the four epilogue warps
+        fence_mbar_init();
+    }
+    if (warp == 2) tc_alloc512(smem_u32(tmem_slot));
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem_base = *tmem_slot;
+
+    const int ntiles = args.tiles_m * args.tiles_n;
+    const int kblocks = args.kblocks;
+
+    if (warp == 0) {
+        // =================================== TMA producer ===================================
+        if (lane == 0) {
+            int stage = 0;
+            uint32_t phase = 0;
+            for (int t = blockIdx.x; t < ntiles; t += gridDim.x) {
+                int tm, tn;
+                oz_tile_of(t, args.tiles_m, args.tiles_n, tm, tn);
+                for (int kb = 0; kb < kblocks; ++kb) {
+                    mbar_wait(empty_bar(stage), phase ^ 1);
+                    mbar_arrive_expect_tx(full_bar(stage), stage_bytes);
+                    for (int s = 0; s < S; ++s) {
+                        tma_load_3d(a_tile(stage, s), &mapA, full_bar(stage), kb * OZ_BK, tm * OZ_BM, s);
+                        tma_load_3d(b_tile(stage, s), &mapB, full_bar(stage), kb * OZ_BK, tn * OZ_BN, s);
+                    }
+                    if (++stage == OZ_STAGES) { stage = 0; phase ^= 1; }
+                }
+            }
+        }
+    } else if (warp == 1) {
+        // =================================== MMA issuer ===================================
+        if (lane == 0) {
+            constexpr uint32_t idesc = oz_idesc();
+            int stage = 0;
+            uint32_t phase = 0, tphase = 0;
+            for (int t = blockIdx.x; t < ntiles; t += gridDim.x) {
+                mbar_wait(tempty_bar, tphase ^ 1);   // the epilogue has drained the accumulators of the previous tile
+                tc_fence_after();
+                for (int kb = 0; kb < kblocks; ++kb) {
+                    mbar_wait(full_bar(stage), phase);
+                    tc_fence_after();
+                    for (int s = 0; s < S; ++s) {
+                        const uint64_t ad = oz_smem_desc(a_tile(stage, s));
+                        for (int q = 0; q < S - s; ++q) {          // digit q of B: accumulator d = s + q
+                            const uint64_t bd = oz_smem_desc(b_tile(stage, q));
+                            const uint32_t dcol = tmem_base + (uint32_t)(s + q) * OZ_BN;
+#pragma unroll
+                            for (int kk = 0; kk < OZ_BK / 32; ++kk) {
+                                // first touch of every accumulator of a tile: k-block 0, s = 0, first K = 32 step
+                                const uint32_t acc = (kb > 0 || s > 0 || kk > 0) ? 1u : 0u;
+                                tc_mma_i8(dcol, ad + (uint64_t)(kk * 32 >> 4), bd + (uint64_t)(kk * 32 >> 4), idesc, acc);
+                            }
+                        }
+                    }
+                    tc_commit(empty_bar(stage));                   // stage back to the producer when these MMAs are done
+                    if (++stage == OZ_STAGES) { stage = 0; phase ^= 1; }
+                }
+                tc_commit(tfull_bar);                              // accumulators complete
+                tphase ^= 1;
+            }
+        }
+    } else if (warp >= 4) {
+        // =================================== epilogue warps ===================================
+        const int q4 = warp & 3;                                   // TMEM lane quarter this warp may access
+        const uint32_t lane_base = tmem_base + ((uint32_t)(q4 * 32) << 16);
+        uint32_t tphase = 0;
+        const int N = args.N;
+        for (int t = blockIdx.x; t < ntiles; t += gridDim.x) {
+            int tm, tn;
+            oz_tile_of(t, args.tiles_m, args.tiles_n, tm, tn);
+            mbar_wait(tfull_bar, tphase);
+            tphase ^= 1;
+            tc_fence_after();
+            const int row = tm * OZ_BM + q4 * 32 + lane;
+            const double rs = (row < N) ? args.scaleA[row] * args.alpha * (1.0 / 4096.0) : 0.0;   // alpha 2^{e_i - 12}
+            for (int c8 = 0; c8 < OZ_BN / 8; ++c8) {
+                double r[8];
+#pragma unroll
+                for (int j = 0; j < 8; ++j) r[j] = 0.0;
+                for (int d = S - 1; d >= 0; --d) {                 // Horner from the least significant digit sum
+                    int v[8];
+                    tc_ld8(lane_base + (uint32_t)(d * OZ_BN + c8 * 8), v);
+                    tc_wait_ld();
+#pragma unroll
+                    for (int j = 0; j < 8; ++j) r[j] = fma(r[j], 1.0 / 128.0, (double)v[j]);
+                }
+                const int col0 = tn * OZ_BN + c8 * 8;
+                if (row < N) {
+#pragma unroll
+                    for (int j = 0; j < 8; ++j) {
+                        const int col = col0 + j;
+                        if (col < N) {
+                            double o = rs * args.scaleB[col] * r[j];
+                            if (args.C != nullptr) o = fma(args.beta, args.C[(long long)row * args.ldc + col], o);
+                            args.Out[(long long)row * args.ldo + col] = o;
+                        }
+                    }
+                }
+            }
+            tc_fence_before();
+            __syncwarp();
+            if (lane == 0) mbar_arrive(tempty_bar);
+        }
+    }
+    tc_fence_before();
+    __syncthreads();
+    if (warp == 2) {
+        tc_fence_after();
+        tc_dealloc512(tmem_base);
+    }
+}
+
+inline int oz_smem_bytes() { return OZ_STAGES * OZ_MAX_S * (OZ_A_TILE + OZ_B_TILE) + 128 + 1024; }
+
+}  // namespace chebdm

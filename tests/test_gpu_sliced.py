@@ -1,0 +1,92 @@
+"""`-m gpu` parity of cheb_dm_product_sliced: Out = alpha A B + beta C with the FP64 operands sliced
+into int8 digits and the digit products on tcgen05.mma kind::i8 (int32 accumulators in tensor memory).
+
+Oracle: oracle.matmul (plain triple loop, FP64).  Tolerance: the rounding bound of an FP64 dot product of N terms
+with |entries| <= 1, 4 N 2^-52 (the same gate as the DMMA product test), for S = 8 digits; fewer digits are checked
+against the slicing bound K (S+1) 2^{-7S} of include/cheb_dm.h, which must also be REACHED within two orders (the
+digits really are truncated: a kernel that silently used more precision, or a wrong bound, fails)."""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+
+def _imports():
+    import oracle
+    import paper_2306_12616_b200 as cd
+    import workloads
+    import gpu_util
+    return oracle, cd, workloads, gpu_util
+
+
+def _run(cd, gu, A, B, Cm, alpha, beta, S, same=False):
+    torch = gu.torch_cuda()
+    N = A.shape[0]
+    plan = cd.Plan(N, 4, sliced=S)
+    dA = gu.to_dev(A)
+    dB = dA if same else gu.to_dev(B)
+    dC = gu.to_dev(Cm) if Cm is not None else None
+    dO = torch.full((N, N), float("nan"), dtype=torch.float64, device="cuda")
+    st = torch.cuda.current_stream().cuda_stream
+    plan.product_sliced(alpha, dA.data_ptr(), dB.data_ptr(), beta, dC.data_ptr() if dC is not None else None, dO.data_ptr(), st)
+    torch.cuda.synchronize()
+    plan.destroy()
+    return dO.cpu().numpy()
+
+
+@pytest.mark.parametrize("N", [1, 2, 7, 63, 64, 65, 128, 130, 200, 333, 500, 777])
+def test_sliced_product_2AB_minus_C_eight_digits(N):
+    oracle, cd, workloads, gu = _imports()
+    A = workloads.random_symmetric(N, seed=10 + N)
+    B = workloads.random_symmetric(N, seed=20 + N)
+    Cm = workloads.random_symmetric(N, seed=30 + N)
+    expect = 2.0 * oracle.matmul(A, B) - Cm
+    got = _run(cd, gu, A, B, Cm, 2.0, -1.0, 8)
+    err = float(np.max(np.abs(got - expect)))
+    print(f"N={N}: max|err| = {err:.3e} (gate {4.0 * N * 2.0 ** -52 + 1e-15:.3e})")
+    assert err <= 4.0 * N * 2.0 ** -52 + 1e-15
+
+
+def test_sliced_square_without_C_and_graded_rows():
+    """A = B (digits formed once), C = NULL, rows of very different magnitude (row-wise scales 2^{e_i})."""
+    oracle, cd, workloads, gu = _imports()
+    N = 300
+    A = workloads.random_symmetric(N, seed=5)
+    g = 2.0 ** np.linspace(-40, 3, N)
+    A = (A * g[:, None]) * g[None, :]          # symmetric, |a_ij| <= g_i g_j
+    expect = oracle.matmul(A, A)
+    got = _run(cd, gu, A, None, None, 1.0, 0.0, 8, same=True)
+    rowmax = np.max(np.abs(A), axis=1)
+    bound = 4.0 * N * 2.0 ** -52 * rowmax[:, None] * rowmax[None, :]
+    assert np.all(np.abs(got - expect) <= bound + 1e-300)
+
+
+@pytest.mark.parametrize("S", [4, 5, 6, 7])
+def test_sliced_fewer_digits_meet_and_reach_the_slicing_bound(S):
+    oracle, cd, workloads, gu = _imports()
+    N = 256
+    A = workloads.random_symmetric(N, seed=77)
+    B = workloads.random_symmetric(N, seed=78)
+    expect = oracle.matmul(A, B)
+    got = _run(cd, gu, A, B, None, 1.0, 0.0, S)
+    ra, rb = np.max(np.abs(A), axis=1), np.max(np.abs(B), axis=1)
+    sa, sb = 2.0 ** np.ceil(np.log2(ra)), 2.0 ** np.ceil(np.log2(rb))   # the power-of-two row scales
+    bound = N * (S + 1) * 2.0 ** (-7 * S) * sa[:, None] * sb[None, :] * 4.0
+    err = np.abs(got - expect)
+    assert np.all(err <= bound)
+    assert np.max(err / bound) >= 1e-3      # truncated digits leave an error of the predicted order, not FP64 rounding
+
+
+def test_sliced_needs_the_plan_option():
+    oracle, cd, workloads, gu = _imports()
+    torch = gu.torch_cuda()
+    plan = cd.Plan(64, 4)
+    a = torch.zeros((64, 64), dtype=torch.float64, device="cuda")
+    o = torch.zeros((64, 64), dtype=torch.float64, device="cuda")
+    with pytest.raises(cd.ChebDMError) as ei:
+        plan.product_sliced(1.0, a.data_ptr(), a.data_ptr(), 0.0, None, o.data_ptr())
+    assert ei.value.status == 6
+    plan.destroy()
+    with pytest.raises(cd.ChebDMError) as ei:
+        cd.Plan(64, 4, sliced=9)
+    assert ei.value.status == 1
