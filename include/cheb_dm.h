@@ -287,10 +287,13 @@ cheb_dm_status_t cheb_dm_product(cheb_dm_plan_t plan, double alpha, const double
  * recombined in FP64:  Out = alpha * A B + beta * C  with  |error_ij| <= K (S+1) 2^{-7S} max_k|a_ik| max_k|b_kj| 4
  * plus FP64 rounding of the recombination; S = 8 (36 int8 products) is below the rounding error of an FP64 dot
  * product.  A, B symmetric N x N device matrices (ld N; B may equal A), C nullable (ld N), Out must not alias A or B.
+ * symmetric != 0: the caller asserts that the result is symmetric (A and B commute, C symmetric -- every product of the
+ * method, whose operands are polynomials of X): only the 128 x 64 tiles that touch the lower triangle are computed and
+ * each is mirrored on store.
  * Stand-alone call (kernel-level tests and benchmark against the DMMA product); the solve does not use it.
  * EUNSUPPORTED unless the plan was made with the option sliced = S. */
 cheb_dm_status_t cheb_dm_product_sliced(cheb_dm_plan_t plan, double alpha, const double* dA, const double* dB,
-                                        double beta, const double* dC, double* dOut, void* cuda_stream);
+                                        double beta, const double* dC, double* dOut, int symmetric, void* cuda_stream);
 
 /* Synchronises `cuda_stream` and reports what the device flagged since the last check (the flags are sticky, so one
  * check after a pipeline of computes sees an error of any of them; the check clears them): CHEB_DM_ECUDA if a CUDA

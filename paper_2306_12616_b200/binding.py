@@ -105,7 +105,7 @@ def lib():
     L.cheb_dm_solve_batch.argtypes = [vp, C.c_int, pp, dp, C.c_int, pp, dp, vp]
     L.cheb_dm_assemble.argtypes = [vp, C.c_int, dp, pp, vp]
     L.cheb_dm_flops_per_solve.argtypes = [vp, dp]
-    L.cheb_dm_product_sliced.argtypes = [vp, C.c_double, vp, vp, C.c_double, vp, vp, vp]
+    L.cheb_dm_product_sliced.argtypes = [vp, C.c_double, vp, vp, C.c_double, vp, vp, C.c_int, vp]
     for n in EXPORTS:
         getattr(L, n).restype = C.c_int
     L.cheb_dm_strerror.argtypes = [C.c_int]
@@ -301,8 +301,8 @@ class Plan:
     def product(self, alpha: float, dA: int, dB: int, beta: float, dC, d_out: int, stream: int = 0):
         _chk(lib().cheb_dm_product(self._h, alpha, dA, dB, beta, dC, d_out, stream), "cheb_dm_product")
 
-    def product_sliced(self, alpha: float, dA: int, dB: int, beta: float, dC, d_out: int, stream: int = 0):
-        _chk(lib().cheb_dm_product_sliced(self._h, alpha, dA, dB, beta, dC, d_out, stream), "cheb_dm_product_sliced")
+    def product_sliced(self, alpha: float, dA: int, dB: int, beta: float, dC, d_out: int, symmetric: bool = False, stream: int = 0):
+        _chk(lib().cheb_dm_product_sliced(self._h, alpha, dA, dB, beta, dC, d_out, 1 if symmetric else 0, stream), "cheb_dm_product_sliced")
 
     def workspace_bytes(self) -> int:
         v = C.c_size_t()

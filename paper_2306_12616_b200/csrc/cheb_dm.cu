@@ -157,6 +157,8 @@ struct cheb_dm_plan_s {
     int8_t* oz_digits;
     double* oz_scale;
     CUtensorMap oz_map[2][2];  // [operand][0: 128-row boxes (left factor), 1: 64-row boxes (right factor)]
+    short2* oz_tiles[2];       // raster-ordered tile lists: [0] every tile, [1] the tiles that touch the lower triangle
+    int oz_ntiles[2];
     // optional per-tile timeline (cheb_dm_set_trace)
     TraceRec* trace_buf;
     int trace_on, trace_res_base, trace_total, trace_nb;  // trace_nb: matrices of the last traced launch
@@ -956,7 +958,28 @@ cheb_dm_status_t prepare_sliced(cheb_dm_plan_s* P) {
                              CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
             if (r != CUDA_SUCCESS) return CHEB_DM_ECUDA;
         }
-    CUDA_TRY(cudaFuncSetAttribute(oz_gemm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, oz_smem_bytes()));
+    {
+        const int tiles_m = ceil_div(P->N, OZ_BM), tiles_n = ceil_div(P->N, OZ_BN);
+        for (int sym = 0; sym < 2; ++sym) {
+            std::vector<short2> list;
+            for (int band = 0; band * OZ_BAND < tiles_n; ++band)
+                for (int tm = 0; tm < tiles_m; ++tm)
+                    for (int tn = band * OZ_BAND; tn < tiles_n && tn < (band + 1) * OZ_BAND; ++tn)
+                        if (!sym || tm * OZ_BM + OZ_BM - 1 >= tn * OZ_BN) list.push_back(make_short2((short)tm, (short)tn));
+            P->oz_ntiles[sym] = (int)list.size();
+            if (cudaMalloc(&P->oz_tiles[sym], sizeof(short2) * list.size()) != cudaSuccess) { cudaGetLastError(); return CHEB_DM_EALLOC; }
+            CUDA_TRY(cudaMemcpy(P->oz_tiles[sym], list.data(), sizeof(short2) * list.size(), cudaMemcpyHostToDevice));
+        }
+    }
+    switch (P->oz_S) {
+        case 2: CUDA_TRY(cudaFuncSetAttribute(oz_gemm_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, oz_smem_bytes())); break;
+        case 3: CUDA_TRY(cudaFuncSetAttribute(oz_gemm_kernel<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, oz_smem_bytes())); break;
+        case 4: CUDA_TRY(cudaFuncSetAttribute(oz_gemm_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, oz_smem_bytes())); break;
+        case 5: CUDA_TRY(cudaFuncSetAttribute(oz_gemm_kernel<5>, cudaFuncAttributeMaxDynamicSharedMemorySize, oz_smem_bytes())); break;
+        case 6: CUDA_TRY(cudaFuncSetAttribute(oz_gemm_kernel<6>, cudaFuncAttributeMaxDynamicSharedMemorySize, oz_smem_bytes())); break;
+        case 7: CUDA_TRY(cudaFuncSetAttribute(oz_gemm_kernel<7>, cudaFuncAttributeMaxDynamicSharedMemorySize, oz_smem_bytes())); break;
+        default: CUDA_TRY(cudaFuncSetAttribute(oz_gemm_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, oz_smem_bytes())); break;
+    }
     return CHEB_DM_OK;
 }
 
@@ -1022,6 +1045,8 @@ cheb_dm_status_t cheb_dm_destroy(cheb_dm_plan_t P) {
     }
     cudaFree(P->oz_digits);
     cudaFree(P->oz_scale);
+    cudaFree(P->oz_tiles[0]);
+    cudaFree(P->oz_tiles[1]);
     cudaFree(P->trace_buf);
     for (int i = 0; i < TIMING_SLOTS; ++i) {
         if (P->ev0[i]) cudaEventDestroy(P->ev0[i]);
@@ -1153,7 +1178,7 @@ cheb_dm_status_t cheb_dm_plan_ex(cheb_dm_plan_t* plan, int N, int M_terms, cheb_
     P->n_async = 0;
     P->timing = 0; P->ev_count = 0;
     P->trace_buf = nullptr; P->trace_on = 0; P->trace_nb = 1;
-    P->oz_S = o.sliced; P->oz_kpad = ((long long)N + OZ_BK - 1) / OZ_BK * OZ_BK; P->oz_digits = nullptr; P->oz_scale = nullptr;
+    P->oz_S = o.sliced; P->oz_kpad = ((long long)N + OZ_BK - 1) / OZ_BK * OZ_BK; P->oz_digits = nullptr; P->oz_scale = nullptr; P->oz_tiles[0] = P->oz_tiles[1] = nullptr;
     for (int i = 0; i < TIMING_SLOTS; ++i) P->ev0[i] = P->ev1[i] = nullptr;
 
     const size_t kp = (size_t)k * p, B = (size_t)P->maxb;
@@ -1653,7 +1678,7 @@ cheb_dm_status_t cheb_dm_product(cheb_dm_plan_t P, double alpha, const double* d
 }
 
 cheb_dm_status_t cheb_dm_product_sliced(cheb_dm_plan_t P, double alpha, const double* dA, const double* dB, double beta,
-                                        const double* dC, double* dOut, void* cuda_stream) {
+                                        const double* dC, double* dOut, int symmetric, void* cuda_stream) {
     if (!P || !dA || !dB || !dOut) return CHEB_DM_EINVAL;
     if (dOut == dA || dOut == dB) return CHEB_DM_EINVAL;
     if (P->oz_S < 2) return CHEB_DM_EUNSUPPORTED;
@@ -1680,9 +1705,22 @@ cheb_dm_status_t cheb_dm_product_sliced(cheb_dm_plan_t P, double alpha, const do
     oa.ldc = N;
     oa.Out = dOut;
     oa.ldo = N;
-    int grid = oa.tiles_m * oa.tiles_n;
+    oa.sym = symmetric ? 1 : 0;
+    oa.ntiles = P->oz_ntiles[oa.sym];
+    oa.tile_list = P->oz_tiles[oa.sym];
+    int grid = oa.ntiles;
     if (grid > P->num_sms) grid = P->num_sms;
-    oz_gemm_kernel<<<grid, OZ_THREADS, oz_smem_bytes(), st>>>(P->oz_map[0][0], P->oz_map[same ? 0 : 1][1], oa);
+    const CUtensorMap& mA = P->oz_map[0][0];
+    const CUtensorMap& mB = P->oz_map[same ? 0 : 1][1];
+    switch (S) {
+        case 2: oz_gemm_kernel<2><<<grid, OZ_THREADS, oz_smem_bytes(), st>>>(mA, mB, oa); break;
+        case 3: oz_gemm_kernel<3><<<grid, OZ_THREADS, oz_smem_bytes(), st>>>(mA, mB, oa); break;
+        case 4: oz_gemm_kernel<4><<<grid, OZ_THREADS, oz_smem_bytes(), st>>>(mA, mB, oa); break;
+        case 5: oz_gemm_kernel<5><<<grid, OZ_THREADS, oz_smem_bytes(), st>>>(mA, mB, oa); break;
+        case 6: oz_gemm_kernel<6><<<grid, OZ_THREADS, oz_smem_bytes(), st>>>(mA, mB, oa); break;
+        case 7: oz_gemm_kernel<7><<<grid, OZ_THREADS, oz_smem_bytes(), st>>>(mA, mB, oa); break;
+        default: oz_gemm_kernel<8><<<grid, OZ_THREADS, oz_smem_bytes(), st>>>(mA, mB, oa); break;
+    }
     CUDA_TRY(cudaGetLastError());
     return CHEB_DM_OK;
 }

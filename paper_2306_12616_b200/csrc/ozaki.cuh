@@ -76,8 +76,8 @@ __device__ __forceinline__ uint64_t oz_smem_desc(uint32_t saddr) {
 }
 // Instruction descriptor of kind::i8: D = S32 (2 at [4,6)), A and B signed int8 (1 at [7,10), [10,13)), both K-major,
 // N >> 3 at [17,23), M >> 4 at [24,29), dense, no saturation.
-__host__ __device__ constexpr uint32_t oz_idesc() {
-    return (2u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(OZ_BN >> 3) << 17) | ((uint32_t)(OZ_BM >> 4) << 24);
+__host__ __device__ constexpr uint32_t oz_idesc(int n) {
+    return (2u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(n >> 3) << 17) | ((uint32_t)(OZ_BM >> 4) << 24);
 }
 
 // ---------------------------------------------------------------------------------------------------
@@ -113,6 +113,10 @@ struct OzArgs {
     int N, S;
     int kblocks;                 // kpad / OZ_BK
     int tiles_m, tiles_n;
+    int sym;                     // 1: the product is symmetric (A and B commute): lower-triangle tiles only, mirrored on store
+    int ntiles;                  // work items
+    const short2* tile_list;     // [ntiles] (tm, tn) in raster order: column bands of OZ_BAND tiles, row-major inside a band, so
+                                 // that the CTAs of a wave share few A and B digit strips (L2 reuse)
     const double* scaleA;        // [N] 2^{e_i}
     const double* scaleB;        // [N] 2^{f_j}
     double alpha, beta;
@@ -122,21 +126,11 @@ struct OzArgs {
     long long ldo;
 };
 
-__device__ __forceinline__ void oz_tile_of(int t, int tiles_m, int tiles_n, int& tm, int& tn) {
-    // column bands of OZ_BAND tiles, row-major inside a band: the CTAs of a wave share few A and B strips
-    const int band_tiles = tiles_m * OZ_BAND;
-    const int band = t / band_tiles;
-    const int r = t - band * band_tiles;
-    const int width = min(OZ_BAND, tiles_n - band * OZ_BAND);
-    tm = r / width;
-    tn = band * OZ_BAND + (r - tm * width);
-}
-
+template <int S>
 __global__ void __launch_bounds__(OZ_THREADS, 1) oz_gemm_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUtensorMap mapB,
                                                                 const OzArgs args) {
     extern __shared__ uint8_t smem_raw[];
     uint8_t* smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
-    const int S = args.S;
     const uint32_t stage_bytes = (uint32_t)S * (OZ_A_TILE + OZ_B_TILE);
     const uint32_t ring_bytes = OZ_STAGES * OZ_MAX_S * (OZ_A_TILE + OZ_B_TILE);
     uint64_t* bars = reinterpret_cast<uint64_t*>(smem + ring_bytes);
@@ -166,7 +160,7 @@ __global__ void __launch_bounds__(OZ_THREADS, 1) oz_gemm_kernel(const __grid_con
     tc_fence_after();
     const uint32_t tmem_base = *tmem_slot;
 
-    const int ntiles = args.tiles_m * args.tiles_n;
+    const int ntiles = args.ntiles;
     const int kblocks = args.kblocks;
 
     if (warp == 0) {
@@ -176,7 +170,8 @@ __global__ void __launch_bounds__(OZ_THREADS, 1) oz_gemm_kernel(const __grid_con
             uint32_t phase = 0;
             for (int t = blockIdx.x; t < ntiles; t += gridDim.x) {
                 int tm, tn;
-                oz_tile_of(t, args.tiles_m, args.tiles_n, tm, tn);
+                tm = args.tile_list[t].x;
+                tn = args.tile_list[t].y;
                 for (int kb = 0; kb < kblocks; ++kb) {
                     mbar_wait(empty_bar(stage), phase ^ 1);
                     mbar_arrive_expect_tx(full_bar(stage), stage_bytes);
@@ -191,7 +186,6 @@ __global__ void __launch_bounds__(OZ_THREADS, 1) oz_gemm_kernel(const __grid_con
     } else if (warp == 1) {
         // =================================== MMA issuer ===================================
         if (lane == 0) {
-            constexpr uint32_t idesc = oz_idesc();
             int stage = 0;
             uint32_t phase = 0, tphase = 0;
             for (int t = blockIdx.x; t < ntiles; t += gridDim.x) {
@@ -200,17 +194,24 @@ __global__ void __launch_bounds__(OZ_THREADS, 1) oz_gemm_kernel(const __grid_con
                 for (int kb = 0; kb < kblocks; ++kb) {
                     mbar_wait(full_bar(stage), phase);
                     tc_fence_after();
+                    // Digit s of A meets the digits q = 0 .. S-1-s of B, whose tiles are consecutive in shared memory (64 rows
+                    // each) and whose accumulators d = s + q are consecutive in tensor memory (64 columns each): one MMA of
+                    // N = 64 (S - s) columns (two when that exceeds 256) instead of S - s MMAs of N = 64 -- the single issuing
+                    // thread cannot feed 32-cycle MMAs fast enough (measured: 1.6 POPS with N = 64, see profiles/).
+#pragma unroll
                     for (int s = 0; s < S; ++s) {
                         const uint64_t ad = oz_smem_desc(a_tile(stage, s));
-                        for (int q = 0; q < S - s; ++q) {          // digit q of B: accumulator d = s + q
-                            const uint64_t bd = oz_smem_desc(b_tile(stage, q));
-                            const uint32_t dcol = tmem_base + (uint32_t)(s + q) * OZ_BN;
+                        const int nq = S - s;                          // digits of B
+                        const int n0 = (nq > 4) ? 4 : nq;              // first MMA: up to 4 digits (N <= 256)
 #pragma unroll
-                            for (int kk = 0; kk < OZ_BK / 32; ++kk) {
-                                // first touch of every accumulator of a tile: k-block 0, s = 0, first K = 32 step
-                                const uint32_t acc = (kb > 0 || s > 0 || kk > 0) ? 1u : 0u;
-                                tc_mma_i8(dcol, ad + (uint64_t)(kk * 32 >> 4), bd + (uint64_t)(kk * 32 >> 4), idesc, acc);
-                            }
+                        for (int kk = 0; kk < OZ_BK / 32; ++kk) {
+                            // first touch of every accumulator of a tile: k-block 0, s = 0, first K = 32 step
+                            const uint32_t acc = (kb > 0 || s > 0 || kk > 0) ? 1u : 0u;
+                            const uint64_t koff = (uint64_t)(kk * 32 >> 4);
+                            tc_mma_i8(tmem_base + (uint32_t)s * OZ_BN, ad + koff, oz_smem_desc(b_tile(stage, 0)) + koff, oz_idesc(64 * n0), acc);
+                            if (nq > 4)
+                                tc_mma_i8(tmem_base + (uint32_t)(s + 4) * OZ_BN, ad + koff, oz_smem_desc(b_tile(stage, 4)) + koff,
+                                          oz_idesc(64 * (nq - 4)), acc);
                         }
                     }
                     tc_commit(empty_bar(stage));                   // stage back to the producer when these MMAs are done
@@ -228,33 +229,37 @@ __global__ void __launch_bounds__(OZ_THREADS, 1) oz_gemm_kernel(const __grid_con
         const int N = args.N;
         for (int t = blockIdx.x; t < ntiles; t += gridDim.x) {
             int tm, tn;
-            oz_tile_of(t, args.tiles_m, args.tiles_n, tm, tn);
+            tm = args.tile_list[t].x;
+            tn = args.tile_list[t].y;
             mbar_wait(tfull_bar, tphase);
             tphase ^= 1;
             tc_fence_after();
             const int row = tm * OZ_BM + q4 * 32 + lane;
             const double rs = (row < N) ? args.scaleA[row] * args.alpha * (1.0 / 4096.0) : 0.0;   // alpha 2^{e_i - 12}
             for (int c8 = 0; c8 < OZ_BN / 8; ++c8) {
+                int v[S][8];
+#pragma unroll
+                for (int d = 0; d < S; ++d) tc_ld8(lane_base + (uint32_t)(d * OZ_BN + c8 * 8), v[d]);
+                tc_wait_ld();
                 double r[8];
 #pragma unroll
                 for (int j = 0; j < 8; ++j) r[j] = 0.0;
-                for (int d = S - 1; d >= 0; --d) {                 // Horner from the least significant digit sum
-                    int v[8];
-                    tc_ld8(lane_base + (uint32_t)(d * OZ_BN + c8 * 8), v);
-                    tc_wait_ld();
 #pragma unroll
-                    for (int j = 0; j < 8; ++j) r[j] = fma(r[j], 1.0 / 128.0, (double)v[j]);
-                }
+                for (int d = S - 1; d >= 0; --d)                   // Horner from the least significant digit sum
+#pragma unroll
+                    for (int j = 0; j < 8; ++j) r[j] = fma(r[j], 1.0 / 128.0, (double)v[d][j]);
                 const int col0 = tn * OZ_BN + c8 * 8;
-                if (row < N) {
 #pragma unroll
-                    for (int j = 0; j < 8; ++j) {
-                        const int col = col0 + j;
-                        if (col < N) {
-                            double o = rs * args.scaleB[col] * r[j];
-                            if (args.C != nullptr) o = fma(args.beta, args.C[(long long)row * args.ldc + col], o);
-                            args.Out[(long long)row * args.ldo + col] = o;
-                        }
+                for (int j = 0; j < 8; ++j) {
+                    const int col = col0 + j;
+                    double o = 0.0;
+                    if (row < N && col < N) {
+                        o = rs * args.scaleB[col] * r[j];
+                        if (args.C != nullptr) o = fma(args.beta, args.C[(long long)row * args.ldc + col], o);
+                        args.Out[(long long)row * args.ldo + col] = o;
+                        // mirror: the transposed element lies in a tile that is not a work item; the lanes of a warp hold 32
+                        // consecutive rows, i.e. 32 consecutive elements of the destination row: coalesced
+                        if (args.sym && (col / OZ_BM) * OZ_BM + OZ_BM - 1 < (row / OZ_BN) * OZ_BN) args.Out[(long long)col * args.ldo + row] = o;
                     }
                 }
             }

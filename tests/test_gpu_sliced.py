@@ -19,7 +19,7 @@ def _imports():
     return oracle, cd, workloads, gpu_util
 
 
-def _run(cd, gu, A, B, Cm, alpha, beta, S, same=False):
+def _run(cd, gu, A, B, Cm, alpha, beta, S, same=False, symmetric=False):
     torch = gu.torch_cuda()
     N = A.shape[0]
     plan = cd.Plan(N, 4, sliced=S)
@@ -28,7 +28,7 @@ def _run(cd, gu, A, B, Cm, alpha, beta, S, same=False):
     dC = gu.to_dev(Cm) if Cm is not None else None
     dO = torch.full((N, N), float("nan"), dtype=torch.float64, device="cuda")
     st = torch.cuda.current_stream().cuda_stream
-    plan.product_sliced(alpha, dA.data_ptr(), dB.data_ptr(), beta, dC.data_ptr() if dC is not None else None, dO.data_ptr(), st)
+    plan.product_sliced(alpha, dA.data_ptr(), dB.data_ptr(), beta, dC.data_ptr() if dC is not None else None, dO.data_ptr(), symmetric, st)
     torch.cuda.synchronize()
     plan.destroy()
     return dO.cpu().numpy()
@@ -77,6 +77,22 @@ def test_sliced_fewer_digits_meet_and_reach_the_slicing_bound(S):
     assert np.max(err / bound) >= 1e-3      # truncated digits leave an error of the predicted order, not FP64 rounding
 
 
+@pytest.mark.parametrize("N", [64, 129, 200, 333, 700])
+def test_sliced_symmetric_tiles_on_commuting_operands(N):
+    """Operands that commute (polynomials of one X, like every product of the method: T_5(X) T_3(X), minus T_2(X)):
+    lower-triangle tiles only, mirrored on store; every element is still written exactly once."""
+    oracle, cd, workloads, gu = _imports()
+    X = workloads.random_symmetric(N, seed=3 + N) / (0.6 * N ** 0.5 + 1.0)
+    T = [np.eye(N), X]
+    for n in range(2, 6):
+        T.append(2.0 * oracle.matmul(X, T[-1]) - T[-2])
+    expect = 2.0 * oracle.matmul(T[5], T[3]) - T[2]          # = T_8(X), symmetric
+    got = _run(cd, gu, T[5], T[3], T[2], 2.0, -1.0, 8, symmetric=True)
+    ra, rb = np.max(np.abs(T[5]), axis=1), np.max(np.abs(T[3]), axis=1)
+    assert np.max(np.abs(got - expect)) <= 4.0 * N * 2.0 ** -52 * max(1.0, ra.max() * rb.max()) + 1e-15
+    assert np.max(np.abs(got - got.T)) <= 8.0 * N * 2.0 ** -52 * max(1.0, ra.max() * rb.max())
+
+
 def test_sliced_needs_the_plan_option():
     oracle, cd, workloads, gu = _imports()
     torch = gu.torch_cuda()
@@ -84,7 +100,7 @@ def test_sliced_needs_the_plan_option():
     a = torch.zeros((64, 64), dtype=torch.float64, device="cuda")
     o = torch.zeros((64, 64), dtype=torch.float64, device="cuda")
     with pytest.raises(cd.ChebDMError) as ei:
-        plan.product_sliced(1.0, a.data_ptr(), a.data_ptr(), 0.0, None, o.data_ptr())
+        plan.product_sliced(1.0, a.data_ptr(), a.data_ptr(), 0.0, None, o.data_ptr(), False)
     assert ei.value.status == 6
     plan.destroy()
     with pytest.raises(cd.ChebDMError) as ei:
