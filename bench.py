@@ -63,6 +63,7 @@ def parse_args():
     ap.add_argument("--fuse", type=int, default=0, help="fuse_sums option of the plan (0 auto, 1 epilogue-fused, 2 pre-formed)")
     ap.add_argument("--giant", type=int, default=0, help="giant option of the plan (0 auto, 1 generic, 2 resident-multiplier kernel)")
     ap.add_argument("--symmetric", type=int, default=0, help="symmetric-tile skipping (0 auto = on, 1 off, 2 on)")
+    ap.add_argument("--sliced", type=int, default=0, help="S > 0: every product of cheb_dm_compute on the sliced int8 tensor path (tcgen05 kind::i8, S digits)")
     ap.add_argument("--k", type=int, default=0)
     ap.add_argument("--p", type=int, default=0)
     return ap.parse_args()
@@ -163,7 +164,8 @@ class Workload:
         self.batched = not args.no_batch
         self.st = torch.cuda.current_stream().cuda_stream
         self.plan = cd.Plan(cfg.N, cfg.M, sched=args.sched, tile=args.tile, k=args.k, p=args.p, fuse_sums=args.fuse, giant=args.giant,
-                            symmetric=args.symmetric, max_batch=self.units if self.batched else 1, host_slots=2)
+                            symmetric=args.symmetric, max_batch=self.units if self.batched else 1, host_slots=2,
+                            sliced=args.sliced, sliced_solve=1 if args.sliced else 0)
         self.hH, self.dH, self.dD, self.hD = [], [], [], []
         for seed in self.seeds:
             H = torch.from_numpy(workloads.hamiltonian(name, seed=seed))

@@ -131,7 +131,10 @@ typedef struct {
                       (cheb_dm_compute_host), 2 = both + copy streams/events (cheb_dm_compute_host_async).         */
     int sliced;     /* digits S of cheb_dm_product_sliced: 0 = off, 2..8: the plan allocates the int8 digit
                       planes of two operands (2 S N kpad bytes, kpad = N rounded up to 64) and their scale vectors.        */
-    int reserved[1];
+    int sliced_solve; /* 1: cheb_dm_compute runs every product of the solve (baby steps and giant steps) on the sliced int8
+                      tensor path (sliced digits, default 8) instead of the FP64 DMMA kernel: one launch per product, each
+                      result sliced once, k + 4 digit sets in the workspace; single solves only (max_batch <= 1), low-order
+                      sums pre-formed.  Pays from N ~ 2000.  cheb_dm_solve / moments keep the DMMA path. */
 } cheb_dm_options_t;
 
 /* Create a plan for N x N matrices and an M_terms-term expansion.  Chooses (k,p), allocates the

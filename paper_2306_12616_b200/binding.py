@@ -37,7 +37,7 @@ class Options(C.Structure):
     _fields_ = [("k", C.c_int), ("p", C.c_int), ("outer", C.c_int), ("sched", C.c_int),
                 ("pairing", C.c_int), ("tile", C.c_int), ("fuse_sums", C.c_int),
                 ("giant", C.c_int), ("symmetric", C.c_int), ("max_batch", C.c_int), ("ldh", C.c_int), ("ldd", C.c_int),
-                ("moments", C.c_int), ("host_slots", C.c_int), ("sliced", C.c_int), ("reserved", C.c_int * 1)]
+                ("moments", C.c_int), ("host_slots", C.c_int), ("sliced", C.c_int), ("sliced_solve", C.c_int)]
 
 
 class ChebDMError(RuntimeError):
@@ -151,11 +151,11 @@ class Plan:
     def __init__(self, N: int, M: int, *, k: int = 0, p: int = 0, outer: int = OUTER_CHEBYSHEV,
                  sched: int = SCHED_GROUPED, pairing: int = PAIR_AUTO, tile: int = TILE_AUTO,
                  fuse_sums: int = 0, giant: int = 0, symmetric: int = 0, max_batch: int = 0, ldh: int = 0, ldd: int = 0,
-                 moments: int = 0, host_slots: int = 0, sliced: int = 0, dtype: int = 0):
+                 moments: int = 0, host_slots: int = 0, sliced: int = 0, sliced_solve: int = 0, dtype: int = 0):
         self._h = C.c_void_p()
         self.N, self.M = N, M
         o = Options(k=k, p=p, outer=outer, sched=sched, pairing=pairing, tile=tile, fuse_sums=fuse_sums, giant=giant, symmetric=symmetric,
-                    max_batch=max_batch, ldh=ldh, ldd=ldd, moments=moments, host_slots=host_slots, sliced=sliced)
+                    max_batch=max_batch, ldh=ldh, ldd=ldd, moments=moments, host_slots=host_slots, sliced=sliced, sliced_solve=sliced_solve)
         _chk(lib().cheb_dm_plan_ex(C.byref(self._h), N, M, dtype, C.byref(o)), "cheb_dm_plan_ex")
         kk, pp = C.c_int(), C.c_int()
         _chk(lib().cheb_dm_get_kp(self._h, C.byref(kk), C.byref(pp)), "cheb_dm_get_kp")

@@ -152,11 +152,11 @@ struct cheb_dm_plan_s {
     long long n_async;
     int pipe_ready;
     // digit planes of cheb_dm_product_sliced (option sliced = S): [operand][digit][N][oz_kpad] int8, scales [operand][N]
-    int oz_S;
+    int oz_S, oz_nsets, oz_solve;   // digit sets: T_1..T_k, two giant-step buffers (sliced_solve), then the two of the stand-alone product
     long long oz_kpad;
-    int8_t* oz_digits;
-    double* oz_scale;
-    CUtensorMap oz_map[2][2];  // [operand][0: 128-row boxes (left factor), 1: 64-row boxes (right factor)]
+    int8_t* oz_digits;         // [set][digit][N][oz_kpad]
+    double* oz_scale;          // [set][N] row scales, then [set][N] diagonal corrections of exact squares
+    std::vector<CUtensorMap> oz_maps;  // [set][0: 128-row boxes (left factor), 1: 64-row boxes (right factor)]
     short2* oz_tiles[2];       // raster-ordered tile lists: [0] every tile, [1] the tiles that touch the lower triangle
     int oz_ntiles[2];
     // optional per-tile timeline (cheb_dm_set_trace)
@@ -762,20 +762,20 @@ cheb_dm_status_t front_end(cheb_dm_plan_s* P, int nb, const double* const* dH, l
 
 // Low-order sums G_l = sum_i coef_{i,l} T_i of Eq. (21) for all l at once (a-5, batched form), nb matrices.
 // full = true: every element (the G_l are operands of the long-K product); false: only the tiles the giant steps read.
-cheb_dm_status_t form_sums(cheb_dm_plan_s* P, int nb, bool full, cudaStream_t st) {
+cheb_dm_status_t form_sums(cheb_dm_plan_s* P, int nb, bool full, int tileM, int tileN, cudaStream_t st) {
     const double* coefT = (P->opt.outer == CHEB_DM_OUTER_POWER) ? P->dT : P->gT;
-    const int symBM = (P->sym && !full) ? P->BM : 0;
+    const int symBM = (P->sym && !full) ? tileM : 0;
     if (P->scalar_sums) {  // FP64-FMA version (ablation)
         const long long pairs = (long long)P->N * P->ld / 2;
         dim3 grid((unsigned)((pairs + 255) / 256), (unsigned)ceil_div(P->p, SUMS_CHUNK), (unsigned)nb);
         form_sums_kernel<<<grid, 256, sizeof(double) * P->k * SUMS_CHUNK, st>>>(T_ptr(P, 0, 1), (long long)P->mat_elems, P->ld, P->N, P->k, P->p,
-                                                                              coefT, G_ptr(P, 0, 0), symBM, P->BN, (long long)P->slot_elems);
+                                                                              coefT, G_ptr(P, 0, 0), symBM, tileN, (long long)P->slot_elems);
     } else {
         const long long warps = ((long long)P->N * P->ld + 31) / 32;
         dim3 grid((unsigned)((warps + 7) / 8), (unsigned)ceil_div(P->p, SUMS_CHUNK), (unsigned)nb);
         const size_t smem = sizeof(double) * (size_t)((((P->k - 1) + 3) & ~3) + 1) * SUMS_CHUNK;
         form_sums_dmma_kernel<<<grid, 256, smem, st>>>(T_ptr(P, 0, 1), (long long)P->mat_elems, P->ld, P->N, P->k, P->p, coefT, G_ptr(P, 0, 0),
-                                                       symBM, P->BN, (long long)P->slot_elems);
+                                                       symBM, tileN, (long long)P->slot_elems);
     }
     ++P->last_launches;
     CUDA_TRY(cudaGetLastError());
@@ -819,12 +819,15 @@ cheb_dm_status_t run_giant_resident(cheb_dm_plan_s* P, double* userD, long long 
 }
 
 // Products of a fixed-mu solve after the front end: baby steps, sums, giant steps.
+cheb_dm_status_t run_products_sliced(cheb_dm_plan_s* P, double* userD, long long ldd, cudaStream_t st);
+
 cheb_dm_status_t run_products(cheb_dm_plan_s* P, int nb, double* const* dD, long long ldd, cudaStream_t st) {
+    if (P->oz_solve) return run_products_sliced(P, dD[0], ldd, st);
     cheb_dm_status_t s = run_table(P, P->baby, nb, dD, ldd, st);
     if (s != CHEB_DM_OK) return s;
     if (P->resident && nb == 1) return run_giant_resident(P, dD[0], ldd, st);
     if (P->preformed) {
-        s = form_sums(P, nb, false, st);
+        s = form_sums(P, nb, false, P->BM, P->BN, st);
         if (s != CHEB_DM_OK) return s;
     }
     return run_table(P, P->giant, nb, dD, ldd, st);
@@ -887,7 +890,7 @@ cheb_dm_status_t assemble_impl(cheb_dm_plan_s* P, int nb, const double* mu, int 
                                cudaStream_t st) {
     cheb_dm_status_t s = front_end(P, nb, nullptr, 0, mu, 0, 1, mu_from_device, st);
     if (s != CHEB_DM_OK) return s;
-    s = form_sums(P, nb, true, st);
+    s = form_sums(P, nb, true, P->BM, P->BN, st);
     if (s != CHEB_DM_OK) return s;
     return run_table(P, P->flat, nb, dD, ldd, st);
 }
@@ -938,23 +941,25 @@ bool batch_args_ok(const cheb_dm_plan_s* P, int nb, const double* const* A, doub
 // Digit planes, scales and TMA descriptors of cheb_dm_product_sliced.
 cheb_dm_status_t prepare_sliced(cheb_dm_plan_s* P) {
     const size_t plane = (size_t)P->N * (size_t)P->oz_kpad;
-    const size_t bytes = 2 * (size_t)P->oz_S * plane;
-    if (cudaMalloc(&P->oz_digits, bytes) != cudaSuccess || cudaMalloc(&P->oz_scale, sizeof(double) * 2 * P->N) != cudaSuccess) {
+    P->oz_nsets = (P->oz_solve ? P->k + 2 : 0) + 2;
+    const size_t bytes = (size_t)P->oz_nsets * (size_t)P->oz_S * plane;
+    if (cudaMalloc(&P->oz_digits, bytes) != cudaSuccess || cudaMalloc(&P->oz_scale, sizeof(double) * 2 * P->oz_nsets * P->N) != cudaSuccess) {
         cudaGetLastError();
         return CHEB_DM_EALLOC;
     }
-    P->ws_bytes += bytes + sizeof(double) * 2 * P->N;
+    P->ws_bytes += bytes + sizeof(double) * 2 * P->oz_nsets * P->N;
     EncodeTiledFn enc = get_encode_fn();
     if (!enc) return CHEB_DM_ECUDA;
-    for (int op = 0; op < 2; ++op)
+    P->oz_maps.resize((size_t)P->oz_nsets * 2);
+    for (int set = 0; set < P->oz_nsets; ++set)
         for (int role = 0; role < 2; ++role) {
             // {k (bytes), row, digit}: a box is one k-block of 64 int8 x 128 (or 64) rows of one digit plane, 64-byte swizzle
             cuuint64_t dims[3] = {(cuuint64_t)P->oz_kpad, (cuuint64_t)P->N, (cuuint64_t)P->oz_S};
             cuuint64_t strides[2] = {(cuuint64_t)P->oz_kpad, (cuuint64_t)plane};
             cuuint32_t box[3] = {(cuuint32_t)OZ_BK, (cuuint32_t)(role == 0 ? OZ_BM : OZ_BN), 1};
             cuuint32_t estr[3] = {1, 1, 1};
-            CUresult r = enc(&P->oz_map[op][role], CU_TENSOR_MAP_DATA_TYPE_UINT8, 3, P->oz_digits + (size_t)op * P->oz_S * plane, dims, strides, box,
-                             estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_64B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+            CUresult r = enc(&P->oz_maps[(size_t)set * 2 + role], CU_TENSOR_MAP_DATA_TYPE_UINT8, 3, P->oz_digits + (size_t)set * P->oz_S * plane, dims,
+                             strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_64B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
                              CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
             if (r != CUDA_SUCCESS) return CHEB_DM_ECUDA;
         }
@@ -980,6 +985,122 @@ cheb_dm_status_t prepare_sliced(cheb_dm_plan_s* P) {
         case 7: CUDA_TRY(cudaFuncSetAttribute(oz_gemm_kernel<7>, cudaFuncAttributeMaxDynamicSharedMemorySize, oz_smem_bytes())); break;
         default: CUDA_TRY(cudaFuncSetAttribute(oz_gemm_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, oz_smem_bytes())); break;
     }
+    return CHEB_DM_OK;
+}
+
+// Digits of an FP64 matrix (leading dimension ld) into digit set `set`.
+cheb_dm_status_t oz_split(cheb_dm_plan_s* P, int set, const double* src, long long ld, cudaStream_t st) {
+    const size_t plane = (size_t)P->N * (size_t)P->oz_kpad;
+    oz_split_kernel<<<ceil_div(P->N * 32, 256), 256, 0, st>>>(src, ld, P->N, P->oz_S, P->oz_digits + (size_t)set * P->oz_S * plane, P->oz_kpad,
+                                                              P->oz_scale + (size_t)set * P->N, P->oz_scale + (size_t)(P->oz_nsets + set) * P->N);
+    CUDA_TRY(cudaGetLastError());
+    return CHEB_DM_OK;
+}
+
+// Out = alpha A B + beta C + G + diag I from the digit sets of A and B (oa carries the epilogue operands).
+cheb_dm_status_t oz_gemm(cheb_dm_plan_s* P, int setA, int setB, OzArgs oa, int symmetric, cudaStream_t st) {
+    const int S = P->oz_S;
+    oa.N = P->N;
+    oa.S = S;
+    oa.kblocks = (int)(P->oz_kpad / OZ_BK);
+    oa.tiles_m = ceil_div(P->N, OZ_BM);
+    oa.tiles_n = ceil_div(P->N, OZ_BN);
+    oa.scaleA = P->oz_scale + (size_t)setA * P->N;
+    oa.scaleB = P->oz_scale + (size_t)setB * P->N;
+    oa.corr = (setA == setB) ? P->oz_scale + (size_t)(P->oz_nsets + setA) * P->N : nullptr;
+    oa.sym = symmetric ? 1 : 0;
+    oa.ntiles = P->oz_ntiles[oa.sym];
+    oa.tile_list = P->oz_tiles[oa.sym];
+    int grid = oa.ntiles;
+    if (grid > P->num_sms) grid = P->num_sms;
+    const CUtensorMap& mA = P->oz_maps[(size_t)setA * 2];
+    const CUtensorMap& mB = P->oz_maps[(size_t)setB * 2 + 1];
+    switch (S) {
+        case 2: oz_gemm_kernel<2><<<grid, OZ_THREADS, oz_smem_bytes(), st>>>(mA, mB, oa); break;
+        case 3: oz_gemm_kernel<3><<<grid, OZ_THREADS, oz_smem_bytes(), st>>>(mA, mB, oa); break;
+        case 4: oz_gemm_kernel<4><<<grid, OZ_THREADS, oz_smem_bytes(), st>>>(mA, mB, oa); break;
+        case 5: oz_gemm_kernel<5><<<grid, OZ_THREADS, oz_smem_bytes(), st>>>(mA, mB, oa); break;
+        case 6: oz_gemm_kernel<6><<<grid, OZ_THREADS, oz_smem_bytes(), st>>>(mA, mB, oa); break;
+        case 7: oz_gemm_kernel<7><<<grid, OZ_THREADS, oz_smem_bytes(), st>>>(mA, mB, oa); break;
+        default: oz_gemm_kernel<8><<<grid, OZ_THREADS, oz_smem_bytes(), st>>>(mA, mB, oa); break;
+    }
+    CUDA_TRY(cudaGetLastError());
+    return CHEB_DM_OK;
+}
+
+// The products of a fixed-mu solve on the sliced int8 path (option sliced_solve): the same task tables as the DMMA path
+// (Algorithm 1 / balanced pairing for the baby steps, Eq. 4 or its Clenshaw form for the giant steps, low-order sums
+// pre-formed in FP64), one launch per product; every result that is an operand later on is sliced once, right after it
+// is formed.  Digit set of workspace matrix m (T_1..T_k, buf0, buf1) = m, like its tensor-map index.
+cheb_dm_status_t run_products_sliced(cheb_dm_plan_s* P, double* userD, long long ldd, cudaStream_t st) {
+    const int k = P->k;
+    cheb_dm_status_t s = oz_split(P, 0, T_ptr(P, 0, 1), P->ld, st);  // T_1 = X
+    if (s != CHEB_DM_OK) return s;
+    ++P->last_launches;
+    const TaskTable* tabs[2] = {&P->baby, &P->giant};
+    for (int tb = 0; tb < 2; ++tb) {
+        const TaskTable& tt = *tabs[tb];
+        if (tb == 1) {
+            s = form_sums(P, 1, true, OZ_BM, OZ_BN, st);  // every element: the product-free step copies a whole G_l
+            if (s != CHEB_DM_OK) return s;
+        }
+        for (int lt = 0; lt < tt.ntl; ++lt) {
+            const Task& t = tt.h[(size_t)lt * P->maxb];
+            double* Out = t.out_is_user ? userD : t.Out;
+            const long long ldo = t.out_is_user ? ldd : t.ldo;
+            const double* G = (t.sum_count == 1) ? t.sum_base : nullptr;
+            if (t.sum_count > 1) return CHEB_DM_EUNSUPPORTED;  // the plan forces pre-formed sums
+            if (t.ktiles == 0) {
+                // product-free step (l = p - 1): Out = G
+                if (!G) return CHEB_DM_EUNSUPPORTED;
+                unpad_copy_kernel<<<P->num_sms * 4, 256, 0, st>>>(G, t.lds, P->N, Out, ldo);
+            } else {
+                OzArgs oa;
+                memset(&oa, 0, sizeof(oa));
+                oa.alpha = t.alpha;
+                oa.beta = t.C ? t.beta : 0.0;
+                oa.C = t.C;
+                oa.ldc = t.ldc;
+                oa.G = G;
+                oa.ldg = t.lds;
+                oa.diag = t.diag_const;
+                oa.Out = Out;
+                oa.ldo = ldo;
+                // Both factors are fetched K-major, i.e. the kernel forms (left) (right)^T.  Baby steps: T_l T_r^T, a one-off use of
+                // the (rounding-level) asymmetry of T_r.  Giant steps: the accumulator B_{l+1} must be the LEFT factor and the
+                // fixed multiplier Y = T_k the transposed one: with Y B^T an antisymmetric error component between eigenvectors
+                // of Y with eigenvalues of opposite sign obeys e_l = 2 Y e_{l+1}^T - e_{l+2} and grows like
+                // (c + sqrt(c^2 + 1))^l, c = sqrt|y_a y_b| (measured: 2e-7 at p = 32, 2e+4 at p = 64);
+                // with B Y^T every component follows the scalar Clenshaw recurrence and stays at the FP64 level.
+                // Baby steps take the higher-index operand as the left factor for the same reason (the serial pairing
+                // T_{n+1} = 2 T_1 T_n - T_{n-1} is such a recurrence in T_n).
+                const bool swap = (tb == 1) || (t.mapB > t.mapA);
+                const int left = swap ? t.mapB : t.mapA, right = swap ? t.mapA : t.mapB;
+                s = oz_gemm(P, left, right, oa, P->sym, st);
+                if (s != CHEB_DM_OK) return s;
+            }
+            ++P->last_launches;
+            // the result is an operand of a later product: T_n of the baby block (n - 1 = its matrix index), or a giant-step
+            // accumulator B_l, l >= 1 (matrix k + (l & 1))
+            if (!t.out_is_user) {
+                const int m = (int)((t.Out - P->ws) / (long long)P->mat_elems);
+                bool needed = (tb == 1);
+                if (tb == 0) {
+                    needed = (m == k - 1);
+                    for (int l2 = lt + 1; l2 < tt.ntl && !needed; ++l2) {
+                        const Task& u = tt.h[(size_t)l2 * P->maxb];
+                        needed = (u.mapA == m || u.mapB == m);
+                    }
+                }
+                if (needed) {
+                    s = oz_split(P, m, t.Out, t.ldo, st);
+                    if (s != CHEB_DM_OK) return s;
+                    ++P->last_launches;
+                }
+            }
+        }
+    }
+    CUDA_TRY(cudaGetLastError());
     return CHEB_DM_OK;
 }
 
@@ -1074,6 +1195,8 @@ cheb_dm_status_t cheb_dm_plan_ex(cheb_dm_plan_t* plan, int N, int M_terms, cheb_
     if ((o.ldh != 0 && o.ldh < N) || (o.ldd != 0 && o.ldd < N)) return CHEB_DM_EINVAL;
     if (o.moments < 0 || o.moments > 2 || o.host_slots < 0 || o.host_slots > 2) return CHEB_DM_EINVAL;
     if (o.sliced != 0 && (o.sliced < 2 || o.sliced > OZ_MAX_S || N > 65535)) return CHEB_DM_EINVAL;
+    if (o.sliced_solve < 0 || o.sliced_solve > 1 || (o.sliced_solve && (o.max_batch > 1 || N > 65535))) return CHEB_DM_EINVAL;
+    if (o.sliced_solve && o.sliced == 0) o.sliced = OZ_MAX_S;
     int k = o.k, p = o.p;
     if (k == 0 && p == 0) {
         k = 1;
@@ -1142,6 +1265,7 @@ cheb_dm_status_t cheb_dm_plan_ex(cheb_dm_plan_t* plan, int N, int M_terms, cheb_
         // (the epilogue warps of gemm_epi.cuh cannot gather k-1 tiles per item as fast as the consumers finish small-N
         // items: with those tile shapes the sums are always pre-formed)
         if (mode == 0) mode = (((double)k * (double)P->mat_elems * 8.0 * P->maxb > 96.0 * 1024 * 1024 || is_epi_tile(P->tile)) && k > 2 && p > 1) ? 2 : 1;
+        if (o.sliced_solve && k > 1 && p > 1) mode = 2;  // the sliced products add one pre-formed FP64 tile
         P->preformed = (mode == 2) ? 1 : 0;
         P->opt.fuse_sums = mode;
     }
@@ -1178,7 +1302,8 @@ cheb_dm_status_t cheb_dm_plan_ex(cheb_dm_plan_t* plan, int N, int M_terms, cheb_
     P->n_async = 0;
     P->timing = 0; P->ev_count = 0;
     P->trace_buf = nullptr; P->trace_on = 0; P->trace_nb = 1;
-    P->oz_S = o.sliced; P->oz_kpad = ((long long)N + OZ_BK - 1) / OZ_BK * OZ_BK; P->oz_digits = nullptr; P->oz_scale = nullptr; P->oz_tiles[0] = P->oz_tiles[1] = nullptr;
+    P->opt.sliced = o.sliced;
+    P->oz_S = o.sliced; P->oz_solve = o.sliced_solve; P->oz_nsets = 0; P->oz_kpad = ((long long)N + OZ_BK - 1) / OZ_BK * OZ_BK; P->oz_digits = nullptr; P->oz_scale = nullptr; P->oz_tiles[0] = P->oz_tiles[1] = nullptr;
     for (int i = 0; i < TIMING_SLOTS; ++i) P->ev0[i] = P->ev1[i] = nullptr;
 
     const size_t kp = (size_t)k * p, B = (size_t)P->maxb;
@@ -1684,45 +1809,21 @@ cheb_dm_status_t cheb_dm_product_sliced(cheb_dm_plan_t P, double alpha, const do
     if (P->oz_S < 2) return CHEB_DM_EUNSUPPORTED;
     if (!device_ok(P)) return CHEB_DM_ECUDA;
     cudaStream_t st = (cudaStream_t)cuda_stream;
-    const int N = P->N, S = P->oz_S;
-    const size_t plane = (size_t)N * (size_t)P->oz_kpad;
+    const int N = P->N;
     const int same = (dA == dB) ? 1 : 0;
-    const int split_blocks = ceil_div(N * 32, 256);
-    oz_split_kernel<<<split_blocks, 256, 0, st>>>(dA, N, N, S, P->oz_digits, P->oz_kpad, P->oz_scale);
-    if (!same) oz_split_kernel<<<split_blocks, 256, 0, st>>>(dB, N, N, S, P->oz_digits + (size_t)S * plane, P->oz_kpad, P->oz_scale + N);
+    const int setA = P->oz_nsets - 2, setB = same ? setA : P->oz_nsets - 1;
+    cheb_dm_status_t s = oz_split(P, setA, dA, N, st);
+    if (s == CHEB_DM_OK && !same) s = oz_split(P, setB, dB, N, st);
+    if (s != CHEB_DM_OK) return s;
     OzArgs oa;
     memset(&oa, 0, sizeof(oa));
-    oa.N = N;
-    oa.S = S;
-    oa.kblocks = (int)(P->oz_kpad / OZ_BK);
-    oa.tiles_m = ceil_div(N, OZ_BM);
-    oa.tiles_n = ceil_div(N, OZ_BN);
-    oa.scaleA = P->oz_scale;
-    oa.scaleB = P->oz_scale + (same ? 0 : N);
     oa.alpha = alpha;
     oa.beta = dC ? beta : 0.0;
     oa.C = dC;
     oa.ldc = N;
     oa.Out = dOut;
     oa.ldo = N;
-    oa.sym = symmetric ? 1 : 0;
-    oa.ntiles = P->oz_ntiles[oa.sym];
-    oa.tile_list = P->oz_tiles[oa.sym];
-    int grid = oa.ntiles;
-    if (grid > P->num_sms) grid = P->num_sms;
-    const CUtensorMap& mA = P->oz_map[0][0];
-    const CUtensorMap& mB = P->oz_map[same ? 0 : 1][1];
-    switch (S) {
-        case 2: oz_gemm_kernel<2><<<grid, OZ_THREADS, oz_smem_bytes(), st>>>(mA, mB, oa); break;
-        case 3: oz_gemm_kernel<3><<<grid, OZ_THREADS, oz_smem_bytes(), st>>>(mA, mB, oa); break;
-        case 4: oz_gemm_kernel<4><<<grid, OZ_THREADS, oz_smem_bytes(), st>>>(mA, mB, oa); break;
-        case 5: oz_gemm_kernel<5><<<grid, OZ_THREADS, oz_smem_bytes(), st>>>(mA, mB, oa); break;
-        case 6: oz_gemm_kernel<6><<<grid, OZ_THREADS, oz_smem_bytes(), st>>>(mA, mB, oa); break;
-        case 7: oz_gemm_kernel<7><<<grid, OZ_THREADS, oz_smem_bytes(), st>>>(mA, mB, oa); break;
-        default: oz_gemm_kernel<8><<<grid, OZ_THREADS, oz_smem_bytes(), st>>>(mA, mB, oa); break;
-    }
-    CUDA_TRY(cudaGetLastError());
-    return CHEB_DM_OK;
+    return oz_gemm(P, setA, setB, oa, symmetric, st);
 }
 
 // ------------------------------------------------------------------------------------------------------

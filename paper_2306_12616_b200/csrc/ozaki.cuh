@@ -3,8 +3,9 @@
 // tcgen05.mma kind::i8 (SASS UTCIMMA) with int32 accumulators in tensor memory, recombination in FP64.
 // sm_100a has no tcgen05 kind::f64 (the products of the solve run on DMMA.8x8x4, gemm_dmma.cuh); this is the
 // only route past the DMMA issue rate for the products  T_{a+b} = 2 T_a T_b - T_|a-b|  (Eq. 7) and
-// the Horner steps of Eq. (4).  Stand-alone product (cheb_dm_product_sliced); not wired into
-// the solve.  Product code; shares nothing with oracle/.
+// the Horner steps of Eq. (4).  Used by the stand-alone product cheb_dm_product_sliced and, with the plan
+// option sliced_solve, for every product of cheb_dm_compute (one launch per product + one slicing pass per result).
+// Product code; shares nothing with oracle/.
 //
 // Slicing (per row i of a symmetric operand; the row of B^T = B is the column of B):
 //     a_ik = 2^{e_i} ( sum_{s<S} q_s[i][k] 2^{-6-7s} + rho ),   q_s in [-64, 64] (int8),  |rho| <= 2^{-7S},
@@ -83,8 +84,13 @@ __host__ __device__ constexpr uint32_t oz_idesc(int n) {
 // ---------------------------------------------------------------------------------------------------
 // Slicing: one warp per row.  digits[s][row][k] (int8, row pitch kpad, zero beyond N), scale[row] = 2^{e_row}.
 // ---------------------------------------------------------------------------------------------------
+// corr[row] = sum_k sum_{s+t >= S} 2^{-7(s+t)} q_s[row][k] q_t[row][k]: the digit products the GEMM drops, for the DIAGONAL of
+// an exact square A A^T.  Off the diagonal, and between different matrices, the dropped products are incoherent sums of
+// magnitude sqrt(K) 2^{-7S}; on the diagonal of a square the s = t terms are sums of squares, a bias of K 64^2/3 2^{-7S}
+// that the squaring chain T_2 -> T_4 -> ... -> T_k amplifies by 4 per doubling (measured at N = 5000, k = 32: |dtr D| = 9.5e-8
+// without this term).  The epilogue adds it back when both factors are the same digit set.
 __global__ void __launch_bounds__(256) oz_split_kernel(const double* __restrict__ A, long long lda, int N, int S, int8_t* __restrict__ digits,
-                                                       long long kpad, double* __restrict__ scale) {
+                                                       long long kpad, double* __restrict__ scale, double* __restrict__ corr) {
     const int warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
     if (warp >= N) return;
     const double* row = A + (long long)warp * lda;
@@ -98,15 +104,35 @@ __global__ void __launch_bounds__(256) oz_split_kernel(const double* __restrict_
     }
     if (lane == 0) scale[warp] = ldexp(1.0, e);
     const long long plane = (long long)N * kpad;
+    double w = 0.0;
     for (long long k = lane; k < kpad; k += 32) {
         double t = (k < N) ? ldexp(row[k], 6 - e) : 0.0;   // |t| < 64
         int8_t* dst = digits + (long long)warp * kpad + k;
-        for (int s = 0; s < S; ++s) {
-            const double q = rint(t);
-            dst[(long long)s * plane] = (int8_t)(int)q;
-            t = (t - q) * 128.0;                            // exact: |t - q| <= 1/2
+        double q[OZ_MAX_S];
+#pragma unroll
+        for (int s = 0; s < OZ_MAX_S; ++s) {
+            q[s] = 0.0;
+            if (s < S) {
+                q[s] = rint(t);
+                dst[(long long)s * plane] = (int8_t)(int)q[s];
+                t = (t - q[s]) * 128.0;                     // exact: |t - q| <= 1/2
+            }
+        }
+        // dropped digit products of this element with itself, least significant first
+#pragma unroll
+        for (int d = 2 * OZ_MAX_S - 2; d >= 0; --d) {
+            double pd = 0.0;
+#pragma unroll
+            for (int s2 = 0; s2 < OZ_MAX_S; ++s2) {
+                const int t2 = d - s2;
+                if (t2 >= 0 && t2 < OZ_MAX_S) pd += q[s2] * q[t2];
+            }
+            if (d >= S) w += ldexp(pd, -7 * d);
         }
     }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) w += __shfl_xor_sync(0xffffffffu, w, o);
+    if (lane == 0) corr[warp] = w;
 }
 
 struct OzArgs {
@@ -119,9 +145,13 @@ struct OzArgs {
                                  // that the CTAs of a wave share few A and B digit strips (L2 reuse)
     const double* scaleA;        // [N] 2^{e_i}
     const double* scaleB;        // [N] 2^{f_j}
+    const double* corr;          // nullable: [N] dropped-product sums of the diagonal (both factors are the same digit set)
     double alpha, beta;
     const double* C;             // nullable, leading dimension ldc
     long long ldc;
+    const double* G;             // nullable: added with weight 1 (pre-formed low-order sum of Eq. 21), leading dimension ldg
+    long long ldg;
+    double diag;                 // added on the diagonal (- T_0 = - I of Eq. 22)
     double* Out;
     long long ldo;
 };
@@ -254,8 +284,11 @@ __global__ void __launch_bounds__(OZ_THREADS, 1) oz_gemm_kernel(const __grid_con
                     const int col = col0 + j;
                     double o = 0.0;
                     if (row < N && col < N) {
+                        if (args.corr != nullptr && row == col) r[j] += args.corr[row];
                         o = rs * args.scaleB[col] * r[j];
                         if (args.C != nullptr) o = fma(args.beta, args.C[(long long)row * args.ldc + col], o);
+                        if (args.G != nullptr) o += args.G[(long long)row * args.ldg + col];
+                        if (row == col) o += args.diag;
                         args.Out[(long long)row * args.ldo + col] = o;
                         // mirror: the transposed element lies in a tile that is not a work item; the lanes of a warp hold 32
                         // consecutive rows, i.e. 32 consecutive elements of the destination row: coalesced

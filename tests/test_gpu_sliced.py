@@ -106,3 +106,59 @@ def test_sliced_needs_the_plan_option():
     with pytest.raises(cd.ChebDMError) as ei:
         cd.Plan(64, 4, sliced=9)
     assert ei.value.status == 1
+
+
+# ----------------------------------------------------------------------------------------------
+# the whole fixed-mu solve on the sliced path (plan option sliced_solve): same gates as the DMMA path
+# ----------------------------------------------------------------------------------------------
+SOLVE_CASES = [("cfg0", 0, 128, None, {}), ("cfg1", 0, 300, None, {}), ("cfg1", 1, 257, None, {}), ("cfg2", 0, 250, None, {}),
+               ("cfg3", 0, 200, 1024, {}), ("cfg4", 0, 200, 2048, {}), ("cfg1", 2, 130, 60, dict(k=6, p=10)),
+               ("cfg4", 0, 333, 2048, {}), ("cfg1", 3, 200, 64, dict(symmetric=1)), ("cfg0", 0, 128, None, dict(outer=1)),
+               ("cfg1", 0, 150, 96, dict(pairing=1, k=24, p=4)), ("cfg1", 1, 150, 256, dict(pairing=3)), ("cfg3", 0, 150, 1024, dict(k=16, p=64))]
+
+
+@pytest.mark.parametrize("cfg,seed,n,M,opts", SOLVE_CASES)
+def test_sliced_solve_parity(cfg, seed, n, M, opts):
+    """cheb_dm_compute with every product on tcgen05 kind::i8 (8 digits): max|D - D_cheb| <= 1e-10, |dtr| <= 1e-9."""
+    import oracle_cases as oc
+    oracle, cd, workloads, gu = _imports()
+    case = oc.case(cfg, seed, n, M)
+    r = gu.gpu_solve(case["H"], case["beta"], case["mu"], case["M"], sliced_solve=1, **opts)
+    dD = float(np.max(np.abs(r["D"] - case["D_cheb"])))
+    dtr = abs(r["trace"] - float(np.trace(case["D_cheb"])))
+    print(f"{cfg} n={case['N']} M={case['M']}: sliced solve max|dD| = {dD:.3e}, |dtr| = {dtr:.3e}")
+    assert dD <= 1e-10
+    assert dtr <= 1e-9
+    assert np.max(np.abs(r["D"] - r["D"].T)) <= 1e-11
+
+
+@pytest.mark.parametrize("cfg", ["cfg2", "cfg4", "cfg3"])
+def test_sliced_solve_full_size(cfg):
+    """Full-size parity of the sliced solve: every element for cfg2; sampled columns + probe vectors that touch every
+    element for cfg4 / cfg3 (as tests/test_gpu_fullsize.py does for the DMMA path)."""
+    import oracle_cases as oc
+    oracle, cd, workloads, gu = _imports()
+    whole = cfg == "cfg2"
+    case = oc.case(cfg, 0, None, None, whole)
+    N = case["N"]
+    r = gu.gpu_solve(case["H"], case["beta"], case["mu"], case["M"], sliced_solve=1)
+    D = r["D"]
+    if whole:
+        dD = float(np.max(np.abs(D - case["D_cheb"])))
+        print(f"{cfg}: sliced solve, full matrix max|dD| = {dD:.3e}")
+        assert dD <= 1e-10
+    else:
+        cols = np.unique(np.concatenate([[0, N - 1], np.random.default_rng(7).integers(0, N, size=1)])).astype(np.int32)
+        want = oracle.dm_cheb_columns(case["H"], case["a"], case["b"], case["c"], cols)
+        dcol = float(np.max(np.abs(D[:, cols].T - want)))
+        rng = np.random.default_rng(11)
+        V = np.vstack([rng.standard_normal((2, N)), rng.choice([-1.0, 1.0], size=(2, N))])
+        want = oracle.dm_cheb_apply(case["H"], case["a"], case["b"], case["c"], V)
+        err = np.max(np.abs(V @ D.T - want), axis=1) / np.max(np.abs(V), axis=1)
+        print(f"{cfg}: sliced solve, columns max|dD| = {dcol:.3e}, probes {err}")
+        assert dcol <= 1e-10
+        assert np.all(err <= 1e-10 * np.sqrt(N))
+    dtr = abs(r["trace"] - case["trace_cheb_scalar"])
+    print(f"{cfg}: sliced solve |tr D - sum_i p_M(x_i)| = {dtr:.3e}")
+    assert dtr <= 1e-9
+    assert np.max(np.abs(D - D.T)) <= 1e-11
