@@ -273,6 +273,44 @@ def job_value(world, units_per_step, steps, max_ms):
     return world * units_per_step * steps / (max_ms * 1e-3)
 
 
+def measure_sliced(torch, cd, workloads, name, args, steps, warmup, flush, dist, world, int8_peak):
+    """The same fixed-mu step with every product on the sliced int8 tensor path (tcgen05 kind::i8, plan option
+    sliced_solve): solves/s, and the digit GEMMs' executed int8 operations against the int8 tensor peak."""
+    import copy
+    a2 = copy.copy(args)
+    a2.sliced = 8
+    w = Workload(torch, cd, workloads, name, a2)
+    plan = w.plan
+    plan.set_timing(True)
+    for _ in range(warmup):
+        w.step()
+    torch.cuda.synchronize()
+    plan.set_timing(True)
+    total_ms = timed_steps(torch, w.step, steps, 0, flush, None, dist)
+    n_rec, prod_ms = plan.product_ms()
+    plan.set_timing(False)
+    plan.check(w.st)
+    total_ms = max_over_ranks(torch, dist, total_ms)
+    ops = plan.sliced_ops_per_compute()
+    kernel_ms = prod_ms / max(n_rec, 1)
+    achieved = ops / (kernel_ms * 1e-3) * 1e-12
+    e2e_steps = max(3, min(steps, 10))
+    e2e_ms = max_over_ranks(torch, dist, timed_steps(torch, w.step_host, e2e_steps, 1, flush, None, dist))
+    res = {"call": "cheb_dm_compute on a plan with sliced_solve = 1, sliced = 8 digits", "value": job_value(world, w.units, steps, total_ms), "unit": UNIT,
+           "ms_per_solve": total_ms / steps / w.units, "tr_D": [float(x) for x in w.dtr.cpu().tolist()],
+           "e2e": {"value": world * w.units * e2e_steps / (e2e_ms * 1e-3), "unit": UNIT},
+           "full_product_equivalent_tflops": (plan.k + plan.p - 2) * 2.0 * w.N ** 3 / (kernel_ms * 1e-3) * 1e-12,
+           "roofline": {"bound": "tensor", "kernel": "oz_gemm_kernel<8> (tcgen05.mma kind::i8, 8 int32 accumulators in tensor memory) + oz_split_kernel + form_sums",
+                        "achieved": achieved, "peak": int8_peak, "unit": "TOP/s", "frac": achieved / int8_peak if int8_peak else None,
+                        "peak_source": "MEASURED_PEAKS.json bf16_tflops (burst) x 2 (nominal int8 : bf16 ratio of the profiling guide)",
+                        "kernel_ms": kernel_ms, "ops_per_launch": ops, "note": "kernel_ms spans all product launches of a solve, slicing passes and the sums pass included"},
+           "gpu_launches_per_step": w.launches_per_step, "workspace_bytes": plan.workspace_bytes()}
+    plan.destroy()
+    del w
+    torch.cuda.empty_cache()
+    return res
+
+
 def measure_workload(torch, cd, workloads, name, args, steps, warmup, flush, sampler, dist, peak_tf, world):
     w = Workload(torch, cd, workloads, name, args)
     plan = w.plan
@@ -477,12 +515,19 @@ def main():
     st = torch.cuda.current_stream().cuda_stream
     peak_tf = max(cd.dmma_peak(40000, st) for _ in range(3))
 
+    try:
+        int8_peak = 2.0 * float(json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json"))).get("bf16_tflops"))
+    except Exception:
+        int8_peak = 2.0 * 1590.0  # the profiling guide's fallback bf16 figure x 2
     main_res = measure_workload(torch, cd, workloads, args.config, args, args.steps, args.warmup, flush, sampler, dist, peak_tf, world)
     others = []
     for name in [s for s in args.others.split(",") if s and s != args.config]:
         big = workloads.CONFIGS[name].N >= 2000
         k_steps = max(2, min(args.steps, 5 if big else 10))
         others.append(measure_workload(torch, cd, workloads, name, args, k_steps, 3, flush, sampler, dist, peak_tf, world))
+        if big and not args.sliced:
+            # N >= 2000: the same step with the products on the sliced int8 tensor path, reported beside it
+            others[-1]["sliced_int8"] = measure_sliced(torch, cd, workloads, name, args, k_steps, 3, flush, dist, world, int8_peak)
     peak_after = cd.dmma_peak(40000, st)
     # sustained DMMA peak: the same microbenchmark back to back for ~2 s (clocks settle under the power cap)
     t_end = time.perf_counter() + 2.0

@@ -317,6 +317,9 @@ cheb_dm_status_t cheb_dm_last_launch_count(cheb_dm_plan_t plan, int* launches_ou
  * giant block, Gram kernel and the long-K assembly). */
 cheb_dm_status_t cheb_dm_flops_per_compute(cheb_dm_plan_t plan, double* flops_out);
 cheb_dm_status_t cheb_dm_flops_per_solve(cheb_dm_plan_t plan, double* flops_out);
+/* Executed int8 tensor operations of one cheb_dm_compute() on a plan with sliced_solve: products x S (S+1)/2 digit
+ * products x 2 x (computed 128 x 64 tiles) x kpad.  EUNSUPPORTED without the option. */
+cheb_dm_status_t cheb_dm_sliced_ops_per_compute(cheb_dm_plan_t plan, double* ops_out);
 
 /* Measurement support (bench.py's roofline object).
  * cheb_dm_set_timing(plan, 1): every following cheb_dm_compute() records a CUDA event on its stream

@@ -23,7 +23,7 @@ EXPORTS = [
     "cheb_dm_compute_host_async", "cheb_dm_wait",
     "cheb_dm_compute_batch", "cheb_dm_compute_batch_host", "cheb_dm_compute_batch_host_async", "cheb_dm_trace_batch",
     "cheb_dm_get_scalars", "cheb_dm_solve", "cheb_dm_solve_batch", "cheb_dm_assemble", "cheb_dm_flops_per_solve",
-    "cheb_dm_product_sliced",
+    "cheb_dm_product_sliced", "cheb_dm_sliced_ops_per_compute",
 ]
 
 
@@ -105,6 +105,7 @@ def lib():
     L.cheb_dm_solve_batch.argtypes = [vp, C.c_int, pp, dp, C.c_int, pp, dp, vp]
     L.cheb_dm_assemble.argtypes = [vp, C.c_int, dp, pp, vp]
     L.cheb_dm_flops_per_solve.argtypes = [vp, dp]
+    L.cheb_dm_sliced_ops_per_compute.argtypes = [vp, dp]
     L.cheb_dm_product_sliced.argtypes = [vp, C.c_double, vp, vp, C.c_double, vp, vp, C.c_int, vp]
     for n in EXPORTS:
         getattr(L, n).restype = C.c_int
@@ -303,6 +304,11 @@ class Plan:
 
     def product_sliced(self, alpha: float, dA: int, dB: int, beta: float, dC, d_out: int, symmetric: bool = False, stream: int = 0):
         _chk(lib().cheb_dm_product_sliced(self._h, alpha, dA, dB, beta, dC, d_out, 1 if symmetric else 0, stream), "cheb_dm_product_sliced")
+
+    def sliced_ops_per_compute(self) -> float:
+        v = C.c_double()
+        _chk(lib().cheb_dm_sliced_ops_per_compute(self._h, C.byref(v)), "cheb_dm_sliced_ops_per_compute")
+        return v.value
 
     def workspace_bytes(self) -> int:
         v = C.c_size_t()

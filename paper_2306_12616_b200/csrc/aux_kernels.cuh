@@ -418,6 +418,9 @@ __global__ void __launch_bounds__(256) diag_traces_kernel(const double* __restri
 }
 
 constexpr int GRAM_BLK = 32;
+// NB = 8-row blocks per side actually formed (4: a full 32 x 32 block of the Gram matrix; 2 or 1 when p - 1 and k - 1 are at
+// most 16 or 8: the padded blocks would cost as many DMMAs as the needed ones and make the pass tensor-bound)
+template <int NB>
 __global__ void __launch_bounds__(256) gram_kernel(const double* __restrict__ Tbase, const double* __restrict__ Ubase, long long stride,
                                                    long long slot_stride, long long nelem, int k, int p,
                                                    double* __restrict__ partial /* [slot][pass][cta][32*32] */) {
@@ -429,11 +432,11 @@ __global__ void __launch_bounds__(256) gram_kernel(const double* __restrict__ Tb
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, g = lane >> 2, t = lane & 3;
     const double* Ts = Tbase + (long long)slot * slot_stride;
     const double* Us = Ubase + (long long)slot * slot_stride;
-    const double* rowp[4];
-    const double* colp[4];
-    bool rowv[4], colv[4];
+    const double* rowp[NB];
+    const double* colp[NB];
+    bool rowv[NB], colv[NB];
 #pragma unroll
-    for (int mb = 0; mb < 4; ++mb) {
+    for (int mb = 0; mb < NB; ++mb) {
         const int r = rb * GRAM_BLK + mb * 8 + g;
         rowv[mb] = r < R;
         rowp[mb] = (r == 0 || !rowv[mb]) ? Ts + (long long)(k - 1) * stride : Us + (long long)(r - 1) * stride;  // U_1 = T_k
@@ -441,11 +444,11 @@ __global__ void __launch_bounds__(256) gram_kernel(const double* __restrict__ Tb
         colv[mb] = q < Cn;
         colp[mb] = Ts + (long long)(colv[mb] ? q : 0) * stride;
     }
-    double acc[4][4][2];
+    double acc[NB][NB][2];
 #pragma unroll
-    for (int i = 0; i < 4; ++i)
+    for (int i = 0; i < NB; ++i)
 #pragma unroll
-        for (int j = 0; j < 4; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
+        for (int j = 0; j < NB; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
     const long long nchunks = nelem / 8;                  // nelem = N ld, ld a multiple of 16
     const long long W = (long long)gridDim.x * 8, w = (long long)blockIdx.x * 8 + warp;
     const long long per = (nchunks + W - 1) / W;
@@ -453,16 +456,16 @@ __global__ void __launch_bounds__(256) gram_kernel(const double* __restrict__ Tb
 #pragma unroll 2
     for (long long ch = c0; ch < c1; ++ch) {
         const long long e = ch * 8 + 2 * t;
-        double2 a[4], b[4];
+        double2 a[NB], b[NB];
 #pragma unroll
-        for (int mb = 0; mb < 4; ++mb) {
+        for (int mb = 0; mb < NB; ++mb) {
             a[mb] = rowv[mb] ? __ldcs(reinterpret_cast<const double2*>(rowp[mb] + e)) : make_double2(0.0, 0.0);
             b[mb] = colv[mb] ? __ldcs(reinterpret_cast<const double2*>(colp[mb] + e)) : make_double2(0.0, 0.0);
         }
 #pragma unroll
-        for (int i = 0; i < 4; ++i)
+        for (int i = 0; i < NB; ++i)
 #pragma unroll
-            for (int j = 0; j < 4; ++j) {
+            for (int j = 0; j < NB; ++j) {
                 dmma_884(acc[i][j][0], acc[i][j][1], a[i].x, b[j].x);
                 dmma_884(acc[i][j][0], acc[i][j][1], a[i].y, b[j].y);
             }
@@ -473,9 +476,9 @@ __global__ void __launch_bounds__(256) gram_kernel(const double* __restrict__ Tb
     for (int wv = 0; wv < 8; ++wv) {
         if (warp == wv) {
 #pragma unroll
-            for (int i = 0; i < 4; ++i)
+            for (int i = 0; i < NB; ++i)
 #pragma unroll
-                for (int j = 0; j < 4; ++j) {
+                for (int j = 0; j < NB; ++j) {
                     s_acc[(i * 8 + g) * GRAM_BLK + j * 8 + 2 * t] += acc[i][j][0];
                     s_acc[(i * 8 + g) * GRAM_BLK + j * 8 + 2 * t + 1] += acc[i][j][1];
                 }
@@ -487,7 +490,7 @@ __global__ void __launch_bounds__(256) gram_kernel(const double* __restrict__ Tb
 }
 
 // traces: [slot][nmat] (T_1..T_k, U_2..U_{p-1}); partial: gram_kernel's output; gram: scratch [slot][(p-1)(k-1)].
-__global__ void __launch_bounds__(256) moments_kernel(const double* __restrict__ traces, int nmat, const double* __restrict__ partial,
+__global__ void __launch_bounds__(1024) moments_kernel(const double* __restrict__ traces, int nmat, const double* __restrict__ partial,
                                                       int nctas, int npasses, double* __restrict__ gram, int k, int p, int N,
                                                       double* __restrict__ tau_all) {
     const int slot = blockIdx.x;
@@ -496,15 +499,29 @@ __global__ void __launch_bounds__(256) moments_kernel(const double* __restrict__
     double* tau = tau_all + (size_t)slot * kp;
     double* G = gram + (size_t)slot * (size_t)(R > 0 ? R : 1) * (Cn > 0 ? Cn : 1);
     const double* tr = traces + (size_t)slot * nmat;
-    for (int e = threadIdx.x; e < R * Cn; e += blockDim.x) {
-        const int r = e / Cn, q = e - r * Cn;
-        const int pass = (r / GRAM_BLK) * npc + q / GRAM_BLK;
-        const double* src = partial + ((size_t)slot * npasses + pass) * nctas * (GRAM_BLK * GRAM_BLK) + (r % GRAM_BLK) * GRAM_BLK + q % GRAM_BLK;
+    // Gram entries across the threads of a quarter block (neighbouring entries are neighbouring addresses), the CTA partials
+    // split over the four quarters, combined in a fixed order
+    __shared__ dd s_q[4][256];
+    const int qtr = threadIdx.x >> 8, et = threadIdx.x & 255;
+    for (int e0 = 0; e0 < R * Cn; e0 += 256) {
+        const int e = e0 + et;
         dd s;
         s.hi = 0.0;
         s.lo = 0.0;
-        for (int cta = 0; cta < nctas; ++cta) s = dd_add_prod(s, src[(size_t)cta * (GRAM_BLK * GRAM_BLK)], 1.0);
-        G[e] = s.hi + s.lo;
+        if (e < R * Cn) {
+            const int r = e / Cn, q = e - r * Cn;
+            const int pass = (r / GRAM_BLK) * npc + q / GRAM_BLK;
+            const double* src = partial + ((size_t)slot * npasses + pass) * nctas * (GRAM_BLK * GRAM_BLK) + (r % GRAM_BLK) * GRAM_BLK + q % GRAM_BLK;
+            for (int cta = qtr; cta < nctas; cta += 4) s = dd_add_prod(s, __ldcs(src + (size_t)cta * (GRAM_BLK * GRAM_BLK)), 1.0);
+        }
+        s_q[qtr][et] = s;
+        __syncthreads();
+        if (qtr == 0 && e < R * Cn) {
+            dd v = s_q[0][et];
+            for (int g = 1; g < 4; ++g) v = dd_add(v, s_q[g][et]);
+            G[e] = v.hi + v.lo;
+        }
+        __syncthreads();
     }
     if (threadIdx.x == 0) tau[0] = (double)N;
     for (int n = 1 + threadIdx.x; n <= k && n < kp; n += blockDim.x) tau[n] = tr[n - 1];
@@ -543,37 +560,121 @@ __global__ void __launch_bounds__(128) mu_weights_kernel(const double* __restric
 struct BisectArgs {
     double n_occ[MAX_BATCH];
 };
-__global__ void __launch_bounds__(1024) mu_bisect_kernel(DevScalars* sc_all, double beta, const BisectArgs B, int iters,
-                                                         const double* __restrict__ costab, int Nq, const double* __restrict__ w_all) {
-    __shared__ dd s_buf[32];
+// Fermi function for the electron count of the bisection only: beyond |y| = 44 it is 0 or 1 to 8e-20, which changes
+// N_e = sum_j f_j w_j by less than 1e-14 (the coefficient tables keep the exact fermi_scaled); with beta~ of several
+// hundred only a few per cent of the N_q nodes then pay for an exp, and neighbouring nodes share a warp.
+__device__ __forceinline__ double fermi_count(double beta_t, double mu_t, double x) {
+    const double y = beta_t * (x - mu_t);
+    if (y > 44.0) return 0.0;
+    if (y < -44.0) return 1.0;
+    if (y > 0.0) {
+        const double e = exp(-y);
+        return e / (1.0 + e);
+    }
+    return 1.0 / (1.0 + exp(y));
+}
+
+// Three halvings per pass: the midpoints a bisection can visit in its next three steps form a binary tree of 7 points
+// (node 1 = mid(lo, hi); node 2c, 2c+1 = the midpoints of the two halves of node c's interval, computed with the same
+// expression 0.5 (lo + hi) the sequential bisection would use), N_e is evaluated at all 7 in one pass over the nodes and
+// one block reduction, and thread 0 then walks the tree with the sequential rule.  The result is bit-identical to one
+// halving per pass; the passes (block reduction latency, not the N_q Fermi values) drop from 101 to 35.
+constexpr int BISECT_LEVELS = 3, BISECT_POINTS = (1 << BISECT_LEVELS) - 1;
+// Work split of a pass: thread t evaluates point c = t % 8 (the eighth is idle) at the nodes j = t / 8, t / 8 + 64, ...:
+// the few nodes near mu that need an exp (an FP64 exp is ~1000 cycles of dependent instructions) are neighbours, so they
+// land on different threads and a pass costs one exp latency, not 7 x (nodes per thread) of them.
+__global__ void __launch_bounds__(512) mu_bisect_kernel(DevScalars* sc_all, double beta, const BisectArgs B, int iters,
+                                                        const double* __restrict__ costab, int Nq, const double* __restrict__ w_all) {
+    __shared__ dd s_part[8][16];
+    __shared__ double s_nepts[8];
     __shared__ double s_lo, s_hi, s_ne;
     DevScalars* sc = sc_all + blockIdx.x;
     const double* w = w_all + (size_t)blockIdx.x * Nq;
     const double n_occ = B.n_occ[blockIdx.x];
     const double a = sc->a, b = sc->b;
     const double beta_t = beta * (b - a) * 0.5;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nw = blockDim.x >> 5;
+    const int c = threadIdx.x & 7, grp = threadIdx.x >> 3, ngrp = blockDim.x >> 3;
     if (threadIdx.x == 0) { s_lo = a; s_hi = b; s_ne = 0.0; }
     __syncthreads();
-    for (int it = 0; it <= iters; ++it) {
-        const double lo = s_lo, hi = s_hi;
-        const double mid = 0.5 * (lo + hi);
-        const double mu_t = (2.0 * mid - (a + b)) / (b - a);
-        dd s;
-        s.hi = 0.0;
-        s.lo = 0.0;
-        for (int j = threadIdx.x; j < Nq; j += blockDim.x) s = dd_add_prod(s, fermi_scaled(beta_t, mu_t, costab[2 * j + 1]), w[j]);
-        s = dd_block_reduce(s, s_buf);
-        if (threadIdx.x == 0) {
-            const double ne = s.hi + s.lo;
-            if (it == iters) {
-                s_ne = ne;  // N_e at the returned mu = (lo+hi)/2
-            } else if (ne < n_occ) {
-                s_lo = mid;
-            } else {
-                s_hi = mid;
+    int done = 0;
+    while (done <= iters) {
+        // levels of this pass: up to 3 halvings; the last pass evaluates N_e at the returned mu only (one point)
+        const int levels = (done == iters) ? 1 : min(BISECT_LEVELS, iters - done);
+        const int npts = (1 << levels) - 1;
+        double lo_[BISECT_POINTS + 1], hi_[BISECT_POINTS + 1], mid[BISECT_POINTS + 1];
+        lo_[1] = s_lo;
+        hi_[1] = s_hi;
+#pragma unroll
+        for (int q = 1; q <= BISECT_POINTS; ++q) {
+            mid[q] = 0.5 * (lo_[q] + hi_[q]);
+            if (2 * q + 1 <= BISECT_POINTS) {
+                lo_[2 * q] = lo_[q];       hi_[2 * q] = mid[q];       // N_e(mid) >= n_occ: hi = mid
+                lo_[2 * q + 1] = mid[q];   hi_[2 * q + 1] = hi_[q];   // N_e(mid) <  n_occ: lo = mid
+            }
+        }
+        double my_mid = 0.0;
+#pragma unroll
+        for (int q = 1; q <= BISECT_POINTS; ++q)
+            if (q == c + 1) my_mid = mid[q];
+        const double mu_t = (2.0 * my_mid - (a + b)) / (b - a);
+        dd s, s1;  // two independent accumulation chains (a double-double step is ~100 cycles of dependent instructions)
+        s.hi = s.lo = s1.hi = s1.lo = 0.0;
+        if (c < npts) {
+            int j = grp;
+            for (; j + ngrp < Nq; j += 2 * ngrp) {
+                s = dd_add_prod(s, fermi_count(beta_t, mu_t, costab[2 * j + 1]), w[j]);
+                s1 = dd_add_prod(s1, fermi_count(beta_t, mu_t, costab[2 * (j + ngrp) + 1]), w[j + ngrp]);
+            }
+            if (j < Nq) s = dd_add_prod(s, fermi_count(beta_t, mu_t, costab[2 * j + 1]), w[j]);
+            s = dd_add(s, s1);
+        }
+        // fixed-order reduction per point: the 4 lanes of a warp with the same c, then the warps
+#pragma unroll
+        for (int o = 16; o >= 8; o >>= 1) {
+            dd other;
+            other.hi = __shfl_down_sync(0xffffffffu, s.hi, o);
+            other.lo = __shfl_down_sync(0xffffffffu, s.lo, o);
+            s = dd_add(s, other);
+        }
+        if (lane < 8) s_part[lane][warp] = s;
+        __syncthreads();
+        if (warp == 0) {
+            {   // lane (qq, c): warps 4 qq .. 4 qq + 3 of point c, then the four quarters (fixed order)
+                const int qq = lane >> 3;
+                dd v;
+                v.hi = v.lo = 0.0;
+                for (int q = 4 * qq; q < 4 * qq + 4 && q < nw; ++q) v = dd_add(v, s_part[c][q]);
+#pragma unroll
+                for (int o = 16; o >= 8; o >>= 1) {
+                    dd other;
+                    other.hi = __shfl_down_sync(0xffffffffu, v.hi, o);
+                    other.lo = __shfl_down_sync(0xffffffffu, v.lo, o);
+                    v = dd_add(v, other);
+                }
+                if (lane < 8) s_nepts[lane] = v.hi + v.lo;
+            }
+            __syncwarp();
+            if (lane == 0) {
+                if (done == iters) {
+                    s_ne = s_nepts[0];  // N_e at the returned mu = (lo + hi) / 2
+                } else {
+                    int q = 1;
+                    double lo = lo_[1], hi = hi_[1];
+                    for (int l = 0; l < levels; ++l) {
+                        double m_q = 0.0;   // select without dynamic indexing of the register array
+#pragma unroll
+                        for (int r = 1; r <= BISECT_POINTS; ++r)
+                            if (r == q) m_q = mid[r];
+                        if (s_nepts[q - 1] < n_occ) { lo = m_q; q = 2 * q + 1; } else { hi = m_q; q = 2 * q; }
+                    }
+                    s_lo = lo;
+                    s_hi = hi;
+                }
             }
         }
         __syncthreads();
+        done += (done == iters) ? 1 : levels;
     }
     if (threadIdx.x == 0) {
         sc->mu = 0.5 * (s_lo + s_hi);

@@ -863,12 +863,19 @@ cheb_dm_status_t blocks_and_moments(cheb_dm_plan_s* P, int nb, cudaStream_t st) 
                                                            (long long)P->mat_elems, (long long)P->slot_elems, P->ld, P->N, k, P->traces, P->ntrmat);
     ++P->last_launches;
     if (p >= 2 && k >= 2) {
-        gram_kernel<<<dim3(P->gram_ctas, P->gram_passes, nb), 256, 0, st>>>(T_ptr(P, 0, 1), P->off_U >= 0 ? mat_ptr(P, 0, P->off_U) : T_ptr(P, 0, 1),
-                                                                           (long long)P->mat_elems, (long long)P->slot_elems,
-                                                                           (long long)P->N * P->ld, k, p, P->gram_part);
+        const double* Tb = T_ptr(P, 0, 1);
+        const double* Ub = P->off_U >= 0 ? mat_ptr(P, 0, P->off_U) : T_ptr(P, 0, 1);
+        const dim3 ggrid(P->gram_ctas, P->gram_passes, nb);
+        const int side = (p - 1 > k - 1) ? p - 1 : k - 1;
+        if (side <= 8)
+            gram_kernel<1><<<ggrid, 256, 0, st>>>(Tb, Ub, (long long)P->mat_elems, (long long)P->slot_elems, (long long)P->N * P->ld, k, p, P->gram_part);
+        else if (side <= 16)
+            gram_kernel<2><<<ggrid, 256, 0, st>>>(Tb, Ub, (long long)P->mat_elems, (long long)P->slot_elems, (long long)P->N * P->ld, k, p, P->gram_part);
+        else
+            gram_kernel<4><<<ggrid, 256, 0, st>>>(Tb, Ub, (long long)P->mat_elems, (long long)P->slot_elems, (long long)P->N * P->ld, k, p, P->gram_part);
         ++P->last_launches;
     }
-    moments_kernel<<<nb, 256, 0, st>>>(P->traces, P->ntrmat, P->gram_part, P->gram_ctas, P->gram_passes, P->gram, k, p, P->N, P->tau);
+    moments_kernel<<<nb, 1024, 0, st>>>(P->traces, P->ntrmat, P->gram_part, P->gram_ctas, P->gram_passes, P->gram, k, p, P->N, P->tau);
     ++P->last_launches;
     CUDA_TRY(cudaGetLastError());
     return CHEB_DM_OK;
@@ -879,7 +886,7 @@ cheb_dm_status_t bisect(cheb_dm_plan_s* P, int nb, double beta, const double* n_
     memset(&ba, 0, sizeof(ba));
     for (int s = 0; s < nb; ++s) ba.n_occ[s] = n_occ[s];
     mu_weights_kernel<<<dim3(P->Nq, nb), 128, 0, st>>>(P->tau, P->costab, P->Nq, P->M, P->k * P->p, P->w);
-    mu_bisect_kernel<<<nb, 1024, 0, st>>>(P->sc, beta, ba, iters, P->costab, P->Nq, P->w);
+    mu_bisect_kernel<<<nb, 512, 0, st>>>(P->sc, beta, ba, iters, P->costab, P->Nq, P->w);
     P->last_launches += 2;
     CUDA_TRY(cudaGetLastError());
     return CHEB_DM_OK;
@@ -1474,6 +1481,15 @@ cheb_dm_status_t cheb_dm_last_launch_count(cheb_dm_plan_t P, int* launches_out) 
 cheb_dm_status_t cheb_dm_flops_per_compute(cheb_dm_plan_t P, double* flops_out) {
     if (!P || !flops_out) return CHEB_DM_EINVAL;
     *flops_out = P->flops_per_compute;
+    return CHEB_DM_OK;
+}
+
+cheb_dm_status_t cheb_dm_sliced_ops_per_compute(cheb_dm_plan_t P, double* ops_out) {
+    if (!P || !ops_out) return CHEB_DM_EINVAL;
+    if (!P->oz_solve) return CHEB_DM_EUNSUPPORTED;
+    const double S = (double)P->oz_S;
+    const double products = (double)P->baby.ntl + (double)(P->p > 1 ? P->p - 1 : 0);
+    *ops_out = products * (S * (S + 1.0) / 2.0) * 2.0 * (double)P->oz_ntiles[P->sym ? 1 : 0] * OZ_BM * OZ_BN * (double)P->oz_kpad;
     return CHEB_DM_OK;
 }
 

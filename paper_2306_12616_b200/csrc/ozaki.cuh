@@ -84,9 +84,10 @@ __host__ __device__ constexpr uint32_t oz_idesc(int n) {
 // ---------------------------------------------------------------------------------------------------
 // Slicing: one warp per row.  digits[s][row][k] (int8, row pitch kpad, zero beyond N), scale[row] = 2^{e_row}.
 // ---------------------------------------------------------------------------------------------------
-// corr[row] = sum_k sum_{s+t >= S} 2^{-7(s+t)} q_s[row][k] q_t[row][k]: the digit products the GEMM drops, for the DIAGONAL of
-// an exact square A A^T.  Off the diagonal, and between different matrices, the dropped products are incoherent sums of
-// magnitude sqrt(K) 2^{-7S}; on the diagonal of a square the s = t terms are sums of squares, a bias of K 64^2/3 2^{-7S}
+// corr[row] = sum_k sum_{2s >= S} 2^{-14 s} q_s[row][k]^2: the coherent part of the digit products the GEMM drops, for the
+// DIAGONAL of an exact square A A^T.  Off the diagonal, between different matrices, and between different digit levels of
+// one element, the dropped products are incoherent sums of magnitude sqrt(K) 2^{-7S}; on the diagonal of a square the
+// s = t terms are sums of squares, a bias of K 64^2/3 2^{-7S}
 // that the squaring chain T_2 -> T_4 -> ... -> T_k amplifies by 4 per doubling (measured at N = 5000, k = 32: |dtr D| = 9.5e-8
 // without this term).  The epilogue adds it back when both factors are the same digit set.
 __global__ void __launch_bounds__(256) oz_split_kernel(const double* __restrict__ A, long long lda, int N, int S, int8_t* __restrict__ digits,
@@ -94,8 +95,18 @@ __global__ void __launch_bounds__(256) oz_split_kernel(const double* __restrict_
     const int warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
     if (warp >= N) return;
     const double* row = A + (long long)warp * lda;
+    // 16-byte loads need an even leading dimension and an aligned base (plan-owned matrices; a caller's odd N falls back)
+    const bool vec = ((lda & 1) == 0) && ((reinterpret_cast<uintptr_t>(A) & 15) == 0);
     double m = 0.0;
-    for (int k = lane; k < N; k += 32) m = fmax(m, fabs(row[k]));
+    if (vec) {
+        for (int k = 2 * lane; k < N; k += 64) {
+            const double2 v = *reinterpret_cast<const double2*>(row + k);
+            m = fmax(m, fabs(v.x));
+            if (k + 1 < N) m = fmax(m, fabs(v.y));
+        }
+    } else {
+        for (int k = lane; k < N; k += 32) m = fmax(m, fabs(row[k]));
+    }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) m = fmax(m, __shfl_xor_sync(0xffffffffu, m, o));
     int e = 0;
@@ -105,30 +116,31 @@ __global__ void __launch_bounds__(256) oz_split_kernel(const double* __restrict_
     if (lane == 0) scale[warp] = ldexp(1.0, e);
     const long long plane = (long long)N * kpad;
     double w = 0.0;
-    for (long long k = lane; k < kpad; k += 32) {
-        double t = (k < N) ? ldexp(row[k], 6 - e) : 0.0;   // |t| < 64
-        int8_t* dst = digits + (long long)warp * kpad + k;
-        double q[OZ_MAX_S];
+    // two consecutive elements per lane and pass: whole 32-byte sectors per digit plane (kpad is a multiple of 64)
+    for (long long k0 = 2 * lane; k0 < kpad; k0 += 64) {
+        double x0 = 0.0, x1 = 0.0;
+        if (vec && k0 + 1 < N) {
+            const double2 v = *reinterpret_cast<const double2*>(row + k0);
+            x0 = v.x;
+            x1 = v.y;
+        } else {
+            if (k0 < N) x0 = row[k0];
+            if (k0 + 1 < N) x1 = row[k0 + 1];
+        }
+        double t0 = ldexp(x0, 6 - e), t1 = ldexp(x1, 6 - e);   // |t| < 64
+        int8_t* dst = digits + (long long)warp * kpad + k0;
+        double wt = 0.0;                                        // Horner in 2^-14 over the squared digits s >= S / 2
 #pragma unroll
         for (int s = 0; s < OZ_MAX_S; ++s) {
-            q[s] = 0.0;
             if (s < S) {
-                q[s] = rint(t);
-                dst[(long long)s * plane] = (int8_t)(int)q[s];
-                t = (t - q[s]) * 128.0;                     // exact: |t - q| <= 1/2
+                const double q0 = rint(t0), q1 = rint(t1);
+                t0 = (t0 - q0) * 128.0;                         // exact: |t - q| <= 1/2
+                t1 = (t1 - q1) * 128.0;
+                *reinterpret_cast<char2*>(dst + (long long)s * plane) = make_char2((signed char)(int)q0, (signed char)(int)q1);
+                if (2 * s >= S) wt += ldexp(q0 * q0 + q1 * q1, -14 * s);
             }
         }
-        // dropped digit products of this element with itself, least significant first
-#pragma unroll
-        for (int d = 2 * OZ_MAX_S - 2; d >= 0; --d) {
-            double pd = 0.0;
-#pragma unroll
-            for (int s2 = 0; s2 < OZ_MAX_S; ++s2) {
-                const int t2 = d - s2;
-                if (t2 >= 0 && t2 < OZ_MAX_S) pd += q[s2] * q[t2];
-            }
-            if (d >= S) w += ldexp(pd, -7 * d);
-        }
+        w += wt;
     }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) w += __shfl_xor_sync(0xffffffffu, w, o);
