@@ -123,6 +123,20 @@ class ClockSampler:
     def end(self):
         self.regions.append((self._t0, time.perf_counter()))
 
+    def window(self, t0, t1):
+        """Clocks inside one wall-clock window (the timed region of one arm)."""
+        if not self.ok:
+            return None
+        inside = [x for x in self.samples if t0 <= x[0] <= t1]
+        if not inside:
+            return None
+        sm = sorted(x[1] for x in inside)
+        mask = 0
+        for x in inside:
+            mask |= x[2]
+        return {"sm_mhz": sm[len(sm) // 2], "sm_min_mhz": sm[0], "power_w_max": max(x[3] for x in inside), "samples": len(inside),
+                "reasons": [n for bit, n in self.REASONS.items() if mask & bit]}
+
     def summary(self):
         if not self.ok:
             return {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "note": "NVML unavailable"}
@@ -273,7 +287,7 @@ def job_value(world, units_per_step, steps, max_ms):
     return world * units_per_step * steps / (max_ms * 1e-3)
 
 
-def measure_sliced(torch, cd, workloads, name, args, steps, warmup, flush, dist, world, int8_peak):
+def measure_sliced(torch, cd, workloads, name, args, steps, warmup, flush, dist, world, int8_peak, sampler=None):
     """The same fixed-mu step with every product on the sliced int8 tensor path (tcgen05 kind::i8, plan option
     sliced_solve): solves/s, and the digit GEMMs' executed int8 operations against the int8 tensor peak."""
     import copy
@@ -286,7 +300,9 @@ def measure_sliced(torch, cd, workloads, name, args, steps, warmup, flush, dist,
         w.step()
     torch.cuda.synchronize()
     plan.set_timing(True)
+    t_w0 = time.perf_counter()
     total_ms = timed_steps(torch, w.step, steps, 0, flush, None, dist)
+    t_w1 = time.perf_counter()
     n_rec, prod_ms = plan.product_ms()
     plan.set_timing(False)
     plan.check(w.st)
@@ -304,7 +320,8 @@ def measure_sliced(torch, cd, workloads, name, args, steps, warmup, flush, dist,
                         "achieved": achieved, "peak": int8_peak, "unit": "TOP/s", "frac": achieved / int8_peak if int8_peak else None,
                         "peak_source": "MEASURED_PEAKS.json bf16_tflops (burst) x 2 (nominal int8 : bf16 ratio of the profiling guide)",
                         "kernel_ms": kernel_ms, "ops_per_launch": ops, "note": "kernel_ms spans all product launches of a solve, slicing passes and the sums pass included"},
-           "gpu_launches_per_step": w.launches_per_step, "workspace_bytes": plan.workspace_bytes()}
+           "gpu_launches_per_step": w.launches_per_step, "workspace_bytes": plan.workspace_bytes(),
+           "clocks": sampler.window(t_w0, t_w1) if sampler else None}
     plan.destroy()
     del w
     torch.cuda.empty_cache()
@@ -320,7 +337,9 @@ def measure_workload(torch, cd, workloads, name, args, steps, warmup, flush, sam
         w.step()
     torch.cuda.synchronize()
     plan.set_timing(True)  # resets the ring after warm-up
+    t_w0 = time.perf_counter()
     total_ms = timed_steps(torch, w.step, steps, 0, flush, sampler, dist)
+    t_w1 = time.perf_counter()
     n_rec, prod_ms = plan.product_ms()  # the timed compute calls only (at most the last 256 of them)
     plan.set_timing(False)
     plan.check(w.st)                     # sticky device flags of the whole timed region
@@ -369,6 +388,7 @@ def measure_workload(torch, cd, workloads, name, args, steps, warmup, flush, sam
                          "products": plan.k + 2 * plan.p - 4, "tr_D": tr_D_mi},
         "mu": w.mu, "tr_D": tr_D, "N_occ": w.cfg.N_occ, "seeds": list(w.seeds),
         "workspace_bytes": plan.workspace_bytes(),
+        "clocks": sampler.window(t_w0, t_w1) if sampler else None,
     }
     plan.destroy()
     del w
@@ -527,7 +547,7 @@ def main():
         others.append(measure_workload(torch, cd, workloads, name, args, k_steps, 3, flush, sampler, dist, peak_tf, world))
         if big and not args.sliced:
             # N >= 2000: the same step with the products on the sliced int8 tensor path, reported beside it
-            others[-1]["sliced_int8"] = measure_sliced(torch, cd, workloads, name, args, k_steps, 3, flush, dist, world, int8_peak)
+            others[-1]["sliced_int8"] = measure_sliced(torch, cd, workloads, name, args, k_steps, 3, flush, dist, world, int8_peak, sampler)
     peak_after = cd.dmma_peak(40000, st)
     # sustained DMMA peak: the same microbenchmark back to back for ~2 s (clocks settle under the power cap)
     t_end = time.perf_counter() + 2.0

@@ -998,7 +998,7 @@ cheb_dm_status_t prepare_sliced(cheb_dm_plan_s* P) {
 // Digits of an FP64 matrix (leading dimension ld) into digit set `set`.
 cheb_dm_status_t oz_split(cheb_dm_plan_s* P, int set, const double* src, long long ld, cudaStream_t st) {
     const size_t plane = (size_t)P->N * (size_t)P->oz_kpad;
-    oz_split_kernel<<<ceil_div(P->N * 32, 256), 256, 0, st>>>(src, ld, P->N, P->oz_S, P->oz_digits + (size_t)set * P->oz_S * plane, P->oz_kpad,
+    oz_split_kernel<<<P->N, 256, 0, st>>>(src, ld, P->N, P->oz_S, P->oz_digits + (size_t)set * P->oz_S * plane, P->oz_kpad,
                                                               P->oz_scale + (size_t)set * P->N, P->oz_scale + (size_t)(P->oz_nsets + set) * P->N);
     CUDA_TRY(cudaGetLastError());
     return CHEB_DM_OK;

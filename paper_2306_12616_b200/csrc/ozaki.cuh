@@ -82,7 +82,7 @@ __host__ __device__ constexpr uint32_t oz_idesc(int n) {
 }
 
 // ---------------------------------------------------------------------------------------------------
-// Slicing: one warp per row.  digits[s][row][k] (int8, row pitch kpad, zero beyond N), scale[row] = 2^{e_row}.
+// Slicing: one block per row.  digits[s][row][k] (int8, row pitch kpad, zero beyond N), scale[row] = 2^{e_row}.
 // ---------------------------------------------------------------------------------------------------
 // corr[row] = sum_k sum_{2s >= S} 2^{-14 s} q_s[row][k]^2: the coherent part of the digit products the GEMM drops, for the
 // DIAGONAL of an exact square A A^T.  Off the diagonal, between different matrices, and between different digit levels of
@@ -92,32 +92,41 @@ __host__ __device__ constexpr uint32_t oz_idesc(int n) {
 // without this term).  The epilogue adds it back when both factors are the same digit set.
 __global__ void __launch_bounds__(256) oz_split_kernel(const double* __restrict__ A, long long lda, int N, int S, int8_t* __restrict__ digits,
                                                        long long kpad, double* __restrict__ scale, double* __restrict__ corr) {
-    const int warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
-    if (warp >= N) return;
-    const double* row = A + (long long)warp * lda;
+    // one block per row (a row is read twice -- maximum, then digits -- and with a warp per row the rows in flight
+    // exceeded the L2: measured 390 MB of DRAM reads for a 200 MB matrix)
+    __shared__ double s_red[8];
+    __shared__ int s_e;
+    const int r = blockIdx.x, lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    const double* row = A + (long long)r * lda;
     // 16-byte loads need an even leading dimension and an aligned base (plan-owned matrices; a caller's odd N falls back)
     const bool vec = ((lda & 1) == 0) && ((reinterpret_cast<uintptr_t>(A) & 15) == 0);
     double m = 0.0;
     if (vec) {
-        for (int k = 2 * lane; k < N; k += 64) {
+        for (int k = 2 * threadIdx.x; k < N; k += 512) {
             const double2 v = *reinterpret_cast<const double2*>(row + k);
             m = fmax(m, fabs(v.x));
             if (k + 1 < N) m = fmax(m, fabs(v.y));
         }
     } else {
-        for (int k = lane; k < N; k += 32) m = fmax(m, fabs(row[k]));
+        for (int k = threadIdx.x; k < N; k += 256) m = fmax(m, fabs(row[k]));
     }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) m = fmax(m, __shfl_xor_sync(0xffffffffu, m, o));
-    int e = 0;
-    if (m > 0.0 && isfinite(m)) {
-        (void)frexp(m, &e);                 // m = f 2^e, f in [0.5, 1)  =>  |a| 2^-e < 1
+    if (lane == 0) s_red[wid] = m;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        for (int q = 1; q < 8; ++q) m = fmax(m, s_red[q]);
+        int e = 0;
+        if (m > 0.0 && isfinite(m)) (void)frexp(m, &e);   // m = f 2^e, f in [0.5, 1)  =>  |a| 2^-e < 1
+        s_e = e;
+        scale[r] = ldexp(1.0, e);
     }
-    if (lane == 0) scale[warp] = ldexp(1.0, e);
+    __syncthreads();
+    const int e = s_e;
     const long long plane = (long long)N * kpad;
     double w = 0.0;
-    // two consecutive elements per lane and pass: whole 32-byte sectors per digit plane (kpad is a multiple of 64)
-    for (long long k0 = 2 * lane; k0 < kpad; k0 += 64) {
+    // two consecutive elements per thread and pass: whole 32-byte sectors per digit plane (kpad is a multiple of 64)
+    for (long long k0 = 2 * threadIdx.x; k0 < kpad; k0 += 512) {
         double x0 = 0.0, x1 = 0.0;
         if (vec && k0 + 1 < N) {
             const double2 v = *reinterpret_cast<const double2*>(row + k0);
@@ -128,8 +137,8 @@ __global__ void __launch_bounds__(256) oz_split_kernel(const double* __restrict_
             if (k0 + 1 < N) x1 = row[k0 + 1];
         }
         double t0 = ldexp(x0, 6 - e), t1 = ldexp(x1, 6 - e);   // |t| < 64
-        int8_t* dst = digits + (long long)warp * kpad + k0;
-        double wt = 0.0;                                        // Horner in 2^-14 over the squared digits s >= S / 2
+        int8_t* dst = digits + (long long)r * kpad + k0;
+        double wt = 0.0;
 #pragma unroll
         for (int s = 0; s < OZ_MAX_S; ++s) {
             if (s < S) {
@@ -144,7 +153,13 @@ __global__ void __launch_bounds__(256) oz_split_kernel(const double* __restrict_
     }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) w += __shfl_xor_sync(0xffffffffu, w, o);
-    if (lane == 0) corr[warp] = w;
+    __syncthreads();
+    if (lane == 0) s_red[wid] = w;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        for (int q = 1; q < 8; ++q) w += s_red[q];
+        corr[r] = w;
+    }
 }
 
 struct OzArgs {
@@ -173,16 +188,19 @@ __global__ void __launch_bounds__(OZ_THREADS, 1) oz_gemm_kernel(const __grid_con
                                                                 const OzArgs args) {
     extern __shared__ uint8_t smem_raw[];
     uint8_t* smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
-    const uint32_t stage_bytes = (uint32_t)S * (OZ_A_TILE + OZ_B_TILE);
     const uint32_t ring_bytes = OZ_STAGES * OZ_MAX_S * (OZ_A_TILE + OZ_B_TILE);
     uint64_t* bars = reinterpret_cast<uint64_t*>(smem + ring_bytes);
     uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(smem + ring_bytes + 64);
     const uint32_t smem_base = smem_u32(smem);
     const uint32_t bar_base = smem_u32(bars);
+    // (Releasing and refilling a stage in S sub-slots -- the A tile of digit s with the B tile of digit S-1-s, both dead
+    // after the MMAs of digit s -- was measured 2.5 % SLOWER than whole-stage barriers: the kernel runs at the board's
+    // power limit, SM clock ~1.78 GHz under ncu, not at a pipeline bubble.)
     auto full_bar = [&](int s) { return bar_base + 8u * s; };
     auto empty_bar = [&](int s) { return bar_base + 8u * (OZ_STAGES + s); };
     const uint32_t tfull_bar = bar_base + 8u * (2 * OZ_STAGES);
     const uint32_t tempty_bar = tfull_bar + 8u;
+    const uint32_t stage_bytes = (uint32_t)S * (OZ_A_TILE + OZ_B_TILE);
     auto a_tile = [&](int stage, int s) { return smem_base + (uint32_t)stage * (OZ_MAX_S * (OZ_A_TILE + OZ_B_TILE)) + (uint32_t)s * OZ_A_TILE; };
     auto b_tile = [&](int stage, int t) { return smem_base + (uint32_t)stage * (OZ_MAX_S * (OZ_A_TILE + OZ_B_TILE)) + OZ_MAX_S * OZ_A_TILE + (uint32_t)t * OZ_B_TILE; };
 
