@@ -138,7 +138,7 @@ typedef struct {
 } cheb_dm_options_t;
 
 /* Create a plan for N x N matrices and an M_terms-term expansion.  Chooses (k,p), allocates the
- * workspace ((k+2) padded matrices, + p when the low-order sums are parked, + scalar tables) and builds the
+ * workspace (per slot k+3 padded matrices, + p when the low-order sums are parked, + p-2 for the giant block, + scalar tables) and builds the
  * product/tile/dependency tables.
  * plan: host pointer, receives the handle.  EINVAL: N<1, M_terms<1, k*p<M; EUNSUPPORTED: dtype. */
 cheb_dm_status_t cheb_dm_plan(cheb_dm_plan_t* plan, int N, int M_terms, cheb_dm_dtype_t dtype);

@@ -126,6 +126,8 @@ struct cheb_dm_plan_s {
     int preformed;       // 1: low-order sums G_l are formed by form_sums_kernel before the giant steps
     int sym;             // 1: symmetric-tile skipping in gemm_dmma_kernel
     int* sym_first;      // device: [tiles_n + 1] item prefix sums of a symmetric task
+    int* sym_panel_target;  // device: [tiles_n] tiles of a symmetric task that write into a column panel (own + mirrored)
+    int panel_sym;       // 1: symmetric giant / chain steps wait per column panel (BM a multiple of BN)
     int resident;        // 1: single solves run their giant steps in giant_resident_kernel (small N)
     int moments_on;      // 1: the workspace holds the G and U blocks (cheb_dm_moments / solve / assemble)
     int res_tiles_m, res_tiles_n, res_grid, res_smem;
@@ -179,7 +181,8 @@ namespace {
 // ---- workspace layout: matrix m of slot s ----
 double* mat_ptr(const cheb_dm_plan_s* P, int s, int m) { return P->ws + (size_t)s * P->slot_elems + (size_t)m * P->mat_elems; }
 double* T_ptr(const cheb_dm_plan_s* P, int s, int n) { return mat_ptr(P, s, n - 1); }             // T_n, 1 <= n <= k
-double* buf_ptr(const cheb_dm_plan_s* P, int s, int i) { return mat_ptr(P, s, P->k + i); }        // ping-pong buffers
+constexpr int NBUF = 3;  // rotating giant-step buffers: B_l lives in buffer l % 3 (see build_tables)
+double* buf_ptr(const cheb_dm_plan_s* P, int s, int i) { return mat_ptr(P, s, P->k + i); }        // giant-step buffers
 double* G_ptr(const cheb_dm_plan_s* P, int s, int l) { return mat_ptr(P, s, P->off_G + l); }      // G_l, 0 <= l < p
 double* U_ptr(const cheb_dm_plan_s* P, int s, int j) {                                            // U_j = T_j(T_k), 1 <= j <= p-1
     return j == 1 ? T_ptr(P, s, P->k) : mat_ptr(P, s, P->off_U + j - 2);
@@ -401,9 +404,15 @@ void build_tables(cheb_dm_plan_s* P) {
     // ---- giant steps ----
     // CHEBYSHEV: B_l = G_l + 2 Y B_{l+1} - B_{l+2} (l = p-1..1), D = G_0 + Y B_1 - B_2, G_l = sum_i g_{i,l} T_i.
     // POWER    : acc_j = S_j + Y acc_{j+1} (Eq. 4), S_j = sum_i d_{i,j} T_i (Eq. 21).
-    // B_l / acc_l lives in buf[l & 1]; Y = T_k.  Without symmetric tiles the column panels of successive steps are
-    // independent chains (step l only waits for the SAME column panel of step l+1: DEP_PANEL_N).  The baby block is
-    // complete when this table is launched (stream order).
+    // B_l / acc_l lives in buf[l % 3]; Y = T_k.  Without symmetric tiles the column panels of successive steps are
+    // independent chains (step l only waits for the SAME column panel of step l+1: DEP_PANEL_N).  With symmetric tiles a
+    // column panel also receives the mirror of the row block(s) it crosses, so step l waits until everything step l+1
+    // writes into its panel is there (DEP_PANEL_SYM) -- the last wave of a step then overlaps the first of the next, and the
+    // publish -> poll -> TMA tail of a step is hidden for all but the last panels.  Three rotating buffers make that safe:
+    // step l writes buf[l % 3] (old content B_{l+3}), whose readers are step l+2 (as the streamed operand, any panel: hence
+    // the second dependency, on the whole of step l+2, which was claimed two levels earlier and never stalls in practice)
+    // and step l+1 (as C, own tile only: the tile of the same panel is complete, and mirror stores only go to tiles that are
+    // not work items, which nobody reads as C).  The baby block is complete when this table is launched (stream order).
     {
         const bool power = (P->opt.outer == CHEB_DM_OUTER_POWER);
         TaskTable& tt = P->giant;
@@ -419,10 +428,10 @@ void build_tables(cheb_dm_plan_s* P) {
                 const bool has_prod = (l + 1 <= p - 1);
                 if (has_prod) {
                     t.mapA = T_map(P, s, k);
-                    t.mapB = buf_map(P, s, (l + 1) & 1);
+                    t.mapB = buf_map(P, s, (l + 1) % NBUF);
                     t.alpha = (power || l == 0) ? 1.0 : 2.0;
                     if (!power && l + 2 <= p - 1) {
-                        t.C = buf_ptr(P, s, (l + 2) & 1);
+                        t.C = buf_ptr(P, s, (l + 2) % NBUF);
                         t.ldc = P->ld;
                         t.beta = -1.0;
                     }
@@ -432,7 +441,7 @@ void build_tables(cheb_dm_plan_s* P) {
                 if (l == 0) {
                     t.out_is_user = 1;
                 } else {
-                    t.Out = buf_ptr(P, s, l & 1);
+                    t.Out = buf_ptr(P, s, l % NBUF);
                     t.ldo = P->ld;
                 }
                 if (P->preformed) {
@@ -454,7 +463,14 @@ void build_tables(cheb_dm_plan_s* P) {
                 if (gsym) {
                     t.sym = 1;
                     t.nitems = stiles;
-                    if (has_prod) add_dep(t, DEP_TASK, idx(lt - 1, s), stiles);
+                    if (has_prod) {
+                        if (P->panel_sym) {
+                            add_dep(t, DEP_PANEL_SYM, idx(lt - 1, s), 0);
+                            if (lt >= 2) add_dep(t, DEP_TASK, idx(lt - 2, s), stiles);
+                        } else {
+                            add_dep(t, DEP_TASK, idx(lt - 1, s), stiles);
+                        }
+                    }
                 } else if (has_prod) {
                     add_dep(t, DEP_PANEL_N, idx(lt - 1, s), tiles_m);
                 }
@@ -488,7 +504,8 @@ void build_tables(cheb_dm_plan_s* P) {
                 t.ldo = P->ld;
                 t.sym = P->sym;
                 t.nitems = stiles;
-                if (j >= 2) add_dep(t, DEP_TASK, idx(lt - 1, s), stiles);
+                // U_{j+1} streams U_j (whole column panel) and reads its own tile of U_{j-1}; every U_j has its own matrix
+                if (j >= 2) add_dep(t, (P->sym && P->panel_sym) ? DEP_PANEL_SYM : DEP_TASK, idx(lt - 1, s), stiles);
                 tt.h[idx(lt, s)] = t;
             }
         }
@@ -576,7 +593,7 @@ cheb_dm_status_t encode_maps(cheb_dm_plan_s* P) {
         bool ok = true;
         for (int s = 0; s < P->maxb && ok; ++s) {
             CUtensorMap* hs = h.data() + (size_t)s * P->nmaps_slot;
-            for (int i = 0; i < P->k + 2 && ok; ++i) ok = encode_one(enc, P, hs + i, mat_ptr(P, s, i), want2d) == CHEB_DM_OK;
+            for (int i = 0; i < P->k + NBUF && ok; ++i) ok = encode_one(enc, P, hs + i, mat_ptr(P, s, i), want2d) == CHEB_DM_OK;
             if (P->moments_on)
                 for (int l = 1; l <= P->p - 1 && ok; ++l) {
                     ok = encode_one(enc, P, hs + P->map_flatA + l - 1, G_ptr(P, s, l), want2d) == CHEB_DM_OK &&
@@ -662,6 +679,7 @@ cheb_dm_status_t launch_tasks(cheb_dm_plan_s* P, const TaskTable& tt, int lt0, i
     la.ldD = ldD;
     la.tma2d = P->tma2d;
     la.sym_first = P->sym_first;
+    la.sym_panel_target = P->sym_panel_target;
     la.error_flag = P->counters;
     la.trace = P->trace_on ? P->trace_buf : nullptr;
     la.trace_base = tt.trace_base + lt0 * tt.items_per_task * nb;  // a table's region holds ntl * maxb * items records
@@ -948,7 +966,7 @@ bool batch_args_ok(const cheb_dm_plan_s* P, int nb, const double* const* A, doub
 // Digit planes, scales and TMA descriptors of cheb_dm_product_sliced.
 cheb_dm_status_t prepare_sliced(cheb_dm_plan_s* P) {
     const size_t plane = (size_t)P->N * (size_t)P->oz_kpad;
-    P->oz_nsets = (P->oz_solve ? P->k + 2 : 0) + 2;
+    P->oz_nsets = (P->oz_solve ? P->k + NBUF : 0) + 2;
     const size_t bytes = (size_t)P->oz_nsets * (size_t)P->oz_S * plane;
     if (cudaMalloc(&P->oz_digits, bytes) != cudaSuccess || cudaMalloc(&P->oz_scale, sizeof(double) * 2 * P->oz_nsets * P->N) != cudaSuccess) {
         cudaGetLastError();
@@ -1149,6 +1167,7 @@ cheb_dm_status_t cheb_dm_destroy(cheb_dm_plan_t P) {
     cudaFree(P->gram_part);
     cudaFree(P->gram);
     cudaFree(P->sym_first);
+    cudaFree(P->sym_panel_target);
     cudaFree(P->sc);
     cudaFree(P->maps);
     cudaFree(P->baby.d);
@@ -1243,6 +1262,7 @@ cheb_dm_status_t cheb_dm_plan_ex(cheb_dm_plan_t* plan, int N, int M_terms, cheb_
         P->scalar_sums = (env && env[0] == '1') ? 1 : 0;
     }
     choose_tile(P);
+    P->panel_sym = (P->sym && P->BM % P->BN == 0) ? 1 : 0;
     P->ld = ((long long)N + 15) / 16 * 16;
     P->mat_elems = (((size_t)N * (size_t)P->ld) + 127) / 128 * 128;
     // Giant steps of single solves in the resident-multiplier kernel: N <= 512 (32 rows of T_k fit in shared memory),
@@ -1281,13 +1301,13 @@ cheb_dm_status_t cheb_dm_plan_ex(cheb_dm_plan_t* plan, int N, int M_terms, cheb_
         P->opt.fuse_sums = 2;
     }
     const bool need_G = P->preformed || P->resident || P->moments_on;
-    P->off_G = need_G ? k + 2 : -1;
-    P->off_U = (P->moments_on && p >= 3) ? k + 2 + (need_G ? p : 0) : -1;
-    P->nmat = k + 2 + (need_G ? p : 0) + ((P->moments_on && p >= 3) ? p - 2 : 0);
+    P->off_G = need_G ? k + NBUF : -1;
+    P->off_U = (P->moments_on && p >= 3) ? k + NBUF + (need_G ? p : 0) : -1;
+    P->nmat = k + NBUF + (need_G ? p : 0) + ((P->moments_on && p >= 3) ? p - 2 : 0);
     P->slot_elems = (size_t)P->nmat * P->mat_elems;
-    P->map_flatA = k + 2;
-    P->map_flatB = k + 2 + (p - 1);
-    P->nmaps_slot = k + 2 + (P->moments_on ? 2 * (p - 1) : 0);
+    P->map_flatA = k + NBUF;
+    P->map_flatB = k + NBUF + (p - 1);
+    P->nmaps_slot = k + NBUF + (P->moments_on ? 2 * (p - 1) : 0);
     P->ntrmat = k + ((P->moments_on && p >= 3) ? p - 2 : 0);
     {
         const long long nchunks = (long long)N * P->ld / 8;
@@ -1299,7 +1319,7 @@ cheb_dm_status_t cheb_dm_plan_ex(cheb_dm_plan_t* plan, int N, int M_terms, cheb_
     }
     P->ws = nullptr; P->costab = P->fn = P->c = P->gT = P->dT = P->Amat = P->tau = P->w = P->one = P->part = nullptr;
     P->traces = P->gram_part = P->gram = nullptr;
-    P->sym_first = nullptr; P->sc = nullptr; P->maps = nullptr; P->counters = nullptr;
+    P->sym_first = nullptr; P->sym_panel_target = nullptr; P->sc = nullptr; P->maps = nullptr; P->counters = nullptr;
     P->have_coeffs = P->explicit_bounds = P->have_moments = P->computed = P->blocks_nb = 0;
     P->beta = P->mu = P->a = P->b = 0.0;
     P->last_launches = 0;
@@ -1381,6 +1401,22 @@ cheb_dm_status_t cheb_dm_plan_ex(cheb_dm_plan_t* plan, int N, int M_terms, cheb_
             }
             if (cudaMalloc(&P->sym_first, sizeof(int) * pf.size()) != cudaSuccess) { cudaGetLastError(); st = CHEB_DM_EALLOC; break; }
             if (cudaMemcpy(P->sym_first, pf.data(), sizeof(int) * pf.size(), cudaMemcpyHostToDevice) != cudaSuccess) { st = CHEB_DM_ECUDA; break; }
+            // column panel q of a symmetric result is written by the work items of panel q and, mirrored, by the work items
+            // (tm, tn != q) of the row block(s) tm whose rows cross the panel's columns: q in [tm R, tm R + R), R = BM / BN
+            std::vector<int> tg(tn_, 0);
+            if (P->panel_sym) {
+                const int R = P->BM / P->BN;
+                for (int tn = 0; tn < tn_; ++tn)
+                    for (int tm = sym_tm0(tn, P->BM, P->BN); tm < tm_; ++tm) {
+                        ++tg[tn];
+                        for (int u = 0; u < R; ++u) {
+                            const int q = tm * R + u;
+                            if (q != tn && q < tn_) ++tg[q];
+                        }
+                    }
+            }
+            if (cudaMalloc(&P->sym_panel_target, sizeof(int) * tg.size()) != cudaSuccess) { cudaGetLastError(); st = CHEB_DM_EALLOC; break; }
+            if (cudaMemcpy(P->sym_panel_target, tg.data(), sizeof(int) * tg.size(), cudaMemcpyHostToDevice) != cudaSuccess) { st = CHEB_DM_ECUDA; break; }
         }
         st = encode_maps(P);
         if (st != CHEB_DM_OK) break;

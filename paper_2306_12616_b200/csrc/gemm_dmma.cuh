@@ -32,7 +32,10 @@ constexpr int TILE_RING = 2;            // producer run-ahead (tile descriptors 
 constexpr int MAX_DEPS = 4;
 constexpr long long WATCHDOG_CLOCKS = 8000000000ll;
 
-enum DepKind : int { DEP_NONE = 0, DEP_TASK = 1, DEP_PANEL_N = 2 };
+// DEP_TASK: every tile of a task; DEP_PANEL_N: the tiles of one column panel of a task (non-symmetric tasks: a panel is
+// written by its own tiles only); DEP_PANEL_SYM: everything a SYMMETRIC task writes into one column panel -- its own tiles
+// plus the tiles of the row block(s) whose mirror lands there (target: LaunchArgs::sym_panel_target[panel]).
+enum DepKind : int { DEP_NONE = 0, DEP_TASK = 1, DEP_PANEL_N = 2, DEP_PANEL_SYM = 3 };
 
 struct Task {
     // operands (indices into the tensor-map table); ktiles == 0 => no product, epilogue only
@@ -90,6 +93,7 @@ struct LaunchArgs {
     long long ldD;
     int tma2d;               // 1: operand maps are 2-D {column, row} with one 16-column box per copy
     const int* sym_first;    // [tiles_n + 1] prefix sums of the per-panel item counts of a symmetric task
+    const int* sym_panel_target;  // [tiles_n] completion count of a column panel of a symmetric task (DEP_PANEL_SYM)
     int* error_flag;         // set to 1 if a dependency wait exceeds the watchdog (never in a correct run)
     TraceRec* trace;         // nullable: per-item timeline, indexed by trace_base + work item of the launch
     int trace_base;
@@ -163,6 +167,24 @@ __device__ __forceinline__ void wait_counter(const int* ctr, int target, int* er
     (void)ld_acquire_gpu(ctr);
 }
 
+// Completion counters of a finished tile (after the gpu-scope fence): its column panel, the task, and -- symmetric task
+// with BM a multiple of BN -- the column panel(s) its mirror lands in (the columns of the mirror are the rows of the tile).
+template <int BM, int BN>
+__device__ __forceinline__ void publish_tile(const LaunchArgs& args, const TileInfo& ti) {
+    int* pd = args.panel_done + (size_t)ti.task * args.panel_stride;
+    red_relaxed_gpu_add(pd + ti.tn, 1);
+    if (BM % BN == 0 && args.tasks[ti.task].sym) {
+        constexpr int R = (BM % BN == 0) ? BM / BN : 1;
+        const int tiles_n = args.tasks[ti.task].tiles_n;
+#pragma unroll
+        for (int u = 0; u < R; ++u) {
+            const int q = ti.tm * R + u;
+            if (q != ti.tn && q < tiles_n) red_relaxed_gpu_add(pd + q, 1);
+        }
+    }
+    red_relaxed_gpu_add(args.task_done + ti.task, 1);
+}
+
 template <class Cfg>
 __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MIN_CTAS) gemm_dmma_kernel(const LaunchArgs args) {
     constexpr int BM = Cfg::BM, BN = Cfg::BN, BK = Cfg::BK, STAGES = Cfg::STAGES;
@@ -225,13 +247,15 @@ __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MIN_CTAS) gemm_dmma_kernel(
                 const int kind = tk->dep_kind[d], idx = tk->dep_idx[d], target = tk->dep_target[d];
                 const int rel = idx - tbase;
                 const int* ctr;
+                int tgt = target;
                 if (kind == DEP_TASK) {
                     if (rel >= 0 && rel < 512 && ((done_tasks[rel >> 6] >> (rel & 63)) & 1ull)) return;
                     ctr = args.task_done + idx;
                 } else {
                     ctr = args.panel_done + (size_t)idx * args.panel_stride + tn;
+                    if (kind == DEP_PANEL_SYM) tgt = __ldg(args.sym_panel_target + tn);
                 }
-                wait_counter(ctr, target, args.error_flag);
+                wait_counter(ctr, tgt, args.error_flag);
                 if (kind == DEP_TASK && rel >= 0 && rel < 512) done_tasks[rel >> 6] |= 1ull << (rel & 63);
             };
             for (;;) {
@@ -334,8 +358,7 @@ __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MIN_CTAS) gemm_dmma_kernel(
                 if (!ti.stop) {
                     mbar_wait(stored_bar(tslot), tphase);  // slot s is used once per ring cycle: same phase as its descriptor
                     fence_acq_rel_gpu();
-                    red_relaxed_gpu_add(args.panel_done + (size_t)ti.task * args.panel_stride + ti.tn, 1);
-                    red_relaxed_gpu_add(args.task_done + ti.task, 1);
+                    publish_tile<BM, BN>(args, ti);
                     if (args.trace != nullptr) {
                         TraceRec r;
                         r.task = ti.task; r.tm = ti.tm; r.tn = ti.tn; r.sm = sm_id();

@@ -124,13 +124,15 @@ __global__ void __launch_bounds__(Cfg::THREADS, 1) gemm_epi_kernel(const LaunchA
             const int kind = tk->dep_kind[d], idx = tk->dep_idx[d], target = tk->dep_target[d];
             const int rel = idx - tbase;
             const int* ctr;
+            int tgt = target;
             if (kind == DEP_TASK) {
                 if (rel >= 0 && rel < 512 && ((done_tasks[rel >> 6] >> (rel & 63)) & 1ull)) return;
                 ctr = args.task_done + idx;
             } else {
                 ctr = args.panel_done + (size_t)idx * args.panel_stride + tn;
+                if (kind == DEP_PANEL_SYM) tgt = __ldg(args.sym_panel_target + tn);
             }
-            wait_counter(ctr, target, args.error_flag);
+            wait_counter(ctr, tgt, args.error_flag);
             if (kind == DEP_TASK && rel >= 0 && rel < 512) done_tasks[rel >> 6] |= 1ull << (rel & 63);
         };
         for (;;) {
@@ -383,8 +385,7 @@ __global__ void __launch_bounds__(Cfg::THREADS, 1) gemm_epi_kernel(const LaunchA
             if (leader) {
                 mbar_wait(epidone_bar(my_slot), my_phase);
                 fence_acq_rel_gpu();
-                red_relaxed_gpu_add(args.panel_done + (size_t)ti.task * args.panel_stride + ti.tn, 1);
-                red_relaxed_gpu_add(args.task_done + ti.task, 1);
+                publish_tile<BM, BN>(args, ti);
                 if (args.trace != nullptr) {
                     TraceRec r;
                     r.task = ti.task; r.tm = ti.tm; r.tn = ti.tn; r.sm = sm_id();

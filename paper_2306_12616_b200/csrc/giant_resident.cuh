@@ -141,7 +141,7 @@ __global__ void __launch_bounds__(GR_THREADS, 1) giant_resident_kernel(const Gia
                 wait_counter(args.panel_done + (size_t)(s - 1) * args.panel_stride + ctr, dep_target, args.error_flag);
                 fence_proxy_async_global();
                 const CUtensorMap* mapB = args.maps + tk->mapB;
-                if (s <= 2) fence_tensormap_acquire(mapB);  // the two ping-pong buffers alternate as operand B
+                if (s <= 3) fence_tensormap_acquire(mapB);  // the three rotating buffers take turns as operand B
                 for (int kt = 0; kt < ktiles; ++kt) {
                     mbar_wait(empty_bar(g, stage), phase ^ 1);
                     const uint32_t dst = smem_u32(ring0) + (g * GR_STAGES + stage) * GR_TILE_BYTES;
