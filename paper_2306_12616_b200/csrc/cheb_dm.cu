@@ -125,7 +125,7 @@ struct cheb_dm_plan_s {
     int scalar_sums;     // CHEB_DM_SCALAR_SUMS=1 at plan time: FP64-FMA form_sums_kernel (ablation)
     int preformed;       // 1: low-order sums G_l are formed by form_sums_kernel before the giant steps
     int sym;             // 1: symmetric-tile skipping in gemm_dmma_kernel
-    int* sym_first;      // device: [tiles_n + 1] item prefix sums of a symmetric task
+    short2* sym_tiles;   // device: [sym items] work item -> (tm, tn) of a symmetric task, raster order
     int* sym_panel_target;  // device: [tiles_n] tiles of a symmetric task that write into a column panel (own + mirrored)
     int panel_sym;       // 1: symmetric giant / chain steps wait per column panel (BM a multiple of BN)
     int resident;        // 1: single solves run their giant steps in giant_resident_kernel (small N)
@@ -678,7 +678,7 @@ cheb_dm_status_t launch_tasks(cheb_dm_plan_s* P, const TaskTable& tt, int lt0, i
     for (int s = 0; s < nb; ++s) la.userD[s] = userD ? userD[s] : nullptr;
     la.ldD = ldD;
     la.tma2d = P->tma2d;
-    la.sym_first = P->sym_first;
+    la.sym_tiles = P->sym_tiles;
     la.sym_panel_target = P->sym_panel_target;
     la.error_flag = P->counters;
     la.trace = P->trace_on ? P->trace_buf : nullptr;
@@ -1166,7 +1166,7 @@ cheb_dm_status_t cheb_dm_destroy(cheb_dm_plan_t P) {
     cudaFree(P->traces);
     cudaFree(P->gram_part);
     cudaFree(P->gram);
-    cudaFree(P->sym_first);
+    cudaFree(P->sym_tiles);
     cudaFree(P->sym_panel_target);
     cudaFree(P->sc);
     cudaFree(P->maps);
@@ -1319,7 +1319,7 @@ cheb_dm_status_t cheb_dm_plan_ex(cheb_dm_plan_t* plan, int N, int M_terms, cheb_
     }
     P->ws = nullptr; P->costab = P->fn = P->c = P->gT = P->dT = P->Amat = P->tau = P->w = P->one = P->part = nullptr;
     P->traces = P->gram_part = P->gram = nullptr;
-    P->sym_first = nullptr; P->sym_panel_target = nullptr; P->sc = nullptr; P->maps = nullptr; P->counters = nullptr;
+    P->sym_tiles = nullptr; P->sym_panel_target = nullptr; P->sc = nullptr; P->maps = nullptr; P->counters = nullptr;
     P->have_coeffs = P->explicit_bounds = P->have_moments = P->computed = P->blocks_nb = 0;
     P->beta = P->mu = P->a = P->b = 0.0;
     P->last_launches = 0;
@@ -1394,13 +1394,26 @@ cheb_dm_status_t cheb_dm_plan_ex(cheb_dm_plan_t* plan, int N, int M_terms, cheb_
         }
         {
             const int tn_ = ceil_div(N, P->BN), tm_ = ceil_div(N, P->BM);
-            std::vector<int> pf(tn_ + 1, 0);
-            for (int tn = 0; tn < tn_; ++tn) {
-                const int tm0 = sym_tm0(tn, P->BM, P->BN);
-                pf[tn + 1] = pf[tn] + (tm0 < tm_ ? tm_ - tm0 : 0);
+            // Work item -> tile of a symmetric task.  Column-panel-major (a panel's tiles are consecutive: with the per-panel
+            // dependencies the next level's first panels are ready early) while a matrix fits the L2 several times over; for
+            // larger matrices in bands of 16 column panels, row block by row block inside a band: a wave of ~148 tiles then
+            // touches ~9 A row blocks and 16 B column panels instead of every A row block (measured at N = 5000 with 64x64
+            // tiles, panel-major: 4.5 GB of DRAM reads per product against 0.6 GB of operands).
+            std::vector<short2> tl;
+            const bool banded = (double)N * (double)P->ld * 8.0 > 48.0 * 1024 * 1024;
+            const int band = banded ? 16 : 1;
+            for (int b0 = 0; b0 < tn_; b0 += band) {
+                if (!banded) {
+                    for (int tm = sym_tm0(b0, P->BM, P->BN); tm < tm_; ++tm) tl.push_back(make_short2((short)tm, (short)b0));
+                } else {
+                    for (int tm = 0; tm < tm_; ++tm)
+                        for (int tn = b0; tn < tn_ && tn < b0 + band; ++tn)
+                            if (tm >= sym_tm0(tn, P->BM, P->BN)) tl.push_back(make_short2((short)tm, (short)tn));
+                }
             }
-            if (cudaMalloc(&P->sym_first, sizeof(int) * pf.size()) != cudaSuccess) { cudaGetLastError(); st = CHEB_DM_EALLOC; break; }
-            if (cudaMemcpy(P->sym_first, pf.data(), sizeof(int) * pf.size(), cudaMemcpyHostToDevice) != cudaSuccess) { st = CHEB_DM_ECUDA; break; }
+            if ((int)tl.size() != sym_items(N, P->BM, P->BN)) { st = CHEB_DM_EINVAL; break; }
+            if (cudaMalloc(&P->sym_tiles, sizeof(short2) * tl.size()) != cudaSuccess) { cudaGetLastError(); st = CHEB_DM_EALLOC; break; }
+            if (cudaMemcpy(P->sym_tiles, tl.data(), sizeof(short2) * tl.size(), cudaMemcpyHostToDevice) != cudaSuccess) { st = CHEB_DM_ECUDA; break; }
             // column panel q of a symmetric result is written by the work items of panel q and, mirrored, by the work items
             // (tm, tn != q) of the row block(s) tm whose rows cross the panel's columns: q in [tm R, tm R + R), R = BM / BN
             std::vector<int> tg(tn_, 0);

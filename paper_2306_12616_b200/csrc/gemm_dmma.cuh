@@ -92,7 +92,9 @@ struct LaunchArgs {
     double* userD[MAX_BATCH];  // per slot: the caller's D
     long long ldD;
     int tma2d;               // 1: operand maps are 2-D {column, row} with one 16-column box per copy
-    const int* sym_first;    // [tiles_n + 1] prefix sums of the per-panel item counts of a symmetric task
+    const short2* sym_tiles; // [items of a symmetric task] (tm, tn) of work item i: the tiles that touch the lower triangle, column-
+                             // panel-major, or -- matrices that do not fit the L2 -- in bands of 16 column panels, row-major inside a
+                             // band, so that the CTAs of a wave share a few A row blocks and B column panels
     const int* sym_panel_target;  // [tiles_n] completion count of a column panel of a symmetric task (DEP_PANEL_SYM)
     int* error_flag;         // set to 1 if a dependency wait exceeds the watchdog (never in a correct run)
     TraceRec* trace;         // nullable: per-item timeline, indexed by trace_base + work item of the launch
@@ -274,14 +276,10 @@ __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MIN_CTAS) gemm_dmma_kernel(
                         tn = local / tiles_m;  // column-panel-major order: a panel's tiles are consecutive
                         tm = local - tn * tiles_m;
                     } else {
-                        // symmetric task: panel tn holds the tiles tm >= floor(tn BN / BM); find the panel by bisection
-                        int lo = 0, hi = tk->tiles_n;
-                        while (hi - lo > 1) {
-                            const int mid = (lo + hi) >> 1;
-                            if (__ldg(args.sym_first + mid) <= local) lo = mid; else hi = mid;
-                        }
-                        tn = lo;
-                        tm = (tn * BN) / BM + (local - __ldg(args.sym_first + tn));
+                        // symmetric task: the plan's item -> tile table (lower-triangle tiles in raster order)
+                        const short2 tt = __ldg(args.sym_tiles + local);
+                        tm = tt.x;
+                        tn = tt.y;
                     }
                     // early dependencies: operands of the low-order sum, which the consumers read before the K loop
                     if (args.use_deps)

@@ -151,13 +151,9 @@ __global__ void __launch_bounds__(Cfg::THREADS, 1) gemm_epi_kernel(const LaunchA
                     tn = local / tiles_m;
                     tm = local - tn * tiles_m;
                 } else {
-                    int lo = 0, hi = tk->tiles_n;
-                    while (hi - lo > 1) {
-                        const int mid = (lo + hi) >> 1;
-                        if (__ldg(args.sym_first + mid) <= local) lo = mid; else hi = mid;
-                    }
-                    tn = lo;
-                    tm = (tn * BN) / BM + (local - __ldg(args.sym_first + tn));
+                    const short2 tt = __ldg(args.sym_tiles + local);  // the plan's item -> tile table (raster order)
+                    tm = tt.x;
+                    tn = tt.y;
                 }
                 if (args.use_deps)
                     for (int d = 0; d < tk->ndeps_early; ++d) wait_dep(tk, d, tn);
