@@ -133,7 +133,7 @@ typedef struct {
                       planes of two operands (2 S N kpad bytes, kpad = N rounded up to 64) and their scale vectors.        */
     int sliced_solve; /* 1: cheb_dm_compute runs every product of the solve (baby steps and giant steps) on the sliced int8
                       tensor path (sliced digits, default 8) instead of the FP64 DMMA kernel: one launch per product, each
-                      result sliced once, k + 4 digit sets in the workspace; single solves only (max_batch <= 1), low-order
+                      result sliced once, k + 5 digit sets in the workspace; single solves only (max_batch <= 1), low-order
                       sums pre-formed.  Pays from N ~ 2000.  cheb_dm_solve / moments keep the DMMA path. */
 } cheb_dm_options_t;
 
