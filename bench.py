@@ -343,11 +343,17 @@ def measure_sliced(torch, cd, workloads, name, args, steps, warmup, flush, dist,
     ops = plan.sliced_ops_per_compute()
     kernel_ms = prod_ms / max(n_rec, 1)
     achieved = ops / (kernel_ms * 1e-3) * 1e-12
+    mi_steps = max(2, min(steps, 5))
+    mi_ms = max_over_ranks(torch, dist, timed_steps(torch, w.step_mu_inclusive, mi_steps, 1, flush, None, dist)) / mi_steps
+    plan.check(w.st)
+    tr_mi = [float(x) for x in w.dtr.cpu().tolist()]
     e2e_steps = max(3, min(steps, 10))
     e2e_ms = max_over_ranks(torch, dist, timed_host_stream(torch, w, e2e_steps, 1, dist))
     res = {"call": "cheb_dm_compute on a plan with sliced_solve = 1, sliced = 8 digits", "value": job_value(world, w.units, steps, total_ms), "unit": UNIT,
            "ms_per_solve": total_ms / steps / w.units, "tr_D": [float(x) for x in w.dtr.cpu().tolist()],
            "e2e": {"value": world * w.units * e2e_steps / (e2e_ms * 1e-3), "unit": UNIT},
+           "mu_inclusive": {"call": "cheb_dm_solve on the same plan (baby block and giant block sliced, nested giant steps)", "ms_per_solve": mi_ms / w.units,
+                            "value": world * w.units / (mi_ms * 1e-3), "unit": UNIT, "tr_D": tr_mi},
            "full_product_equivalent_tflops": (plan.k + plan.p - 2) * 2.0 * w.N ** 3 / (kernel_ms * 1e-3) * 1e-12,
            "roofline": {"bound": "tensor", "kernel": "oz_gemm_kernel<8> (tcgen05.mma kind::i8, 8 int32 accumulators in tensor memory) + oz_split_kernel + form_sums",
                         "achieved": achieved, "peak": int8_peak, "unit": "TOP/s", "frac": achieved / int8_peak if int8_peak else None,

@@ -131,10 +131,12 @@ typedef struct {
                       (cheb_dm_compute_host), 2 = both + copy streams/events (cheb_dm_compute_host_async).         */
     int sliced;     /* digits S of cheb_dm_product_sliced: 0 = off, 2..8: the plan allocates the int8 digit
                       planes of two operands (2 S N kpad bytes, kpad = N rounded up to 64) and their scale vectors.        */
-    int sliced_solve; /* 1: cheb_dm_compute runs every product of the solve (baby steps and giant steps) on the sliced int8
-                      tensor path (sliced digits, default 8) instead of the FP64 DMMA kernel: one launch per product, each
-                      result sliced once, k + 5 digit sets in the workspace; single solves only (max_batch <= 1), low-order
-                      sums pre-formed.  Pays from N ~ 2000.  cheb_dm_solve / moments keep the DMMA path. */
+    int sliced_solve; /* 1: every product of the plan (baby steps, giant steps, and the giant block of cheb_dm_moments /
+                      cheb_dm_solve) runs on the sliced int8 tensor path (sliced digits, default 8) instead of the FP64 DMMA
+                      kernel: one launch per product, each result sliced once, k + 5 (+ p - 2 with moments) digit sets in the
+                      workspace; single solves only (max_batch <= 1), low-order sums pre-formed; cheb_dm_solve / assemble then
+                      assemble D with the nested giant steps instead of the long-K product.  Pays from N ~ 2000 (DESIGN.md
+                      section 6). */
 } cheb_dm_options_t;
 
 /* Create a plan for N x N matrices and an M_terms-term expansion.  Chooses (k,p), allocates the

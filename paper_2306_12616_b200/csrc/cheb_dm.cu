@@ -110,7 +110,7 @@ struct cheb_dm_plan_s {
     long long ld;        // padded leading dimension of workspace matrices (multiple of 16)
     long long ldh, ldd;  // leading dimensions of the caller's device matrices
     size_t mat_elems;    // elements per workspace matrix
-    int nmat;            // matrices per slot: T_1..T_k | buf0 buf1 | G_0..G_{p-1} (if any) | U_2..U_{p-1} (if any)
+    int nmat;            // matrices per slot: T_1..T_k | buf0 buf1 buf2 | G_0..G_{p-1} (if any) | U_2..U_{p-1} (if any)
     size_t slot_elems;   // nmat * mat_elems
     int off_G, off_U;    // first matrix of the G / U blocks inside a slot (-1: absent)
     double* ws;          // maxb slots
@@ -154,7 +154,7 @@ struct cheb_dm_plan_s {
     long long n_async;
     int pipe_ready;
     // digit planes of cheb_dm_product_sliced (option sliced = S): [operand][digit][N][oz_kpad] int8, scales [operand][N]
-    int oz_S, oz_nsets, oz_solve;   // digit sets: T_1..T_k, two giant-step buffers (sliced_solve), then the two of the stand-alone product
+    int oz_S, oz_nsets, oz_solve;   // digit sets: T_1..T_k, the three giant-step buffers (sliced_solve), then the two of the stand-alone product
     long long oz_kpad;
     int8_t* oz_digits;         // [set][digit][N][oz_kpad]
     double* oz_scale;          // [set][N] row scales, then [set][N] diagonal corrections of exact squares
@@ -871,10 +871,21 @@ cheb_dm_status_t compute_impl(cheb_dm_plan_s* P, int nb, const double* const* dH
 }
 
 // Baby block, giant block and moments of nb matrices (front end with bounds already run).
+cheb_dm_status_t sliced_baby(cheb_dm_plan_s* P, cudaStream_t st);
+cheb_dm_status_t sliced_giant(cheb_dm_plan_s* P, double* userD, long long ldd, cudaStream_t st);
+cheb_dm_status_t sliced_table(cheb_dm_plan_s* P, const TaskTable& tt, int kind, double* userD, long long ldd, cudaStream_t st);
+
 cheb_dm_status_t blocks_and_moments(cheb_dm_plan_s* P, int nb, cudaStream_t st) {
-    cheb_dm_status_t s = run_table(P, P->baby, nb, nullptr, 0, st);
-    if (s != CHEB_DM_OK) return s;
-    s = run_table(P, P->chain, nb, nullptr, 0, st);
+    cheb_dm_status_t s;
+    if (P->oz_solve) {  // the blocks on the sliced int8 path (their FP64 results feed the Gram kernel as usual)
+        s = sliced_baby(P, st);
+        if (s != CHEB_DM_OK) return s;
+        s = sliced_table(P, P->chain, 2 /* SLICED_CHAIN */, nullptr, 0, st);
+    } else {
+        s = run_table(P, P->baby, nb, nullptr, 0, st);
+        if (s != CHEB_DM_OK) return s;
+        s = run_table(P, P->chain, nb, nullptr, 0, st);
+    }
     if (s != CHEB_DM_OK) return s;
     const int k = P->k, p = P->p;
     diag_traces_kernel<<<dim3(P->ntrmat, nb), 256, 0, st>>>(T_ptr(P, 0, 1), P->off_U >= 0 ? mat_ptr(P, 0, P->off_U) : T_ptr(P, 0, 1),
@@ -915,6 +926,8 @@ cheb_dm_status_t assemble_impl(cheb_dm_plan_s* P, int nb, const double* mu, int 
                                cudaStream_t st) {
     cheb_dm_status_t s = front_end(P, nb, nullptr, 0, mu, 0, 1, mu_from_device, st);
     if (s != CHEB_DM_OK) return s;
+    // sliced path: the nested giant steps on the digit sets left by the blocks (T_k; the accumulators are re-sliced)
+    if (P->oz_solve) return sliced_giant(P, dD[0], ldd, st);
     s = form_sums(P, nb, true, P->BM, P->BN, st);
     if (s != CHEB_DM_OK) return s;
     return run_table(P, P->flat, nb, dD, ldd, st);
@@ -966,7 +979,7 @@ bool batch_args_ok(const cheb_dm_plan_s* P, int nb, const double* const* A, doub
 // Digit planes, scales and TMA descriptors of cheb_dm_product_sliced.
 cheb_dm_status_t prepare_sliced(cheb_dm_plan_s* P) {
     const size_t plane = (size_t)P->N * (size_t)P->oz_kpad;
-    P->oz_nsets = (P->oz_solve ? P->k + NBUF : 0) + 2;
+    P->oz_nsets = (P->oz_solve ? P->k + NBUF + ((P->moments_on && P->p >= 3) ? P->p - 2 : 0) : 0) + 2;
     const size_t bytes = (size_t)P->oz_nsets * (size_t)P->oz_S * plane;
     if (cudaMalloc(&P->oz_digits, bytes) != cudaSuccess || cudaMalloc(&P->oz_scale, sizeof(double) * 2 * P->oz_nsets * P->N) != cudaSuccess) {
         cudaGetLastError();
@@ -1053,80 +1066,105 @@ cheb_dm_status_t oz_gemm(cheb_dm_plan_s* P, int setA, int setB, OzArgs oa, int s
     return CHEB_DM_OK;
 }
 
-// The products of a fixed-mu solve on the sliced int8 path (option sliced_solve): the same task tables as the DMMA path
-// (Algorithm 1 / balanced pairing for the baby steps, Eq. 4 or its Clenshaw form for the giant steps, low-order sums
-// pre-formed in FP64), one launch per product; every result that is an operand later on is sliced once, right after it
-// is formed.  Digit set of workspace matrix m (T_1..T_k, buf0, buf1) = m, like its tensor-map index.
-cheb_dm_status_t run_products_sliced(cheb_dm_plan_s* P, double* userD, long long ldd, cudaStream_t st) {
+// Digit set of a workspace matrix of slot 0: T_1..T_k and the three giant-step buffers keep their matrix index, the giant
+// block U_2..U_{p-1} follows.
+int oz_set_of_matrix(const cheb_dm_plan_s* P, int m) {
+    if (m < P->k + NBUF) return m;
+    return P->k + NBUF + (m - P->off_U);
+}
+// ... and of an operand given by its tensor-map index (T_1..T_k, buffers, then the U_1..U_{p-1} run of the long-K product).
+int oz_set_of_map(const cheb_dm_plan_s* P, int idx) {
+    if (idx < P->k + NBUF) return idx;
+    const int j = idx - P->map_flatB + 1;  // U_j; U_1 = T_k
+    return j == 1 ? P->k - 1 : P->k + NBUF + (j - 2);
+}
+
+enum SlicedKind { SLICED_BABY = 0, SLICED_GIANT = 1, SLICED_CHAIN = 2 };
+
+// One task table on the sliced int8 path (option sliced_solve): the same tasks as the DMMA path (Algorithm 1 / balanced
+// pairing for the baby steps, Eq. 4 or its Clenshaw form for the giant steps, U_{j+1} = 2 Y U_j - U_{j-1} for the giant
+// block), one launch per product; every result that is an operand later on is sliced once, right after it is formed.
+cheb_dm_status_t sliced_table(cheb_dm_plan_s* P, const TaskTable& tt, int kind, double* userD, long long ldd, cudaStream_t st) {
     const int k = P->k;
-    cheb_dm_status_t s = oz_split(P, 0, T_ptr(P, 0, 1), P->ld, st);  // T_1 = X
-    if (s != CHEB_DM_OK) return s;
-    ++P->last_launches;
-    const TaskTable* tabs[2] = {&P->baby, &P->giant};
-    for (int tb = 0; tb < 2; ++tb) {
-        const TaskTable& tt = *tabs[tb];
-        if (tb == 1) {
-            s = form_sums(P, 1, true, OZ_BM, OZ_BN, st);  // every element: the product-free step copies a whole G_l
+    cheb_dm_status_t s = CHEB_DM_OK;
+    for (int lt = 0; lt < tt.ntl; ++lt) {
+        const Task& t = tt.h[(size_t)lt * P->maxb];
+        double* Out = t.out_is_user ? userD : t.Out;
+        const long long ldo = t.out_is_user ? ldd : t.ldo;
+        const double* G = (t.sum_count == 1) ? t.sum_base : nullptr;
+        if (t.sum_count > 1) return CHEB_DM_EUNSUPPORTED;  // the plan forces pre-formed sums
+        if (t.ktiles == 0) {
+            // product-free step (l = p - 1): Out = G
+            if (!G) return CHEB_DM_EUNSUPPORTED;
+            unpad_copy_kernel<<<P->num_sms * 4, 256, 0, st>>>(G, t.lds, P->N, Out, ldo);
+        } else {
+            OzArgs oa;
+            memset(&oa, 0, sizeof(oa));
+            oa.alpha = t.alpha;
+            oa.beta = t.C ? t.beta : 0.0;
+            oa.C = t.C;
+            oa.ldc = t.ldc;
+            oa.G = G;
+            oa.ldg = t.lds;
+            oa.diag = t.diag_const;
+            oa.Out = Out;
+            oa.ldo = ldo;
+            // Both factors are fetched K-major, i.e. the kernel forms (left) (right)^T.  Baby steps: T_l T_r^T, a one-off use of
+            // the (rounding-level) asymmetry of T_r.  Giant steps and giant block: the accumulator (B_{l+1}, U_j) must be the
+            // LEFT factor and the fixed multiplier Y = T_k the transposed one: with Y B^T an antisymmetric error component
+            // between eigenvectors of Y with eigenvalues of opposite sign obeys e_l = 2 Y e_{l+1}^T - e_{l+2} and grows like
+            // (c + sqrt(c^2 + 1))^l, c = sqrt|y_a y_b| (measured: 2e-7 at p = 32, 2e+4 at p = 64; reading A15);
+            // with B Y^T every component follows the scalar recurrence and stays at the FP64 level.  Baby steps take the
+            // higher-index operand as the left factor for the same reason (the serial pairing is such a recurrence in T_n).
+            const int sa = oz_set_of_map(P, t.mapA), sb = oz_set_of_map(P, t.mapB);
+            const bool swap = (kind != SLICED_BABY) || (sb > sa);
+            s = oz_gemm(P, swap ? sb : sa, swap ? sa : sb, oa, P->sym, st);
             if (s != CHEB_DM_OK) return s;
         }
-        for (int lt = 0; lt < tt.ntl; ++lt) {
-            const Task& t = tt.h[(size_t)lt * P->maxb];
-            double* Out = t.out_is_user ? userD : t.Out;
-            const long long ldo = t.out_is_user ? ldd : t.ldo;
-            const double* G = (t.sum_count == 1) ? t.sum_base : nullptr;
-            if (t.sum_count > 1) return CHEB_DM_EUNSUPPORTED;  // the plan forces pre-formed sums
-            if (t.ktiles == 0) {
-                // product-free step (l = p - 1): Out = G
-                if (!G) return CHEB_DM_EUNSUPPORTED;
-                unpad_copy_kernel<<<P->num_sms * 4, 256, 0, st>>>(G, t.lds, P->N, Out, ldo);
-            } else {
-                OzArgs oa;
-                memset(&oa, 0, sizeof(oa));
-                oa.alpha = t.alpha;
-                oa.beta = t.C ? t.beta : 0.0;
-                oa.C = t.C;
-                oa.ldc = t.ldc;
-                oa.G = G;
-                oa.ldg = t.lds;
-                oa.diag = t.diag_const;
-                oa.Out = Out;
-                oa.ldo = ldo;
-                // Both factors are fetched K-major, i.e. the kernel forms (left) (right)^T.  Baby steps: T_l T_r^T, a one-off use of
-                // the (rounding-level) asymmetry of T_r.  Giant steps: the accumulator B_{l+1} must be the LEFT factor and the
-                // fixed multiplier Y = T_k the transposed one: with Y B^T an antisymmetric error component between eigenvectors
-                // of Y with eigenvalues of opposite sign obeys e_l = 2 Y e_{l+1}^T - e_{l+2} and grows like
-                // (c + sqrt(c^2 + 1))^l, c = sqrt|y_a y_b| (measured: 2e-7 at p = 32, 2e+4 at p = 64);
-                // with B Y^T every component follows the scalar Clenshaw recurrence and stays at the FP64 level.
-                // Baby steps take the higher-index operand as the left factor for the same reason (the serial pairing
-                // T_{n+1} = 2 T_1 T_n - T_{n-1} is such a recurrence in T_n).
-                const bool swap = (tb == 1) || (t.mapB > t.mapA);
-                const int left = swap ? t.mapB : t.mapA, right = swap ? t.mapA : t.mapB;
-                s = oz_gemm(P, left, right, oa, P->sym, st);
-                if (s != CHEB_DM_OK) return s;
+        ++P->last_launches;
+        // is the result an operand of a later product?  T_n of the baby block: if a later baby product reads it, or n = k;
+        // a giant-step accumulator B_l, l >= 1: always; U_{j+1}: by the next product of the chain
+        if (!t.out_is_user) {
+            const int m = (int)((t.Out - P->ws) / (long long)P->mat_elems);
+            bool needed = (kind == SLICED_GIANT) || (kind == SLICED_CHAIN && lt + 1 < tt.ntl);
+            if (kind == SLICED_BABY) {
+                needed = (m == k - 1);
+                for (int l2 = lt + 1; l2 < tt.ntl && !needed; ++l2) {
+                    const Task& u = tt.h[(size_t)l2 * P->maxb];
+                    needed = (u.mapA == m || u.mapB == m);
+                }
             }
-            ++P->last_launches;
-            // the result is an operand of a later product: T_n of the baby block (n - 1 = its matrix index), or a giant-step
-            // accumulator B_l, l >= 1 (matrix k + (l & 1))
-            if (!t.out_is_user) {
-                const int m = (int)((t.Out - P->ws) / (long long)P->mat_elems);
-                bool needed = (tb == 1);
-                if (tb == 0) {
-                    needed = (m == k - 1);
-                    for (int l2 = lt + 1; l2 < tt.ntl && !needed; ++l2) {
-                        const Task& u = tt.h[(size_t)l2 * P->maxb];
-                        needed = (u.mapA == m || u.mapB == m);
-                    }
-                }
-                if (needed) {
-                    s = oz_split(P, m, t.Out, t.ldo, st);
-                    if (s != CHEB_DM_OK) return s;
-                    ++P->last_launches;
-                }
+            if (needed) {
+                s = oz_split(P, oz_set_of_matrix(P, m), t.Out, t.ldo, st);
+                if (s != CHEB_DM_OK) return s;
+                ++P->last_launches;
             }
         }
     }
     CUDA_TRY(cudaGetLastError());
     return CHEB_DM_OK;
+}
+
+// Baby block (T_1 is in place: front end).
+cheb_dm_status_t sliced_baby(cheb_dm_plan_s* P, cudaStream_t st) {
+    cheb_dm_status_t s = oz_split(P, 0, T_ptr(P, 0, 1), P->ld, st);  // T_1 = X
+    if (s != CHEB_DM_OK) return s;
+    ++P->last_launches;
+    return sliced_table(P, P->baby, SLICED_BABY, nullptr, 0, st);
+}
+
+// Low-order sums (FP64, every element: the product-free step copies a whole G_l) and the giant steps.
+cheb_dm_status_t sliced_giant(cheb_dm_plan_s* P, double* userD, long long ldd, cudaStream_t st) {
+    cheb_dm_status_t s = form_sums(P, 1, true, OZ_BM, OZ_BN, st);
+    if (s != CHEB_DM_OK) return s;
+    return sliced_table(P, P->giant, SLICED_GIANT, userD, ldd, st);
+}
+
+// The products of a fixed-mu solve on the sliced path.
+cheb_dm_status_t run_products_sliced(cheb_dm_plan_s* P, double* userD, long long ldd, cudaStream_t st) {
+    cheb_dm_status_t s = sliced_baby(P, st);
+    if (s != CHEB_DM_OK) return s;
+    return sliced_giant(P, userD, ldd, st);
 }
 
 }  // namespace

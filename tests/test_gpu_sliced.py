@@ -162,3 +162,65 @@ def test_sliced_solve_full_size(cfg):
     print(f"{cfg}: sliced solve |tr D - sum_i p_M(x_i)| = {dtr:.3e}")
     assert dtr <= 1e-9
     assert np.max(np.abs(D - D.T)) <= 1e-11
+
+
+@pytest.mark.parametrize("cfg,seed,n,M,opts", [("cfg1", 0, 300, None, {}), ("cfg2", 0, 250, None, {}), ("cfg3", 0, 200, 1024, {}),
+                                                ("cfg4", 0, 200, 2048, {}), ("cfg1", 2, 130, 60, dict(k=6, p=10)), ("cfg1", 0, 64, 12, dict(k=6, p=2))])
+def test_sliced_mu_inclusive_solve(cfg, seed, n, M, opts):
+    """cheb_dm_solve / cheb_dm_moments / cheb_dm_assemble on a sliced_solve plan: baby block and giant block on the int8
+    path, moments by the Gram kernel, bisection, nested giant steps; (tau, mu, D) against the oracle as in test_gpu_solve."""
+    oracle, cd, workloads, gu = _imports()
+    torch = gu.torch_cuda()
+    c = workloads.CONFIGS[cfg]
+    H = workloads.hamiltonian(cfg, seed=seed, n=n)
+    N = H.shape[0]
+    M = c.M if M is None else M
+    nocc = workloads.n_occ(cfg, N)
+    a, b = oracle.gershgorin(H)
+    _, tau = oracle.dm_cheb(H, a, b, np.zeros(M), want_tau=True)
+    mu_or = oracle.solve_mu(tau, c.beta, a, b, nocc, iters=100)
+    D_or = oracle.dm_cheb(H, a, b, oracle.cheb_coeffs(c.beta, mu_or, a, b, M))
+    plan = cd.Plan(N, M, sliced_solve=1, **opts)
+    st = torch.cuda.current_stream().cuda_stream
+    dH = gu.to_dev(H)
+    dD = torch.full((N, N), float("nan"), dtype=torch.float64, device="cuda")
+    plan.coeffs(c.beta, 123.0, None)
+    mu = plan.solve(dH.data_ptr(), nocc, dD.data_ptr(), 100, True, st)
+    plan.check(st)
+    assert abs(mu - mu_or) <= 1e-10 * max(1.0, b - a)
+    D = dD.cpu().numpy()
+    err = float(np.max(np.abs(D - D_or)))
+    print(f"{cfg} n={N} M={M}: sliced cheb_dm_solve mu={mu:.12f} (oracle {mu_or:.12f}) max|dD|={err:.3e}")
+    assert err <= 1e-10
+    assert abs(float(np.trace(D)) - nocc) <= 1e-7
+    tau_gpu = plan.moments(dH.data_ptr(), True, st)[:M]
+    assert np.max(np.abs(tau_gpu - tau)) <= 1e-10 * N
+    mu2 = mu_or + 0.05
+    plan.assemble([mu2], [dD.data_ptr()], st)
+    torch.cuda.synchronize()
+    D2 = oracle.dm_cheb(H, a, b, oracle.cheb_coeffs(c.beta, mu2, a, b, M))
+    assert np.max(np.abs(dD.cpu().numpy() - D2)) <= 1e-10
+    plan.destroy()
+
+
+def test_sliced_mu_inclusive_solve_full_size_cfg2():
+    """cheb_dm_solve on a sliced_solve plan at full size (cfg2, N=1000): (mu, D) against the oracle, every element."""
+    import oracle_cases as oc
+    oracle, cd, workloads, gu = _imports()
+    torch = gu.torch_cuda()
+    case = oc.case("cfg2", 0, None, None, True)
+    N, M = case["N"], case["M"]
+    plan = cd.Plan(N, M, sliced_solve=1)
+    st = torch.cuda.current_stream().cuda_stream
+    dH = gu.to_dev(case["H"])
+    dD = torch.full((N, N), float("nan"), dtype=torch.float64, device="cuda")
+    plan.coeffs(case["beta"], 0.0, None)
+    mu = plan.solve(dH.data_ptr(), case["nocc"], dD.data_ptr(), 100, True, st)
+    plan.check(st)
+    assert abs(mu - case["mu"]) <= 1e-10 * (case["b"] - case["a"])
+    D = dD.cpu().numpy()
+    err = float(np.max(np.abs(D - case["D_cheb"])))
+    print(f"cfg2: sliced cheb_dm_solve mu = {mu:.12f} (oracle {case['mu']:.12f}), max|dD| = {err:.3e}")
+    assert err <= 1e-10
+    assert abs(float(np.trace(D)) - case["nocc"]) <= 1e-6
+    plan.destroy()
