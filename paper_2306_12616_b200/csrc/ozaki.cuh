@@ -19,7 +19,7 @@
 // P_0..P_{S-1} live in tensor memory at once (S x 64 columns <= 512), so every digit tile is fetched once per k-block
 // and used by up to S MMAs: S(S+1)/2 MMA blocks per 2S tile loads (a plain int8 GEMM loads 2 per block and is
 // L2-bound on this part).  k-block = 64 int8 (64-byte swizzle rows), stage = S A-tiles (128 x 64 B) + S B-tiles
-// (64 x 64 B), two stages.  Warp 0: TMA producer, warp 1: MMA issuer (one lane), warp 2: TMEM allocator, warps 4-7:
+// (64 x 64 B), two stages.  Warp 0: TMA producer, warp 1: MMA issuer (one lane), warp 2: TMEM allocator, warps 4-11:
 // epilogue (tcgen05.ld of the S accumulators, Horner recombination in FP64, scaling, alpha/beta, store).
 #pragma once
 #include "common.cuh"
@@ -30,7 +30,7 @@ constexpr int OZ_MAX_S = 8;
 constexpr int OZ_BM = 128, OZ_BN = 64, OZ_BK = 64;          // output tile, k-block in int8 elements (= bytes)
 constexpr int OZ_A_TILE = OZ_BM * OZ_BK, OZ_B_TILE = OZ_BN * OZ_BK;   // 8 KB, 4 KB
 constexpr int OZ_STAGES = 2;
-constexpr int OZ_THREADS = 256;
+constexpr int OZ_THREADS = 384;                               // warps 0-3: TMA, MMA issue, TMEM allocation, idle; warps 4-11: epilogue
 constexpr int OZ_BAND = 16;                                  // column tiles per raster band (L2 reuse of the digit strips)
 
 // ---- tcgen05 wrappers ----
@@ -211,7 +211,7 @@ __global__ void __launch_bounds__(OZ_THREADS, 1) oz_gemm_kernel(const __grid_con
             mbar_init(empty_bar(s), 1);
         }
         mbar_init(tfull_bar, 1);
-        mbar_init(tempty_bar, 4);   // the four epilogue warps
+        mbar_init(tempty_bar, 8);   // the eight epilogue warps
         fence_mbar_init();
     }
     if (warp == 2) tc_alloc512(smem_u32(tmem_slot));
@@ -283,7 +283,12 @@ __global__ void __launch_bounds__(OZ_THREADS, 1) oz_gemm_kernel(const __grid_con
         }
     } else if (warp >= 4) {
         // =================================== epilogue warps ===================================
+        // eight epilogue warps: two per TMEM lane quarter (a warp may only access the quarter warp % 4), each taking half of
+        // the 64 columns -- the epilogue is a chain of latencies (tcgen05.ld, the C / G tiles from L2, stores) that holds the
+        // tensor pipe up (all 512 TMEM columns are in use: no second accumulator set to overlap with); measured with four warps:
+        // ~17 us of a 77 us tile at N = 2000
         const int q4 = warp & 3;                                   // TMEM lane quarter this warp may access
+        const int chalf = (warp - 4) >> 2;                         // column half
         const uint32_t lane_base = tmem_base + ((uint32_t)(q4 * 32) << 16);
         uint32_t tphase = 0;
         const int N = args.N;
@@ -296,7 +301,18 @@ __global__ void __launch_bounds__(OZ_THREADS, 1) oz_gemm_kernel(const __grid_con
             tc_fence_after();
             const int row = tm * OZ_BM + q4 * 32 + lane;
             const double rs = (row < N) ? args.scaleA[row] * args.alpha * (1.0 / 4096.0) : 0.0;   // alpha 2^{e_i - 12}
-            for (int c8 = 0; c8 < OZ_BN / 8; ++c8) {
+            for (int c8 = chalf * (OZ_BN / 16); c8 < (chalf + 1) * (OZ_BN / 16); ++c8) {
+                const int col0 = tn * OZ_BN + c8 * 8;
+                // the C / G / scale operands of the chunk are requested before the accumulators are read from tensor memory
+                double cv[8], gv[8], sb[8];
+#pragma unroll
+                for (int j = 0; j < 8; ++j) {
+                    const int col = col0 + j;
+                    const bool in = (row < N && col < N);
+                    sb[j] = in ? args.scaleB[col] : 0.0;
+                    cv[j] = (in && args.C != nullptr) ? args.C[(long long)row * args.ldc + col] : 0.0;
+                    gv[j] = (in && args.G != nullptr) ? args.G[(long long)row * args.ldg + col] : 0.0;
+                }
                 int v[S][8];
 #pragma unroll
                 for (int d = 0; d < S; ++d) tc_ld8(lane_base + (uint32_t)(d * OZ_BN + c8 * 8), v[d]);
@@ -308,16 +324,14 @@ __global__ void __launch_bounds__(OZ_THREADS, 1) oz_gemm_kernel(const __grid_con
                 for (int d = S - 1; d >= 0; --d)                   // Horner from the least significant digit sum
 #pragma unroll
                     for (int j = 0; j < 8; ++j) r[j] = fma(r[j], 1.0 / 128.0, (double)v[d][j]);
-                const int col0 = tn * OZ_BN + c8 * 8;
 #pragma unroll
                 for (int j = 0; j < 8; ++j) {
                     const int col = col0 + j;
-                    double o = 0.0;
                     if (row < N && col < N) {
                         if (args.corr != nullptr && row == col) r[j] += args.corr[row];
-                        o = rs * args.scaleB[col] * r[j];
-                        if (args.C != nullptr) o = fma(args.beta, args.C[(long long)row * args.ldc + col], o);
-                        if (args.G != nullptr) o += args.G[(long long)row * args.ldg + col];
+                        double o = rs * sb[j] * r[j];
+                        o = fma(args.beta, cv[j], o);
+                        o += gv[j];
                         if (row == col) o += args.diag;
                         args.Out[(long long)row * args.ldo + col] = o;
                         // mirror: the transposed element lies in a tile that is not a work item; the lanes of a warp hold 32
