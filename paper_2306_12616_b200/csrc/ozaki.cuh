@@ -300,18 +300,35 @@ __global__ void __launch_bounds__(OZ_THREADS, 1) oz_gemm_kernel(const __grid_con
             tphase ^= 1;
             tc_fence_after();
             const int row = tm * OZ_BM + q4 * 32 + lane;
+            const bool vecC = (args.C == nullptr) || (((args.ldc & 1) == 0) && ((reinterpret_cast<uintptr_t>(args.C) & 15) == 0));
+            const bool vecG = (args.G == nullptr) || (((args.ldg & 1) == 0) && ((reinterpret_cast<uintptr_t>(args.G) & 15) == 0));
+            const bool vecS = (reinterpret_cast<uintptr_t>(args.scaleB) & 15) == 0;
+            const bool vecO = ((args.ldo & 1) == 0) && ((reinterpret_cast<uintptr_t>(args.Out) & 15) == 0);
             const double rs = (row < N) ? args.scaleA[row] * args.alpha * (1.0 / 4096.0) : 0.0;   // alpha 2^{e_i - 12}
             for (int c8 = chalf * (OZ_BN / 16); c8 < (chalf + 1) * (OZ_BN / 16); ++c8) {
                 const int col0 = tn * OZ_BN + c8 * 8;
                 // the C / G / scale operands of the chunk are requested before the accumulators are read from tensor memory
                 double cv[8], gv[8], sb[8];
+                if (row < N && col0 + 7 < N && vecC && vecG && vecS) {   // whole chunk inside, 16-byte aligned rows: 128-bit loads
 #pragma unroll
-                for (int j = 0; j < 8; ++j) {
-                    const int col = col0 + j;
-                    const bool in = (row < N && col < N);
-                    sb[j] = in ? args.scaleB[col] : 0.0;
-                    cv[j] = (in && args.C != nullptr) ? args.C[(long long)row * args.ldc + col] : 0.0;
-                    gv[j] = (in && args.G != nullptr) ? args.G[(long long)row * args.ldg + col] : 0.0;
+                    for (int j = 0; j < 8; j += 2) {
+                        const double2 s2 = *reinterpret_cast<const double2*>(args.scaleB + col0 + j);
+                        sb[j] = s2.x; sb[j + 1] = s2.y;
+                        double2 c2 = make_double2(0.0, 0.0), g2 = make_double2(0.0, 0.0);
+                        if (args.C != nullptr) c2 = *reinterpret_cast<const double2*>(args.C + (long long)row * args.ldc + col0 + j);
+                        if (args.G != nullptr) g2 = *reinterpret_cast<const double2*>(args.G + (long long)row * args.ldg + col0 + j);
+                        cv[j] = c2.x; cv[j + 1] = c2.y;
+                        gv[j] = g2.x; gv[j + 1] = g2.y;
+                    }
+                } else {
+#pragma unroll
+                    for (int j = 0; j < 8; ++j) {
+                        const int col = col0 + j;
+                        const bool in = (row < N && col < N);
+                        sb[j] = in ? args.scaleB[col] : 0.0;
+                        cv[j] = (in && args.C != nullptr) ? args.C[(long long)row * args.ldc + col] : 0.0;
+                        gv[j] = (in && args.G != nullptr) ? args.G[(long long)row * args.ldg + col] : 0.0;
+                    }
                 }
                 int v[S][8];
 #pragma unroll
@@ -324,16 +341,29 @@ __global__ void __launch_bounds__(OZ_THREADS, 1) oz_gemm_kernel(const __grid_con
                 for (int d = S - 1; d >= 0; --d)                   // Horner from the least significant digit sum
 #pragma unroll
                     for (int j = 0; j < 8; ++j) r[j] = fma(r[j], 1.0 / 128.0, (double)v[d][j]);
+                double ov[8];
+#pragma unroll
+                for (int j = 0; j < 8; ++j) {
+                    const int col = col0 + j;
+                    if (args.corr != nullptr && row == col && row < N) r[j] += args.corr[row];
+                    double o = rs * sb[j] * r[j];
+                    o = fma(args.beta, cv[j], o);
+                    o += gv[j];
+                    if (row == col) o += args.diag;
+                    ov[j] = o;
+                }
+                const bool whole = vecO && row < N && col0 + 7 < N;
+                if (whole) {
+#pragma unroll
+                    for (int j = 0; j < 8; j += 2)
+                        *reinterpret_cast<double2*>(args.Out + (long long)row * args.ldo + col0 + j) = make_double2(ov[j], ov[j + 1]);
+                }
 #pragma unroll
                 for (int j = 0; j < 8; ++j) {
                     const int col = col0 + j;
                     if (row < N && col < N) {
-                        if (args.corr != nullptr && row == col) r[j] += args.corr[row];
-                        double o = rs * sb[j] * r[j];
-                        o = fma(args.beta, cv[j], o);
-                        o += gv[j];
-                        if (row == col) o += args.diag;
-                        args.Out[(long long)row * args.ldo + col] = o;
+                        const double o = ov[j];
+                        if (!whole) args.Out[(long long)row * args.ldo + col] = o;
                         // mirror: the transposed element lies in a tile that is not a work item; the lanes of a warp hold 32
                         // consecutive rows, i.e. 32 consecutive elements of the destination row: coalesced
                         if (args.sym && (col / OZ_BM) * OZ_BM + OZ_BM - 1 < (row / OZ_BN) * OZ_BN) args.Out[(long long)col * args.ldo + row] = o;
