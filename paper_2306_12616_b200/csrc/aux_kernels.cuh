@@ -135,6 +135,7 @@ struct FrontArgs {
     int* counters;                   // range to zero
     int ncounters;
     int do_bounds, do_coeffs, mu_from_device;
+    int segs;                        // warps of a block that share a row in the bounds / rescale passes (1, 2, 4, 8 or 16)
     double beta;
     const double* costab;
     int Nq, M;
@@ -168,34 +169,68 @@ __global__ void __launch_bounds__(512) front_end_kernel(const FrontArgs A) {
         const bool vec = ((ldh & 1) == 0) && ((reinterpret_cast<uintptr_t>(H) & 15) == 0);
         if (!A.explicit_bounds) {
             double lo = INFINITY, hi = -INFINITY;
-            for (int row = gwarp; row < N; row += nwarps) {
-                const double* hr = H + (long long)row * ldh;
+            // `segs` consecutive warps of a block share a row (segment seg = columns [seg seglen, (seg+1) seglen)); their
+            // partial sums are combined in a fixed order through shared memory.  segs = 1 for small N (a warp per row);
+            // for N = 5000 a warp per row left 264 rows for a second round (2 x 79 serial iterations per warp).
+            const int segs = A.segs, rpb = warps_per_block / segs;          // rows per block and round
+            const int seg = warp % segs, rloc = warp / segs;
+            const int seglen = (((N + segs - 1) / segs) + 1) & ~1;           // even: 16-byte loads stay aligned
+            const int j0 = seg * seglen, j1 = min(N, j0 + seglen);
+            for (int rbase = sblock * rpb; rbase < N; rbase += sblocks * rpb) {
+                const int row = rbase + rloc;
                 double r = 0.0, hii = 0.0;
-                if (vec) {
-                    for (int j = 2 * lane; j < N; j += 64) {
-                        if (j + 1 < N) {
-                            const double2 v = *reinterpret_cast<const double2*>(hr + j);
+                if (row < N) {
+                    const double* hr = H + (long long)row * ldh;
+                    if (vec) {
+                        // pairs [j, j+1] below jend, four 16-byte loads in flight per lane; an odd last column apart
+                        const int jend = j1 & ~1;
+                        int j = j0 + 2 * lane;
+                        for (; j + 192 < jend; j += 256) {
+                            double2 v[4];
+#pragma unroll
+                            for (int u = 0; u < 4; ++u) v[u] = __ldg(reinterpret_cast<const double2*>(hr + j + 64 * u));
+#pragma unroll
+                            for (int u = 0; u < 4; ++u) {
+                                if (j + 64 * u == row) hii = v[u].x; else r += fabs(v[u].x);
+                                if (j + 64 * u + 1 == row) hii = v[u].y; else r += fabs(v[u].y);
+                            }
+                        }
+                        for (; j < jend; j += 64) {
+                            const double2 v = __ldg(reinterpret_cast<const double2*>(hr + j));
                             if (j == row) hii = v.x; else r += fabs(v.x);
                             if (j + 1 == row) hii = v.y; else r += fabs(v.y);
-                        } else {
+                        }
+                        if ((j1 & 1) && j0 < j1 && lane == 0) {
+                            const double v = hr[j1 - 1];
+                            if (j1 - 1 == row) hii = v; else r += fabs(v);
+                        }
+                    } else {
+                        for (int j = j0 + lane; j < j1; j += 32) {
                             const double v = hr[j];
                             if (j == row) hii = v; else r += fabs(v);
                         }
-                    }
-                } else {
-                    for (int j = lane; j < N; j += 32) {
-                        const double v = hr[j];
-                        if (j == row) hii = v; else r += fabs(v);
                     }
                 }
 #pragma unroll
                 for (int o = 16; o > 0; o >>= 1) {
                     r += __shfl_xor_sync(0xffffffffu, r, o);
-                    hii += __shfl_xor_sync(0xffffffffu, hii, o);  // exactly one lane holds h_ii, the rest 0
+                    hii += __shfl_xor_sync(0xffffffffu, hii, o);  // exactly one lane of one segment holds h_ii, the rest 0
                 }
-                lo = fmin(lo, hii - r);
-                hi = fmax(hi, hii + r);
-                if (!(isfinite(r) && isfinite(hii))) { lo = -INFINITY; hi = INFINITY; }
+                if (segs > 1) {
+                    if (lane == 0) { s_lo[warp] = r; s_hi[warp] = hii; }   // (s_lo / s_hi double as the segment scratch here)
+                    __syncthreads();
+                    if (seg == 0) {
+                        r = 0.0;
+                        hii = 0.0;
+                        for (int q = 0; q < segs; ++q) { r += s_lo[warp + q]; hii += s_hi[warp + q]; }
+                    }
+                    __syncthreads();
+                }
+                if (seg == 0 && row < N) {
+                    lo = fmin(lo, hii - r);
+                    hi = fmax(hi, hii + r);
+                    if (!(isfinite(r) && isfinite(hii))) { lo = -INFINITY; hi = INFINITY; }
+                }
             }
             if (lane == 0) { s_lo[warp] = lo; s_hi[warp] = hi; }
             __syncthreads();
@@ -248,28 +283,49 @@ __global__ void __launch_bounds__(512) front_end_kernel(const FrontArgs A) {
         // ---- phase 2: rescale ----
         const double inv = 1.0 / (b - a), shift = a + b;
         double* X = A.X + (long long)slot * A.slot_stride;
-        for (int row = gwarp; row < N; row += nwarps) {
-            const double* hr = H + (long long)row * ldh;
-            double* xr = X + (long long)row * A.ldx;
-            if (vec) {
-                for (int j = 2 * lane; j < N; j += 64) {
-                    if (j + 1 < N) {
-                        const double2 v = *reinterpret_cast<const double2*>(hr + j);
+        {
+            const int segs = A.segs, rpb = warps_per_block / segs;
+            const int seg = warp % segs, rloc = warp / segs;
+            const int seglen = (((N + segs - 1) / segs) + 1) & ~1;
+            const int j0 = seg * seglen, j1 = min(N, j0 + seglen);
+            for (int rbase = sblock * rpb; rbase < N; rbase += sblocks * rpb) {
+                const int row = rbase + rloc;
+                if (row >= N) continue;
+                const double* hr = H + (long long)row * ldh;
+                double* xr = X + (long long)row * A.ldx;
+                if (vec) {
+                    const int jend = j1 & ~1;
+                    int j = j0 + 2 * lane;
+                    for (; j + 192 < jend; j += 256) {
+                        double2 v[4];
+#pragma unroll
+                        for (int u = 0; u < 4; ++u) v[u] = __ldg(reinterpret_cast<const double2*>(hr + j + 64 * u));
+#pragma unroll
+                        for (int u = 0; u < 4; ++u) {
+                            double h0 = 2.0 * v[u].x, h1 = 2.0 * v[u].y;
+                            if (j + 64 * u == row) h0 -= shift;
+                            if (j + 64 * u + 1 == row) h1 -= shift;
+                            *reinterpret_cast<double2*>(xr + j + 64 * u) = make_double2(h0 * inv, h1 * inv);
+                        }
+                    }
+                    for (; j < jend; j += 64) {
+                        const double2 v = __ldg(reinterpret_cast<const double2*>(hr + j));
                         double h0 = 2.0 * v.x, h1 = 2.0 * v.y;
                         if (j == row) h0 -= shift;
                         if (j + 1 == row) h1 -= shift;
                         *reinterpret_cast<double2*>(xr + j) = make_double2(h0 * inv, h1 * inv);
-                    } else {
+                    }
+                    if ((j1 & 1) && j0 < j1 && lane == 0) {
+                        double h = 2.0 * hr[j1 - 1];
+                        if (j1 - 1 == row) h -= shift;
+                        xr[j1 - 1] = h * inv;
+                    }
+                } else {
+                    for (int j = j0 + lane; j < j1; j += 32) {
                         double h = 2.0 * hr[j];
                         if (j == row) h -= shift;
                         xr[j] = h * inv;
                     }
-                }
-            } else {
-                for (int j = lane; j < N; j += 32) {
-                    double h = 2.0 * hr[j];
-                    if (j == row) h -= shift;
-                    xr[j] = h * inv;
                 }
             }
         }

@@ -756,6 +756,19 @@ cheb_dm_status_t front_end(cheb_dm_plan_s* P, int nb, const double* const* dH, l
     fa.part = P->part;
     fa.counters = P->counters + 1;  // [0] is the sticky error flag
     fa.ncounters = (int)P->counters_ints - 1;
+    {
+        // rows are dealt to the blocks of a matrix in rounds of 16 / segs rows; segs = the power of two that minimises
+        // rounds x elements per warp and round
+        const int grid = front_grid_for(P, nb);
+        const int sblocks = grid / nb > 0 ? grid / nb : 1;
+        long long best = -1;
+        fa.segs = 1;
+        for (int sg = 1; sg <= 16; sg *= 2) {
+            const long long rounds = ceil_div(P->N, sblocks * (16 / sg));
+            const long long cost = rounds * ceil_div(P->N, sg);
+            if (best < 0 || cost < best) { best = cost; fa.segs = sg; }
+        }
+    }
     fa.do_bounds = do_bounds;
     fa.do_coeffs = do_coeffs;
     fa.mu_from_device = mu_from_device;
