@@ -72,6 +72,17 @@ def test_batch_ragged_n257_three_of_four_slots(tile):
     plan.destroy()
 
 
+def test_batch_front_end_rows_shared_by_warps():
+    """Eight matrices of N = 801: the cooperative front end has 37 blocks per matrix, so two warps share a row (odd N:
+    the last column apart).  Bounds, D and trace of every matrix against the oracle."""
+    oracle, cd, workloads, gu, oc = _imports()
+    cases = [oc.case("cfg2", s % 2, 801, 32, True) for s in range(8)]
+    plan, Ds, trs, scal = _run_batch(cd, gu, [c["H"] for c in cases], cases[0]["beta"], [c["mu"] for c in cases], cases[0]["M"])
+    for c, D, tr, sc in zip(cases, Ds, trs, scal):
+        _compare(c, D, tr, sc)
+    plan.destroy()
+
+
 @pytest.mark.parametrize("fuse,symmetric,outer,sched", [(1, 2, 0, 0), (2, 2, 0, 0), (1, 1, 0, 0), (2, 1, 0, 0), (0, 0, 1, 0), (0, 0, 0, 1)])
 def test_batch_cfg0_x8_variants(fuse, symmetric, outer, sched):
     """cfg0 (N=128: one or two tiles per product) x 8, sums fused / pre-formed, with and without symmetric tiles,

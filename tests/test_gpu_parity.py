@@ -69,6 +69,33 @@ def test_gershgorin_bounds_and_rescale(cfg, n):
     r["plan"].destroy()
 
 
+@pytest.mark.parametrize("n,ldh", [(4999, 4999), (4999, 5000), (4802, 4802)])
+def test_gershgorin_bounds_and_rescale_rows_shared_by_warps(n, ldh):
+    """a-1 at N ~ 5000, where 16 warps of a block share a row of H in the bounds and rescale passes: odd N (the last
+    column apart), odd pitch (scalar loads) and even pitch (16-byte loads).  M = 4: the products are not the point."""
+    oracle, cd, workloads, gu, _ = _imports()
+    torch = gu.torch_cuda()
+    st = torch.cuda.current_stream().cuda_stream
+    H = workloads.hamiltonian("cfg3", seed=1, n=n)
+    a, b = oracle.gershgorin(H)
+    Hp = np.full((n, ldh), 3.25)
+    Hp[:, :n] = H
+    dH = gu.to_dev(Hp)
+    dD = torch.empty((n, n), dtype=torch.float64, device="cuda")
+    plan = cd.Plan(n, 4, ldh=ldh)
+    plan.coeffs(5.0, 0.0, None)
+    plan.compute(dH.data_ptr(), dD.data_ptr(), st)
+    plan.check(st)
+    ga, gb = plan.get_bounds(st)
+    scale = max(abs(a), abs(b))
+    assert abs(ga - a) <= n * 2.0 ** -52 * scale and abs(gb - b) <= n * 2.0 ** -52 * scale
+    dX = torch.empty((n, n), dtype=torch.float64, device="cuda")
+    plan.get_T(1, dX.data_ptr(), st)
+    torch.cuda.synchronize()
+    assert np.max(np.abs(dX.cpu().numpy() - oracle.scale(H, a, b))) <= 1e-14
+    plan.destroy()
+
+
 def test_gershgorin_degenerate_identity_widens():
     _, cd, _, gu, _ = _imports()
     H = 3.0 * np.eye(40)
