@@ -295,7 +295,8 @@ cheb_dm_status_t cheb_dm_product(cheb_dm_plan_t plan, double alpha, const double
  * symmetric != 0: the caller asserts that the result is symmetric (A and B commute, C symmetric -- every product of the
  * method, whose operands are polynomials of X): only the 128 x 64 tiles that touch the lower triangle are computed and
  * each is mirrored on store.
- * Stand-alone call (kernel-level tests and benchmark against the DMMA product); the solve does not use it.
+ * Stand-alone call (kernel-level tests and benchmark against the DMMA product); with the option sliced_solve every
+ * product of the solve runs through the same two kernels.
  * EUNSUPPORTED unless the plan was made with the option sliced = S. */
 cheb_dm_status_t cheb_dm_product_sliced(cheb_dm_plan_t plan, double alpha, const double* dA, const double* dB,
                                         double beta, const double* dC, double* dOut, int symmetric, void* cuda_stream);

@@ -61,6 +61,33 @@ def test_sliced_square_without_C_and_graded_rows():
     assert np.all(np.abs(got - expect) <= bound + 1e-300)
 
 
+def test_sliced_zero_rows_zero_operand_and_extreme_exponents():
+    """Degenerate scales: rows and columns that are entirely zero (scale of an empty row), an all-zero operand, and
+    operands near both ends of the FP64 exponent range (2^-480 and 2^+480: the products stay representable)."""
+    oracle, cd, workloads, gu = _imports()
+    N = 150
+    A = workloads.random_symmetric(N, seed=41)
+    B = workloads.random_symmetric(N, seed=42)
+    for i in (0, 17, 149):     # (both operands stay symmetric: the contract of cheb_dm_product_sliced)
+        A[i, :] = 0.0
+        A[:, i] = 0.0
+        B[(i + 3) % N, :] = 0.0
+        B[:, (i + 3) % N] = 0.0
+    got = _run(cd, gu, A, B, None, 1.0, 0.0, 8)
+    expect = oracle.matmul(A, B)
+    assert np.max(np.abs(got - expect)) <= 4.0 * N * 2.0 ** -52
+    assert np.all(got[[0, 17, 149], :] == 0.0) and np.all(got[:, [3, 20, 2]] == 0.0)
+    Z = np.zeros((N, N))
+    assert np.all(_run(cd, gu, Z, B, None, 2.0, 0.0, 8) == 0.0)
+    Cm = workloads.random_symmetric(N, seed=43)
+    assert np.array_equal(_run(cd, gu, A, Z, Cm, 2.0, -1.0, 8), -Cm)
+    for e in (-480, 480):
+        As, Bs = A * 2.0 ** e, B * 2.0 ** e
+        got = _run(cd, gu, As, Bs, None, 1.0, 0.0, 8)
+        assert np.all(np.isfinite(got))
+        assert np.max(np.abs(got * 2.0 ** (-2 * e) - expect)) <= 4.0 * N * 2.0 ** -52
+
+
 @pytest.mark.parametrize("S", [4, 5, 6, 7])
 def test_sliced_fewer_digits_meet_and_reach_the_slicing_bound(S):
     oracle, cd, workloads, gu = _imports()
