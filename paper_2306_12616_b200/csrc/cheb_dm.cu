@@ -1042,8 +1042,23 @@ cheb_dm_status_t prepare_sliced(cheb_dm_plan_s* P) {
 // Digits of an FP64 matrix (leading dimension ld) into digit set `set`.
 cheb_dm_status_t oz_split(cheb_dm_plan_s* P, int set, const double* src, long long ld, cudaStream_t st) {
     const size_t plane = (size_t)P->N * (size_t)P->oz_kpad;
-    oz_split_kernel<<<P->N, 256, 0, st>>>(src, ld, P->N, P->oz_S, P->oz_digits + (size_t)set * P->oz_S * plane, P->oz_kpad,
-                                                              P->oz_scale + (size_t)set * P->N, P->oz_scale + (size_t)(P->oz_nsets + set) * P->N);
+    {
+        int8_t* dig = P->oz_digits + (size_t)set * P->oz_S * plane;
+        double* sc = P->oz_scale + (size_t)set * P->N;
+        double* cr = P->oz_scale + (size_t)(P->oz_nsets + set) * P->N;
+        const int passes = (int)((P->oz_kpad + 1023) / 1024);
+#define OZ_SPLIT_REG(PS) oz_split_reg_kernel<PS><<<P->N, 256, 0, st>>>(src, ld, P->N, P->oz_S, dig, P->oz_kpad, sc, cr)
+        switch (passes) {  // rows up to 6144 elements stay in registers between the maximum and the digits
+            case 1: OZ_SPLIT_REG(1); break;
+            case 2: OZ_SPLIT_REG(2); break;
+            case 3: OZ_SPLIT_REG(3); break;
+            case 4: OZ_SPLIT_REG(4); break;
+            case 5: OZ_SPLIT_REG(5); break;
+            case 6: OZ_SPLIT_REG(6); break;
+            default: oz_split_kernel<<<P->N, 256, 0, st>>>(src, ld, P->N, P->oz_S, dig, P->oz_kpad, sc, cr);
+        }
+#undef OZ_SPLIT_REG
+    }
     CUDA_TRY(cudaGetLastError());
     return CHEB_DM_OK;
 }

@@ -81,6 +81,50 @@ __host__ __device__ constexpr uint32_t oz_idesc(int n) {
     return (2u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(n >> 3) << 17) | ((uint32_t)(OZ_BM >> 4) << 24);
 }
 
+// Digits of four consecutive elements of a row in integer arithmetic: F = rint(a 2^(6 - e) 128^(S-1)) (|F| <= 2^(7S-1): one
+// exact scaling and one rounding, the same residual |rho| <= 128^-(S-1) / 2 as S successive roundings), then the balanced
+// base-128 digits of F read as bit fields of G = F + sum_j 64 128^j:  F = sum_j d_j 128^j, d_j = ((G >> 7j) & 127) - 64 in
+// [-64, 63], the leading one (unmasked) in [-64, 64]; digit plane s holds q_s = d_(S-1-s).  (Successive rint / subtract /
+// scale steps in FP64 cost ~150 instructions per element and made the pass issue-bound.)
+struct OzDigitizer {
+    int S, sh;
+    bool one_mul;
+    double mul;
+    long long bias;
+    int sq[OZ_MAX_S];  // sums of squared digits of the planes the diagonal correction needs (2 s >= S)
+    __device__ __forceinline__ OzDigitizer(int S_, int e) : S(S_), sh(6 - e + 7 * (S_ - 1)) {
+        one_mul = (sh > -1000 && sh < 1000);
+        mul = one_mul ? ldexp(1.0, sh) : 0.0;
+        bias = 0;
+        for (int jd = 0; jd < S; ++jd) bias += 64ll << (7 * jd);
+#pragma unroll
+        for (int s = 0; s < OZ_MAX_S; ++s) sq[s] = 0;
+    }
+    __device__ __forceinline__ void emit(const double (&x)[4], int8_t* dst, long long plane) {
+        long long G[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) G[u] = __double2ll_rn(one_mul ? x[u] * mul : ldexp(x[u], sh)) + bias;
+#pragma unroll
+        for (int s = 0; s < OZ_MAX_S; ++s) {
+            if (s < S) {
+                const int pos = 7 * (S - 1 - s);
+                int q[4];
+#pragma unroll
+                for (int u = 0; u < 4; ++u) q[u] = (s == 0) ? (int)(G[u] >> pos) - 64 : ((int)(G[u] >> pos) & 127) - 64;
+                *reinterpret_cast<char4*>(dst + (long long)s * plane) = make_char4((signed char)q[0], (signed char)q[1], (signed char)q[2], (signed char)q[3]);
+                if (2 * s >= S) sq[s] += q[0] * q[0] + q[1] * q[1] + q[2] * q[2] + q[3] * q[3];  // (N <= 65535: at most 64 x 4 x 4096 per thread)
+            }
+        }
+    }
+    __device__ __forceinline__ double corr() const {
+        double w = 0.0;
+#pragma unroll
+        for (int s = 0; s < OZ_MAX_S; ++s)
+            if (s < S && 2 * s >= S) w += ldexp((double)sq[s], -14 * s);
+        return w;
+    }
+};
+
 // ---------------------------------------------------------------------------------------------------
 // Slicing: one block per row.  digits[s][row][k] (int8, row pitch kpad, zero beyond N), scale[row] = 2^{e_row}.
 // ---------------------------------------------------------------------------------------------------
@@ -124,33 +168,80 @@ __global__ void __launch_bounds__(256) oz_split_kernel(const double* __restrict_
     __syncthreads();
     const int e = s_e;
     const long long plane = (long long)N * kpad;
-    double w = 0.0;
-    // two consecutive elements per thread and pass: whole 32-byte sectors per digit plane (kpad is a multiple of 64)
-    for (long long k0 = 2 * threadIdx.x; k0 < kpad; k0 += 512) {
-        double x0 = 0.0, x1 = 0.0;
-        if (vec && k0 + 1 < N) {
-            const double2 v = *reinterpret_cast<const double2*>(row + k0);
-            x0 = v.x;
-            x1 = v.y;
+    OzDigitizer dg(S, e);
+    // four consecutive elements per thread and pass: whole 32-byte sectors per digit plane (kpad is a multiple of 64)
+    for (long long k0 = 4 * threadIdx.x; k0 < kpad; k0 += 1024) {
+        double x[4] = {0.0, 0.0, 0.0, 0.0};
+        if (vec && k0 + 3 < N) {
+            const double2 v0 = *reinterpret_cast<const double2*>(row + k0), v1 = *reinterpret_cast<const double2*>(row + k0 + 2);
+            x[0] = v0.x; x[1] = v0.y; x[2] = v1.x; x[3] = v1.y;
         } else {
-            if (k0 < N) x0 = row[k0];
-            if (k0 + 1 < N) x1 = row[k0 + 1];
-        }
-        double t0 = ldexp(x0, 6 - e), t1 = ldexp(x1, 6 - e);   // |t| < 64
-        int8_t* dst = digits + (long long)r * kpad + k0;
-        double wt = 0.0;
 #pragma unroll
-        for (int s = 0; s < OZ_MAX_S; ++s) {
-            if (s < S) {
-                const double q0 = rint(t0), q1 = rint(t1);
-                t0 = (t0 - q0) * 128.0;                         // exact: |t - q| <= 1/2
-                t1 = (t1 - q1) * 128.0;
-                *reinterpret_cast<char2*>(dst + (long long)s * plane) = make_char2((signed char)(int)q0, (signed char)(int)q1);
-                if (2 * s >= S) wt += ldexp(q0 * q0 + q1 * q1, -14 * s);
-            }
+            for (int u = 0; u < 4; ++u)
+                if (k0 + u < N) x[u] = row[k0 + u];
         }
-        w += wt;
+        dg.emit(x, digits + (long long)r * kpad + k0, plane);
     }
+    double w = dg.corr();
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) w += __shfl_xor_sync(0xffffffffu, w, o);
+    __syncthreads();
+    if (lane == 0) s_red[wid] = w;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        for (int q = 1; q < 8; ++q) w += s_red[q];
+        corr[r] = w;
+    }
+}
+
+// The same with the row held in registers between the two phases (kpad <= 1024 PASSES): every load of the row is in flight
+// at once (a row per block and two dependent passes left ~24 KB per SM in flight: 0.37 of the HBM peak at N = 5000, and
+// 4.5 waves of latency-bound blocks at N = 2000) and the row is read once.
+template <int PASSES>
+__global__ void __launch_bounds__(256) oz_split_reg_kernel(const double* __restrict__ A, long long lda, int N, int S, int8_t* __restrict__ digits,
+                                                           long long kpad, double* __restrict__ scale, double* __restrict__ corr) {
+    __shared__ double s_red[8];
+    __shared__ int s_e;
+    const int r = blockIdx.x, lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    const double* row = A + (long long)r * lda;
+    const bool vec = ((lda & 1) == 0) && ((reinterpret_cast<uintptr_t>(A) & 15) == 0);
+    double x[PASSES][4];
+#pragma unroll
+    for (int i = 0; i < PASSES; ++i) {
+        const int k0 = 4 * threadIdx.x + 1024 * i;
+        if (vec && k0 + 3 < N) {
+            const double2 v0 = *reinterpret_cast<const double2*>(row + k0), v1 = *reinterpret_cast<const double2*>(row + k0 + 2);
+            x[i][0] = v0.x; x[i][1] = v0.y; x[i][2] = v1.x; x[i][3] = v1.y;
+        } else {
+#pragma unroll
+            for (int u = 0; u < 4; ++u) x[i][u] = (k0 + u < N) ? row[k0 + u] : 0.0;
+        }
+    }
+    double m = 0.0;
+#pragma unroll
+    for (int i = 0; i < PASSES; ++i)
+#pragma unroll
+        for (int u = 0; u < 4; ++u) m = fmax(m, fabs(x[i][u]));
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) m = fmax(m, __shfl_xor_sync(0xffffffffu, m, o));
+    if (lane == 0) s_red[wid] = m;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        for (int q = 1; q < 8; ++q) m = fmax(m, s_red[q]);
+        int e = 0;
+        if (m > 0.0 && isfinite(m)) (void)frexp(m, &e);
+        s_e = e;
+        scale[r] = ldexp(1.0, e);
+    }
+    __syncthreads();
+    OzDigitizer dg(S, s_e);
+    const long long plane = (long long)N * kpad;
+#pragma unroll
+    for (int i = 0; i < PASSES; ++i) {
+        const long long k0 = 4 * threadIdx.x + 1024 * i;
+        if (k0 < kpad) dg.emit(x[i], digits + (long long)r * kpad + k0, plane);
+    }
+    double w = dg.corr();
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) w += __shfl_xor_sync(0xffffffffu, w, o);
     __syncthreads();
