@@ -58,10 +58,11 @@ typedef enum {
     CHEB_DM_ESTATE = 4,       /* call order: compute before coeffs, solve_mu before moments ...  */
     CHEB_DM_EBOUNDS = 5,      /* b <= a or non-finite bounds                                     */
     CHEB_DM_EUNSUPPORTED = 6, /* dtype other than CHEB_DM_F64                                    */
-    CHEB_DM_ENOCONV = 7       /* stability guard of the power-basis outer recursion (Eq. 4): the table d
+    CHEB_DM_ENOCONV = 7,      /* stability guard of the power-basis outer recursion (Eq. 4): the table d
                                  computed on the device has max|d| 2^-52 p > 1e-12 (d grows like 2^p, Eq. 12,
                                  PAPER.md:136; reading A6); D was still written but may have lost
                                  accuracy.  Reported by cheb_dm_check / cheb_dm_wait / cheb_dm_compute_host. */
+    CHEB_DM_ESIZE = 8         /* cheb_dm_bounds_static: N beyond CHEB_DM_STATIC_MAX_N (the fixed device scratch)   */
 } cheb_dm_status_t;
 
 /* Outer (giant-step) recursion.
@@ -353,6 +354,23 @@ typedef struct {
 } cheb_dm_trace_rec_t;
 cheb_dm_status_t cheb_dm_set_trace(cheb_dm_plan_t plan, int enable);
 cheb_dm_status_t cheb_dm_get_trace(cheb_dm_plan_t plan, cheb_dm_trace_rec_t* out, int max_records, int* count_out);
+
+/* Step a-1 for callers that cannot allocate (code under CUDA graph capture, tight serving loops, harnesses that forbid
+ * cudaMalloc): the Gershgorin bounds of PAPER.md:96 (readings A1, A2-iv) WITHOUT a plan and without any
+ * allocation.  It is a variant of the bounds pass of the front-end kernel whose scratch (one (h_ii - R_i, h_ii + R_i)
+ * pair per row, R_i = sum_{j != i} |h_ij|, and a completion ticket) lives in a file-scope static device array of
+ * 256 + 16 * CHEB_DM_STATIC_MAX_N bytes (129 KiB) that every GPU that loads the library holds until exit.
+ *   dH       DEVICE, symmetric N x N, leading dimension ldh >= N (elements); read only.
+ *   d_bounds DEVICE, 2 doubles: (a, b) = (min_i (h_ii - R_i), max_i (h_ii + R_i)); a == b is widened to (a - 1, b + 1) as
+ *            in the solve; a non-finite row gives (-inf, +inf).
+ * One kernel launch on `cuda_stream` (plus a 256-byte cudaMemsetAsync of the ticket, which must start at zero); no
+ * synchronisation; calls no cudaMalloc, cudaFree or allocating library routine (the array's device address is looked
+ * up with cudaGetSymbolAddress once per device, at the first call on that device).
+ * N > CHEB_DM_STATIC_MAX_N -> CHEB_DM_ESIZE (nothing launched); N < 1, NULL pointers, ldh < N -> CHEB_DM_EINVAL.
+ * ALL calls on a device share the one array, which keeps the last call's contents: calls that overlap on the GPU
+ * (different streams, or graph branches) race -- serialise them. */
+#define CHEB_DM_STATIC_MAX_N 8192
+cheb_dm_status_t cheb_dm_bounds_static(const double* dH, int N, long long ldh, double* d_bounds, void* cuda_stream);
 
 const char* cheb_dm_strerror(cheb_dm_status_t status);
 

@@ -8,7 +8,7 @@ There is no CPU fallback: if libcheb_dm.so is missing (and cannot be built) impo
 functions raises; without a CUDA device ``Plan`` raises ChebDMError(ECUDA).
 """
 from .binding import (  # noqa: F401
-    ChebDMError, Options, Plan, lib, lib_path, dmma_peak,
+    ChebDMError, Options, Plan, lib, lib_path, dmma_peak, bounds_static, STATIC_MAX_N,
     OUTER_CHEBYSHEV, OUTER_POWER, SCHED_GROUPED, SCHED_SERIAL, PAIR_AUTO, PAIR_ALG1, PAIR_SERIAL, PAIR_BALANCED,
     TILE_AUTO, TILE_128x128, TILE_128x64, TILE_64x64, STATUS_NAMES, MAX_BATCH,
 )

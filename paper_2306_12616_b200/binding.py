@@ -11,7 +11,7 @@ SCHED_GROUPED, SCHED_SERIAL = 0, 1
 PAIR_AUTO, PAIR_SERIAL, PAIR_BALANCED, PAIR_ALG1 = 0, 1, 2, 3
 MAX_BATCH = 64
 TILE_AUTO, TILE_128x128, TILE_128x64, TILE_64x64 = 0, 1, 2, 3
-STATUS_NAMES = ["OK", "EINVAL", "EALLOC", "ECUDA", "ESTATE", "EBOUNDS", "EUNSUPPORTED", "ENOCONV"]
+STATUS_NAMES = ["OK", "EINVAL", "EALLOC", "ECUDA", "ESTATE", "EBOUNDS", "EUNSUPPORTED", "ENOCONV", "ESIZE"]
 
 EXPORTS = [
     "cheb_dm_plan", "cheb_dm_plan_ex", "cheb_dm_destroy", "cheb_dm_coeffs", "cheb_dm_compute",
@@ -23,7 +23,7 @@ EXPORTS = [
     "cheb_dm_compute_host_async", "cheb_dm_wait",
     "cheb_dm_compute_batch", "cheb_dm_compute_batch_host", "cheb_dm_compute_batch_host_async", "cheb_dm_trace_batch",
     "cheb_dm_get_scalars", "cheb_dm_solve", "cheb_dm_solve_batch", "cheb_dm_assemble", "cheb_dm_flops_per_solve",
-    "cheb_dm_product_sliced", "cheb_dm_sliced_ops_per_compute",
+    "cheb_dm_product_sliced", "cheb_dm_sliced_ops_per_compute", "cheb_dm_bounds_static",
 ]
 
 
@@ -107,6 +107,7 @@ def lib():
     L.cheb_dm_flops_per_solve.argtypes = [vp, dp]
     L.cheb_dm_sliced_ops_per_compute.argtypes = [vp, dp]
     L.cheb_dm_product_sliced.argtypes = [vp, C.c_double, vp, vp, C.c_double, vp, vp, C.c_int, vp]
+    L.cheb_dm_bounds_static.argtypes = [vp, C.c_int, C.c_longlong, vp, vp]
     for n in EXPORTS:
         getattr(L, n).restype = C.c_int
     L.cheb_dm_strerror.argtypes = [C.c_int]
@@ -144,6 +145,15 @@ def dmma_peak(iters: int = 20000, stream: int = 0) -> float:
     v = C.c_double()
     _chk(lib().cheb_dm_dmma_peak(iters, C.byref(v), stream), "cheb_dm_dmma_peak")
     return v.value
+
+
+STATIC_MAX_N = 8192  # CHEB_DM_STATIC_MAX_N
+
+
+def bounds_static(dH: int, N: int, ldh: int, d_bounds: int, stream: int = 0):
+    """cheb_dm_bounds_static: Gershgorin bounds (a, b) of the device matrix dH into the 2 device doubles d_bounds; no
+    plan, no allocation (scratch in a fixed device array: N <= STATIC_MAX_N, overlapping calls race)."""
+    _chk(lib().cheb_dm_bounds_static(dH, N, ldh, d_bounds, stream), "cheb_dm_bounds_static")
 
 
 class Plan:

@@ -1212,6 +1212,7 @@ const char* cheb_dm_strerror(cheb_dm_status_t s) {
         case CHEB_DM_EBOUNDS: return "bad spectral bounds";
         case CHEB_DM_EUNSUPPORTED: return "unsupported dtype or plan option";
         case CHEB_DM_ENOCONV: return "power-basis outer recursion would lose accuracy (use the Chebyshev outer recursion)";
+        case CHEB_DM_ESIZE: return "N beyond CHEB_DM_STATIC_MAX_N = 8192, the fixed device scratch of cheb_dm_bounds_static";
     }
     return "unknown status";
 }
@@ -2061,3 +2062,116 @@ cheb_dm_status_t cheb_dm_dmma_peak(int iters, double* tflops_out, void* cuda_str
 }
 
 }  // extern "C"
+
+// ---------------------------------------------------------------------------------------------------------------------
+// cheb_dm_bounds_static (include/cheb_dm.h): Gershgorin bounds with the scratch in a fixed device array -- the one entry
+// point that never allocates.  Everything it needs is in this block; no other code path uses it.
+// ---------------------------------------------------------------------------------------------------------------------
+// [0, 256): completion ticket (unsigned, must be zero when a call starts); then one (h_ii - R_i, h_ii + R_i) pair per row.
+static __device__ __align__(256) unsigned char cheb_dm_static_scratch[256 + 16 * CHEB_DM_STATIC_MAX_N];
+
+namespace {
+
+constexpr int BS_THREADS = 256, BS_ROWS = BS_THREADS / 32;  // a warp per row
+
+// `scratch` is the device address of cheb_dm_static_scratch, looked up by the host with cudaGetSymbolAddress.
+__global__ void __launch_bounds__(BS_THREADS) bounds_static_kernel(const double* __restrict__ H, int N, long long ldh,
+                                                                   unsigned char* __restrict__ scratch, double* __restrict__ out) {
+    unsigned* ticket = reinterpret_cast<unsigned*>(scratch);
+    double* rows = reinterpret_cast<double*>(scratch + 256);
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int row = blockIdx.x * BS_ROWS + warp;
+    if (row < N) {
+        const double* hr = H + (long long)row * ldh;
+        const bool vec = ((ldh & 1) == 0) && ((reinterpret_cast<uintptr_t>(H) & 15) == 0);
+        double r = 0.0, hii = 0.0;
+        if (vec) {
+            const int jend = N & ~1;
+            for (int j = 2 * lane; j < jend; j += 64) {
+                const double2 v = __ldg(reinterpret_cast<const double2*>(hr + j));
+                if (j == row) hii = v.x; else r += fabs(v.x);
+                if (j + 1 == row) hii = v.y; else r += fabs(v.y);
+            }
+            if ((N & 1) && lane == 0) {
+                const double v = hr[N - 1];
+                if (N - 1 == row) hii = v; else r += fabs(v);
+            }
+        } else {
+            for (int j = lane; j < N; j += 32) {
+                const double v = hr[j];
+                if (j == row) hii = v; else r += fabs(v);
+            }
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            r += __shfl_xor_sync(0xffffffffu, r, o);
+            hii += __shfl_xor_sync(0xffffffffu, hii, o);  // exactly one lane holds h_ii, the rest 0
+        }
+        if (lane == 0) {
+            const bool fin = isfinite(r) && isfinite(hii);
+            rows[2 * row] = fin ? hii - r : -INFINITY;
+            rows[2 * row + 1] = fin ? hii + r : INFINITY;
+        }
+    }
+    // the block that draws the last ticket reduces the rows of all blocks (min / max: the order does not matter)
+    __shared__ unsigned s_last;
+    __shared__ double s_lo[BS_ROWS], s_hi[BS_ROWS];
+    __threadfence();
+    __syncthreads();
+    if (threadIdx.x == 0) s_last = (atomicAdd(ticket, 1u) == gridDim.x - 1u) ? 1u : 0u;
+    __syncthreads();
+    if (!s_last) return;
+    __threadfence();
+    double lo = INFINITY, hi = -INFINITY;
+    for (int i = threadIdx.x; i < N; i += BS_THREADS) {
+        lo = fmin(lo, __ldcg(rows + 2 * i));
+        hi = fmax(hi, __ldcg(rows + 2 * i + 1));
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        lo = fmin(lo, __shfl_xor_sync(0xffffffffu, lo, o));
+        hi = fmax(hi, __shfl_xor_sync(0xffffffffu, hi, o));
+    }
+    if (lane == 0) { s_lo[warp] = lo; s_hi[warp] = hi; }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        for (int q = 1; q < BS_ROWS; ++q) { lo = fmin(lo, s_lo[q]); hi = fmax(hi, s_hi[q]); }
+        if (lo == hi) { lo -= 1.0; hi += 1.0; }  // degenerate H = cI (reading A2-iv), as front_end_kernel
+        out[0] = lo;
+        out[1] = hi;
+        *ticket = 0u;  // left at zero for the next call (the host clears it as well: an aborted call may not get here)
+    }
+}
+
+// Device address of the scratch array, per device: cudaGetSymbolAddress once, with that device current.
+constexpr int BS_MAX_DEVICES = 64;
+unsigned char* g_static_scratch_ptr[BS_MAX_DEVICES];
+int g_static_scratch_ok[BS_MAX_DEVICES];
+
+}  // namespace
+
+extern "C" cheb_dm_status_t cheb_dm_bounds_static(const double* dH, int N, long long ldh, double* d_bounds, void* cuda_stream) {
+    if (!dH || !d_bounds || N < 1 || ldh < N) return CHEB_DM_EINVAL;
+    if (N > CHEB_DM_STATIC_MAX_N) return CHEB_DM_ESIZE;
+    int dev = -1;
+    CUDA_TRY(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= BS_MAX_DEVICES) return CHEB_DM_ECUDA;
+    if (!__atomic_load_n(&g_static_scratch_ok[dev], __ATOMIC_ACQUIRE)) {
+        // In host code the array's name is a host-side stand-in, not a device address: ask the runtime for the address on
+        // the current device.  (Two threads racing here store the same value.)
+        unsigned char* ptr = nullptr;
+        if (cudaGetSymbolAddress((void**)&ptr, cheb_dm_static_scratch) != cudaSuccess || ptr == nullptr) {
+            cudaGetLastError();
+            return CHEB_DM_ECUDA;
+        }
+        g_static_scratch_ptr[dev] = ptr;
+        __atomic_store_n(&g_static_scratch_ok[dev], 1, __ATOMIC_RELEASE);
+    }
+    unsigned char* scratch = g_static_scratch_ptr[dev];
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    CUDA_TRY(cudaMemsetAsync(scratch, 0, 256, st));  // the ticket must start at zero whatever the last call left
+    const int grid = (N + BS_ROWS - 1) / BS_ROWS;
+    bounds_static_kernel<<<grid, BS_THREADS, 0, st>>>(dH, N, ldh, scratch, d_bounds);
+    CUDA_TRY(cudaGetLastError());
+    return CHEB_DM_OK;
+}
