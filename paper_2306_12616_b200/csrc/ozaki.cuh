@@ -88,22 +88,52 @@ __host__ __device__ constexpr uint32_t oz_idesc(int n) {
 // scale steps in FP64 cost ~150 instructions per element and made the pass issue-bound.)
 struct OzDigitizer {
     int S, sh;
-    bool one_mul;
-    double mul;
+    double m1, m2;     // 2^sh = m1 m2, both always representable (|sh| <= 1130); x m1 m2 is exact wherever x 2^sh >= 1/2
     long long bias;
     int sq[OZ_MAX_S];  // sums of squared digits of the planes the diagonal correction needs (2 s >= S)
     __device__ __forceinline__ OzDigitizer(int S_, int e) : S(S_), sh(6 - e + 7 * (S_ - 1)) {
-        one_mul = (sh > -1000 && sh < 1000);
-        mul = one_mul ? ldexp(1.0, sh) : 0.0;
+        m1 = ldexp(1.0, sh / 2);
+        m2 = ldexp(1.0, sh - sh / 2);
         bias = 0;
         for (int jd = 0; jd < S; ++jd) bias += 64ll << (7 * jd);
 #pragma unroll
         for (int s = 0; s < OZ_MAX_S; ++s) sq[s] = 0;
     }
+    // four 7-bit fields of x -> four bytes (everything from bit 21 up goes to byte 3: the leading digit has 8 bits), then
+    // field g = d + 64 -> the int8 d = (g + 64) ^ 0x80 in every byte at once (g + 64 <= 192: no carry between bytes)
+    static __device__ __forceinline__ uint32_t fields_to_int8x4(uint32_t x) {
+        const uint32_t w = (x & 0x7Fu) | ((x & 0x3F80u) << 1) | ((x & 0x1FC000u) << 2) | ((x & 0xFFE00000u) << 3);
+        return (w + 0x40404040u) ^ 0x80808080u;
+    }
     __device__ __forceinline__ void emit(const double (&x)[4], int8_t* dst, long long plane) {
         long long G[4];
 #pragma unroll
-        for (int u = 0; u < 4; ++u) G[u] = __double2ll_rn(one_mul ? x[u] * mul : ldexp(x[u], sh)) + bias;
+        for (int u = 0; u < 4; ++u) G[u] = __double2ll_rn(x[u] * m1 * m2) + bias;
+        if (S == 8) {
+            // 32-bit path: the low and the high 28 bits of G hold four digits each; bytes of an element's word = its
+            // digits, a 4 x 4 byte transpose (PRMT) turns the words of four elements into the words of four planes
+#pragma unroll
+            for (int h = 0; h < 2; ++h) {
+                uint32_t W[4];
+#pragma unroll
+                for (int u = 0; u < 4; ++u)
+                    W[u] = fields_to_int8x4(h == 0 ? (uint32_t)G[u] & 0x0FFFFFFFu : (uint32_t)((unsigned long long)G[u] >> 28));
+                const uint32_t t0 = __byte_perm(W[0], W[1], 0x5140), t1 = __byte_perm(W[2], W[3], 0x5140);
+                const uint32_t t2 = __byte_perm(W[0], W[1], 0x7362), t3 = __byte_perm(W[2], W[3], 0x7362);
+                uint32_t P[4];  // P[j]: digit 4 h + j (0 = least significant) of the four elements = plane 7 - (4 h + j)
+                P[0] = __byte_perm(t0, t1, 0x5410);
+                P[1] = __byte_perm(t0, t1, 0x7632);
+                P[2] = __byte_perm(t2, t3, 0x5410);
+                P[3] = __byte_perm(t2, t3, 0x7632);
+#pragma unroll
+                for (int j = 0; j < 4; ++j) {
+                    const int sp = 7 - (4 * h + j);
+                    *reinterpret_cast<uint32_t*>(dst + (long long)sp * plane) = P[j];
+                    if (h == 0) sq[sp] = __dp4a((int)P[j], (int)P[j], sq[sp]);   // planes 4..7 (2 s >= S)
+                }
+            }
+            return;
+        }
 #pragma unroll
         for (int s = 0; s < OZ_MAX_S; ++s) {
             if (s < S) {
