@@ -35,6 +35,19 @@ __global__ void unpad_copy_kernel(const double* __restrict__ src, long long ldx,
     }
 }
 
+// The same for a symmetric source of which only the symBM x symBN tiles that touch the lower triangle were formed
+// (form_sums with symmetric-tile skipping): an element of a skipped tile is read from its mirror image, which lies
+// strictly below the diagonal and therefore in a formed tile.
+__global__ void unpad_copy_sym_kernel(const double* __restrict__ src, long long ldx, int N, double* __restrict__ dst, long long ldd,
+                                      int symBM, int symBN) {
+    const long long total = (long long)N * N;
+    for (long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x; e < total; e += (long long)gridDim.x * blockDim.x) {
+        const int i = (int)(e / N), j = (int)(e - (long long)i * N);
+        const bool skipped = (i / symBM) * symBM + symBM - 1 < (j / symBN) * symBN;
+        dst[(long long)i * ldd + j] = skipped ? src[(long long)j * ldx + i] : src[(long long)i * ldx + j];
+    }
+}
+
 // ---------------------------------------------------------------------------------------------------
 // Double-double helpers (error-free transformations) for the scalar reductions: the parity gate on D
 // needs sum_n |delta c_n| << 1e-10 with N_q up to 8192 quadrature terms per coefficient.

@@ -1124,7 +1124,10 @@ cheb_dm_status_t sliced_table(cheb_dm_plan_s* P, const TaskTable& tt, int kind, 
         if (t.ktiles == 0) {
             // product-free step (l = p - 1): Out = G
             if (!G) return CHEB_DM_EUNSUPPORTED;
-            unpad_copy_kernel<<<P->num_sms * 4, 256, 0, st>>>(G, t.lds, P->N, Out, ldo);
+            if (P->sym)  // only the tiles of G that touch the lower triangle exist (sliced_giant)
+                unpad_copy_sym_kernel<<<P->num_sms * 4, 256, 0, st>>>(G, t.lds, P->N, Out, ldo, OZ_BM, OZ_BN);
+            else
+                unpad_copy_kernel<<<P->num_sms * 4, 256, 0, st>>>(G, t.lds, P->N, Out, ldo);
         } else {
             OzArgs oa;
             memset(&oa, 0, sizeof(oa));
@@ -1181,9 +1184,10 @@ cheb_dm_status_t sliced_baby(cheb_dm_plan_s* P, cudaStream_t st) {
     return sliced_table(P, P->baby, SLICED_BABY, nullptr, 0, st);
 }
 
-// Low-order sums (FP64, every element: the product-free step copies a whole G_l) and the giant steps.
+// Low-order sums (FP64; with symmetric tiles only the 128 x 64 tiles the products read: the product-free step, which
+// needs a whole matrix, mirrors the rest) and the giant steps.
 cheb_dm_status_t sliced_giant(cheb_dm_plan_s* P, double* userD, long long ldd, cudaStream_t st) {
-    cheb_dm_status_t s = form_sums(P, 1, true, OZ_BM, OZ_BN, st);
+    cheb_dm_status_t s = form_sums(P, 1, !P->sym, OZ_BM, OZ_BN, st);
     if (s != CHEB_DM_OK) return s;
     return sliced_table(P, P->giant, SLICED_GIANT, userD, ldd, st);
 }
