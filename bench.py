@@ -355,7 +355,7 @@ def measure_sliced(torch, cd, workloads, name, args, steps, warmup, flush, dist,
            "mu_inclusive": {"call": "cheb_dm_solve on the same plan (baby block and giant block sliced, nested giant steps)", "ms_per_solve": mi_ms / w.units,
                             "value": world * w.units / (mi_ms * 1e-3), "unit": UNIT, "tr_D": tr_mi},
            "full_product_equivalent_tflops": (plan.k + plan.p - 2) * 2.0 * w.N ** 3 / (kernel_ms * 1e-3) * 1e-12,
-           "roofline": {"bound": "tensor", "kernel": "oz_gemm_kernel<8> (tcgen05.mma kind::i8, 8 int32 accumulators in tensor memory) + oz_split_kernel + form_sums",
+           "roofline": {"bound": "tensor", "kernel": "oz_gemm_kernel<8> (tcgen05.mma kind::i8, 8 int32 accumulators in tensor memory) + oz_split_reg_kernel + form_sums",
                         "achieved": achieved, "peak": int8_peak, "unit": "TOP/s", "frac": achieved / int8_peak if int8_peak else None,
                         "peak_source": "MEASURED_PEAKS.json bf16_tflops (burst) x 2 (nominal int8 : bf16 ratio of the profiling guide)",
                         "kernel_ms": kernel_ms, "ops_per_launch": ops, "note": "kernel_ms spans all product launches of a solve, slicing passes and the sums pass included"},
