@@ -87,7 +87,7 @@ __global__ void __launch_bounds__(Cfg::THREADS, 1) gemm_epi_kernel(const LaunchA
     if (threadIdx.x == 0) {
         for (int s = 0; s < STAGES; ++s) {
             mbar_init(full_bar(s), 1);
-            mbar_init(empty_bar(s), Cfg::CONSUMER_WARPS);
+            mbar_init(empty_bar(s), Cfg::CONSUMER_WARPS / Cfg::KSPLIT);  // the warps that read the stage (see the K loop)
         }
         for (int s = 0; s < RING; ++s) {
             mbar_init(tfull_bar(s), 1);
@@ -443,35 +443,44 @@ __global__ void __launch_bounds__(Cfg::THREADS, 1) gemm_epi_kernel(const LaunchA
 #pragma unroll
             for (int j = 0; j < FN; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
 
-        // A stage goes back to the producer one iteration late (see gemm_dmma.cuh: the arrive may overtake loads in flight)
+        // A stage goes back to the producer one iteration late (see gemm_dmma.cuh: the arrive may overtake loads in flight).
+        // With two k-halves the halves take ALTERNATE k-tiles of the item (kh = kt & 1), each warp all k4-steps of its
+        // stages: the two warps of a scheduler sub-partition (w and w + 4) then work on different stages and one warp's
+        // wait behind a stage barrier (barrier, then the LDS latency in front of the first DMMAs: a quarter of the loop's
+        // stall samples) is covered by the other's DMMAs.  When both halves shared every stage they reached the barrier
+        // together and the DMMA pipe idled for both (per-instruction samples, profiles/r02_ablations.md section 7).
+        constexpr bool ALT = (Cfg::KSPLIT == 2);
+        constexpr int K4 = BK / 4;
         int prev_stage = -1;
         for (int kt = 0; kt < ktiles; ++kt) {
-            mbar_wait(full_bar(stage), phase);
-            if (tracing && kt == 0) trc[ti_slot * 4 + 1] = global_ns();
-            const uint8_t* sbase = smem + stage * Cfg::STAGE_BYTES + kh * (Cfg::K4_PER_HALF / 2) * 1024;
+            if (!ALT || (kt & 1) == kh) {
+                mbar_wait(full_bar(stage), phase);
+                if (tracing && kt == 0) trc[ti_slot * 4 + 1] = global_ns();
+                const uint8_t* sbase = smem + stage * Cfg::STAGE_BYTES;
 #pragma unroll
-            for (int j = 0; j < Cfg::K4_PER_HALF; ++j) {
-                const int jh = j >> 1, par = j & 1;
-                double a[FM], b[FN];
+                for (int j = 0; j < K4; ++j) {
+                    const int jh = j >> 1, par = j & 1;
+                    double a[FM], b[FN];
 #pragma unroll
-                for (int i = 0; i < FM; ++i)
-                    a[i] = *reinterpret_cast<const double*>(sbase + ((aoff[par] ^ ((i & 1) << 6)) + (i >> 1) * SLAB_BYTES + jh * 1024));
+                    for (int i = 0; i < FM; ++i)
+                        a[i] = *reinterpret_cast<const double*>(sbase + ((aoff[par] ^ ((i & 1) << 6)) + (i >> 1) * SLAB_BYTES + jh * 1024));
 #pragma unroll
-                for (int i = 0; i < FN; ++i)
-                    b[i] = *reinterpret_cast<const double*>(sbase + ((boff[par] ^ ((i & 1) << 6)) + (i >> 1) * SLAB_BYTES + jh * 1024));
-                if (j == 0 && prev_stage >= 0) {
-                    __syncwarp();
-                    if (lane == 0) mbar_arrive(empty_bar(prev_stage));
+                    for (int i = 0; i < FN; ++i)
+                        b[i] = *reinterpret_cast<const double*>(sbase + ((boff[par] ^ ((i & 1) << 6)) + (i >> 1) * SLAB_BYTES + jh * 1024));
+                    if (j == 0 && prev_stage >= 0) {
+                        __syncwarp();
+                        if (lane == 0) mbar_arrive(empty_bar(prev_stage));
+                    }
+#pragma unroll
+                    for (int im = 0; im < FM; ++im)
+#pragma unroll
+                        for (int jn = 0; jn < FN; ++jn) dmma_884(acc[im][jn][0], acc[im][jn][1], a[im], b[jn]);
                 }
-#pragma unroll
-                for (int im = 0; im < FM; ++im)
-#pragma unroll
-                    for (int jn = 0; jn < FN; ++jn) dmma_884(acc[im][jn][0], acc[im][jn][1], a[im], b[jn]);
+                prev_stage = stage;
             }
-            prev_stage = stage;
             if (++stage == STAGES) { stage = 0; phase ^= 1; }
         }
-        {
+        if (prev_stage >= 0) {
             __syncwarp();
             int dep = 0;
 #pragma unroll
