@@ -86,7 +86,7 @@ __global__ void __launch_bounds__(GR_THREADS, 1) giant_resident_kernel(const Gia
         for (int g = 0; g < 2; ++g) {
             for (int s = 0; s < GR_STAGES; ++s) {
                 mbar_init(full_bar(g, s), 1);
-                mbar_init(empty_bar(g, s), GR_CONSUMER_WARPS);
+                mbar_init(empty_bar(g, s), GR_CONSUMER_WARPS / 2);  // the k-half that reads the stage
             }
             mbar_init(stored_bar(g), GR_CONSUMER_WARPS / 2);  // the four epilogue warps
         }
@@ -330,42 +330,46 @@ __global__ void __launch_bounds__(GR_THREADS, 1) giant_resident_kernel(const Gia
             const int ns_ = (g + 1 < npanels) ? s : s + 1, ng_ = (g + 1 < npanels) ? g + 1 : 0;  // next tile
             if (kts == 0) load_pre(ns_, ng_, nxt);
             int prev_stage = -1;  // stages are released one iteration late (see gemm_dmma.cuh)
+            // the two k-halves take ALTERNATE k-tiles (kh = kt & 1), all eight k4-steps of their stages: the two warps of a
+            // scheduler sub-partition (w, w + 4) then never wait behind the same stage barrier together
             for (int kt = 0; kt < kts; ++kt) {
-                mbar_wait(full_bar(g, stage[g]), phase[g]);
-                if (kt == 0) {
-                    // the late dependencies of this tile hold: fetch C now, and the next tile's G one tile ahead
-                    if (tracing) t_first = global_ns();
-                    if (kh == 0 && Cp != nullptr) {  // workspace matrix: even ld, 16-byte aligned rows, zero pad columns
+                if ((kt & 1) == kh) {
+                    mbar_wait(full_bar(g, stage[g]), phase[g]);
+                    if (kt == 0) {
+                        // the late dependencies of this tile hold: fetch C now, and the next tile's G one tile ahead
+                        if (tracing) t_first = global_ns();
+                        if (Cp != nullptr) {  // workspace matrix: even ld, 16-byte aligned rows, zero pad columns (kh == 0 here)
 #pragma unroll
-                        for (int i = 0; i < 2; ++i)
+                            for (int i = 0; i < 2; ++i)
 #pragma unroll
-                            for (int j = 0; j < 2; ++j)
-                                if (row0 + i * 8 < N && col0 + j * 8 < N)
-                                    creg[i][j] = __ldcg(reinterpret_cast<const double2*>(Cp + (long long)(row0 + i * 8) * ldc + col0 + j * 8));
+                                for (int j = 0; j < 2; ++j)
+                                    if (row0 + i * 8 < N && col0 + j * 8 < N)
+                                        creg[i][j] = __ldcg(reinterpret_cast<const double2*>(Cp + (long long)(row0 + i * 8) * ldc + col0 + j * 8));
+                        }
+                        load_pre(ns_, ng_, nxt);
                     }
-                    load_pre(ns_, ng_, nxt);
+                    const uint8_t* sa = a_res + kt * GR_TILE_BYTES;
+                    const uint8_t* sbm = ring0 + (g * GR_STAGES + stage[g]) * GR_TILE_BYTES;
+#pragma unroll
+                    for (int j = 0; j < GR_BK / 4; ++j) {
+                        const int jh = j >> 1, par = j & 1;
+                        double a[2], b[2];
+#pragma unroll
+                        for (int i = 0; i < 2; ++i) {
+                            a[i] = *reinterpret_cast<const double*>(sa + ((aoff[par] ^ ((i & 1) << 6)) + jh * 1024));
+                            b[i] = *reinterpret_cast<const double*>(sbm + ((boff[par] ^ ((i & 1) << 6)) + jh * 1024));
+                        }
+                        if (j == 0 && prev_stage >= 0) {  // previous stage back to the producer (after this stage's barrier)
+                            __syncwarp();
+                            if (lane == 0) mbar_arrive(empty_bar(g, prev_stage));
+                        }
+#pragma unroll
+                        for (int im = 0; im < 2; ++im)
+#pragma unroll
+                            for (int jn = 0; jn < 2; ++jn) dmma_884(acc[im][jn][0], acc[im][jn][1], a[im], b[jn]);
+                    }
+                    prev_stage = stage[g];
                 }
-                const uint8_t* sa = a_res + kt * GR_TILE_BYTES + kh * 2048;  // k4-steps [4 kh, 4 kh + 4): k-rows [16 kh, 16 kh + 16)
-                const uint8_t* sbm = ring0 + (g * GR_STAGES + stage[g]) * GR_TILE_BYTES + kh * 2048;
-#pragma unroll
-                for (int j = 0; j < GR_BK / 8; ++j) {
-                    const int jh = j >> 1, par = j & 1;
-                    double a[2], b[2];
-#pragma unroll
-                    for (int i = 0; i < 2; ++i) {
-                        a[i] = *reinterpret_cast<const double*>(sa + ((aoff[par] ^ ((i & 1) << 6)) + jh * 1024));
-                        b[i] = *reinterpret_cast<const double*>(sbm + ((boff[par] ^ ((i & 1) << 6)) + jh * 1024));
-                    }
-                    if (j == 0 && prev_stage >= 0) {  // previous stage back to the producer (after this stage's barrier)
-                        __syncwarp();
-                        if (lane == 0) mbar_arrive(empty_bar(g, prev_stage));
-                    }
-#pragma unroll
-                    for (int im = 0; im < 2; ++im)
-#pragma unroll
-                        for (int jn = 0; jn < 2; ++jn) dmma_884(acc[im][jn][0], acc[im][jn][1], a[im], b[jn]);
-                }
-                prev_stage = stage[g];
                 if (++stage[g] == GR_STAGES) { stage[g] = 0; phase[g] ^= 1; }
             }
             if (prev_stage >= 0) {
