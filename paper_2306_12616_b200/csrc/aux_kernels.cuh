@@ -657,6 +657,7 @@ __global__ void __launch_bounds__(512) mu_bisect_kernel(DevScalars* sc_all, doub
     __shared__ dd s_part[8][16];
     __shared__ double s_nepts[8];
     __shared__ double s_lo, s_hi, s_ne;
+    __shared__ int s_fixed;  // a pass left [lo, hi] unchanged: every further halving is a no-op
     DevScalars* sc = sc_all + blockIdx.x;
     const double* w = w_all + (size_t)blockIdx.x * Nq;
     const double n_occ = B.n_occ[blockIdx.x];
@@ -664,7 +665,7 @@ __global__ void __launch_bounds__(512) mu_bisect_kernel(DevScalars* sc_all, doub
     const double beta_t = beta * (b - a) * 0.5;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nw = blockDim.x >> 5;
     const int c = threadIdx.x & 7, grp = threadIdx.x >> 3, ngrp = blockDim.x >> 3;
-    if (threadIdx.x == 0) { s_lo = a; s_hi = b; s_ne = 0.0; }
+    if (threadIdx.x == 0) { s_lo = a; s_hi = b; s_ne = 0.0; s_fixed = 0; }
     __syncthreads();
     int done = 0;
     while (done <= iters) {
@@ -737,13 +738,18 @@ __global__ void __launch_bounds__(512) mu_bisect_kernel(DevScalars* sc_all, doub
                             if (r == q) m_q = mid[r];
                         if (s_nepts[q - 1] < n_occ) { lo = m_q; q = 2 * q + 1; } else { hi = m_q; q = 2 * q; }
                     }
+                    // (the interval reaches the spacing of the doubles after ~60 halvings; the state is a function of
+                    // (lo, hi) alone, so once a pass does not move it the remaining halvings would not either)
+                    if (lo == lo_[1] && hi == hi_[1]) s_fixed = 1;
                     s_lo = lo;
                     s_hi = hi;
                 }
             }
         }
         __syncthreads();
-        done += (done == iters) ? 1 : levels;
+        if (done == iters) done += 1;
+        else if (s_fixed) done = iters;  // skip the no-op halvings; the result is bitwise that of `iters` halvings
+        else done += levels;
     }
     if (threadIdx.x == 0) {
         sc->mu = 0.5 * (s_lo + s_hi);
