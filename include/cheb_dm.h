@@ -256,6 +256,8 @@ cheb_dm_status_t cheb_dm_moments(cheb_dm_plan_t plan, const double* dH, double* 
 /* Chemical potential for a target electron count: solves N_e(mu) = sum_n c_n(mu) tau_n = n_occ by
  * bisection on [a,b] with exactly `iters` halvings (if N_e(mid) < n_occ then lo = mid else
  * hi = mid; result (lo+hi)/2), all on the device; mu_out: host pointer.  Synchronises the stream.
+ * (The kernel stops once a pass leaves [lo, hi] unchanged -- the interval has reached the spacing of the doubles and the
+ * remaining halvings are no-ops -- so the result is bitwise that of `iters` halvings.)
  * ESTATE unless cheb_dm_moments() ran on this plan. */
 cheb_dm_status_t cheb_dm_solve_mu(cheb_dm_plan_t plan, double beta, double n_occ, int iters,
                                   double* mu_out, void* cuda_stream);
