@@ -1363,7 +1363,7 @@ cheb_dm_status_t cheb_dm_plan_ex(cheb_dm_plan_t* plan, int N, int M_terms, cheb_
         // (the epilogue warps of gemm_epi.cuh cannot gather k-1 tiles per item as fast as the consumers finish small-N
         // items: with those tile shapes the sums are always pre-formed)
         if (mode == 0) mode = (((double)k * (double)P->mat_elems * 8.0 * P->maxb > 96.0 * 1024 * 1024 || is_epi_tile(P->tile)) && k > 2 && p > 1) ? 2 : 1;
-        if (o.sliced_solve && k > 1 && p > 1) mode = 2;  // the sliced products add one pre-formed FP64 tile
+        if (o.sliced_solve) mode = 2;  // the sliced products add one pre-formed FP64 tile (any k, p: also G_l = g_l0 I for k = 1)
         P->preformed = (mode == 2) ? 1 : 0;
         P->opt.fuse_sums = mode;
     }

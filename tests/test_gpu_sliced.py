@@ -192,7 +192,8 @@ def test_sliced_solve_full_size(cfg):
 
 
 @pytest.mark.parametrize("cfg,seed,n,M,opts", [("cfg1", 0, 300, None, {}), ("cfg2", 0, 250, None, {}), ("cfg3", 0, 200, 1024, {}),
-                                                ("cfg4", 0, 200, 2048, {}), ("cfg1", 2, 130, 60, dict(k=6, p=10)), ("cfg1", 0, 64, 12, dict(k=6, p=2))])
+                                                ("cfg4", 0, 200, 2048, {}), ("cfg1", 2, 130, 60, dict(k=6, p=10)), ("cfg1", 0, 64, 12, dict(k=6, p=2)),
+                                                ("cfg1", 1, 70, 8, dict(k=8, p=1)), ("cfg1", 1, 70, 6, dict(k=1, p=6)), ("cfg0", 0, 33, 9, dict(k=3, p=3))])
 def test_sliced_mu_inclusive_solve(cfg, seed, n, M, opts):
     """cheb_dm_solve / cheb_dm_moments / cheb_dm_assemble on a sliced_solve plan: baby block and giant block on the int8
     path, moments by the Gram kernel, bisection, nested giant steps; (tau, mu, D) against the oracle as in test_gpu_solve."""
@@ -250,4 +251,34 @@ def test_sliced_mu_inclusive_solve_full_size_cfg2():
     print(f"cfg2: sliced cheb_dm_solve mu = {mu:.12f} (oracle {case['mu']:.12f}), max|dD| = {err:.3e}")
     assert err <= 1e-10
     assert abs(float(np.trace(D)) - case["nocc"]) <= 1e-6
+    plan.destroy()
+
+
+@pytest.mark.parametrize("n,M,k,p,ldh,ldd", [(130, 12, 12, 1, 130, 137), (65, 8, 1, 8, 66, 65), (200, 9, 3, 3, 208, 203), (129, 2, 2, 1, 129, 129)])
+def test_sliced_solve_degenerate_shapes_and_pitches(n, M, k, p, ldh, ldd):
+    """p = 1 (no product in the outer sum: D = G_0, written through the mirroring copy of the lower-triangle sums), k = 1 (no
+    baby step: the multiplier is X itself), padded and odd pitches of H and D; the padding of D is never written."""
+    oracle, cd, workloads, gu = _imports()
+    torch = gu.torch_cuda()
+    st = torch.cuda.current_stream().cuda_stream
+    H = workloads.hamiltonian("cfg1", seed=5, n=n)
+    a, b = oracle.gershgorin(H)
+    beta, mu = 6.0, 0.05
+    D_or = oracle.dm_cheb(H, a, b, oracle.cheb_coeffs(beta, mu, a, b, M))
+    Hp = np.full((n, ldh), 4.25)
+    Hp[:, :n] = H
+    dH = gu.to_dev(Hp)
+    dD = torch.full((n, ldd), -7.0, dtype=torch.float64, device="cuda")
+    dtr = torch.zeros(1, dtype=torch.float64, device="cuda")
+    plan = cd.Plan(n, M, k=k, p=p, ldh=ldh, ldd=ldd, sliced_solve=1)
+    assert (plan.k, plan.p) == (k, p)
+    plan.coeffs(beta, mu, None)
+    plan.compute(dH.data_ptr(), dD.data_ptr(), st)
+    plan.trace(dD.data_ptr(), dtr.data_ptr(), st)
+    plan.check(st)
+    got = dD.cpu().numpy()
+    assert np.max(np.abs(got[:, :n] - D_or)) <= 1e-10
+    assert np.all(got[:, n:] == -7.0)
+    assert abs(float(dtr.item()) - float(np.trace(D_or))) <= 1e-9
+    assert np.max(np.abs(got[:, :n] - got[:, :n].T)) <= 1e-11
     plan.destroy()
