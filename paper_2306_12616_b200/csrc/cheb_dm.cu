@@ -793,8 +793,10 @@ cheb_dm_status_t front_end(cheb_dm_plan_s* P, int nb, const double* const* dH, l
 
 // Low-order sums G_l = sum_i coef_{i,l} T_i of Eq. (21) for all l at once (a-5, batched form), nb matrices.
 // full = true: every element (the G_l are operands of the long-K product); false: only the tiles the giant steps read.
-cheb_dm_status_t form_sums(cheb_dm_plan_s* P, int nb, bool full, int tileM, int tileN, cudaStream_t st) {
-    const double* coefT = (P->opt.outer == CHEB_DM_OUTER_POWER) ? P->dT : P->gT;
+// cheb_tables: the sums multiply U_l = T_l(T_k) (long-K assembly of cheb_dm_solve / cheb_dm_assemble), so their coefficients
+// are the Chebyshev table g whatever the outer recursion of the plan.
+cheb_dm_status_t form_sums(cheb_dm_plan_s* P, int nb, bool full, int tileM, int tileN, cudaStream_t st, bool cheb_tables = false) {
+    const double* coefT = (P->opt.outer == CHEB_DM_OUTER_POWER && !cheb_tables) ? P->dT : P->gT;
     const int symBM = (P->sym && !full) ? tileM : 0;
     if (P->scalar_sums) {  // FP64-FMA version (ablation)
         const long long pairs = (long long)P->N * P->ld / 2;
@@ -941,7 +943,7 @@ cheb_dm_status_t assemble_impl(cheb_dm_plan_s* P, int nb, const double* mu, int 
     if (s != CHEB_DM_OK) return s;
     // sliced path: the nested giant steps on the digit sets left by the blocks (T_k; the accumulators are re-sliced)
     if (P->oz_solve) return sliced_giant(P, dD[0], ldd, st);
-    s = form_sums(P, nb, true, P->BM, P->BN, st);
+    s = form_sums(P, nb, true, P->BM, P->BN, st, true);
     if (s != CHEB_DM_OK) return s;
     return run_table(P, P->flat, nb, dD, ldd, st);
 }

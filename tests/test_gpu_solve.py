@@ -38,7 +38,9 @@ def _oracle_solution(oracle, workloads, cfg, seed, n, M):
 CASES = [("cfg0", 0, 128, None, {}), ("cfg1", 0, 300, None, {}), ("cfg1", 1, 257, None, {}), ("cfg2", 0, 250, None, {}),
          ("cfg3", 0, 200, 1024, {}), ("cfg4", 0, 200, 2048, {}), ("cfg1", 2, 130, 60, dict(k=6, p=10)),
          ("cfg1", 0, 64, 12, dict(k=12, p=1)), ("cfg1", 0, 64, 12, dict(k=1, p=12)), ("cfg1", 0, 64, 12, dict(k=6, p=2)),
-         ("cfg2", 0, 150, 70, dict(k=2, p=35, tile=3)), ("cfg1", 3, 700, 64, dict(tile=1)), ("cfg1", 3, 333, 64, dict(symmetric=1))]
+         ("cfg2", 0, 150, 70, dict(k=2, p=35, tile=3)), ("cfg1", 3, 700, 64, dict(tile=1)), ("cfg1", 3, 333, 64, dict(symmetric=1)),
+         # power-basis outer recursion (Eq. 4): the long-K assembly still runs on the Chebyshev table g (its operands are U_l = T_l(T_k))
+         ("cfg1", 2, 127, 10, dict(k=3, p=4, outer=1)), ("cfg0", 0, 128, None, dict(outer=1))]
 
 
 @pytest.mark.parametrize("cfg,seed,n,M,opts", CASES)
