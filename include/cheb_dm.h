@@ -275,7 +275,8 @@ cheb_dm_status_t cheb_dm_solve_mu(cheb_dm_plan_t plan, double beta, double n_occ
  * cheb_dm_assemble: D for NEW chemical potentials from the blocks left in the workspace by the last
  * cheb_dm_moments / cheb_dm_solve[_batch] call on the same matrices (each new mu costs the coefficient tables,
  * the sums and one long-K product -- the use in a self-consistency or MD loop); mu: HOST array of nbatch values.
- * ESTATE if no such call preceded or nbatch differs. */
+ * ESTATE if no such call preceded, nbatch differs, or cheb_dm_coeffs changed the bounds (or the bounds mode) since: the
+ * blocks are polynomials of X(a, b).  A new beta alone keeps them (beta is read at the call). */
 cheb_dm_status_t cheb_dm_solve(cheb_dm_plan_t plan, const double* dH, double n_occ, int iters, double* dD,
                                double* mu_out, void* cuda_stream);
 cheb_dm_status_t cheb_dm_solve_batch(cheb_dm_plan_t plan, int nbatch, const double* const* dH, const double* n_occ,

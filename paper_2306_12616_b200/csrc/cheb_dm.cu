@@ -1373,6 +1373,12 @@ cheb_dm_status_t cheb_dm_plan_ex(cheb_dm_plan_t* plan, int N, int M_terms, cheb_
         P->preformed = 1;
         P->opt.fuse_sums = 2;
     }
+    if (P->resident && !P->preformed) {
+        // a batch plan whose giant-step tasks gather the sums in their epilogues (fuse_sums = 1): the resident kernel reads
+        // one pre-formed G tile per step, so single solves on such a plan (nbatch = 1) run in the generic kernel too
+        P->resident = 0;
+        P->opt.giant = 1;
+    }
     const bool need_G = P->preformed || P->resident || P->moments_on;
     P->off_G = need_G ? k + NBUF : -1;
     P->off_U = (P->moments_on && p >= 3) ? k + NBUF + (need_G ? p : 0) : -1;
@@ -1562,6 +1568,16 @@ cheb_dm_status_t cheb_dm_coeffs(cheb_dm_plan_t P, double beta, double mu, const 
     if (!isfinite(beta) || !isfinite(mu) || !(beta > 0.0)) return CHEB_DM_EINVAL;
     if (bounds) {
         if (!isfinite(bounds[0]) || !isfinite(bounds[1]) || !(bounds[1] > bounds[0])) return CHEB_DM_EBOUNDS;
+    }
+    // The blocks a cheb_dm_moments / cheb_dm_solve call left in the workspace are polynomials of X = X(a, b): new bounds (or
+    // a new bounds mode) make them stale -- cheb_dm_assemble / cheb_dm_solve_mu then return ESTATE instead of a D for the old
+    // scaling.  A new beta or mu alone keeps them.
+    const int was_explicit = P->explicit_bounds;
+    if ((bounds != nullptr) != (was_explicit != 0) || (bounds && (bounds[0] != P->a || bounds[1] != P->b))) {
+        P->blocks_nb = 0;
+        P->have_moments = 0;
+    }
+    if (bounds) {
         P->a = bounds[0];
         P->b = bounds[1];
         P->explicit_bounds = 1;

@@ -163,3 +163,33 @@ def test_batch_argument_checks():
         cd.Plan(16, 4, max_batch=65)
     assert ei.value.status == 1
     plan.destroy()
+
+
+@pytest.mark.parametrize("n,tile", [(200, 0), (129, 4), (64, 7), (300, 0)])
+def test_single_solves_on_a_batch_plan(n, tile):
+    """cheb_dm_compute, cheb_dm_compute_batch with nbatch = 1 and cheb_dm_compute_host on a plan made with max_batch = 3 at
+    N < 450, where the batch's giant-step tasks gather the sums in their epilogues: the resident-multiplier kernel (which
+    reads pre-formed sums) must not take such a solve."""
+    oracle, cd, workloads, gu, oc = _imports()
+    torch = gu.torch_cuda()
+    st = torch.cuda.current_stream().cuda_stream
+    M, beta, mu = 24, 9.0, 0.04
+    H = workloads.hamiltonian("cfg1", seed=2, n=n)
+    a, b = oracle.gershgorin(H)
+    D_or = oracle.dm_cheb(H, a, b, oracle.cheb_coeffs(beta, mu, a, b, M))
+    plan = cd.Plan(n, M, max_batch=3, tile=tile)
+    plan.coeffs(beta, mu, None)
+    dH = gu.to_dev(H)
+    dD = torch.full((n, n), float("nan"), dtype=torch.float64, device="cuda")
+    plan.compute(dH.data_ptr(), dD.data_ptr(), st)
+    plan.check(st)
+    assert np.max(np.abs(dD.cpu().numpy() - D_or)) <= TOL_D
+    dD.fill_(float("nan"))
+    plan.compute_batch([dH.data_ptr()], [dD.data_ptr()], [mu], st)
+    plan.check(st)
+    assert np.max(np.abs(dD.cpu().numpy() - D_or)) <= TOL_D
+    hH = torch.from_numpy(H.copy()).pin_memory()
+    hD = torch.empty((n, n), dtype=torch.float64).pin_memory()
+    plan.compute_host(hH.data_ptr(), hD.data_ptr(), 0, st)
+    assert np.max(np.abs(hD.numpy() - D_or)) <= TOL_D
+    plan.destroy()

@@ -134,3 +134,39 @@ def test_solve_needs_the_moments_option_and_call_order():
         plan.assemble([0.0], [dD.data_ptr()])
     assert ei.value.status == 4
     plan.destroy()
+
+
+def test_assemble_after_new_coeffs_beta_keeps_the_blocks_new_bounds_do_not():
+    """The blocks a solve leaves behind are polynomials of X(a, b): cheb_dm_coeffs with a new beta keeps them (assemble gives
+    the D of the new beta), with new bounds or a new bounds mode it invalidates them (ESTATE) -- never a D for the old
+    scaling."""
+    oracle, cd, workloads, gu = _imports()
+    torch = gu.torch_cuda()
+    st = torch.cuda.current_stream().cuda_stream
+    n, M = 129, 14
+    H = workloads.hamiltonian("cfg1", seed=6, n=n)
+    a, b = oracle.gershgorin(H)
+    dH, dD = gu.to_dev(H), torch.empty((n, n), dtype=torch.float64, device="cuda")
+    plan = cd.Plan(n, M)
+    plan.coeffs(5.0, 0.0, None)
+    plan.solve(dH.data_ptr(), 0.4 * n, dD.data_ptr(), 100, True, st)
+    plan.coeffs(12.0, 0.0, None)                     # beta only
+    plan.assemble([0.2], [dD.data_ptr()], st)
+    plan.check(st)
+    D_or = oracle.dm_cheb(H, a, b, oracle.cheb_coeffs(12.0, 0.2, a, b, M))
+    assert np.max(np.abs(dD.cpu().numpy() - D_or)) <= 1e-10
+    plan.coeffs(12.0, 0.0, (a - 1.0, b + 1.0))       # explicit bounds: another X
+    for call in (lambda: plan.assemble([0.2], [dD.data_ptr()], st), lambda: plan.solve_mu(12.0, 0.4 * n, 100, st)):
+        with pytest.raises(cd.ChebDMError) as ei:
+            call()
+        assert ei.value.status == 4
+    plan.solve(dH.data_ptr(), 0.4 * n, dD.data_ptr(), 100, True, st)    # blocks for the explicit bounds
+    plan.assemble([0.2], [dD.data_ptr()], st)
+    plan.check(st)
+    D_or = oracle.dm_cheb(H, a - 1.0, b + 1.0, oracle.cheb_coeffs(12.0, 0.2, a - 1.0, b + 1.0, M))
+    assert np.max(np.abs(dD.cpu().numpy() - D_or)) <= 1e-10
+    plan.coeffs(12.0, 0.0, None)                     # back to Gershgorin bounds: stale again
+    with pytest.raises(cd.ChebDMError) as ei:
+        plan.assemble([0.2], [dD.data_ptr()], st)
+    assert ei.value.status == 4
+    plan.destroy()
