@@ -1348,7 +1348,10 @@ cheb_dm_status_t cheb_dm_plan_ex(cheb_dm_plan_t* plan, int N, int M_terms, cheb_
     if (o.giant != 1 && N <= 32 * GR_MAX_KTILES && p >= 2 && P->BK == GR_BK && P->box_slabs == 2 &&
         o.sched == CHEB_DM_SCHED_GROUPED && P->res_grid <= P->num_sms &&
         (long long)k * GR_SUM_CHUNK * 8 <= 2ll * GR_STAGES * GR_TILE_BYTES) {
-        if (cudaFuncSetAttribute(giant_resident_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, P->res_smem) == cudaSuccess) {
+        // (the attribute belongs to the kernel, not to the plan: opt in to the largest size any plan can ask for, or a later plan
+        // for a smaller N would lower it under the feet of an earlier one)
+        if (cudaFuncSetAttribute(giant_resident_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                 giant_resident_smem_bytes(GR_MAX_KTILES)) == cudaSuccess) {
             int per_sm = 0;
             if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, giant_resident_kernel, GR_THREADS, P->res_smem) == cudaSuccess && per_sm >= 1)
                 P->resident = 1;

@@ -641,3 +641,35 @@ def test_host_entry_points_sync_and_pipelined():
     plan.compute_host(hH[2].data_ptr(), out.data_ptr(), tr1.data_ptr(), st)
     assert np.array_equal(out.numpy(), ref[2])
     plan.destroy()
+
+
+def test_several_plans_alive_at_once_and_launched_on_separate_streams():
+    """A later plan must not change what an earlier one needs (kernel attributes are per kernel, not per plan: a plan for a
+    smaller N once lowered the resident kernel's shared-memory opt-in), and plans launched on separate streams run
+    concurrently without sharing anything but the GPU."""
+    oracle, cd, workloads, gu, _ = _imports()
+    torch = gu.torch_cuda()
+    specs = [(500, 8, {}), (200, 12, {}), (129, 10, dict(max_batch=2)), (300, 9, dict(sliced_solve=1))]
+    plans, data = [], []
+    for n, M, opts in specs:                      # the N = 500 plan first, smaller ones after it
+        plan = cd.Plan(n, M, **opts)
+        plan.coeffs(7.0, 0.03, None)
+        nb = opts.get("max_batch", 1)
+        Hs = [workloads.hamiltonian("cfg1", seed=40 + n + q, n=n) for q in range(nb)]
+        plans.append(plan)
+        data.append((Hs, [gu.to_dev(h) for h in Hs], [torch.full((n, n), float("nan"), dtype=torch.float64, device="cuda") for _ in Hs]))
+    streams = [torch.cuda.Stream() for _ in specs]
+    torch.cuda.synchronize()
+    for rep in range(2):
+        for (n, M, opts), plan, (Hs, dH, dD), s in zip(specs, plans, data, streams):
+            if len(Hs) == 1:
+                plan.compute(dH[0].data_ptr(), dD[0].data_ptr(), s.cuda_stream)
+            else:
+                plan.compute_batch([x.data_ptr() for x in dH], [x.data_ptr() for x in dD], [0.03] * len(Hs), s.cuda_stream)
+    torch.cuda.synchronize()
+    for (n, M, opts), plan, (Hs, dH, dD), s in zip(specs, plans, data, streams):
+        plan.check(s.cuda_stream)
+        for H, d in zip(Hs, dD):
+            a, b = oracle.gershgorin(H)
+            assert np.max(np.abs(d.cpu().numpy() - oracle.dm_cheb(H, a, b, oracle.cheb_coeffs(7.0, 0.03, a, b, M)))) <= TOL_D
+        plan.destroy()
