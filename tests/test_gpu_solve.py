@@ -170,3 +170,71 @@ def test_assemble_after_new_coeffs_beta_keeps_the_blocks_new_bounds_do_not():
         plan.assemble([0.2], [dD.data_ptr()], st)
     assert ei.value.status == 4
     plan.destroy()
+
+
+def test_cuda_graph_capture_of_the_mu_inclusive_sliced_and_static_entry_points():
+    """cheb_dm_solve[_batch] with mu_out = NULL (mu never leaves the device), cheb_dm_assemble, the sliced solve and
+    cheb_dm_bounds_static allocate nothing and never synchronise: each is captured into a CUDA graph and its replays on new
+    H contents are bit-identical to the eager calls."""
+    oracle, cd, workloads, gu = _imports()
+    torch = gu.torch_cuda()
+    n, M, beta = 200, 30, 12.0
+    Hs = [workloads.hamiltonian("cfg1", seed=s, n=n) for s in range(3)]
+
+    def blocks_plan():
+        p = cd.Plan(n, M)
+        p.coeffs(beta, 0.02, None)
+        d, o = gu.to_dev(Hs[0]), torch.empty((n, n), dtype=torch.float64, device="cuda")
+        p.solve(d.data_ptr(), 80.0, o.data_ptr(), 100, True, 0)
+        return p
+
+    cases = [
+        ("solve", lambda: cd.Plan(n, M), 1, lambda p, dH, dD, st: p.solve(dH[0].data_ptr(), 80.0, dD[0].data_ptr(), 100, False, st)),
+        ("solve_batch", lambda: cd.Plan(n, M, max_batch=2), 2,
+         lambda p, dH, dD, st: p.solve_batch([x.data_ptr() for x in dH], [80.0, 80.0], [x.data_ptr() for x in dD], 100, False, st)),
+        ("sliced compute", lambda: cd.Plan(n, M, sliced_solve=1), 1, lambda p, dH, dD, st: p.compute(dH[0].data_ptr(), dD[0].data_ptr(), st)),
+        ("sliced solve", lambda: cd.Plan(n, M, sliced_solve=1), 1,
+         lambda p, dH, dD, st: p.solve(dH[0].data_ptr(), 80.0, dD[0].data_ptr(), 100, False, st)),
+        ("assemble", blocks_plan, 1, lambda p, dH, dD, st: p.assemble([0.07], [dD[0].data_ptr()], st)),
+    ]
+    for name, make_plan, nb, call in cases:
+        plan = make_plan()
+        plan.coeffs(beta, 0.02, None)
+        dH = [torch.empty((n, n), dtype=torch.float64, device="cuda") for _ in range(nb)]
+        dD = [torch.empty((n, n), dtype=torch.float64, device="cuda") for _ in range(nb)]
+        st = torch.cuda.current_stream().cuda_stream
+        eager = []
+        for H in Hs:
+            for x in dH:
+                x.copy_(torch.from_numpy(H))
+            call(plan, dH, dD, st)
+            torch.cuda.synchronize()
+            eager.append([d.cpu().numpy().copy() for d in dD])
+        side, g = torch.cuda.Stream(), torch.cuda.CUDAGraph()
+        torch.cuda.synchronize()
+        with torch.cuda.graph(g, stream=side):
+            call(plan, dH, dD, torch.cuda.current_stream().cuda_stream)
+        for H, De in zip(Hs, eager):
+            for x in dH:
+                x.copy_(torch.from_numpy(H))
+            for x in dD:
+                x.fill_(float("nan"))
+            g.replay()
+            torch.cuda.synchronize()
+            for d, e in zip(dD, De):
+                assert np.array_equal(d.cpu().numpy(), e), name
+        plan.check(st)
+        del g
+        plan.destroy()
+    # the no-allocation bounds entry point (its reason to exist: callers under capture)
+    d, out = gu.to_dev(Hs[1]), torch.zeros(2, dtype=torch.float64, device="cuda")
+    cd.bounds_static(d.data_ptr(), n, n, out.data_ptr(), 0)
+    torch.cuda.synchronize()
+    e = out.cpu().numpy().copy()
+    side, g = torch.cuda.Stream(), torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g, stream=side):
+        cd.bounds_static(d.data_ptr(), n, n, out.data_ptr(), torch.cuda.current_stream().cuda_stream)
+    out.zero_()
+    g.replay()
+    torch.cuda.synchronize()
+    assert np.array_equal(out.cpu().numpy(), e) and tuple(e) == pytest.approx(oracle.gershgorin(Hs[1]), rel=1e-13)
