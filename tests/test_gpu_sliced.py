@@ -282,3 +282,37 @@ def test_sliced_solve_degenerate_shapes_and_pitches(n, M, k, p, ldh, ldd):
     assert abs(float(dtr.item()) - float(np.trace(D_or))) <= 1e-9
     assert np.max(np.abs(got[:, :n] - got[:, :n].T)) <= 1e-11
     plan.destroy()
+
+
+def test_sliced_product_beyond_the_register_resident_slicing_kernel():
+    """N = 6200 > 6144 columns: the slicing pass falls back to the two-pass kernel (rows no longer fit the registers of a
+    block).  Sampled elements against exact dot products (math.fsum), the whole matrix against the DMMA product."""
+    import math
+    oracle, cd, workloads, gu = _imports()
+    torch = gu.torch_cuda()
+    N = 6200
+    st = torch.cuda.current_stream().cuda_stream
+    rs = np.random.RandomState(6200)
+    A = rs.standard_normal((N, N))
+    A = (A + A.T) * 0.5
+    A /= np.abs(A).max()
+    B = rs.standard_normal((N, N))
+    B = (B + B.T) * 0.5
+    B /= np.abs(B).max()
+    dA, dB = gu.to_dev(A), gu.to_dev(B)
+    dO = torch.full((N, N), float("nan"), dtype=torch.float64, device="cuda")
+    dR = torch.full((N, N), float("nan"), dtype=torch.float64, device="cuda")
+    plan = cd.Plan(N, 4, sliced=8)
+    plan.product_sliced(1.0, dA.data_ptr(), dB.data_ptr(), 0.0, None, dO.data_ptr(), False, st)
+    plan.product(1.0, dA.data_ptr(), dB.data_ptr(), 0.0, None, dR.data_ptr(), st)
+    torch.cuda.synchronize()
+    got, ref = dO.cpu().numpy(), dR.cpu().numpy()
+    tol = 4.0 * N * 2.0 ** -52
+    for i, j in zip(rs.randint(0, N, 300), rs.randint(0, N, 300)):
+        exact = math.fsum(A[i, :] * B[:, j])
+        assert abs(got[i, j] - exact) <= tol and abs(ref[i, j] - exact) <= tol, (i, j)
+    for i in (0, N - 1):       # first and last row and column entirely
+        exact = np.array([math.fsum(A[i, :] * B[:, j]) for j in range(0, N, 7)])
+        assert np.max(np.abs(got[i, ::7] - exact)) <= tol and np.max(np.abs(got[::7, i] - np.array([math.fsum(A[r, :] * B[:, i]) for r in range(0, N, 7)]))) <= tol
+    assert np.max(np.abs(got - ref)) <= 2.0 * tol
+    plan.destroy()
