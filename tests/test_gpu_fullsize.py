@@ -122,3 +122,29 @@ def test_cfg4_alg1_pairing_is_selectable_and_looser_on_the_trace():
     print(f"cfg4 |dtr D|: Algorithm 1 pairing {d_alg1:.2e}, balanced (default) {d_bal:.2e}")
     assert d_bal <= 5e-11
     assert np.max(np.abs(r["D"][:, cols].T - want)) <= 1e-10
+
+
+@pytest.mark.parametrize("N,M,opts", [(6145, 6, {}), (8192, 5, {}), (7001, 6, dict(sliced_solve=1))])
+def test_beyond_the_paper_sizes_probe_vectors(N, M, opts):
+    """Sizes above the paper's range (N = 5000): banded tile table, > 32-bit byte offsets inside a matrix (8 N^2 = 0.5 GB at
+    N = 8192), the DMMA and the sliced path.  Few terms so that the oracle's vector recurrence (M N^2 per vector) stays
+    cheap: probe vectors touch every element of D; columns 0 and N - 1 element by element."""
+    import oracle
+    import workloads
+    import gpu_util as gu
+    H = workloads.hamiltonian("cfg3", seed=3, n=N)
+    a, b = oracle.gershgorin(H)
+    beta, mu = 8.0, 0.05
+    c = oracle.cheb_coeffs(beta, mu, a, b, M)
+    r = gu.gpu_solve(H, beta, mu, M, **opts)
+    D = r["D"]
+    assert abs(r["bounds"][0] - a) <= N * 2.0 ** -52 * abs(a) and abs(r["bounds"][1] - b) <= N * 2.0 ** -52 * abs(b)
+    cols = np.array([0, N // 2 + 1, N - 1], dtype=np.int32)
+    assert np.max(np.abs(D[:, cols].T - oracle.dm_cheb_columns(H, a, b, c, cols))) <= 1e-10
+    rng = np.random.default_rng(5)
+    V = np.vstack([rng.standard_normal((2, N)), rng.choice([-1.0, 1.0], size=(1, N))])
+    err = np.max(np.abs(V @ D.T - oracle.dm_cheb_apply(H, a, b, c, V)), axis=1) / np.max(np.abs(V), axis=1)
+    print(f"N={N} M={M} {opts}: probe errors {err}")
+    assert np.all(err <= 1e-10 * np.sqrt(N))
+    assert np.max(np.abs(D - D.T)) <= 1e-11
+    assert abs(r["trace"] - float(np.trace(D))) <= 1e-9
