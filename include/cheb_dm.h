@@ -113,7 +113,9 @@ typedef struct {
                       them (reported as 2).  No mode makes the per-term AXPY passes of PAPER.md:234.          */
     int giant;   /* giant steps at N <= 512: 0 = auto, 1 = generic grouped kernel, 2 = resident-multiplier kernel (each
                     CTA keeps its 32 rows of T_k in shared memory for all p-1 products and runs two column
-                    panels as independent chains; needs tile 4, 5 or 7 and grouped scheduling, else falls back) */
+                    panels as independent chains; needs tile 4, 5 or 7 and grouped scheduling, else falls back; a plan with
+                    max_batch > 1 whose batches gather the sums in the epilogues (fuse_sums = 1) runs its single solves in the
+                    generic kernel as well: reported as 1) */
     int symmetric; /* symmetric-tile skipping: 0 = auto (on), 1 = off, 2 = on.  Every matrix of the solve is a polynomial
                     of X, hence symmetric (the paper's magma_dgemm does not use this): only the tiles of a
                     product that touch the lower triangle are computed, each mirrors its 8x8 blocks into the skipped
