@@ -367,6 +367,31 @@ def measure_sliced(torch, cd, workloads, name, args, steps, warmup, flush, dist,
     return res
 
 
+def measure_graph_replay(torch, w, steps, flush, dist, world):
+    """Extra arm (reported beside `value`, never instead of it): the same step -- cheb_dm_compute_batch + cheb_dm_trace_batch --
+    captured ONCE into a CUDA graph (the calls allocate nothing and never synchronise) and replayed: what is left of a step
+    when the host's launch gaps are gone.  None for the serial ablation (its per-solve cheb_dm_coeffs are host calls)."""
+    if not w.batched:
+        return None
+    try:
+        side, g = torch.cuda.Stream(), torch.cuda.CUDAGraph()
+        torch.cuda.synchronize()
+        with torch.cuda.graph(g, stream=side):
+            cs = torch.cuda.current_stream().cuda_stream
+            w.plan.compute_batch(w.pH, w.pD, w.mu, cs)
+            w.plan.trace_batch(w.pD, w.dtr.data_ptr(), cs)
+        n = max(3, min(steps, 10))
+        ms = max_over_ranks(torch, dist, timed_steps(torch, g.replay, n, 2, flush, None, dist))
+        w.plan.check(w.st)
+        tr = [float(x) for x in w.dtr.cpu().tolist()]
+        del g
+        return {"value": world * w.units * n / (ms * 1e-3), "unit": UNIT, "ms_per_step": ms / n, "steps": n, "tr_D": tr,
+                "how": "one step captured into a CUDA graph, replayed; CUDA events around each replay, L2 flush between replays"}
+    except Exception as e:  # never let the extra arm take the bench line down
+        torch.cuda.synchronize()
+        return {"error": repr(e)[:200]}
+
+
 def measure_workload(torch, cd, workloads, name, args, steps, warmup, flush, sampler, dist, peak_tf, world):
     w = Workload(torch, cd, workloads, name, args)
     plan = w.plan
@@ -402,6 +427,7 @@ def measure_workload(torch, cd, workloads, name, args, steps, warmup, flush, sam
     e2e_ms = max_over_ranks(torch, dist, e2e_ms)
     # the same with a wait after every step (latency of ONE step from host buffers to host buffers, nothing overlapped)
     e2e_sync_ms = max_over_ranks(torch, dist, timed_steps(torch, w.step_host, e2e_steps, 1, flush, None, dist))
+    graph_arm = measure_graph_replay(torch, w, steps, flush, dist, world)
     traffic, traffic_src = ncu_traffic(name)
     res = {
         "workload": name, "N": w.N, "M_terms": w.M, "k": plan.k, "p": plan.p, "solves_per_step": w.units,
@@ -430,6 +456,7 @@ def measure_workload(torch, cd, workloads, name, args, steps, warmup, flush, sam
                          "value": world * w.units / (mi_ms * 1e-3), "unit": UNIT, "vs_fixed_mu": mi_ms / ms_per_step if ms_per_step > 0 else None,
                          "flops_per_solve": plan.flops_per_solve(), "tflops": w.units * plan.flops_per_solve() / (mi_ms * 1e-3) * 1e-12,
                          "products": plan.k + 2 * plan.p - 4, "tr_D": tr_D_mi},
+        "graph_replay": graph_arm,
         "mu": w.mu, "tr_D": tr_D, "N_occ": w.cfg.N_occ, "seeds": list(w.seeds),
         "workspace_bytes": plan.workspace_bytes(),
         "clocks": sampler.window(t_w0, t_w1) if sampler else None,
@@ -628,6 +655,7 @@ def main():
                              peak_alt_bf16_ratio=(peaks.get("bf16_tflops") or 0) * 40.0 / 2250.0 or None),
             "clocks": clocks,
             "mu": main_res["mu"], "tr_D": main_res["tr_D"], "mu_inclusive": main_res["mu_inclusive"],
+            "graph_replay": main_res.get("graph_replay"),
             "other_workloads": others,
         }
         if not args.no_cpu_baseline and world == 1:
